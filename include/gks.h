@@ -1,0 +1,138 @@
+/*
+ * gks.h — C ABI of libgks_b200: one two-stage fourth-order (S2O4) step of the high-order
+ * gas-kinetic scheme (GKS) for 3-D weakly compressible isothermal flow on a rectilinear
+ * Cartesian grid, plus the body-force term carrying ALM and IBM forcing.
+ *
+ * Source of the method: arxiv/paper_2603_11102.  Citations are "PAPER.md:<line>".
+ *   state            Q = (rho, rho*U, rho*V, rho*W)
+ *   equilibrium      isothermal Maxwellian, lambda = 1/(2 RT) constant    PAPER.md:49-51 (Eq. 2)
+ *   finite volume    dQ/dt = L(Q) = -(1/|Omega|) sum_p F_p(t)             PAPER.md:59-66 (Eq. 4-5)
+ *   face flux        2x2 Gauss points per face                            PAPER.md:68-71 (Eq. 6)
+ *   distribution     f = g0 (1 - tau (a1 u + a2 v + a3 w + A) + A t)      PAPER.md:75-81 (Eq. 7), tau = mu/p
+ *   coefficients     <a_s> = dQ0/ds, <a1 u + a2 v + a3 w + A> = 0         PAPER.md:84 (Eq. 8), Appendix :501-558
+ *   reconstruction   5th-order WENO, dimension by dimension
+ *   time stepping    two-stage fourth-order
+ *   ALM              f = F/(eps^3 pi^1.5) exp(-(r/eps)^2), cut at 3 eps    PAPER.md:137 (Eq. 10), :293
+ *   IBM              direct forcing with Lagrangian points                PAPER.md:143-175 (Eq. 11-12)
+ *   momentum update  (rho U)~ = (rho U)^{n+1} + f dt/V                    PAPER.md:189 (Eq. 13)
+ * Every point on which the paper is silent is fixed by a numbered reading S1..S24 in DESIGN.md.
+ *
+ * Conventions
+ *   - All floating point is IEEE fp64.  Field layout W[c][k][j][i], i fastest, c in {rho, rhoU, rhoV, rhoW},
+ *     interior cells only (4*nz*ny*nx doubles) at this boundary; the library keeps its own padded copy.
+ *   - Pointers marked "host or device" are classified with cudaPointerGetAttributes; the copy is
+ *     enqueued on the context's stream.  The caller owns every array it passes; the library copies
+ *     what it needs during the call and never retains a caller pointer, except `workspace`.
+ *   - `workspace` is DEVICE memory owned by the caller (e.g. a torch tensor), at least
+ *     gks_workspace_bytes(cfg) bytes, 256-byte aligned, kept alive until gks_destroy.  No call
+ *     allocates device memory.  All kernels are enqueued on `cuda_stream` (a cudaStream_t; NULL = the
+ *     legacy default stream).  gks_step is asynchronous; gks_get_state synchronises the stream when
+ *     the destination is host memory.
+ *   - Every call returns a gks_status, never throws or aborts.  On error the context is unchanged
+ *     and gks_last_error(ctx) (or gks_last_error(NULL) for gks_create failures) holds a message.
+ *   - A context is not thread-safe.
+ *   - There is no CPU fallback: without a CUDA device gks_create returns GKS_ERR_CUDA.
+ */
+#ifndef GKS_B200_H
+#define GKS_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gks_ctx gks_ctx; /* opaque */
+
+typedef enum {
+  GKS_OK = 0,
+  GKS_ERR_INVALID_ARG = 1,
+  GKS_ERR_WORKSPACE = 2, /* workspace NULL, too small or misaligned */
+  GKS_ERR_CUDA = 3,      /* a CUDA runtime call failed; message in gks_last_error */
+  GKS_ERR_STATE = 4,     /* call order, e.g. gks_step before gks_set_state */
+  GKS_ERR_NONFINITE = 5  /* gks_check_finite found a NaN/Inf */
+} gks_status;
+
+/* Boundary kinds (PAPER.md:215 periodic + no-slip isothermal wall; :267 Riemann-invariant
+ * inlet/outlet + extrapolation; :287 slip wall; :374 symmetry).  Ghost-cell formulas: DESIGN.md S17-S21. */
+typedef enum {
+  GKS_BC_PERIODIC = 0,
+  GKS_BC_WALL_NOSLIP = 1,
+  GKS_BC_WALL_SLIP = 2, /* also "symmetry" */
+  GKS_BC_INFLOW = 3,
+  GKS_BC_OUTFLOW_CONVECTIVE = 4,
+  GKS_BC_EXTRAPOLATE = 5
+} gks_bc;
+
+typedef struct {
+  int nx, ny, nz;               /* interior cells per axis, each >= 6 */
+  const double *xf, *yf, *zf;   /* HOST face coordinates, n+1 each, strictly increasing; NULL => uniform */
+  double x0, y0, z0;            /* origin of the low faces (used when the axis is uniform) */
+  double dx, dy, dz;            /* spacing (used when the axis is uniform), > 0 */
+  double RT;                    /* isothermal constant R*T > 0; lambda = 1/(2 RT), c_s = sqrt(RT) */
+  double nu;                    /* kinematic viscosity >= 0; mu = rho_ref*nu, tau = mu/p */
+  double rho_ref;               /* reference density > 0 (1 in all configs) */
+  int bc[6];                    /* gks_bc for xlo, xhi, ylo, yhi, zlo, zhi; periodic must be paired */
+  double inflow[4];             /* rho, U, V, W for GKS_BC_INFLOW; |velocity normal to an outflow face| is
+                                   the convective speed of GKS_BC_OUTFLOW_CONVECTIVE */
+  double weno_eps;              /* WENO-JS epsilon; 0 => 1e-6 */
+} gks_config;
+
+/* Bytes of device workspace gks_create needs for this configuration (0 if cfg is invalid). */
+size_t gks_workspace_bytes(const gks_config *cfg);
+
+/* Validate cfg, carve `workspace` (device), upload coordinates.  *out is set only on GKS_OK. */
+gks_status gks_create(const gks_config *cfg, void *workspace, size_t workspace_bytes,
+                      void *cuda_stream, gks_ctx **out);
+gks_status gks_destroy(gks_ctx *ctx);
+
+/* W: host or device, 4*nz*ny*nx doubles, W[c][k][j][i].  set_state also initialises the
+ * convective-outflow ghost state (S20).  get_state synchronises for host destinations. */
+gks_status gks_set_state(gks_ctx *ctx, const double *W);
+gks_status gks_get_state(gks_ctx *ctx, double *W);
+
+/* One S2O4 step W^n -> W^{n+1} (W* = W^n + dt/2 L + dt^2/8 dL,
+ * W^{n+1} = W^n + dt L + dt^2/6 (dL(W^n) + 2 dL(W*))) computed without external force
+ * (PAPER.md:187), then the forcing of Eq. 13: uniform/bulk term, IBM, ALM.  dt > 0.
+ * Asynchronous on the context's stream. */
+gks_status gks_step(gks_ctx *ctx, double dt);
+
+/* Uniform acceleration g: momentum += dt * rho * g each step.  (0,0,0) disables. */
+gks_status gks_set_body_force(gks_ctx *ctx, double gx, double gy, double gz);
+/* "Constant moment flux" forcing of the channel: after each step shift (rho U_axis)
+ * uniformly so that its volume-weighted mean equals `target`.  axis in {0,1,2}; axis < 0 disables. */
+gks_status gks_set_bulk_flux(gks_ctx *ctx, int axis, double target_bulk_momentum);
+
+/* ALM (Eq. 10): n actuator points; pos and force are n*3 doubles (x,y,z per point),
+ * host or device; force = point force ON THE FLUID; eps > 0 is the Gaussian width; the kernel is
+ * sampled at cell centres and cut at r <= 3 eps.  n = 0 clears.  n <= GKS_MAX_ALM_POINTS. */
+gks_status alm_set_points(gks_ctx *ctx, int n, const double *pos, const double *force, double eps);
+
+/* IBM: n Lagrangian points; pos n*3 doubles, weights n doubles = V_p = dx*dS
+ * (PAPER.md:155); host or device.  Velocities default to 0 (stationary body).
+ * Each point must lie inside the domain and the grid must be locally uniform over its 3x3x3
+ * support, else GKS_ERR_INVALID_ARG.  n = 0 clears.  n <= GKS_MAX_IBM_POINTS. */
+gks_status ibm_set_points(gks_ctx *ctx, int n, const double *pos, const double *weights);
+gks_status ibm_set_velocities(gks_ctx *ctx, const double *vel /* n*3, or NULL => 0 */);
+
+/* Test hook: fill ghosts of the CURRENT state and evaluate the face-averaged flux F and its
+ * time derivative dF/dt (Eq. 6-7) for sweep direction dir in {0,1,2}.  Output (host or device):
+ * 4 * (faces) doubles each, faces laid out like cells but with n_dir+1 entries along `dir`,
+ * component-major: F[c][k][j][i].  Does not modify the state. */
+gks_status gks_debug_eval_flux(gks_ctx *ctx, int dir, double *F, double *dFdt);
+
+/* Synchronising check of the current state; GKS_ERR_NONFINITE if any interior value is NaN/Inf. */
+gks_status gks_check_finite(gks_ctx *ctx);
+
+/* Number of kernels this context has launched since gks_create (for bench.py's gpu_launches). */
+long long gks_launch_count(const gks_ctx *ctx);
+
+const char *gks_last_error(const gks_ctx *ctx);
+
+#define GKS_MAX_ALM_POINTS 65536
+#define GKS_MAX_IBM_POINTS 4194304
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GKS_B200_H */

@@ -1,0 +1,23 @@
+import os
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def pytest_configure(config):
+    config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
+    config.addinivalue_line("markers", "slow: longer CPU test")
+
+
+def rel_linf(a, b):
+    """Error norm S24: density and momentum normalised separately; momentum components
+    jointly by the largest momentum magnitude.  a = tested, b = oracle; shape (4, nz, ny, nx)."""
+    import numpy as np
+    e_rho = np.abs(a[0] - b[0]).max() / np.abs(b[0]).max()
+    mmag = np.sqrt((b[1:] ** 2).sum(0)).max()
+    e_m = np.abs(a[1:] - b[1:]).max() / (mmag if mmag > 0 else 1.0)
+    return max(e_rho, e_m)
