@@ -1,0 +1,320 @@
+"""Pins of the oracle's whole step against invariants, exact solutions and closed forms (P6-P12, P14).
+
+CPU only.  Sizes are chosen so that the file runs in about a minute.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import binding as ob
+from paper_2603_11102_b200 import workloads as wl
+from paper_2603_11102_b200.workloads import GridConfig
+
+P, NS, SL, IN, OUT, EX = range(6)
+
+
+def run(cfg, W0, dt, steps, setup=None):
+    o = ob.Oracle(cfg)
+    if setup:
+        setup(o)
+    o.set_state(W0)
+    for _ in range(steps):
+        o.step(dt)
+    W = o.get_state()
+    o.close()
+    return W
+
+
+def const_state(n, q):
+    W = np.empty((4, n[2], n[1], n[0]))
+    for c in range(4):
+        W[c] = q[c]
+    return W
+
+
+# ---------------------------------------------------------------- P6 free-stream preservation
+@pytest.mark.parametrize("bc,q", [
+    ((P,) * 6, (1.0, 0.1, -0.05, 0.02)),
+    ((EX,) * 6, (1.0, 0.1, -0.05, 0.02)),
+    ((IN, EX, P, P, SL, SL), (1.0, 0.1, 0.03, 0.0)),
+    ((IN, OUT, EX, EX, P, P), (1.0, 0.1, 0.0, 0.0)),
+])
+def test_P6_free_stream_is_preserved_bit_for_bit(bc, q):
+    n = (8, 7, 9)
+    yf = np.cumsum(np.r_[0.0, np.linspace(0.5, 1.5, n[1])])        # a stretched axis as well
+    cfg = GridConfig(n=n, faces=(None, yf, None), spacing=(0.3, 1.0, 0.2), nu=1e-3, bc=bc, inflow=q)
+    W0 = const_state(n, q)
+    W = run(cfg, W0, 0.05, 2)
+    assert np.array_equal(W, W0)
+
+
+# ---------------------------------------------------------------- P7 conservation
+def test_P7_mass_and_momentum_conserved_on_periodic_box():
+    w = wl.taylor_green(12)
+    W = run(w.cfg, w.W0, w.dt, 2)
+    for c in range(4):
+        scale = np.abs(w.W0[c]).sum() + 1.0
+        assert abs(W[c].sum() - w.W0[c].sum()) / scale < 1e-13
+    assert np.abs(W - w.W0).max() > 1e-6                             # it did move
+
+
+def test_P7_mass_conserved_between_noslip_walls_on_stretched_grid():
+    w = wl.channel((8, 12, 6))
+    cfg = w.cfg
+    vol = np.einsum("k,j,i->kji", cfg.widths(2), cfg.widths(1), cfg.widths(0))
+    W = run(cfg, w.W0, w.dt, 2)
+    m0, m1 = (w.W0[0] * vol).sum(), (W[0] * vol).sum()
+    assert abs(m1 - m0) / m0 < 1e-13
+    assert np.abs(W[0] - w.W0[0]).max() > 1e-9
+
+
+# ---------------------------------------------------------------- P8 order of accuracy (exact simple wave)
+GL4_X = np.array([-0.8611363115940526, -0.3399810435848563, 0.3399810435848563, 0.8611363115940526]) * 0.5
+GL4_W = np.array([0.3478548451374538, 0.6521451548625461, 0.6521451548625461, 0.3478548451374538]) * 0.5
+
+
+def simple_wave_exact(n, t, RT=1.0, amp=0.05):
+    """Cell averages (4-point Gauss per axis) of the isothermal simple wave along (1,1,1)/sqrt(3):
+    U = c ln(rho) along n (Riemann invariant U - c ln rho = 0), rho constant on d xi/dt = U + c."""
+    c = math.sqrt(RT)
+    h = 2 * math.pi / n
+    x1 = ((np.arange(n) + 0.5)[:, None] + GL4_X[None, :]).ravel() * h       # n*4 nodes per axis
+    w1 = np.tile(GL4_W, n)
+    Z, Y, X = np.meshgrid(x1, x1, x1, indexing="ij")
+    s = X + Y + Z                                                            # phase sqrt(3) xi
+    k = math.sqrt(3.0)
+    rho_i = lambda s0: 1.0 + amp * np.sin(s0)
+    # characteristic foot: s = s0 + k (U(rho_i(s0)) + c) t ; Newton on s0
+    s0 = s - k * c * t
+    for _ in range(50):
+        r = rho_i(s0)
+        f = s0 + k * (c * np.log(r) + c) * t - s
+        df = 1.0 + k * c * t * amp * np.cos(s0) / r
+        step = f / df
+        s0 -= step
+        if np.abs(step).max() < 1e-15:
+            break
+    rho = rho_i(s0)
+    U = c * np.log(rho) / k                                                  # each Cartesian component
+    W = np.stack([rho, rho * U, rho * U, rho * U])
+    Wq = W.reshape(4, n, 4, n, 4, n, 4)
+    wq = GL4_W
+    return np.einsum("ckajbic,a,b,c->ckji".replace("c,a", "c,a"), Wq, wq, wq, wq) if False else \
+        np.einsum("zkajbic,a,b,c->zkji", Wq, wq, wq, wq)
+
+
+def simple_wave_error(n):
+    cfg = GridConfig(n=(n, n, n), spacing=(2 * math.pi / n,) * 3, nu=0.0, bc=(P,) * 6)
+    T = 1.0
+    steps = math.ceil(T / (0.4 * (2 * math.pi / n) / 1.1))
+    W = run(cfg, simple_wave_exact(n, 0.0), T / steps, steps)
+    ref = simple_wave_exact(n, T)
+    return np.abs(W[0] - ref[0]).mean(), np.abs(W[1:] - ref[1:]).mean()
+
+
+def test_P8_order_of_accuracy_on_exact_simple_wave():
+    e16, m16 = simple_wave_error(16)
+    e32, m32 = simple_wave_error(32)
+    order_rho = math.log2(e16 / e32)
+    order_m = math.log2(m16 / m32)
+    assert e32 < 2e-6
+    assert order_rho >= 3.5 and order_m >= 3.5, (e16, e32, m16, m32)
+
+
+# ---------------------------------------------------------------- P9 viscous decay (pins tau = mu/p, S3)
+@pytest.mark.parametrize("RT,rho,rho_ref", [(1.0, 1.0, 1.0), (0.64, 1.3, 1.0), (1.5, 0.8, 1.1)])
+def test_P9_shear_wave_decays_at_mu_over_rho(RT, rho, rho_ref):
+    """V = V0 sin(x) exp(-(mu/rho) t) is an exact solution of the isothermal Navier-Stokes equations;
+    mu = tau p = rho_ref nu whatever RT is (reading S3)."""
+    n = (32, 6, 6)
+    nu, V0 = 0.02, 0.01
+    h = 2 * math.pi / n[0]
+    cfg = GridConfig(n=n, spacing=(h, h, h), RT=RT, nu=nu, rho_ref=rho_ref, bc=(P,) * 6)
+    xf = cfg.face_coords(0)
+    sin_avg = (np.cos(xf[:-1]) - np.cos(xf[1:])) / h
+    W0 = const_state(n, (rho, 0.0, 0.0, 0.0))
+    W0[2] = rho * V0 * sin_avg[None, None, :]
+    dt = 0.4 * h / (math.sqrt(RT) + V0)
+    steps = 20
+    W = run(cfg, W0, dt, steps)
+    amp = (W[2] * sin_avg[None, None, :]).sum() / (sin_avg ** 2).sum() / (n[1] * n[2]) / (rho * V0)
+    rate = -math.log(amp) / (steps * dt)
+    assert rate == pytest.approx(nu * rho_ref / rho, rel=2e-3)     # WENO-JS adds < 0.2 % at 32 cells per wave
+    assert np.abs(W[0] - rho).max() < 1e-9                          # density stays uniform
+
+
+# ---------------------------------------------------------------- P10 acoustic speed sqrt(RT)
+@pytest.mark.parametrize("RT", [1.0, 0.64])
+def test_P10_acoustic_wave_travels_at_sqrt_RT(RT):
+    n = (32, 6, 6)
+    a = 1e-4
+    cs = math.sqrt(RT)
+    h = 2 * math.pi / n[0]
+    cfg = GridConfig(n=n, spacing=(h, h, h), RT=RT, nu=0.0, bc=(P,) * 6)
+    xf = cfg.face_coords(0)
+    s_avg = (np.cos(xf[:-1]) - np.cos(xf[1:])) / h
+    c_avg = (np.sin(xf[1:]) - np.sin(xf[:-1])) / h
+    W0 = const_state(n, (1.0, 0.0, 0.0, 0.0))
+    W0[0] += a * s_avg[None, None, :]
+    W0[1] = (1.0 + a * s_avg) * (a * cs * s_avg)
+    period = 2 * math.pi / cs
+    steps = math.ceil(period / (0.4 * h / (cs + a)))
+    W = run(cfg, W0, period / steps, steps)
+    d = W[0, 0, 0, :] - 1.0
+    S, Cc = (d * s_avg).sum() / (s_avg ** 2).sum(), (d * c_avg).sum() / (c_avg ** 2).sum()
+    # rho - 1 = a sin(x - c t): after one nominal period the phase lag is 2 pi (1 - c/c_s)
+    phase = math.atan2(-Cc, S)
+    assert abs(phase) / (2 * math.pi) < 1e-3
+    assert math.hypot(S, Cc) == pytest.approx(a, rel=1e-3)
+
+
+# ---------------------------------------------------------------- P11 ALM integral
+ALM_CUT_INTEGRAL = math.erf(3.0) - 6.0 / math.sqrt(math.pi) * math.exp(-9.0)     # = 0.99956...
+
+
+@pytest.mark.parametrize("offset", [(0.0, 0.0, 0.0), (0.5, 0.5, 0.5), (0.21, 0.37, 0.48)])
+def test_P11_alm_spreads_the_point_force(offset):
+    n = (32, 32, 32)
+    h = 0.1
+    cfg = GridConfig(n=n, spacing=(h, h, h), bc=(EX,) * 6)
+    o = ob.Oracle(cfg)
+    o.set_state(const_state(n, (1.0, 0.1, 0.0, 0.0)))
+    X = np.array([16.0, 16.0, 16.0]) * h + np.array(offset) * h
+    F = np.array([-0.3, 0.2, 0.05])
+    dt = 0.01
+    o.alm_set_points(X[None], F[None], 2 * h)
+    dM = o.eval_forcing(dt)
+    total = dM.reshape(3, -1).sum(1) * h ** 3 / dt
+    assert np.allclose(total / F, ALM_CUT_INTEGRAL, rtol=0, atol=1e-4)
+    # touched cells all lie within 3 eps, and the kernel value there is Eq. 10
+    k, j, i = np.nonzero(dM[0])
+    r = np.sqrt(((i + 0.5) * h - X[0]) ** 2 + ((j + 0.5) * h - X[1]) ** 2 + ((k + 0.5) * h - X[2]) ** 2)
+    assert r.max() <= 3 * 2 * h and len(r) > 0.95 * 4 / 3 * math.pi * 6 ** 3
+    expect = dt * F[0] * np.exp(-(r / (2 * h)) ** 2) / ((2 * h) ** 3 * math.pi ** 1.5)
+    assert np.allclose(dM[0][k, j, i], expect, rtol=1e-13)
+    o.alm_set_cut(0.0)                                            # no cut: the integral is 1
+    total = o.eval_forcing(dt).reshape(3, -1).sum(1) * h ** 3 / dt
+    assert np.allclose(total / F, 1.0, rtol=0, atol=1e-10)
+    o.close()
+
+
+def test_P11_alm_wraps_on_periodic_axes_and_drops_outside_walls():
+    n = (16, 16, 16)
+    h = 0.1
+    cfg = GridConfig(n=n, spacing=(h, h, h), bc=(P, P, P, P, SL, SL))
+    o = ob.Oracle(cfg)
+    o.set_state(const_state(n, (1.0, 0.0, 0.0, 0.0)))
+    F = np.array([[1.0, 0.0, 0.0]])
+    o.alm_set_points(np.array([[0.03, 0.8, 0.8]]), F, 2 * h)      # support crosses the periodic x face
+    tot = o.eval_forcing(1.0)[0].sum() * h ** 3
+    assert abs(tot - ALM_CUT_INTEGRAL) < 1e-4
+    o.alm_set_points(np.array([[0.8, 0.8, 0.0]]), F, 2 * h)       # centred on the slip wall: half is lost
+    tot = o.eval_forcing(1.0)[0].sum() * h ** 3
+    assert abs(tot - 0.5 * ALM_CUT_INTEGRAL) < 1e-3
+    o.close()
+
+
+# ---------------------------------------------------------------- P12 IBM
+def ibm_case(vel_field=None):
+    n = (12, 10, 8)
+    h = 0.25
+    cfg = GridConfig(n=n, spacing=(h, h, h), bc=(EX, EX, EX, EX, P, P))
+    rng = np.random.default_rng(7)
+    pos = np.stack([rng.uniform(2 * h, (n[0] - 2) * h, 40), rng.uniform(2 * h, (n[1] - 2) * h, 40),
+                    rng.uniform(0, n[2] * h, 40)], axis=1)        # z is periodic: any z allowed
+    vol = rng.uniform(0.5, 1.5, 40) * h ** 3
+    return cfg, pos, vol
+
+
+def test_P12_ibm_interpolates_constants_exactly_and_conserves_impulse():
+    cfg, pos, vol = ibm_case()
+    n = cfg.n
+    o = ob.Oracle(cfg)
+    rho = 1.2
+    U = np.array([0.1, -0.04, 0.07])
+    W0 = const_state(n, (rho, *(rho * U)))
+    o.set_state(W0)
+    o.ibm_set_points(pos, vol)
+    Up = o.ibm_interpolate()
+    assert np.allclose(Up, U[None, :], rtol=0, atol=2e-16)
+    dM = o.eval_forcing(0.1)
+    h3 = 0.25 ** 3
+    impulse = dM.reshape(3, -1).sum(1) * h3
+    expect = (rho * (0.0 - Up) * vol[:, None]).sum(0)            # sum_p rho (v_p - U_p) V_p, v_p = 0
+    assert np.allclose(impulse, expect, rtol=1e-13)
+    # a fluid already moving with the body gets no force
+    vp = np.tile(U, (len(pos), 1))
+    o.ibm_set_velocities(vp)
+    assert np.abs(o.eval_forcing(0.1)).max() < 1e-16
+    o.close()
+
+
+def test_P12_ibm_reads_the_unforced_field_and_rejects_outside_points():
+    cfg, pos, vol = ibm_case()
+    o = ob.Oracle(cfg)
+    with pytest.raises(ob.OracleError):
+        o.ibm_set_points(np.array([[-0.1, 1.0, 1.0]]), np.array([1.0]))
+    # one step with and without an (overlapping) ALM point: the IBM increment is the same (S12)
+    rng = np.random.default_rng(3)
+    W0 = const_state(cfg.n, (1.0, 0.1, 0.0, 0.0)) * (1 + 0.01 * rng.standard_normal((4, 8, 10, 12)))
+    o.set_state(W0)
+    o.ibm_set_points(pos, vol)
+    d_ibm = o.eval_forcing(0.05)
+    o.alm_set_points(pos[:1], np.array([[0.1, 0.0, 0.0]]), 0.3)
+    d_both = o.eval_forcing(0.05)
+    o.ibm_set_points(pos[:0], vol[:0])
+    d_alm = o.eval_forcing(0.05)
+    assert np.allclose(d_both, d_ibm + d_alm, rtol=0, atol=1e-17)
+    o.close()
+
+
+# ---------------------------------------------------------------- bulk flux (S16) and body force
+def test_bulk_flux_restores_target_and_body_force_adds_rho_g_dt():
+    w = wl.channel((8, 12, 6))
+    cfg = w.cfg
+    vol = np.einsum("k,j,i->kji", cfg.widths(2), cfg.widths(1), cfg.widths(0))
+    W = run(cfg, w.W0, w.dt, 1, setup=lambda o: o.set_bulk_flux(0, 0.1))
+    assert (W[1] * vol).sum() / vol.sum() == pytest.approx(0.1, rel=1e-13)
+    Wn = run(cfg, w.W0, w.dt, 1)
+    Wg = run(cfg, w.W0, w.dt, 1, setup=lambda o: o.set_body_force(0.0, 0.0, 0.3))
+    assert np.allclose(Wg[3] - Wn[3], w.dt * Wn[0] * 0.3, rtol=1e-12, atol=1e-18)
+    assert np.array_equal(Wg[:3], Wn[:3])
+
+
+# ---------------------------------------------------------------- P14 axis symmetry
+def permute_axes(W):
+    """relabel (x,y,z) -> (y,z,x): new field W'(x,y,z) = old field at (z,x,y) with components rotated"""
+    # array axes are (c, z, y, x); new x runs over old z, new y over old x, new z over old y
+    Wn = np.transpose(W, (0, 2, 3, 1))          # (c, new z=old y, new y=old x, new x=old z)
+    return np.stack([Wn[0], Wn[3], Wn[1], Wn[2]])   # new U = old W, new V = old U, new W = old V
+
+
+def test_P14_one_dimensional_data_gives_the_same_result_along_every_axis():
+    n, h = 12, 2 * math.pi / 12
+    x = (np.arange(n) + 0.5) * h
+    prof_r = 1.0 + 0.05 * np.sin(x)
+    prof_u = 0.1 * np.cos(x)
+    res = []
+    for axis in range(3):
+        shape = [1, 1, 1]
+        shape[2 - axis] = n
+        W0 = np.zeros((4, n, n, n))
+        W0[0] = prof_r.reshape(shape)
+        W0[1 + axis] = (prof_r * prof_u).reshape(shape)
+        cfg = GridConfig(n=(n, n, n), spacing=(h, h, h), nu=1e-3, bc=(P,) * 6)
+        W = run(cfg, W0, 0.2, 2)
+        idx = [0, 0, 0]
+        idx[2 - axis] = slice(None)
+        res.append((W[0][tuple(idx)], W[1 + axis][tuple(idx)]))
+    for axis in (1, 2):
+        assert np.allclose(res[axis][0], res[0][0], rtol=0, atol=5e-16)
+        assert np.allclose(res[axis][1], res[0][1], rtol=0, atol=5e-16)
+
+
+def test_P14_axis_permutation_commutes_up_to_the_pass_order():
+    w = wl.taylor_green(12)
+    W_a = permute_axes(run(w.cfg, w.W0, w.dt, 1))
+    W_b = run(w.cfg, permute_axes(w.W0), w.dt, 1)
+    diff = np.abs(W_a - W_b).max()
+    assert diff < 1e-6                       # only S9 (order of the tangential WENO passes) differs: O(h^5)
