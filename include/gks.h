@@ -121,6 +121,11 @@ gks_status ibm_set_velocities(gks_ctx *ctx, const double *vel /* n*3, or NULL =>
  * component-major: F[c][k][j][i].  Does not modify the state. */
 gks_status gks_debug_eval_flux(gks_ctx *ctx, int dir, double *F, double *dFdt);
 
+/* Test hook: choose the sweep implementation.  0 (default) = fused production kernels
+ * (reconstruction + flux in one kernel per direction, slabs staged through shared memory by TMA);
+ * 1 = unfused cross-check kernels (three kernels per direction, intermediates in HBM). */
+gks_status gks_debug_set_sweep(gks_ctx *ctx, int mode);
+
 /* Synchronising check of the current state; GKS_ERR_NONFINITE if any interior value is NaN/Inf. */
 gks_status gks_check_finite(gks_ctx *ctx);
 

@@ -1,0 +1,278 @@
+/*
+ * gks_api_step.cu — second half of the C ABI: state transfer, gks_step, forcing setters, test hooks.
+ */
+#include <cmath>
+#include <cstring>
+#include <vector>
+
+#include "gks_internal.h"
+
+#define CUDA_TRY(ctx, call)                                                                                  \
+  do {                                                                                                       \
+    cudaError_t e_ = (call);                                                                                 \
+    if (e_ != cudaSuccess) return gks_set_err(ctx, GKS_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_));   \
+  } while (0)
+
+namespace {
+
+size_t interior_doubles(const gks_ctx *ctx) { return 4 * (size_t)ctx->g.n[0] * ctx->g.n[1] * ctx->g.n[2]; }
+
+/* host copy of a small caller array that may live on the device */
+gks_status fetch_host(gks_ctx *ctx, const double *src, size_t count, std::vector<double> &dst) {
+  dst.resize(count);
+  if (count == 0) return GKS_OK;
+  if (gks_is_device_ptr(src)) {
+    CUDA_TRY(ctx, cudaMemcpyAsync(dst.data(), src, count * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+  } else {
+    memcpy(dst.data(), src, count * sizeof(double));
+  }
+  return GKS_OK;
+}
+
+/* all sweeps of one stage into ctx->flux[] */
+void sweeps(gks_ctx *ctx, const double *W, bool need_F) {
+  for (int d = 0; d < 3; ++d)
+    ctx->launches += gks_launch_sweep_unfused(ctx->g, ctx->ph, d, W, ctx->tmpN, ctx->tmpT, ctx->flux[d], need_F,
+                                              ctx->stream);
+}
+
+} /* namespace */
+
+extern "C" {
+
+gks_status gks_set_state(gks_ctx *ctx, const double *W) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (!W) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "W is NULL");
+  const double *src = W;
+  if (!gks_is_device_ptr(W)) { /* host: stage through Pbuf (free between steps) */
+    CUDA_TRY(ctx, cudaMemcpyAsync(ctx->Pbuf, W, interior_doubles(ctx) * sizeof(double), cudaMemcpyHostToDevice,
+                                  ctx->stream));
+    src = ctx->Pbuf;
+  }
+  ctx->launches += gks_launch_pack(ctx->g, src, ctx->Wn, ctx->stream);
+  ctx->launches += gks_launch_outflow_init(ctx->g, ctx->ph, ctx->Wn, ctx->stream);
+  CUDA_TRY(ctx, cudaGetLastError());
+  ctx->have_state = true;
+  return GKS_OK;
+}
+
+gks_status gks_get_state(gks_ctx *ctx, double *W) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (!W) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "W is NULL");
+  if (!ctx->have_state) return gks_set_err(ctx, GKS_ERR_STATE, "gks_get_state before gks_set_state");
+  if (gks_is_device_ptr(W)) {
+    ctx->launches += gks_launch_unpack(ctx->g, ctx->Wn, W, ctx->stream);
+    CUDA_TRY(ctx, cudaGetLastError());
+  } else {
+    ctx->launches += gks_launch_unpack(ctx->g, ctx->Wn, ctx->Pbuf, ctx->stream);
+    CUDA_TRY(ctx, cudaGetLastError());
+    CUDA_TRY(ctx, cudaMemcpyAsync(W, ctx->Pbuf, interior_doubles(ctx) * sizeof(double), cudaMemcpyDeviceToHost,
+                                  ctx->stream));
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+  }
+  return GKS_OK;
+}
+
+gks_status gks_step(gks_ctx *ctx, double dt) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (!ctx->have_state) return gks_set_err(ctx, GKS_ERR_STATE, "gks_step before gks_set_state");
+  if (!(dt > 0) || !std::isfinite(dt)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "dt must be > 0");
+  const GksGrid &g = ctx->g;
+  const GksPhys &ph = ctx->ph;
+  cudaStream_t s = ctx->stream;
+  /* stage 1: ghosts of W^n, F and dF/dt of the three sweeps, W* and P */
+  ctx->launches += gks_launch_ghost_fill(g, ph, ctx->Wn, ctx->Wn, s);
+  sweeps(ctx, ctx->Wn, true);
+  ctx->launches += gks_launch_stage1(g, ctx->Wn, ctx->flux, dt, ctx->Ws, ctx->Pbuf, s);
+  /* stage 2: ghosts of W* (outflow ghost state taken from W^n, S20), dF/dt only, W^{n+1} in place of W^n */
+  ctx->launches += gks_launch_ghost_fill(g, ph, ctx->Ws, ctx->Wn, s);
+  sweeps(ctx, ctx->Ws, false);
+  ctx->launches += gks_launch_stage2(g, ctx->Pbuf, ctx->flux, dt, ctx->Wn, s);
+  /* forcing (Eq. 13), every increment from the un-forced field: read-only kernels first */
+  const bool uniform = ctx->gacc[0] != 0.0 || ctx->gacc[1] != 0.0 || ctx->gacc[2] != 0.0;
+  if (ctx->bulk_axis >= 0) ctx->launches += gks_launch_bulk_reduce(g, ctx->Wn, ctx->bulk_axis, ctx->red, s);
+  if (ctx->n_ibm > 0)
+    ctx->launches += gks_launch_ibm_interp(g, ctx->Wn, ctx->n_ibm, ctx->ibm_pos, ctx->ibm_vol, ctx->ibm_vel,
+                                           ctx->ibm_coef, s);
+  if (uniform || ctx->bulk_axis >= 0)
+    ctx->launches += gks_launch_uniform_force(g, ctx->Wn, dt, ctx->gacc, ctx->bulk_axis, ctx->bulk_target,
+                                              ctx->total_volume, ctx->red, s);
+  if (ctx->n_ibm > 0) ctx->launches += gks_launch_ibm_spread(g, ctx->Wn, ctx->n_ibm, ctx->ibm_pos, ctx->ibm_coef, s);
+  if (ctx->n_alm > 0)
+    ctx->launches += gks_launch_alm(g, ctx->Wn, ctx->n_alm, ctx->alm_pos, ctx->alm_force, ctx->alm_eps, dt,
+                                    ctx->alm_lo, ctx->alm_cnt, s);
+  ctx->launches += gks_launch_outflow_advance(g, ph, ctx->Wn, dt, s);
+  CUDA_TRY(ctx, cudaGetLastError());
+  return GKS_OK;
+}
+
+gks_status gks_set_body_force(gks_ctx *ctx, double gx, double gy, double gz) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (!std::isfinite(gx) || !std::isfinite(gy) || !std::isfinite(gz))
+    return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "acceleration must be finite");
+  ctx->gacc[0] = gx;
+  ctx->gacc[1] = gy;
+  ctx->gacc[2] = gz;
+  return GKS_OK;
+}
+
+gks_status gks_set_bulk_flux(gks_ctx *ctx, int axis, double target) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (axis > 2) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "axis must be 0, 1, 2 or negative");
+  ctx->bulk_axis = axis < 0 ? -1 : axis;
+  ctx->bulk_target = target;
+  return GKS_OK;
+}
+
+gks_status alm_set_points(gks_ctx *ctx, int n, const double *pos, const double *force, double eps) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (n < 0 || n > GKS_MAX_ALM_POINTS) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "n out of range");
+  if (n == 0) {
+    ctx->n_alm = 0;
+    return GKS_OK;
+  }
+  if (!pos || !force) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "pos/force is NULL");
+  if (!(eps > 0) || !std::isfinite(eps)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "eps must be > 0");
+  std::vector<double> hp;
+  if (gks_status st = fetch_host(ctx, pos, 3 * (size_t)n, hp)) return st;
+  /* bounding box of the cut supports in unwrapped cell indices (cells whose centre can lie within
+     3 eps of a point); conservative by one cell, the kernel applies the exact cut */
+  const double R = 3.0 * eps;
+  int lo[3], cnt[3];
+  for (int a = 0; a < 3; ++a) {
+    const int nn = ctx->g.n[a];
+    const double *xf = ctx->h_xf[a] + GKS_NG;
+    const double L = xf[nn] - xf[0];
+    double pmin = hp[a], pmax = hp[a];
+    for (int p = 1; p < n; ++p) {
+      pmin = fmin(pmin, hp[3 * p + a]);
+      pmax = fmax(pmax, hp[3 * p + a]);
+    }
+    if (!std::isfinite(pmin) || !std::isfinite(pmax)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "non-finite position");
+    /* unwrapped index of the cell containing x (periodic: any x; else clamped to the domain) */
+    auto cell_of = [&](double x) {
+      long long m = 0;
+      if (ctx->g.periodic[a]) {
+        m = (long long)floor((x - xf[0]) / L);
+        x -= m * L;
+      }
+      int c = gks_host_find_cell(ctx, a, x);
+      if (c < 0) c = x < xf[0] ? 0 : nn - 1;
+      return (long long)c + m * nn;
+    };
+    long long l = cell_of(pmin - R) - 1, h = cell_of(pmax + R) + 1;
+    if (ctx->g.periodic[a]) {
+      if (2.0 * R >= L) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "alm: 6 eps must be smaller than a periodic axis");
+      if (h - l + 1 > nn) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "alm: point cloud + support wider than a periodic axis");
+    } else {
+      if (l < 0) l = 0;
+      if (h > nn - 1) h = nn - 1;
+    }
+    if (h < l) h = l;
+    lo[a] = (int)l;
+    cnt[a] = (int)(h - l + 1);
+  }
+  const cudaMemcpyKind kind = gks_is_device_ptr(pos) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  const cudaMemcpyKind kindf = gks_is_device_ptr(force) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  CUDA_TRY(ctx, cudaMemcpyAsync(ctx->alm_pos, pos, 3 * (size_t)n * sizeof(double), kind, ctx->stream));
+  CUDA_TRY(ctx, cudaMemcpyAsync(ctx->alm_force, force, 3 * (size_t)n * sizeof(double), kindf, ctx->stream));
+  if (kind == cudaMemcpyHostToDevice || kindf == cudaMemcpyHostToDevice)
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream)); /* caller may reuse its arrays at once */
+  for (int a = 0; a < 3; ++a) {
+    ctx->alm_lo[a] = lo[a];
+    ctx->alm_cnt[a] = cnt[a];
+  }
+  ctx->n_alm = n;
+  ctx->alm_eps = eps;
+  return GKS_OK;
+}
+
+gks_status ibm_set_points(gks_ctx *ctx, int n, const double *pos, const double *weights) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (n < 0 || n > ctx->ibm_capacity)
+    return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "n out of range (capacity of this context: %d)", ctx->ibm_capacity);
+  if (n == 0) {
+    ctx->n_ibm = 0;
+    return GKS_OK;
+  }
+  if (!pos || !weights) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "pos/weights is NULL");
+  std::vector<double> hp;
+  if (gks_status st = fetch_host(ctx, pos, 3 * (size_t)n, hp)) return st;
+  for (int p = 0; p < n; ++p)
+    for (int a = 0; a < 3; ++a) {
+      const int c0 = gks_host_find_cell(ctx, a, hp[3 * p + a]);
+      if (c0 < 0) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "ibm: point %d lies outside the domain", p);
+      const double *w = ctx->h_w[a] + GKS_NG;
+      if (fabs(w[c0 - 1] - w[c0]) > 1e-9 * w[c0] || fabs(w[c0 + 1] - w[c0]) > 1e-9 * w[c0])
+        return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "ibm: grid not locally uniform over the support of point %d", p);
+    }
+  const cudaMemcpyKind kp = gks_is_device_ptr(pos) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  const cudaMemcpyKind kw = gks_is_device_ptr(weights) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  CUDA_TRY(ctx, cudaMemcpyAsync(ctx->ibm_pos, pos, 3 * (size_t)n * sizeof(double), kp, ctx->stream));
+  CUDA_TRY(ctx, cudaMemcpyAsync(ctx->ibm_vol, weights, (size_t)n * sizeof(double), kw, ctx->stream));
+  CUDA_TRY(ctx, cudaMemsetAsync(ctx->ibm_vel, 0, 3 * (size_t)n * sizeof(double), ctx->stream));
+  CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+  ctx->n_ibm = n;
+  return GKS_OK;
+}
+
+gks_status ibm_set_velocities(gks_ctx *ctx, const double *vel) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  const size_t bytes = 3 * (size_t)ctx->n_ibm * sizeof(double);
+  if (bytes == 0) return GKS_OK;
+  if (!vel) {
+    CUDA_TRY(ctx, cudaMemsetAsync(ctx->ibm_vel, 0, bytes, ctx->stream));
+    return GKS_OK;
+  }
+  const cudaMemcpyKind k = gks_is_device_ptr(vel) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  CUDA_TRY(ctx, cudaMemcpyAsync(ctx->ibm_vel, vel, bytes, k, ctx->stream));
+  if (k == cudaMemcpyHostToDevice) CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+  return GKS_OK;
+}
+
+gks_status gks_debug_eval_flux(gks_ctx *ctx, int dir, double *F, double *dFdt) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (dir < 0 || dir > 2 || !F || !dFdt) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "bad dir or NULL output");
+  if (!ctx->have_state) return gks_set_err(ctx, GKS_ERR_STATE, "gks_debug_eval_flux before gks_set_state");
+  const GksGrid &g = ctx->g;
+  ctx->launches += gks_launch_ghost_fill(g, ctx->ph, ctx->Wn, ctx->Wn, ctx->stream);
+  ctx->launches += gks_launch_sweep_unfused(g, ctx->ph, dir, ctx->Wn, ctx->tmpN, ctx->tmpT, ctx->flux[dir], true,
+                                            ctx->stream);
+  const size_t nf = 4 * (size_t)(g.n[0] + (dir == 0)) * (g.n[1] + (dir == 1)) * (g.n[2] + (dir == 2));
+  double *outs[2] = {F, dFdt};
+  for (int h = 0; h < 2; ++h) {
+    const double *src = ctx->flux[dir] + (size_t)h * 4 * g.FS;
+    if (gks_is_device_ptr(outs[h])) {
+      ctx->launches += gks_launch_unpack_faces(g, dir, src, outs[h], ctx->stream);
+    } else {
+      ctx->launches += gks_launch_unpack_faces(g, dir, src, ctx->Pbuf, ctx->stream);
+      CUDA_TRY(ctx, cudaMemcpyAsync(outs[h], ctx->Pbuf, nf * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+      CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    }
+  }
+  CUDA_TRY(ctx, cudaGetLastError());
+  return GKS_OK;
+}
+
+gks_status gks_debug_set_sweep(gks_ctx *ctx, int mode) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (mode != 0 && mode != 1) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "mode must be 0 or 1");
+  ctx->sweep_mode = mode;
+  return GKS_OK;
+}
+
+gks_status gks_check_finite(gks_ctx *ctx) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (!ctx->have_state) return gks_set_err(ctx, GKS_ERR_STATE, "no state set");
+  int *flag = (int *)(ctx->red + 1536);
+  int h = 0;
+  CUDA_TRY(ctx, cudaMemsetAsync(flag, 0, sizeof(int), ctx->stream));
+  ctx->launches += gks_launch_check_finite(ctx->g, ctx->Wn, flag, ctx->stream);
+  CUDA_TRY(ctx, cudaMemcpyAsync(&h, flag, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+  CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+  if (h) return gks_set_err(ctx, GKS_ERR_NONFINITE, "state holds a NaN or Inf");
+  return GKS_OK;
+}
+
+} /* extern "C" */

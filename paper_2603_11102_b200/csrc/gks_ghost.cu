@@ -1,0 +1,198 @@
+/*
+ * gks_ghost.cu — ghost-cell fill for the six boundary kinds (formulas
+ * DESIGN.md S17-S21), convective-outflow ghost state (S20), pack/unpack between the C-ABI interior
+ * layout and the padded HBM layout.
+ *
+ * Pass order x, y, z; pass y also covers the i-ghosts, pass z covers i- and j-ghosts, so edges and
+ * corners are defined.  One thread fills the 3 ghosts x 4 components of one line end.
+ */
+#include "gks_internal.h"
+
+namespace {
+
+enum { BC_PERIODIC = 0, BC_NOSLIP = 1, BC_SLIP = 2, BC_INFLOW = 3, BC_OUTFLOW = 4, BC_EXTRAP = 5 };
+
+/* AX = axis being filled; (u,v) run over the two other axes: u the lower one */
+template <int AX>
+__global__ void __launch_bounds__(128) k_ghost(GksGrid g, GksPhys ph, double *W,
+                                               const double *Wstate /* may alias W */, int ulo, int ucnt, int vlo,
+                                               int vcnt) {
+  constexpr int UA = AX == 0 ? 1 : 0, VA = AX == 2 ? 1 : 2;
+  const int iu = blockIdx.x * blockDim.x + threadIdx.x;
+  const int iv = blockIdx.y;
+  const int side = blockIdx.z;
+  if (iu >= ucnt || iv >= vcnt) return;
+  int p[3];
+  p[UA] = ulo + iu;
+  p[VA] = vlo + iv;
+  p[AX] = 0;
+  const bool tang_interior = p[UA] >= 0 && p[UA] < g.n[UA] && p[VA] >= 0 && p[VA] < g.n[VA];
+  const long long base = g.idx(p[0], p[1], p[2]); /* cell 0 of the line */
+  const long long sa = g.st[AX];
+  const int n = g.n[AX];
+  const int kind = ph.bc[2 * AX + side];
+  const int first = side == 0 ? 0 : n - 1;
+
+  double qin[4] = {0, 0, 0, 0};
+  if (kind == BC_INFLOW) {
+    const double sign = side == 0 ? -1.0 : 1.0;
+    const double rhoI = W[base + first * sa];
+    const double UnI = sign * W[(1 + AX) * g.FS + base + first * sa] / rhoI;
+    const double Unb = sign * ph.inflow[1 + AX];
+    const double rhob = rhoI * exp((UnI - Unb) / sqrt(ph.RT));
+    qin[0] = rhob;
+    qin[1] = rhob * ph.inflow[1];
+    qin[2] = rhob * ph.inflow[2];
+    qin[3] = rhob * ph.inflow[3];
+  }
+#pragma unroll
+  for (int gi = 1; gi <= GKS_NG; ++gi) {
+    const int ghost = side == 0 ? -gi : n - 1 + gi;
+    const int mirror = side == 0 ? gi - 1 : n - gi;
+    const int image = side == 0 ? n - gi : gi - 1;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+      double *w = W + c * g.FS + base;
+      double q;
+      switch (kind) {
+        case BC_PERIODIC: q = w[image * sa]; break;
+        case BC_NOSLIP: q = c == 0 ? w[mirror * sa] : -w[mirror * sa]; break;
+        case BC_SLIP: q = c == 1 + AX ? -w[mirror * sa] : w[mirror * sa]; break;
+        case BC_INFLOW: q = qin[c]; break;
+        case BC_OUTFLOW:
+          q = tang_interior ? Wstate[c * g.FS + base + ghost * sa] : w[first * sa];
+          break;
+        default: q = w[first * sa]; break;
+      }
+      w[ghost * sa] = q;
+    }
+  }
+}
+
+/* S20: initialise (dt < 0) or advance (dt >= 0) the convective-outflow ghost state of axis AX */
+template <int AX>
+__global__ void __launch_bounds__(128) k_outflow(GksGrid g, GksPhys ph, double *__restrict__ W, double dt) {
+  constexpr int UA = AX == 0 ? 1 : 0, VA = AX == 2 ? 1 : 2;
+  const int iu = blockIdx.x * blockDim.x + threadIdx.x;
+  const int iv = blockIdx.y;
+  const int side = blockIdx.z & 1;
+  const int c = blockIdx.z >> 1;
+  if (iu >= g.n[UA] || iv >= g.n[VA]) return;
+  if (ph.bc[2 * AX + side] != BC_OUTFLOW) return;
+  int p[3];
+  p[UA] = iu;
+  p[VA] = iv;
+  p[AX] = 0;
+  double *w = W + c * g.FS + g.idx(p[0], p[1], p[2]);
+  const long long sa = g.st[AX];
+  const int n = g.n[AX];
+  const double *xc = g.xc[AX] + GKS_NG;
+  const double Uc = fabs(ph.inflow[1 + AX]);
+  double prev = w[(side == 0 ? 0 : n - 1) * sa];
+  for (int gi = 1; gi <= GKS_NG; ++gi) {
+    const int ghost = side == 0 ? -gi : n - 1 + gi;
+    const int inner = side == 0 ? -gi + 1 : n - 2 + gi;
+    double phi;
+    if (dt < 0) {
+      phi = prev; /* start from the last interior value */
+    } else {
+      const double C = Uc * dt / fabs(xc[ghost] - xc[inner]);
+      phi = w[ghost * sa];
+      phi = phi - C * (phi - prev);
+      prev = phi;
+    }
+    w[ghost * sa] = phi;
+  }
+}
+
+__global__ void __launch_bounds__(256) k_pack(GksGrid g, double *__restrict__ Wint, double *__restrict__ Wpad,
+                                              int to_padded, int ex, int ey, int ez) {
+  /* interior box (n + e) per axis; e = 1 along the sweep direction for face arrays */
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z;
+  const int nx = g.n[0] + ex, ny = g.n[1] + ey, nz = g.n[2] + ez;
+  if (i >= nx || j >= ny || k >= nz) return;
+  const long long ip = g.idx(i, j, k);
+  const long long ii = ((long long)k * ny + j) * nx + i;
+  const long long N = (long long)nx * ny * nz;
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    if (to_padded) Wpad[c * g.FS + ip] = Wint[c * N + ii];
+    else Wint[c * N + ii] = Wpad[c * g.FS + ip];
+  }
+}
+
+__global__ void __launch_bounds__(256) k_check_finite(GksGrid g, const double *__restrict__ W, int *flag) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z;
+  if (i >= g.n[0] || j >= g.n[1] || k >= g.n[2]) return;
+  const long long ip = g.idx(i, j, k);
+  bool bad = false;
+#pragma unroll
+  for (int c = 0; c < 4; ++c) bad |= !isfinite(W[c * g.FS + ip]);
+  if (bad) atomicOr(flag, 1);
+}
+
+template <int AX>
+void launch_ghost_axis(const GksGrid &g, const GksPhys &ph, double *W, const double *Wstate, cudaStream_t s) {
+  constexpr int UA = AX == 0 ? 1 : 0, VA = AX == 2 ? 1 : 2;
+  /* x pass: interior (j,k); y pass: all i, interior k; z pass: all i, all j */
+  const int ulo = (AX == 0) ? 0 : -GKS_NG, ucnt = (AX == 0) ? g.n[UA] : g.n[UA] + 2 * GKS_NG;
+  const int vlo = (AX == 2) ? -GKS_NG : 0, vcnt = (AX == 2) ? g.n[VA] + 2 * GKS_NG : g.n[VA];
+  dim3 grid((ucnt + 127) / 128, vcnt, 2);
+  k_ghost<AX><<<grid, 128, 0, s>>>(g, ph, W, Wstate, ulo, ucnt, vlo, vcnt);
+}
+
+template <int AX>
+int launch_outflow_axis(const GksGrid &g, const GksPhys &ph, double *W, double dt, cudaStream_t s) {
+  if (ph.bc[2 * AX] != BC_OUTFLOW && ph.bc[2 * AX + 1] != BC_OUTFLOW) return 0;
+  constexpr int UA = AX == 0 ? 1 : 0, VA = AX == 2 ? 1 : 2;
+  dim3 grid((g.n[UA] + 127) / 128, g.n[VA], 8);
+  k_outflow<AX><<<grid, 128, 0, s>>>(g, ph, W, dt);
+  return 1;
+}
+
+} /* namespace */
+
+int gks_launch_ghost_fill(const GksGrid &g, const GksPhys &ph, double *W, const double *Wstate, cudaStream_t s) {
+  launch_ghost_axis<0>(g, ph, W, Wstate, s);
+  launch_ghost_axis<1>(g, ph, W, Wstate, s);
+  launch_ghost_axis<2>(g, ph, W, Wstate, s);
+  return 3;
+}
+
+int gks_launch_outflow_init(const GksGrid &g, const GksPhys &ph, double *W, cudaStream_t s) {
+  return launch_outflow_axis<0>(g, ph, W, -1.0, s) + launch_outflow_axis<1>(g, ph, W, -1.0, s) +
+         launch_outflow_axis<2>(g, ph, W, -1.0, s);
+}
+
+int gks_launch_outflow_advance(const GksGrid &g, const GksPhys &ph, double *W, double dt, cudaStream_t s) {
+  return launch_outflow_axis<0>(g, ph, W, dt, s) + launch_outflow_axis<1>(g, ph, W, dt, s) +
+         launch_outflow_axis<2>(g, ph, W, dt, s);
+}
+
+static dim3 grid2d(int nx, int ny, int nz) { return dim3((nx + 63) / 64, (ny + 3) / 4, nz); }
+
+int gks_launch_pack(const GksGrid &g, const double *Wint, double *Wpad, cudaStream_t s) {
+  k_pack<<<grid2d(g.n[0], g.n[1], g.n[2]), dim3(64, 4), 0, s>>>(g, const_cast<double *>(Wint), Wpad, 1, 0, 0, 0);
+  return 1;
+}
+
+int gks_launch_unpack(const GksGrid &g, const double *Wpad, double *Wint, cudaStream_t s) {
+  k_pack<<<grid2d(g.n[0], g.n[1], g.n[2]), dim3(64, 4), 0, s>>>(g, Wint, const_cast<double *>(Wpad), 0, 0, 0, 0);
+  return 1;
+}
+
+int gks_launch_unpack_faces(const GksGrid &g, int dir, const double *Fpad, double *Fout, cudaStream_t s) {
+  const int ex = dir == 0, ey = dir == 1, ez = dir == 2;
+  k_pack<<<grid2d(g.n[0] + ex, g.n[1] + ey, g.n[2] + ez), dim3(64, 4), 0, s>>>(
+      g, Fout, const_cast<double *>(Fpad), 0, ex, ey, ez);
+  return 1;
+}
+
+int gks_launch_check_finite(const GksGrid &g, const double *W, int *flag, cudaStream_t s) {
+  k_check_finite<<<grid2d(g.n[0], g.n[1], g.n[2]), dim3(64, 4), 0, s>>>(g, W, flag);
+  return 1;
+}

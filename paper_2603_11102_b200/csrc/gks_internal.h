@@ -1,0 +1,112 @@
+/*
+ * gks_internal.h — internal declarations of libgks_b200 (CUDA path).  Not part of the C ABI.
+ *
+ * HBM layout.  Every field lives in ONE index space: the padded cell box with NG = 3 ghost layers,
+ *   idx(i,j,k) = ((k+3)*PY + (j+3))*PX + (i+3),   i fastest, PX = round_up(nx+6, 4) doubles,
+ * fields are separated by FS = PX*PY*PZ doubles (component-major, W[c][k][j][i]).
+ * Face-based arrays (fluxes of sweep direction d) reuse the same index space: face f along d
+ * (between cells f-1 and f, f = 0..n_d) is stored at cell index f.
+ */
+#ifndef GKS_INTERNAL_H
+#define GKS_INTERNAL_H
+
+#include <cuda_runtime.h>
+#include <stddef.h>
+
+#include "../../include/gks.h"
+
+#define GKS_NG 3
+
+/* Geometry handed to kernels by value. */
+struct GksGrid {
+  int n[3];          /* interior cells */
+  int P[3];          /* padded extents (P[0] is the pitch) */
+  long long st[3];   /* strides of i, j, k in doubles: 1, PX, PX*PY */
+  long long FS;      /* field stride */
+  /* per-axis coordinate tables on the device, indexed with (cell index + 3), length n+6 (+1 for xf) */
+  const double *xf[3];     /* faces  -3 .. n+3 */
+  const double *xc[3];     /* centres -3 .. n+2 */
+  const double *w[3];      /* widths */
+  const double *inv_w[3];  /* 1/width */
+  const double *inv_hn[3]; /* 1/(xc[f]-xc[f-1]) for face f = -2 .. n+2, stored at f+3 */
+  int uniform[3];
+  double x0[3], dx[3];
+  int periodic[3];
+  __host__ __device__ long long idx(int i, int j, int k) const {
+    return ((long long)(k + GKS_NG) * P[1] + (j + GKS_NG)) * P[0] + (i + GKS_NG);
+  }
+};
+
+struct GksPhys {
+  double RT, lambda, mu, weno_eps; /* mu = rho_ref*nu */
+  double inflow[4];
+  int bc[6];
+};
+
+struct gks_ctx {
+  gks_config cfg;
+  GksGrid g;
+  GksPhys ph;
+  cudaStream_t stream;
+  bool have_state;
+  int sweep_mode;             /* 0 fused, 1 unfused */
+  long long launches;
+  char err[512];
+
+  /* workspace carve (device) */
+  double *Wn, *Ws, *Pbuf;      /* padded 4-field states; Pbuf doubles as staging between steps */
+  double *flux[3];             /* per direction: F[4] then dF[4], padded index space */
+  double *tmpN, *tmpT;         /* unfused sweep intermediates: 8 and 24 padded fields */
+  double *coords;              /* coordinate tables */
+  double *red;                 /* reduction scratch (partials + result) */
+  double *alm_pos, *alm_force; /* GKS_MAX_ALM_POINTS*3 each */
+  double *ibm_pos, *ibm_vol, *ibm_vel, *ibm_coef; /* capacity fixed at create */
+  int ibm_capacity;
+
+  /* host-side mirrors of the coordinate tables (validation, bounding boxes) */
+  double *h_xf[3], *h_xc[3], *h_w[3];
+
+  /* forcing state */
+  double gacc[3];
+  int bulk_axis;
+  double bulk_target, total_volume;
+  int n_alm;
+  double alm_eps;
+  int alm_lo[3], alm_cnt[3];   /* bounding box of the ALM support in (unwrapped) cell indices */
+  int n_ibm;
+};
+
+/* ---- host helpers shared by the API translation units ---- */
+gks_status gks_set_err(gks_ctx *ctx, gks_status st, const char *fmt, ...);
+bool gks_is_device_ptr(const void *p);
+int gks_host_find_cell(const gks_ctx *ctx, int a, double x); /* interior cell containing x, or -1 */
+
+/* ---- kernel launchers (each returns the number of kernels it enqueued) ---- */
+int gks_launch_ghost_fill(const GksGrid &g, const GksPhys &ph, double *W, const double *Wstate, cudaStream_t s);
+int gks_launch_outflow_init(const GksGrid &g, const GksPhys &ph, double *W, cudaStream_t s);
+int gks_launch_outflow_advance(const GksGrid &g, const GksPhys &ph, double *W, double dt, cudaStream_t s);
+int gks_launch_pack(const GksGrid &g, const double *Wint, double *Wpad, cudaStream_t s);
+int gks_launch_unpack(const GksGrid &g, const double *Wpad, double *Wint, cudaStream_t s);
+int gks_launch_unpack_faces(const GksGrid &g, int dir, const double *Fpad, double *Fout, cudaStream_t s);
+
+/* sweep of one direction: fills flux[dir] (F and dF; stage 2 needs only dF) */
+int gks_launch_sweep_unfused(const GksGrid &g, const GksPhys &ph, int dir, const double *W, double *tmpN,
+                             double *tmpT, double *flux, bool need_F, cudaStream_t s);
+
+int gks_launch_stage1(const GksGrid &g, const double *Wn, double *const flux[3], double dt, double *Ws,
+                      double *Pbuf, cudaStream_t s);
+int gks_launch_stage2(const GksGrid &g, const double *Pbuf, double *const flux[3], double dt, double *Wn,
+                      cudaStream_t s);
+
+int gks_launch_bulk_reduce(const GksGrid &g, const double *W, int axis, double *red, cudaStream_t s);
+int gks_launch_uniform_force(const GksGrid &g, double *W, double dt, const double gacc[3], int bulk_axis,
+                             double bulk_target, double total_volume, const double *red, cudaStream_t s);
+int gks_launch_ibm_interp(const GksGrid &g, const double *W, int n, const double *pos, const double *vol,
+                          const double *vel, double *coef, cudaStream_t s);
+int gks_launch_ibm_spread(const GksGrid &g, double *W, int n, const double *pos, const double *coef,
+                          cudaStream_t s);
+int gks_launch_alm(const GksGrid &g, double *W, int n, const double *pos, const double *force, double eps,
+                   double dt, const int lo[3], const int cnt[3], cudaStream_t s);
+int gks_launch_check_finite(const GksGrid &g, const double *W, int *flag, cudaStream_t s);
+
+#endif

@@ -1,0 +1,55 @@
+/*
+ * gks_update.cu — flux divergence (Eq. 5) fused with the two S2O4 stage updates
+ * (formulas DESIGN.md S11):
+ *   stage 1:  L = -sum_d (F_d+ - F_d-)/Delta_d, dL likewise from dF/dt, kept in registers;
+ *             W* = W^n + dt/2 L + dt^2/8 dL,   P = W^n + dt L + dt^2/6 dL
+ *   stage 2:  W^{n+1} = P + dt^2/3 dL(W*)
+ * HBM-bound: per cell and component stage 1 reads 12 face values (6 distinct lines, neighbours hit
+ * L1/L2) + W and writes 2; stage 2 reads 6 + P and writes 1.
+ */
+#include "gks_internal.h"
+
+namespace {
+
+template <bool STAGE1>
+__global__ void __launch_bounds__(256) k_update(GksGrid g, const double *__restrict__ Win,
+                                                const double *__restrict__ fx, const double *__restrict__ fy,
+                                                const double *__restrict__ fz, double dt,
+                                                double *__restrict__ out1, double *__restrict__ out2) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z;
+  if (i >= g.n[0] || j >= g.n[1]) return;
+  const long long id = g.idx(i, j, k);
+  const double iwx = g.inv_w[0][i + GKS_NG], iwy = g.inv_w[1][j + GKS_NG], iwz = g.inv_w[2][k + GKS_NG];
+  const long long sy = g.st[1], sz = g.st[2];
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    const long long o = c * g.FS + id, od = (4 + c) * g.FS + id;
+    const double dL = -((fx[od + 1] - fx[od]) * iwx + (fy[od + sy] - fy[od]) * iwy + (fz[od + sz] - fz[od]) * iwz);
+    if (STAGE1) {
+      const double L = -((fx[o + 1] - fx[o]) * iwx + (fy[o + sy] - fy[o]) * iwy + (fz[o + sz] - fz[o]) * iwz);
+      const double w = Win[o];
+      out1[o] = w + 0.5 * dt * L + (dt * dt / 8.0) * dL;
+      out2[o] = w + dt * L + (dt * dt / 6.0) * dL;
+    } else {
+      out1[o] = Win[o] + (dt * dt / 3.0) * dL;
+    }
+  }
+}
+
+} /* namespace */
+
+int gks_launch_stage1(const GksGrid &g, const double *Wn, double *const flux[3], double dt, double *Ws,
+                      double *Pbuf, cudaStream_t s) {
+  dim3 blk(64, 4), grid((g.n[0] + 63) / 64, (g.n[1] + 3) / 4, g.n[2]);
+  k_update<true><<<grid, blk, 0, s>>>(g, Wn, flux[0], flux[1], flux[2], dt, Ws, Pbuf);
+  return 1;
+}
+
+int gks_launch_stage2(const GksGrid &g, const double *Pbuf, double *const flux[3], double dt, double *Wn,
+                      cudaStream_t s) {
+  dim3 blk(64, 4), grid((g.n[0] + 63) / 64, (g.n[1] + 3) / 4, g.n[2]);
+  k_update<false><<<grid, blk, 0, s>>>(g, Pbuf, flux[0], flux[1], flux[2], dt, Wn, nullptr);
+  return 1;
+}

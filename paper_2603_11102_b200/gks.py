@@ -1,0 +1,235 @@
+"""Thin Python binding of libgks_b200.so (include/gks.h).  Argument marshalling only: every step of
+the path runs in the library's CUDA kernels.  PyTorch supplies device memory and the stream.
+
+There is no CPU fallback: if the library is missing or no CUDA device is present this module raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libgks_b200.so")
+_LIB = None
+_dp = C.POINTER(C.c_double)
+
+GKS_OK = 0
+STATUS = {0: "GKS_OK", 1: "GKS_ERR_INVALID_ARG", 2: "GKS_ERR_WORKSPACE", 3: "GKS_ERR_CUDA",
+          4: "GKS_ERR_STATE", 5: "GKS_ERR_NONFINITE"}
+
+EXPORTS = ["gks_workspace_bytes", "gks_create", "gks_destroy", "gks_set_state", "gks_get_state", "gks_step",
+           "gks_set_body_force", "gks_set_bulk_flux", "alm_set_points", "ibm_set_points", "ibm_set_velocities",
+           "gks_debug_eval_flux", "gks_debug_set_sweep", "gks_check_finite", "gks_launch_count", "gks_last_error"]
+
+
+class GksConfig(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
+                ("xf", _dp), ("yf", _dp), ("zf", _dp),
+                ("x0", C.c_double), ("y0", C.c_double), ("z0", C.c_double),
+                ("dx", C.c_double), ("dy", C.c_double), ("dz", C.c_double),
+                ("RT", C.c_double), ("nu", C.c_double), ("rho_ref", C.c_double),
+                ("bc", C.c_int * 6), ("inflow", C.c_double * 4), ("weno_eps", C.c_double)]
+
+
+class GksError(RuntimeError):
+    def __init__(self, status, message):
+        super().__init__("%s: %s" % (STATUS.get(status, status), message))
+        self.status = status
+
+
+def lib():
+    """Load libgks_b200.so (built in-tree by paper_2603_11102_b200/build.py).  Fails loudly if absent."""
+    global _LIB
+    if _LIB is None:
+        if not os.path.exists(_LIB_PATH):
+            raise ImportError("libgks_b200.so is not built (run `python -m paper_2603_11102_b200.build`); "
+                              "there is no CPU fallback")
+        L = C.CDLL(_LIB_PATH)
+        vp = C.c_void_p
+        L.gks_workspace_bytes.argtypes = [C.POINTER(GksConfig)]
+        L.gks_workspace_bytes.restype = C.c_size_t
+        L.gks_create.argtypes = [C.POINTER(GksConfig), vp, C.c_size_t, vp, C.POINTER(vp)]
+        L.gks_destroy.argtypes = [vp]
+        L.gks_set_state.argtypes = [vp, vp]
+        L.gks_get_state.argtypes = [vp, vp]
+        L.gks_step.argtypes = [vp, C.c_double]
+        L.gks_set_body_force.argtypes = [vp, C.c_double, C.c_double, C.c_double]
+        L.gks_set_bulk_flux.argtypes = [vp, C.c_int, C.c_double]
+        L.alm_set_points.argtypes = [vp, C.c_int, vp, vp, C.c_double]
+        L.ibm_set_points.argtypes = [vp, C.c_int, vp, vp]
+        L.ibm_set_velocities.argtypes = [vp, vp]
+        L.gks_debug_eval_flux.argtypes = [vp, C.c_int, vp, vp]
+        L.gks_debug_set_sweep.argtypes = [vp, C.c_int]
+        L.gks_check_finite.argtypes = [vp]
+        L.gks_launch_count.argtypes = [vp]
+        L.gks_launch_count.restype = C.c_longlong
+        L.gks_last_error.argtypes = [vp]
+        L.gks_last_error.restype = C.c_char_p
+        _LIB = L
+    return _LIB
+
+
+def make_config(cfg):
+    """workloads.GridConfig -> (GksConfig, keep-alive list)"""
+    c = GksConfig()
+    c.nx, c.ny, c.nz = cfg.n
+    keep = [None if f is None else np.ascontiguousarray(f, dtype=np.float64) for f in cfg.faces]
+    c.xf, c.yf, c.zf = [None if f is None else f.ctypes.data_as(_dp) for f in keep]
+    c.x0, c.y0, c.z0 = cfg.origin
+    c.dx, c.dy, c.dz = cfg.spacing
+    c.RT, c.nu, c.rho_ref = cfg.RT, cfg.nu, cfg.rho_ref
+    c.bc = (C.c_int * 6)(*cfg.bc)
+    c.inflow = (C.c_double * 4)(*cfg.inflow)
+    c.weno_eps = cfg.weno_eps
+    return c, keep
+
+
+def _ptr(x):
+    """host numpy array or torch tensor (host or device) -> (address, keep-alive)"""
+    if x is None:
+        return None, None
+    if isinstance(x, np.ndarray):
+        a = np.ascontiguousarray(x, dtype=np.float64)
+        return a.ctypes.data, a
+    import torch
+    if isinstance(x, torch.Tensor):
+        assert x.dtype == torch.float64 and x.is_contiguous()
+        return x.data_ptr(), x
+    a = np.ascontiguousarray(np.asarray(x, dtype=np.float64))
+    return a.ctypes.data, a
+
+
+class Gks:
+    """One solver context on the current CUDA device.  `stream` is a torch.cuda.Stream (default: a new one)."""
+
+    def __init__(self, cfg, stream=None, device="cuda:0"):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: the gas-kinetic step has no CPU fallback")
+        L = lib()
+        self._torch = torch
+        self.device = torch.device(device)
+        self.n = tuple(cfg.n)
+        c, keep = make_config(cfg)
+        nbytes = L.gks_workspace_bytes(C.byref(c))
+        if nbytes == 0:
+            h = C.c_void_p()
+            st = L.gks_create(C.byref(c), None, 0, None, C.byref(h))
+            raise GksError(st, L.gks_last_error(None).decode())
+        with torch.cuda.device(self.device):
+            self.stream = stream if stream is not None else torch.cuda.Stream(device=self.device)
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        base = self.workspace.data_ptr()
+        aligned = (base + 255) // 256 * 256
+        self.workspace_bytes = nbytes
+        self._h = C.c_void_p()
+        st = L.gks_create(C.byref(c), C.c_void_p(aligned), nbytes, C.c_void_p(self.stream.cuda_stream),
+                          C.byref(self._h))
+        if st != GKS_OK:
+            self._h = None
+            raise GksError(st, L.gks_last_error(None).decode())
+        self.n_ibm = 0
+
+    # -- helpers
+    def _check(self, st):
+        if st != GKS_OK:
+            raise GksError(st, lib().gks_last_error(self._h).decode())
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().gks_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def shape(self):
+        nx, ny, nz = self.n
+        return (4, nz, ny, nx)
+
+    def face_shape(self, d):
+        nx, ny, nz = self.n
+        return (4, nz + (d == 2), ny + (d == 1), nx + (d == 0))
+
+    # -- the C ABI, same names
+    def set_state(self, W):
+        p, keep = _ptr(W)
+        self._check(lib().gks_set_state(self._h, p))
+        if isinstance(keep, np.ndarray):
+            self.synchronize()      # pageable host source: be safe before the caller frees it
+
+    def get_state(self, out=None):
+        """Returns a host numpy array, or fills `out` (numpy array or torch tensor, host or device)."""
+        if out is None:
+            out = np.empty(self.shape)
+        p, _ = _ptr(out)
+        self._check(lib().gks_get_state(self._h, p))
+        return out
+
+    def step(self, dt):
+        self._check(lib().gks_step(self._h, float(dt)))
+
+    def set_body_force(self, gx, gy, gz):
+        self._check(lib().gks_set_body_force(self._h, gx, gy, gz))
+
+    def set_bulk_flux(self, axis, target):
+        self._check(lib().gks_set_bulk_flux(self._h, int(axis), float(target)))
+
+    def alm_set_points(self, pos, force, eps):
+        n = 0 if pos is None else (pos.shape[0] if hasattr(pos, "shape") else len(pos))
+        pp, k1 = _ptr(pos)
+        pf, k2 = _ptr(force)
+        self._check(lib().alm_set_points(self._h, n, pp, pf, float(eps)))
+
+    def ibm_set_points(self, pos, weights):
+        n = 0 if pos is None else (pos.shape[0] if hasattr(pos, "shape") else len(pos))
+        pp, k1 = _ptr(pos)
+        pw, k2 = _ptr(weights)
+        self._check(lib().ibm_set_points(self._h, n, pp, pw))
+        self.n_ibm = n
+
+    def ibm_set_velocities(self, vel):
+        pv, k = _ptr(vel)
+        self._check(lib().ibm_set_velocities(self._h, pv))
+
+    def debug_eval_flux(self, d):
+        F, dF = np.empty(self.face_shape(d)), np.empty(self.face_shape(d))
+        self._check(lib().gks_debug_eval_flux(self._h, d, F.ctypes.data, dF.ctypes.data))
+        return F, dF
+
+    def debug_set_sweep(self, mode):
+        """0 = fused production kernels, 1 = unfused cross-check kernels"""
+        self._check(lib().gks_debug_set_sweep(self._h, int(mode)))
+
+    def check_finite(self):
+        self._check(lib().gks_check_finite(self._h))
+
+    @property
+    def launch_count(self):
+        return lib().gks_launch_count(self._h)
+
+    def synchronize(self):
+        self.stream.synchronize()
+
+
+def run_workload(w, steps=None, sweep=None):
+    """Run a workloads.Workload through the C ABI; returns the final state (host numpy array)."""
+    g = Gks(w.cfg)
+    if sweep is not None:
+        g.debug_set_sweep(sweep)
+    if w.bulk_flux is not None:
+        g.set_bulk_flux(*w.bulk_flux)
+    if w.ibm is not None:
+        g.ibm_set_points(*w.ibm)
+    g.set_state(w.W0)
+    for s in range(w.steps if steps is None else steps):
+        if w.alm is not None:
+            g.alm_set_points(*w.alm(s))
+        g.step(w.dt)
+    W = g.get_state()
+    g.close()
+    return W

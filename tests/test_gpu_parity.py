@@ -1,0 +1,146 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle, element by element on the same
+seeded inputs.  Bar (BASELINE.json north_star): relative L-inf (norm S24) <= 1e-11 after one step,
+<= 1e-9 after ten steps, fp64."""
+import numpy as np
+import pytest
+
+from conftest import rel_linf
+from paper_2603_11102_b200 import workloads as wl
+from paper_2603_11102_b200.workloads import GridConfig
+
+pytestmark = pytest.mark.gpu
+
+TOL1, TOL10 = 1e-11, 1e-9
+P, NS, SL, IN, OUT, EX = range(6)
+
+
+def run_oracle(w, steps):
+    from oracle import binding as ob
+    o = ob.Oracle(w.cfg)
+    if w.bulk_flux is not None:
+        o.set_bulk_flux(*w.bulk_flux)
+    if w.ibm is not None:
+        o.ibm_set_points(*w.ibm)
+    o.set_state(w.W0)
+    for s in range(steps):
+        if w.alm is not None:
+            o.alm_set_points(*w.alm(s))
+        o.step(w.dt)
+    W = o.get_state()
+    o.close()
+    return W
+
+
+def run_gpu(w, steps, sweep=None):
+    from paper_2603_11102_b200 import gks
+    return gks.run_workload(w, steps, sweep=sweep)
+
+
+@pytest.mark.parametrize("sweep", [0, 1])
+def test_C1_taylor_green_one_and_ten_steps(sweep):
+    w = wl.by_name("C1")
+    e1 = rel_linf(run_gpu(w, 1, sweep), run_oracle(w, 1))
+    assert e1 <= TOL1, e1
+    e10 = rel_linf(run_gpu(w, 10, sweep), run_oracle(w, 10))
+    assert e10 <= TOL10, e10
+
+
+@pytest.mark.parametrize("sweep", [0, 1])
+@pytest.mark.parametrize("d", [0, 1, 2])
+def test_face_fluxes_match_the_oracle(d, sweep):
+    from oracle import binding as ob
+    from paper_2603_11102_b200 import gks
+    w = wl.taylor_green(20)
+    o = ob.Oracle(w.cfg)
+    o.set_state(w.W0)
+    Fo, dFo = o.eval_flux(d)
+    g = gks.Gks(w.cfg)
+    g.debug_set_sweep(sweep)
+    g.set_state(w.W0)
+    Fg, dFg = g.debug_eval_flux(d)
+    g.close()
+    assert np.abs(Fg - Fo).max() <= 1e-13 * np.abs(Fo).max()
+    assert np.abs(dFg - dFo).max() <= 1e-12 * np.abs(dFo).max()
+
+
+@pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5"])
+def test_small_variants_of_the_configs(name):
+    """reduced grids with the structure of configs 2-5 (walls + stretching + bulk flux; IBM cylinder with
+    inflow/convective outflow; rotating ALM rotor; ALM + IBM nacelle/tower)"""
+    w = wl.by_name(name, small=True)
+    e1 = rel_linf(run_gpu(w, 1), run_oracle(w, 1))
+    assert e1 <= TOL1, e1
+    e10 = rel_linf(run_gpu(w, 10), run_oracle(w, 10))
+    assert e10 <= TOL10, e10
+
+
+@pytest.mark.parametrize("n", [(6, 6, 6), (37, 11, 9), (7, 70, 6), (9, 6, 45)])
+@pytest.mark.parametrize("bc", [(P,) * 6, (IN, OUT, NS, SL, EX, EX), (EX, IN, P, P, OUT, NS), (SL, SL, OUT, IN, P, P)])
+def test_ragged_sizes_and_every_boundary_kind(n, bc):
+    """minimum size, sizes that are no multiple of any tile, stretched axes, all six boundary kinds"""
+    rng = np.random.default_rng(hash((n, bc)) % 2 ** 32)
+    zf = np.cumsum(np.r_[0.0, rng.uniform(0.8, 1.2, n[2])]) * 0.1
+    cfg = GridConfig(n=n, faces=(None, None, zf), spacing=(0.1, 0.12, 0.1), nu=2e-3, bc=bc,
+                     inflow=(1.0, 0.1, 0.1, 0.1))
+    W0 = np.empty((4, n[2], n[1], n[0]))
+    W0[0] = 1.0 + 0.02 * rng.standard_normal(W0[0].shape)
+    W0[1:] = 0.1 + 0.03 * rng.standard_normal(W0[1:].shape)
+    w = wl.Workload("ragged", cfg, W0, wl.cfl_dt(cfg, W0), 3)
+    e1 = rel_linf(run_gpu(w, 1), run_oracle(w, 1))
+    assert e1 <= TOL1, e1
+    e3 = rel_linf(run_gpu(w, 3), run_oracle(w, 3))
+    assert e3 <= 10 * TOL1, e3
+
+
+def test_body_force_and_device_pointers():
+    import torch
+    from oracle import binding as ob
+    from paper_2603_11102_b200 import gks
+    w = wl.by_name("C2", small=True)
+    o = ob.Oracle(w.cfg)
+    o.set_body_force(0.01, -0.02, 0.03)
+    o.set_state(w.W0)
+    o.step(w.dt)
+    g = gks.Gks(w.cfg)
+    g.set_body_force(0.01, -0.02, 0.03)
+    with torch.cuda.stream(g.stream):
+        Wd = torch.from_numpy(w.W0).to("cuda:0")
+        out = torch.empty_like(Wd)
+    g.stream.synchronize()
+    g.set_state(Wd)                       # device pointers in and out
+    g.step(w.dt)
+    g.get_state(out)
+    g.synchronize()
+    assert rel_linf(out.cpu().numpy(), o.get_state()) <= TOL1
+    g.check_finite()
+    assert g.launch_count > 0
+    g.close()
+
+
+def test_error_paths_on_the_device():
+    from paper_2603_11102_b200 import gks
+    w = wl.by_name("C1")
+    g = gks.Gks(w.cfg)
+    with pytest.raises(gks.GksError) as e:
+        g.step(w.dt)                      # before set_state
+    assert e.value.status == 4
+    g.set_state(w.W0)
+    with pytest.raises(gks.GksError):
+        g.step(-1.0)
+    with pytest.raises(gks.GksError):
+        g.alm_set_points(np.zeros((1, 3)), np.zeros((1, 3)), 0.0)
+    with pytest.raises(gks.GksError):
+        g.alm_set_points(np.zeros((1, 3)), np.zeros((1, 3)), 2.0)      # 6 eps wider than the periodic box
+    g.alm_set_points(np.zeros((0, 3)), np.zeros((0, 3)), 1.0)          # n = 0 clears
+    bad = w.W0.copy()
+    bad[1, 3, 4, 5] = np.nan
+    g.set_state(bad)
+    with pytest.raises(gks.GksError) as e:
+        g.check_finite()
+    assert e.value.status == 5
+    g.close()
+    cfg = GridConfig(n=(8, 8, 8), spacing=(0.1,) * 3, bc=(EX,) * 6)
+    g = gks.Gks(cfg)
+    with pytest.raises(gks.GksError):
+        g.ibm_set_points(np.array([[-0.5, 0.1, 0.1]]), np.array([1.0]))  # outside the domain
+    g.close()
