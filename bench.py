@@ -1,0 +1,278 @@
+#!/usr/bin/env python
+"""bench.py — S2O4 GKS Mcell-steps/s (fp64) on the 256^3 periodic Taylor-Green box (workload M0).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload M0|C1..C5]
+
+A "step" is one pass of the whole hot path (ghost fill, three fused sweeps, stage update, twice, then
+forcing) over the whole grid.  Prints ONE JSON line (rank 0).  See DESIGN.md §Measurement for the
+definitions of `roofline`, `e2e` and `cpu_baseline`.
+
+Multi-GPU: the path is built for one GPU (BASELINE.json north_star: no sharding, no collectives), so
+--gpus N runs N independent replicas, one per rank ("replicas only", weak scaling).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "S2O4 GKS Mcell-steps/s (fp64)"
+UNIT = "Mcell-steps/s"
+# Algorithmic fp64 flops of one cell-step (plain count of +,-,*,/ and one per
+# erfc/exp/sqrt, smoothness indicators shared between the two points of a cell, Navier-Stokes closed
+# form for the Gauss-point flux): per face 4726 (stage 1) + 4654 (stage 2), 3 faces per cell, + update.
+FLOPS_PER_FACE = {True: 4726.0, False: 4654.0}     # need_F (stage 1) / dF only (stage 2)
+FLOPS_PER_CELL_STEP = 3 * (FLOPS_PER_FACE[True] + FLOPS_PER_FACE[False]) + 60.0
+
+
+def read_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return json.load(f), "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=lambda: self.lines.extend(self.proc.stdout), daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm, smax, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1]))
+                smax = float(f[2])
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": smax,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def setup_solver(w, gks, device):
+    g = gks.Gks(w.cfg, device=device)
+    if w.bulk_flux is not None:
+        g.set_bulk_flux(*w.bulk_flux)
+    if w.ibm is not None:
+        g.ibm_set_points(*w.ibm)
+    return g
+
+
+def oracle_rate(sample_n, steps, warmup=0):
+    """Mcell-steps/s of the CPU oracle, as it stands, on a Taylor-Green box of sample_n^3 cells."""
+    from oracle import binding as ob
+    from paper_2603_11102_b200 import workloads as wl
+    w = wl.taylor_green(sample_n)
+    o = ob.Oracle(w.cfg)
+    o.set_state(w.W0)
+    for _ in range(warmup):
+        o.step(w.dt)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        o.step(w.dt)
+    dt = time.perf_counter() - t0
+    o.close()
+    cores = len(os.sched_getaffinity(0))
+    return w.cfg.cells * steps / dt / 1e6, dt, cores
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the CPU oracle (the only reference this tier has), timed as it stands on the
+    host cores; each step is one oracle step on a bounded sample (64^3 box of the same workload)."""
+    if rank != 0:
+        return
+    sample = 64
+    rate, secs, cores = oracle_rate(sample, args.steps, args.warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": secs / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": "M0 periodic Taylor-Green 256^3 (oracle timed on a %d^3 sample)" % sample},
+            "cpu_baseline": {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": "%d step(s) of the %d^3 Taylor-Green box" % (args.steps, sample)},
+            "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="M0")
+    ap.add_argument("--sweep", type=int, default=0, help="0 fused (production), 1 unfused cross-check kernels")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        return run_reference(args, rank, world)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2603_11102_b200 import gks, workloads as wl
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    device = "cuda:%d" % local_rank
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device(device))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    w = wl.by_name(args.workload)
+    g = setup_solver(w, gks, device)
+    g.debug_set_sweep(args.sweep)
+    cells = w.cfg.cells
+    with torch.cuda.stream(g.stream):
+        Wd = torch.from_numpy(w.W0).to(device)
+    g.stream.synchronize()
+    g.set_state(Wd)
+    step_no = [0]
+
+    def one_step():
+        if w.alm is not None:
+            g.alm_set_points(*w.alm(step_no[0]))
+        g.step(w.dt)
+        step_no[0] += 1
+
+    for _ in range(max(args.warmup, 3)):
+        one_step()
+    g.synchronize()
+    fp64_peak = g.debug_fp64_peak() if rank == 0 else None
+
+    # ---- timed region: exactly K steps, device-resident state, CUDA events on the solver's stream
+    g.profile_enable(True)
+    g.profile_read()
+    l0 = g.launch_count
+    sampler = ClockSampler(local_rank)
+    barrier()
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(g.stream)
+    for _ in range(args.steps):
+        one_step()
+    e1.record(g.stream)
+    g.synchronize()
+    barrier()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1)
+    launches = g.launch_count - l0
+    prof = g.profile_read()
+    g.profile_enable(False)
+    g.check_finite()
+
+    # ---- end to end through the C ABI with HOST buffers (pinned): H2D + step + D2H every step
+    Hin = torch.from_numpy(w.W0.copy()).pin_memory()
+    Hout = torch.empty_like(Hin).pin_memory()
+    nbytes = Hin.numel() * 8
+    g.set_state(Hin)
+    g.step(w.dt)
+    g.get_state(Hout)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.e2e_steps):
+        g.set_state(Hin)
+        g.step(w.dt)
+        g.get_state(Hout)          # synchronises
+        Hin, Hout = Hout, Hin
+    barrier()
+    e2e_s = time.perf_counter() - t0
+
+    t = torch.tensor([ms, e2e_s * 1e3], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms, e2e_ms = t.tolist()
+    if rank == 0:
+        peaks, peak_src = read_peaks()
+        value = cells * world * args.steps / (ms * 1e-3) / 1e6
+        e2e_value = cells * world * args.e2e_steps / (e2e_ms * 1e-3) / 1e6
+        sweep_ms = sum(prof[k][0] for k in ("sweep_x", "sweep_y", "sweep_z"))
+        sweep_n = sum(prof[k][1] for k in ("sweep_x", "sweep_y", "sweep_z"))
+        faces = cells  # one face per cell and direction (+ one boundary plane, < 0.5 %)
+        flops_per_launch = 0.5 * (FLOPS_PER_FACE[True] + FLOPS_PER_FACE[False]) * faces
+        ach = flops_per_launch / (sweep_ms / max(sweep_n, 1) * 1e-3) / 1e12 if sweep_ms > 0 else None
+        traffic = None
+        tp = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tp) and args.workload == "M0" and args.sweep == 0:
+            with open(tp) as f:
+                traffic = json.load(f).get("sweep_dram_bytes_per_launch")
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "%s %s %dx%dx%d" % (args.workload, w.name, *w.cfg.n),
+                       "sweep": "fused" if args.sweep == 0 else "unfused",
+                       "multi_gpu": "replicas only" if world > 1 else "single GPU",
+                       "l2": "inputs larger than L2 (state %.0f MB per field set)" % (cells * 32 / 1e6)},
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
+                    "steps": args.e2e_steps},
+            "gpu_launches": int(launches),
+            "roofline": {"bound": "alu", "kernel": "sweep (reconstruction + flux), mean of 6 launches per step",
+                         "achieved": ach, "peak": fp64_peak, "unit": "TFLOP/s",
+                         "frac": (ach / fp64_peak) if (ach and fp64_peak) else None, "traffic": traffic,
+                         "peak_source": "fp64 DFMA microbenchmark in this run (gks_debug_fp64_peak)",
+                         "flops_per_launch": flops_per_launch,
+                         "share_of_step": sweep_ms / ms if ms > 0 else None},
+            "hbm": {"bytes_per_cell_step_algorithmic": 192,
+                    "achieved_gbs": 192.0 * cells * args.steps / (ms * 1e-3) / 1e9,
+                    "peak_gbs": peaks.get("hbm_gbs"), "peak_source": peak_src},
+            "kernel_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()},
+        }
+        if not args.no_cpu_baseline and world == 1:
+            rate, secs, cores = oracle_rate(64, 2)
+            line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                    "sample": "2 steps of the 64^3 Taylor-Green box (same workload, reduced n)",
+                                    "seconds": secs}
+        print(json.dumps(line), flush=True)
+    g.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -129,6 +129,20 @@ gks_status gks_debug_set_sweep(gks_ctx *ctx, int mode);
 /* Synchronising check of the current state; GKS_ERR_NONFINITE if any interior value is NaN/Inf. */
 gks_status gks_check_finite(gks_ctx *ctx);
 
+/* Per-kernel-class device timing.  When enabled, gks_step brackets each class of kernels with CUDA
+ * events on the context's stream; gks_profile_read synchronises, ADDS the elapsed milliseconds and
+ * interval counts of everything recorded since the last read into ms[GKS_PROF_N] / count[GKS_PROF_N]
+ * (host arrays the caller zeroes) and resets the recorder.  At most 4096 intervals are kept between
+ * reads (later ones are dropped). */
+enum { GKS_PROF_GHOST = 0, GKS_PROF_SWEEP_X = 1, GKS_PROF_SWEEP_Y = 2, GKS_PROF_SWEEP_Z = 3,
+       GKS_PROF_UPDATE = 4, GKS_PROF_FORCING = 5, GKS_PROF_N = 6 };
+gks_status gks_profile_enable(gks_ctx *ctx, int on);
+gks_status gks_profile_read(gks_ctx *ctx, double *ms, long long *count);
+
+/* Calibration: sustained fp64 FMA throughput of this GPU in TFLOP/s (2 flop per DFMA), measured with
+ * a register-resident DFMA kernel on the context's stream (about 50 ms).  Synchronises. */
+gks_status gks_debug_fp64_peak(gks_ctx *ctx, double *tflops);
+
 /* Number of kernels this context has launched since gks_create (for bench.py's gpu_launches). */
 long long gks_launch_count(const gks_ctx *ctx);
 

@@ -279,6 +279,7 @@ gks_status gks_create(const gks_config *cfg, void *workspace, size_t workspace_b
 gks_status gks_destroy(gks_ctx *ctx) {
   if (!ctx) return GKS_ERR_INVALID_ARG;
   cudaStreamSynchronize(ctx->stream);
+  gks_prof_free(ctx);
   for (int a = 0; a < 3; ++a) free(ctx->h_xf[a]);
   delete ctx;
   return GKS_OK;

@@ -32,9 +32,12 @@ gks_status fetch_host(gks_ctx *ctx, const double *src, size_t count, std::vector
 
 /* all sweeps of one stage into ctx->flux[] */
 void sweeps(gks_ctx *ctx, const double *W, bool need_F) {
-  for (int d = 0; d < 3; ++d)
+  for (int d = 0; d < 3; ++d) {
+    gks_prof_begin(ctx, GKS_PROF_SWEEP_X + d);
     ctx->launches += gks_launch_sweep_unfused(ctx->g, ctx->ph, d, W, ctx->tmpN, ctx->tmpT, ctx->flux[d], need_F,
                                               ctx->stream);
+    gks_prof_end(ctx);
+  }
 }
 
 } /* namespace */
@@ -82,13 +85,22 @@ gks_status gks_step(gks_ctx *ctx, double dt) {
   const GksPhys &ph = ctx->ph;
   cudaStream_t s = ctx->stream;
   /* stage 1: ghosts of W^n, F and dF/dt of the three sweeps, W* and P */
+  gks_prof_begin(ctx, GKS_PROF_GHOST);
   ctx->launches += gks_launch_ghost_fill(g, ph, ctx->Wn, ctx->Wn, s);
+  gks_prof_end(ctx);
   sweeps(ctx, ctx->Wn, true);
+  gks_prof_begin(ctx, GKS_PROF_UPDATE);
   ctx->launches += gks_launch_stage1(g, ctx->Wn, ctx->flux, dt, ctx->Ws, ctx->Pbuf, s);
+  gks_prof_end(ctx);
   /* stage 2: ghosts of W* (outflow ghost state taken from W^n, S20), dF/dt only, W^{n+1} in place of W^n */
+  gks_prof_begin(ctx, GKS_PROF_GHOST);
   ctx->launches += gks_launch_ghost_fill(g, ph, ctx->Ws, ctx->Wn, s);
+  gks_prof_end(ctx);
   sweeps(ctx, ctx->Ws, false);
+  gks_prof_begin(ctx, GKS_PROF_UPDATE);
   ctx->launches += gks_launch_stage2(g, ctx->Pbuf, ctx->flux, dt, ctx->Wn, s);
+  gks_prof_end(ctx);
+  gks_prof_begin(ctx, GKS_PROF_FORCING);
   /* forcing (Eq. 13), every increment from the un-forced field: read-only kernels first */
   const bool uniform = ctx->gacc[0] != 0.0 || ctx->gacc[1] != 0.0 || ctx->gacc[2] != 0.0;
   if (ctx->bulk_axis >= 0) ctx->launches += gks_launch_bulk_reduce(g, ctx->Wn, ctx->bulk_axis, ctx->red, s);
@@ -103,6 +115,7 @@ gks_status gks_step(gks_ctx *ctx, double dt) {
     ctx->launches += gks_launch_alm(g, ctx->Wn, ctx->n_alm, ctx->alm_pos, ctx->alm_force, ctx->alm_eps, dt,
                                     ctx->alm_lo, ctx->alm_cnt, s);
   ctx->launches += gks_launch_outflow_advance(g, ph, ctx->Wn, dt, s);
+  gks_prof_end(ctx);
   CUDA_TRY(ctx, cudaGetLastError());
   return GKS_OK;
 }

@@ -74,7 +74,16 @@ struct gks_ctx {
   double alm_eps;
   int alm_lo[3], alm_cnt[3];   /* bounding box of the ALM support in (unwrapped) cell indices */
   int n_ibm;
+
+  /* per-class event timing (gks_profile.cu) */
+  int prof_on, prof_n;
+  cudaEvent_t *prof_ev;        /* 2 * GKS_PROF_MAX events, created on first enable */
+  int *prof_cat;
 };
+#define GKS_PROF_MAX 4096
+void gks_prof_begin(gks_ctx *ctx, int cat);
+void gks_prof_end(gks_ctx *ctx);
+void gks_prof_free(gks_ctx *ctx);
 
 /* ---- host helpers shared by the API translation units ---- */
 gks_status gks_set_err(gks_ctx *ctx, gks_status st, const char *fmt, ...);

@@ -19,7 +19,8 @@ STATUS = {0: "GKS_OK", 1: "GKS_ERR_INVALID_ARG", 2: "GKS_ERR_WORKSPACE", 3: "GKS
 
 EXPORTS = ["gks_workspace_bytes", "gks_create", "gks_destroy", "gks_set_state", "gks_get_state", "gks_step",
            "gks_set_body_force", "gks_set_bulk_flux", "alm_set_points", "ibm_set_points", "ibm_set_velocities",
-           "gks_debug_eval_flux", "gks_debug_set_sweep", "gks_check_finite", "gks_launch_count", "gks_last_error"]
+           "gks_debug_eval_flux", "gks_debug_set_sweep", "gks_debug_fp64_peak",
+           "gks_profile_enable", "gks_profile_read", "gks_check_finite", "gks_launch_count", "gks_last_error"]
 
 
 class GksConfig(C.Structure):
@@ -61,6 +62,9 @@ def lib():
         L.gks_debug_eval_flux.argtypes = [vp, C.c_int, vp, vp]
         L.gks_debug_set_sweep.argtypes = [vp, C.c_int]
         L.gks_check_finite.argtypes = [vp]
+        L.gks_profile_enable.argtypes = [vp, C.c_int]
+        L.gks_profile_read.argtypes = [vp, _dp, C.POINTER(C.c_longlong)]
+        L.gks_debug_fp64_peak.argtypes = [vp, _dp]
         L.gks_launch_count.argtypes = [vp]
         L.gks_launch_count.restype = C.c_longlong
         L.gks_last_error.argtypes = [vp]
@@ -204,6 +208,23 @@ class Gks:
     def debug_set_sweep(self, mode):
         """0 = fused production kernels, 1 = unfused cross-check kernels"""
         self._check(lib().gks_debug_set_sweep(self._h, int(mode)))
+
+    PROF_NAMES = ("ghost", "sweep_x", "sweep_y", "sweep_z", "update", "forcing")
+
+    def profile_enable(self, on=True):
+        self._check(lib().gks_profile_enable(self._h, int(on)))
+
+    def profile_read(self):
+        """{class: (milliseconds, intervals)} accumulated since the last read; synchronises"""
+        ms = (C.c_double * 6)()
+        cnt = (C.c_longlong * 6)()
+        self._check(lib().gks_profile_read(self._h, ms, cnt))
+        return {n: (ms[i], cnt[i]) for i, n in enumerate(self.PROF_NAMES)}
+
+    def debug_fp64_peak(self):
+        v = C.c_double()
+        self._check(lib().gks_debug_fp64_peak(self._h, C.byref(v)))
+        return v.value
 
     def check_finite(self):
         self._check(lib().gks_check_finite(self._h))
