@@ -272,6 +272,12 @@ gks_status gks_create(const gks_config *cfg, void *workspace, size_t workspace_b
     delete ctx;
     return GKS_ERR_CUDA;
   }
+  if (!gks_fused_init(ctx)) {
+    set_err(nullptr, GKS_ERR_CUDA, "cuTensorMapEncodeTiled unavailable or failed (TMA descriptors of the fused sweep)");
+    for (int a = 0; a < 3; ++a) free(ctx->h_xf[a]);
+    delete ctx;
+    return GKS_ERR_CUDA;
+  }
   *out = ctx;
   return GKS_OK;
 }

@@ -34,8 +34,11 @@ gks_status fetch_host(gks_ctx *ctx, const double *src, size_t count, std::vector
 void sweeps(gks_ctx *ctx, const double *W, bool need_F) {
   for (int d = 0; d < 3; ++d) {
     gks_prof_begin(ctx, GKS_PROF_SWEEP_X + d);
-    ctx->launches += gks_launch_sweep_unfused(ctx->g, ctx->ph, d, W, ctx->tmpN, ctx->tmpT, ctx->flux[d], need_F,
-                                              ctx->stream);
+    if (ctx->sweep_mode == 0)
+      ctx->launches += gks_launch_sweep_fused(ctx, d, W == ctx->Wn ? 0 : 1, ctx->flux[d], need_F);
+    else
+      ctx->launches += gks_launch_sweep_unfused(ctx->g, ctx->ph, d, W, ctx->tmpN, ctx->tmpT, ctx->flux[d], need_F,
+                                                ctx->stream);
     gks_prof_end(ctx);
   }
 }
@@ -250,8 +253,11 @@ gks_status gks_debug_eval_flux(gks_ctx *ctx, int dir, double *F, double *dFdt) {
   if (!ctx->have_state) return gks_set_err(ctx, GKS_ERR_STATE, "gks_debug_eval_flux before gks_set_state");
   const GksGrid &g = ctx->g;
   ctx->launches += gks_launch_ghost_fill(g, ctx->ph, ctx->Wn, ctx->Wn, ctx->stream);
-  ctx->launches += gks_launch_sweep_unfused(g, ctx->ph, dir, ctx->Wn, ctx->tmpN, ctx->tmpT, ctx->flux[dir], true,
-                                            ctx->stream);
+  if (ctx->sweep_mode == 0)
+    ctx->launches += gks_launch_sweep_fused(ctx, dir, 0, ctx->flux[dir], true);
+  else
+    ctx->launches += gks_launch_sweep_unfused(g, ctx->ph, dir, ctx->Wn, ctx->tmpN, ctx->tmpT, ctx->flux[dir], true,
+                                              ctx->stream);
   const size_t nf = 4 * (size_t)(g.n[0] + (dir == 0)) * (g.n[1] + (dir == 1)) * (g.n[2] + (dir == 2));
   double *outs[2] = {F, dFdt};
   for (int h = 0; h < 2; ++h) {

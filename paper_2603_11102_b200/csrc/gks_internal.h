@@ -75,6 +75,9 @@ struct gks_ctx {
   int alm_lo[3], alm_cnt[3];   /* bounding box of the ALM support in (unwrapped) cell indices */
   int n_ibm;
 
+  /* TMA tensor maps of the two state buffers (Wn, Ws) for the three sweep directions (opaque CUtensorMap) */
+  alignas(64) unsigned char tmaps[2][3][128];
+
   /* per-class event timing (gks_profile.cu) */
   int prof_on, prof_n;
   cudaEvent_t *prof_ev;        /* 2 * GKS_PROF_MAX events, created on first enable */
@@ -101,6 +104,10 @@ int gks_launch_unpack_faces(const GksGrid &g, int dir, const double *Fpad, doubl
 /* sweep of one direction: fills flux[dir] (F and dF; stage 2 needs only dF) */
 int gks_launch_sweep_unfused(const GksGrid &g, const GksPhys &ph, int dir, const double *W, double *tmpN,
                              double *tmpT, double *flux, bool need_F, cudaStream_t s);
+
+/* fused sweep (gks_sweep_fused.cu); which = 0 reads Wn, 1 reads Ws */
+bool gks_fused_init(gks_ctx *ctx);
+int gks_launch_sweep_fused(gks_ctx *ctx, int dir, int which, double *flux, bool need_F);
 
 int gks_launch_stage1(const GksGrid &g, const double *Wn, double *const flux[3], double dt, double *Ws,
                       double *Pbuf, cudaStream_t s);
