@@ -259,6 +259,8 @@ gks_status gks_create(const gks_config *cfg, void *workspace, size_t workspace_b
   ph.RT = cfg->RT;
   ph.lambda = 1.0 / (2.0 * cfg->RT);
   ph.mu = cfg->rho_ref * cfg->nu;
+  ph.theta = sqrt(ph.lambda);
+  ph.cx = 0.5 / sqrt(3.14159265358979323846 * ph.lambda);
   ph.weno_eps = cfg->weno_eps > 0 ? cfg->weno_eps : 1e-6;
   for (int i = 0; i < 4; ++i) ph.inflow[i] = cfg->inflow[i];
   for (int i = 0; i < 6; ++i) ph.bc[i] = cfg->bc[i];

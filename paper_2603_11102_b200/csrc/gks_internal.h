@@ -39,6 +39,7 @@ struct GksGrid {
 
 struct GksPhys {
   double RT, lambda, mu, weno_eps; /* mu = rho_ref*nu */
+  double theta, cx;                /* sqrt(lambda), 1/(2 sqrt(pi lambda)): collision constants */
   double inflow[4];
   int bc[6];
 };

@@ -22,79 +22,116 @@ namespace gksd {
 
 #define GKS_SQRT3 1.7320508075688772935
 
-/* common-denominator Jiang-Shu factors t_k from the 5 averages */
-__device__ __forceinline__ void js_t(double q0, double q1, double q2, double q3, double q4, double eps,
-                                     double &t0, double &t1, double &t2) {
-  const double a0 = q0 - 2.0 * q1 + q2, b0 = q0 - 4.0 * q1 + 3.0 * q2;
-  const double a1 = q1 - 2.0 * q2 + q3, b1 = q1 - q3;
-  const double a2 = q2 - 2.0 * q3 + q4, b2 = 3.0 * q2 - 4.0 * q3 + q4;
-  const double k13 = 13.0 / 12.0;
-  double s0 = eps + (k13 * a0 * a0 + 0.25 * b0 * b0);
-  double s1 = eps + (k13 * a1 * a1 + 0.25 * b1 * b1);
-  double s2 = eps + (k13 * a2 * a2 + 0.25 * b2 * b2);
+/* Full-width fp64 constants live in constant memory so that DFMA/DMUL take them as c[bank][offset]
+ * operands (no per-use UMOV pairs).  Values with an all-zero low word (0.25, 0.5, 3.0, ...) are
+ * written as literals: they encode as instruction immediates. */
+static __constant__ double GKC[16] = {
+    13.0 / 12.0,                                        /* 0  smoothness: (13/12) a^2 */
+    ((210.0 - GKS_SQRT3) / 1080.0) / (11.0 / 18.0),     /* 1  Gauss-point linear weight dA / dB */
+    ((210.0 + GKS_SQRT3) / 1080.0) / (11.0 / 18.0),     /* 2  Gauss-point linear weight dC / dB */
+    GKS_SQRT3 / 12.0,                                   /* 3  h = x_G / 2, x_G = sqrt(3)/6 */
+    1.0 / 6.0,                                          /* 4  edge linear weight .1/.6 */
+    1.0 / 12.0,                                         /* 5 */
+    -(1.0 / 12.0 - GKS_SQRT3 / 54.0),                                     /* 6  e1 = -k0 */
+    -((1.0 / 12.0 - GKS_SQRT3 / 54.0) + (-2.0 / 3.0 + 13.0 * GKS_SQRT3 / 54.0)), /* 7  e2 = -(k0+k1) */
+    (2.0 / 3.0 + 13.0 * GKS_SQRT3 / 54.0) + (-1.0 / 12.0 - GKS_SQRT3 / 54.0),    /* 8  e3 = k3+k4 */
+    -1.0 / 12.0 - GKS_SQRT3 / 54.0,                                       /* 9  e4 = k4 */
+    0, 0, 0, 0, 0, 0};
+
+/* reciprocal to fp64 round-off: hardware seed (2^-23) + two Newton steps, no slow path */
+__device__ __forceinline__ double fast_rcp(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  double e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-x, r, 1.0);
+  return fma(r, e, r);
+}
+
+/* Shared front end of every WENO5-JS evaluation, in difference form.  With D_m = q_m - q_{m-1}:
+ *   second differences a_k (sub-stencil curvature), centred slopes g_k (twice the slope of sub-stencil k's
+ *   quadratic at the centre of the middle cell; g0 = q0-4q1+3q2, g1 = q3-q1, g2 = -(3q2-4q3+q4)),
+ *   Jiang-Shu beta_k = 13/12 a_k^2 + 1/4 g_k^2, and the common-denominator factors
+ *   t0 = s1 s2, t1 = s0 s2, t2 = s0 s1 with s_k = (eps + beta_k)^2. */
+struct JsFront {
+  double a0, a1, a2, g0, g1, g2, t0, t1, t2;
+};
+__device__ __forceinline__ void js_front(double D1, double D2, double D3, double D4, double eps, JsFront &f) {
+  f.a0 = D2 - D1;
+  f.a1 = D3 - D2;
+  f.a2 = D4 - D3;
+  f.g0 = fma(3.0, D2, -D1);
+  f.g1 = D2 + D3;
+  f.g2 = fma(3.0, D3, -D4);
+  const double k13 = GKC[0];
+  double s0 = fma(0.25 * f.g0, f.g0, fma(k13 * f.a0, f.a0, eps));
+  double s1 = fma(0.25 * f.g1, f.g1, fma(k13 * f.a1, f.a1, eps));
+  double s2 = fma(0.25 * f.g2, f.g2, fma(k13 * f.a2, f.a2, eps));
   s0 *= s0;
   s1 *= s1;
   s2 *= s2;
-  t0 = s1 * s2;
-  t1 = s0 * s2;
-  t2 = s0 * s1;
+  f.t0 = s1 * s2;
+  f.t1 = s0 * s2;
+  f.t2 = s0 * s1;
 }
 
-/* WENO5-JS values at BOTH edges of the middle cell: vl at x = -1/2, vr at x = +1/2 */
+/* WENO5-JS values at BOTH edges of the middle cell: vl at x = -1/2, vr at x = +1/2.
+ * Candidate k at x = +-1/2 is q2 +- g_k/4 + a_k/12; linear weights (.1,.6,.3) right, mirrored left;
+ * nonlinear weights over the common denominator (one reciprocal for both edges). */
 __device__ __forceinline__ void weno5_edges(double q0, double q1, double q2, double q3, double q4,
                                             double eps, double &vl, double &vr) {
-  double t0, t1, t2;
-  js_t(q0, q1, q2, q3, q4, eps, t0, t1, t2);
-  /* right edge: candidates (2,-7,11)/6, (-1,5,2)/6, (2,5,-1)/6 with linear weights .1,.6,.3 */
-  const double r0 = 2.0 * q0 - 7.0 * q1 + 11.0 * q2;
-  const double r1 = -q1 + 5.0 * q2 + 2.0 * q3;
-  const double r2 = 2.0 * q2 + 5.0 * q3 - q4;
-  /* left edge (mirror): candidates (-1,5,2)/6 on (q0,q1,q2), (2,5,-1)/6 on (q1,q2,q3), (11,-7,2)/6 on (q2,q3,q4);
-     linear weights .3,.6,.1 */
-  const double l0 = -q0 + 5.0 * q1 + 2.0 * q2;
-  const double l1 = 2.0 * q1 + 5.0 * q2 - q3;
-  const double l2 = 11.0 * q2 - 7.0 * q3 + 2.0 * q4;
-  const double ar0 = 0.1 * t0, ar1 = 0.6 * t1, ar2 = 0.3 * t2;
-  const double al0 = 0.3 * t0, al1 = 0.6 * t1, al2 = 0.1 * t2;
-  const double numr = ar0 * r0 + ar1 * r1 + ar2 * r2, denr = ar0 + ar1 + ar2;
-  const double numl = al0 * l0 + al1 * l1 + al2 * l2, denl = al0 + al1 + al2;
-  const double inv = 1.0 / (6.0 * denr * denl);
-  vr = numr * denl * inv;
-  vl = numl * denr * inv;
+  JsFront f;
+  js_front(q1 - q0, q2 - q1, q3 - q2, q4 - q3, eps, f);
+  const double w6 = GKC[4];
+  const double ar0 = w6 * f.t0, ar2 = 0.5 * f.t2; /* (.1,.6,.3)/.6 */
+  const double al0 = 0.5 * f.t0, al2 = w6 * f.t2; /* (.3,.6,.1)/.6 */
+  const double P0 = fma(3.0, f.g0, f.a0), P1 = fma(3.0, f.g1, f.a1), P2 = fma(3.0, f.g2, f.a2);
+  const double M0 = fma(-3.0, f.g0, f.a0), M1 = fma(-3.0, f.g1, f.a1), M2 = fma(-3.0, f.g2, f.a2);
+  const double numr = fma(ar2, P2, fma(f.t1, P1, ar0 * P0)), denr = ar0 + f.t1 + ar2;
+  const double numl = fma(al2, M2, fma(f.t1, M1, al0 * M0)), denl = al0 + f.t1 + al2;
+  const double inv = fast_rcp(denr * denl) * GKC[5];
+  vr = fma(numr * denl, inv, q2);
+  vl = fma(numl * denr, inv, q2);
 }
 
-/* WENO5-JS values at the Gauss points: vm at x = -sqrt(3)/6, vp at x = +sqrt(3)/6 (S7) */
+/* WENO5-JS values at the Gauss points (vm at -sqrt(3)/6, vp at +sqrt(3)/6; S7) and, if SLOPE,
+ * the derivative of the quartic through the 5 averages there (S8; per unit cell width).
+ * At x^2 = 1/12 the quadratic term of every candidate vanishes: candidate k is q2 +- (x_G/2) g_k. */
+template <bool SLOPE>
+__device__ __forceinline__ void weno5_gauss_slope(double q0, double q1, double q2, double q3, double q4, double eps,
+                                                  double &vm, double &vp, double &sm, double &sp) {
+  const double D1 = q1 - q0, D2 = q2 - q1, D3 = q3 - q2, D4 = q4 - q3;
+  JsFront f;
+  js_front(D1, D2, D3, D4, eps, f);
+  const double dA = GKC[1], dC = GKC[2], h = GKC[3];
+  const double ap0 = dA * f.t0, ap2 = dC * f.t2;
+  const double am0 = dC * f.t0, am2 = dA * f.t2;
+  const double c1 = f.t1 * f.g1;
+  const double nump = fma(ap2, f.g2, fma(ap0, f.g0, c1)), denp = ap0 + f.t1 + ap2;
+  const double numm = fma(am2, f.g2, fma(am0, f.g0, c1)), denm = am0 + f.t1 + am2;
+  const double inv = fast_rcp(denp * denm) * h;
+  vp = fma(nump * denm, inv, q2);
+  vm = fma(-(numm * denp), inv, q2);
+  if (SLOPE) {
+    const double e1 = GKC[6], e2 = GKC[7], e3 = GKC[8], e4 = GKC[9];
+    sp = fma(e4, D4, fma(e3, D3, fma(e2, D2, e1 * D1)));
+    sm = fma(e1, D4, fma(e2, D3, fma(e3, D2, e4 * D1)));
+  }
+}
+
 __device__ __forceinline__ void weno5_gauss(double q0, double q1, double q2, double q3, double q4,
                                             double eps, double &vm, double &vp) {
-  double t0, t1, t2;
-  js_t(q0, q1, q2, q3, q4, eps, t0, t1, t2);
-  const double c12 = GKS_SQRT3 / 12.0, c3 = GKS_SQRT3 / 3.0, c4 = GKS_SQRT3 / 4.0;
-  const double dA = (210.0 - GKS_SQRT3) / 1080.0, dB = 11.0 / 18.0, dC = (210.0 + GKS_SQRT3) / 1080.0;
-  const double e01 = c12 * (q3 - q1); /* shared by the two middle candidates */
-  const double pp0 = c12 * q0 - c3 * q1 + (1.0 + c4) * q2;
-  const double pp1 = q2 + e01;
-  const double pp2 = (1.0 - c4) * q2 + c3 * q3 - c12 * q4;
-  const double pm0 = -c12 * q0 + c3 * q1 + (1.0 - c4) * q2;
-  const double pm1 = q2 - e01;
-  const double pm2 = (1.0 + c4) * q2 - c3 * q3 + c12 * q4;
-  const double bt1 = dB * t1;
-  const double ap0 = dA * t0, ap2 = dC * t2;
-  const double am0 = dC * t0, am2 = dA * t2;
-  const double nump = ap0 * pp0 + bt1 * pp1 + ap2 * pp2, denp = ap0 + bt1 + ap2;
-  const double numm = am0 * pm0 + bt1 * pm1 + am2 * pm2, denm = am0 + bt1 + am2;
-  const double inv = 1.0 / (denp * denm);
-  vp = nump * denm * inv;
-  vm = numm * denp * inv;
+  double d0, d1;
+  weno5_gauss_slope<false>(q0, q1, q2, q3, q4, eps, vm, vp, d0, d1);
 }
 
 /* derivative of the quartic through the 5 averages at the Gauss points, per unit cell width (S8) */
 __device__ __forceinline__ void quartic_slope_gauss(double q0, double q1, double q2, double q3, double q4,
                                                     double &sm, double &sp) {
-  const double k0 = 1.0 / 12.0 - GKS_SQRT3 / 54.0, k1 = -2.0 / 3.0 + 13.0 * GKS_SQRT3 / 54.0;
-  const double k2 = -4.0 * GKS_SQRT3 / 9.0, k3 = 2.0 / 3.0 + 13.0 * GKS_SQRT3 / 54.0;
-  const double k4 = -1.0 / 12.0 - GKS_SQRT3 / 54.0;
-  sp = k0 * q0 + k1 * q1 + k2 * q2 + k3 * q3 + k4 * q4;
-  sm = -(k0 * q4 + k1 * q3 + k2 * q2 + k3 * q1 + k4 * q0);
+  const double D1 = q1 - q0, D2 = q2 - q1, D3 = q3 - q2, D4 = q4 - q3;
+  const double e1 = GKC[6], e2 = GKC[7], e3 = GKC[8], e4 = GKC[9];
+  sp = fma(e4, D4, fma(e3, D3, fma(e2, D2, e1 * D1)));
+  sm = fma(e1, D4, fma(e2, D3, fma(e3, D2, e4 * D1)));
 }
 
 /* index-space slope at the face between qb and qc from 4 averages qa,qb,qc,qd (S5) */
@@ -117,7 +154,7 @@ __device__ __forceinline__ void collision_factors(double Ul, double Ur, double l
 /* Q0 from Ql, Qr; NRM = 1 + dir is the index of the normal momentum */
 template <int DIR>
 __device__ __forceinline__ void collision(const double Ql[4], const double Qr[4], double lambda, double Q0[4]) {
-  const double Ul = Ql[1 + DIR] / Ql[0], Ur = Qr[1 + DIR] / Qr[0];
+  const double Ul = Ql[1 + DIR] * fast_rcp(Ql[0]), Ur = Qr[1 + DIR] * fast_rcp(Qr[0]);
   double el, xl, er, xr;
   collision_factors(Ul, Ur, lambda, el, xl, er, xr);
 #pragma unroll
@@ -130,7 +167,7 @@ template <int DIR, bool NEED_F>
 __device__ __forceinline__ void gauss_point_flux(const double Q0[4], const double dQ[3][4], double RT,
                                                  double mu, double F[4], double dF[4]) {
   const double rho = Q0[0];
-  const double ir = 1.0 / rho;
+  const double ir = fast_rcp(rho);
   const double u[3] = {Q0[1] * ir, Q0[2] * ir, Q0[3] * ir};
   /* Q_t = -sum_s d_s F_Euler^s:  rho_t = -sum_s d_s m_s ;
      m_i,t = -sum_s (U_s d_s m_i + m_i d_s U_s) - RT d_i rho,  d_s U_s = (d_s m_s - U_s d_s rho)/rho */

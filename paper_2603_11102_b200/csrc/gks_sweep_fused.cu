@@ -194,10 +194,9 @@ __global__ void __launch_bounds__(TA *TB * 4, 2)
     for (int item = tid; item < FH * 2; item += NT) {
       const int side = item & 1, fh = item >> 1;
       const double *q = (side ? QR : QL) + fh * 4;
-      const double rho = q[0], U = q[1 + DIR] / rho;
-      const double theta = sqrt(ph.lambda);
-      const double e = 0.5 * erfc(side ? theta * U : -theta * U);
-      const double x = (0.5 / sqrt(3.14159265358979323846 * ph.lambda)) * exp(-ph.lambda * U * U);
+      const double rho = q[0], U = q[1 + DIR] * gksd::fast_rcp(rho);
+      const double e = 0.5 * erfc(side ? ph.theta * U : -ph.theta * U);
+      const double x = ph.cx * exp(-ph.lambda * U * U);
       CF[fh * 4 + 2 * side] = e;
       CF[fh * 4 + 2 * side + 1] = rho * x;
     }
@@ -233,8 +232,7 @@ __global__ void __launch_bounds__(TA *TB * 4, 2)
       const double *q = QL + fh * 4 + c;
       double vm, vp, sm_, sp_;
       const double q0 = q[-2 * s1 * 4], q1 = q[-s1 * 4], q2 = q[0], q3 = q[s1 * 4], q4 = q[2 * s1 * 4];
-      gksd::weno5_gauss(q0, q1, q2, q3, q4, eps, vm, vp);
-      gksd::quartic_slope_gauss(q0, q1, q2, q3, q4, sm_, sp_);
+      gksd::weno5_gauss_slope<true>(q0, q1, q2, q3, q4, eps, vm, vp, sm_, sp_);
       r[0 * NF * 4] = vm;
       r[1 * NF * 4] = vp;
       r[4 * NF * 4] = sm_ * iw1;
@@ -261,8 +259,7 @@ __global__ void __launch_bounds__(TA *TB * 4, 2)
         {
           const int o = g1 * NF * 4;
           const double q0 = rs[0][o], q1 = rs[1][o], q2 = rs[2][o], q3 = rs[3][o], q4 = rs[4][o];
-          gksd::weno5_gauss(q0, q1, q2, q3, q4, eps, vm, vp);
-          gksd::quartic_slope_gauss(q0, q1, q2, q3, q4, sm_, sp_);
+          gksd::weno5_gauss_slope<true>(q0, q1, q2, q3, q4, eps, vm, vp, sm_, sp_);
           xb[0 * 16 + 2 * g1] = vm;
           xb[0 * 16 + 2 * g1 + 1] = vp;
           xb[3 * 16 + 2 * g1] = sm_ * iw2;
