@@ -53,79 +53,166 @@ __device__ __forceinline__ double fast_rcp(double x) {
  *   quadratic at the centre of the middle cell; g0 = q0-4q1+3q2, g1 = q3-q1, g2 = -(3q2-4q3+q4)),
  *   Jiang-Shu beta_k = 13/12 a_k^2 + 1/4 g_k^2, and the common-denominator factors
  *   t0 = s1 s2, t1 = s0 s2, t2 = s0 s1 with s_k = (eps + beta_k)^2. */
-struct JsFront {
-  double a0, a1, a2, g0, g1, g2, t0, t1, t2;
+/* N independent stencils at once: every statement is replicated N times back to back so that the
+ * instruction stream interleaves N dependency chains (the fp64 pipe needs the ILP at 16 warps/SM). */
+template <int N>
+struct JsFrontV {
+  double a0[N], a1[N], a2[N], g0[N], g1[N], g2[N], t0[N], t1[N], t2[N];
 };
-__device__ __forceinline__ void js_front(double D1, double D2, double D3, double D4, double eps, JsFront &f) {
-  f.a0 = D2 - D1;
-  f.a1 = D3 - D2;
-  f.a2 = D4 - D3;
-  f.g0 = fma(3.0, D2, -D1);
-  f.g1 = D2 + D3;
-  f.g2 = fma(3.0, D3, -D4);
+template <int N>
+__device__ __forceinline__ void js_front_v(const double (&D1)[N], const double (&D2)[N], const double (&D3)[N],
+                                           const double (&D4)[N], double eps, JsFrontV<N> &f) {
   const double k13 = GKC[0];
-  double s0 = fma(0.25 * f.g0, f.g0, fma(k13 * f.a0, f.a0, eps));
-  double s1 = fma(0.25 * f.g1, f.g1, fma(k13 * f.a1, f.a1, eps));
-  double s2 = fma(0.25 * f.g2, f.g2, fma(k13 * f.a2, f.a2, eps));
-  s0 *= s0;
-  s1 *= s1;
-  s2 *= s2;
-  f.t0 = s1 * s2;
-  f.t1 = s0 * s2;
-  f.t2 = s0 * s1;
-}
-
-/* WENO5-JS values at BOTH edges of the middle cell: vl at x = -1/2, vr at x = +1/2.
- * Candidate k at x = +-1/2 is q2 +- g_k/4 + a_k/12; linear weights (.1,.6,.3) right, mirrored left;
- * nonlinear weights over the common denominator (one reciprocal for both edges). */
-__device__ __forceinline__ void weno5_edges(double q0, double q1, double q2, double q3, double q4,
-                                            double eps, double &vl, double &vr) {
-  JsFront f;
-  js_front(q1 - q0, q2 - q1, q3 - q2, q4 - q3, eps, f);
-  const double w6 = GKC[4];
-  const double ar0 = w6 * f.t0, ar2 = 0.5 * f.t2; /* (.1,.6,.3)/.6 */
-  const double al0 = 0.5 * f.t0, al2 = w6 * f.t2; /* (.3,.6,.1)/.6 */
-  const double P0 = fma(3.0, f.g0, f.a0), P1 = fma(3.0, f.g1, f.a1), P2 = fma(3.0, f.g2, f.a2);
-  const double M0 = fma(-3.0, f.g0, f.a0), M1 = fma(-3.0, f.g1, f.a1), M2 = fma(-3.0, f.g2, f.a2);
-  const double numr = fma(ar2, P2, fma(f.t1, P1, ar0 * P0)), denr = ar0 + f.t1 + ar2;
-  const double numl = fma(al2, M2, fma(f.t1, M1, al0 * M0)), denl = al0 + f.t1 + al2;
-  const double inv = fast_rcp(denr * denl) * GKC[5];
-  vr = fma(numr * denl, inv, q2);
-  vl = fma(numl * denr, inv, q2);
-}
-
-/* WENO5-JS values at the Gauss points (vm at -sqrt(3)/6, vp at +sqrt(3)/6; S7) and, if SLOPE,
- * the derivative of the quartic through the 5 averages there (S8; per unit cell width).
- * At x^2 = 1/12 the quadratic term of every candidate vanishes: candidate k is q2 +- (x_G/2) g_k. */
-template <bool SLOPE>
-__device__ __forceinline__ void weno5_gauss_slope(double q0, double q1, double q2, double q3, double q4, double eps,
-                                                  double &vm, double &vp, double &sm, double &sp) {
-  const double D1 = q1 - q0, D2 = q2 - q1, D3 = q3 - q2, D4 = q4 - q3;
-  JsFront f;
-  js_front(D1, D2, D3, D4, eps, f);
-  const double dA = GKC[1], dC = GKC[2], h = GKC[3];
-  const double ap0 = dA * f.t0, ap2 = dC * f.t2;
-  const double am0 = dC * f.t0, am2 = dA * f.t2;
-  const double c1 = f.t1 * f.g1;
-  const double nump = fma(ap2, f.g2, fma(ap0, f.g0, c1)), denp = ap0 + f.t1 + ap2;
-  const double numm = fma(am2, f.g2, fma(am0, f.g0, c1)), denm = am0 + f.t1 + am2;
-  const double inv = fast_rcp(denp * denm) * h;
-  vp = fma(nump * denm, inv, q2);
-  vm = fma(-(numm * denp), inv, q2);
-  if (SLOPE) {
-    const double e1 = GKC[6], e2 = GKC[7], e3 = GKC[8], e4 = GKC[9];
-    sp = fma(e4, D4, fma(e3, D3, fma(e2, D2, e1 * D1)));
-    sm = fma(e1, D4, fma(e2, D3, fma(e3, D2, e4 * D1)));
+  double s0[N], s1[N], s2[N];
+#pragma unroll
+  for (int n = 0; n < N; ++n) {
+    f.a0[n] = D2[n] - D1[n];
+    f.a1[n] = D3[n] - D2[n];
+    f.a2[n] = D4[n] - D3[n];
+  }
+#pragma unroll
+  for (int n = 0; n < N; ++n) {
+    f.g0[n] = fma(3.0, D2[n], -D1[n]);
+    f.g1[n] = D2[n] + D3[n];
+    f.g2[n] = fma(3.0, D3[n], -D4[n]);
+  }
+#pragma unroll
+  for (int n = 0; n < N; ++n) {
+    s0[n] = fma(k13 * f.a0[n], f.a0[n], eps);
+    s1[n] = fma(k13 * f.a1[n], f.a1[n], eps);
+    s2[n] = fma(k13 * f.a2[n], f.a2[n], eps);
+  }
+#pragma unroll
+  for (int n = 0; n < N; ++n) {
+    s0[n] = fma(0.25 * f.g0[n], f.g0[n], s0[n]);
+    s1[n] = fma(0.25 * f.g1[n], f.g1[n], s1[n]);
+    s2[n] = fma(0.25 * f.g2[n], f.g2[n], s2[n]);
+  }
+#pragma unroll
+  for (int n = 0; n < N; ++n) {
+    s0[n] *= s0[n];
+    s1[n] *= s1[n];
+    s2[n] *= s2[n];
+  }
+#pragma unroll
+  for (int n = 0; n < N; ++n) {
+    f.t0[n] = s1[n] * s2[n];
+    f.t1[n] = s0[n] * s2[n];
+    f.t2[n] = s0[n] * s1[n];
   }
 }
 
-__device__ __forceinline__ void weno5_gauss(double q0, double q1, double q2, double q3, double q4,
-                                            double eps, double &vm, double &vp) {
-  double d0, d1;
-  weno5_gauss_slope<false>(q0, q1, q2, q3, q4, eps, vm, vp, d0, d1);
+template <int N>
+__device__ __forceinline__ void fast_rcp_v(const double (&x)[N], double (&r)[N]) {
+  double e[N];
+#pragma unroll
+  for (int n = 0; n < N; ++n) asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r[n]) : "d"(x[n]));
+#pragma unroll
+  for (int n = 0; n < N; ++n) e[n] = fma(-x[n], r[n], 1.0);
+#pragma unroll
+  for (int n = 0; n < N; ++n) r[n] = fma(r[n], e[n], r[n]);
+#pragma unroll
+  for (int n = 0; n < N; ++n) e[n] = fma(-x[n], r[n], 1.0);
+#pragma unroll
+  for (int n = 0; n < N; ++n) r[n] = fma(r[n], e[n], r[n]);
 }
 
-/* derivative of the quartic through the 5 averages at the Gauss points, per unit cell width (S8) */
+/* WENO5-JS values at BOTH edges of the middle cell for N stencils: vl at x = -1/2, vr at x = +1/2.
+ * Candidate k at x = +-1/2 is q2 +- g_k/4 + a_k/12; linear weights (.1,.6,.3) right, mirrored left;
+ * nonlinear weights over the common denominator (one reciprocal for both edges). */
+template <int N>
+__device__ __forceinline__ void weno5_edges_v(const double (&q)[5][N], double eps, double (&vl)[N], double (&vr)[N]) {
+  double D1[N], D2[N], D3[N], D4[N];
+#pragma unroll
+  for (int n = 0; n < N; ++n) {
+    D1[n] = q[1][n] - q[0][n];
+    D2[n] = q[2][n] - q[1][n];
+    D3[n] = q[3][n] - q[2][n];
+    D4[n] = q[4][n] - q[3][n];
+  }
+  JsFrontV<N> f;
+  js_front_v<N>(D1, D2, D3, D4, eps, f);
+  const double w6 = GKC[4], w12 = GKC[5];
+  double numr[N], numl[N], denr[N], denl[N], prod[N], inv[N];
+#pragma unroll
+  for (int n = 0; n < N; ++n) {
+    const double ar0 = w6 * f.t0[n], ar2 = 0.5 * f.t2[n]; /* (.1,.6,.3)/.6 */
+    const double al0 = 0.5 * f.t0[n], al2 = w6 * f.t2[n]; /* (.3,.6,.1)/.6 */
+    const double P0 = fma(3.0, f.g0[n], f.a0[n]), P1 = fma(3.0, f.g1[n], f.a1[n]), P2 = fma(3.0, f.g2[n], f.a2[n]);
+    const double M0 = fma(-3.0, f.g0[n], f.a0[n]), M1 = fma(-3.0, f.g1[n], f.a1[n]), M2 = fma(-3.0, f.g2[n], f.a2[n]);
+    numr[n] = fma(ar2, P2, fma(f.t1[n], P1, ar0 * P0));
+    denr[n] = ar0 + f.t1[n] + ar2;
+    numl[n] = fma(al2, M2, fma(f.t1[n], M1, al0 * M0));
+    denl[n] = al0 + f.t1[n] + al2;
+    prod[n] = denr[n] * denl[n];
+  }
+  fast_rcp_v<N>(prod, inv);
+#pragma unroll
+  for (int n = 0; n < N; ++n) {
+    const double iv = inv[n] * w12;
+    vr[n] = fma(numr[n] * denl[n], iv, q[2][n]);
+    vl[n] = fma(numl[n] * denr[n], iv, q[2][n]);
+  }
+}
+
+/* WENO5-JS values at the Gauss points (vm at -sqrt(3)/6, vp at +sqrt(3)/6; S7) and the derivative of
+ * the quartic through the 5 averages there (S8; per unit cell width; dead code when unused), N stencils.
+ * At x^2 = 1/12 the quadratic term of every candidate vanishes: candidate k is q2 +- (x_G/2) g_k. */
+template <int N>
+__device__ __forceinline__ void weno5_gauss_v(const double (&q)[5][N], double eps, double (&vm)[N], double (&vp)[N],
+                                              double (&sm)[N], double (&sp)[N]) {
+  double D1[N], D2[N], D3[N], D4[N];
+#pragma unroll
+  for (int n = 0; n < N; ++n) {
+    D1[n] = q[1][n] - q[0][n];
+    D2[n] = q[2][n] - q[1][n];
+    D3[n] = q[3][n] - q[2][n];
+    D4[n] = q[4][n] - q[3][n];
+  }
+  JsFrontV<N> f;
+  js_front_v<N>(D1, D2, D3, D4, eps, f);
+  const double dA = GKC[1], dC = GKC[2], h = GKC[3];
+  double nump[N], numm[N], denp[N], denm[N], prod[N], inv[N];
+#pragma unroll
+  for (int n = 0; n < N; ++n) {
+    const double ap0 = dA * f.t0[n], ap2 = dC * f.t2[n];
+    const double am0 = dC * f.t0[n], am2 = dA * f.t2[n];
+    const double c1 = f.t1[n] * f.g1[n];
+    nump[n] = fma(ap2, f.g2[n], fma(ap0, f.g0[n], c1));
+    denp[n] = ap0 + f.t1[n] + ap2;
+    numm[n] = fma(am2, f.g2[n], fma(am0, f.g0[n], c1));
+    denm[n] = am0 + f.t1[n] + am2;
+    prod[n] = denp[n] * denm[n];
+  }
+  fast_rcp_v<N>(prod, inv);
+  const double e1 = GKC[6], e2 = GKC[7], e3 = GKC[8], e4 = GKC[9];
+#pragma unroll
+  for (int n = 0; n < N; ++n) {
+    const double iv = inv[n] * h;
+    vp[n] = fma(nump[n] * denm[n], iv, q[2][n]);
+    vm[n] = fma(-(numm[n] * denp[n]), iv, q[2][n]);
+    sp[n] = fma(e4, D4[n], fma(e3, D3[n], fma(e2, D2[n], e1 * D1[n])));
+    sm[n] = fma(e1, D4[n], fma(e2, D3[n], fma(e3, D2[n], e4 * D1[n])));
+  }
+}
+
+/* scalar wrappers (unfused cross-check kernels) */
+__device__ __forceinline__ void weno5_edges(double q0, double q1, double q2, double q3, double q4,
+                                            double eps, double &vl, double &vr) {
+  const double q[5][1] = {{q0}, {q1}, {q2}, {q3}, {q4}};
+  double l[1], r[1];
+  weno5_edges_v<1>(q, eps, l, r);
+  vl = l[0];
+  vr = r[0];
+}
+__device__ __forceinline__ void weno5_gauss(double q0, double q1, double q2, double q3, double q4,
+                                            double eps, double &vm, double &vp) {
+  const double q[5][1] = {{q0}, {q1}, {q2}, {q3}, {q4}};
+  double m[1], p[1], a[1], b[1];
+  weno5_gauss_v<1>(q, eps, m, p, a, b);
+  vm = m[0];
+  vp = p[0];
+}
 __device__ __forceinline__ void quartic_slope_gauss(double q0, double q1, double q2, double q3, double q4,
                                                     double &sm, double &sp) {
   const double D1 = q1 - q0, D2 = q2 - q1, D3 = q3 - q2, D4 = q4 - q3;
@@ -139,16 +226,53 @@ __device__ __forceinline__ double normal_slope(double qa, double qb, double qc, 
   return (15.0 * (qc - qb) - (qd - qa)) * (1.0 / 12.0);
 }
 
+/* Half-range Maxwellian moments (S4) need erf(z) and exp(-z^2), z = sqrt(lambda) U_n.  For |z| <= 1/2
+ * (normal Mach number below 0.7: every cell of a weakly compressible flow) both come from their
+ * Maclaurin series in z^2 (terms fall like 0.25^n/n!; 12 and 14 terms reach 1e-17), about 26 DFMA with
+ * constant-bank coefficients; otherwise the CUDA math library is used. */
+#define GKS_2ISPI 1.1283791670955125739 /* 2/sqrt(pi) */
+static __constant__ double GK_ERF[12] = {
+    GKS_2ISPI / 1.0,          -GKS_2ISPI / 3.0,           GKS_2ISPI / (2.0 * 5.0),       -GKS_2ISPI / (6.0 * 7.0),
+    GKS_2ISPI / (24.0 * 9.0), -GKS_2ISPI / (120.0 * 11.0), GKS_2ISPI / (720.0 * 13.0),   -GKS_2ISPI / (5040.0 * 15.0),
+    GKS_2ISPI / (40320.0 * 17.0), -GKS_2ISPI / (362880.0 * 19.0), GKS_2ISPI / (3628800.0 * 21.0),
+    -GKS_2ISPI / (39916800.0 * 23.0)};
+static __constant__ double GK_EXP[14] = {1.0, -1.0, 1.0 / 2.0, -1.0 / 6.0, 1.0 / 24.0, -1.0 / 120.0, 1.0 / 720.0,
+                                         -1.0 / 5040.0, 1.0 / 40320.0, -1.0 / 362880.0, 1.0 / 3628800.0,
+                                         -1.0 / 39916800.0, 1.0 / 479001600.0, -1.0 / 6227020800.0};
+
+/* erf(z) and exp(-z^2) */
+__device__ __forceinline__ void erf_expm2(double z, double &erfz, double &ex) {
+  const double w = z * z;
+  if (w <= 0.25) {
+    double pe = GK_ERF[11], px = GK_EXP[13];
+    px = fma(px, w, GK_EXP[12]);
+#pragma unroll
+    for (int n = 10; n >= 0; --n) {
+      pe = fma(pe, w, GK_ERF[n]);
+      px = fma(px, w, GK_EXP[n + 1]);
+    }
+    px = fma(px, w, GK_EXP[0]);
+    erfz = pe * z;
+    ex = px;
+  } else {
+    erfz = erf(z);
+    ex = exp(-w);
+  }
+}
+
 /* collision factors from the normal velocities of the left / right states (S4):
  * el = <u^0>_{>0}(Ul), xl = exp(-lam Ul^2)/(2 sqrt(pi lam)); er = <u^0>_{<0}(Ur), xr likewise (positive) */
 __device__ __forceinline__ void collision_factors(double Ul, double Ur, double lambda, double &el,
                                                   double &xl, double &er, double &xr) {
   const double theta = sqrt(lambda);
   const double c = 0.5 / sqrt(3.14159265358979323846 * lambda);
-  el = 0.5 * erfc(-theta * Ul);
-  er = 0.5 * erfc(theta * Ur);
-  xl = c * exp(-lambda * Ul * Ul);
-  xr = c * exp(-lambda * Ur * Ur);
+  double fl, fr, gl, gr;
+  erf_expm2(theta * Ul, fl, gl);
+  erf_expm2(theta * Ur, fr, gr);
+  el = 0.5 + 0.5 * fl; /* erfc(-z)/2 */
+  er = 0.5 - 0.5 * fr; /* erfc(+z)/2 */
+  xl = c * gl;
+  xr = c * gr;
 }
 
 /* Q0 from Ql, Qr; NRM = 1 + dir is the index of the normal momentum */

@@ -166,25 +166,43 @@ __global__ void __launch_bounds__(TA *TB * 4, 2)
     mbar_wait(&bar[it & 1], (it >> 1) & 1);
     if (dbg == 3) { __syncthreads(); if (tid == 0 && it + 2 < np) issue(it + 2); continue; }
 
-    /* ---- A: both edge values of each cell, per component ---- */
-    for (int item = tid; item < T::NCA * T::NCB * 4; item += NT) {
-      const int cc = item & 3, cell = item >> 2;
-      const int xa = cell % T::NCA, xb = cell / T::NCA;
-      /* slab coordinates of the cell and stride along the normal */
-      const int sa = T::NA ? xa + 2 : xa + 1, sb = T::NA ? xb : xb + 2;
-      const double *w = W + (cc * EB + sb) * EA + sa;
+    /* ---- A: both edge values of each cell, per component; two cells per thread at a time ---- */
+    {
+      constexpr int NITEM = T::NCA * T::NCB * 4;
       constexpr int sn = T::NA ? 1 : EA;
-      double vl, vr;
-      gksd::weno5_edges(w[-2 * sn], w[-sn], w[0], w[sn], w[2 * sn], eps, vl, vr);
-      const int cn = T::NA ? xa : xb;           /* cell along the normal: global f0-1+cn */
-      const int ct = T::NA ? xb : xa;           /* halo index along t1 */
-      if (cn >= 1) {                            /* left edge = face cn-1: Qr */
-        const int fh = T::NA ? ct * HA + (cn - 1) : (cn - 1) * HA + ct;
-        QR[fh * 4 + cc] = vl;
-      }
-      if (cn < TN) {                            /* right edge = face cn: Ql */
-        const int fh = T::NA ? ct * HA + cn : cn * HA + ct;
-        QL[fh * 4 + cc] = vr;
+      for (int item0 = tid; item0 < NITEM; item0 += 2 * NT) {
+        double q[5][2], vl[2], vr[2];
+        int cnv[2], ctv[2], ccv[2];
+        bool ok[2];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+          const int item = item0 + u * NT;
+          ok[u] = item < NITEM;
+          const int it2 = ok[u] ? item : item0;
+          const int cc = it2 & 3, cell = it2 >> 2;
+          const int xa = cell % T::NCA, xb = cell / T::NCA;
+          const int sa = T::NA ? xa + 2 : xa + 1, sb = T::NA ? xb : xb + 2;
+          const double *w = W + (cc * EB + sb) * EA + sa;
+#pragma unroll
+          for (int k = 0; k < 5; ++k) q[k][u] = w[(k - 2) * sn];
+          cnv[u] = T::NA ? xa : xb; /* cell along the normal: global f0-1+cn */
+          ctv[u] = T::NA ? xb : xa; /* halo index along t1 */
+          ccv[u] = cc;
+        }
+        gksd::weno5_edges_v<2>(q, eps, vl, vr);
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+          if (!ok[u]) continue;
+          const int cn = cnv[u], ct = ctv[u];
+          if (cn >= 1) { /* left edge = face cn-1: Qr */
+            const int fh = T::NA ? ct * HA + (cn - 1) : (cn - 1) * HA + ct;
+            QR[fh * 4 + ccv[u]] = vl[u];
+          }
+          if (cn < TN) { /* right edge = face cn: Ql */
+            const int fh = T::NA ? ct * HA + cn : cn * HA + ct;
+            QL[fh * 4 + ccv[u]] = vr[u];
+          }
+        }
       }
     }
     __syncthreads();
@@ -195,8 +213,10 @@ __global__ void __launch_bounds__(TA *TB * 4, 2)
       const int side = item & 1, fh = item >> 1;
       const double *q = (side ? QR : QL) + fh * 4;
       const double rho = q[0], U = q[1 + DIR] * gksd::fast_rcp(rho);
-      const double e = 0.5 * erfc(side ? ph.theta * U : -ph.theta * U);
-      const double x = ph.cx * exp(-ph.lambda * U * U);
+      double erfz, ex;
+      gksd::erf_expm2(ph.theta * U, erfz, ex);
+      const double e = side ? 0.5 - 0.5 * erfz : 0.5 + 0.5 * erfz; /* erfc(+z)/2 right, erfc(-z)/2 left */
+      const double x = ph.cx * ex;
       CF[fh * 4 + 2 * side] = e;
       CF[fh * 4 + 2 * side + 1] = rho * x;
     }
@@ -229,18 +249,21 @@ __global__ void __launch_bounds__(TA *TB * 4, 2)
       double *r = ring + (size_t)slot * 6 * NF * 4 + fid * 4 + c;
       constexpr int s1 = T::NA ? HA : 1;                         /* halo-face stride along t1 */
       const int fh = T::NA ? (t1_local + 2) * HA + fa : fb * HA + (t1_local + 2);
-      const double *q = QL + fh * 4 + c;
-      double vm, vp, sm_, sp_;
-      const double q0 = q[-2 * s1 * 4], q1 = q[-s1 * 4], q2 = q[0], q3 = q[s1 * 4], q4 = q[2 * s1 * 4];
-      gksd::weno5_gauss_slope<true>(q0, q1, q2, q3, q4, eps, vm, vp, sm_, sp_);
-      r[0 * NF * 4] = vm;
-      r[1 * NF * 4] = vp;
-      r[4 * NF * 4] = sm_ * iw1;
-      r[5 * NF * 4] = sp_ * iw1;
-      const double *d = QR + fh * 4 + c;
-      gksd::weno5_gauss(d[-2 * s1 * 4], d[-s1 * 4], d[0], d[s1 * 4], d[2 * s1 * 4], eps, vm, vp);
-      r[2 * NF * 4] = vm;
-      r[3 * NF * 4] = vp;
+      const double *q = QL + fh * 4 + c; /* Q0 */
+      const double *d = QR + fh * 4 + c; /* Dn */
+      double qq[5][2], vm[2], vp[2], sm_[2], sp_[2];
+#pragma unroll
+      for (int k = 0; k < 5; ++k) {
+        qq[k][0] = q[(k - 2) * s1 * 4];
+        qq[k][1] = d[(k - 2) * s1 * 4];
+      }
+      gksd::weno5_gauss_v<2>(qq, eps, vm, vp, sm_, sp_);
+      r[0 * NF * 4] = vm[0];
+      r[1 * NF * 4] = vp[0];
+      r[2 * NF * 4] = vm[1];
+      r[3 * NF * 4] = vp[1];
+      r[4 * NF * 4] = sm_[0] * iw1;
+      r[5 * NF * 4] = sp_[0] * iw1;
     }
     __syncthreads();
     if (dbg == 6) continue;
@@ -254,23 +277,22 @@ __global__ void __launch_bounds__(TA *TB * 4, 2)
       for (int k = 0; k < 5; ++k) rs[k] = ring + (size_t)((it + 1 + k) % 5) * 6 * NF * 4 + fid * 4 + c;
       double *xb = XBuf + fid * T::XBS + c * 4;     /* [fld][c][g], g = 2*g1 + g2 */
 #pragma unroll
-      for (int g1 = 0; g1 < 2; ++g1) {
-        double vm, vp, sm_, sp_;
-        {
-          const int o = g1 * NF * 4;
-          const double q0 = rs[0][o], q1 = rs[1][o], q2 = rs[2][o], q3 = rs[3][o], q4 = rs[4][o];
-          gksd::weno5_gauss_slope<true>(q0, q1, q2, q3, q4, eps, vm, vp, sm_, sp_);
-          xb[0 * 16 + 2 * g1] = vm;
-          xb[0 * 16 + 2 * g1 + 1] = vp;
-          xb[3 * 16 + 2 * g1] = sm_ * iw2;
-          xb[3 * 16 + 2 * g1 + 1] = sp_ * iw2;
-        }
+      for (int fld = 0; fld < 3; ++fld) { /* Q0, Dn, Dt1: the two g1 instances of a field go together */
+        double qq[5][2], vm[2], vp[2], sm_[2], sp_[2];
 #pragma unroll
-        for (int fld = 1; fld < 3; ++fld) {
-          const int o = (2 * fld + g1) * NF * 4;
-          gksd::weno5_gauss(rs[0][o], rs[1][o], rs[2][o], rs[3][o], rs[4][o], eps, vm, vp);
-          xb[fld * 16 + 2 * g1] = vm;
-          xb[fld * 16 + 2 * g1 + 1] = vp;
+        for (int k = 0; k < 5; ++k) {
+          qq[k][0] = rs[k][(2 * fld) * NF * 4];
+          qq[k][1] = rs[k][(2 * fld + 1) * NF * 4];
+        }
+        gksd::weno5_gauss_v<2>(qq, eps, vm, vp, sm_, sp_);
+#pragma unroll
+        for (int g1 = 0; g1 < 2; ++g1) {
+          xb[fld * 16 + 2 * g1] = vm[g1];
+          xb[fld * 16 + 2 * g1 + 1] = vp[g1];
+          if (fld == 0) {
+            xb[3 * 16 + 2 * g1] = sm_[g1] * iw2;
+            xb[3 * 16 + 2 * g1 + 1] = sp_[g1] * iw2;
+          }
         }
       }
       __syncwarp();
