@@ -11,6 +11,8 @@ Multi-GPU: the path is built for one GPU (BASELINE.json north_star: no sharding,
 --gpus N runs N independent replicas, one per rank ("replicas only", weak scaling).
 """
 import argparse
+import csv
+import glob
 import json
 import os
 import subprocess
@@ -236,10 +238,12 @@ def main():
         flops_per_launch = 0.5 * (FLOPS_PER_FACE[True] + FLOPS_PER_FACE[False]) * faces
         ach = flops_per_launch / (sweep_ms / max(sweep_n, 1) * 1e-3) / 1e12 if sweep_ms > 0 else None
         traffic = None
-        tp = os.path.join(ROOT, "profiles", "traffic.json")
-        if os.path.exists(tp) and args.workload == "M0" and args.sweep == 0:
-            with open(tp) as f:
-                traffic = json.load(f).get("sweep_dram_bytes_per_launch")
+        tps = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_traffic.csv")))
+        if tps and args.workload == "M0" and args.sweep == 0:
+            with open(tps[-1]) as f:      # latest round's ncu --set full capture (text summary, not executed)
+                for row in csv.DictReader(f):
+                    if row["kernel"] == "sweep_mean_of_6":
+                        traffic = float(row["dram_bytes_per_launch"])
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
