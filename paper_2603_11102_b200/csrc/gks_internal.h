@@ -78,6 +78,7 @@ struct gks_ctx {
 
   /* TMA tensor maps of the two state buffers (Wn, Ws) for the three sweep directions (opaque CUtensorMap) */
   alignas(64) unsigned char tmaps[2][3][128];
+  int num_sms;                 /* SMs of the device: the fused sweep launches persistent CTAs */
 
   /* per-class event timing (gks_profile.cu) */
   int prof_on, prof_n;

@@ -260,6 +260,36 @@ __device__ __forceinline__ void erf_expm2(double z, double &erfz, double &ex) {
   }
 }
 
+/* N independent arguments at once (statement-interleaved Horner chains); the library fallback for
+ * |z| > 1/2 is taken per element afterwards */
+template <int N>
+__device__ __forceinline__ void erf_expm2_v(const double (&z)[N], double (&erfz)[N], double (&ex)[N]) {
+  double w[N], pe[N], px[N];
+#pragma unroll
+  for (int n = 0; n < N; ++n) {
+    w[n] = z[n] * z[n];
+    pe[n] = GK_ERF[11];
+    px[n] = fma(GK_EXP[13], w[n], GK_EXP[12]);
+  }
+#pragma unroll
+  for (int k = 10; k >= 0; --k) {
+#pragma unroll
+    for (int n = 0; n < N; ++n) {
+      pe[n] = fma(pe[n], w[n], GK_ERF[k]);
+      px[n] = fma(px[n], w[n], GK_EXP[k + 1]);
+    }
+  }
+#pragma unroll
+  for (int n = 0; n < N; ++n) {
+    erfz[n] = pe[n] * z[n];
+    ex[n] = fma(px[n], w[n], GK_EXP[0]);
+    if (w[n] > 0.25) {
+      erfz[n] = erf(z[n]);
+      ex[n] = exp(-w[n]);
+    }
+  }
+}
+
 /* collision factors from the normal velocities of the left / right states (S4):
  * el = <u^0>_{>0}(Ul), xl = exp(-lam Ul^2)/(2 sqrt(pi lam)); er = <u^0>_{<0}(Ur), xr likewise (positive) */
 __device__ __forceinline__ void collision_factors(double Ul, double Ur, double lambda, double &el,

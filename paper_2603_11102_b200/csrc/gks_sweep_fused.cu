@@ -71,6 +71,11 @@ __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, u
       : "memory");
 }
 
+/* named barriers (bar.sync / bar.arrive with a thread count): producer <-> consumer hand-over */
+__device__ __forceinline__ void bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void bar_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+enum { BAR_PROD = 1, BAR_FULL0 = 2, BAR_EMPTY0 = 4 }; /* FULL0/FULL1 = 2,3; EMPTY0/EMPTY1 = 4,5; 0 = __syncthreads */
+
 /* ---------------- compile-time geometry of a tile ---------------- */
 template <int DIR, int TA, int TB>
 struct Tile {
@@ -78,7 +83,9 @@ struct Tile {
   static constexpr int TN = NA ? TA : TB;           /* faces along the normal */
   static constexpr int T1 = NA ? TB : TA;           /* faces along t1 */
   static constexpr int NF = TA * TB;                /* faces per CTA and plane */
-  static constexpr int NT = NF * 4;                 /* threads */
+  static constexpr int NC = NF * 4;                 /* consumer threads (4 per face) */
+  static constexpr int NP = NC / 2;                 /* producer threads */
+  static constexpr int NT = NC + NP;                /* threads per CTA */
   static constexpr int CA = NA ? TN + 5 : T1 + 5;   /* cells of the W slab along a / b; the slab always starts at
                                                        cell a0-3: TMA needs a 16-byte aligned box start (even index) */
   static constexpr int CB = NA ? T1 + 4 : TN + 5;
@@ -94,249 +101,357 @@ struct Tile {
   static constexpr int AXT1 = DIR == 0 ? 1 : 0;
   static constexpr int WSLAB = 4 * EB * EA;         /* doubles per staged slab */
   static constexpr int WSLAB_PAD = (WSLAB + 15) & ~15;
-  static constexpr int XBS = 68;                    /* padded per-face stride of the transpose buffer */
   /* shared memory carve (doubles) */
-  static constexpr int OFF_W = 0;
-  static constexpr int OFF_Q = OFF_W + 2 * WSLAB_PAD;      /* QL|QR (then Q0|Dn), [2][FH][4] */
-  static constexpr int OFF_CF = OFF_Q + 2 * FH * 4;        /* collision factors [FH][4] */
-  static constexpr int OFF_XB = OFF_Q;                     /* transpose buffer aliases Q|CF (phases E,F) */
-  static constexpr int QCF = 3 * FH * 4;
-  static constexpr int XB = NF * XBS;
-  static constexpr int OFF_RING = OFF_Q + (QCF > XB ? QCF : XB);
-  static constexpr int RING = 5 * 6 * NF * 4;
+  static constexpr int OFF_W = 0;                          /* 2 slabs (TMA destinations) */
+  static constexpr int OFF_S = OFF_W + 2 * WSLAB_PAD;      /* producer staging: QL|QR [2][FH][4] */
+  static constexpr int OFF_CF = OFF_S + 2 * FH * 4;        /* collision factors [FH][4] */
+  static constexpr int OFF_Q = OFF_CF + FH * 4;            /* 2 hand-over buffers, each Q0|Dn [2][FH][4] */
+  static constexpr int OFF_XB = OFF_Q + 2 * 2 * FH * 4;    /* transpose buffer, 64 doubles per face, XOR-swizzled */
+  static constexpr int OFF_RING = OFF_XB + NF * 64;        /* 4-plane ring of pass-1 results [4][6][NF][4] */
+  static constexpr int RING = 4 * 6 * NF * 4;
   static constexpr int OFF_BAR = OFF_RING + RING;
   static constexpr size_t SMEM_BYTES = (size_t)(OFF_BAR + 2) * 8;
+  static constexpr int CTAS_PER_SM = (2 * (SMEM_BYTES + 1024) <= 233472 && 2 * NT <= 1024) ? 2 : 1;
+  static_assert(SMEM_BYTES + 1024 <= 233472, "the CTA must fit in shared memory");
+  static_assert(NC % 32 == 0 && NP % 32 == 0, "whole warps per role");
 };
 
+/* one contiguous run of marched planes of one tile column: output planes [mb, mb+len) */
+struct Seg {
+  int a0, b0, p0, np;   /* tile origin; first staged plane (mb-2); planes to stage (len+4) */
+};
+
+/*
+ * Persistent and warp-specialised.  The work of one launch is the list of (tile column, marched plane)
+ * pairs in column-major order; CTA b owns the contiguous range [b*PPC, (b+1)*PPC) of it, i.e. a few
+ * column segments, so that all CTAs finish together (no wave quantisation).  Threads [0, NC) are
+ * CONSUMERS (4 per face: tangential passes + flux), threads [NC, NC+NP) are PRODUCERS (normal
+ * reconstruction + collision on the halo faces, one to two planes ahead).  The two groups meet only at
+ * the named barriers FULL/EMPTY of the double-buffered Q0|Dn hand-over.
+ */
 template <int DIR, bool NEED_F, int TA, int TB>
-__global__ void __launch_bounds__(TA *TB * 4, 2)
-    k_sweep_fused(const __grid_constant__ CUtensorMap tmap, GksGrid g, GksPhys ph, double *__restrict__ flux, int MC, int dbg) {
+__global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, Tile<DIR, TA, TB>::CTAS_PER_SM)
+    k_sweep_fused(const __grid_constant__ CUtensorMap tmap, GksGrid g, GksPhys ph, double *__restrict__ flux,
+                  int ncol_a, long long total, long long PPC) {
   using T = Tile<DIR, TA, TB>;
-  constexpr int TN = T::TN, T1 = T::T1, NF = T::NF, NT = T::NT, EA = T::EA, EB = T::EB, HA = T::HA, FH = T::FH;
+  constexpr int TN = T::TN, NF = T::NF, NC = T::NC, NP = T::NP, NT = T::NT, EA = T::EA, EB = T::EB, HA = T::HA,
+                FH = T::FH;
   extern __shared__ __align__(128) double sm[];
   double *const Wp = sm + T::OFF_W;
-  double *const QL = sm + T::OFF_Q;            /* [FH][4] */
-  double *const QR = QL + FH * 4;              /* [FH][4] */
+  double *const QLs = sm + T::OFF_S;           /* [FH][4] */
+  double *const QRs = QLs + FH * 4;            /* [FH][4] */
   double *const CF = sm + T::OFF_CF;           /* [FH][4]: el, rho_l*xl, er, rho_r*xr */
+  double *const Qb = sm + T::OFF_Q;            /* [2][2][FH][4] */
   double *const XBuf = sm + T::OFF_XB;
-  double *const ring = sm + T::OFF_RING;       /* [5][6][NF][4] */
+  double *const ring = sm + T::OFF_RING;       /* [4][6][NF][4] */
   uint64_t *const bar = reinterpret_cast<uint64_t *>(sm + T::OFF_BAR);
 
   const int tid = threadIdx.x;
-  const int a0 = blockIdx.x * TA, b0 = blockIdx.y * TB;
-  const int m0 = blockIdx.z * MC;
-  const int m1 = min(m0 + MC, g.n[T::AXM]);
-  const int p0 = m0 - 2, np = (m1 - m0) + 4;   /* planes p0 .. p0+np-1 */
+  const int n2 = g.n[T::AXM];
   const double eps = ph.weno_eps;
-
-  /* face owned in phases D-F */
-  const int c = tid & 3, fid = tid >> 2;
-  const int fa = fid % TA, fb = fid / TA;       /* a fastest: coalesced output */
-  const int ga = a0 + fa, gb = b0 + fb;         /* global indices along a and b */
-  const int n_a = g.n[0] + (T::NA ? 1 : 0), n_b = g.n[T::AXB] + (T::NA ? 0 : 1);
-  const bool face_ok = ga < n_a && gb < n_b;
-  const int t1_local = T::NA ? fb : fa, t1_glob = T::NA ? gb : ga;
-  const double iw1 = g.inv_w[T::AXT1][min(t1_glob, g.n[T::AXT1] - 1) + GKS_NG];
-
-  /* TMA coordinates (padded index space: cell -3 <-> 0) */
-  const int ca0 = a0, cb0 = T::NA ? b0 + 1 : b0;
-  auto issue = [&](int it) {
-    uint64_t *b = &bar[it & 1];
-    double *dst = Wp + (it & 1) * T::WSLAB_PAD;
-    const int pm = p0 + it + GKS_NG;
-    mbar_expect_tx(b, T::WSLAB * 8);
-    if (DIR == 2) tma_load_4d(dst, &tmap, b, ca0, pm, cb0, 0);
-    else tma_load_4d(dst, &tmap, b, ca0, cb0, pm, 0);
+  long long L0 = (long long)blockIdx.x * PPC, L1 = L0 + PPC;
+  if (L0 > total) L0 = total;
+  if (L1 > total) L1 = total;
+  auto seg_at = [&](long long l) {
+    const int col = (int)(l / n2), mb = (int)(l - (long long)col * n2);
+    const long long left = L1 - l;
+    const int len = (int)(left < (long long)(n2 - mb) ? left : (long long)(n2 - mb));
+    Seg s;
+    s.a0 = (col % ncol_a) * TA;
+    s.b0 = (col / ncol_a) * TB;
+    s.p0 = mb - 2;
+    s.np = len + 4;
+    return s;
   };
+  int planes_total = 0;                        /* staged planes of this CTA over all its segments */
+  for (long long l = L0; l < L1;) {
+    const Seg s = seg_at(l);
+    planes_total += s.np;
+    l += s.np - 4;
+  }
+
   if (tid == 0) {
     mbar_init(&bar[0], 1);
     mbar_init(&bar[1], 1);
     fence_barrier_init();
   }
   __syncthreads();
-  if (dbg == 1) return;
-  if (tid == 0) {
-    issue(0);
-    if (np > 1) issue(1);
+
+  if (tid >= NC) {
+    /* ======================= PRODUCER ======================= */
+    const int pt = tid - NC;
+    /* TMA prefetch cursor (used by pt == 0 only): next plane to request and its running number */
+    long long lpf = L0;
+    Seg spf = seg_at(L0 < L1 ? L0 : 0);
+    int itpf = 0, gpf = 0;
+    auto issue_next = [&]() {
+      if (lpf >= L1) return;
+      uint64_t *b = &bar[gpf & 1];
+      double *dst = Wp + (gpf & 1) * T::WSLAB_PAD;
+      const int pm = spf.p0 + itpf + GKS_NG;   /* padded index space: cell -3 <-> 0 */
+      const int ca0 = spf.a0, cb0 = T::NA ? spf.b0 + 1 : spf.b0;
+      mbar_expect_tx(b, T::WSLAB * 8);
+      if (DIR == 2) tma_load_4d(dst, &tmap, b, ca0, pm, cb0, 0);
+      else tma_load_4d(dst, &tmap, b, ca0, cb0, pm, 0);
+      ++gpf;
+      if (++itpf == spf.np) {
+        lpf += spf.np - 4;
+        itpf = 0;
+        if (lpf < L1) spf = seg_at(lpf);
+      }
+    };
+    if (pt == 0) {
+      issue_next();
+      issue_next();
+    }
+    constexpr int sn = T::NA ? 1 : EA;         /* slab stride along the normal */
+    int gi = 0;                                /* running plane number: selects slab, hand-over buffer, parities */
+    for (long long l = L0; l < L1;) {
+      const Seg s = seg_at(l);
+      l += s.np - 4;
+      for (int it = 0; it < s.np; ++it, ++gi) {
+        const double *W = Wp + (gi & 1) * T::WSLAB_PAD;
+        mbar_wait(&bar[gi & 1], (gi >> 1) & 1);
+
+        /* ---- A: both edge values of each cell, per component (one smoothness-indicator set serves the
+         *         face on either side); two cells per thread at a time, a single one in the ragged tail ---- */
+        {
+          constexpr int NITEM = T::NCA * T::NCB * 4;
+          auto locate = [&](int item, const double *&w, int &cn, int &ct, int &cc) {
+            cc = item & 3;
+            const int cell = item >> 2;
+            const int xa = cell % T::NCA, xb = cell / T::NCA;
+            const int sa = T::NA ? xa + 2 : xa + 1, sb = T::NA ? xb : xb + 2;
+            w = W + (cc * EB + sb) * EA + sa;
+            cn = T::NA ? xa : xb; /* cell along the normal: global f0-1+cn */
+            ct = T::NA ? xb : xa; /* halo index along t1 */
+          };
+          auto store = [&](int cn, int ct, int cc, double vl, double vr) {
+            if (cn >= 1) { /* left edge = face cn-1: Qr */
+              const int fh = T::NA ? ct * HA + (cn - 1) : (cn - 1) * HA + ct;
+              QRs[fh * 4 + cc] = vl;
+            }
+            if (cn < TN) { /* right edge = face cn: Ql */
+              const int fh = T::NA ? ct * HA + cn : cn * HA + ct;
+              QLs[fh * 4 + cc] = vr;
+            }
+          };
+          int item0 = pt;
+          for (; item0 + NP < NITEM; item0 += 2 * NP) {
+            double q[5][2], vl[2], vr[2];
+            int cnv[2], ctv[2], ccv[2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+              const double *w;
+              locate(item0 + u * NP, w, cnv[u], ctv[u], ccv[u]);
+#pragma unroll
+              for (int k = 0; k < 5; ++k) q[k][u] = w[(k - 2) * sn];
+            }
+            gksd::weno5_edges_v<2>(q, eps, vl, vr);
+#pragma unroll
+            for (int u = 0; u < 2; ++u) store(cnv[u], ctv[u], ccv[u], vl[u], vr[u]);
+          }
+          if (item0 < NITEM) {
+            double q[5][1], vl[1], vr[1];
+            int cn, ct, cc;
+            const double *w;
+            locate(item0, w, cn, ct, cc);
+#pragma unroll
+            for (int k = 0; k < 5; ++k) q[k][0] = w[(k - 2) * sn];
+            gksd::weno5_edges_v<1>(q, eps, vl, vr);
+            store(cn, ct, cc, vl[0], vr[0]);
+          }
+        }
+        bar_sync(BAR_PROD, NP);
+
+        /* ---- B: collision factors (S4), one thread per (face, side), two independent chains at a time ---- */
+        for (int item0 = pt; item0 < FH * 2; item0 += 2 * NP) {
+          double z[2], rho[2], erfz[2], ex[2], ir[2];
+          int at[2];
+          bool ok[2];
+#pragma unroll
+          for (int u = 0; u < 2; ++u) {
+            const int item = item0 + u * NP;
+            ok[u] = item < FH * 2;
+            const int it2 = ok[u] ? item : item0;
+            const int side = it2 & 1, fh = it2 >> 1;
+            const double *q = (side ? QRs : QLs) + fh * 4;
+            rho[u] = q[0];
+            z[u] = q[1 + DIR];
+            at[u] = fh * 4 + 2 * side;
+          }
+          gksd::fast_rcp_v<2>(rho, ir);
+#pragma unroll
+          for (int u = 0; u < 2; ++u) z[u] = ph.theta * (z[u] * ir[u]);
+          gksd::erf_expm2_v<2>(z, erfz, ex);
+#pragma unroll
+          for (int u = 0; u < 2; ++u) {
+            if (!ok[u]) continue;
+            const double h = (at[u] & 2) ? -0.5 : 0.5;   /* erfc(+z)/2 right, erfc(-z)/2 left */
+            CF[at[u]] = fma(h, erfz[u], 0.5);
+            CF[at[u] + 1] = rho[u] * (ph.cx * ex[u]);
+          }
+        }
+        bar_sync(BAR_PROD, NP);
+
+        /* the hand-over buffer (gi & 1) was last read by pass 1 of plane gi-2 */
+        if (gi >= 2) bar_sync(BAR_EMPTY0 + (gi & 1), NT);
+
+        /* ---- C: Q0 and Dn on the halo faces -> hand-over buffer ---- */
+        {
+          double *const Q0o = Qb + (gi & 1) * (2 * FH * 4);
+          double *const Dno = Q0o + FH * 4;
+#pragma unroll 2
+          for (int item = pt; item < FH * 4; item += NP) {
+            const int cc = item & 3, fh = item >> 2;
+            const int ha = fh % HA, hb = fh / HA;
+            const double el = CF[fh * 4], er = CF[fh * 4 + 2];
+            double q0 = QLs[item] * el + QRs[item] * er;
+            if (cc == 1 + DIR) q0 += CF[fh * 4 + 1] - CF[fh * 4 + 3];
+            /* normal slope from the 4 cells around the face; face nf sits between slab cells nf+2, nf+3 */
+            const int sa = T::NA ? ha + 3 : ha + 1, sb = T::NA ? hb : hb + 3;
+            const double *w = W + (cc * EB + sb) * EA + sa;
+            const int nf_glob = (T::NA ? s.a0 + ha : s.b0 + hb);
+            const double ihn = g.inv_hn[DIR][min(nf_glob, g.n[DIR]) + GKS_NG];
+            Q0o[item] = q0;
+            Dno[item] = gksd::normal_slope(w[-2 * sn], w[-sn], w[0], w[sn]) * ihn;
+          }
+        }
+        __threadfence_block();
+        bar_arrive(BAR_FULL0 + (gi & 1), NT);
+        bar_sync(BAR_PROD, NP);                        /* slab (gi & 1) and the staging arrays are free again */
+        if (pt == 0) issue_next();                     /* plane gi+2 (possibly of the next segment) */
+      }
+    }
+    return;
   }
-  if (dbg == 2) { mbar_wait(&bar[0], 0); mbar_wait(&bar[1], 0); return; }
 
-  for (int it = 0; it < np; ++it) {
-    const double *W = Wp + (it & 1) * T::WSLAB_PAD;
-    mbar_wait(&bar[it & 1], (it >> 1) & 1);
-    if (dbg == 3) { __syncthreads(); if (tid == 0 && it + 2 < np) issue(it + 2); continue; }
+  /* ======================= CONSUMER ======================= */
+  const int c = tid & 3, fid = tid >> 2;
+  const int fa = fid % TA, fb = fid / TA;       /* a fastest: coalesced output */
+  const int n_a = g.n[0] + (T::NA ? 1 : 0), n_b = g.n[T::AXB] + (T::NA ? 0 : 1);
+  const int t1_local = T::NA ? fb : fa;
+  constexpr int s1 = T::NA ? HA : 1;                         /* halo-face stride along t1 */
+  const int fh0 = T::NA ? (t1_local + 2) * HA + fa : fb * HA + (t1_local + 2);
+  double *const rg = ring + fid * 4 + c;        /* this thread's private column of the ring */
+  constexpr int RS = 6 * NF * 4, RF = NF * 4;   /* ring strides: plane slot, field */
+  /* transpose buffer: element (field, component cc, Gauss point gq) of face fid lives at
+   * fid*64 + field*16 + 4*(cc ^ (fid&3)) + (gq ^ cc): conflict-free for the component-major writes
+   * and for the Gauss-point-major reads of a half warp */
+  double *const xw = XBuf + fid * 64 + 4 * (c ^ (fid & 3));                /* writes: + field*16 + (gq ^ c) */
+  const double *const xr = XBuf + fid * 64;                                 /* reads:  + field*16 + ro[cc] */
+  int ro[4];
+#pragma unroll
+  for (int cc = 0; cc < 4; ++cc) ro[cc] = 4 * (cc ^ (fid & 3)) + (c ^ cc);
 
-    /* ---- A: both edge values of each cell, per component; two cells per thread at a time ---- */
-    {
-      constexpr int NITEM = T::NCA * T::NCB * 4;
-      constexpr int sn = T::NA ? 1 : EA;
-      for (int item0 = tid; item0 < NITEM; item0 += 2 * NT) {
-        double q[5][2], vl[2], vr[2];
-        int cnv[2], ctv[2], ccv[2];
-        bool ok[2];
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-          const int item = item0 + u * NT;
-          ok[u] = item < NITEM;
-          const int it2 = ok[u] ? item : item0;
-          const int cc = it2 & 3, cell = it2 >> 2;
-          const int xa = cell % T::NCA, xb = cell / T::NCA;
-          const int sa = T::NA ? xa + 2 : xa + 1, sb = T::NA ? xb : xb + 2;
-          const double *w = W + (cc * EB + sb) * EA + sa;
-#pragma unroll
-          for (int k = 0; k < 5; ++k) q[k][u] = w[(k - 2) * sn];
-          cnv[u] = T::NA ? xa : xb; /* cell along the normal: global f0-1+cn */
-          ctv[u] = T::NA ? xb : xa; /* halo index along t1 */
-          ccv[u] = cc;
-        }
-        gksd::weno5_edges_v<2>(q, eps, vl, vr);
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-          if (!ok[u]) continue;
-          const int cn = cnv[u], ct = ctv[u];
-          if (cn >= 1) { /* left edge = face cn-1: Qr */
-            const int fh = T::NA ? ct * HA + (cn - 1) : (cn - 1) * HA + ct;
-            QR[fh * 4 + ccv[u]] = vl[u];
-          }
-          if (cn < TN) { /* right edge = face cn: Ql */
-            const int fh = T::NA ? ct * HA + cn : cn * HA + ct;
-            QL[fh * 4 + ccv[u]] = vr[u];
-          }
-        }
-      }
-    }
-    __syncthreads();
-    if (dbg == 4) { __syncthreads(); if (tid == 0 && it + 2 < np) issue(it + 2); continue; }
-
-    /* ---- B: collision factors, one thread per (face, side) ---- */
-    for (int item = tid; item < FH * 2; item += NT) {
-      const int side = item & 1, fh = item >> 1;
-      const double *q = (side ? QR : QL) + fh * 4;
-      const double rho = q[0], U = q[1 + DIR] * gksd::fast_rcp(rho);
-      double erfz, ex;
-      gksd::erf_expm2(ph.theta * U, erfz, ex);
-      const double e = side ? 0.5 - 0.5 * erfz : 0.5 + 0.5 * erfz; /* erfc(+z)/2 right, erfc(-z)/2 left */
-      const double x = ph.cx * ex;
-      CF[fh * 4 + 2 * side] = e;
-      CF[fh * 4 + 2 * side + 1] = rho * x;
-    }
-    __syncthreads();
-
-    /* ---- C: Q0 and Dn on the halo faces, in place of Ql / Qr ---- */
-    for (int item = tid; item < FH * 4; item += NT) {
-      const int cc = item & 3, fh = item >> 2;
-      const int ha = fh % HA, hb = fh / HA;
-      const double el = CF[fh * 4], er = CF[fh * 4 + 2];
-      double q0 = QL[item] * el + QR[item] * er;
-      if (cc == 1 + DIR) q0 += CF[fh * 4 + 1] - CF[fh * 4 + 3];
-      /* normal slope from the 4 cells around the face; face nf sits between slab cells nf+2, nf+3 */
-      const int sa = T::NA ? ha + 3 : ha + 1, sb = T::NA ? hb : hb + 3;
-      const double *w = W + (cc * EB + sb) * EA + sa;
-      constexpr int sn = T::NA ? 1 : EA;
-      const int nf_glob = (T::NA ? a0 + ha : b0 + hb);
-      const double ihn = g.inv_hn[DIR][min(nf_glob, g.n[DIR]) + GKS_NG];
-      const double dn = gksd::normal_slope(w[-2 * sn], w[-sn], w[0], w[sn]) * ihn;
-      QL[item] = q0;
-      QR[item] = dn;
-    }
-    __syncthreads();
-    if (tid == 0 && it + 2 < np) issue(it + 2);   /* slab buffer (it&1) is free again */
-    if (dbg == 5) continue;
-
-    /* ---- D: tangential pass 1 -> ring slot ---- */
-    {
-      const int slot = it % 5;
-      double *r = ring + (size_t)slot * 6 * NF * 4 + fid * 4 + c;
-      constexpr int s1 = T::NA ? HA : 1;                         /* halo-face stride along t1 */
-      const int fh = T::NA ? (t1_local + 2) * HA + fa : fb * HA + (t1_local + 2);
-      const double *q = QL + fh * 4 + c; /* Q0 */
-      const double *d = QR + fh * 4 + c; /* Dn */
-      double qq[5][2], vm[2], vp[2], sm_[2], sp_[2];
-#pragma unroll
-      for (int k = 0; k < 5; ++k) {
-        qq[k][0] = q[(k - 2) * s1 * 4];
-        qq[k][1] = d[(k - 2) * s1 * 4];
-      }
-      gksd::weno5_gauss_v<2>(qq, eps, vm, vp, sm_, sp_);
-      r[0 * NF * 4] = vm[0];
-      r[1 * NF * 4] = vp[0];
-      r[2 * NF * 4] = vm[1];
-      r[3 * NF * 4] = vp[1];
-      r[4 * NF * 4] = sm_[0] * iw1;
-      r[5 * NF * 4] = sp_[0] * iw1;
-    }
-    __syncthreads();
-    if (dbg == 6) continue;
-
-    if (it >= 4) {
-      /* ---- E: tangential pass 2 for plane m = p-2 (ring holds planes p-4 .. p) ---- */
-      const int m = p0 + it - 2;
-      const double iw2 = g.inv_w[T::AXM][m + GKS_NG];
-      const double *rs[5];
-#pragma unroll
-      for (int k = 0; k < 5; ++k) rs[k] = ring + (size_t)((it + 1 + k) % 5) * 6 * NF * 4 + fid * 4 + c;
-      double *xb = XBuf + fid * T::XBS + c * 4;     /* [fld][c][g], g = 2*g1 + g2 */
-#pragma unroll
-      for (int fld = 0; fld < 3; ++fld) { /* Q0, Dn, Dt1: the two g1 instances of a field go together */
+  int gi = 0;
+  for (long long l = L0; l < L1;) {
+    const Seg s = seg_at(l);
+    l += s.np - 4;
+    const int ga = s.a0 + fa, gb = s.b0 + fb;     /* global indices along a and b */
+    const bool face_ok = ga < n_a && gb < n_b;
+    const int t1_glob = T::NA ? gb : ga;
+    const double iw1 = g.inv_w[T::AXT1][min(t1_glob, g.n[T::AXT1] - 1) + GKS_NG];
+    for (int it = 0; it < s.np; ++it, ++gi) {
+      bar_sync(BAR_FULL0 + (gi & 1), NT);
+      /* ---- D: tangential pass 1 (along t1) on Q0 and Dn of plane it ---- */
+      double d6[6];
+      {
+        const double *q = Qb + (gi & 1) * (2 * FH * 4) + fh0 * 4 + c; /* Q0 */
+        const double *d = q + FH * 4;                                 /* Dn */
         double qq[5][2], vm[2], vp[2], sm_[2], sp_[2];
 #pragma unroll
         for (int k = 0; k < 5; ++k) {
-          qq[k][0] = rs[k][(2 * fld) * NF * 4];
-          qq[k][1] = rs[k][(2 * fld + 1) * NF * 4];
+          qq[k][0] = q[(k - 2) * s1 * 4];
+          qq[k][1] = d[(k - 2) * s1 * 4];
         }
         gksd::weno5_gauss_v<2>(qq, eps, vm, vp, sm_, sp_);
-#pragma unroll
-        for (int g1 = 0; g1 < 2; ++g1) {
-          xb[fld * 16 + 2 * g1] = vm[g1];
-          xb[fld * 16 + 2 * g1 + 1] = vp[g1];
-          if (fld == 0) {
-            xb[3 * 16 + 2 * g1] = sm_[g1] * iw2;
-            xb[3 * 16 + 2 * g1 + 1] = sp_[g1] * iw2;
-          }
-        }
+        d6[0] = vm[0];
+        d6[1] = vp[0];
+        d6[2] = vm[1];
+        d6[3] = vp[1];
+        d6[4] = sm_[0] * iw1;
+        d6[5] = sp_[0] * iw1;
       }
-      __syncwarp();
-      /* ---- F: flux at Gauss point gp = c of this face; sum over the 4 lanes; write ---- */
-      {
-        const int gp = c;
-        const double *x = XBuf + fid * T::XBS + gp;
-        double Q0[4], dQ[3][4], F[4], dF[4];
+      /* the loaded values have been consumed: the hand-over buffer may be refilled (plane gi+2) */
+      if (gi + 2 < planes_total) bar_arrive(BAR_EMPTY0 + (gi & 1), NT);
+
+    double *const rnew = rg + (it & 3) * RS;     /* slot of plane it-4, dead once pass 2 below has read it */
+    if (it < 4) {
 #pragma unroll
-        for (int cc = 0; cc < 4; ++cc) {
-          Q0[cc] = x[0 * 16 + cc * 4];
-          dQ[DIR][cc] = x[1 * 16 + cc * 4];
-          dQ[T::AXT1][cc] = x[2 * 16 + cc * 4];
-          dQ[T::AXM][cc] = x[3 * 16 + cc * 4];
-        }
-        gksd::gauss_point_flux<DIR, NEED_F>(Q0, dQ, ph.RT, ph.mu, F, dF);
-#pragma unroll
-        for (int cc = 0; cc < 4; ++cc) {
-          if (NEED_F) {
-            F[cc] += __shfl_xor_sync(0xffffffffu, F[cc], 1);
-            F[cc] += __shfl_xor_sync(0xffffffffu, F[cc], 2);
-          }
-          dF[cc] += __shfl_xor_sync(0xffffffffu, dF[cc], 1);
-          dF[cc] += __shfl_xor_sync(0xffffffffu, dF[cc], 2);
-        }
-        if (face_ok) {
-          int pidx[3];
-          pidx[0] = ga;
-          pidx[T::AXB] = gb;
-          pidx[T::AXM] = m;
-          const long long id = g.idx(pidx[0], pidx[1], pidx[2]);
-          double fsel = 0.0, dsel = 0.0;
-#pragma unroll
-          for (int cc = 0; cc < 4; ++cc)
-            if (cc == c) {
-              if (NEED_F) fsel = F[cc];
-              dsel = dF[cc];
-            }
-          if (NEED_F) flux[c * g.FS + id] = 0.25 * fsel;
-          flux[(4 + c) * g.FS + id] = 0.25 * dsel;
-        }
-      }
-      __syncthreads();   /* the transpose buffer aliases QL/QR/CF of the next plane */
+      for (int v = 0; v < 6; ++v) rnew[v * RF] = d6[v];
+      continue;
     }
+    /* ---- E: tangential pass 2 (along t2, the marched axis) for plane m = it-2; the ring holds planes
+     *         it-4 .. it-1 (plane it-4+k in slot (it+k)&3), plane it comes straight from d6 ---- */
+    const int m = s.p0 + it - 2;
+    const double iw2 = g.inv_w[T::AXM][m + GKS_NG];
+    const double *rs[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) rs[k] = rg + ((it + k) & 3) * RS;
+#pragma unroll
+    for (int fld = 0; fld < 3; ++fld) { /* Q0, Dn, Dt1: the two g1 instances of a field go together */
+      double qq[5][2], vm[2], vp[2], sm_[2], sp_[2];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        qq[k][0] = rs[k][(2 * fld) * RF];
+        qq[k][1] = rs[k][(2 * fld + 1) * RF];
+      }
+      qq[4][0] = d6[2 * fld];
+      qq[4][1] = d6[2 * fld + 1];
+      rnew[(2 * fld) * RF] = d6[2 * fld];          /* rs[0] aliases rnew: stored after the loads above */
+      rnew[(2 * fld + 1) * RF] = d6[2 * fld + 1];
+      gksd::weno5_gauss_v<2>(qq, eps, vm, vp, sm_, sp_);
+#pragma unroll
+      for (int g1 = 0; g1 < 2; ++g1) {            /* Gauss point gq = 2*g1 + g2 */
+        xw[fld * 16 + ((2 * g1) ^ c)] = vm[g1];
+        xw[fld * 16 + ((2 * g1 + 1) ^ c)] = vp[g1];
+        if (fld == 0) {
+          xw[3 * 16 + ((2 * g1) ^ c)] = sm_[g1] * iw2;
+          xw[3 * 16 + ((2 * g1 + 1) ^ c)] = sp_[g1] * iw2;
+        }
+      }
+    }
+    __syncwarp();
+    /* ---- F: flux at Gauss point gp = c of this face; sum over the 4 lanes; write ---- */
+    {
+      double Q0[4], dQ[3][4], F[4], dF[4];
+#pragma unroll
+      for (int cc = 0; cc < 4; ++cc) {
+        Q0[cc] = xr[0 * 16 + ro[cc]];
+        dQ[DIR][cc] = xr[1 * 16 + ro[cc]];
+        dQ[T::AXT1][cc] = xr[2 * 16 + ro[cc]];
+        dQ[T::AXM][cc] = xr[3 * 16 + ro[cc]];
+      }
+      gksd::gauss_point_flux<DIR, NEED_F>(Q0, dQ, ph.RT, ph.mu, F, dF);
+      __syncwarp();                               /* every lane has consumed its reads: the buffer is reusable */
+#pragma unroll
+      for (int cc = 0; cc < 4; ++cc) {
+        if (NEED_F) {
+          F[cc] += __shfl_xor_sync(0xffffffffu, F[cc], 1);
+          F[cc] += __shfl_xor_sync(0xffffffffu, F[cc], 2);
+        }
+        dF[cc] += __shfl_xor_sync(0xffffffffu, dF[cc], 1);
+        dF[cc] += __shfl_xor_sync(0xffffffffu, dF[cc], 2);
+      }
+      if (face_ok) {
+        int pidx[3];
+        pidx[0] = ga;
+        pidx[T::AXB] = gb;
+        pidx[T::AXM] = m;
+        const long long id = g.idx(pidx[0], pidx[1], pidx[2]);
+        double fsel = 0.0, dsel = 0.0;
+#pragma unroll
+        for (int cc = 0; cc < 4; ++cc)
+          if (cc == c) {
+            if (NEED_F) fsel = F[cc];
+            dsel = dF[cc];
+          }
+        if (NEED_F) flux[c * g.FS + id] = 0.25 * fsel;
+        flux[(4 + c) * g.FS + id] = 0.25 * dsel;
+      }
+    }
+  }
   }
 }
 
@@ -349,8 +464,8 @@ typedef CUresult (*encode_fn_t)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, 
                                 const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
                                 CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-/* tile shapes: x-faces 8x8 (normal along a), y/z-faces 16x4 (t1 along a, 4 faces along the normal) */
-template <int DIR> struct Shape { static constexpr int TA = DIR == 0 ? 8 : 16, TB = DIR == 0 ? 8 : 4; };
+/* tile shapes: 128 faces per CTA; x-faces 8 (normal, along a) x 16 (t1), y/z-faces 16 (t1, along a) x 8 (normal) */
+template <int DIR> struct Shape { static constexpr int TA = DIR == 0 ? 8 : 16, TB = DIR == 0 ? 16 : 8; };
 
 template <int DIR>
 bool encode_dir(encode_fn_t enc, const GksGrid &g, double *base, CUtensorMap *out) {
@@ -378,15 +493,14 @@ int launch_dir(gks_ctx *ctx, const CUtensorMap &map, double *flux) {
   }
   const int ext_a = g.n[0] + (T::NA ? 1 : 0), ext_b = g.n[T::AXB] + (T::NA ? 0 : 1), n2 = g.n[T::AXM];
   const int ga = (ext_a + TA - 1) / TA, gb = (ext_b + TB - 1) / TB;
-  /* chunks along the marched axis: enough CTAs for ~6 waves of 2 CTAs/SM, each at least 32 planes */
-  long long cols = (long long)ga * gb;
-  int nch = (int)((1776 + cols - 1) / cols);
-  const int maxch = n2 / 32 > 1 ? n2 / 32 : 1;
-  if (nch > maxch) nch = maxch;
-  if (nch < 1) nch = 1;
-  const int MC = (n2 + nch - 1) / nch;
-  nch = (n2 + MC - 1) / MC;
-  kern<<<dim3(ga, gb, nch), T::NT, T::SMEM_BYTES, ctx->stream>>>(map, g, ctx->ph, flux, MC, getenv("GKS_DBG") ? atoi(getenv("GKS_DBG")) : 0);
+  /* persistent CTAs: the (column, plane) list is cut into equal contiguous ranges, one per resident CTA;
+     a range shorter than 8 planes is not worth its 4 priming planes */
+  const long long total = (long long)ga * gb * n2;
+  const long long slots = (long long)ctx->num_sms * T::CTAS_PER_SM;
+  long long PPC = (total + slots - 1) / slots;
+  if (PPC < 8) PPC = 8;
+  const int nblk = (int)((total + PPC - 1) / PPC);
+  kern<<<nblk, T::NT, T::SMEM_BYTES, ctx->stream>>>(map, g, ctx->ph, flux, ga, total, PPC);
   return 1;
 }
 
@@ -401,6 +515,12 @@ bool gks_fused_init(gks_ctx *ctx) {
     return false;
   }
   encode_fn_t enc = (encode_fn_t)fn;
+  int dev = 0, nsm = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm < 1) {
+    cudaGetLastError();
+    return false;
+  }
+  ctx->num_sms = nsm;
   double *bases[2] = {ctx->Wn, ctx->Ws};
   for (int b = 0; b < 2; ++b) {
     CUtensorMap *m = reinterpret_cast<CUtensorMap *>(ctx->tmaps[b][0]);
