@@ -71,10 +71,9 @@ __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, u
       : "memory");
 }
 
-/* named barriers (bar.sync / bar.arrive with a thread count): producer <-> consumer hand-over */
-__device__ __forceinline__ void bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
-__device__ __forceinline__ void bar_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
-enum { BAR_PROD = 1, BAR_FULL0 = 2, BAR_EMPTY0 = 4 }; /* FULL0/FULL1 = 2,3; EMPTY0/EMPTY1 = 4,5; 0 = __syncthreads */
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 
 /* ---------------- compile-time geometry of a tile ---------------- */
 template <int DIR, int TA, int TB>
@@ -83,9 +82,8 @@ struct Tile {
   static constexpr int TN = NA ? TA : TB;           /* faces along the normal */
   static constexpr int T1 = NA ? TB : TA;           /* faces along t1 */
   static constexpr int NF = TA * TB;                /* faces per CTA and plane */
-  static constexpr int NC = NF * 4;                 /* consumer threads (4 per face) */
-  static constexpr int NP = NC / 2;                 /* producer threads */
-  static constexpr int NT = NC + NP;                /* threads per CTA */
+  static constexpr int NT = NF * 4;                 /* threads per CTA (4 per face) */
+  static constexpr int NW = NT / 32;                /* warps */
   static constexpr int CA = NA ? TN + 5 : T1 + 5;   /* cells of the W slab along a / b; the slab always starts at
                                                        cell a0-3: TMA needs a 16-byte aligned box start (even index) */
   static constexpr int CB = NA ? T1 + 4 : TN + 5;
@@ -94,7 +92,7 @@ struct Tile {
   static constexpr int HA = NA ? TN : T1 + 4;       /* halo-face box (faces needed by pass 1) */
   static constexpr int HB = NA ? T1 + 4 : TN;
   static constexpr int FH = HA * HB;
-  static constexpr int NCA = NA ? TN + 1 : T1 + 4;  /* cells reconstructed in phase A */
+  static constexpr int NCA = NA ? TN + 1 : T1 + 4;  /* cells reconstructed in stage A */
   static constexpr int NCB = NA ? T1 + 4 : TN + 1;
   static constexpr int AXB = DIR == 2 ? 2 : 1;      /* global axis of b */
   static constexpr int AXM = DIR == 2 ? 1 : 2;      /* global axis marched (= t2) */
@@ -103,17 +101,15 @@ struct Tile {
   static constexpr int WSLAB_PAD = (WSLAB + 15) & ~15;
   /* shared memory carve (doubles) */
   static constexpr int OFF_W = 0;                          /* 2 slabs (TMA destinations) */
-  static constexpr int OFF_S = OFF_W + 2 * WSLAB_PAD;      /* producer staging: QL|QR [2][FH][4] */
-  static constexpr int OFF_CF = OFF_S + 2 * FH * 4;        /* collision factors [FH][4] */
-  static constexpr int OFF_Q = OFF_CF + FH * 4;            /* 2 hand-over buffers, each Q0|Dn [2][FH][4] */
-  static constexpr int OFF_XB = OFF_Q + 2 * 2 * FH * 4;    /* transpose buffer, 64 doubles per face, XOR-swizzled */
+  static constexpr int SBUF = 3 * FH * 4;                  /* one stage buffer: QL->Q0 | QR | Dn, each [FH][4] */
+  static constexpr int OFF_S = OFF_W + 2 * WSLAB_PAD;      /* 3 stage buffers (plane j lives in buffer j % 3) */
+  static constexpr int OFF_XB = OFF_S + 3 * SBUF;          /* transpose buffer, 64 doubles per face, XOR-swizzled */
   static constexpr int OFF_RING = OFF_XB + NF * 64;        /* 4-plane ring of pass-1 results [4][6][NF][4] */
   static constexpr int RING = 4 * 6 * NF * 4;
-  static constexpr int OFF_BAR = OFF_RING + RING;
-  static constexpr size_t SMEM_BYTES = (size_t)(OFF_BAR + 2) * 8;
-  static constexpr int CTAS_PER_SM = (2 * (SMEM_BYTES + 1024) <= 233472 && 2 * NT <= 1024) ? 2 : 1;
+  static constexpr int OFF_BAR = OFF_RING + RING;          /* mbarriers: 2 TMA + 1 iteration barrier */
+  static constexpr size_t SMEM_BYTES = (size_t)(OFF_BAR + 4) * 8;
   static_assert(SMEM_BYTES + 1024 <= 233472, "the CTA must fit in shared memory");
-  static_assert(NC % 32 == 0 && NP % 32 == 0, "whole warps per role");
+  static_assert(NT <= 1024 && NT % 32 == 0, "whole warps");
 };
 
 /* one contiguous run of marched planes of one tile column: output planes [mb, mb+len) */
@@ -122,29 +118,32 @@ struct Seg {
 };
 
 /*
- * Persistent and warp-specialised.  The work of one launch is the list of (tile column, marched plane)
- * pairs in column-major order; CTA b owns the contiguous range [b*PPC, (b+1)*PPC) of it, i.e. a few
- * column segments, so that all CTAs finish together (no wave quantisation).  Threads [0, NC) are
- * CONSUMERS (4 per face: tangential passes + flux), threads [NC, NC+NP) are PRODUCERS (normal
- * reconstruction + collision on the halo faces, one to two planes ahead).  The two groups meet only at
- * the named barriers FULL/EMPTY of the double-buffered Q0|Dn hand-over.
+ * Persistent, symmetric and software-pipelined.  The work of one launch is the list of (tile column,
+ * marched plane) pairs in column-major order; CTA b owns the contiguous range [b*PPC, (b+1)*PPC) of it,
+ * i.e. a few column segments (each costs 4 priming planes), so that all CTAs finish together.
+ *
+ * Every warp runs the same program.  Iteration i works on three different staged planes at once:
+ *     stage A  on plane i    : normal WENO edge values QL, QR and the normal slope Dn      -> S[i % 3]
+ *     stage BC on plane i-1  : collision Q0(QL, QR), in place                              -> S[(i-1) % 3]
+ *     stage D  on plane i-2  : tangential pass 1 (reads Q0, Dn of the t1 neighbours)       <- S[(i-2) % 3]
+ *     stage EF on plane i-2  : tangential pass 2 out of the thread-private ring, flux, store
+ * A, BC and D touch three different buffers, so an iteration needs ONE CTA-wide hand-over, and that one
+ * is split: a warp arrives on the iteration mbarrier after A, BC, D and waits for it only at the top of
+ * the next iteration, after its EF (about half of the iteration's arithmetic) - warps may drift by half
+ * an iteration without anyone waiting.
  */
 template <int DIR, bool NEED_F, int TA, int TB>
-__global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, Tile<DIR, TA, TB>::CTAS_PER_SM)
+__global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
     k_sweep_fused(const __grid_constant__ CUtensorMap tmap, GksGrid g, GksPhys ph, double *__restrict__ flux,
                   int ncol_a, long long total, long long PPC) {
   using T = Tile<DIR, TA, TB>;
-  constexpr int TN = T::TN, NF = T::NF, NC = T::NC, NP = T::NP, NT = T::NT, EA = T::EA, EB = T::EB, HA = T::HA,
-                FH = T::FH;
+  constexpr int TN = T::TN, NF = T::NF, NT = T::NT, EA = T::EA, EB = T::EB, HA = T::HA, FH = T::FH;
   extern __shared__ __align__(128) double sm[];
   double *const Wp = sm + T::OFF_W;
-  double *const QLs = sm + T::OFF_S;           /* [FH][4] */
-  double *const QRs = QLs + FH * 4;            /* [FH][4] */
-  double *const CF = sm + T::OFF_CF;           /* [FH][4]: el, rho_l*xl, er, rho_r*xr */
-  double *const Qb = sm + T::OFF_Q;            /* [2][2][FH][4] */
+  double *const Sb = sm + T::OFF_S;            /* [3][3][FH][4] */
   double *const XBuf = sm + T::OFF_XB;
   double *const ring = sm + T::OFF_RING;       /* [4][6][NF][4] */
-  uint64_t *const bar = reinterpret_cast<uint64_t *>(sm + T::OFF_BAR);
+  uint64_t *const bar = reinterpret_cast<uint64_t *>(sm + T::OFF_BAR);   /* [0],[1] TMA slabs; [2] iteration */
 
   const int tid = threadIdx.x;
   const int n2 = g.n[T::AXM];
@@ -152,6 +151,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, Tile<DIR, TA, TB>::CTAS
   long long L0 = (long long)blockIdx.x * PPC, L1 = L0 + PPC;
   if (L0 > total) L0 = total;
   if (L1 > total) L1 = total;
+  if (L0 >= L1) return;
   auto seg_at = [&](long long l) {
     const int col = (int)(l / n2), mb = (int)(l - (long long)col * n2);
     const long long left = L1 - l;
@@ -163,175 +163,57 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, Tile<DIR, TA, TB>::CTAS
     s.np = len + 4;
     return s;
   };
-  int planes_total = 0;                        /* staged planes of this CTA over all its segments */
+  int J = 0;                                   /* staged planes of this CTA over all its segments */
   for (long long l = L0; l < L1;) {
     const Seg s = seg_at(l);
-    planes_total += s.np;
+    J += s.np;
     l += s.np - 4;
   }
+  /* three cursors walk the same plane list: TMA (plane i+1), stage A (plane i), stages D/EF (plane i-2) */
+  struct Cur {
+    long long l;
+    Seg s;
+    int it;
+  };
+  auto cur_next = [&](Cur &c) {
+    if (++c.it == c.s.np) {
+      c.l += c.s.np - 4;
+      c.it = 0;
+      if (c.l < L1) c.s = seg_at(c.l);
+    }
+  };
+  Cur cT, cA, cD;
+  cT.l = L0; cT.s = seg_at(L0); cT.it = 0;
+  cA = cT;
+  cD = cT;
 
   if (tid == 0) {
     mbar_init(&bar[0], 1);
     mbar_init(&bar[1], 1);
+    mbar_init(&bar[2], T::NW);
     fence_barrier_init();
   }
   __syncthreads();
 
-  if (tid >= NC) {
-    /* ======================= PRODUCER ======================= */
-    const int pt = tid - NC;
-    /* TMA prefetch cursor (used by pt == 0 only): next plane to request and its running number */
-    long long lpf = L0;
-    Seg spf = seg_at(L0 < L1 ? L0 : 0);
-    int itpf = 0, gpf = 0;
-    auto issue_next = [&]() {
-      if (lpf >= L1) return;
-      uint64_t *b = &bar[gpf & 1];
-      double *dst = Wp + (gpf & 1) * T::WSLAB_PAD;
-      const int pm = spf.p0 + itpf + GKS_NG;   /* padded index space: cell -3 <-> 0 */
-      const int ca0 = spf.a0, cb0 = T::NA ? spf.b0 + 1 : spf.b0;
-      mbar_expect_tx(b, T::WSLAB * 8);
-      if (DIR == 2) tma_load_4d(dst, &tmap, b, ca0, pm, cb0, 0);
-      else tma_load_4d(dst, &tmap, b, ca0, cb0, pm, 0);
-      ++gpf;
-      if (++itpf == spf.np) {
-        lpf += spf.np - 4;
-        itpf = 0;
-        if (lpf < L1) spf = seg_at(lpf);
-      }
-    };
-    if (pt == 0) {
-      issue_next();
-      issue_next();
-    }
-    constexpr int sn = T::NA ? 1 : EA;         /* slab stride along the normal */
-    int gi = 0;                                /* running plane number: selects slab, hand-over buffer, parities */
-    for (long long l = L0; l < L1;) {
-      const Seg s = seg_at(l);
-      l += s.np - 4;
-      for (int it = 0; it < s.np; ++it, ++gi) {
-        const double *W = Wp + (gi & 1) * T::WSLAB_PAD;
-        mbar_wait(&bar[gi & 1], (gi >> 1) & 1);
+  auto issue = [&](const Cur &c, int j) {       /* request staged plane j (described by cursor c) */
+    uint64_t *b = &bar[j & 1];
+    double *dst = Wp + (j & 1) * T::WSLAB_PAD;
+    const int pm = c.s.p0 + c.it + GKS_NG;      /* padded index space: cell -3 <-> 0 */
+    const int ca0 = c.s.a0, cb0 = T::NA ? c.s.b0 + 1 : c.s.b0;
+    mbar_expect_tx(b, T::WSLAB * 8);
+    if (DIR == 2) tma_load_4d(dst, &tmap, b, ca0, pm, cb0, 0);
+    else tma_load_4d(dst, &tmap, b, ca0, cb0, pm, 0);
+  };
+  if (tid == 0) issue(cT, 0);
+  cur_next(cT);
 
-        /* ---- A: both edge values of each cell, per component (one smoothness-indicator set serves the
-         *         face on either side); two cells per thread at a time, a single one in the ragged tail ---- */
-        {
-          constexpr int NITEM = T::NCA * T::NCB * 4;
-          auto locate = [&](int item, const double *&w, int &cn, int &ct, int &cc) {
-            cc = item & 3;
-            const int cell = item >> 2;
-            const int xa = cell % T::NCA, xb = cell / T::NCA;
-            const int sa = T::NA ? xa + 2 : xa + 1, sb = T::NA ? xb : xb + 2;
-            w = W + (cc * EB + sb) * EA + sa;
-            cn = T::NA ? xa : xb; /* cell along the normal: global f0-1+cn */
-            ct = T::NA ? xb : xa; /* halo index along t1 */
-          };
-          auto store = [&](int cn, int ct, int cc, double vl, double vr) {
-            if (cn >= 1) { /* left edge = face cn-1: Qr */
-              const int fh = T::NA ? ct * HA + (cn - 1) : (cn - 1) * HA + ct;
-              QRs[fh * 4 + cc] = vl;
-            }
-            if (cn < TN) { /* right edge = face cn: Ql */
-              const int fh = T::NA ? ct * HA + cn : cn * HA + ct;
-              QLs[fh * 4 + cc] = vr;
-            }
-          };
-          int item0 = pt;
-          for (; item0 + NP < NITEM; item0 += 2 * NP) {
-            double q[5][2], vl[2], vr[2];
-            int cnv[2], ctv[2], ccv[2];
-#pragma unroll
-            for (int u = 0; u < 2; ++u) {
-              const double *w;
-              locate(item0 + u * NP, w, cnv[u], ctv[u], ccv[u]);
-#pragma unroll
-              for (int k = 0; k < 5; ++k) q[k][u] = w[(k - 2) * sn];
-            }
-            gksd::weno5_edges_v<2>(q, eps, vl, vr);
-#pragma unroll
-            for (int u = 0; u < 2; ++u) store(cnv[u], ctv[u], ccv[u], vl[u], vr[u]);
-          }
-          if (item0 < NITEM) {
-            double q[5][1], vl[1], vr[1];
-            int cn, ct, cc;
-            const double *w;
-            locate(item0, w, cn, ct, cc);
-#pragma unroll
-            for (int k = 0; k < 5; ++k) q[k][0] = w[(k - 2) * sn];
-            gksd::weno5_edges_v<1>(q, eps, vl, vr);
-            store(cn, ct, cc, vl[0], vr[0]);
-          }
-        }
-        bar_sync(BAR_PROD, NP);
-
-        /* ---- B: collision factors (S4), one thread per (face, side), two independent chains at a time ---- */
-        for (int item0 = pt; item0 < FH * 2; item0 += 2 * NP) {
-          double z[2], rho[2], erfz[2], ex[2], ir[2];
-          int at[2];
-          bool ok[2];
-#pragma unroll
-          for (int u = 0; u < 2; ++u) {
-            const int item = item0 + u * NP;
-            ok[u] = item < FH * 2;
-            const int it2 = ok[u] ? item : item0;
-            const int side = it2 & 1, fh = it2 >> 1;
-            const double *q = (side ? QRs : QLs) + fh * 4;
-            rho[u] = q[0];
-            z[u] = q[1 + DIR];
-            at[u] = fh * 4 + 2 * side;
-          }
-          gksd::fast_rcp_v<2>(rho, ir);
-#pragma unroll
-          for (int u = 0; u < 2; ++u) z[u] = ph.theta * (z[u] * ir[u]);
-          gksd::erf_expm2_v<2>(z, erfz, ex);
-#pragma unroll
-          for (int u = 0; u < 2; ++u) {
-            if (!ok[u]) continue;
-            const double h = (at[u] & 2) ? -0.5 : 0.5;   /* erfc(+z)/2 right, erfc(-z)/2 left */
-            CF[at[u]] = fma(h, erfz[u], 0.5);
-            CF[at[u] + 1] = rho[u] * (ph.cx * ex[u]);
-          }
-        }
-        bar_sync(BAR_PROD, NP);
-
-        /* the hand-over buffer (gi & 1) was last read by pass 1 of plane gi-2 */
-        if (gi >= 2) bar_sync(BAR_EMPTY0 + (gi & 1), NT);
-
-        /* ---- C: Q0 and Dn on the halo faces -> hand-over buffer ---- */
-        {
-          double *const Q0o = Qb + (gi & 1) * (2 * FH * 4);
-          double *const Dno = Q0o + FH * 4;
-#pragma unroll 2
-          for (int item = pt; item < FH * 4; item += NP) {
-            const int cc = item & 3, fh = item >> 2;
-            const int ha = fh % HA, hb = fh / HA;
-            const double el = CF[fh * 4], er = CF[fh * 4 + 2];
-            double q0 = QLs[item] * el + QRs[item] * er;
-            if (cc == 1 + DIR) q0 += CF[fh * 4 + 1] - CF[fh * 4 + 3];
-            /* normal slope from the 4 cells around the face; face nf sits between slab cells nf+2, nf+3 */
-            const int sa = T::NA ? ha + 3 : ha + 1, sb = T::NA ? hb : hb + 3;
-            const double *w = W + (cc * EB + sb) * EA + sa;
-            const int nf_glob = (T::NA ? s.a0 + ha : s.b0 + hb);
-            const double ihn = g.inv_hn[DIR][min(nf_glob, g.n[DIR]) + GKS_NG];
-            Q0o[item] = q0;
-            Dno[item] = gksd::normal_slope(w[-2 * sn], w[-sn], w[0], w[sn]) * ihn;
-          }
-        }
-        __threadfence_block();
-        bar_arrive(BAR_FULL0 + (gi & 1), NT);
-        bar_sync(BAR_PROD, NP);                        /* slab (gi & 1) and the staging arrays are free again */
-        if (pt == 0) issue_next();                     /* plane gi+2 (possibly of the next segment) */
-      }
-    }
-    return;
-  }
-
-  /* ======================= CONSUMER ======================= */
+  /* ---- static roles of this thread ---- */
+  /* D / EF: face fid, component c (A-D) or Gauss point c (F) */
   const int c = tid & 3, fid = tid >> 2;
   const int fa = fid % TA, fb = fid / TA;       /* a fastest: coalesced output */
   const int n_a = g.n[0] + (T::NA ? 1 : 0), n_b = g.n[T::AXB] + (T::NA ? 0 : 1);
   const int t1_local = T::NA ? fb : fa;
-  constexpr int s1 = T::NA ? HA : 1;                         /* halo-face stride along t1 */
+  constexpr int s1 = T::NA ? HA : 1;            /* halo-face stride along t1 */
   const int fh0 = T::NA ? (t1_local + 2) * HA + fa : fb * HA + (t1_local + 2);
   double *const rg = ring + fid * 4 + c;        /* this thread's private column of the ring */
   constexpr int RS = 6 * NF * 4, RF = NF * 4;   /* ring strides: plane slot, field */
@@ -343,38 +225,134 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, Tile<DIR, TA, TB>::CTAS
   int ro[4];
 #pragma unroll
   for (int cc = 0; cc < 4; ++cc) ro[cc] = 4 * (cc ^ (fid & 3)) + (c ^ cc);
+  constexpr int sn = T::NA ? 1 : EA;            /* slab stride along the normal */
+  constexpr int QLo = 0, QRo = FH * 4, DNo = 2 * FH * 4;   /* offsets inside a stage buffer */
 
-  int gi = 0;
-  for (long long l = L0; l < L1;) {
-    const Seg s = seg_at(l);
-    l += s.np - 4;
-    const int ga = s.a0 + fa, gb = s.b0 + fb;     /* global indices along a and b */
-    const bool face_ok = ga < n_a && gb < n_b;
-    const int t1_glob = T::NA ? gb : ga;
-    const double iw1 = g.inv_w[T::AXT1][min(t1_glob, g.n[T::AXT1] - 1) + GKS_NG];
-    for (int it = 0; it < s.np; ++it, ++gi) {
-      bar_sync(BAR_FULL0 + (gi & 1), NT);
-      /* ---- D: tangential pass 1 (along t1) on Q0 and Dn of plane it ---- */
-      double d6[6];
-      {
-        const double *q = Qb + (gi & 1) * (2 * FH * 4) + fh0 * 4 + c; /* Q0 */
-        const double *d = q + FH * 4;                                 /* Dn */
-        double qq[5][2], vm[2], vp[2], sm_[2], sp_[2];
-#pragma unroll
-        for (int k = 0; k < 5; ++k) {
-          qq[k][0] = q[(k - 2) * s1 * 4];
-          qq[k][1] = d[(k - 2) * s1 * 4];
+  for (int i = 0; i < J + 2; ++i) {
+    if (i > 0) mbar_wait(&bar[2], (i - 1) & 1);   /* every warp has finished A, BC, D of iteration i-1 */
+    if (i + 1 < J) {
+      if (tid == 0) issue(cT, i + 1);             /* slab (i+1)&1 was last read by stage A of iteration i-1 */
+      cur_next(cT);
+    }
+
+    /* ================= stage A: plane i =================
+     * both WENO5 edge values of each cell, per component (one smoothness-indicator set serves the face on
+     * either side), and the normal slope at the cell's right face; two cells at a time where a thread owns two */
+    if (i < J) {
+      const double *W = Wp + (i & 1) * T::WSLAB_PAD;
+      double *const S = Sb + (i % 3) * T::SBUF;
+      mbar_wait(&bar[i & 1], (i >> 1) & 1);
+      constexpr int NITEM = T::NCA * T::NCB * 4;
+      const int n0 = T::NA ? cA.s.a0 : cA.s.b0;   /* global index of normal face 0 of the tile */
+      auto locate = [&](int item, const double *&w, int &cn, int &ct, int &cc) {
+        cc = item & 3;
+        const int cell = item >> 2;
+        const int xa = cell % T::NCA, xb = cell / T::NCA;
+        const int sa = T::NA ? xa + 2 : xa + 1, sb = T::NA ? xb : xb + 2;
+        w = W + (cc * EB + sb) * EA + sa;
+        cn = T::NA ? xa : xb; /* cell along the normal: global f0-1+cn */
+        ct = T::NA ? xb : xa; /* halo index along t1 */
+      };
+      auto store = [&](int cn, int ct, int cc, double vl, double vr, double dn) {
+        if (cn >= 1) { /* left edge = face cn-1: Qr */
+          const int fh = T::NA ? ct * HA + (cn - 1) : (cn - 1) * HA + ct;
+          S[QRo + fh * 4 + cc] = vl;
         }
-        gksd::weno5_gauss_v<2>(qq, eps, vm, vp, sm_, sp_);
-        d6[0] = vm[0];
-        d6[1] = vp[0];
-        d6[2] = vm[1];
-        d6[3] = vp[1];
-        d6[4] = sm_[0] * iw1;
-        d6[5] = sp_[0] * iw1;
+        if (cn < TN) { /* right edge = face cn: Ql, and the slope at that face */
+          const int fh = T::NA ? ct * HA + cn : cn * HA + ct;
+          S[QLo + fh * 4 + cc] = vr;
+          S[DNo + fh * 4 + cc] = dn * g.inv_hn[DIR][min(n0 + cn, g.n[DIR]) + GKS_NG];
+        }
+      };
+      int item0 = tid;
+      for (; item0 + NT < NITEM; item0 += 2 * NT) {
+        double q[5][2], vl[2], vr[2];
+        int cnv[2], ctv[2], ccv[2];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+          const double *w;
+          locate(item0 + u * NT, w, cnv[u], ctv[u], ccv[u]);
+#pragma unroll
+          for (int k = 0; k < 5; ++k) q[k][u] = w[(k - 2) * sn];
+        }
+        gksd::weno5_edges_v<2>(q, eps, vl, vr);
+#pragma unroll
+        for (int u = 0; u < 2; ++u)
+          store(cnv[u], ctv[u], ccv[u], vl[u], vr[u], gksd::normal_slope(q[1][u], q[2][u], q[3][u], q[4][u]));
       }
-      /* the loaded values have been consumed: the hand-over buffer may be refilled (plane gi+2) */
-      if (gi + 2 < planes_total) bar_arrive(BAR_EMPTY0 + (gi & 1), NT);
+      if (item0 < NITEM) {
+        double q[5][1], vl[1], vr[1];
+        int cn, ct, cc;
+        const double *w;
+        locate(item0, w, cn, ct, cc);
+#pragma unroll
+        for (int k = 0; k < 5; ++k) q[k][0] = w[(k - 2) * sn];
+        gksd::weno5_edges_v<1>(q, eps, vl, vr);
+        store(cn, ct, cc, vl[0], vr[0], gksd::normal_slope(q[1][0], q[2][0], q[3][0], q[4][0]));
+      }
+      cur_next(cA);
+    }
+
+    /* ================= stage BC: plane i-1 =================
+     * collision (S4): the 4 lanes of a halo face split the two sides; lane (side = cc & 1) evaluates that
+     * side's half-Maxwellian factors, the group exchanges them by shuffle, every lane forms its component
+     * of Q0 in place of QL */
+    if (i >= 1 && i - 1 < J) {
+      double *const S = Sb + ((i - 1) % 3) * T::SBUF;
+      static_assert((FH * 4) % 32 == 0, "whole warps in the collision stage");
+      const int gl = (tid & 31) & ~3;               /* first lane of this face group */
+      for (int item = tid; item < FH * 4; item += NT) {
+        const int cc = item & 3, fh = item >> 2, side = cc & 1;
+        const double *qs = S + (side ? QRo : QLo) + fh * 4;
+        const double rho = qs[0];
+        const double z = ph.theta * (qs[1 + DIR] * gksd::fast_rcp(rho));
+        double erfz, ex;
+        gksd::erf_expm2_warp(z, erfz, ex);
+        const double e = fma(side ? -0.5 : 0.5, erfz, 0.5);   /* erfc(-z)/2 left, erfc(+z)/2 right */
+        const double x = rho * (ph.cx * ex);
+        const double el = __shfl_sync(0xffffffffu, e, gl), er = __shfl_sync(0xffffffffu, e, gl + 1);
+        const double xl = __shfl_sync(0xffffffffu, x, gl), xr = __shfl_sync(0xffffffffu, x, gl + 1);
+        double q0 = S[QLo + item] * el + S[QRo + item] * er;
+        if (cc == 1 + DIR) q0 += xl - xr;
+        S[QLo + item] = q0;
+      }
+    }
+
+    /* ================= stage D: plane i-2, tangential pass 1 (along t1) on Q0 and Dn ================= */
+    const bool have = i >= 2;
+    double d6[6];
+    int ga = 0, gb = 0;
+    if (have) {
+      ga = cD.s.a0 + fa;
+      gb = cD.s.b0 + fb;
+      const int t1_glob = T::NA ? gb : ga;
+      const double iw1 = g.inv_w[T::AXT1][min(t1_glob, g.n[T::AXT1] - 1) + GKS_NG];
+      const double *q = Sb + ((i - 2) % 3) * T::SBUF + QLo + fh0 * 4 + c; /* Q0 */
+      const double *d = q + DNo;                                          /* Dn */
+      double qq[5][2], vm[2], vp[2], sm_[2], sp_[2];
+#pragma unroll
+      for (int k = 0; k < 5; ++k) {
+        qq[k][0] = q[(k - 2) * s1 * 4];
+        qq[k][1] = d[(k - 2) * s1 * 4];
+      }
+      gksd::weno5_gauss_v<2>(qq, eps, vm, vp, sm_, sp_);
+      d6[0] = vm[0];
+      d6[1] = vp[0];
+      d6[2] = vm[1];
+      d6[3] = vp[1];
+      d6[4] = sm_[0] * iw1;
+      d6[5] = sp_[0] * iw1;
+    }
+    /* this warp is done with the shared stage buffers of iteration i */
+    __syncwarp();
+    if ((tid & 31) == 0) mbar_arrive(&bar[2]);
+    if (!have) continue;
+
+    /* ================= stage EF: plane i-2 ================= */
+    const int it = cD.it;
+    const int m = cD.s.p0 + it - 2;
+    const bool face_ok = ga < n_a && gb < n_b;
+    cur_next(cD);
 
     double *const rnew = rg + (it & 3) * RS;     /* slot of plane it-4, dead once pass 2 below has read it */
     if (it < 4) {
@@ -384,7 +362,6 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, Tile<DIR, TA, TB>::CTAS
     }
     /* ---- E: tangential pass 2 (along t2, the marched axis) for plane m = it-2; the ring holds planes
      *         it-4 .. it-1 (plane it-4+k in slot (it+k)&3), plane it comes straight from d6 ---- */
-    const int m = s.p0 + it - 2;
     const double iw2 = g.inv_w[T::AXM][m + GKS_NG];
     const double *rs[4];
 #pragma unroll
@@ -452,7 +429,6 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, Tile<DIR, TA, TB>::CTAS
       }
     }
   }
-  }
 }
 
 } /* namespace */
@@ -496,7 +472,7 @@ int launch_dir(gks_ctx *ctx, const CUtensorMap &map, double *flux) {
   /* persistent CTAs: the (column, plane) list is cut into equal contiguous ranges, one per resident CTA;
      a range shorter than 8 planes is not worth its 4 priming planes */
   const long long total = (long long)ga * gb * n2;
-  const long long slots = (long long)ctx->num_sms * T::CTAS_PER_SM;
+  const long long slots = (long long)ctx->num_sms;
   long long PPC = (total + slots - 1) / slots;
   if (PPC < 8) PPC = 8;
   const int nblk = (int)((total + PPC - 1) / PPC);
