@@ -26,7 +26,7 @@ namespace gksd {
  * operands (no per-use UMOV pairs).  Values with an all-zero low word (0.25, 0.5, 3.0, ...) are
  * written as literals: they encode as instruction immediates. */
 static __constant__ double GKC[16] = {
-    13.0 / 12.0,                                        /* 0  smoothness: (13/12) a^2 */
+    13.0 / 3.0,                                         /* 0  smoothness, scaled by 4: (13/3) a^2 + g^2 */
     ((210.0 - GKS_SQRT3) / 1080.0) / (11.0 / 18.0),     /* 1  Gauss-point linear weight dA / dB */
     ((210.0 + GKS_SQRT3) / 1080.0) / (11.0 / 18.0),     /* 2  Gauss-point linear weight dC / dB */
     GKS_SQRT3 / 12.0,                                   /* 3  h = x_G / 2, x_G = sqrt(3)/6 */
@@ -51,7 +51,7 @@ __device__ __forceinline__ double fast_rcp(double x) {
 /* Shared front end of every WENO5-JS evaluation, in difference form.  With D_m = q_m - q_{m-1}:
  *   second differences a_k (sub-stencil curvature), centred slopes g_k (twice the slope of sub-stencil k's
  *   quadratic at the centre of the middle cell; g0 = q0-4q1+3q2, g1 = q3-q1, g2 = -(3q2-4q3+q4)),
- *   Jiang-Shu beta_k = 13/12 a_k^2 + 1/4 g_k^2, and the common-denominator factors
+ *   Jiang-Shu beta_k = 13/12 a_k^2 + 1/4 g_k^2 (carried as 4 beta_k), and the common-denominator factors
  *   t0 = s1 s2, t1 = s0 s2, t2 = s0 s1 with s_k = (eps + beta_k)^2. */
 /* N independent stencils at once: every statement is replicated N times back to back so that the
  * instruction stream interleaves N dependency chains (the fp64 pipe needs the ILP at 16 warps/SM). */
@@ -62,7 +62,10 @@ struct JsFrontV {
 template <int N>
 __device__ __forceinline__ void js_front_v(const double (&D1)[N], const double (&D2)[N], const double (&D3)[N],
                                            const double (&D4)[N], double eps, JsFrontV<N> &f) {
+  /* s_k = 4 (eps + beta_k) = (13/3) a_k^2 + g_k^2 + 4 eps: the common factor 4 (exact in binary) cancels
+     in the weight ratios */
   const double k13 = GKC[0];
+  const double eps4 = 4.0 * eps;
   double s0[N], s1[N], s2[N];
 #pragma unroll
   for (int n = 0; n < N; ++n) {
@@ -78,15 +81,15 @@ __device__ __forceinline__ void js_front_v(const double (&D1)[N], const double (
   }
 #pragma unroll
   for (int n = 0; n < N; ++n) {
-    s0[n] = fma(k13 * f.a0[n], f.a0[n], eps);
-    s1[n] = fma(k13 * f.a1[n], f.a1[n], eps);
-    s2[n] = fma(k13 * f.a2[n], f.a2[n], eps);
+    s0[n] = fma(k13 * f.a0[n], f.a0[n], eps4);
+    s1[n] = fma(k13 * f.a1[n], f.a1[n], eps4);
+    s2[n] = fma(k13 * f.a2[n], f.a2[n], eps4);
   }
 #pragma unroll
   for (int n = 0; n < N; ++n) {
-    s0[n] = fma(0.25 * f.g0[n], f.g0[n], s0[n]);
-    s1[n] = fma(0.25 * f.g1[n], f.g1[n], s1[n]);
-    s2[n] = fma(0.25 * f.g2[n], f.g2[n], s2[n]);
+    s0[n] = fma(f.g0[n], f.g0[n], s0[n]);
+    s1[n] = fma(f.g1[n], f.g1[n], s1[n]);
+    s2[n] = fma(f.g2[n], f.g2[n], s2[n]);
   }
 #pragma unroll
   for (int n = 0; n < N; ++n) {
@@ -133,25 +136,31 @@ __device__ __forceinline__ void weno5_edges_v(const double (&q)[5][N], double ep
   JsFrontV<N> f;
   js_front_v<N>(D1, D2, D3, D4, eps, f);
   const double w6 = GKC[4], w12 = GKC[5];
-  double numr[N], numl[N], denr[N], denl[N], prod[N], inv[N];
+  double numr[N], numl[N], denr[N], denl[N], prod[N], r0[N];
 #pragma unroll
   for (int n = 0; n < N; ++n) {
-    const double ar0 = w6 * f.t0[n], ar2 = 0.5 * f.t2[n]; /* (.1,.6,.3)/.6 */
-    const double al0 = 0.5 * f.t0[n], al2 = w6 * f.t2[n]; /* (.3,.6,.1)/.6 */
-    const double P0 = fma(3.0, f.g0[n], f.a0[n]), P1 = fma(3.0, f.g1[n], f.a1[n]), P2 = fma(3.0, f.g2[n], f.a2[n]);
-    const double M0 = fma(-3.0, f.g0[n], f.a0[n]), M1 = fma(-3.0, f.g1[n], f.a1[n]), M2 = fma(-3.0, f.g2[n], f.a2[n]);
-    numr[n] = fma(ar2, P2, fma(f.t1[n], P1, ar0 * P0));
-    denr[n] = ar0 + f.t1[n] + ar2;
-    numl[n] = fma(al2, M2, fma(f.t1[n], M1, al0 * M0));
-    denl[n] = al0 + f.t1[n] + al2;
+    /* linear weights (.1,.6,.3)/.6 right, (.3,.6,.1)/.6 left; candidates 12 (p_k - q2) = a_k +- 3 g_k */
+    const double ug0 = f.t0[n] * f.g0[n], ug1 = f.t1[n] * f.g1[n], ug2 = f.t2[n] * f.g2[n];
+    const double ua0 = f.t0[n] * f.a0[n], ua1 = f.t1[n] * f.a1[n], ua2 = f.t2[n] * f.a2[n];
+    const double Gr = fma(w6, ug0, fma(0.5, ug2, ug1)), Ar = fma(w6, ua0, fma(0.5, ua2, ua1));
+    const double Gl = fma(0.5, ug0, fma(w6, ug2, ug1)), Al = fma(0.5, ua0, fma(w6, ua2, ua1));
+    numr[n] = fma(3.0, Gr, Ar);
+    numl[n] = fma(-3.0, Gl, Al);
+    denr[n] = fma(w6, f.t0[n], fma(0.5, f.t2[n], f.t1[n]));
+    denl[n] = fma(0.5, f.t0[n], fma(w6, f.t2[n], f.t1[n]));
     prod[n] = denr[n] * denl[n];
   }
-  fast_rcp_v<N>(prod, inv);
+#pragma unroll
+  for (int n = 0; n < N; ++n) asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r0[n]) : "d"(prod[n]));
 #pragma unroll
   for (int n = 0; n < N; ++n) {
-    const double iv = inv[n] * w12;
-    vr[n] = fma(numr[n] * denl[n], iv, q[2][n]);
-    vl[n] = fma(numl[n] * denr[n], iv, q[2][n]);
+    /* 1/prod = r0 (1 + e + e^2 + ...), e = 1 - prod r0 ~ 2^-23: the cubic truncation is below 2^-66 */
+    const double e = fma(-prod[n], r0[n], 1.0);
+    const double t = fma(e, e, e);
+    const double rw = r0[n] * w12;
+    const double yr = (numr[n] * denl[n]) * rw, yl = (numl[n] * denr[n]) * rw;
+    vr[n] = fma(yr, t, q[2][n] + yr);
+    vl[n] = fma(yl, t, q[2][n] + yl);
   }
 }
 
@@ -172,25 +181,28 @@ __device__ __forceinline__ void weno5_gauss_v(const double (&q)[5][N], double ep
   JsFrontV<N> f;
   js_front_v<N>(D1, D2, D3, D4, eps, f);
   const double dA = GKC[1], dC = GKC[2], h = GKC[3];
-  double nump[N], numm[N], denp[N], denm[N], prod[N], inv[N];
+  double nump[N], numm[N], denp[N], denm[N], prod[N], r0[N];
 #pragma unroll
   for (int n = 0; n < N; ++n) {
-    const double ap0 = dA * f.t0[n], ap2 = dC * f.t2[n];
-    const double am0 = dC * f.t0[n], am2 = dA * f.t2[n];
-    const double c1 = f.t1[n] * f.g1[n];
-    nump[n] = fma(ap2, f.g2[n], fma(ap0, f.g0[n], c1));
-    denp[n] = ap0 + f.t1[n] + ap2;
-    numm[n] = fma(am2, f.g2[n], fma(am0, f.g0[n], c1));
-    denm[n] = am0 + f.t1[n] + am2;
+    const double u0 = f.t0[n] * f.g0[n], u1 = f.t1[n] * f.g1[n], u2 = f.t2[n] * f.g2[n];
+    nump[n] = fma(dA, u0, fma(dC, u2, u1));
+    numm[n] = fma(dC, u0, fma(dA, u2, u1));
+    denp[n] = fma(dA, f.t0[n], fma(dC, f.t2[n], f.t1[n]));
+    denm[n] = fma(dC, f.t0[n], fma(dA, f.t2[n], f.t1[n]));
     prod[n] = denp[n] * denm[n];
   }
-  fast_rcp_v<N>(prod, inv);
+#pragma unroll
+  for (int n = 0; n < N; ++n) asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r0[n]) : "d"(prod[n]));
   const double e1 = GKC[6], e2 = GKC[7], e3 = GKC[8], e4 = GKC[9];
 #pragma unroll
   for (int n = 0; n < N; ++n) {
-    const double iv = inv[n] * h;
-    vp[n] = fma(nump[n] * denm[n], iv, q[2][n]);
-    vm[n] = fma(-(numm[n] * denp[n]), iv, q[2][n]);
+    /* 1/prod = r0 (1 + e + e^2 + ...), e = 1 - prod r0 ~ 2^-23: the cubic truncation is below 2^-66 */
+    const double e = fma(-prod[n], r0[n], 1.0);
+    const double t = fma(e, e, e);
+    const double rh = r0[n] * h;
+    const double yp = (nump[n] * denm[n]) * rh, ym = (numm[n] * denp[n]) * rh;
+    vp[n] = fma(yp, t, q[2][n] + yp);
+    vm[n] = fma(-ym, t, q[2][n] - ym);
     sp[n] = fma(e4, D4[n], fma(e3, D3[n], fma(e2, D2[n], e1 * D1[n])));
     sm[n] = fma(e1, D4[n], fma(e2, D3[n], fma(e3, D2[n], e4 * D1[n])));
   }

@@ -109,7 +109,7 @@ struct Tile {
   static constexpr int OFF_BAR = OFF_RING + RING;          /* mbarriers: 2 TMA + 1 iteration barrier */
   static constexpr size_t SMEM_BYTES = (size_t)(OFF_BAR + 4) * 8;
   static_assert(SMEM_BYTES + 1024 <= 233472, "the CTA must fit in shared memory");
-  static_assert(NT <= 1024 && NT % 32 == 0, "whole warps");
+  static_assert(NT <= 1024 && NT % 32 == 0 && (NT & (NT - 1)) == 0, "whole warps, power of two");
 };
 
 /* one contiguous run of marched planes of one tile column: output planes [mb, mb+len) */
@@ -264,14 +264,18 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
           S[DNo + fh * 4 + cc] = dn * g.inv_hn[DIR][min(n0 + cn, g.n[DIR]) + GKS_NG];
         }
       };
-      int item0 = tid;
-      for (; item0 + NT < NITEM; item0 += 2 * NT) {
+      /* every thread owns item tid; the NITEM - NT extra items go to a window of warps that rotates with
+         the iteration, so that no warp is systematically the slowest */
+      constexpr int NXA = NITEM - NT;
+      static_assert(NXA >= 0 && NXA <= NT / 2, "stage A: at most two items per thread, extras on half the CTA");
+      const int xa_id = (tid - 32 * ((i * 5) % T::NW)) & (NT - 1);
+      if (xa_id < NXA) {
         double q[5][2], vl[2], vr[2];
         int cnv[2], ctv[2], ccv[2];
 #pragma unroll
         for (int u = 0; u < 2; ++u) {
           const double *w;
-          locate(item0 + u * NT, w, cnv[u], ctv[u], ccv[u]);
+          locate(u ? NT + xa_id : tid, w, cnv[u], ctv[u], ccv[u]);
 #pragma unroll
           for (int k = 0; k < 5; ++k) q[k][u] = w[(k - 2) * sn];
         }
@@ -279,12 +283,11 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
 #pragma unroll
         for (int u = 0; u < 2; ++u)
           store(cnv[u], ctv[u], ccv[u], vl[u], vr[u], gksd::normal_slope(q[1][u], q[2][u], q[3][u], q[4][u]));
-      }
-      if (item0 < NITEM) {
+      } else {
         double q[5][1], vl[1], vr[1];
         int cn, ct, cc;
         const double *w;
-        locate(item0, w, cn, ct, cc);
+        locate(tid, w, cn, ct, cc);
 #pragma unroll
         for (int k = 0; k < 5; ++k) q[k][0] = w[(k - 2) * sn];
         gksd::weno5_edges_v<1>(q, eps, vl, vr);
@@ -301,7 +304,12 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
       double *const S = Sb + ((i - 1) % 3) * T::SBUF;
       static_assert((FH * 4) % 32 == 0, "whole warps in the collision stage");
       const int gl = (tid & 31) & ~3;               /* first lane of this face group */
-      for (int item = tid; item < FH * 4; item += NT) {
+      constexpr int NXB = FH * 4 - NT;              /* extra items: a rotating window of whole warps, disjoint from A's */
+      static_assert(NXB >= 0 && NXB <= NT / 4 && NXB % 32 == 0, "stage BC: extras on whole warps");
+      const int xb_id = (tid - 32 * ((i * 5 + T::NW / 2) % T::NW)) & (NT - 1);
+      const int nitem = xb_id < NXB ? 2 : 1;
+      for (int u = 0; u < nitem; ++u) {
+        const int item = u ? NT + xb_id : tid;
         const int cc = item & 3, fh = item >> 2, side = cc & 1;
         const double *qs = S + (side ? QRo : QLo) + fh * 4;
         const double rho = qs[0];
