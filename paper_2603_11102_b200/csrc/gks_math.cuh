@@ -48,6 +48,15 @@ __device__ __forceinline__ double fast_rcp(double x) {
   return fma(r, e, r);
 }
 
+/* reciprocal from the hardware seed r0 (2^-23) with one cubic correction: 1/x = r0 (1 + e + e^2 + O(e^3)),
+ * e = 1 - x r0; truncation below 2^-66, three dependent operations after the seed */
+__device__ __forceinline__ double fast_rcp3(double x) {
+  double r0;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r0) : "d"(x));
+  const double e = fma(-x, r0, 1.0);
+  return fma(r0, fma(e, e, e), r0);
+}
+
 /* Shared front end of every WENO5-JS evaluation, in difference form.  With D_m = q_m - q_{m-1}:
  *   second differences a_k (sub-stencil curvature), centred slopes g_k (twice the slope of sub-stencil k's
  *   quadratic at the centre of the middle cell; g0 = q0-4q1+3q2, g1 = q3-q1, g2 = -(3q2-4q3+q4)),
@@ -320,6 +329,22 @@ __device__ __forceinline__ void erf_expm2_warp(double z, double &erfz, double &e
   } else {
     erf_expm2(z, erfz, ex);
   }
+}
+
+/* one of the two functions per lane: func = 0 -> erf(z), func = 1 -> exp(-z^2); the lanes of a warp run the
+ * same Horner recurrence on their own coefficient set (series length chosen warp-uniformly as above) */
+__device__ __forceinline__ double erf_or_expm2_warp(double z, int func) {
+  const double w = z * z;
+  const bool small = !(w > 1.0 / 64.0);
+  if (__all_sync(0xffffffffu, small)) {
+    double p = func ? GK_EXP[7] : GK_ERF[7];
+#pragma unroll
+    for (int n = 6; n >= 0; --n) p = fma(p, w, func ? GK_EXP[n] : GK_ERF[n]);
+    return func ? p : p * z;
+  }
+  double erfz, ex;
+  erf_expm2(z, erfz, ex);
+  return func ? ex : erfz;
 }
 
 /* collision factors from the normal velocities of the left / right states (S4):

@@ -35,6 +35,10 @@
 #include "gks_internal.h"
 #include "gks_math.cuh"
 
+#ifndef GKS_E_WIDTH
+#define GKS_E_WIDTH 2
+#endif
+
 namespace {
 
 /* ---------------- PTX helpers: mbarrier + TMA ---------------- */
@@ -51,16 +55,17 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+  /* try_wait suspends the warp in hardware up to the time hint (ns) instead of spinning on issue slots */
   asm volatile(
       "{\n"
       ".reg .pred P1;\n"
       "WAIT_LOOP:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1, %2;\n"
       "@P1 bra DONE;\n"
       "bra WAIT_LOOP;\n"
       "DONE:\n"
       "}\n" ::"r"(smem_u32(bar)),
-      "r"(parity)
+      "r"(parity), "r"(0x989680)
       : "memory");
 }
 __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1, int c2,
@@ -297,9 +302,8 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
     }
 
     /* ================= stage BC: plane i-1 =================
-     * collision (S4): the 4 lanes of a halo face split the two sides; lane (side = cc & 1) evaluates that
-     * side's half-Maxwellian factors, the group exchanges them by shuffle, every lane forms its component
-     * of Q0 in place of QL */
+     * collision (S4): the 4 lanes of a halo face split the four half-Maxwellian factors (left / right side,
+     * erf / exp series), exchange them by shuffle, and every lane forms its component of Q0 in place of QL */
     if (i >= 1 && i - 1 < J) {
       double *const S = Sb + ((i - 1) % 3) * T::SBUF;
       static_assert((FH * 4) % 32 == 0, "whole warps in the collision stage");
@@ -310,16 +314,15 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
       const int nitem = xb_id < NXB ? 2 : 1;
       for (int u = 0; u < nitem; ++u) {
         const int item = u ? NT + xb_id : tid;
-        const int cc = item & 3, fh = item >> 2, side = cc & 1;
+        const int cc = item & 3, fh = item >> 2, side = cc & 1, func = cc >> 1;
         const double *qs = S + (side ? QRo : QLo) + fh * 4;
         const double rho = qs[0];
-        const double z = ph.theta * (qs[1 + DIR] * gksd::fast_rcp(rho));
-        double erfz, ex;
-        gksd::erf_expm2_warp(z, erfz, ex);
-        const double e = fma(side ? -0.5 : 0.5, erfz, 0.5);   /* erfc(-z)/2 left, erfc(+z)/2 right */
-        const double x = rho * (ph.cx * ex);
-        const double el = __shfl_sync(0xffffffffu, e, gl), er = __shfl_sync(0xffffffffu, e, gl + 1);
-        const double xl = __shfl_sync(0xffffffffu, x, gl), xr = __shfl_sync(0xffffffffu, x, gl + 1);
+        const double z = ph.theta * (qs[1 + DIR] * gksd::fast_rcp3(rho));
+        /* lane (side, func): func 0 -> erfc(-+z)/2 of that side, func 1 -> rho exp(-z^2) / (2 sqrt(pi lambda)) */
+        const double v = gksd::erf_or_expm2_warp(z, func);
+        const double r = func ? rho * (ph.cx * v) : fma(side ? -0.5 : 0.5, v, 0.5);
+        const double el = __shfl_sync(0xffffffffu, r, gl), er = __shfl_sync(0xffffffffu, r, gl + 1);
+        const double xl = __shfl_sync(0xffffffffu, r, gl + 2), xr = __shfl_sync(0xffffffffu, r, gl + 3);
         double q0 = S[QLo + item] * el + S[QRo + item] * er;
         if (cc == 1 + DIR) q0 += xl - xr;
         S[QLo + item] = q0;
@@ -374,26 +377,29 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
     const double *rs[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) rs[k] = rg + ((it + k) & 3) * RS;
+    /* the six evaluations (field Q0, Dn, Dt1) x (g1 = -, +) run EW at a time, statement-interleaved */
+    constexpr int EW = GKS_E_WIDTH;
+    static_assert(6 % EW == 0, "E width");
 #pragma unroll
-    for (int fld = 0; fld < 3; ++fld) { /* Q0, Dn, Dt1: the two g1 instances of a field go together */
-      double qq[5][2], vm[2], vp[2], sm_[2], sp_[2];
+    for (int e0 = 0; e0 < 6; e0 += EW) {
+      double qq[5][EW], vm[EW], vp[EW], sm_[EW], sp_[EW];
 #pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        qq[k][0] = rs[k][(2 * fld) * RF];
-        qq[k][1] = rs[k][(2 * fld + 1) * RF];
+      for (int u = 0; u < EW; ++u) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) qq[k][u] = rs[k][(e0 + u) * RF];
+        qq[4][u] = d6[e0 + u];
       }
-      qq[4][0] = d6[2 * fld];
-      qq[4][1] = d6[2 * fld + 1];
-      rnew[(2 * fld) * RF] = d6[2 * fld];          /* rs[0] aliases rnew: stored after the loads above */
-      rnew[(2 * fld + 1) * RF] = d6[2 * fld + 1];
-      gksd::weno5_gauss_v<2>(qq, eps, vm, vp, sm_, sp_);
 #pragma unroll
-      for (int g1 = 0; g1 < 2; ++g1) {            /* Gauss point gq = 2*g1 + g2 */
-        xw[fld * 16 + ((2 * g1) ^ c)] = vm[g1];
-        xw[fld * 16 + ((2 * g1 + 1) ^ c)] = vp[g1];
+      for (int u = 0; u < EW; ++u) rnew[(e0 + u) * RF] = d6[e0 + u];   /* rs[0] aliases rnew: stored after the loads */
+      gksd::weno5_gauss_v<EW>(qq, eps, vm, vp, sm_, sp_);
+#pragma unroll
+      for (int u = 0; u < EW; ++u) {              /* evaluation e = 2*fld + g1; Gauss point gq = 2*g1 + g2 */
+        const int fld = (e0 + u) >> 1, g1 = (e0 + u) & 1;
+        xw[fld * 16 + ((2 * g1) ^ c)] = vm[u];
+        xw[fld * 16 + ((2 * g1 + 1) ^ c)] = vp[u];
         if (fld == 0) {
-          xw[3 * 16 + ((2 * g1) ^ c)] = sm_[g1] * iw2;
-          xw[3 * 16 + ((2 * g1 + 1) ^ c)] = sp_[g1] * iw2;
+          xw[3 * 16 + ((2 * g1) ^ c)] = sm_[u] * iw2;
+          xw[3 * 16 + ((2 * g1 + 1) ^ c)] = sp_[u] * iw2;
         }
       }
     }
