@@ -226,6 +226,16 @@ gks_status gks_create(const gks_config *cfg, void *workspace, size_t workspace_b
     g.dx[a] = dx[a];
     g.periodic[a] = cfg->bc[2 * a] == GKS_BC_PERIODIC;
   }
+  /* On a periodic axis face n is face 0, cell for cell, unless another axis carries convective-outflow
+     ghosts: those are state on interior lines but zero-gradient on tangential-ghost lines (S20),
+     which breaks the identity.  Where it holds, the fused sweep stores n faces and readers wrap. */
+  for (int a = 0; a < 3; ++a) {
+    bool other_outflow = false;
+    for (int b = 0; b < 3; ++b)
+      if (b != a && (cfg->bc[2 * b] == GKS_BC_OUTFLOW_CONVECTIVE || cfg->bc[2 * b + 1] == GKS_BC_OUTFLOW_CONVECTIVE))
+        other_outflow = true;
+    g.wrapf[a] = g.periodic[a] && !other_outflow;
+  }
   g.st[0] = 1;
   g.st[1] = g.P[0];
   g.st[2] = (long long)g.P[0] * g.P[1];

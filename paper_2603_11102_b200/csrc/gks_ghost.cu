@@ -113,7 +113,9 @@ __global__ void __launch_bounds__(256) k_pack(GksGrid g, double *__restrict__ Wi
   const int k = blockIdx.z;
   const int nx = g.n[0] + ex, ny = g.n[1] + ey, nz = g.n[2] + ez;
   if (i >= nx || j >= ny || k >= nz) return;
-  const long long ip = g.idx(i, j, k);
+  /* face arrays: on a periodic axis face n is stored as face 0 */
+  const long long ip = g.idx((ex && g.wrapf[0] && i == g.n[0]) ? 0 : i, (ey && g.wrapf[1] && j == g.n[1]) ? 0 : j,
+                             (ez && g.wrapf[2] && k == g.n[2]) ? 0 : k);
   const long long ii = ((long long)k * ny + j) * nx + i;
   const long long N = (long long)nx * ny * nz;
 #pragma unroll

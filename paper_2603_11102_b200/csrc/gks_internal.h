@@ -32,6 +32,7 @@ struct GksGrid {
   int uniform[3];
   double x0[3], dx[3];
   int periodic[3];
+  int wrapf[3];      /* face n of this axis is not stored: it is face 0 (periodic axis, see gks_create) */
   __host__ __device__ long long idx(int i, int j, int k) const {
     return ((long long)(k + GKS_NG) * P[1] + (j + GKS_NG)) * P[0] + (i + GKS_NG);
   }

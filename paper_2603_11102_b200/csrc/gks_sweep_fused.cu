@@ -216,7 +216,8 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
   /* D / EF: face fid, component c (A-D) or Gauss point c (F) */
   const int c = tid & 3, fid = tid >> 2;
   const int fa = fid % TA, fb = fid / TA;       /* a fastest: coalesced output */
-  const int n_a = g.n[0] + (T::NA ? 1 : 0), n_b = g.n[T::AXB] + (T::NA ? 0 : 1);
+  /* faces to store: n+1 along the normal, n on a periodic axis (face n is face 0) */
+  const int n_a = g.n[0] + (T::NA && !g.wrapf[0] ? 1 : 0), n_b = g.n[T::AXB] + (!T::NA && !g.wrapf[T::AXB] ? 1 : 0);
   const int t1_local = T::NA ? fb : fa;
   constexpr int s1 = T::NA ? HA : 1;            /* halo-face stride along t1 */
   const int fh0 = T::NA ? (t1_local + 2) * HA + fa : fb * HA + (t1_local + 2);
@@ -481,7 +482,8 @@ int launch_dir(gks_ctx *ctx, const CUtensorMap &map, double *flux) {
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES);
     attr_done = true;
   }
-  const int ext_a = g.n[0] + (T::NA ? 1 : 0), ext_b = g.n[T::AXB] + (T::NA ? 0 : 1), n2 = g.n[T::AXM];
+  const int ext_a = g.n[0] + (T::NA && !g.wrapf[0] ? 1 : 0), ext_b = g.n[T::AXB] + (!T::NA && !g.wrapf[T::AXB] ? 1 : 0);
+  const int n2 = g.n[T::AXM];
   const int ga = (ext_a + TA - 1) / TA, gb = (ext_b + TB - 1) / TB;
   /* persistent CTAs: the (column, plane) list is cut into equal contiguous ranges, one per resident CTA;
      a range shorter than 8 planes is not worth its 4 priming planes */

@@ -22,13 +22,17 @@ __global__ void __launch_bounds__(256) k_update(GksGrid g, const double *__restr
   if (i >= g.n[0] || j >= g.n[1]) return;
   const long long id = g.idx(i, j, k);
   const double iwx = g.inv_w[0][i + GKS_NG], iwy = g.inv_w[1][j + GKS_NG], iwz = g.inv_w[2][k + GKS_NG];
-  const long long sy = g.st[1], sz = g.st[2];
+  /* upper face of the cell along each axis; where face n of an axis is face 0 (g.wrapf: periodic axis) the sweep
+     does not store it and the last cell reads face 0 */
+  const long long sx = (g.wrapf[0] && i == g.n[0] - 1) ? -(long long)(g.n[0] - 1) : 1;
+  const long long sy = (g.wrapf[1] && j == g.n[1] - 1) ? -(long long)(g.n[1] - 1) * g.st[1] : g.st[1];
+  const long long sz = (g.wrapf[2] && k == g.n[2] - 1) ? -(long long)(g.n[2] - 1) * g.st[2] : g.st[2];
 #pragma unroll
   for (int c = 0; c < 4; ++c) {
     const long long o = c * g.FS + id, od = (4 + c) * g.FS + id;
-    const double dL = -((fx[od + 1] - fx[od]) * iwx + (fy[od + sy] - fy[od]) * iwy + (fz[od + sz] - fz[od]) * iwz);
+    const double dL = -((fx[od + sx] - fx[od]) * iwx + (fy[od + sy] - fy[od]) * iwy + (fz[od + sz] - fz[od]) * iwz);
     if (STAGE1) {
-      const double L = -((fx[o + 1] - fx[o]) * iwx + (fy[o + sy] - fy[o]) * iwy + (fz[o + sz] - fz[o]) * iwz);
+      const double L = -((fx[o + sx] - fx[o]) * iwx + (fy[o + sy] - fy[o]) * iwy + (fz[o + sz] - fz[o]) * iwz);
       const double w = Win[o];
       out1[o] = w + 0.5 * dt * L + (dt * dt / 8.0) * dL;
       out2[o] = w + dt * L + (dt * dt / 6.0) * dL;
