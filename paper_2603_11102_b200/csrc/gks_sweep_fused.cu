@@ -124,8 +124,11 @@ struct Seg {
 
 /*
  * Persistent, symmetric and software-pipelined.  The work of one launch is the list of (tile column,
- * marched plane) pairs in column-major order; CTA b owns the contiguous range [b*PPC, (b+1)*PPC) of it,
- * i.e. a few column segments (each costs 4 priming planes), so that all CTAs finish together.
+ * marched plane) pairs.  With G CTAs and C columns, every CTA first marches floor(C/G) whole columns
+ * (CTA b: columns b, b+G, ...: neighbouring columns move through the same planes together, so the halo
+ * of a slab is read from L2, not from HBM); the planes of the remaining C mod G columns are cut into G
+ * equal contiguous ranges (a few column segments per CTA, each costs 4 priming planes), so that all
+ * CTAs finish together.
  *
  * Every warp runs the same program.  Iteration i works on three different staged planes at once:
  *     stage A  on plane i    : normal WENO edge values QL, QR and the normal slope Dn      -> S[i % 3]
@@ -140,7 +143,7 @@ struct Seg {
 template <int DIR, bool NEED_F, int TA, int TB>
 __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
     k_sweep_fused(const __grid_constant__ CUtensorMap tmap, GksGrid g, GksPhys ph, double *__restrict__ flux,
-                  int ncol_a, long long total, long long PPC) {
+                  int ncol_a, int nfull, long long rem, long long PPC) {
   using T = Tile<DIR, TA, TB>;
   constexpr int TN = T::TN, NF = T::NF, NT = T::NT, EA = T::EA, EB = T::EB, HA = T::HA, FH = T::FH;
   extern __shared__ __align__(128) double sm[];
@@ -153,14 +156,30 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
   const int tid = threadIdx.x;
   const int n2 = g.n[T::AXM];
   const double eps = ph.weno_eps;
-  long long L0 = (long long)blockIdx.x * PPC, L1 = L0 + PPC;
-  if (L0 > total) L0 = total;
-  if (L1 > total) L1 = total;
+  /* This CTA's plane list, addressed by a private index v in [0, L1):
+   *   v <  nfull*n2 : whole columns blockIdx.x + gridDim.x*w, w = v / n2 - all CTAs march neighbouring
+   *                   columns through the same planes at the same time (halo slabs are shared in L2);
+   *   v >= nfull*n2 : this CTA's share [r0, r1) of the planes of the remaining columns, column-major. */
+  const long long full = (long long)nfull * n2;
+  const long long r0 = (long long)blockIdx.x * PPC < rem ? (long long)blockIdx.x * PPC : rem;
+  const long long r1 = r0 + PPC < rem ? r0 + PPC : rem;
+  const long long L0 = 0, L1 = full + (r1 - r0);
   if (L0 >= L1) return;
-  auto seg_at = [&](long long l) {
-    const int col = (int)(l / n2), mb = (int)(l - (long long)col * n2);
-    const long long left = L1 - l;
-    const int len = (int)(left < (long long)(n2 - mb) ? left : (long long)(n2 - mb));
+  auto seg_at = [&](long long v) {
+    int col, mb, len;
+    if (v < full) {
+      const int w = (int)(v / n2);
+      col = (int)blockIdx.x + (int)gridDim.x * w;
+      mb = (int)(v - (long long)w * n2);
+      len = n2 - mb;
+    } else {
+      const long long r = r0 + (v - full);
+      const int cr = (int)(r / n2);
+      col = nfull * (int)gridDim.x + cr;
+      mb = (int)(r - (long long)cr * n2);
+      const long long left = r1 - r;
+      len = (int)(left < (long long)(n2 - mb) ? left : (long long)(n2 - mb));
+    }
     Seg s;
     s.a0 = (col % ncol_a) * TA;
     s.b0 = (col / ncol_a) * TB;
@@ -487,12 +506,13 @@ int launch_dir(gks_ctx *ctx, const CUtensorMap &map, double *flux) {
   const int ga = (ext_a + TA - 1) / TA, gb = (ext_b + TB - 1) / TB;
   /* persistent CTAs: the (column, plane) list is cut into equal contiguous ranges, one per resident CTA;
      a range shorter than 8 planes is not worth its 4 priming planes */
-  const long long total = (long long)ga * gb * n2;
-  const long long slots = (long long)ctx->num_sms;
-  long long PPC = (total + slots - 1) / slots;
-  if (PPC < 8) PPC = 8;
-  const int nblk = (int)((total + PPC - 1) / PPC);
-  kern<<<nblk, T::NT, T::SMEM_BYTES, ctx->stream>>>(map, g, ctx->ph, flux, ga, total, PPC);
+  const int ncols = ga * gb;
+  int grid = ctx->num_sms, nfull = ncols / grid;
+  long long rem = (long long)(ncols - nfull * grid) * n2;      /* planes of the columns that do not fill a wave */
+  long long PPC = (rem + grid - 1) / grid;
+  if (PPC < 8) PPC = 8;                                        /* a range shorter than 8 planes is not worth its priming */
+  if (nfull == 0) grid = (int)((rem + PPC - 1) / PPC);
+  kern<<<grid, T::NT, T::SMEM_BYTES, ctx->stream>>>(map, g, ctx->ph, flux, ga, nfull, rem, PPC);
   return 1;
 }
 
