@@ -1,0 +1,155 @@
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (persistent fused sweeps,
+one CTA per SM, whole-column waves + split remainder), north_star tolerance 1e-11 after one step.
+
+The oracle cannot run 256^3 ... 512x256x256 in seconds, so it computes SAMPLED outputs one sub-box at a time:
+one S2O4 step has a finite domain of dependence (3 cells per stage and axis: normal stencil -3..+2, the two
+tangential passes +-2 each; two stages -> 6 cells; IBM interpolation + spreading add 3), so the oracle run
+on a sub-box cut out of the same initial state, with any boundary condition on the cut faces, reproduces
+the cells further than MARGIN = 10 cells from every cut face exactly.  Sub-box faces that coincide with a
+non-periodic domain face keep the domain's boundary condition (margin 0 there); periodic axes wrap.
+The small full configurations (C2, C3) are compared cell for cell over the whole grid."""
+import numpy as np
+import pytest
+
+from conftest import rel_linf
+from paper_2603_11102_b200 import workloads as wl
+from paper_2603_11102_b200.workloads import GridConfig
+
+pytestmark = pytest.mark.gpu
+
+TOL1 = 1e-11
+MARGIN = 10
+EX = wl.BC_EXTRAPOLATE
+
+
+def oracle_step_on_subbox(w, lo, size, steps=1):
+    """Oracle result on the sub-box [lo, lo+size) of workload w and the slices of its trusted core."""
+    from oracle import binding as ob
+    cfg = w.cfg
+    assert all(f is None for f in cfg.faces), "sub-boxes are cut from uniform grids"
+    n = (cfg.n[0], cfg.n[1], cfg.n[2])
+    bc = list(cfg.bc)
+    sub_bc, core = [], []
+    for a in range(3):
+        periodic = bc[2 * a] == wl.BC_PERIODIC
+        if not periodic:
+            assert 0 <= lo[a] and lo[a] + size[a] <= n[a]
+        at_lo = (not periodic) and lo[a] == 0
+        at_hi = (not periodic) and lo[a] + size[a] == n[a]
+        sub_bc += [bc[2 * a] if at_lo else EX, bc[2 * a + 1] if at_hi else EX]
+        core.append(slice(0 if at_lo else MARGIN, size[a] if at_hi else size[a] - MARGIN))
+    idx = [np.arange(lo[a], lo[a] + size[a]) % n[a] for a in range(3)]
+    W0 = w.W0[:, idx[2]][:, :, idx[1]][:, :, :, idx[0]].copy()
+    origin = tuple(cfg.origin[a] + lo[a] * cfg.spacing[a] for a in range(3))
+    sub = GridConfig(n=tuple(size), origin=origin, spacing=cfg.spacing, RT=cfg.RT, nu=cfg.nu, rho_ref=cfg.rho_ref,
+                     bc=tuple(sub_bc), inflow=cfg.inflow, weno_eps=cfg.weno_eps)
+    o = ob.Oracle(sub)
+    seen = {"ibm": 0, "alm": 0}
+    hi = [origin[a] + size[a] * cfg.spacing[a] for a in range(3)]
+    if w.ibm is not None:
+        pos, vol = w.ibm
+        inside = np.all([(pos[:, a] > origin[a]) & (pos[:, a] < hi[a]) for a in range(3)], axis=0)
+        # a point whose 3-point support is cut by a sub-box face is only seen by cells outside the core
+        o.ibm_set_points(pos[inside], vol[inside])
+        seen["ibm"] = int(inside.sum())
+    o.set_state(W0)
+    for s in range(steps):
+        if w.alm is not None:
+            pos, force, eps = w.alm(s)
+            near = np.all([(pos[:, a] > origin[a] - 3.5 * eps) & (pos[:, a] < hi[a] + 3.5 * eps) for a in range(3)], axis=0)
+            o.alm_set_points(pos[near], force[near], eps)
+            seen["alm"] = int(near.sum())
+        o.step(w.dt)
+    W = o.get_state()
+    o.close()
+    return W, idx, (core[2], core[1], core[0]), seen
+
+
+def check_samples(w, Wg, boxes, size=(28, 28, 28), need=()):
+    """need: per box, the forcing kinds ('alm', 'ibm') that must act inside the sub-box (the sample is then a
+    test of that forcing, not only of the fluid step)"""
+    scale_rho = np.abs(Wg[0]).max()
+    scale_m = np.sqrt((Wg[1:] ** 2).sum(0)).max()
+    worst = 0.0
+    for b, lo in enumerate(boxes):
+        Wo, idx, core, seen = oracle_step_on_subbox(w, lo, size)
+        for kind in (need[b] if b < len(need) else ()):
+            assert seen[kind] > 0, (w.name, lo, kind)
+        G = Wg[:, idx[2]][:, :, idx[1]][:, :, :, idx[0]]
+        d = np.abs(G - Wo)[(slice(None),) + core]
+        assert d.size > 0
+        err = max(d[0].max() / scale_rho, d[1:].max() / scale_m)   # norm S24 with the full field's scales
+        worst = max(worst, err)
+        assert err <= TOL1, (w.name, lo, err)
+    return worst
+
+
+def box_around(w, x, size=28):
+    """sub-box origin that puts the physical point x at the centre of the trusted core"""
+    lo = []
+    for a in range(3):
+        i = int(np.floor((x[a] - w.cfg.origin[a]) / w.cfg.spacing[a])) - size // 2
+        if w.cfg.bc[2 * a] != wl.BC_PERIODIC:
+            i = min(max(i, 0), w.cfg.n[a] - size)
+        lo.append(i)
+    return tuple(lo)
+
+
+def test_M0_metric_box_256_sampled():
+    """the box bench.py times: 256^3 periodic Taylor-Green; sub-boxes in the interior, across the periodic
+    seam of every axis, in the remainder columns of the persistent schedule and at tile corners"""
+    from paper_2603_11102_b200 import gks
+    w = wl.by_name("M0")
+    Wg = gks.run_workload(w, steps=1)
+    boxes = [(100, 117, 3), (-14, -14, -14), (242, 5, 120), (57, 240, 243), (120, 120, 120), (7, 250, 64)]
+    check_samples(w, Wg, boxes)
+    # properties that hold at any size: conservation on the periodic box (P7) and finiteness
+    mscale = float(np.abs(w.W0[1:]).sum(dtype=np.longdouble))
+    for c in range(4):
+        s0, s1 = w.W0[c].sum(dtype=np.longdouble), Wg[c].sum(dtype=np.longdouble)
+        ref = abs(float(s0)) if c == 0 else 1e-3 * mscale
+        assert abs(float(s1 - s0)) <= 1e-12 * ref, (c, float(s1 - s0), ref)
+    assert np.isfinite(Wg).all()
+
+
+@pytest.mark.parametrize("name", ["C2", "C3"])
+def test_full_channel_and_cylinder_cell_for_cell(name):
+    """C2 128x96x64 (stretched walls, bulk-flux forcing) and C3 256x128x64 (IBM cylinder, inflow / convective
+    outflow): the oracle runs the whole grid"""
+    from oracle import binding as ob
+    from paper_2603_11102_b200 import gks
+    w = wl.by_name(name)
+    Wg = gks.run_workload(w, steps=1)
+    o = ob.Oracle(w.cfg)
+    if w.bulk_flux is not None:
+        o.set_bulk_flux(*w.bulk_flux)
+    if w.ibm is not None:
+        o.ibm_set_points(*w.ibm)
+    o.set_state(w.W0)
+    o.step(w.dt)
+    err = rel_linf(Wg, o.get_state())
+    o.close()
+    assert err <= TOL1, err
+
+
+def test_C4_rotor_384x192x192_sampled():
+    """ALM rotor: sub-boxes through the rotor disc (hub, blade tips), at the inflow face, on the slip wall,
+    across the periodic y seam and at the convective outflow"""
+    from paper_2603_11102_b200 import gks
+    w = wl.by_name("C4")
+    Wg = gks.run_workload(w, steps=1)
+    pos = w.alm(0)[0]                        # 3 blades x 64 points, root to tip
+    boxes = [box_around(w, pos[0]), box_around(w, pos[63]), box_around(w, pos[64 + 63]), (0, 90, 90), (200, 96, 0),
+             (150, -14, 80), (356, 80, 80), (356, 164, 164)]
+    check_samples(w, Wg, boxes, need=[("alm",), ("alm",), ("alm",)])
+
+
+def test_C5_turbine_512x256x256_sampled():
+    """ALM rotor + IBM nacelle and tower: sub-boxes at the hub / nacelle, along the tower, at the tower foot
+    on the ground (slip wall), in the wake, at inflow and outflow"""
+    from paper_2603_11102_b200 import gks
+    w = wl.by_name("C5")
+    Wg = gks.run_workload(w, steps=1)
+    boxes = [(116, 114, 86), (124, 114, 40), (122, 114, 0), (116, 114, 120), (300, 100, 100), (0, 120, 90),
+             (484, 120, 90), (250, -14, 228)]
+    check_samples(w, Wg, boxes, need=[("alm", "ibm"), ("ibm",), ("ibm",), ("alm",)])
