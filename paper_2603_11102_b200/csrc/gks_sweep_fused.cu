@@ -436,28 +436,34 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
       }
       gksd::gauss_point_flux<DIR, NEED_F>(Q0, dQ, ph.RT, ph.mu, F, dF);
       __syncwarp();                               /* every lane has consumed its reads: the buffer is reusable */
+      /* face average: the 4 lanes of a face (one Gauss point each) leave their F, dF in the warp-private
+         buffer, lane c sums component c in the order (g0+g1)+(g2+g3).  Row v of face fid sits at
+         ((v ^ (fid&3)) * 4 + gp), faces of a pair are offset by 2 doubles: conflict-free stores, 128-bit loads */
+      double *const xs = XBuf + fid * 64 + 2 * (fid & 1);
+      const int f3 = fid & 3;
 #pragma unroll
-      for (int cc = 0; cc < 4; ++cc) {
-        if (NEED_F) {
-          F[cc] += __shfl_xor_sync(0xffffffffu, F[cc], 1);
-          F[cc] += __shfl_xor_sync(0xffffffffu, F[cc], 2);
-        }
-        dF[cc] += __shfl_xor_sync(0xffffffffu, dF[cc], 1);
-        dF[cc] += __shfl_xor_sync(0xffffffffu, dF[cc], 2);
+      for (int v = 0; v < 4; ++v) {
+        if (NEED_F) xs[(v ^ f3) * 4 + c] = F[v];
+        xs[16 + (v ^ f3) * 4 + c] = dF[v];
       }
+      __syncwarp();
+      double fsel = 0.0, dsel;
+      {
+        const double2 *r = reinterpret_cast<const double2 *>(xs + (c ^ f3) * 4);
+        if (NEED_F) {
+          const double2 u0 = r[0], u1 = r[1];
+          fsel = (u0.x + u0.y) + (u1.x + u1.y);
+        }
+        const double2 w0 = r[8], w1 = r[9];
+        dsel = (w0.x + w0.y) + (w1.x + w1.y);
+      }
+      __syncwarp();                               /* pass 2 of the next plane writes the buffer again */
       if (face_ok) {
         int pidx[3];
         pidx[0] = ga;
         pidx[T::AXB] = gb;
         pidx[T::AXM] = m;
         const long long id = g.idx(pidx[0], pidx[1], pidx[2]);
-        double fsel = 0.0, dsel = 0.0;
-#pragma unroll
-        for (int cc = 0; cc < 4; ++cc)
-          if (cc == c) {
-            if (NEED_F) fsel = F[cc];
-            dsel = dF[cc];
-          }
         if (NEED_F) flux[c * g.FS + id] = 0.25 * fsel;
         flux[(4 + c) * g.FS + id] = 0.25 * dsel;
       }
