@@ -49,6 +49,7 @@ def lib():
         L.gkso_alm_set_cut.argtypes = [vp, C.c_double]
         L.gkso_ibm_set_points.argtypes = [vp, C.c_int, _dp, _dp]
         L.gkso_ibm_set_velocities.argtypes = [vp, _dp]
+        L.gkso_ibm_set_iterations.argtypes = [vp, C.c_int, C.c_double]
         L.gkso_eval_flux.argtypes = [vp, C.c_int, _dp, _dp]
         L.gkso_eval_L.argtypes = [vp, _dp, _dp]
         L.gkso_get_padded.argtypes = [vp, _dp]
@@ -164,6 +165,9 @@ class Oracle:
         pos, weights = _arr(pos).reshape(-1, 3), _arr(weights).reshape(-1)
         _check(lib().gkso_ibm_set_points(self._h, len(pos), _p(pos), _p(weights)))
         self.n_ibm = len(pos)
+
+    def ibm_set_iterations(self, max_iter, tol=0.0):
+        _check(lib().gkso_ibm_set_iterations(self._h, int(max_iter), float(tol)))
 
     def ibm_set_velocities(self, vel):
         if vel is None:

@@ -333,6 +333,8 @@ struct gkso_ctx {
   double alm_eps = 0, alm_cut = 3.0;
   int n_ibm = 0;
   std::vector<double> ibm_pos, ibm_vol, ibm_vel;
+  int ibm_maxit = 1;       /* multi-direct-forcing passes per step; 1 = single pass (S15) */
+  double ibm_tol = 0.0;    /* stop once max_p |v_p - U_p| < tol (checked from the second pass on) */
 
   int P(int a) const { return n[a] + 2 * NG; }
   size_t ncell_p() const { return (size_t)P(0) * P(1) * P(2); }
@@ -646,24 +648,40 @@ void eval_forcing(const gkso_ctx &s, const std::vector<double> &Wp, double dt, s
         for (int i = 0; i < s.n[0]; ++i) at(s.bulk_axis, i, j, k) += delta;
   }
 
-  /* IBM (S13-S15): U_p by interpolation; spread rho_ijk (v_p - U_p) phi phi phi V_p/|Omega_ijk| */
+  /* IBM (S13-S15, S25): pass s interpolates U_p^s from the un-forced field plus the increments of the passes
+     before it (Eq. 11), spreads rho_ijk (v_p - U_p^s) phi phi phi V_p/|Omega_ijk|, and the increments add up
+     (Eq. 12).  From the second pass on the iteration stops once max_p |v_p - U_p^s| < tol. */
   if (s.n_ibm > 0) {
-    std::vector<double> Up;
-    ibm_interpolate(s, Wp, Up);
-    for (int p = 0; p < s.n_ibm; ++p) {
-      Support3 sp;
-      ibm_support(s, &s.ibm_pos[3 * p], sp);
-      for (int mk = 0; mk < 3; ++mk)
-        for (int mj = 0; mj < 3; ++mj)
-          for (int mi = 0; mi < 3; ++mi) {
-            const int i = sp.idx[0][mi], j = sp.idx[1][mj], k = sp.idx[2][mk];
-            if (i < 0 || j < 0 || k < 0) continue;
-            const double wgt = sp.phi[0][mi] * sp.phi[1][mj] * sp.phi[2][mk];
-            const double vol = s.ax[0].w(i) * s.ax[1].w(j) * s.ax[2].w(k);
-            const double rho = Wp[s.id(0, i, j, k)];
-            for (int c = 0; c < 3; ++c)
-              at(c, i, j, k) += rho * (s.ibm_vel[3 * p + c] - Up[3 * p + c]) * wgt * s.ibm_vol[p] / vol;
-          }
+    std::vector<double> Wit(Wp), Up;
+    for (int pass = 0; pass < s.ibm_maxit; ++pass) {
+      ibm_interpolate(s, Wit, Up);
+      if (pass > 0) {
+        double res = 0.0;
+        for (int p = 0; p < s.n_ibm; ++p) {
+          double r2 = 0.0;
+          for (int c = 0; c < 3; ++c) r2 += (s.ibm_vel[3 * p + c] - Up[3 * p + c]) * (s.ibm_vel[3 * p + c] - Up[3 * p + c]);
+          res = std::max(res, std::sqrt(r2));
+        }
+        if (res < s.ibm_tol) break;
+      }
+      for (int p = 0; p < s.n_ibm; ++p) {
+        Support3 sp;
+        ibm_support(s, &s.ibm_pos[3 * p], sp);
+        for (int mk = 0; mk < 3; ++mk)
+          for (int mj = 0; mj < 3; ++mj)
+            for (int mi = 0; mi < 3; ++mi) {
+              const int i = sp.idx[0][mi], j = sp.idx[1][mj], k = sp.idx[2][mk];
+              if (i < 0 || j < 0 || k < 0) continue;
+              const double wgt = sp.phi[0][mi] * sp.phi[1][mj] * sp.phi[2][mk];
+              const double vol = s.ax[0].w(i) * s.ax[1].w(j) * s.ax[2].w(k);
+              const double rho = Wp[s.id(0, i, j, k)];
+              for (int c = 0; c < 3; ++c) {
+                const double inc = rho * (s.ibm_vel[3 * p + c] - Up[3 * p + c]) * wgt * s.ibm_vol[p] / vol;
+                at(c, i, j, k) += inc;
+                Wit[s.id(1 + c, i, j, k)] += inc;
+              }
+            }
+      }
     }
   }
 
@@ -914,6 +932,14 @@ int gkso_ibm_set_points(gkso_ctx *s, int n, const double *pos, const double *wei
   s->ibm_pos.assign(pos, pos + 3 * (size_t)n);
   s->ibm_vol.assign(weights, weights + (size_t)n);
   s->ibm_vel.assign(3 * (size_t)n, 0.0);
+  return 0;
+}
+
+int gkso_ibm_set_iterations(gkso_ctx *s, int max_iter, double tol) {
+  if (!s) return fail("null argument");
+  if (max_iter < 1 || !(tol >= 0.0)) return fail("ibm: max_iter must be >= 1 and tol >= 0");
+  s->ibm_maxit = max_iter;
+  s->ibm_tol = tol;
   return 0;
 }
 

@@ -44,6 +44,8 @@ int gkso_alm_set_points(gkso_ctx *ctx, int n, const double *pos, const double *f
 int gkso_alm_set_cut(gkso_ctx *ctx, double cut_in_eps); /* test flag: radius of the cut in units of eps (default 3; <=0 => no cut) */
 int gkso_ibm_set_points(gkso_ctx *ctx, int n, const double *pos, const double *weights);
 int gkso_ibm_set_velocities(gkso_ctx *ctx, const double *vel);
+/* multi-direct-forcing passes per step (Eq. 11-12; S25); default 1, tol 0 */
+int gkso_ibm_set_iterations(gkso_ctx *ctx, int max_iter, double tol);
 /* face-averaged F and dF/dt of the current state, direction dir; F[c][k][j][i] with n_dir+1 faces along dir */
 int gkso_eval_flux(gkso_ctx *ctx, int dir, double *F, double *dFdt);
 /* L and dL/dt (Eq. 5) of the current state, interior cells, [c][k][j][i] */

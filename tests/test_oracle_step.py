@@ -269,6 +269,68 @@ def test_P12_ibm_reads_the_unforced_field_and_rejects_outside_points():
     o.close()
 
 
+# ---------------------------------------------------------------- P15 IBM multi-direct-forcing passes (S25)
+def test_P15_isolated_point_contracts_by_one_minus_Vp_over_8h3_per_pass():
+    """One Lagrangian point in a uniform fluid: the spread increment interpolated back at the point is
+    (v - U) (V_p/h^3) (sum phi^2)^3 = (v - U) V_p/(8 h^3) (P12: sum phi^2 = 1/2 per axis), so every pass
+    multiplies the slip velocity by q = 1 - V_p/(8 h^3) and the impulse after S passes is the geometric sum
+    rho V_p (v - U_0) (1 - q^S)/(1 - q) (Eq. 12).  V_p = 8 h^3 removes the slip in ONE pass."""
+    n, h = (10, 10, 10), 0.2
+    cfg = GridConfig(n=n, spacing=(h, h, h), bc=(EX,) * 6)
+    rho, U0 = 1.3, np.array([0.1, -0.05, 0.02])
+    X = np.array([[1.03, 0.97, 1.11]])
+    v = np.array([[0.02, 0.01, -0.03]])
+    for Vp, S in [(h ** 3, 1), (h ** 3, 4), (2.5 * h ** 3, 3), (8 * h ** 3, 2)]:
+        o = ob.Oracle(cfg)
+        o.set_state(const_state(n, (rho, *(rho * U0))))
+        o.ibm_set_points(X, np.array([Vp]))
+        o.ibm_set_velocities(v)
+        o.ibm_set_iterations(S)
+        dM = o.eval_forcing(0.1)
+        q = 1.0 - Vp / (8 * h ** 3)
+        gsum = S if q == 1.0 else (1 - q ** S) / (1 - q)
+        impulse = dM.reshape(3, -1).sum(1) * h ** 3
+        assert np.allclose(impulse, rho * Vp * (v[0] - U0) * gsum, rtol=1e-12, atol=1e-18)
+        # slip after the S passes: apply the increment and interpolate again
+        W = const_state(n, (rho, *(rho * U0)))
+        W[1:] += dM
+        o.set_state(W)
+        slip = v[0] - o.ibm_interpolate()[0]
+        assert np.allclose(slip, (v[0] - U0) * q ** S, rtol=1e-11, atol=1e-17)
+        o.close()
+
+
+def test_P15_passes_reduce_the_slip_stop_at_the_tolerance_and_default_to_one():
+    cfg, pos, vol = ibm_case()
+    rng = np.random.default_rng(11)
+    W0 = const_state(cfg.n, (1.0, 0.1, 0.02, -0.03)) * (1 + 0.02 * rng.standard_normal((4, 8, 10, 12)))
+
+    def slip_after(max_iter, tol=0.0):
+        o = ob.Oracle(cfg)
+        o.set_state(W0)
+        o.ibm_set_points(pos, vol)
+        if max_iter is not None:
+            o.ibm_set_iterations(max_iter, tol)
+        dM = o.eval_forcing(0.05)
+        W = W0.copy()
+        W[1:] += dM
+        o.set_state(W)
+        r = np.linalg.norm(o.ibm_interpolate(), axis=1).max()      # v_p = 0
+        o.close()
+        return r, dM
+
+    r = [slip_after(k)[0] for k in (1, 2, 4, 8)]
+    assert r[0] > r[1] > r[2] > r[3] and r[3] < 0.5 * r[0]
+    assert np.array_equal(slip_after(None)[1], slip_after(1)[1])           # default = one pass (S15)
+    # tolerance: the slip before pass k is r[k-1]; with tol between r after 2 and after 1 pass exactly 2 passes run
+    r1, r2 = slip_after(1)[0], slip_after(2)[0]
+    tol = 0.5 * (r1 + r2)
+    assert np.array_equal(slip_after(50, tol)[1], slip_after(2)[1])
+    assert np.array_equal(slip_after(50, 10 * r1)[1], slip_after(1)[1])    # the first pass always runs
+    with pytest.raises(ob.OracleError):
+        ob.Oracle(cfg).ibm_set_iterations(0)
+
+
 # ---------------------------------------------------------------- bulk flux (S16) and body force
 def test_bulk_flux_restores_target_and_body_force_adds_rho_g_dt():
     w = wl.channel((8, 12, 6))
