@@ -115,6 +115,13 @@ gks_status alm_set_points(gks_ctx *ctx, int n, const double *pos, const double *
 gks_status ibm_set_points(gks_ctx *ctx, int n, const double *pos, const double *weights);
 gks_status ibm_set_velocities(gks_ctx *ctx, const double *vel /* n*3, or NULL => 0 */);
 
+/* IBM multi-direct-forcing passes per step (Eq. 11-12; S25): pass s interpolates
+ * U_p^s from the un-forced field plus the IBM increments of the passes before it and spreads
+ * rho_ijk (v_p - U_p^s) phi phi phi V_p/|Omega_ijk|; the increments add up (Eq. 12).  From the second pass
+ * on the passes stop once max_p |v_p - U_p^s| < tol (decided on the device: gks_step stays asynchronous).
+ * Default max_iter = 1, tol = 0 (single pass).  1 <= max_iter <= 64, tol >= 0, else GKS_ERR_INVALID_ARG. */
+gks_status ibm_set_iterations(gks_ctx *ctx, int max_iter, double tol);
+
 /* Test hook: fill ghosts of the CURRENT state and evaluate the face-averaged flux F and its
  * time derivative dF/dt (Eq. 6-7) for sweep direction dir in {0,1,2}.  Output (host or device):
  * 4 * (faces) doubles each, faces laid out like cells but with n_dir+1 entries along `dir`,

@@ -197,6 +197,7 @@ gks_status gks_create(const gks_config *cfg, void *workspace, size_t workspace_b
   ctx->cfg.xf = ctx->cfg.yf = ctx->cfg.zf = nullptr; /* caller pointers are not retained */
   ctx->stream = (cudaStream_t)cuda_stream;
   ctx->bulk_axis = -1;
+  ctx->ibm_maxit = 1;
   char *base = (char *)workspace;
   ctx->Wn = (double *)(base + L.off_Wn);
   ctx->Ws = (double *)(base + L.off_Ws);

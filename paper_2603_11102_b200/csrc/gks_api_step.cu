@@ -107,13 +107,22 @@ gks_status gks_step(gks_ctx *ctx, double dt) {
   /* forcing (Eq. 13), every increment from the un-forced field: read-only kernels first */
   const bool uniform = ctx->gacc[0] != 0.0 || ctx->gacc[1] != 0.0 || ctx->gacc[2] != 0.0;
   if (ctx->bulk_axis >= 0) ctx->launches += gks_launch_bulk_reduce(g, ctx->Wn, ctx->bulk_axis, ctx->red, s);
-  if (ctx->n_ibm > 0)
-    ctx->launches += gks_launch_ibm_interp(g, ctx->Wn, ctx->n_ibm, ctx->ibm_pos, ctx->ibm_vol, ctx->ibm_vel,
-                                           ctx->ibm_coef, s);
+  if (ctx->n_ibm > 0) {
+    /* multi-direct-forcing passes (Eq. 11-12): pass k interpolates from the un-forced field plus the IBM
+       increments of the passes before it, in place; nothing else has touched the momentum yet (S12) */
+    unsigned long long *res = reinterpret_cast<unsigned long long *>(ctx->red + GKS_RED_IBM_RES);
+    if (ctx->ibm_maxit > 1)
+      CUDA_TRY(ctx, cudaMemsetAsync(res, 0, GKS_IBM_MAX_PASSES * sizeof(unsigned long long), s));
+    for (int pass = 0; pass < ctx->ibm_maxit; ++pass) {
+      ctx->launches += gks_launch_ibm_interp(g, ctx->Wn, ctx->n_ibm, ctx->ibm_pos, ctx->ibm_vol, ctx->ibm_vel,
+                                             ctx->ibm_coef, pass, ctx->ibm_tol, res, s);
+      ctx->launches += gks_launch_ibm_spread(g, ctx->Wn, ctx->n_ibm, ctx->ibm_pos, ctx->ibm_coef, pass, ctx->ibm_tol,
+                                             res, s);
+    }
+  }
   if (uniform || ctx->bulk_axis >= 0)
     ctx->launches += gks_launch_uniform_force(g, ctx->Wn, dt, ctx->gacc, ctx->bulk_axis, ctx->bulk_target,
                                               ctx->total_volume, ctx->red, s);
-  if (ctx->n_ibm > 0) ctx->launches += gks_launch_ibm_spread(g, ctx->Wn, ctx->n_ibm, ctx->ibm_pos, ctx->ibm_coef, s);
   if (ctx->n_alm > 0)
     ctx->launches += gks_launch_alm(g, ctx->Wn, ctx->n_alm, ctx->alm_pos, ctx->alm_force, ctx->alm_eps, dt,
                                     ctx->alm_lo, ctx->alm_cnt, s);
@@ -230,6 +239,15 @@ gks_status ibm_set_points(gks_ctx *ctx, int n, const double *pos, const double *
   CUDA_TRY(ctx, cudaMemsetAsync(ctx->ibm_vel, 0, 3 * (size_t)n * sizeof(double), ctx->stream));
   CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
   ctx->n_ibm = n;
+  return GKS_OK;
+}
+
+gks_status ibm_set_iterations(gks_ctx *ctx, int max_iter, double tol) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (max_iter < 1 || max_iter > GKS_IBM_MAX_PASSES || !(tol >= 0.0) || !std::isfinite(tol))
+    return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "ibm: max_iter must be in 1..%d and tol finite and >= 0", GKS_IBM_MAX_PASSES);
+  ctx->ibm_maxit = max_iter;
+  ctx->ibm_tol = tol;
   return GKS_OK;
 }
 

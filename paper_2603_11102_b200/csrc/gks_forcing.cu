@@ -108,12 +108,23 @@ __device__ __forceinline__ void ibm_support(const GksGrid &g, const double *X, S
   }
 }
 
+/* Stop rule of the multi-direct-forcing passes (S25), evaluated on the device so
+ * that gks_step stays asynchronous: res[k] holds max_p |v_p - U_p| seen by pass k >= 1 as the bit pattern of
+ * a non-negative double (ordered like an unsigned integer), zeroed at the start of every step.  Pass k is
+ * skipped when pass k or any earlier pass found a slip below tol; a skipped pass leaves res[k] = 0 < tol,
+ * which carries the decision forward. */
+__device__ __forceinline__ bool ibm_below_tol(const unsigned long long *res, int k, double tol) {
+  return __longlong_as_double((long long)res[k]) < tol;
+}
+
 /* U_p = sum phi phi phi (m/rho);  coef_p = (v_p - U_p) V_p */
 __global__ void __launch_bounds__(128) k_ibm_interp(GksGrid g, const double *__restrict__ W, int n,
                                                     const double *__restrict__ pos, const double *__restrict__ vol,
-                                                    const double *__restrict__ vel, double *__restrict__ coef) {
+                                                    const double *__restrict__ vel, double *__restrict__ coef,
+                                                    int pass, double tol, unsigned long long *__restrict__ res) {
   const int p = blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= n) return;
+  if (pass >= 2 && ibm_below_tol(res, pass - 1, tol)) return;
   const double X[3] = {pos[3 * p], pos[3 * p + 1], pos[3 * p + 2]};
   Support sp;
   ibm_support(g, X, sp);
@@ -129,16 +140,24 @@ __global__ void __launch_bounds__(128) k_ibm_interp(GksGrid g, const double *__r
 #pragma unroll
         for (int c = 0; c < 3; ++c) U[c] += wgt * (W[(1 + c) * g.FS + id] * ir);
       }
+  double r2 = 0.0;
 #pragma unroll
-  for (int c = 0; c < 3; ++c) coef[3 * p + c] = (vel[3 * p + c] - U[c]) * vol[p];
+  for (int c = 0; c < 3; ++c) {
+    const double d = vel[3 * p + c] - U[c];
+    r2 += d * d;
+    coef[3 * p + c] = d * vol[p];
+  }
+  if (pass >= 1) atomicMax(&res[pass], (unsigned long long)__double_as_longlong(sqrt(r2)));
 }
 
 /* one thread per (point, support cell): m_ijk += rho_ijk coef_p phi phi phi / |Omega_ijk| */
 __global__ void __launch_bounds__(128) k_ibm_spread(GksGrid g, double *__restrict__ W, int n,
-                                                    const double *__restrict__ pos, const double *__restrict__ coef) {
+                                                    const double *__restrict__ pos, const double *__restrict__ coef,
+                                                    int pass, double tol, const unsigned long long *__restrict__ res) {
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const int p = (int)(t / 27);
   if (p >= n) return;
+  if (pass >= 1 && ibm_below_tol(res, pass, tol)) return;
   const int m = (int)(t % 27), mi = m % 3, mj = (m / 3) % 3, mk = m / 9;
   const double X[3] = {pos[3 * p], pos[3 * p + 1], pos[3 * p + 2]};
   Support sp;
@@ -233,15 +252,16 @@ int gks_launch_uniform_force(const GksGrid &g, double *W, double dt, const doubl
 }
 
 int gks_launch_ibm_interp(const GksGrid &g, const double *W, int n, const double *pos, const double *vol,
-                          const double *vel, double *coef, cudaStream_t s) {
-  k_ibm_interp<<<(n + 127) / 128, 128, 0, s>>>(g, W, n, pos, vol, vel, coef);
+                          const double *vel, double *coef, int pass, double tol, unsigned long long *res,
+                          cudaStream_t s) {
+  k_ibm_interp<<<(n + 127) / 128, 128, 0, s>>>(g, W, n, pos, vol, vel, coef, pass, tol, res);
   return 1;
 }
 
-int gks_launch_ibm_spread(const GksGrid &g, double *W, int n, const double *pos, const double *coef,
-                          cudaStream_t s) {
+int gks_launch_ibm_spread(const GksGrid &g, double *W, int n, const double *pos, const double *coef, int pass,
+                          double tol, const unsigned long long *res, cudaStream_t s) {
   const long long t = (long long)n * 27;
-  k_ibm_spread<<<(unsigned)((t + 127) / 128), 128, 0, s>>>(g, W, n, pos, coef);
+  k_ibm_spread<<<(unsigned)((t + 127) / 128), 128, 0, s>>>(g, W, n, pos, coef, pass, tol, res);
   return 1;
 }
 

@@ -76,6 +76,8 @@ struct gks_ctx {
   double alm_eps;
   int alm_lo[3], alm_cnt[3];   /* bounding box of the ALM support in (unwrapped) cell indices */
   int n_ibm;
+  int ibm_maxit;               /* multi-direct-forcing passes per step (1 = single pass) */
+  double ibm_tol;              /* stop once max_p |v_p - U_p| < tol, from the second pass on */
 
   /* TMA tensor maps of the two state buffers (Wn, Ws) for the three sweep directions (opaque CUtensorMap) */
   alignas(64) unsigned char tmaps[2][3][128];
@@ -86,6 +88,8 @@ struct gks_ctx {
   cudaEvent_t *prof_ev;        /* 2 * GKS_PROF_MAX events, created on first enable */
   int *prof_cat;
 };
+#define GKS_IBM_MAX_PASSES 64
+#define GKS_RED_IBM_RES 1600   /* ctx->red + this: GKS_IBM_MAX_PASSES residual slots (bit patterns) */
 #define GKS_PROF_MAX 4096
 void gks_prof_begin(gks_ctx *ctx, int cat);
 void gks_prof_end(gks_ctx *ctx);
@@ -121,9 +125,10 @@ int gks_launch_bulk_reduce(const GksGrid &g, const double *W, int axis, double *
 int gks_launch_uniform_force(const GksGrid &g, double *W, double dt, const double gacc[3], int bulk_axis,
                              double bulk_target, double total_volume, const double *red, cudaStream_t s);
 int gks_launch_ibm_interp(const GksGrid &g, const double *W, int n, const double *pos, const double *vol,
-                          const double *vel, double *coef, cudaStream_t s);
-int gks_launch_ibm_spread(const GksGrid &g, double *W, int n, const double *pos, const double *coef,
+                          const double *vel, double *coef, int pass, double tol, unsigned long long *res,
                           cudaStream_t s);
+int gks_launch_ibm_spread(const GksGrid &g, double *W, int n, const double *pos, const double *coef, int pass,
+                          double tol, const unsigned long long *res, cudaStream_t s);
 int gks_launch_alm(const GksGrid &g, double *W, int n, const double *pos, const double *force, double eps,
                    double dt, const int lo[3], const int cnt[3], cudaStream_t s);
 int gks_launch_check_finite(const GksGrid &g, const double *W, int *flag, cudaStream_t s);

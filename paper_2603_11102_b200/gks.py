@@ -18,7 +18,7 @@ STATUS = {0: "GKS_OK", 1: "GKS_ERR_INVALID_ARG", 2: "GKS_ERR_WORKSPACE", 3: "GKS
           4: "GKS_ERR_STATE", 5: "GKS_ERR_NONFINITE"}
 
 EXPORTS = ["gks_workspace_bytes", "gks_create", "gks_destroy", "gks_set_state", "gks_get_state", "gks_step",
-           "gks_set_body_force", "gks_set_bulk_flux", "alm_set_points", "ibm_set_points", "ibm_set_velocities",
+           "gks_set_body_force", "gks_set_bulk_flux", "alm_set_points", "ibm_set_points", "ibm_set_velocities", "ibm_set_iterations",
            "gks_debug_eval_flux", "gks_debug_set_sweep", "gks_debug_fp64_peak",
            "gks_profile_enable", "gks_profile_read", "gks_check_finite", "gks_launch_count", "gks_last_error"]
 
@@ -59,6 +59,7 @@ def lib():
         L.alm_set_points.argtypes = [vp, C.c_int, vp, vp, C.c_double]
         L.ibm_set_points.argtypes = [vp, C.c_int, vp, vp]
         L.ibm_set_velocities.argtypes = [vp, vp]
+        L.ibm_set_iterations.argtypes = [vp, C.c_int, C.c_double]
         L.gks_debug_eval_flux.argtypes = [vp, C.c_int, vp, vp]
         L.gks_debug_set_sweep.argtypes = [vp, C.c_int]
         L.gks_check_finite.argtypes = [vp]
@@ -195,6 +196,9 @@ class Gks:
         pw, k2 = _ptr(weights)
         self._check(lib().ibm_set_points(self._h, n, pp, pw))
         self.n_ibm = n
+
+    def ibm_set_iterations(self, max_iter, tol=0.0):
+        self._check(lib().ibm_set_iterations(self._h, int(max_iter), float(tol)))
 
     def ibm_set_velocities(self, vel):
         pv, k = _ptr(vel)

@@ -144,3 +144,61 @@ def test_error_paths_on_the_device():
     with pytest.raises(gks.GksError):
         g.ibm_set_points(np.array([[-0.5, 0.1, 0.1]]), np.array([1.0]))  # outside the domain
     g.close()
+
+
+@pytest.mark.parametrize("passes,tol", [(3, 0.0), (8, 0.0), (20, None)])
+def test_ibm_multi_direct_forcing_passes(passes, tol):
+    """IBM passes (Eq. 11-12, S25) on the small cylinder and turbine cases: a fixed number of passes, and the
+    device-side stop rule with a tolerance that the oracle reaches after a few passes (tol = None: chosen from
+    the oracle's own slip history so that the stop falls strictly inside the allowed passes)"""
+    from oracle import binding as ob
+    from paper_2603_11102_b200 import gks
+    for name in ("C3", "C5"):
+        w = wl.by_name(name, small=True)
+        t = tol
+        if t is None:
+            # slip seen by pass k of the first step = max |U_p| after k passes (v_p = 0)
+            slips = []
+            for k in (2, 3, 4):
+                o = ob.Oracle(w.cfg)
+                o.ibm_set_points(*w.ibm)
+                o.ibm_set_iterations(k)
+                o.set_state(w.W0)
+                if w.alm is not None:
+                    o.alm_set_points(np.zeros((0, 3)), np.zeros((0, 3)), 1.0)
+                o.step(w.dt)
+                slips.append(np.linalg.norm(o.ibm_interpolate(), axis=1).max())
+                o.close()
+            t = 0.5 * (slips[0] + slips[1])        # between the slip after 2 and after 3 passes
+        o = ob.Oracle(w.cfg)
+        g = gks.Gks(w.cfg)
+        for s in (o, g):
+            s.ibm_set_points(*w.ibm)
+            s.ibm_set_iterations(passes, t)
+            s.set_state(w.W0)
+        for step in range(3):
+            if w.alm is not None:
+                o.alm_set_points(*w.alm(step))
+                g.alm_set_points(*w.alm(step))
+            o.step(w.dt)
+            g.step(w.dt)
+        e = rel_linf(g.get_state(), o.get_state())
+        assert e <= 3 * TOL1, (name, e)
+        # the passes did something: the result differs from the single-pass one
+        g1 = gks.Gks(w.cfg)
+        g1.ibm_set_points(*w.ibm)
+        g1.set_state(w.W0)
+        for step in range(3):
+            if w.alm is not None:
+                g1.alm_set_points(*w.alm(step))
+            g1.step(w.dt)
+        assert rel_linf(g1.get_state(), o.get_state()) > 1e-8
+        g1.close()
+        g.close()
+        o.close()
+    gg = gks.Gks(wl.by_name("C3", small=True).cfg)
+    with pytest.raises(gks.GksError):
+        gg.ibm_set_iterations(0)
+    with pytest.raises(gks.GksError):
+        gg.ibm_set_iterations(65)
+    gg.close()
