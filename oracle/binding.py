@@ -55,6 +55,7 @@ def lib():
         L.gkso_get_padded.argtypes = [vp, _dp]
         L.gkso_eval_forcing.argtypes = [vp, C.c_double, _dp]
         L.gkso_ibm_interpolate.argtypes = [vp, _dp]
+        L.gkso_cfl_dt.argtypes = [vp, C.c_double, _dp]
         L.gkso_last_error.restype = C.c_char_p
         L.gkso_moments.argtypes = [C.c_double, C.c_double, C.c_int, _dp]
         L.gkso_moments.restype = None
@@ -202,6 +203,11 @@ class Oracle:
         dM = np.empty((3, nz, ny, nx))
         _check(lib().gkso_eval_forcing(self._h, float(dt), _p(dM)))
         return dM
+
+    def cfl_dt(self, cfl):
+        out = np.zeros(1)
+        _check(lib().gkso_cfl_dt(self._h, float(cfl), _p(out)))
+        return float(out[0])
 
     def ibm_interpolate(self):
         Up = np.empty((self.n_ibm, 3))

@@ -990,6 +990,26 @@ int gkso_eval_forcing(gkso_ctx *s, double dt, double *dM) {
   return 0;
 }
 
+/* Time step of the CFL condition: dt = CFL min{dx, dy, dz} / (|U|_max + C), C = sqrt(1/(2 lambda))
+ * = sqrt(RT); |U|_max over the interior cells of the current state, the minimum over every cell width. */
+int gkso_cfl_dt(gkso_ctx *s, double cfl, double *dt) {
+  if (!s || !dt) return fail("bad argument");
+  if (!s->have_state) return fail("no state set");
+  if (!(cfl > 0.0)) return fail("cfl must be > 0");
+  double umax = 0.0, dmin = 1e300;
+  for (int k = 0; k < s->n[2]; ++k)
+    for (int j = 0; j < s->n[1]; ++j)
+      for (int i = 0; i < s->n[0]; ++i) {
+        const double rho = s->W[s->id(0, i, j, k)];
+        const double mx = s->W[s->id(1, i, j, k)], my = s->W[s->id(2, i, j, k)], mz = s->W[s->id(3, i, j, k)];
+        umax = std::max(umax, std::sqrt(mx * mx + my * my + mz * mz) / rho);
+      }
+  for (int a = 0; a < 3; ++a)
+    for (int i = 0; i < s->n[a]; ++i) dmin = std::min(dmin, s->ax[a].w(i));
+  *dt = cfl * dmin / (umax + std::sqrt(s->RT));
+  return 0;
+}
+
 int gkso_ibm_interpolate(gkso_ctx *s, double *Up) {
   if (!s || !Up) return fail("bad argument");
   if (!s->have_state) return fail("no state set");

@@ -56,6 +56,8 @@ int gkso_get_padded(gkso_ctx *ctx, double *Wp);
 int gkso_eval_forcing(gkso_ctx *ctx, double dt, double *dM);
 /* interpolated fluid velocity at the IBM points (n*3) for the current state */
 int gkso_ibm_interpolate(gkso_ctx *ctx, double *Up);
+/* dt of the CFL condition */
+int gkso_cfl_dt(gkso_ctx *ctx, double cfl, double *dt);
 const char *gkso_last_error(void);
 
 /* ---- building blocks, exported so that tests can pin each one separately ---- */

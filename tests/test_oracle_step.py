@@ -380,3 +380,34 @@ def test_P14_axis_permutation_commutes_up_to_the_pass_order():
     W_b = run(w.cfg, permute_axes(w.W0), w.dt, 1)
     diff = np.abs(W_a - W_b).max()
     assert diff < 1e-6                       # only S9 (order of the tangential WENO passes) differs: O(h^5)
+
+
+# ---------------------------------------------------------------- P16 CFL time step
+def test_P16_cfl_dt_closed_forms_and_invariants():
+    """dt = CFL min(dx,dy,dz)/(|U|max + sqrt(RT)): numbers worked by hand on a uniform state, the global minimum
+    width on a stretched axis, the largest speed wherever it sits, linear in CFL, Galilean shift of |U|max"""
+    n = (6, 7, 8)
+    yf = np.array([0.0, 0.3, 0.5, 0.62, 0.7, 0.9, 1.3, 1.8])            # smallest width 0.08
+    cfg = GridConfig(n=n, faces=(None, yf, None), spacing=(0.25, 1.0, 0.1), RT=0.64, bc=(EX,) * 6)
+    o = ob.Oracle(cfg)
+    W = const_state(n, (2.0, 2.0 * 0.3, 2.0 * -0.4, 0.0))               # |U| = 0.5, c = 0.8
+    o.set_state(W)
+    assert o.cfl_dt(0.4) == pytest.approx(0.4 * 0.08 / (0.5 + 0.8), rel=1e-15)
+    assert o.cfl_dt(0.8) == pytest.approx(2 * o.cfl_dt(0.4), rel=1e-15)
+    W[:, 5, 3, 2] = (0.5, 0.0, 0.0, 0.5 * 1.2)                          # one fast cell: |U| = 1.2
+    o.set_state(W)
+    assert o.cfl_dt(0.4) == pytest.approx(0.4 * 0.08 / (1.2 + 0.8), rel=1e-15)
+    o.close()
+    cfg2 = GridConfig(n=n, spacing=(0.25, 0.2, 0.05), RT=1.0, bc=(EX,) * 6)   # uniform grid: dz is the smallest
+    o = ob.Oracle(cfg2)
+    o.set_state(const_state(n, (1.0, 0.0, 0.0, 0.0)))
+    assert o.cfl_dt(1.0) == pytest.approx(0.05, rel=1e-15)             # fluid at rest: dt = dz / c_s
+    with pytest.raises(ob.OracleError):
+        o.cfl_dt(0.0)
+    o.close()
+    # the input recipe's dt (workloads.cfl_dt, numpy) is the same number
+    w = wl.by_name("C2", small=True)
+    o = ob.Oracle(w.cfg)
+    o.set_state(w.W0)
+    assert o.cfl_dt(0.4) == pytest.approx(w.dt, rel=1e-14)
+    o.close()
