@@ -122,6 +122,12 @@ gks_status ibm_set_velocities(gks_ctx *ctx, const double *vel /* n*3, or NULL =>
  * Default max_iter = 1, tol = 0 (single pass).  1 <= max_iter <= 64, tol >= 0, else GKS_ERR_INVALID_ARG. */
 gks_status ibm_set_iterations(gks_ctx *ctx, int max_iter, double tol);
 
+/* Time step of the CFL condition: dt = cfl * min{dx, dy, dz} / (|U|_max + sqrt(RT)), |U|_max over
+ * the interior cells of the current state (one reduction kernel), the minimum over every cell width.
+ * `dt` may be a host pointer (the call then synchronises the stream) or a device pointer (asynchronous).
+ * cfl <= 0 -> GKS_ERR_INVALID_ARG; before gks_set_state -> GKS_ERR_STATE. */
+gks_status gks_cfl_dt(gks_ctx *ctx, double cfl, double *dt);
+
 /* Test hook: fill ghosts of the CURRENT state and evaluate the face-averaged flux F and its
  * time derivative dF/dt (Eq. 6-7) for sweep direction dir in {0,1,2}.  Output (host or device):
  * 4 * (faces) doubles each, faces laid out like cells but with n_dir+1 entries along `dir`,

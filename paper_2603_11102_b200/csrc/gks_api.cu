@@ -245,6 +245,7 @@ gks_status gks_create(const gks_config *cfg, void *workspace, size_t workspace_b
   std::vector<double> tab(L.coords_doubles, 0.0);
   size_t o = 0;
   double vol[3];
+  ctx->dmin = 1e300;
   for (int a = 0; a < 3; ++a) {
     const size_t len = (size_t)n[a] + 8;
     double *xf = &tab[o], *xc = &tab[o + len], *w = &tab[o + 2 * len], *iw = &tab[o + 3 * len],
@@ -262,6 +263,8 @@ gks_status gks_create(const gks_config *cfg, void *workspace, size_t workspace_b
     ctx->h_w[a] = ctx->h_xf[a] + 2 * len;
     memcpy(ctx->h_xf[a], xf, 3 * len * sizeof(double));
     vol[a] = xf[GKS_NG + n[a]] - xf[GKS_NG];
+    for (int i = 0; i < n[a]; ++i)
+      if (w[GKS_NG + i] < ctx->dmin) ctx->dmin = w[GKS_NG + i];
     o += 5 * len;
   }
   ctx->total_volume = vol[0] * vol[1] * vol[2];

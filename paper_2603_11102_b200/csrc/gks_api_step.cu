@@ -292,6 +292,24 @@ gks_status gks_debug_eval_flux(gks_ctx *ctx, int dir, double *F, double *dFdt) {
   return GKS_OK;
 }
 
+gks_status gks_cfl_dt(gks_ctx *ctx, double cfl, double *dt) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (!dt) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "dt is NULL");
+  if (!(cfl > 0) || !std::isfinite(cfl)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "cfl must be > 0");
+  if (!ctx->have_state) return gks_set_err(ctx, GKS_ERR_STATE, "gks_cfl_dt before gks_set_state");
+  double *scr = ctx->red + GKS_RED_CFL;
+  CUDA_TRY(ctx, cudaMemsetAsync(scr, 0, 2 * sizeof(double), ctx->stream));
+  ctx->launches += gks_launch_cfl_dt(ctx->g, ctx->Wn, cfl, ctx->dmin, sqrt(ctx->ph.RT), scr, ctx->stream);
+  CUDA_TRY(ctx, cudaGetLastError());
+  if (gks_is_device_ptr(dt)) {
+    CUDA_TRY(ctx, cudaMemcpyAsync(dt, scr + 1, sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
+  } else {
+    CUDA_TRY(ctx, cudaMemcpyAsync(dt, scr + 1, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+  }
+  return GKS_OK;
+}
+
 gks_status gks_debug_set_sweep(gks_ctx *ctx, int mode) {
   if (!ctx) return GKS_ERR_INVALID_ARG;
   if (mode != 0 && mode != 1) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "mode must be 0 or 1");

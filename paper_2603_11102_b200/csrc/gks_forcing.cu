@@ -51,6 +51,34 @@ __global__ void __launch_bounds__(256) k_bulk_final(double *__restrict__ red) {
   if (threadIdx.x == 0) red[RED_BLOCKS] = sh[0];
 }
 
+/* ---- CFL time step: |U|_max over the interior, then dt = CFL dmin / (|U|_max + sqrt(RT)) ---- */
+__global__ void __launch_bounds__(256) k_umax(GksGrid g, const double *__restrict__ W, unsigned long long *__restrict__ out) {
+  __shared__ double sh[256];
+  const long long N = (long long)g.n[0] * g.n[1] * g.n[2];
+  double acc = 0.0;
+  for (long long t = (long long)blockIdx.x * 256 + threadIdx.x; t < N; t += (long long)gridDim.x * 256) {
+    const int i = (int)(t % g.n[0]);
+    const int j = (int)((t / g.n[0]) % g.n[1]);
+    const int k = (int)(t / ((long long)g.n[0] * g.n[1]));
+    const long long id = g.idx(i, j, k);
+    const double mx = W[g.FS + id], my = W[2 * g.FS + id], mz = W[3 * g.FS + id];
+    acc = fmax(acc, sqrt(mx * mx + my * my + mz * mz) / W[id]);
+  }
+  sh[threadIdx.x] = acc;
+  __syncthreads();
+  for (int s = 128; s > 0; s >>= 1) {
+    if (threadIdx.x < s) sh[threadIdx.x] = fmax(sh[threadIdx.x], sh[threadIdx.x + s]);
+    __syncthreads();
+  }
+  /* non-negative doubles order like their bit patterns */
+  if (threadIdx.x == 0) atomicMax(out, (unsigned long long)__double_as_longlong(sh[0]));
+}
+
+__global__ void k_cfl_final(const unsigned long long *__restrict__ umax_bits, double cfl, double dmin, double cs,
+                            double *__restrict__ dt) {
+  *dt = cfl * dmin / (__longlong_as_double((long long)*umax_bits) + cs);
+}
+
 /* m += dt rho g ;  m_axis += target - sum(m_axis |Omega|)/sum|Omega|   (S16) */
 __global__ void __launch_bounds__(256) k_uniform_force(GksGrid g, double *__restrict__ W, double dt, double gx,
                                                        double gy, double gz, int bulk_axis, double target,
@@ -241,6 +269,14 @@ __global__ void __launch_bounds__(128) k_alm(GksGrid g, double *__restrict__ W, 
 int gks_launch_bulk_reduce(const GksGrid &g, const double *W, int axis, double *red, cudaStream_t s) {
   k_bulk_partial<<<RED_BLOCKS, 256, 0, s>>>(g, W, axis, red);
   k_bulk_final<<<1, 256, 0, s>>>(red);
+  return 2;
+}
+
+int gks_launch_cfl_dt(const GksGrid &g, const double *W, double cfl, double dmin, double cs, double *scratch,
+                      cudaStream_t s) {
+  /* scratch[0]: bit pattern of |U|_max (zeroed by the caller), scratch[1]: dt */
+  k_umax<<<RED_BLOCKS, 256, 0, s>>>(g, W, reinterpret_cast<unsigned long long *>(scratch));
+  k_cfl_final<<<1, 1, 0, s>>>(reinterpret_cast<const unsigned long long *>(scratch), cfl, dmin, cs, scratch + 1);
   return 2;
 }
 

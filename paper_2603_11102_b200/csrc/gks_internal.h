@@ -72,6 +72,7 @@ struct gks_ctx {
   double gacc[3];
   int bulk_axis;
   double bulk_target, total_volume;
+  double dmin;                 /* smallest cell width of the grid (CFL condition) */
   int n_alm;
   double alm_eps;
   int alm_lo[3], alm_cnt[3];   /* bounding box of the ALM support in (unwrapped) cell indices */
@@ -89,6 +90,7 @@ struct gks_ctx {
   int *prof_cat;
 };
 #define GKS_IBM_MAX_PASSES 64
+#define GKS_RED_CFL 1680       /* ctx->red + this: |U|_max bits, dt */
 #define GKS_RED_IBM_RES 1600   /* ctx->red + this: GKS_IBM_MAX_PASSES residual slots (bit patterns) */
 #define GKS_PROF_MAX 4096
 void gks_prof_begin(gks_ctx *ctx, int cat);
@@ -131,6 +133,8 @@ int gks_launch_ibm_spread(const GksGrid &g, double *W, int n, const double *pos,
                           double tol, const unsigned long long *res, cudaStream_t s);
 int gks_launch_alm(const GksGrid &g, double *W, int n, const double *pos, const double *force, double eps,
                    double dt, const int lo[3], const int cnt[3], cudaStream_t s);
+int gks_launch_cfl_dt(const GksGrid &g, const double *W, double cfl, double dmin, double cs, double *scratch,
+                      cudaStream_t s);
 int gks_launch_check_finite(const GksGrid &g, const double *W, int *flag, cudaStream_t s);
 
 #endif

@@ -18,7 +18,7 @@ STATUS = {0: "GKS_OK", 1: "GKS_ERR_INVALID_ARG", 2: "GKS_ERR_WORKSPACE", 3: "GKS
           4: "GKS_ERR_STATE", 5: "GKS_ERR_NONFINITE"}
 
 EXPORTS = ["gks_workspace_bytes", "gks_create", "gks_destroy", "gks_set_state", "gks_get_state", "gks_step",
-           "gks_set_body_force", "gks_set_bulk_flux", "alm_set_points", "ibm_set_points", "ibm_set_velocities", "ibm_set_iterations",
+           "gks_set_body_force", "gks_set_bulk_flux", "alm_set_points", "ibm_set_points", "ibm_set_velocities", "ibm_set_iterations", "gks_cfl_dt",
            "gks_debug_eval_flux", "gks_debug_set_sweep", "gks_debug_fp64_peak",
            "gks_profile_enable", "gks_profile_read", "gks_check_finite", "gks_launch_count", "gks_last_error"]
 
@@ -60,6 +60,7 @@ def lib():
         L.ibm_set_points.argtypes = [vp, C.c_int, vp, vp]
         L.ibm_set_velocities.argtypes = [vp, vp]
         L.ibm_set_iterations.argtypes = [vp, C.c_int, C.c_double]
+        L.gks_cfl_dt.argtypes = [vp, C.c_double, vp]
         L.gks_debug_eval_flux.argtypes = [vp, C.c_int, vp, vp]
         L.gks_debug_set_sweep.argtypes = [vp, C.c_int]
         L.gks_check_finite.argtypes = [vp]
@@ -196,6 +197,15 @@ class Gks:
         pw, k2 = _ptr(weights)
         self._check(lib().ibm_set_points(self._h, n, pp, pw))
         self.n_ibm = n
+
+    def cfl_dt(self, cfl, out=None):
+        """dt of PAPER.md:91 for the current state; out = a 1-element torch CUDA tensor keeps the call asynchronous"""
+        if out is not None:
+            self._check(lib().gks_cfl_dt(self._h, float(cfl), out.data_ptr()))
+            return out
+        host = np.zeros(1)
+        self._check(lib().gks_cfl_dt(self._h, float(cfl), host.ctypes.data))
+        return float(host[0])
 
     def ibm_set_iterations(self, max_iter, tol=0.0):
         self._check(lib().ibm_set_iterations(self._h, int(max_iter), float(tol)))

@@ -202,3 +202,28 @@ def test_ibm_multi_direct_forcing_passes(passes, tol):
     with pytest.raises(gks.GksError):
         gg.ibm_set_iterations(65)
     gg.close()
+
+
+def test_cfl_dt_matches_the_oracle():
+    """PAPER.md:91 on the device: the same number as the oracle's loop (both take max of sqrt(m.m)/rho; fma
+    contraction may move the last bit), host and device output pointers, stretched grid, after a step"""
+    import torch
+    from oracle import binding as ob
+    from paper_2603_11102_b200 import gks
+    for name in ("C1", "C2", "C5"):
+        w = wl.by_name(name, small=(name != "C1"))
+        o = ob.Oracle(w.cfg)
+        g = gks.Gks(w.cfg)
+        o.set_state(w.W0)
+        g.set_state(w.W0)
+        assert g.cfl_dt(0.4) == pytest.approx(o.cfl_dt(0.4), rel=1e-14)
+        o.step(w.dt)
+        g.step(w.dt)
+        out = torch.zeros(1, dtype=torch.float64, device="cuda:0")
+        g.cfl_dt(0.7, out)
+        g.synchronize()
+        assert float(out.cpu()[0]) == pytest.approx(o.cfl_dt(0.7), rel=1e-12)
+        with pytest.raises(gks.GksError):
+            g.cfl_dt(-1.0)
+        g.close()
+        o.close()
