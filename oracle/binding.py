@@ -22,6 +22,14 @@ class GksoConfig(C.Structure):
                 ("bc", C.c_int * 6), ("inflow", C.c_double * 4), ("weno_eps", C.c_double)]
 
 
+class GksoRotor(C.Structure):
+    _fields_ = [("nblades", C.c_int), ("npts", C.c_int), ("hub", C.c_double * 3),
+                ("R", C.c_double), ("r_hub", C.c_double), ("omega", C.c_double), ("theta0", C.c_double),
+                ("u_ref", C.c_double), ("eps", C.c_double), ("chord", _dp), ("twist", _dp),
+                ("npolar", C.c_int), ("alpha", _dp), ("cl", _dp), ("cd", _dp),
+                ("freestream_correction", C.c_int), ("tip_correction", C.c_int)]
+
+
 def build(force=False):
     """Compile the oracle with the system g++ (make -C oracle)."""
     so = os.path.join(_HERE, "libgks_oracle.so")
@@ -56,6 +64,8 @@ def lib():
         L.gkso_eval_forcing.argtypes = [vp, C.c_double, _dp]
         L.gkso_ibm_interpolate.argtypes = [vp, _dp]
         L.gkso_cfl_dt.argtypes = [vp, C.c_double, _dp]
+        L.gkso_alm_set_rotor.argtypes = [vp, C.POINTER(GksoRotor)]
+        L.gkso_alm_rotor_eval.argtypes = [vp, _dp, _dp]
         L.gkso_last_error.restype = C.c_char_p
         L.gkso_moments.argtypes = [C.c_double, C.c_double, C.c_int, _dp]
         L.gkso_moments.restype = None
@@ -203,6 +213,29 @@ class Oracle:
         dM = np.empty((3, nz, ny, nx))
         _check(lib().gkso_eval_forcing(self._h, float(dt), _p(dM)))
         return dM
+
+    def alm_set_rotor(self, r):
+        """r: workloads.Rotor (duck-typed) or None to clear"""
+        if r is None:
+            _check(lib().gkso_alm_set_rotor(self._h, None))
+            self._rotor_n = 0
+            return
+        keep = [_arr(x) for x in (r.chord, r.twist, r.alpha, r.cl, r.cd)]
+        assert len(keep[0]) == r.npts and len(keep[1]) == r.npts and len(keep[3]) == len(keep[2]) == len(keep[4])
+        c = GksoRotor()
+        c.nblades, c.npts = r.nblades, r.npts
+        c.hub = (C.c_double * 3)(*r.hub)
+        c.R, c.r_hub, c.omega, c.theta0, c.u_ref, c.eps = r.R, r.r_hub, r.omega, r.theta0, r.u_ref, r.eps
+        c.chord, c.twist, c.alpha, c.cl, c.cd = [_p(x) for x in keep]
+        c.npolar = len(keep[2])
+        c.freestream_correction, c.tip_correction = int(r.freestream_correction), int(r.tip_correction)
+        _check(lib().gkso_alm_set_rotor(self._h, C.byref(c)))
+        self._rotor_n = r.nblades * r.npts
+
+    def alm_rotor_eval(self):
+        pos, force = np.empty((self._rotor_n, 3)), np.empty((self._rotor_n, 3))
+        _check(lib().gkso_alm_rotor_eval(self._h, _p(pos), _p(force)))
+        return pos, force
 
     def cfl_dt(self, cfl):
         out = np.zeros(1)

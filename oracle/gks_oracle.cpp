@@ -333,6 +333,14 @@ struct gkso_ctx {
   double alm_eps = 0, alm_cut = 3.0;
   int n_ibm = 0;
   std::vector<double> ibm_pos, ibm_vol, ibm_vel;
+  /* on-line actuator-line rotor (Eq. 9, Eq. 14): when set, every step samples the flow at
+     the actuator points, evaluates the blade-element forces and replaces the point set of alm_set_points */
+  struct Rotor {
+    bool on = false;
+    int nb = 0, np = 0, fs_corr = 0, tip_corr = 0;
+    double hub[3] = {0, 0, 0}, R = 0, rhub = 0, omega = 0, theta0 = 0, uref = 0, time = 0;
+    std::vector<double> chord, twist, pa, pcl, pcd;
+  } rotor;
   int ibm_maxit = 1;       /* multi-direct-forcing passes per step; 1 = single pass (S15) */
   double ibm_tol = 0.0;    /* stop once max_p |v_p - U_p| < tol (checked from the second pass on) */
 
@@ -620,6 +628,110 @@ void ibm_interpolate(const gkso_ctx &s, const std::vector<double> &Wp, std::vect
   }
 }
 
+/* ------------------------------------------------------------------------------------------
+ * Actuator-line front half: flow sampling, force calculation.
+ * ------------------------------------------------------------------------------------------ */
+/* trilinear interpolation of (rho, U, V, W) between the 8 cell centres around X ("The trilinear interpolation
+ * method is used to interpolate the simulated velocity to each actuator point"); velocities, not
+ * momenta, are interpolated.  Periodic axes wrap; beyond the outermost centres of a non-periodic axis the
+ * outermost cell is used (zero gradient; ghost cells of the un-forced field are not defined) - reading S26. */
+void sample_trilinear(const gkso_ctx &s, const std::vector<double> &Wp, const double X[3], double out[4]) {
+  int i0[3], i1[3];
+  double t[3];
+  for (int a = 0; a < 3; ++a) {
+    const Axis &A = s.ax[a];
+    double x = X[a];
+    if (A.periodic) x -= std::floor((x - A.lo()) / A.len()) * A.len();
+    int c = A.find_cell(x);
+    if (c < 0) c = x < A.lo() ? 0 : A.n - 1;
+    const int lo = x < A.xc(c) ? c - 1 : c; /* xc(lo) <= x < xc(lo+1), centres of ghost cells included */
+    t[a] = (x - A.xc(lo)) / (A.xc(lo + 1) - A.xc(lo));
+    i0[a] = lo;
+    i1[a] = lo + 1;
+    if (A.periodic) {
+      i0[a] = (i0[a] + A.n) % A.n;
+      i1[a] = i1[a] % A.n;
+    } else {
+      i0[a] = std::min(std::max(i0[a], 0), A.n - 1);
+      i1[a] = std::min(std::max(i1[a], 0), A.n - 1);
+    }
+  }
+  for (int c = 0; c < 4; ++c) out[c] = 0.0;
+  for (int dk = 0; dk < 2; ++dk)
+    for (int dj = 0; dj < 2; ++dj)
+      for (int di = 0; di < 2; ++di) {
+        const int i = di ? i1[0] : i0[0], j = dj ? i1[1] : i0[1], k = dk ? i1[2] : i0[2];
+        const double wgt = (di ? t[0] : 1.0 - t[0]) * (dj ? t[1] : 1.0 - t[1]) * (dk ? t[2] : 1.0 - t[2]);
+        const double rho = Wp[s.id(0, i, j, k)];
+        out[0] += wgt * rho;
+        for (int c = 1; c < 4; ++c) out[c] += wgt * Wp[s.id(c, i, j, k)] / rho;
+      }
+}
+
+/* tabulated 2-D airfoil data, linear in alpha, end values beyond the table */
+void polar_lookup(const gkso_ctx::Rotor &r, double alpha, double &cl, double &cd) {
+  const int n = (int)r.pa.size();
+  if (alpha <= r.pa[0]) { cl = r.pcl[0]; cd = r.pcd[0]; return; }
+  if (alpha >= r.pa[n - 1]) { cl = r.pcl[n - 1]; cd = r.pcd[n - 1]; return; }
+  int m = 0;
+  while (r.pa[m + 1] < alpha) ++m;
+  const double t = (alpha - r.pa[m]) / (r.pa[m + 1] - r.pa[m]);
+  cl = r.pcl[m] + t * (r.pcl[m + 1] - r.pcl[m]);
+  cd = r.pcd[m] + t * (r.pcd[m + 1] - r.pcd[m]);
+}
+
+/* Eq. 14: f_tip = 2/pi acos(exp(-g1 N (R - r)/(2 r sin phi))), g1 = exp(-c1 (N lambda - c2)) + 0.1 */
+double tip_factor(int N, double R, double r, double sinphi, double tsr, double c1, double c2) {
+  if (!(sinphi > 0.0)) return 1.0; /* reading S27: no correction for a reversed flow angle */
+  const double g1 = std::exp(-c1 * (N * tsr - c2)) + 0.1;
+  return 2.0 / PI * std::acos(std::exp(-g1 * N * (R - r) / (2.0 * r * sinphi)));
+}
+
+/* positions of the actuator points at the rotor's clock and the point forces ON THE FLUID.
+ * Rotor axis +x; blade b at azimuth psi = theta0 + omega t + 2 pi b/N; radial unit (0, cos psi, sin psi),
+ * rotational unit e_theta = (0, -sin psi, cos psi); station k at r = r_hub + (k + 1/2) w, w = (R - r_hub)/npts. */
+void rotor_forces(const gkso_ctx &s, const std::vector<double> &Wp, std::vector<double> &pos,
+                  std::vector<double> &force) {
+  const gkso_ctx::Rotor &R = s.rotor;
+  pos.assign(3 * (size_t)R.nb * R.np, 0.0);
+  force.assign(3 * (size_t)R.nb * R.np, 0.0);
+  const double w = (R.R - R.rhub) / R.np;
+  for (int b = 0; b < R.nb; ++b) {
+    const double psi = R.theta0 + R.omega * R.time + 2.0 * PI * b / R.nb;
+    const double er[3] = {0.0, std::cos(psi), std::sin(psi)}, et[3] = {0.0, -std::sin(psi), std::cos(psi)};
+    for (int k = 0; k < R.np; ++k) {
+      const size_t p = (size_t)b * R.np + k;
+      const double r = R.rhub + (k + 0.5) * w, c = R.chord[k];
+      double X[3], q[4];
+      for (int a = 0; a < 3; ++a) X[a] = R.hub[a] + r * er[a];
+      sample_trilinear(s, Wp, X, q);                         /* flow sampling */
+      double Ux = q[1], Ut = q[2] * et[1] + q[3] * et[2];   /* U^2D = (U_x, U_theta) */
+      double phi = std::atan2(Ux, R.omega * r - Ut);         /* flow angle between U_rel and the rotor plane */
+      double cl, cd;
+      polar_lookup(R, phi - R.twist[k], cl, cd);             /* alpha = phi - gamma */
+      if (R.fs_corr) { /* U_inf^2D = U^2D / (1 - C_D c /(4 sqrt(pi) eps)), then U_rel again */
+        const double f = 1.0 / (1.0 - cd * c / (4.0 * std::sqrt(PI) * s.alm_eps));
+        Ux *= f;
+        Ut *= f;
+        phi = std::atan2(Ux, R.omega * r - Ut);
+        polar_lookup(R, phi - R.twist[k], cl, cd);
+      }
+      const double urel2 = Ux * Ux + (Ut - R.omega * r) * (Ut - R.omega * r);
+      const double L = 0.5 * q[0] * c * w * cl * urel2, D = 0.5 * q[0] * c * w * cd * urel2; /* Eq. 9 */
+      double Fx = L * std::cos(phi) + D * std::sin(phi), Ft = L * std::sin(phi) - D * std::cos(phi);
+      if (R.tip_corr) {
+        const double tsr = R.omega * R.R / R.uref;
+        Fx *= tip_factor(R.nb, R.R, r, std::sin(phi), tsr, 0.1219, 21.52);
+        Ft *= tip_factor(R.nb, R.R, r, std::sin(phi), tsr, 0.0984, 13.026);
+      }
+      for (int a = 0; a < 3; ++a) {
+        pos[3 * p + a] = X[a];
+        force[3 * p + a] = -(a == 0 ? Fx : Ft * et[a]);       /* reaction on the fluid */
+      }
+    }
+  }
+}
+
 void eval_forcing(const gkso_ctx &s, const std::vector<double> &Wp, double dt, std::vector<double> &dM) {
   const size_t N = s.ncell();
   dM.assign(3 * N, 0.0);
@@ -872,6 +984,11 @@ int gkso_step(gkso_ctx *s, double dt) {
               Wn[s->id(c, i, j, k)] + dt * L[o] + dt * dt / 6.0 * (dL[o] + 2.0 * dL2[o]);
         }
   /* 6: forcing increments from the un-forced W^{n+1}, then added (Eq. 13; density gets none) */
+  if (s->rotor.on) { /* ALM front half on the un-forced field at the rotor's clock t^n (S12, S26) */
+    rotor_forces(*s, Wnew, s->alm_pos, s->alm_force);
+    s->n_alm = s->rotor.nb * s->rotor.np;
+    s->rotor.time += dt;
+  }
   std::vector<double> dM;
   eval_forcing(*s, Wnew, dt, dM);
   for (int c = 0; c < 3; ++c)
@@ -981,9 +1098,58 @@ int gkso_get_padded(gkso_ctx *s, double *Wp) {
   return 0;
 }
 
+int gkso_alm_set_rotor(gkso_ctx *s, const gkso_rotor *r) {
+  if (!s) return fail("null argument");
+  if (!r) { /* NULL clears the rotor and its points */
+    s->rotor = gkso_ctx::Rotor();
+    s->n_alm = 0;
+    return 0;
+  }
+  if (r->nblades < 1 || r->npts < 1 || !r->chord || !r->twist || r->npolar < 2 || !r->alpha || !r->cl || !r->cd)
+    return fail("rotor: bad sizes or null tables");
+  if (!(r->R > r->r_hub) || !(r->r_hub >= 0) || !(r->eps > 0)) return fail("rotor: need R > r_hub >= 0 and eps > 0");
+  if (r->tip_correction && !(r->u_ref > 0)) return fail("rotor: the tip correction needs u_ref > 0 (tip speed ratio)");
+  for (int m = 1; m < r->npolar; ++m)
+    if (!(r->alpha[m] > r->alpha[m - 1])) return fail("rotor: polar angles must increase");
+  for (int a = 0; a < 3; ++a) {
+    const Axis &A = s->ax[a];
+    if (A.periodic && 2.0 * s->alm_cut * r->eps > A.len()) return fail("alm: support wider than a periodic axis");
+  }
+  gkso_ctx::Rotor &R = s->rotor;
+  R.on = true;
+  R.nb = r->nblades; R.np = r->npts;
+  for (int a = 0; a < 3; ++a) R.hub[a] = r->hub[a];
+  R.R = r->R; R.rhub = r->r_hub; R.omega = r->omega; R.theta0 = r->theta0; R.uref = r->u_ref; R.time = 0.0;
+  R.fs_corr = r->freestream_correction; R.tip_corr = r->tip_correction;
+  R.chord.assign(r->chord, r->chord + r->npts);
+  R.twist.assign(r->twist, r->twist + r->npts);
+  R.pa.assign(r->alpha, r->alpha + r->npolar);
+  R.pcl.assign(r->cl, r->cl + r->npolar);
+  R.pcd.assign(r->cd, r->cd + r->npolar);
+  s->alm_eps = r->eps;
+  s->n_alm = 0;
+  return 0;
+}
+
+/* test hook: positions and forces on the fluid of the actuator points for the CURRENT state and rotor clock */
+int gkso_alm_rotor_eval(gkso_ctx *s, double *pos, double *force) {
+  if (!s || !pos || !force) return fail("bad argument");
+  if (!s->have_state) return fail("no state set");
+  if (!s->rotor.on) return fail("no rotor set");
+  std::vector<double> p, f;
+  rotor_forces(*s, s->W, p, f);
+  std::memcpy(pos, p.data(), p.size() * sizeof(double));
+  std::memcpy(force, f.data(), f.size() * sizeof(double));
+  return 0;
+}
+
 int gkso_eval_forcing(gkso_ctx *s, double dt, double *dM) {
   if (!s || !dM) return fail("bad argument");
   if (!s->have_state) return fail("no state set");
+  if (s->rotor.on) {
+    rotor_forces(*s, s->W, s->alm_pos, s->alm_force);
+    s->n_alm = s->rotor.nb * s->rotor.np;
+  }
   std::vector<double> d;
   eval_forcing(*s, s->W, dt, d);
   std::memcpy(dM, d.data(), d.size() * sizeof(double));

@@ -56,6 +56,22 @@ int gkso_get_padded(gkso_ctx *ctx, double *Wp);
 int gkso_eval_forcing(gkso_ctx *ctx, double dt, double *dM);
 /* interpolated fluid velocity at the IBM points (n*3) for the current state */
 int gkso_ibm_interpolate(gkso_ctx *ctx, double *Up);
+/* On-line actuator-line rotor (Eq. 9, Eq. 14; S26-S27): axis +x, blade b at azimuth
+ * theta0 + omega t + 2 pi b / nblades, station k at r_hub + (k + 1/2)(R - r_hub)/npts.  Every step samples the
+ * un-forced field at the points (trilinear), evaluates lift and drag from the tabulated polar and spreads the
+ * reaction with Eq. 10.  NULL clears.  The rotor clock starts at 0 and advances by dt per step. */
+typedef struct {
+  int nblades, npts;
+  double hub[3];
+  double R, r_hub, omega, theta0, u_ref, eps;
+  const double *chord, *twist;         /* npts each: chord length and local twist angle gamma [rad] */
+  int npolar;
+  const double *alpha, *cl, *cd;       /* tabulated 2-D airfoil data, alpha [rad] increasing */
+  int freestream_correction;           /* U_inf^2D = U^2D / (1 - C_D c/(4 sqrt(pi) eps)) */
+  int tip_correction;                  /* Eq. 14, (c1, c2) = (0.1219, 21.52) axial, (0.0984, 13.026) tangential */
+} gkso_rotor;
+int gkso_alm_set_rotor(gkso_ctx *ctx, const gkso_rotor *rotor);
+int gkso_alm_rotor_eval(gkso_ctx *ctx, double *pos, double *force); /* test hook: nblades*npts*3 each */
 /* dt of the CFL condition */
 int gkso_cfl_dt(gkso_ctx *ctx, double cfl, double *dt);
 const char *gkso_last_error(void);

@@ -66,6 +66,43 @@ class Workload:
     notes: str = ""
 
 
+@dataclass
+class Rotor:
+    """Input data of the on-line actuator-line rotor: geometry, tabulated polar, switches.
+    Axis +x; blade b at azimuth theta0 + omega t + 2 pi b / nblades; station k at r_hub + (k+1/2)(R-r_hub)/npts."""
+    nblades: int
+    npts: int
+    hub: Tuple[float, float, float]
+    R: float
+    r_hub: float
+    omega: float
+    theta0: float
+    u_ref: float
+    eps: float
+    chord: np.ndarray        # (npts,)
+    twist: np.ndarray        # (npts,) local twist angle gamma [rad]
+    alpha: np.ndarray        # (npolar,) increasing [rad]
+    cl: np.ndarray
+    cd: np.ndarray
+    freestream_correction: bool = False
+    tip_correction: bool = False
+
+
+def synthetic_rotor(hub, R, eps, u_ref=U_INF, tsr=7.0, nblades=3, npts=64, seed=20260314, **switches):
+    """A seeded stand-in for the paper's blade data (NREL 5 MW / NTNU tables are not available): tapered
+    chord, twist falling from root to tip, and a smooth polar with a linear range, stall and a drag bucket."""
+    rng = np.random.default_rng(seed)
+    s = (np.arange(npts) + 0.5) / npts
+    chord = R * (0.09 - 0.055 * s) * (1.0 + 0.03 * rng.standard_normal(npts))
+    twist = np.deg2rad(14.0 * (1.0 - s) ** 1.5 - 1.0 + 0.2 * rng.standard_normal(npts))
+    alpha = np.deg2rad(np.linspace(-30.0, 40.0, 71))
+    a_st = np.deg2rad(13.0)
+    cl = 2 * np.pi * 0.9 * a_st * np.tanh(alpha / a_st) * (1.0 - 0.25 * np.clip((np.abs(alpha) - a_st) / a_st, 0, 1))
+    cd = 0.008 + 0.9 * np.sin(alpha) ** 2
+    return Rotor(nblades=nblades, npts=npts, hub=tuple(hub), R=R, r_hub=0.05 * R, omega=tsr * u_ref / R, theta0=0.1,
+                 u_ref=u_ref, eps=eps, chord=chord, twist=twist, alpha=alpha, cl=cl, cd=cd, **switches)
+
+
 # ----------------------------------------------------------------------------------------------
 _G3_X = np.array([-np.sqrt(3.0 / 5.0), 0.0, np.sqrt(3.0 / 5.0)]) * 0.5   # nodes on [-1/2, 1/2]
 _G3_W = np.array([5.0, 8.0, 5.0]) / 18.0

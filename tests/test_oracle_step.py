@@ -411,3 +411,164 @@ def test_P16_cfl_dt_closed_forms_and_invariants():
     o.set_state(w.W0)
     assert o.cfl_dt(0.4) == pytest.approx(w.dt, rel=1e-14)
     o.close()
+
+
+# ---------------------------------------------------------------- P17 actuator-line front half (S26, S27)
+def rotor_case(**kw):
+    n, h = (24, 24, 24), 0.125
+    cfg = GridConfig(n=n, spacing=(h, h, h), bc=(EX, EX, P, P, EX, EX))
+    r = wl.synthetic_rotor(hub=(1.5, 1.5, 1.5), R=1.0, eps=2 * h, npts=16, **kw)
+    return cfg, r
+
+
+def rel_velocity(r, pos, U):
+    """blade-relative velocity vectors of the points in a uniform flow U (geometry only: U - omega x r)"""
+    d = pos - np.asarray(r.hub)
+    v_blade = r.omega * np.stack([np.zeros(len(d)), -d[:, 2], d[:, 1]], axis=1)     # omega e_x x d
+    return np.asarray(U)[None, :] - v_blade
+
+
+def test_P17_geometry_and_trilinear_sampling():
+    cfg, r = rotor_case()
+    o = ob.Oracle(cfg)
+    o.set_state(const_state(cfg.n, (1.0, 0.1, 0.0, 0.0)))
+    o.alm_set_rotor(r)
+    pos, _ = o.alm_rotor_eval()
+    d = pos - np.asarray(r.hub)
+    w = (r.R - r.r_hub) / r.npts
+    rad = np.hypot(d[:, 1], d[:, 2]).reshape(r.nblades, r.npts)
+    assert np.allclose(d[:, 0], 0) and np.allclose(rad, r.r_hub + (np.arange(r.npts) + 0.5) * w, rtol=1e-14)
+    az = np.arctan2(d[:, 2], d[:, 1]).reshape(r.nblades, r.npts)
+    assert np.allclose(az[0], r.theta0) and np.allclose(np.diff(np.unwrap(az[:, 0])), 2 * np.pi / r.nblades)
+    # the clock advances by dt per step: after a step the azimuth has turned by omega dt
+    o.step(0.01)
+    pos2, _ = o.alm_rotor_eval()
+    az2 = np.arctan2(pos2[0, 2] - r.hub[2], pos2[0, 1] - r.hub[1])
+    assert az2 - r.theta0 == pytest.approx(r.omega * 0.01, rel=1e-12)
+    o.close()
+    # sampling is exact for a velocity field that is trilinear in (x, y, z): force with a pure-drag polar is
+    # 1/2 rho c w cd |U_rel| U_rel with U_rel from the exact field at the point
+    x, y, z = [cfg.centres(a) for a in range(3)]
+    Z, Y, X = np.meshgrid(z, y, x, indexing="ij")
+    U = np.stack([0.1 + 0.02 * X + 0.01 * Y * Z, 0.03 * X * Y - 0.01, 0.02 * Z + 0.01 * X * Y * Z])
+    rho = 1.1
+    W = np.concatenate([np.full((1,) + X.shape, rho), rho * U])
+    r2 = wl.synthetic_rotor(hub=(1.5, 1.5, 1.5), R=0.8, eps=0.25, npts=12)
+    r2.cl = np.zeros_like(r2.cl)
+    r2.cd = np.full_like(r2.cd, 0.7)
+    o = ob.Oracle(GridConfig(n=cfg.n, spacing=cfg.spacing, bc=(EX,) * 6))
+    o.set_state(W)
+    o.alm_set_rotor(r2)
+    pos, F = o.alm_rotor_eval()
+    px, py, pz = pos.T
+    Uex = np.stack([0.1 + 0.02 * px + 0.01 * py * pz, 0.03 * px * py - 0.01, 0.02 * pz + 0.01 * px * py * pz], axis=1)
+    d = pos - np.asarray(r2.hub)
+    rad = np.hypot(d[:, 1], d[:, 2])
+    et = np.stack([np.zeros(len(d)), -d[:, 2] / rad, d[:, 1] / rad], axis=1)
+    # the blade element only sees the axial and rotational components (U^2D); the radial one is dropped
+    U2d = Uex[:, :1] * np.array([[1.0, 0, 0]]) + (Uex * et).sum(1, keepdims=True) * et
+    Urel = U2d - r2.omega * rad[:, None] * et
+    w2 = (r2.R - r2.r_hub) / r2.npts
+    drag_on_blade = 0.5 * rho * np.tile(r2.chord, r2.nblades)[:, None] * w2 * 0.7 * np.linalg.norm(Urel, axis=1)[:, None] * Urel
+    assert np.allclose(F, -drag_on_blade, rtol=1e-12, atol=1e-18)
+    o.close()
+
+
+def test_P17_lift_is_normal_and_drag_parallel_to_the_relative_flow():
+    """two-dimensional airfoil theory (Eq. 9): with C_D = 0 the force is perpendicular to U_rel and
+    has magnitude 1/2 rho c w C_L |U_rel|^2; with C_L = 0 it is parallel; thrust on the fluid points upstream
+    and the tangential reaction opposes the rotation for an attached-flow blade"""
+    cfg, r = rotor_case()
+    rho, U = 1.2, np.array([0.1, 0.0, 0.0])
+    w = (r.R - r.r_hub) / r.npts
+    chord = np.tile(r.chord, r.nblades)
+    o = ob.Oracle(cfg)
+    o.set_state(const_state(cfg.n, (rho, *(rho * U))))
+    lift_only = wl.synthetic_rotor(hub=r.hub, R=r.R, eps=r.eps, npts=r.npts)
+    lift_only.cd = np.zeros_like(r.cd)
+    o.alm_set_rotor(lift_only)
+    pos, F = o.alm_rotor_eval()
+    Urel = rel_velocity(r, pos, U)
+    assert np.abs((F * Urel).sum(1)).max() <= 1e-15 * np.abs(F).max() * np.abs(Urel).max()
+    d = pos - np.asarray(r.hub)
+    rad = np.hypot(d[:, 1], d[:, 2])
+    phi = np.arctan2(U[0], r.omega * rad)                      # uniform axial wind: U_theta = 0
+    cl = np.interp(phi - np.tile(r.twist, r.nblades), r.alpha, lift_only.cl)
+    assert np.allclose(np.linalg.norm(F, axis=1), 0.5 * rho * chord * w * np.abs(cl) * (Urel ** 2).sum(1), rtol=1e-12)
+    assert (F[:, 0] < 0).all()                                 # the fluid is pushed upstream (thrust reaction)
+    et = np.stack([np.zeros(len(d)), -d[:, 2] / rad, d[:, 1] / rad], axis=1)
+    assert ((F * et).sum(1) < 0).all()                         # and against the rotation (torque reaction)
+    drag_only = wl.synthetic_rotor(hub=r.hub, R=r.R, eps=r.eps, npts=r.npts)
+    drag_only.cl = np.zeros_like(r.cl)
+    o.alm_set_rotor(drag_only)
+    pos, F = o.alm_rotor_eval()
+    cross = np.cross(F, rel_velocity(r, pos, U))
+    assert np.abs(cross).max() <= 1e-15 * np.abs(F).max() * np.abs(Urel).max()
+    assert ((F * rel_velocity(r, pos, U)).sum(1) < 0).all()    # reaction of a drag: against U_rel
+    o.close()
+
+
+def test_P17_corrections():
+    """free-stream correction: with a constant C_D and a constant chord the forces equal those of
+    the uncorrected model in a flow scaled by 1/(1 - C_D c/(4 sqrt(pi) eps)); tip correction (Eq. 14): factors in
+    (0, 1], -> 1 towards the root, -> 0 at the tip, axial and tangential differ, a no-op when switched off"""
+    cfg, r = rotor_case()
+    rho, U = 1.0, np.array([0.1, 0.004, -0.003])
+    mk = lambda **kw: wl.synthetic_rotor(hub=r.hub, R=r.R, eps=r.eps, npts=r.npts, **kw)
+    base, corr = mk(), mk(freestream_correction=True)
+    for q in (base, corr):
+        q.chord = np.full(r.npts, 0.08)
+        q.cd = np.full_like(r.cd, 0.3)
+    k = 1.0 / (1.0 - 0.3 * 0.08 / (4 * math.sqrt(math.pi) * r.eps))
+    o = ob.Oracle(cfg)
+    o.set_state(const_state(cfg.n, (rho, *(rho * U))))
+    o.alm_set_rotor(corr)
+    F_corr = o.alm_rotor_eval()[1]
+    o.set_state(const_state(cfg.n, (rho, *(rho * U * k))))
+    o.alm_set_rotor(base)
+    F_scaled = o.alm_rotor_eval()[1]
+    assert k > 1.01 and np.allclose(F_corr, F_scaled, rtol=1e-12, atol=1e-18)
+    # tip correction
+    o.set_state(const_state(cfg.n, (rho, 0.1, 0.0, 0.0)))
+    fine = dict(npts=200)
+    o.alm_set_rotor(wl.synthetic_rotor(hub=r.hub, R=r.R, eps=r.eps, **fine))
+    pos, F0 = o.alm_rotor_eval()
+    o.alm_set_rotor(wl.synthetic_rotor(hub=r.hub, R=r.R, eps=r.eps, tip_correction=True, **fine))
+    F1 = o.alm_rotor_eval()[1]
+    d = pos - np.asarray(r.hub)
+    rad = np.hypot(d[:, 1], d[:, 2])[:200]
+    et = np.stack([np.zeros(200), -d[:200, 2] / rad, d[:200, 1] / rad], axis=1)
+    f_ax = F1[:200, 0] / F0[:200, 0]
+    f_tan = (F1[:200] * et).sum(1) / (F0[:200] * et).sum(1)
+    for f in (f_ax, f_tan):
+        assert (f > 0).all() and (f <= 1.0).all() and (np.diff(f[rad > 0.3]) < 0).all()
+        assert f[rad < 0.2].min() > 0.99 and f[-1] < 0.2
+    assert np.abs(f_ax - f_tan).max() > 1e-3
+    # worked value: N = 3, lambda = 7, r = 0.9 R, phi from a uniform wind: f = 2/pi acos(exp(-g1 N (R-r)/(2 r sin phi)))
+    i = np.argmin(np.abs(rad - 0.9))
+    sphi = math.sin(math.atan2(0.1, 0.7 * rad[i]))
+    g1 = math.exp(-0.1219 * (3 * 7.0 - 21.52)) + 0.1
+    assert f_ax[i] == pytest.approx(2 / math.pi * math.acos(math.exp(-g1 * 3 * (1.0 - rad[i]) / (2 * rad[i] * sphi))), rel=1e-10)
+    with pytest.raises(ob.OracleError):
+        bad = mk(tip_correction=True)
+        bad.u_ref = 0.0
+        o.alm_set_rotor(bad)
+    o.close()
+
+
+def test_P17_rotor_step_equals_prescribed_points_step():
+    """a step with the on-line rotor = a step with alm_set_points fed with the forces the rotor evaluates on the
+    un-forced field (S12, S26): here checked through the linearity of the forcing, increment by increment"""
+    cfg, r = rotor_case()
+    rng = np.random.default_rng(5)
+    W0 = const_state(cfg.n, (1.0, 0.1, 0.0, 0.0)) * (1 + 0.01 * rng.standard_normal((4,) + cfg.n[::-1]))
+    o = ob.Oracle(cfg)
+    o.set_state(W0)
+    o.alm_set_rotor(r)
+    pos, F = o.alm_rotor_eval()
+    dM_rotor = o.eval_forcing(0.02)
+    o.alm_set_rotor(None)
+    o.alm_set_points(pos, F, r.eps)
+    assert np.array_equal(dM_rotor, o.eval_forcing(0.02))
+    assert np.abs(dM_rotor).max() > 0
+    o.close()
