@@ -108,6 +108,30 @@ gks_status gks_set_bulk_flux(gks_ctx *ctx, int axis, double target_bulk_momentum
  * sampled at cell centres and cut at r <= 3 eps.  n = 0 clears.  n <= GKS_MAX_ALM_POINTS. */
 gks_status alm_set_points(gks_ctx *ctx, int n, const double *pos, const double *force, double eps);
 
+/* On-line actuator-line rotor (Eq. 9, Eq. 14; S26-S27): instead of prescribed point
+ * forces, every gks_step (i) places nblades*npts actuator points - rotor axis +x, blade b at azimuth
+ * theta0 + omega t + 2 pi b/nblades, station k at r_hub + (k+1/2)(R - r_hub)/npts, t = the rotor clock, 0 at this
+ * call and advanced by dt per step -, (ii) samples (rho, U) of the un-forced W^{n+1} at the points by trilinear
+ * interpolation, (iii) evaluates lift and drag (Eq. 9) from the tabulated polar at alpha = phi - twist,
+ * phi = atan2(U_x, omega r - U_theta), optionally with the free-stream correction of PAPER.md:107 and the tip
+ * correction of Eq. 14, and (iv) spreads the reaction with Eq. 10 - all on the device.
+ * Tables (host or device pointers) are copied during the call: chord, twist [rad] npts each; alpha [rad,
+ * increasing], cl, cd npolar each.  npts <= 4096, npolar <= 1024, nblades*npts <= GKS_MAX_ALM_POINTS.
+ * NULL clears the rotor; alm_set_points also replaces it.  Errors: GKS_ERR_INVALID_ARG. */
+typedef struct {
+  int nblades, npts;
+  double hub[3];
+  double R, r_hub, omega, theta0, u_ref, eps;
+  const double *chord, *twist;
+  int npolar;
+  const double *alpha, *cl, *cd;
+  int freestream_correction, tip_correction;
+} alm_rotor;
+gks_status alm_set_rotor(gks_ctx *ctx, const alm_rotor *rotor);
+/* Test hook: positions and forces ON THE FLUID (nblades*npts*3 doubles each, host or device) of the actuator
+ * points for the CURRENT state and rotor clock; synchronises the stream. */
+gks_status alm_rotor_eval(gks_ctx *ctx, double *pos, double *force);
+
 /* IBM: n Lagrangian points; pos n*3 doubles, weights n doubles = V_p = dx*dS
  * (PAPER.md:155); host or device.  Velocities default to 0 (stationary body).
  * Each point must lie inside the domain and the grid must be locally uniform over its 3x3x3

@@ -43,6 +43,41 @@ void sweeps(gks_ctx *ctx, const double *W, bool need_F) {
   }
 }
 
+/* bounding box, in unwrapped cell indices, of the cells whose centre can lie within 3 eps of a point cloud
+   spanning [pmin, pmax]; conservative by one cell, the kernel applies the exact cut */
+gks_status alm_bbox(gks_ctx *ctx, const double pmin[3], const double pmax[3], double eps, int lo[3], int cnt[3]) {
+  const double R = 3.0 * eps;
+  for (int a = 0; a < 3; ++a) {
+    const int nn = ctx->g.n[a];
+    const double *xf = ctx->h_xf[a] + GKS_NG;
+    const double L = xf[nn] - xf[0];
+    if (!std::isfinite(pmin[a]) || !std::isfinite(pmax[a])) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "non-finite position");
+    /* unwrapped index of the cell containing x (periodic: any x; else clamped to the domain) */
+    auto cell_of = [&](double x) {
+      long long m = 0;
+      if (ctx->g.periodic[a]) {
+        m = (long long)floor((x - xf[0]) / L);
+        x -= m * L;
+      }
+      int c = gks_host_find_cell(ctx, a, x);
+      if (c < 0) c = x < xf[0] ? 0 : nn - 1;
+      return (long long)c + m * nn;
+    };
+    long long l = cell_of(pmin[a] - R) - 1, h = cell_of(pmax[a] + R) + 1;
+    if (ctx->g.periodic[a]) {
+      if (2.0 * R >= L) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "alm: 6 eps must be smaller than a periodic axis");
+      if (h - l + 1 > nn) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "alm: point cloud + support wider than a periodic axis");
+    } else {
+      if (l < 0) l = 0;
+      if (h > nn - 1) h = nn - 1;
+    }
+    if (h < l) h = l;
+    lo[a] = (int)l;
+    cnt[a] = (int)(h - l + 1);
+  }
+  return GKS_OK;
+}
+
 } /* namespace */
 
 extern "C" {
@@ -106,6 +141,12 @@ gks_status gks_step(gks_ctx *ctx, double dt) {
   gks_prof_begin(ctx, GKS_PROF_FORCING);
   /* forcing (Eq. 13), every increment from the un-forced field: read-only kernels first */
   const bool uniform = ctx->gacc[0] != 0.0 || ctx->gacc[1] != 0.0 || ctx->gacc[2] != 0.0;
+  if (ctx->rotor_on) { /* ALM front half on the un-forced field at the rotor clock t^n (S12, S26) */
+    ctx->launches += gks_launch_rotor_forces(g, ctx->Wn, ctx->rotor, ctx->rotor_time, ctx->alm_eps, ctx->alm_pos,
+                                             ctx->alm_force, s);
+    ctx->n_alm = ctx->rotor.nb * ctx->rotor.np;
+    ctx->rotor_time += dt;
+  }
   if (ctx->bulk_axis >= 0) ctx->launches += gks_launch_bulk_reduce(g, ctx->Wn, ctx->bulk_axis, ctx->red, s);
   if (ctx->n_ibm > 0) {
     /* multi-direct-forcing passes (Eq. 11-12): pass k interpolates from the un-forced field plus the IBM
@@ -153,6 +194,7 @@ gks_status gks_set_bulk_flux(gks_ctx *ctx, int axis, double target) {
 gks_status alm_set_points(gks_ctx *ctx, int n, const double *pos, const double *force, double eps) {
   if (!ctx) return GKS_ERR_INVALID_ARG;
   if (n < 0 || n > GKS_MAX_ALM_POINTS) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "n out of range");
+  ctx->rotor_on = 0;   /* prescribed points replace an on-line rotor */
   if (n == 0) {
     ctx->n_alm = 0;
     return GKS_OK;
@@ -161,43 +203,16 @@ gks_status alm_set_points(gks_ctx *ctx, int n, const double *pos, const double *
   if (!(eps > 0) || !std::isfinite(eps)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "eps must be > 0");
   std::vector<double> hp;
   if (gks_status st = fetch_host(ctx, pos, 3 * (size_t)n, hp)) return st;
-  /* bounding box of the cut supports in unwrapped cell indices (cells whose centre can lie within
-     3 eps of a point); conservative by one cell, the kernel applies the exact cut */
-  const double R = 3.0 * eps;
-  int lo[3], cnt[3];
+  double pmin[3], pmax[3];
   for (int a = 0; a < 3; ++a) {
-    const int nn = ctx->g.n[a];
-    const double *xf = ctx->h_xf[a] + GKS_NG;
-    const double L = xf[nn] - xf[0];
-    double pmin = hp[a], pmax = hp[a];
+    pmin[a] = pmax[a] = hp[a];
     for (int p = 1; p < n; ++p) {
-      pmin = fmin(pmin, hp[3 * p + a]);
-      pmax = fmax(pmax, hp[3 * p + a]);
+      pmin[a] = fmin(pmin[a], hp[3 * p + a]);
+      pmax[a] = fmax(pmax[a], hp[3 * p + a]);
     }
-    if (!std::isfinite(pmin) || !std::isfinite(pmax)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "non-finite position");
-    /* unwrapped index of the cell containing x (periodic: any x; else clamped to the domain) */
-    auto cell_of = [&](double x) {
-      long long m = 0;
-      if (ctx->g.periodic[a]) {
-        m = (long long)floor((x - xf[0]) / L);
-        x -= m * L;
-      }
-      int c = gks_host_find_cell(ctx, a, x);
-      if (c < 0) c = x < xf[0] ? 0 : nn - 1;
-      return (long long)c + m * nn;
-    };
-    long long l = cell_of(pmin - R) - 1, h = cell_of(pmax + R) + 1;
-    if (ctx->g.periodic[a]) {
-      if (2.0 * R >= L) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "alm: 6 eps must be smaller than a periodic axis");
-      if (h - l + 1 > nn) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "alm: point cloud + support wider than a periodic axis");
-    } else {
-      if (l < 0) l = 0;
-      if (h > nn - 1) h = nn - 1;
-    }
-    if (h < l) h = l;
-    lo[a] = (int)l;
-    cnt[a] = (int)(h - l + 1);
   }
+  int lo[3], cnt[3];
+  if (gks_status st = alm_bbox(ctx, pmin, pmax, eps, lo, cnt)) return st;
   const cudaMemcpyKind kind = gks_is_device_ptr(pos) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
   const cudaMemcpyKind kindf = gks_is_device_ptr(force) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
   CUDA_TRY(ctx, cudaMemcpyAsync(ctx->alm_pos, pos, 3 * (size_t)n * sizeof(double), kind, ctx->stream));
@@ -210,6 +225,75 @@ gks_status alm_set_points(gks_ctx *ctx, int n, const double *pos, const double *
   }
   ctx->n_alm = n;
   ctx->alm_eps = eps;
+  return GKS_OK;
+}
+
+gks_status alm_set_rotor(gks_ctx *ctx, const alm_rotor *r) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (!r) {
+    ctx->rotor_on = 0;
+    ctx->n_alm = 0;
+    return GKS_OK;
+  }
+  if (r->nblades < 1 || r->npts < 1 || r->npts > GKS_MAX_ROTOR_STATIONS || r->npolar < 2 || r->npolar > GKS_MAX_POLAR ||
+      (long long)r->nblades * r->npts > GKS_MAX_ALM_POINTS)
+    return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "rotor: sizes out of range");
+  if (!r->chord || !r->twist || !r->alpha || !r->cl || !r->cd) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "rotor: NULL table");
+  if (!(r->R > r->r_hub) || !(r->r_hub >= 0) || !(r->eps > 0) || !std::isfinite(r->R) || !std::isfinite(r->eps) ||
+      !std::isfinite(r->omega) || !std::isfinite(r->theta0))
+    return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "rotor: need R > r_hub >= 0, eps > 0 and finite parameters");
+  if (r->tip_correction && !(r->u_ref > 0))
+    return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "rotor: the tip correction needs u_ref > 0 (tip speed ratio)");
+  std::vector<double> t[5];
+  const double *src[5] = {r->chord, r->twist, r->alpha, r->cl, r->cd};
+  const size_t cnt5[5] = {(size_t)r->npts, (size_t)r->npts, (size_t)r->npolar, (size_t)r->npolar, (size_t)r->npolar};
+  for (int q = 0; q < 5; ++q)
+    if (gks_status st = fetch_host(ctx, src[q], cnt5[q], t[q])) return st;
+  for (int m = 1; m < r->npolar; ++m)
+    if (!(t[2][m] > t[2][m - 1])) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "rotor: polar angles must increase");
+  /* the blades sweep the disc of radius R about the hub in the plane x = hub[0]: its bounding box is constant */
+  const double pmin[3] = {r->hub[0], r->hub[1] - r->R, r->hub[2] - r->R};
+  const double pmax[3] = {r->hub[0], r->hub[1] + r->R, r->hub[2] + r->R};
+  int lo[3], cnt[3];
+  if (gks_status st = alm_bbox(ctx, pmin, pmax, r->eps, lo, cnt)) return st;
+  const size_t off[5] = {0, GKS_MAX_ROTOR_STATIONS, 2 * GKS_MAX_ROTOR_STATIONS, 2 * GKS_MAX_ROTOR_STATIONS + GKS_MAX_POLAR,
+                         2 * GKS_MAX_ROTOR_STATIONS + 2 * GKS_MAX_POLAR};
+  for (int q = 0; q < 5; ++q)
+    CUDA_TRY(ctx, cudaMemcpyAsync(ctx->rotor_tab + off[q], t[q].data(), cnt5[q] * sizeof(double), cudaMemcpyHostToDevice,
+                                  ctx->stream));
+  CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));   /* the staging vectors go out of scope */
+  GksRotor &R = ctx->rotor;
+  R.nb = r->nblades; R.np = r->npts; R.npolar = r->npolar;
+  R.fs_corr = r->freestream_correction != 0; R.tip_corr = r->tip_correction != 0;
+  for (int a = 0; a < 3; ++a) R.hub[a] = r->hub[a];
+  R.R = r->R; R.rhub = r->r_hub; R.omega = r->omega; R.theta0 = r->theta0; R.uref = r->u_ref;
+  R.chord = ctx->rotor_tab + off[0]; R.twist = ctx->rotor_tab + off[1]; R.alpha = ctx->rotor_tab + off[2];
+  R.cl = ctx->rotor_tab + off[3]; R.cd = ctx->rotor_tab + off[4];
+  for (int a = 0; a < 3; ++a) {
+    ctx->alm_lo[a] = lo[a];
+    ctx->alm_cnt[a] = cnt[a];
+  }
+  ctx->alm_eps = r->eps;
+  ctx->n_alm = 0;
+  ctx->rotor_on = 1;
+  ctx->rotor_time = 0.0;
+  return GKS_OK;
+}
+
+gks_status alm_rotor_eval(gks_ctx *ctx, double *pos, double *force) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (!pos || !force) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "pos/force is NULL");
+  if (!ctx->have_state) return gks_set_err(ctx, GKS_ERR_STATE, "alm_rotor_eval before gks_set_state");
+  if (!ctx->rotor_on) return gks_set_err(ctx, GKS_ERR_STATE, "no rotor set");
+  const int n = ctx->rotor.nb * ctx->rotor.np;
+  ctx->launches += gks_launch_rotor_forces(ctx->g, ctx->Wn, ctx->rotor, ctx->rotor_time, ctx->alm_eps, ctx->alm_pos,
+                                           ctx->alm_force, ctx->stream);
+  CUDA_TRY(ctx, cudaGetLastError());
+  const cudaMemcpyKind kp = gks_is_device_ptr(pos) ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+  const cudaMemcpyKind kf = gks_is_device_ptr(force) ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+  CUDA_TRY(ctx, cudaMemcpyAsync(pos, ctx->alm_pos, 3 * (size_t)n * sizeof(double), kp, ctx->stream));
+  CUDA_TRY(ctx, cudaMemcpyAsync(force, ctx->alm_force, 3 * (size_t)n * sizeof(double), kf, ctx->stream));
+  CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
   return GKS_OK;
 }
 

@@ -45,6 +45,15 @@ struct GksPhys {
   int bc[6];
 };
 
+/* on-line actuator-line rotor handed to the kernel by value; table pointers are device memory */
+struct GksRotor {
+  int nb, np, npolar, fs_corr, tip_corr;
+  double hub[3], R, rhub, omega, theta0, uref;
+  const double *chord, *twist, *alpha, *cl, *cd;
+};
+#define GKS_MAX_ROTOR_STATIONS 4096
+#define GKS_MAX_POLAR 1024
+
 struct gks_ctx {
   gks_config cfg;
   GksGrid g;
@@ -76,6 +85,10 @@ struct gks_ctx {
   int n_alm;
   double alm_eps;
   int alm_lo[3], alm_cnt[3];   /* bounding box of the ALM support in (unwrapped) cell indices */
+  GksRotor rotor;              /* valid when rotor_on */
+  int rotor_on;
+  double rotor_time;           /* rotor clock: 0 at alm_set_rotor, + dt per step */
+  double *rotor_tab;           /* device: chord, twist (GKS_MAX_ROTOR_STATIONS each), alpha, cl, cd (GKS_MAX_POLAR each) */
   int n_ibm;
   int ibm_maxit;               /* multi-direct-forcing passes per step (1 = single pass) */
   double ibm_tol;              /* stop once max_p |v_p - U_p| < tol, from the second pass on */
@@ -135,6 +148,8 @@ int gks_launch_alm(const GksGrid &g, double *W, int n, const double *pos, const 
                    double dt, const int lo[3], const int cnt[3], cudaStream_t s);
 int gks_launch_cfl_dt(const GksGrid &g, const double *W, double cfl, double dmin, double cs, double *scratch,
                       cudaStream_t s);
+int gks_launch_rotor_forces(const GksGrid &g, const double *W, const GksRotor &r, double time, double eps,
+                            double *pos, double *force, cudaStream_t s);
 int gks_launch_check_finite(const GksGrid &g, const double *W, int *flag, cudaStream_t s);
 
 #endif

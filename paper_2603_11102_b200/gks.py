@@ -18,9 +18,17 @@ STATUS = {0: "GKS_OK", 1: "GKS_ERR_INVALID_ARG", 2: "GKS_ERR_WORKSPACE", 3: "GKS
           4: "GKS_ERR_STATE", 5: "GKS_ERR_NONFINITE"}
 
 EXPORTS = ["gks_workspace_bytes", "gks_create", "gks_destroy", "gks_set_state", "gks_get_state", "gks_step",
-           "gks_set_body_force", "gks_set_bulk_flux", "alm_set_points", "ibm_set_points", "ibm_set_velocities", "ibm_set_iterations", "gks_cfl_dt",
+           "gks_set_body_force", "gks_set_bulk_flux", "alm_set_points", "ibm_set_points", "ibm_set_velocities", "ibm_set_iterations", "gks_cfl_dt", "alm_set_rotor", "alm_rotor_eval",
            "gks_debug_eval_flux", "gks_debug_set_sweep", "gks_debug_fp64_peak",
            "gks_profile_enable", "gks_profile_read", "gks_check_finite", "gks_launch_count", "gks_last_error"]
+
+
+class AlmRotor(C.Structure):
+    _fields_ = [("nblades", C.c_int), ("npts", C.c_int), ("hub", C.c_double * 3),
+                ("R", C.c_double), ("r_hub", C.c_double), ("omega", C.c_double), ("theta0", C.c_double),
+                ("u_ref", C.c_double), ("eps", C.c_double), ("chord", _dp), ("twist", _dp),
+                ("npolar", C.c_int), ("alpha", _dp), ("cl", _dp), ("cd", _dp),
+                ("freestream_correction", C.c_int), ("tip_correction", C.c_int)]
 
 
 class GksConfig(C.Structure):
@@ -61,6 +69,8 @@ def lib():
         L.ibm_set_velocities.argtypes = [vp, vp]
         L.ibm_set_iterations.argtypes = [vp, C.c_int, C.c_double]
         L.gks_cfl_dt.argtypes = [vp, C.c_double, vp]
+        L.alm_set_rotor.argtypes = [vp, C.POINTER(AlmRotor)]
+        L.alm_rotor_eval.argtypes = [vp, vp, vp]
         L.gks_debug_eval_flux.argtypes = [vp, C.c_int, vp, vp]
         L.gks_debug_set_sweep.argtypes = [vp, C.c_int]
         L.gks_check_finite.argtypes = [vp]
@@ -197,6 +207,28 @@ class Gks:
         pw, k2 = _ptr(weights)
         self._check(lib().ibm_set_points(self._h, n, pp, pw))
         self.n_ibm = n
+
+    def alm_set_rotor(self, r):
+        """r: workloads.Rotor (duck-typed) or None to clear; tables are copied by the library during the call"""
+        if r is None:
+            self._check(lib().alm_set_rotor(self._h, None))
+            self._rotor_n = 0
+            return
+        keep = [np.ascontiguousarray(np.asarray(x, dtype=np.float64)) for x in (r.chord, r.twist, r.alpha, r.cl, r.cd)]
+        c = AlmRotor()
+        c.nblades, c.npts = r.nblades, r.npts
+        c.hub = (C.c_double * 3)(*r.hub)
+        c.R, c.r_hub, c.omega, c.theta0, c.u_ref, c.eps = r.R, r.r_hub, r.omega, r.theta0, r.u_ref, r.eps
+        c.chord, c.twist, c.alpha, c.cl, c.cd = [x.ctypes.data_as(_dp) for x in keep]
+        c.npolar = len(keep[2])
+        c.freestream_correction, c.tip_correction = int(r.freestream_correction), int(r.tip_correction)
+        self._check(lib().alm_set_rotor(self._h, C.byref(c)))
+        self._rotor_n = r.nblades * r.npts
+
+    def alm_rotor_eval(self):
+        pos, force = np.empty((self._rotor_n, 3)), np.empty((self._rotor_n, 3))
+        self._check(lib().alm_rotor_eval(self._h, pos.ctypes.data, force.ctypes.data))
+        return pos, force
 
     def cfl_dt(self, cfl, out=None):
         """dt of PAPER.md:91 for the current state; out = a 1-element torch CUDA tensor keeps the call asynchronous"""

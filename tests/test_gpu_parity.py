@@ -227,3 +227,48 @@ def test_cfl_dt_matches_the_oracle():
             g.cfl_dt(-1.0)
         g.close()
         o.close()
+
+
+@pytest.mark.parametrize("switches", [{}, {"freestream_correction": True, "tip_correction": True}])
+def test_online_rotor_matches_the_oracle(switches):
+    """actuator-line front half on the device (S26-S27): point positions and forces of the test hook, then 1 and
+    10 steps of the small rotor (C4) and turbine (C5: rotor + IBM nacelle and tower) boxes with the rotor on line"""
+    from oracle import binding as ob
+    from paper_2603_11102_b200 import gks
+    for name in ("C4", "C5"):
+        w = wl.by_name(name, small=True)
+        pos0, _, eps = w.alm(0)
+        hub = pos0.reshape(3, -1, 3).mean(axis=(0, 1))          # the prescribed blades are 120 degrees apart
+        Rr = np.linalg.norm(pos0 - hub, axis=1).max() * 64.5 / 64.0
+        r = wl.synthetic_rotor(hub=hub, R=float(Rr), eps=eps, npts=48, **switches)
+        for steps, tol in ((1, TOL1), (10, TOL10)):
+            o, g = ob.Oracle(w.cfg), gks.Gks(w.cfg)
+            for s in (o, g):
+                if w.ibm is not None:
+                    s.ibm_set_points(*w.ibm)
+                s.set_state(w.W0)
+                s.alm_set_rotor(r)
+            if steps == 1:
+                po, fo = o.alm_rotor_eval()
+                pg, fg = g.alm_rotor_eval()
+                assert np.abs(pg - po).max() <= 1e-14 * np.abs(po).max()
+                assert np.abs(fg - fo).max() <= 1e-12 * np.abs(fo).max() and np.abs(fo).max() > 0
+            for _ in range(steps):
+                o.step(w.dt)
+                g.step(w.dt)
+            e = rel_linf(g.get_state(), o.get_state())
+            assert e <= tol, (name, steps, e)
+            if steps == 10:       # the clocks agree: the blades have turned by omega * 10 dt on both sides
+                po, fo = o.alm_rotor_eval()
+                pg, fg = g.alm_rotor_eval()
+                assert np.abs(pg - po).max() <= 1e-13 * np.abs(po).max()
+                assert np.abs(fg - fo).max() <= 1e-9 * np.abs(fo).max()
+            g.close()
+            o.close()
+    g = gks.Gks(wl.by_name("C4", small=True).cfg)
+    bad = wl.synthetic_rotor(hub=(1, 1, 1), R=0.5, eps=0.1)
+    bad.alpha = bad.alpha[::-1].copy()
+    with pytest.raises(gks.GksError):
+        g.alm_set_rotor(bad)
+    g.alm_set_rotor(None)
+    g.close()
