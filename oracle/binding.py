@@ -75,6 +75,9 @@ def lib():
         L.gkso_weno5_face.restype = C.c_double
         L.gkso_weno5_gauss.argtypes = [_dp, C.c_double, _dp]
         L.gkso_weno5_gauss.restype = None
+        L.gkso_linear5_gauss.argtypes = [_dp, _dp]
+        L.gkso_linear5_gauss.restype = None
+        L.gkso_set_reconstruction.argtypes = [vp, C.c_int]
         L.gkso_quartic_slope_gauss.argtypes = [_dp, _dp]
         L.gkso_quartic_slope_gauss.restype = None
         L.gkso_normal_slope.argtypes = [_dp]
@@ -177,6 +180,9 @@ class Oracle:
         _check(lib().gkso_ibm_set_points(self._h, len(pos), _p(pos), _p(weights)))
         self.n_ibm = len(pos)
 
+    def set_reconstruction(self, tangential_linear):
+        _check(lib().gkso_set_reconstruction(self._h, int(tangential_linear)))
+
     def ibm_set_iterations(self, max_iter, tol=0.0):
         _check(lib().gkso_ibm_set_iterations(self._h, int(max_iter), float(tol)))
 
@@ -269,6 +275,12 @@ def weno5_face(q, eps=1e-6):
 def weno5_gauss(q, eps=1e-6):
     q, out = _arr(q), np.empty(2)
     lib().gkso_weno5_gauss(_p(q), eps, _p(out))
+    return out
+
+
+def linear5_gauss(q):
+    q, out = _arr(q), np.empty(2)
+    lib().gkso_linear5_gauss(_p(q), _p(out))
     return out
 
 

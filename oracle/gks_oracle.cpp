@@ -120,11 +120,35 @@ double weno5_gauss_plus(const double q[5], double eps) {
   return js_combine(p, d, beta, eps);
 }
 
+/* The same candidates combined with the LINEAR weights d_k (reading S7's alternative): the value
+ * at the Gauss point of the quartic through all five averages. */
+double linear5_gauss_plus(const double q[5]) {
+  const double s3 = std::sqrt(3.0);
+  const double p[3] = {s3 / 12.0 * q[0] - s3 / 3.0 * q[1] + (1.0 + s3 / 4.0) * q[2],
+                       -s3 / 12.0 * q[1] + q[2] + s3 / 12.0 * q[3],
+                       (1.0 - s3 / 4.0) * q[2] + s3 / 3.0 * q[3] - s3 / 12.0 * q[4]};
+  const double d[3] = {(210.0 - s3) / 1080.0, 11.0 / 18.0, (210.0 + s3) / 1080.0};
+  return d[0] * p[0] + d[1] * p[1] + d[2] * p[2];
+}
+
+/* tangential reconstruction of one field: WENO5-JS (S7) or, with `linear`, the linear-weight variant */
+void tangential_gauss(const double q[5], double eps, bool linear, double out[2]);
+
 /* values at (-sqrt(3)/6, +sqrt(3)/6); the minus point is the mirror image (reverse the stencil) */
 void weno5_gauss(const double q[5], double eps, double out[2]) {
   const double qr[5] = {q[4], q[3], q[2], q[1], q[0]};
   out[0] = weno5_gauss_plus(qr, eps);
   out[1] = weno5_gauss_plus(q, eps);
+}
+
+void tangential_gauss(const double q[5], double eps, bool linear, double out[2]) {
+  if (!linear) {
+    weno5_gauss(q, eps, out);
+    return;
+  }
+  const double qr[5] = {q[4], q[3], q[2], q[1], q[0]};
+  out[0] = linear5_gauss_plus(qr);
+  out[1] = linear5_gauss_plus(q);
 }
 
 /* derivative at x = +-sqrt(3)/6 of the quartic whose 5 cell averages are q, per unit cell width (S8) */
@@ -341,6 +365,7 @@ struct gkso_ctx {
     double hub[3] = {0, 0, 0}, R = 0, rhub = 0, omega = 0, theta0 = 0, uref = 0, time = 0;
     std::vector<double> chord, twist, pa, pcl, pcd;
   } rotor;
+  bool tangential_linear = false; /* scheme variant: linear weights in the two tangential passes (f4) */
   int ibm_maxit = 1;       /* multi-direct-forcing passes per step; 1 = single pass (S15) */
   double ibm_tol = 0.0;    /* stop once max_p |v_p - U_p| < tol (checked from the second pass on) */
 
@@ -502,7 +527,7 @@ void face_flux(const gkso_ctx &s, const std::vector<double> &W, int dir, std::ve
         for (int fld = 0; fld < 8; ++fld) {
           double q[5], v[2];
           for (int m = 0; m < 5; ++m) q[m] = NQ[fb.at(f, i1 - 2 + m, i2) * 8 + fld];
-          weno5_gauss(q, eps, v);
+          tangential_gauss(q, eps, s.tangential_linear, v);
           o[0 * 12 + fld] = v[0];
           o[1 * 12 + fld] = v[1];
           if (fld < 4) { /* slope of Q0 along t1 */
@@ -528,7 +553,7 @@ void face_flux(const gkso_ctx &s, const std::vector<double> &W, int dir, std::ve
           for (int fld = 0; fld < 12; ++fld) {
             double q[5];
             for (int m = 0; m < 5; ++m) q[m] = T1[fb.at(f, i1, i2 - 2 + m) * 24 + g1 * 12 + fld];
-            weno5_gauss(q, eps, val[fld]);
+            tangential_gauss(q, eps, s.tangential_linear, val[fld]);
             if (fld < 4) {
               quartic_slope_gauss(q, Dt2[fld]);
               Dt2[fld][0] /= A2.w(i2);
@@ -1052,6 +1077,13 @@ int gkso_ibm_set_points(gkso_ctx *s, int n, const double *pos, const double *wei
   return 0;
 }
 
+int gkso_set_reconstruction(gkso_ctx *s, int tangential_linear) {
+  if (!s) return fail("null argument");
+  if (tangential_linear != 0 && tangential_linear != 1) return fail("tangential_linear must be 0 or 1");
+  s->tangential_linear = tangential_linear != 0;
+  return 0;
+}
+
 int gkso_ibm_set_iterations(gkso_ctx *s, int max_iter, double tol) {
   if (!s) return fail("null argument");
   if (max_iter < 1 || !(tol >= 0.0)) return fail("ibm: max_iter must be >= 1 and tol >= 0");
@@ -1191,6 +1223,7 @@ void gkso_micro_solve(double U, double V, double W, double lambda, const double 
 }
 double gkso_weno5_face(const double q[5], double eps) { return weno5_face(q, eps); }
 void gkso_weno5_gauss(const double q[5], double eps, double out[2]) { weno5_gauss(q, eps, out); }
+void gkso_linear5_gauss(const double q[5], double out[2]) { tangential_gauss(q, 0.0, true, out); }
 void gkso_quartic_slope_gauss(const double q[5], double out[2]) { quartic_slope_gauss(q, out); }
 double gkso_normal_slope(const double q[4]) { return normal_slope(q); }
 void gkso_collision(const double Ql[4], const double Qr[4], int dir, double RT, double Q0[4]) {

@@ -44,6 +44,9 @@ int gkso_alm_set_points(gkso_ctx *ctx, int n, const double *pos, const double *f
 int gkso_alm_set_cut(gkso_ctx *ctx, double cut_in_eps); /* test flag: radius of the cut in units of eps (default 3; <=0 => no cut) */
 int gkso_ibm_set_points(gkso_ctx *ctx, int n, const double *pos, const double *weights);
 int gkso_ibm_set_velocities(gkso_ctx *ctx, const double *vel);
+/* scheme variant (the alternative of reading S7): 1 = the two tangential passes combine the
+ * sub-stencil candidates with the linear weights (quartic interpolation); 0 = WENO5-JS everywhere (default) */
+int gkso_set_reconstruction(gkso_ctx *ctx, int tangential_linear);
 /* multi-direct-forcing passes per step (Eq. 11-12; S25); default 1, tol 0 */
 int gkso_ibm_set_iterations(gkso_ctx *ctx, int max_iter, double tol);
 /* face-averaged F and dF/dt of the current state, direction dir; F[c][k][j][i] with n_dir+1 faces along dir */
@@ -85,6 +88,7 @@ void gkso_micro_solve(double U, double V, double W, double lambda, const double 
 double gkso_weno5_face(const double q[5], double eps);
 /* WENO5-JS values at the two Gauss points -sqrt(3)/6, +sqrt(3)/6 of the middle cell (S7) */
 void gkso_weno5_gauss(const double q[5], double eps, double out[2]);
+void gkso_linear5_gauss(const double q[5], double out[2]);
 /* derivative (per unit cell width) of the quartic through 5 averages at the two Gauss points (S8) */
 void gkso_quartic_slope_gauss(const double q[5], double out[2]);
 /* index-space normal slope at the face between q[1] and q[2] from 4 averages q[0..3] (S5) */

@@ -572,3 +572,47 @@ def test_P17_rotor_step_equals_prescribed_points_step():
     assert np.array_equal(dM_rotor, o.eval_forcing(0.02))
     assert np.abs(dM_rotor).max() > 0
     o.close()
+
+
+# ---------------------------------------------------------------- P18 linear-weight tangential variant (f4)
+def test_P18_linear_tangential_variant():
+    """the variant's operator is the quartic through the five averages: SURVEY's Gauss-point value row, exact for
+    cell averages of polynomials up to degree 4 whatever their smoothness indicators, the limit eps -> large of
+    WENO-JS; the step keeps the free stream, conserves, is fourth-order on the simple wave and equals the WENO
+    step on data that vary along one axis only up to the normal reconstruction"""
+    s3 = math.sqrt(3.0)
+    row = np.array([-1 / 4320 + 7 * s3 / 432, 1 / 1080 - 25 * s3 / 216, 719 / 720, 1 / 1080 + 25 * s3 / 216,
+                    -1 / 4320 - 7 * s3 / 432])
+    rng = np.random.default_rng(2)
+    for _ in range(5):
+        q = rng.standard_normal(5)
+        vm, vp = ob.linear5_gauss(q)
+        assert vp == pytest.approx(row @ q, rel=1e-13, abs=1e-15) and vm == pytest.approx(row[::-1] @ q, rel=1e-13, abs=1e-15)
+        assert np.allclose(ob.weno5_gauss(q, eps=1e12), [vm, vp], rtol=1e-10)
+    # exact on cell averages of a quartic with an O(1) kink-free but steep profile (nonlinear weights would bias it)
+    poly = np.polynomial.Polynomial(rng.standard_normal(5) * [1, 3, 5, 7, 9])
+    A = poly.integ()
+    q = np.array([A(m + 0.5) - A(m - 0.5) for m in range(-2, 3)])
+    vm, vp = ob.linear5_gauss(q)
+    assert vp == pytest.approx(poly(s3 / 6), rel=1e-12) and vm == pytest.approx(poly(-s3 / 6), rel=1e-12)
+    assert abs(ob.weno5_gauss(q)[1] - poly(s3 / 6)) > 1e-6 * abs(poly(s3 / 6))
+    lin = lambda o: o.set_reconstruction(1)
+    # free stream and conservation
+    n = (8, 7, 6)
+    cfg = GridConfig(n=n, spacing=(0.1, 0.12, 0.09), nu=1e-3, bc=(P,) * 6)
+    W0 = const_state(n, (1.1, 0.11, -0.05, 0.02))
+    assert np.array_equal(run(cfg, W0, 0.02, 2, setup=lin), W0)
+    W0 = W0 * (1 + 0.01 * rng.standard_normal(W0.shape))
+    W = run(cfg, W0, 0.02, 1, setup=lin)
+    assert np.allclose(W.reshape(4, -1).sum(1), W0.reshape(4, -1).sum(1), rtol=1e-13, atol=1e-13)
+    assert not np.array_equal(W, run(cfg, W0, 0.02, 1))                   # it IS a different scheme
+    # order of accuracy on the exact simple wave (P8's solution)
+    def err(nn):
+        c = GridConfig(n=(nn, nn, nn), spacing=(2 * math.pi / nn,) * 3, nu=0.0, bc=(P,) * 6)
+        steps = math.ceil(1.0 / (0.4 * (2 * math.pi / nn) / 1.1))
+        Wn = run(c, simple_wave_exact(nn, 0.0), 1.0 / steps, steps, setup=lin)
+        return np.abs(Wn[0] - simple_wave_exact(nn, 1.0)[0]).mean()
+    e16, e32 = err(16), err(32)
+    assert math.log2(e16 / e32) >= 3.5 and e32 < 2e-6
+    with pytest.raises(ob.OracleError):
+        ob.Oracle(cfg).set_reconstruction(2)
