@@ -32,6 +32,9 @@ UNIT = "Mcell-steps/s"
 # erfc/exp/sqrt, smoothness indicators shared between the two points of a cell, Navier-Stokes closed
 # form for the Gauss-point flux): per face 4726 (stage 1) + 4654 (stage 2), 3 faces per cell, + update.
 FLOPS_PER_FACE = {True: 4726.0, False: 4654.0}     # need_F (stage 1) / dF only (stage 2)
+# linear-weight tangential variant (--variant linear): an evaluation is 3 candidates x 5 + 5 = 20 flops per value,
+# pass 1 = 8 fields x 40 + 4 slopes x 20 = 400, pass 2 = 24 x 40 + 8 x 20 = 1120, normal phase 518, flux 416 / 344
+FLOPS_PER_FACE_LINEAR = {True: 2454.0, False: 2382.0}
 FLOPS_PER_CELL_STEP = 3 * (FLOPS_PER_FACE[True] + FLOPS_PER_FACE[False]) + 60.0
 
 
@@ -140,6 +143,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="M0")
     ap.add_argument("--sweep", type=int, default=0, help="0 fused (production), 1 unfused cross-check kernels")
+    ap.add_argument("--variant", default="weno", choices=["weno", "linear"],
+                    help="weno: the scheme as read from the paper (default, the metric); linear: linear-weight tangential passes")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
     args = ap.parse_args()
@@ -168,6 +173,8 @@ def main():
     w = wl.by_name(args.workload)
     g = setup_solver(w, gks, device)
     g.debug_set_sweep(args.sweep)
+    if args.variant == "linear":
+        g.set_reconstruction(1)
     cells = w.cfg.cells
     with torch.cuda.stream(g.stream):
         Wd = torch.from_numpy(w.W0).to(device)
@@ -235,11 +242,12 @@ def main():
         sweep_ms = sum(prof[k][0] for k in ("sweep_x", "sweep_y", "sweep_z"))
         sweep_n = sum(prof[k][1] for k in ("sweep_x", "sweep_y", "sweep_z"))
         faces = cells  # one face per cell and direction (+ one boundary plane, < 0.5 %)
-        flops_per_launch = 0.5 * (FLOPS_PER_FACE[True] + FLOPS_PER_FACE[False]) * faces
+        fpf = FLOPS_PER_FACE_LINEAR if args.variant == "linear" else FLOPS_PER_FACE
+        flops_per_launch = 0.5 * (fpf[True] + fpf[False]) * faces
         ach = flops_per_launch / (sweep_ms / max(sweep_n, 1) * 1e-3) / 1e12 if sweep_ms > 0 else None
         traffic = None
         tps = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_traffic.csv")))
-        if tps and args.workload == "M0" and args.sweep == 0:
+        if tps and args.workload == "M0" and args.sweep == 0 and args.variant == "weno":
             with open(tps[-1]) as f:      # latest round's ncu --set full capture (text summary, not executed)
                 for row in csv.DictReader(f):
                     if row["kernel"] == "sweep_mean_of_6":
@@ -249,7 +257,7 @@ def main():
             "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": "%s %s %dx%dx%d" % (args.workload, w.name, *w.cfg.n),
-                       "sweep": "fused" if args.sweep == 0 else "unfused",
+                       "sweep": "fused" if args.sweep == 0 else "unfused", "variant": args.variant,
                        "multi_gpu": "replicas only" if world > 1 else "single GPU",
                        "l2": "inputs larger than L2 (state %.0f MB per field set)" % (cells * 32 / 1e6)},
             "clocks": clocks,

@@ -146,6 +146,12 @@ gks_status ibm_set_velocities(gks_ctx *ctx, const double *vel /* n*3, or NULL =>
  * Default max_iter = 1, tol = 0 (single pass).  1 <= max_iter <= 64, tol >= 0, else GKS_ERR_INVALID_ARG. */
 gks_status ibm_set_iterations(gks_ctx *ctx, int max_iter, double tol);
 
+/* Scheme variant for cost comparison (the alternative of DESIGN.md reading S7): with
+ * tangential_linear = 1 the two tangential passes combine the sub-stencil candidates with the LINEAR weights
+ * (quartic interpolation to the Gauss points) instead of the WENO5-JS nonlinear ones; the normal reconstruction,
+ * the slopes and everything else are unchanged.  Default 0.  Other values: GKS_ERR_INVALID_ARG. */
+gks_status gks_set_reconstruction(gks_ctx *ctx, int tangential_linear);
+
 /* Time step of the CFL condition: dt = cfl * min{dx, dy, dz} / (|U|_max + sqrt(RT)), |U|_max over
  * the interior cells of the current state (one reduction kernel), the minimum over every cell width.
  * `dt` may be a host pointer (the call then synchronises the stream) or a device pointer (asynchronous).

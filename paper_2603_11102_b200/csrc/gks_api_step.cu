@@ -326,6 +326,14 @@ gks_status ibm_set_points(gks_ctx *ctx, int n, const double *pos, const double *
   return GKS_OK;
 }
 
+gks_status gks_set_reconstruction(gks_ctx *ctx, int tangential_linear) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (tangential_linear != 0 && tangential_linear != 1)
+    return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "tangential_linear must be 0 or 1");
+  ctx->ph.tang_linear = tangential_linear;
+  return GKS_OK;
+}
+
 gks_status ibm_set_iterations(gks_ctx *ctx, int max_iter, double tol) {
   if (!ctx) return GKS_ERR_INVALID_ARG;
   if (max_iter < 1 || max_iter > GKS_IBM_MAX_PASSES || !(tol >= 0.0) || !std::isfinite(tol))

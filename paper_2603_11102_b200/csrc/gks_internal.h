@@ -43,6 +43,7 @@ struct GksPhys {
   double theta, cx;                /* sqrt(lambda), 1/(2 sqrt(pi lambda)): collision constants */
   double inflow[4];
   int bc[6];
+  int tang_linear;                 /* scheme variant: linear weights in the tangential passes */
 };
 
 /* on-line actuator-line rotor handed to the kernel by value; table pointers are device memory */

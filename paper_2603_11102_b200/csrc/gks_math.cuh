@@ -36,7 +36,8 @@ static __constant__ double GKC[16] = {
     -((1.0 / 12.0 - GKS_SQRT3 / 54.0) + (-2.0 / 3.0 + 13.0 * GKS_SQRT3 / 54.0)), /* 7  e2 = -(k0+k1) */
     (2.0 / 3.0 + 13.0 * GKS_SQRT3 / 54.0) + (-1.0 / 12.0 - GKS_SQRT3 / 54.0),    /* 8  e3 = k3+k4 */
     -1.0 / 12.0 - GKS_SQRT3 / 54.0,                                       /* 9  e4 = k4 */
-    0, 0, 0, 0, 0, 0};
+    (GKS_SQRT3 / 12.0) * (11.0 / 18.0),                 /* 10 h dB: linear-weight variant */
+    0, 0, 0, 0, 0};
 
 /* reciprocal to fp64 round-off: hardware seed (2^-23) + two Newton steps, no slow path */
 __device__ __forceinline__ double fast_rcp(double x) {
@@ -176,7 +177,7 @@ __device__ __forceinline__ void weno5_edges_v(const double (&q)[5][N], double ep
 /* WENO5-JS values at the Gauss points (vm at -sqrt(3)/6, vp at +sqrt(3)/6; S7) and the derivative of
  * the quartic through the 5 averages there (S8; per unit cell width; dead code when unused), N stencils.
  * At x^2 = 1/12 the quadratic term of every candidate vanishes: candidate k is q2 +- (x_G/2) g_k. */
-template <int N>
+template <int N, bool LIN = false>
 __device__ __forceinline__ void weno5_gauss_v(const double (&q)[5][N], double eps, double (&vm)[N], double (&vp)[N],
                                               double (&sm)[N], double (&sp)[N]) {
   double D1[N], D2[N], D3[N], D4[N];
@@ -186,6 +187,20 @@ __device__ __forceinline__ void weno5_gauss_v(const double (&q)[5][N], double ep
     D2[n] = q[2][n] - q[1][n];
     D3[n] = q[3][n] - q[2][n];
     D4[n] = q[4][n] - q[3][n];
+  }
+  if (LIN) {
+    /* scheme variant: the candidates q2 +- h g_k combined with the LINEAR weights (quartic interpolation) */
+    const double dA = GKC[1], dC = GKC[2], hb = GKC[10];
+    const double e1 = GKC[6], e2 = GKC[7], e3 = GKC[8], e4 = GKC[9];
+#pragma unroll
+    for (int n = 0; n < N; ++n) {
+      const double g0 = fma(3.0, D2[n], -D1[n]), g1 = D2[n] + D3[n], g2 = fma(3.0, D3[n], -D4[n]);
+      vp[n] = fma(hb, fma(dA, g0, fma(dC, g2, g1)), q[2][n]);
+      vm[n] = fma(-hb, fma(dC, g0, fma(dA, g2, g1)), q[2][n]);
+      sp[n] = fma(e4, D4[n], fma(e3, D3[n], fma(e2, D2[n], e1 * D1[n])));
+      sm[n] = fma(e1, D4[n], fma(e2, D3[n], fma(e3, D2[n], e4 * D1[n])));
+    }
+    return;
   }
   JsFrontV<N> f;
   js_front_v<N>(D1, D2, D3, D4, eps, f);
@@ -227,10 +242,11 @@ __device__ __forceinline__ void weno5_edges(double q0, double q1, double q2, dou
   vr = r[0];
 }
 __device__ __forceinline__ void weno5_gauss(double q0, double q1, double q2, double q3, double q4,
-                                            double eps, double &vm, double &vp) {
+                                            double eps, double &vm, double &vp, bool linear = false) {
   const double q[5][1] = {{q0}, {q1}, {q2}, {q3}, {q4}};
   double m[1], p[1], a[1], b[1];
-  weno5_gauss_v<1>(q, eps, m, p, a, b);
+  if (linear) weno5_gauss_v<1, true>(q, eps, m, p, a, b);
+  else weno5_gauss_v<1, false>(q, eps, m, p, a, b);
   vm = m[0];
   vp = p[0];
 }

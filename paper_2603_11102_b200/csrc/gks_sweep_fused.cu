@@ -140,7 +140,7 @@ struct Seg {
  * the next iteration, after its EF (about half of the iteration's arithmetic) - warps may drift by half
  * an iteration without anyone waiting.
  */
-template <int DIR, bool NEED_F, int TA, int TB>
+template <int DIR, bool NEED_F, bool LIN, int TA, int TB>
 __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
     k_sweep_fused(const __grid_constant__ CUtensorMap tmap, GksGrid g, GksPhys ph, double *__restrict__ flux,
                   int ncol_a, int nfull, long long rem, long long PPC) {
@@ -366,7 +366,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
         qq[k][0] = q[(k - 2) * s1 * 4];
         qq[k][1] = d[(k - 2) * s1 * 4];
       }
-      gksd::weno5_gauss_v<2>(qq, eps, vm, vp, sm_, sp_);
+      gksd::weno5_gauss_v<2, LIN>(qq, eps, vm, vp, sm_, sp_);
       d6[0] = vm[0];
       d6[1] = vp[0];
       d6[2] = vm[1];
@@ -411,7 +411,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
       }
 #pragma unroll
       for (int u = 0; u < EW; ++u) rnew[(e0 + u) * RF] = d6[e0 + u];   /* rs[0] aliases rnew: stored after the loads */
-      gksd::weno5_gauss_v<EW>(qq, eps, vm, vp, sm_, sp_);
+      gksd::weno5_gauss_v<EW, LIN>(qq, eps, vm, vp, sm_, sp_);
 #pragma unroll
       for (int u = 0; u < EW; ++u) {              /* evaluation e = 2*fld + g1; Gauss point gq = 2*g1 + g2 */
         const int fld = (e0 + u) >> 1, g1 = (e0 + u) & 1;
@@ -496,12 +496,12 @@ bool encode_dir(encode_fn_t enc, const GksGrid &g, double *base, CUtensorMap *ou
              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-template <int DIR, bool NEED_F>
+template <int DIR, bool NEED_F, bool LIN>
 int launch_dir(gks_ctx *ctx, const CUtensorMap &map, double *flux) {
   constexpr int TA = Shape<DIR>::TA, TB = Shape<DIR>::TB;
   using T = Tile<DIR, TA, TB>;
   const GksGrid &g = ctx->g;
-  auto kern = k_sweep_fused<DIR, NEED_F, TA, TB>;
+  auto kern = k_sweep_fused<DIR, NEED_F, LIN, TA, TB>;
   static bool attr_done = false;
   if (!attr_done) {
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES);
@@ -551,9 +551,14 @@ bool gks_fused_init(gks_ctx *ctx) {
 
 int gks_launch_sweep_fused(gks_ctx *ctx, int dir, int which, double *flux, bool need_F) {
   const CUtensorMap &m = *reinterpret_cast<const CUtensorMap *>(ctx->tmaps[which][dir]);
+  const bool lin = ctx->ph.tang_linear != 0;
+#define GKS_DISPATCH(D)                                                                                   \
+  (need_F ? (lin ? launch_dir<D, true, true>(ctx, m, flux) : launch_dir<D, true, false>(ctx, m, flux))  \
+          : (lin ? launch_dir<D, false, true>(ctx, m, flux) : launch_dir<D, false, false>(ctx, m, flux)))
   switch (dir) {
-    case 0: return need_F ? launch_dir<0, true>(ctx, m, flux) : launch_dir<0, false>(ctx, m, flux);
-    case 1: return need_F ? launch_dir<1, true>(ctx, m, flux) : launch_dir<1, false>(ctx, m, flux);
-    default: return need_F ? launch_dir<2, true>(ctx, m, flux) : launch_dir<2, false>(ctx, m, flux);
+    case 0: return GKS_DISPATCH(0);
+    case 1: return GKS_DISPATCH(1);
+    default: return GKS_DISPATCH(2);
   }
+#undef GKS_DISPATCH
 }

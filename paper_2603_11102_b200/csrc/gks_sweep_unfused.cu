@@ -71,7 +71,7 @@ __global__ void __launch_bounds__(256) k_pass1(GksGrid g, GksPhys ph, Box3 box, 
     const double *q = N + f * g.FS + id;
     const double q0 = q[-2 * s1], q1 = q[-s1], q2 = q[0], q3 = q[s1], q4 = q[2 * s1];
     double vm, vp;
-    gksd::weno5_gauss(q0, q1, q2, q3, q4, ph.weno_eps, vm, vp);
+    gksd::weno5_gauss(q0, q1, q2, q3, q4, ph.weno_eps, vm, vp, ph.tang_linear != 0);
     T[(0 * 12 + f) * g.FS + id] = vm;
     T[(1 * 12 + f) * g.FS + id] = vp;
     if (f < 4) {
@@ -100,7 +100,7 @@ __global__ void __launch_bounds__(256) k_pass2(GksGrid g, GksPhys ph, Box3 box, 
     for (int f = 0; f < 12; ++f) {
       const double *q = T + (g1 * 12 + f) * g.FS + id;
       const double q0 = q[-2 * s2], q1 = q[-s2], q2 = q[0], q3 = q[s2], q4 = q[2 * s2];
-      gksd::weno5_gauss(q0, q1, q2, q3, q4, ph.weno_eps, v[f][0], v[f][1]);
+      gksd::weno5_gauss(q0, q1, q2, q3, q4, ph.weno_eps, v[f][0], v[f][1], ph.tang_linear != 0);
       if (f < 4) {
         gksd::quartic_slope_gauss(q0, q1, q2, q3, q4, d2[f][0], d2[f][1]);
         d2[f][0] *= iw;

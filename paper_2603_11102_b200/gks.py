@@ -18,7 +18,7 @@ STATUS = {0: "GKS_OK", 1: "GKS_ERR_INVALID_ARG", 2: "GKS_ERR_WORKSPACE", 3: "GKS
           4: "GKS_ERR_STATE", 5: "GKS_ERR_NONFINITE"}
 
 EXPORTS = ["gks_workspace_bytes", "gks_create", "gks_destroy", "gks_set_state", "gks_get_state", "gks_step",
-           "gks_set_body_force", "gks_set_bulk_flux", "alm_set_points", "ibm_set_points", "ibm_set_velocities", "ibm_set_iterations", "gks_cfl_dt", "alm_set_rotor", "alm_rotor_eval",
+           "gks_set_body_force", "gks_set_bulk_flux", "alm_set_points", "ibm_set_points", "ibm_set_velocities", "ibm_set_iterations", "gks_cfl_dt", "alm_set_rotor", "alm_rotor_eval", "gks_set_reconstruction",
            "gks_debug_eval_flux", "gks_debug_set_sweep", "gks_debug_fp64_peak",
            "gks_profile_enable", "gks_profile_read", "gks_check_finite", "gks_launch_count", "gks_last_error"]
 
@@ -71,6 +71,7 @@ def lib():
         L.gks_cfl_dt.argtypes = [vp, C.c_double, vp]
         L.alm_set_rotor.argtypes = [vp, C.POINTER(AlmRotor)]
         L.alm_rotor_eval.argtypes = [vp, vp, vp]
+        L.gks_set_reconstruction.argtypes = [vp, C.c_int]
         L.gks_debug_eval_flux.argtypes = [vp, C.c_int, vp, vp]
         L.gks_debug_set_sweep.argtypes = [vp, C.c_int]
         L.gks_check_finite.argtypes = [vp]
@@ -229,6 +230,9 @@ class Gks:
         pos, force = np.empty((self._rotor_n, 3)), np.empty((self._rotor_n, 3))
         self._check(lib().alm_rotor_eval(self._h, pos.ctypes.data, force.ctypes.data))
         return pos, force
+
+    def set_reconstruction(self, tangential_linear):
+        self._check(lib().gks_set_reconstruction(self._h, int(tangential_linear)))
 
     def cfl_dt(self, cfl, out=None):
         """dt of PAPER.md:91 for the current state; out = a 1-element torch CUDA tensor keeps the call asynchronous"""

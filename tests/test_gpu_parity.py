@@ -272,3 +272,42 @@ def test_online_rotor_matches_the_oracle(switches):
         g.alm_set_rotor(bad)
     g.alm_set_rotor(None)
     g.close()
+
+
+@pytest.mark.parametrize("sweep", [0, 1])
+def test_linear_tangential_variant_matches_the_oracle(sweep):
+    """scheme variant of SURVEY 8f f4 (linear weights in the two tangential passes): both sweep implementations
+    against the oracle's variant on C1 (1 and 10 steps), the small channel and a ragged mixed-boundary box"""
+    from oracle import binding as ob
+    from paper_2603_11102_b200 import gks
+    rng = np.random.default_rng(12)
+    n = (19, 9, 23)
+    cfg = GridConfig(n=n, spacing=(0.1, 0.12, 0.1), nu=2e-3, bc=(IN, OUT, P, P, NS, SL), inflow=(1.0, 0.1, 0.0, 0.0))
+    W0 = np.empty((4, n[2], n[1], n[0]))
+    W0[0] = 1.0 + 0.02 * rng.standard_normal(W0[0].shape)
+    W0[1:] = 0.1 + 0.03 * rng.standard_normal(W0[1:].shape)
+    cases = [(wl.by_name("C1"), 1, TOL1), (wl.by_name("C1"), 10, TOL10), (wl.by_name("C2", small=True), 3, 10 * TOL1),
+             (wl.Workload("ragged", cfg, W0, wl.cfl_dt(cfg, W0), 3), 3, 10 * TOL1)]
+    for w, steps, tol in cases:
+        o, g = ob.Oracle(w.cfg), gks.Gks(w.cfg)
+        g.debug_set_sweep(sweep)
+        for s in (o, g):
+            s.set_reconstruction(1)
+            if w.bulk_flux is not None:
+                s.set_bulk_flux(*w.bulk_flux)
+            s.set_state(w.W0)
+        for _ in range(steps):
+            o.step(w.dt)
+            g.step(w.dt)
+        Wg = g.get_state()
+        e = rel_linf(Wg, o.get_state())
+        assert e <= tol, (w.name, steps, e)
+        o.close()
+        if steps == 1:      # and it is not the WENO scheme
+            g.set_reconstruction(0)
+            g.set_state(w.W0)
+            g.step(w.dt)
+            assert rel_linf(g.get_state(), Wg) > 1e-9
+            with pytest.raises(gks.GksError):
+                g.set_reconstruction(3)
+        g.close()
