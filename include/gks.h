@@ -61,7 +61,8 @@ typedef enum {
   GKS_BC_WALL_SLIP = 2, /* also "symmetry" */
   GKS_BC_INFLOW = 3,
   GKS_BC_OUTFLOW_CONVECTIVE = 4,
-  GKS_BC_EXTRAPOLATE = 5
+  GKS_BC_EXTRAPOLATE = 5,
+  GKS_BC_HALO = 6 /* cut face of a domain decomposition: the 3 ghost layers are supplied with gks_halo_unpack */
 } gks_bc;
 
 typedef struct {
@@ -96,6 +97,26 @@ gks_status gks_get_state(gks_ctx *ctx, double *W);
  * (PAPER.md:187), then the forcing of Eq. 13: uniform/bulk term, IBM, ALM.  dt > 0.
  * Asynchronous on the context's stream. */
 gks_status gks_step(gks_ctx *ctx, double dt);
+
+/* Domain decomposition (x-slabs over several GPUs).  A sub-domain is an
+ * ordinary context whose cut faces carry GKS_BC_HALO.  Such a face must lie on a uniform axis; a convective
+ * outflow may then only sit on that same axis; gks_set_bulk_flux is refused (it needs a global sum).
+ * The ghost fill leaves HALO ghosts alone; the driver moves them:
+ *   gks_halo_pack(ctx, which, face, buf)   copies the 3 interior planes next to `face` (0..5 = xlo,xhi,ylo,...)
+ *       of state `which` (0: W^n / W^{n+1}, 1: the first-stage state W*) to buf, a DEVICE or host array of
+ *       gks_halo_doubles(ctx, face) doubles laid out [c][layer][v][u] (layer = increasing index along the axis,
+ *       u the lower and v the higher of the two tangential axes, interior cells only);
+ *   gks_halo_unpack(ctx, which, face, buf) writes the 3 ghost planes beyond `face` from such an array (what the
+ *       neighbour packed at its opposite face).
+ * gks_step is split at the two points where a stage needs its neighbours:
+ *   gks_step_begin(ctx, dt)   ghosts of W^n (HALO ghosts must be in place), sweeps, W* and P;
+ *   gks_step_finish(ctx, dt)  ghosts of W* (HALO ghosts of W* must be in place), sweeps, W^{n+1}, forcing.
+ * gks_step = begin + finish.  Errors: GKS_ERR_INVALID_ARG (face without HALO, NULL), GKS_ERR_STATE (order). */
+size_t gks_halo_doubles(const gks_ctx *ctx, int face);
+gks_status gks_halo_pack(gks_ctx *ctx, int which, int face, double *buf);
+gks_status gks_halo_unpack(gks_ctx *ctx, int which, int face, const double *buf);
+gks_status gks_step_begin(gks_ctx *ctx, double dt);
+gks_status gks_step_finish(gks_ctx *ctx, double dt);
 
 /* Uniform acceleration g: momentum += dt * rho * g each step.  (0,0,0) disables. */
 gks_status gks_set_body_force(gks_ctx *ctx, double gx, double gy, double gz);

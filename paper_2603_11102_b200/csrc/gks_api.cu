@@ -51,7 +51,12 @@ const char *validate(const gks_config *c) {
   const double d[3] = {c->dx, c->dy, c->dz};
   for (int a = 0; a < 3; ++a) {
     const int lo = c->bc[2 * a], hi = c->bc[2 * a + 1];
-    if (lo < 0 || lo > 5 || hi < 0 || hi > 5) return "unknown boundary kind";
+    if (lo < 0 || lo > 6 || hi < 0 || hi > 6) return "unknown boundary kind";
+    if ((lo == GKS_BC_HALO || hi == GKS_BC_HALO) && f[a]) return "a HALO face needs a uniform axis";
+    if (lo == GKS_BC_HALO || hi == GKS_BC_HALO)
+      for (int b = 0; b < 3; ++b)
+        if (b != a && (c->bc[2 * b] == GKS_BC_OUTFLOW_CONVECTIVE || c->bc[2 * b + 1] == GKS_BC_OUTFLOW_CONVECTIVE))
+          return "with a HALO face a convective outflow may only sit on the same axis";
     if ((lo == GKS_BC_PERIODIC) != (hi == GKS_BC_PERIODIC)) return "periodic faces must be paired";
     if (f[a]) {
       for (int i = 0; i < n[a]; ++i)

@@ -115,10 +115,11 @@ gks_status gks_get_state(gks_ctx *ctx, double *W) {
   return GKS_OK;
 }
 
-gks_status gks_step(gks_ctx *ctx, double dt) {
+gks_status gks_step_begin(gks_ctx *ctx, double dt) {
   if (!ctx) return GKS_ERR_INVALID_ARG;
   if (!ctx->have_state) return gks_set_err(ctx, GKS_ERR_STATE, "gks_step before gks_set_state");
   if (!(dt > 0) || !std::isfinite(dt)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "dt must be > 0");
+  if (ctx->mid_step) return gks_set_err(ctx, GKS_ERR_STATE, "gks_step_begin twice without gks_step_finish");
   const GksGrid &g = ctx->g;
   const GksPhys &ph = ctx->ph;
   cudaStream_t s = ctx->stream;
@@ -130,6 +131,19 @@ gks_status gks_step(gks_ctx *ctx, double dt) {
   gks_prof_begin(ctx, GKS_PROF_UPDATE);
   ctx->launches += gks_launch_stage1(g, ctx->Wn, ctx->flux, dt, ctx->Ws, ctx->Pbuf, s);
   gks_prof_end(ctx);
+  CUDA_TRY(ctx, cudaGetLastError());
+  ctx->mid_step = true;
+  return GKS_OK;
+}
+
+gks_status gks_step_finish(gks_ctx *ctx, double dt) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (!ctx->mid_step) return gks_set_err(ctx, GKS_ERR_STATE, "gks_step_finish without gks_step_begin");
+  if (!(dt > 0) || !std::isfinite(dt)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "dt must be > 0");
+  const GksGrid &g = ctx->g;
+  const GksPhys &ph = ctx->ph;
+  cudaStream_t s = ctx->stream;
+  ctx->mid_step = false;
   /* stage 2: ghosts of W* (outflow ghost state taken from W^n, S20), dF/dt only, W^{n+1} in place of W^n */
   gks_prof_begin(ctx, GKS_PROF_GHOST);
   ctx->launches += gks_launch_ghost_fill(g, ph, ctx->Ws, ctx->Wn, s);
@@ -173,6 +187,47 @@ gks_status gks_step(gks_ctx *ctx, double dt) {
   return GKS_OK;
 }
 
+gks_status gks_step(gks_ctx *ctx, double dt) {
+  if (gks_status st = gks_step_begin(ctx, dt)) return st;
+  return gks_step_finish(ctx, dt);
+}
+
+size_t gks_halo_doubles(const gks_ctx *ctx, int face) {
+  if (!ctx || face < 0 || face > 5) return 0;
+  const int ax = face >> 1, ua = ax == 0 ? 1 : 0, va = ax == 2 ? 1 : 2;
+  return (size_t)4 * GKS_NG * ctx->g.n[ua] * ctx->g.n[va];
+}
+
+namespace {
+gks_status halo_move(gks_ctx *ctx, int which, int face, double *buf, int unpack) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (!buf) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "buf is NULL");
+  if (face < 0 || face > 5 || ctx->ph.bc[face] != GKS_BC_HALO)
+    return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "face %d is not a GKS_BC_HALO face", face);
+  if (which != 0 && which != 1) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "which must be 0 (W^n) or 1 (W*)");
+  if (!ctx->have_state) return gks_set_err(ctx, GKS_ERR_STATE, "no state set");
+  if (which == 1 && !ctx->mid_step) return gks_set_err(ctx, GKS_ERR_STATE, "W* exists only between gks_step_begin and gks_step_finish");
+  double *W = which == 0 ? ctx->Wn : ctx->Ws;
+  const size_t bytes = gks_halo_doubles(ctx, face) * sizeof(double);
+  if (gks_is_device_ptr(buf)) {
+    ctx->launches += gks_launch_halo(ctx->g, W, buf, face, unpack, ctx->stream);
+  } else { /* host buffer: stage through the tangential-pass scratch of the unfused sweep (idle here) */
+    double *stage = ctx->tmpT;
+    if (unpack) CUDA_TRY(ctx, cudaMemcpyAsync(stage, buf, bytes, cudaMemcpyHostToDevice, ctx->stream));
+    ctx->launches += gks_launch_halo(ctx->g, W, stage, face, unpack, ctx->stream);
+    if (!unpack) CUDA_TRY(ctx, cudaMemcpyAsync(buf, stage, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+  }
+  CUDA_TRY(ctx, cudaGetLastError());
+  return GKS_OK;
+}
+} /* namespace */
+
+gks_status gks_halo_pack(gks_ctx *ctx, int which, int face, double *buf) { return halo_move(ctx, which, face, buf, 0); }
+gks_status gks_halo_unpack(gks_ctx *ctx, int which, int face, const double *buf) {
+  return halo_move(ctx, which, face, const_cast<double *>(buf), 1);
+}
+
 gks_status gks_set_body_force(gks_ctx *ctx, double gx, double gy, double gz) {
   if (!ctx) return GKS_ERR_INVALID_ARG;
   if (!std::isfinite(gx) || !std::isfinite(gy) || !std::isfinite(gz))
@@ -186,6 +241,9 @@ gks_status gks_set_body_force(gks_ctx *ctx, double gx, double gy, double gz) {
 gks_status gks_set_bulk_flux(gks_ctx *ctx, int axis, double target) {
   if (!ctx) return GKS_ERR_INVALID_ARG;
   if (axis > 2) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "axis must be 0, 1, 2 or negative");
+  for (int f = 0; f < 6; ++f)
+    if (axis >= 0 && ctx->ph.bc[f] == GKS_BC_HALO)
+      return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "the bulk-flux forcing needs a global sum: not available on a sub-domain");
   ctx->bulk_axis = axis < 0 ? -1 : axis;
   ctx->bulk_target = target;
   return GKS_OK;

@@ -10,7 +10,7 @@
 
 namespace {
 
-enum { BC_PERIODIC = 0, BC_NOSLIP = 1, BC_SLIP = 2, BC_INFLOW = 3, BC_OUTFLOW = 4, BC_EXTRAP = 5 };
+enum { BC_PERIODIC = 0, BC_NOSLIP = 1, BC_SLIP = 2, BC_INFLOW = 3, BC_OUTFLOW = 4, BC_EXTRAP = 5, BC_HALO = 6 };
 
 /* AX = axis being filled; (u,v) run over the two other axes: u the lower one */
 template <int AX>
@@ -31,6 +31,7 @@ __global__ void __launch_bounds__(128) k_ghost(GksGrid g, GksPhys ph, double *W,
   const long long sa = g.st[AX];
   const int n = g.n[AX];
   const int kind = ph.bc[2 * AX + side];
+  if (kind == BC_HALO) return;   /* ghosts of a cut face come from the neighbouring sub-domain */
   const int first = side == 0 ? 0 : n - 1;
 
   double qin[4] = {0, 0, 0, 0};
@@ -103,6 +104,26 @@ __global__ void __launch_bounds__(128) k_outflow(GksGrid g, GksPhys ph, double *
     }
     w[ghost * sa] = phi;
   }
+}
+
+/* the 3 interior planes next to a face (pack) or the 3 ghost planes beyond it (unpack) <-> buf[c][layer][v][u] */
+template <int AX>
+__global__ void __launch_bounds__(128) k_halo(GksGrid g, double *__restrict__ W, double *__restrict__ buf, int side,
+                                              int unpack) {
+  constexpr int UA = AX == 0 ? 1 : 0, VA = AX == 2 ? 1 : 2;
+  const int iu = blockIdx.x * blockDim.x + threadIdx.x;
+  const int iv = blockIdx.y;
+  const int layer = blockIdx.z % GKS_NG, c = blockIdx.z / GKS_NG;
+  if (iu >= g.n[UA] || iv >= g.n[VA]) return;
+  const int n = g.n[AX];
+  int p[3];
+  p[UA] = iu;
+  p[VA] = iv;
+  p[AX] = unpack ? (side == 0 ? -GKS_NG + layer : n + layer) : (side == 0 ? layer : n - GKS_NG + layer);
+  const long long id = c * g.FS + g.idx(p[0], p[1], p[2]);
+  const long long b = (((long long)c * GKS_NG + layer) * g.n[VA] + iv) * g.n[UA] + iu;
+  if (unpack) W[id] = buf[b];
+  else buf[b] = W[id];
 }
 
 __global__ void __launch_bounds__(256) k_pack(GksGrid g, double *__restrict__ Wint, double *__restrict__ Wpad,
@@ -184,6 +205,16 @@ int gks_launch_pack(const GksGrid &g, const double *Wint, double *Wpad, cudaStre
 
 int gks_launch_unpack(const GksGrid &g, const double *Wpad, double *Wint, cudaStream_t s) {
   k_pack<<<grid2d(g.n[0], g.n[1], g.n[2]), dim3(64, 4), 0, s>>>(g, Wint, const_cast<double *>(Wpad), 0, 0, 0, 0);
+  return 1;
+}
+
+int gks_launch_halo(const GksGrid &g, double *W, double *buf, int face, int unpack, cudaStream_t s) {
+  const int ax = face >> 1, side = face & 1;
+  const int ua = ax == 0 ? 1 : 0, va = ax == 2 ? 1 : 2;
+  dim3 grid((g.n[ua] + 127) / 128, g.n[va], 4 * GKS_NG);
+  if (ax == 0) k_halo<0><<<grid, 128, 0, s>>>(g, W, buf, side, unpack);
+  else if (ax == 1) k_halo<1><<<grid, 128, 0, s>>>(g, W, buf, side, unpack);
+  else k_halo<2><<<grid, 128, 0, s>>>(g, W, buf, side, unpack);
   return 1;
 }
 

@@ -61,6 +61,7 @@ struct gks_ctx {
   GksPhys ph;
   cudaStream_t stream;
   bool have_state;
+  bool mid_step;              /* between gks_step_begin and gks_step_finish */
   int sweep_mode;             /* 0 fused, 1 unfused */
   long long launches;
   char err[512];
@@ -122,6 +123,7 @@ int gks_launch_outflow_init(const GksGrid &g, const GksPhys &ph, double *W, cuda
 int gks_launch_outflow_advance(const GksGrid &g, const GksPhys &ph, double *W, double dt, cudaStream_t s);
 int gks_launch_pack(const GksGrid &g, const double *Wint, double *Wpad, cudaStream_t s);
 int gks_launch_unpack(const GksGrid &g, const double *Wpad, double *Wint, cudaStream_t s);
+int gks_launch_halo(const GksGrid &g, double *W, double *buf, int face, int unpack, cudaStream_t s);
 int gks_launch_unpack_faces(const GksGrid &g, int dir, const double *Fpad, double *Fout, cudaStream_t s);
 
 /* sweep of one direction: fills flux[dir] (F and dF; stage 2 needs only dF) */

@@ -18,7 +18,8 @@ STATUS = {0: "GKS_OK", 1: "GKS_ERR_INVALID_ARG", 2: "GKS_ERR_WORKSPACE", 3: "GKS
           4: "GKS_ERR_STATE", 5: "GKS_ERR_NONFINITE"}
 
 EXPORTS = ["gks_workspace_bytes", "gks_create", "gks_destroy", "gks_set_state", "gks_get_state", "gks_step",
-           "gks_set_body_force", "gks_set_bulk_flux", "alm_set_points", "ibm_set_points", "ibm_set_velocities", "ibm_set_iterations", "gks_cfl_dt", "alm_set_rotor", "alm_rotor_eval", "gks_set_reconstruction",
+           "gks_set_body_force", "gks_set_bulk_flux", "alm_set_points", "ibm_set_points", "ibm_set_velocities", "ibm_set_iterations", "gks_cfl_dt", "alm_set_rotor", "alm_rotor_eval", "gks_set_reconstruction", "gks_halo_doubles", "gks_halo_pack", "gks_halo_unpack", "gks_step_begin",
+           "gks_step_finish",
            "gks_debug_eval_flux", "gks_debug_set_sweep", "gks_debug_fp64_peak",
            "gks_profile_enable", "gks_profile_read", "gks_check_finite", "gks_launch_count", "gks_last_error"]
 
@@ -72,6 +73,12 @@ def lib():
         L.alm_set_rotor.argtypes = [vp, C.POINTER(AlmRotor)]
         L.alm_rotor_eval.argtypes = [vp, vp, vp]
         L.gks_set_reconstruction.argtypes = [vp, C.c_int]
+        L.gks_halo_doubles.argtypes = [vp, C.c_int]
+        L.gks_halo_doubles.restype = C.c_size_t
+        L.gks_halo_pack.argtypes = [vp, C.c_int, C.c_int, vp]
+        L.gks_halo_unpack.argtypes = [vp, C.c_int, C.c_int, vp]
+        L.gks_step_begin.argtypes = [vp, C.c_double]
+        L.gks_step_finish.argtypes = [vp, C.c_double]
         L.gks_debug_eval_flux.argtypes = [vp, C.c_int, vp, vp]
         L.gks_debug_set_sweep.argtypes = [vp, C.c_int]
         L.gks_check_finite.argtypes = [vp]
@@ -230,6 +237,24 @@ class Gks:
         pos, force = np.empty((self._rotor_n, 3)), np.empty((self._rotor_n, 3))
         self._check(lib().alm_rotor_eval(self._h, pos.ctypes.data, force.ctypes.data))
         return pos, force
+
+    def step_begin(self, dt):
+        self._check(lib().gks_step_begin(self._h, float(dt)))
+
+    def step_finish(self, dt):
+        self._check(lib().gks_step_finish(self._h, float(dt)))
+
+    def halo_doubles(self, face):
+        return int(lib().gks_halo_doubles(self._h, int(face)))
+
+    def halo_pack(self, which, face, buf):
+        """buf: torch tensor (CUDA or CPU, float64, contiguous) of halo_doubles(face) elements"""
+        assert buf.is_contiguous() and buf.numel() == self.halo_doubles(face)
+        self._check(lib().gks_halo_pack(self._h, int(which), int(face), buf.data_ptr()))
+
+    def halo_unpack(self, which, face, buf):
+        assert buf.is_contiguous() and buf.numel() == self.halo_doubles(face)
+        self._check(lib().gks_halo_unpack(self._h, int(which), int(face), buf.data_ptr()))
 
     def set_reconstruction(self, tangential_linear):
         self._check(lib().gks_set_reconstruction(self._h, int(tangential_linear)))

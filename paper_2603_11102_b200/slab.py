@@ -1,0 +1,153 @@
+"""x-slab domain decomposition of the S2O4 GKS step over several GPUs ("the computational
+domain is divided along the x-direction ... the ghost cells are exchanged between neighbouring GPUs").
+
+Rank r owns the cells i in [x_lo[r], x_lo[r+1]) of the global grid; its sub-domain is an ordinary `gks.Gks`
+context whose cut faces carry GKS_BC_HALO.  Per step the 3 ghost planes x 4 fields of each cut face move
+twice: the state W^n before `step_begin`, the first-stage state W* before `step_finish`
+(include/gks.h, "Domain decomposition").  Actuator points are replicated on every rank: the Gaussian
+gather of a rank only adds to the cells it owns, so a support that straddles a cut needs no exchange.
+
+This module holds host logic only (who owns what, who talks to whom, in which order); every number is moved by
+`gks_halo_pack` / `gks_halo_unpack` kernels and by the transport:
+  * `LocalTransport`  - all sub-domains live in ONE process (one GPU): buffers are handed over directly.  This
+    is how the decomposition is validated on a single-GPU box (no kernels wait on one another);
+  * `DistTransport`   - one process per GPU, `torch.distributed` point-to-point (NCCL on device tensors; gloo on
+    CPU tensors in the CPU tests of the plumbing).
+Not covered yet: IBM points and the on-line rotor next to a cut (they read across it), bulk-flux forcing.
+"""
+from dataclasses import replace
+
+import numpy as np
+
+BC_PERIODIC, BC_HALO = 0, 6
+XLO, XHI = 0, 1
+
+
+class SlabDecomposition:
+    """Who owns which x-range of a global GridConfig, and the sub-domain configuration of every rank."""
+
+    def __init__(self, cfg, world):
+        if cfg.faces[0] is not None:
+            raise ValueError("x-slabs need a uniform x axis")
+        if world < 1 or cfg.n[0] // world < 6:
+            raise ValueError("every slab needs at least 6 cells along x")
+        self.cfg, self.world = cfg, world
+        base, extra = divmod(cfg.n[0], world)
+        sizes = [base + (1 if r < extra else 0) for r in range(world)]
+        self.x_lo = np.concatenate([[0], np.cumsum(sizes)]).astype(int)
+        self.periodic = cfg.bc[0] == BC_PERIODIC
+
+    def owned(self, rank):
+        return int(self.x_lo[rank]), int(self.x_lo[rank + 1])
+
+    def neighbours(self, rank):
+        """(rank on the low-x side, rank on the high-x side); None at a physical boundary"""
+        if self.world == 1:
+            return None, None
+        lo = rank - 1 if rank > 0 else (self.world - 1 if self.periodic else None)
+        hi = rank + 1 if rank < self.world - 1 else (0 if self.periodic else None)
+        return lo, hi
+
+    def local_cfg(self, rank):
+        i0, i1 = self.owned(rank)
+        lo, hi = self.neighbours(rank)
+        bc = list(self.cfg.bc)
+        if self.world > 1:
+            bc[0] = BC_HALO if lo is not None else self.cfg.bc[0]
+            bc[1] = BC_HALO if hi is not None else self.cfg.bc[1]
+        origin = (self.cfg.origin[0] + i0 * self.cfg.spacing[0], self.cfg.origin[1], self.cfg.origin[2])
+        return replace(self.cfg, n=(i1 - i0, self.cfg.n[1], self.cfg.n[2]), origin=origin, bc=tuple(bc))
+
+    def scatter(self, W, rank):
+        i0, i1 = self.owned(rank)
+        return np.ascontiguousarray(W[..., i0:i1])
+
+    def gather(self, parts):
+        return np.concatenate(parts, axis=-1)
+
+    def schedule(self, rank):
+        """The exchange of one halo, as a list of (face to pack, destination rank, face the destination unpacks).
+        Message tags are (sender's packed face), unique per (sender, receiver) pair even when world == 2 and
+        periodic (the same neighbour on both sides)."""
+        lo, hi = self.neighbours(rank)
+        out = []
+        if lo is not None:
+            out.append((XLO, lo, XHI))
+        if hi is not None:
+            out.append((XHI, hi, XLO))
+        return out
+
+
+class LocalTransport:
+    """All sub-domains in this process: `exchange` hands every packed buffer to the solver that unpacks it."""
+
+    def __init__(self, decomposition):
+        self.d = decomposition
+
+    def exchange(self, solvers, which, new_buffer):
+        packed = {}
+        for r, s in enumerate(solvers):
+            for face, dst, dst_face in self.d.schedule(r):
+                buf = new_buffer(s, face)
+                s.halo_pack(which, face, buf)
+                packed[(dst, dst_face)] = buf
+        for s in solvers:                         # every solver has its own stream: packs before unpacks
+            s.synchronize()
+        for (dst, dst_face), buf in packed.items():
+            solvers[dst].halo_unpack(which, dst_face, buf)
+
+
+class DistTransport:
+    """One process per sub-domain; point-to-point messages through torch.distributed (nccl or gloo)."""
+
+    def __init__(self, decomposition, rank, group=None):
+        import torch.distributed as dist
+        self.d, self.rank, self.dist, self.group = decomposition, rank, dist, group
+
+    def exchange(self, solver, which, new_buffer):
+        dist = self.dist
+        sched = self.d.schedule(self.rank)
+        sends, recvs, ops = [], [], []
+        for face, dst, dst_face in sched:                       # sends in the order of the packed face
+            sbuf = new_buffer(solver, face)
+            solver.halo_pack(which, face, sbuf)
+            sends.append(sbuf)
+            ops.append(dist.P2POp(dist.isend, sbuf, dst, group=self.group, tag=face))
+        # what arrives for my face `face` was packed by `dst` at its face `dst_face`.  NCCL matches the messages
+        # of a pair of ranks by order, not by tag: receives are posted in the order of the SENDER's packed face
+        # (this matters when both neighbours are the same rank: two slabs on a periodic axis)
+        for face, dst, dst_face in sorted(sched, key=lambda e: e[2]):
+            rbuf = new_buffer(solver, face)
+            recvs.append((face, rbuf))
+            ops.append(dist.P2POp(dist.irecv, rbuf, dst, group=self.group, tag=dst_face))
+        if ops:
+            solver.synchronize()                  # the packs are on the solver's stream
+            for req in dist.batch_isend_irecv(ops):
+                req.wait()
+        for face, rbuf in recvs:
+            solver.halo_unpack(which, face, rbuf)
+
+
+class SlabStepper:
+    """The step of include/gks.h "Domain decomposition" for the sub-domain(s) of this process.
+
+    solvers: the list of all sub-domain solvers (LocalTransport) or the single solver of this rank
+    (DistTransport).  new_buffer(solver, face) -> a contiguous float64 torch tensor of solver.halo_doubles(face)
+    elements on the device the transport moves (CUDA for nccl / local, CPU for gloo)."""
+
+    def __init__(self, transport, solvers, new_buffer):
+        self.t, self.solvers, self.new_buffer = transport, solvers, new_buffer
+        self.many = isinstance(solvers, (list, tuple))
+
+    def _each(self, fn):
+        for s in (self.solvers if self.many else [self.solvers]):
+            fn(s)
+
+    def step(self, dt, before_forcing=None):
+        """before_forcing(solver): e.g. alm_set_points for this step (replicated point list)"""
+        if before_forcing is not None:
+            self._each(before_forcing)
+        self.t.exchange(self.solvers, 0, self.new_buffer)      # ghosts of W^n
+        self._each(lambda s: s.step_begin(dt))
+        self.t.exchange(self.solvers, 1, self.new_buffer)      # ghosts of W*
+        self._each(lambda s: s.step_finish(dt))

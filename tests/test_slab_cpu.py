@@ -1,0 +1,135 @@
+"""Host logic of the x-slab decomposition (paper_2603_11102_b200/slab.py) without a GPU: ownership, sub-domain
+configurations, the exchange schedule, and the torch.distributed transport with world_size 2 and 3 over gloo,
+driven by a numpy stand-in for the solver that implements gks_halo_pack / gks_halo_unpack as array slices."""
+import os
+import socket
+
+import numpy as np
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+from paper_2603_11102_b200 import slab, workloads as wl
+from paper_2603_11102_b200.workloads import GridConfig
+
+NG = 3
+
+
+class FakeSolver:
+    """padded field [c][k][j][i] with 3 ghost layers in x only; pack / unpack follow include/gks.h"""
+
+    def __init__(self, cfg, W):
+        self.n = cfg.n
+        self.W = np.full((4, cfg.n[2], cfg.n[1], cfg.n[0] + 2 * NG), np.nan)
+        self.W[..., NG:-NG] = W
+        self.Ws = self.W.copy()
+
+    def halo_doubles(self, face):
+        return 4 * NG * self.n[1] * self.n[2]
+
+    def _arr(self, which):
+        return self.W if which == 0 else self.Ws
+
+    def halo_pack(self, which, face, buf):
+        A = self._arr(which)
+        sl = A[..., NG:2 * NG] if face == 0 else A[..., -2 * NG:-NG]
+        buf.copy_(torch.from_numpy(np.ascontiguousarray(np.moveaxis(sl, -1, 1)).reshape(-1)))   # [c][layer][k][j]
+
+    def halo_unpack(self, which, face, buf):
+        A = self._arr(which)
+        planes = np.moveaxis(buf.numpy().reshape(4, NG, self.n[2], self.n[1]), 1, -1)
+        if face == 0:
+            A[..., :NG] = planes
+        else:
+            A[..., -NG:] = planes
+
+    def synchronize(self):
+        pass
+
+
+def test_ownership_and_local_configurations():
+    cfg = GridConfig(n=(32, 8, 8), spacing=(0.1, 0.1, 0.1), bc=(0,) * 6)
+    d = slab.SlabDecomposition(cfg, 3)
+    assert [d.owned(r) for r in range(3)] == [(0, 11), (11, 22), (22, 32)]
+    assert d.neighbours(0) == (2, 1) and d.neighbours(2) == (1, 0)
+    c1 = d.local_cfg(1)
+    assert c1.n == (11, 8, 8) and c1.bc[:2] == (6, 6) and c1.origin[0] == pytest.approx(1.1)
+    w = wl.by_name("C4", small=True)                                   # inflow / outflow along x
+    d = slab.SlabDecomposition(w.cfg, 4)
+    assert d.neighbours(0) == (None, 1) and d.neighbours(3) == (2, None)
+    assert d.local_cfg(0).bc[:2] == (wl.BC_INFLOW, 6) and d.local_cfg(3).bc[:2] == (6, wl.BC_OUTFLOW_CONVECTIVE)
+    assert d.local_cfg(2).bc[2:] == w.cfg.bc[2:]
+    parts = [d.scatter(w.W0, r) for r in range(4)]
+    assert np.array_equal(d.gather(parts), w.W0)
+    assert slab.SlabDecomposition(cfg, 1).local_cfg(0).bc == cfg.bc and slab.SlabDecomposition(cfg, 1).schedule(0) == []
+    with pytest.raises(ValueError):
+        slab.SlabDecomposition(cfg, 6)                                  # 5 cells per slab: too thin
+
+
+def _check_ghosts(d, rank, s, W, which):
+    """ghost planes of the sub-domain = the global field's planes next door (periodic wrap included)"""
+    i0, i1 = d.owned(rank)
+    nx = d.cfg.n[0]
+    lo, hi = d.neighbours(rank)
+    A = s._arr(which)
+    if lo is not None:
+        idx = np.arange(i0 - NG, i0) % nx
+        assert np.array_equal(A[..., :NG], W[..., idx])
+    if hi is not None:
+        idx = np.arange(i1, i1 + NG) % nx
+        assert np.array_equal(A[..., -NG:], W[..., idx])
+
+
+@pytest.mark.parametrize("world,periodic", [(2, True), (3, True), (3, False)])
+def test_local_transport_moves_the_right_planes(world, periodic):
+    rng = np.random.default_rng(world)
+    bc = (0, 0) if periodic else (wl.BC_INFLOW, wl.BC_EXTRAPOLATE)
+    cfg = GridConfig(n=(20, 5, 4), spacing=(0.1,) * 3, bc=bc + (0, 0, 0, 0))
+    W = rng.standard_normal((4, 4, 5, 20))
+    d = slab.SlabDecomposition(cfg, world)
+    solvers = [FakeSolver(d.local_cfg(r), d.scatter(W, r)) for r in range(world)]
+    t = slab.LocalTransport(d)
+    newbuf = lambda s, face: torch.empty(s.halo_doubles(face), dtype=torch.float64)
+    t.exchange(solvers, 0, newbuf)
+    for r, s in enumerate(solvers):
+        _check_ghosts(d, r, s, W, 0)
+
+
+def _dist_worker(rank, world, port, periodic, W, q):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        bc = (0, 0) if periodic else (wl.BC_INFLOW, wl.BC_EXTRAPOLATE)
+        cfg = GridConfig(n=(W.shape[-1], W.shape[2], W.shape[1]), spacing=(0.1,) * 3, bc=bc + (0, 0, 0, 0))
+        d = slab.SlabDecomposition(cfg, world)
+        s = FakeSolver(d.local_cfg(rank), d.scatter(W, rank))
+        s.Ws[..., NG:-NG] *= 2.0                               # a different field for which = 1
+        t = slab.DistTransport(d, rank)
+        newbuf = lambda sv, face: torch.empty(sv.halo_doubles(face), dtype=torch.float64)
+        t.exchange(s, 0, newbuf)
+        t.exchange(s, 1, newbuf)
+        _check_ghosts(d, rank, s, W, 0)
+        _check_ghosts(d, rank, s, 2.0 * W, 1)
+        q.put((rank, "ok"))
+    except Exception as e:                                      # noqa: BLE001 - reported to the parent
+        q.put((rank, repr(e)))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world,periodic", [(2, True), (2, False), (3, True)])
+def test_dist_transport_over_gloo(world, periodic):
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    W = np.random.default_rng(7).standard_normal((4, 3, 4, 19))
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_dist_worker, args=(r, world, port, periodic, W, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = dict(q.get(timeout=120) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+    assert res == {r: "ok" for r in range(world)}, res
