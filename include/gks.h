@@ -108,15 +108,22 @@ gks_status gks_step(gks_ctx *ctx, double dt);
  *       u the lower and v the higher of the two tangential axes, interior cells only);
  *   gks_halo_unpack(ctx, which, face, buf) writes the 3 ghost planes beyond `face` from such an array (what the
  *       neighbour packed at its opposite face).
- * gks_step is split at the two points where a stage needs its neighbours:
+ * gks_step is split at the points where it needs its neighbours:
  *   gks_step_begin(ctx, dt)   ghosts of W^n (HALO ghosts must be in place), sweeps, W* and P;
- *   gks_step_finish(ctx, dt)  ghosts of W* (HALO ghosts of W* must be in place), sweeps, W^{n+1}, forcing.
- * gks_step = begin + finish.  Errors: GKS_ERR_INVALID_ARG (face without HALO, NULL), GKS_ERR_STATE (order). */
+ *   gks_step_finish(ctx, dt)  ghosts of W* (HALO ghosts of W* must be in place), sweeps, un-forced W^{n+1};
+ *   gks_step_force(ctx, dt)   forcing of Eq. 13.  IBM points within 1.5 cells of a cut read across it: with IBM
+ *       the HALO ghosts of the un-forced W^{n+1} (which = 0) must be in place.  Every sub-domain is given the
+ *       Lagrangian points that lie inside it or at most 2 cells beyond a HALO face, interpolates U_p from the
+ *       same cells as its neighbour, and adds only to the cells it owns.  Not available on a sub-domain:
+ *       more than one IBM pass, the on-line rotor, the bulk-flux forcing (GKS_ERR_INVALID_ARG).
+ * gks_step = begin + finish + force.  Errors: GKS_ERR_INVALID_ARG (face without HALO, NULL), GKS_ERR_STATE
+ * (order of the calls). */
 size_t gks_halo_doubles(const gks_ctx *ctx, int face);
 gks_status gks_halo_pack(gks_ctx *ctx, int which, int face, double *buf);
 gks_status gks_halo_unpack(gks_ctx *ctx, int which, int face, const double *buf);
 gks_status gks_step_begin(gks_ctx *ctx, double dt);
 gks_status gks_step_finish(gks_ctx *ctx, double dt);
+gks_status gks_step_force(gks_ctx *ctx, double dt);
 
 /* Uniform acceleration g: momentum += dt * rho * g each step.  (0,0,0) disables. */
 gks_status gks_set_body_force(gks_ctx *ctx, double gx, double gy, double gz);

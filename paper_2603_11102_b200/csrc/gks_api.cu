@@ -233,6 +233,8 @@ gks_status gks_create(const gks_config *cfg, void *workspace, size_t workspace_b
     g.x0[a] = x0[a];
     g.dx[a] = dx[a];
     g.periodic[a] = cfg->bc[2 * a] == GKS_BC_PERIODIC;
+    g.halo[2 * a] = cfg->bc[2 * a] == GKS_BC_HALO;
+    g.halo[2 * a + 1] = cfg->bc[2 * a + 1] == GKS_BC_HALO;
   }
   /* On a periodic axis face n is face 0, cell for cell, unless another axis carries convective-outflow
      ghosts: those are state on interior lines but zero-gradient on tangential-ghost lines (S20),

@@ -119,7 +119,7 @@ gks_status gks_step_begin(gks_ctx *ctx, double dt) {
   if (!ctx) return GKS_ERR_INVALID_ARG;
   if (!ctx->have_state) return gks_set_err(ctx, GKS_ERR_STATE, "gks_step before gks_set_state");
   if (!(dt > 0) || !std::isfinite(dt)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "dt must be > 0");
-  if (ctx->mid_step) return gks_set_err(ctx, GKS_ERR_STATE, "gks_step_begin twice without gks_step_finish");
+  if (ctx->mid_step) return gks_set_err(ctx, GKS_ERR_STATE, "gks_step_begin inside an unfinished step");
   const GksGrid &g = ctx->g;
   const GksPhys &ph = ctx->ph;
   cudaStream_t s = ctx->stream;
@@ -132,18 +132,17 @@ gks_status gks_step_begin(gks_ctx *ctx, double dt) {
   ctx->launches += gks_launch_stage1(g, ctx->Wn, ctx->flux, dt, ctx->Ws, ctx->Pbuf, s);
   gks_prof_end(ctx);
   CUDA_TRY(ctx, cudaGetLastError());
-  ctx->mid_step = true;
+  ctx->mid_step = 1;
   return GKS_OK;
 }
 
 gks_status gks_step_finish(gks_ctx *ctx, double dt) {
   if (!ctx) return GKS_ERR_INVALID_ARG;
-  if (!ctx->mid_step) return gks_set_err(ctx, GKS_ERR_STATE, "gks_step_finish without gks_step_begin");
+  if (ctx->mid_step != 1) return gks_set_err(ctx, GKS_ERR_STATE, "gks_step_finish without gks_step_begin");
   if (!(dt > 0) || !std::isfinite(dt)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "dt must be > 0");
   const GksGrid &g = ctx->g;
   const GksPhys &ph = ctx->ph;
   cudaStream_t s = ctx->stream;
-  ctx->mid_step = false;
   /* stage 2: ghosts of W* (outflow ghost state taken from W^n, S20), dF/dt only, W^{n+1} in place of W^n */
   gks_prof_begin(ctx, GKS_PROF_GHOST);
   ctx->launches += gks_launch_ghost_fill(g, ph, ctx->Ws, ctx->Wn, s);
@@ -152,6 +151,25 @@ gks_status gks_step_finish(gks_ctx *ctx, double dt) {
   gks_prof_begin(ctx, GKS_PROF_UPDATE);
   ctx->launches += gks_launch_stage2(g, ctx->Pbuf, ctx->flux, dt, ctx->Wn, s);
   gks_prof_end(ctx);
+  CUDA_TRY(ctx, cudaGetLastError());
+  ctx->mid_step = 2;
+  return GKS_OK;
+}
+
+gks_status gks_step_force(gks_ctx *ctx, double dt) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (ctx->mid_step != 2) return gks_set_err(ctx, GKS_ERR_STATE, "gks_step_force without gks_step_finish");
+  if (!(dt > 0) || !std::isfinite(dt)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "dt must be > 0");
+  const GksGrid &g = ctx->g;
+  const GksPhys &ph = ctx->ph;
+  cudaStream_t s = ctx->stream;
+  bool any_halo = false;
+  for (int f = 0; f < 6; ++f) any_halo = any_halo || g.halo[f];
+  if (any_halo && ctx->n_ibm > 0 && ctx->ibm_maxit > 1)
+    return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "IBM passes > 1 need an exchange per pass: not available on a sub-domain");
+  if (any_halo && ctx->rotor_on)
+    return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "the on-line rotor samples across cuts: not available on a sub-domain");
+  ctx->mid_step = 0;
   gks_prof_begin(ctx, GKS_PROF_FORCING);
   /* forcing (Eq. 13), every increment from the un-forced field: read-only kernels first */
   const bool uniform = ctx->gacc[0] != 0.0 || ctx->gacc[1] != 0.0 || ctx->gacc[2] != 0.0;
@@ -189,7 +207,8 @@ gks_status gks_step_finish(gks_ctx *ctx, double dt) {
 
 gks_status gks_step(gks_ctx *ctx, double dt) {
   if (gks_status st = gks_step_begin(ctx, dt)) return st;
-  return gks_step_finish(ctx, dt);
+  if (gks_status st = gks_step_finish(ctx, dt)) return st;
+  return gks_step_force(ctx, dt);
 }
 
 size_t gks_halo_doubles(const gks_ctx *ctx, int face) {
@@ -206,7 +225,7 @@ gks_status halo_move(gks_ctx *ctx, int which, int face, double *buf, int unpack)
     return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "face %d is not a GKS_BC_HALO face", face);
   if (which != 0 && which != 1) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "which must be 0 (W^n) or 1 (W*)");
   if (!ctx->have_state) return gks_set_err(ctx, GKS_ERR_STATE, "no state set");
-  if (which == 1 && !ctx->mid_step) return gks_set_err(ctx, GKS_ERR_STATE, "W* exists only between gks_step_begin and gks_step_finish");
+  if (which == 1 && ctx->mid_step != 1) return gks_set_err(ctx, GKS_ERR_STATE, "W* exists only between gks_step_begin and gks_step_finish");
   double *W = which == 0 ? ctx->Wn : ctx->Ws;
   const size_t bytes = gks_halo_doubles(ctx, face) * sizeof(double);
   if (gks_is_device_ptr(buf)) {
@@ -369,7 +388,17 @@ gks_status ibm_set_points(gks_ctx *ctx, int n, const double *pos, const double *
   for (int p = 0; p < n; ++p)
     for (int a = 0; a < 3; ++a) {
       const int c0 = gks_host_find_cell(ctx, a, hp[3 * p + a]);
-      if (c0 < 0) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "ibm: point %d lies outside the domain", p);
+      if (c0 < 0) {
+        /* a point of the neighbouring sub-domain, at most 2 cells beyond a HALO face (uniform axis): its
+           support reaches cells owned here and reads the HALO ghosts */
+        const double *xf = ctx->h_xf[a] + GKS_NG;
+        const double x = hp[3 * p + a], h = ctx->g.dx[a];
+        const int nn = ctx->g.n[a];
+        if ((ctx->g.halo[2 * a] && x < xf[0] && x >= xf[0] - 2.0 * h) ||
+            (ctx->g.halo[2 * a + 1] && x > xf[nn] && x <= xf[nn] + 2.0 * h))
+          continue;
+        return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "ibm: point %d lies outside the domain", p);
+      }
       const double *w = ctx->h_w[a] + GKS_NG;
       if (fabs(w[c0 - 1] - w[c0]) > 1e-9 * w[c0] || fabs(w[c0 + 1] - w[c0]) > 1e-9 * w[c0])
         return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "ibm: grid not locally uniform over the support of point %d", p);

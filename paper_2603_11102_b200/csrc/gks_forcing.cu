@@ -97,12 +97,14 @@ __global__ void __launch_bounds__(256) k_uniform_force(GksGrid g, double *__rest
 }
 
 /* ---- IBM ---- */
-/* interior cell containing x on axis a (caller guarantees lo <= x <= hi) */
+/* cell containing x on axis a (caller guarantees lo <= x <= hi; beyond a HALO face, which needs a uniform axis,
+ * the two nearest ghost cells count as well: a Lagrangian point of the neighbouring sub-domain) */
+constexpr int IBM_DROP = -2147483647 - 1;   /* support cell outside the domain: no weight */
 __device__ __forceinline__ int find_cell(const GksGrid &g, int a, double x) {
   const int n = g.n[a];
   if (g.uniform[a]) {
     int c = (int)floor((x - g.x0[a]) / g.dx[a]);
-    return max(0, min(n - 1, c));
+    return max(g.halo[2 * a] ? -2 : 0, min(g.halo[2 * a + 1] ? n + 1 : n - 1, c));
   }
   const double *xf = g.xf[a] + GKS_NG;
   int lo = 0, hi = n;
@@ -128,9 +130,9 @@ __device__ __forceinline__ void ibm_support(const GksGrid &g, const double *X, S
     for (int m = 0; m < 3; ++m) {
       const int i = c0 - 1 + m;
       sp.phi[a][m] = gksd::delta3((xc[i] - X[a]) * ih);
-      int w = i;
-      if (i < 0) w = g.periodic[a] ? i + g.n[a] : -1;
-      else if (i >= g.n[a]) w = g.periodic[a] ? i - g.n[a] : -1;
+      int w = i;   /* ghost cells of a HALO face keep their index: readable, but owned by the neighbour */
+      if (i < 0) w = g.periodic[a] ? i + g.n[a] : (g.halo[2 * a] ? i : IBM_DROP);
+      else if (i >= g.n[a]) w = g.periodic[a] ? i - g.n[a] : (g.halo[2 * a + 1] ? i : IBM_DROP);
       sp.idx[a][m] = w;
     }
   }
@@ -161,7 +163,7 @@ __global__ void __launch_bounds__(128) k_ibm_interp(GksGrid g, const double *__r
     for (int mj = 0; mj < 3; ++mj)
       for (int mi = 0; mi < 3; ++mi) {
         const int i = sp.idx[0][mi], j = sp.idx[1][mj], k = sp.idx[2][mk];
-        if (i < 0 || j < 0 || k < 0) continue;
+        if (i == IBM_DROP || j == IBM_DROP || k == IBM_DROP) continue;
         const double wgt = sp.phi[0][mi] * sp.phi[1][mj] * sp.phi[2][mk];
         const long long id = g.idx(i, j, k);
         const double ir = 1.0 / W[id];
@@ -191,7 +193,8 @@ __global__ void __launch_bounds__(128) k_ibm_spread(GksGrid g, double *__restric
   Support sp;
   ibm_support(g, X, sp);
   const int i = sp.idx[0][mi], j = sp.idx[1][mj], k = sp.idx[2][mk];
-  if (i < 0 || j < 0 || k < 0) return;
+  /* only cells this sub-domain owns (dropped cells and HALO ghosts fall outside [0, n)) */
+  if (i < 0 || j < 0 || k < 0 || i >= g.n[0] || j >= g.n[1] || k >= g.n[2]) return;
   const double wgt = sp.phi[0][mi] * sp.phi[1][mj] * sp.phi[2][mk];
   if (wgt == 0.0) return;
   const long long id = g.idx(i, j, k);

@@ -32,6 +32,7 @@ struct GksGrid {
   int uniform[3];
   double x0[3], dx[3];
   int periodic[3];
+  int halo[6];       /* face carries GKS_BC_HALO: its ghost layers hold the neighbouring sub-domain's cells */
   int wrapf[3];      /* face n of this axis is not stored: it is face 0 (periodic axis, see gks_create) */
   __host__ __device__ long long idx(int i, int j, int k) const {
     return ((long long)(k + GKS_NG) * P[1] + (j + GKS_NG)) * P[0] + (i + GKS_NG);
@@ -61,7 +62,7 @@ struct gks_ctx {
   GksPhys ph;
   cudaStream_t stream;
   bool have_state;
-  bool mid_step;              /* between gks_step_begin and gks_step_finish */
+  int mid_step;               /* 0 idle, 1 after gks_step_begin, 2 after gks_step_finish (forcing pending) */
   int sweep_mode;             /* 0 fused, 1 unfused */
   long long launches;
   char err[512];

@@ -13,7 +13,9 @@ This module holds host logic only (who owns what, who talks to whom, in which or
     is how the decomposition is validated on a single-GPU box (no kernels wait on one another);
   * `DistTransport`   - one process per GPU, `torch.distributed` point-to-point (NCCL on device tensors; gloo on
     CPU tensors in the CPU tests of the plumbing).
-Not covered yet: IBM points and the on-line rotor next to a cut (they read across it), bulk-flux forcing.
+IBM points within 1.5 cells of a cut are given to both sub-domains (`SlabDecomposition.ibm_points`); both
+interpolate the same U_p after a third exchange (the un-forced W^{n+1}) and each adds to the cells it owns.
+Not covered yet: more than one IBM pass, the on-line rotor (it samples across cuts), bulk-flux forcing.
 """
 from dataclasses import replace
 
@@ -64,6 +66,28 @@ class SlabDecomposition:
 
     def gather(self, parts):
         return np.concatenate(parts, axis=-1)
+
+    def ibm_points(self, rank, pos, vol):
+        """Lagrangian points sub-domain `rank` must know: those inside it and those of a neighbour whose 3-point
+        support (1.5 cells) reaches across a cut.  On a periodic x axis the images beyond the seam are shifted by
+        the period so that they sit next to the slab."""
+        i0, i1 = self.owned(rank)
+        h, x0 = self.cfg.spacing[0], self.cfg.origin[0]
+        lo, hi = self.neighbours(rank)
+        a = x0 + i0 * h - (1.5 * h if lo is not None else 0.0)
+        b = x0 + i1 * h + (1.5 * h if hi is not None else 0.0)
+        L = self.cfg.n[0] * h
+        out_p, out_v = [], []
+        for shift in ((0.0, -L, L) if (self.periodic and self.world > 1) else (0.0,)):
+            x = pos[:, 0] + shift
+            m = (x >= a) & (x <= b)
+            if shift != 0.0:                      # images only where they are NOT already inside the slab proper
+                m &= (x < x0 + i0 * h) | (x > x0 + i1 * h)
+            q = pos[m].copy()
+            q[:, 0] += shift
+            out_p.append(q)
+            out_v.append(vol[m])
+        return np.concatenate(out_p), np.concatenate(out_v)
 
     def schedule(self, rank):
         """The exchange of one halo, as a list of (face to pack, destination rank, face the destination unpacks).
@@ -143,11 +167,15 @@ class SlabStepper:
         for s in (self.solvers if self.many else [self.solvers]):
             fn(s)
 
-    def step(self, dt, before_forcing=None):
-        """before_forcing(solver): e.g. alm_set_points for this step (replicated point list)"""
+    def step(self, dt, before_forcing=None, ibm=False):
+        """before_forcing(solver): e.g. alm_set_points for this step (replicated point list);
+        ibm: Lagrangian points are set (on any rank): the un-forced W^{n+1} is exchanged before the forcing"""
         if before_forcing is not None:
             self._each(before_forcing)
         self.t.exchange(self.solvers, 0, self.new_buffer)      # ghosts of W^n
         self._each(lambda s: s.step_begin(dt))
         self.t.exchange(self.solvers, 1, self.new_buffer)      # ghosts of W*
         self._each(lambda s: s.step_finish(dt))
+        if ibm:
+            self.t.exchange(self.solvers, 0, self.new_buffer)  # ghosts of the un-forced W^{n+1}
+        self._each(lambda s: s.step_force(dt))

@@ -18,12 +18,15 @@ def run_slabs(w, world, steps, linear=False):
     for r, s in enumerate(solvers):
         if linear:
             s.set_reconstruction(1)
+        if w.ibm is not None:
+            s.ibm_set_points(*d.ibm_points(r, *w.ibm))
         s.set_state(d.scatter(w.W0, r))
     newbuf = lambda s, face: torch.empty(s.halo_doubles(face), dtype=torch.float64, device="cuda:0")
     stepper = slab.SlabStepper(slab.LocalTransport(d), solvers, newbuf)
     for k in range(steps):
         pts = w.alm(k) if w.alm is not None else None
-        stepper.step(w.dt, before_forcing=(lambda s: s.alm_set_points(*pts)) if pts is not None else None)
+        stepper.step(w.dt, before_forcing=(lambda s: s.alm_set_points(*pts)) if pts is not None else None,
+                     ibm=w.ibm is not None)
     W = d.gather([s.get_state() for s in solvers])
     for s in solvers:
         s.close()
@@ -35,6 +38,8 @@ def run_single(w, steps, linear=False):
     g = gks.Gks(w.cfg)
     if linear:
         g.set_reconstruction(1)
+    if w.ibm is not None:
+        g.ibm_set_points(*w.ibm)
     g.set_state(w.W0)
     for k in range(steps):
         if w.alm is not None:
@@ -68,6 +73,32 @@ def test_rotor_box_in_four_slabs_with_the_rotor_on_a_cut():
     o.set_state(w.W0)
     for k in range(3):
         o.alm_set_points(*w.alm(k))
+        o.step(w.dt)
+    assert rel_linf(Ws, o.get_state()) <= 3e-11
+    o.close()
+
+
+@pytest.mark.parametrize("name", ["C3", "C5"])
+def test_ibm_bodies_across_cuts(name):
+    """small cylinder (C3: 64 cells along x, cylinder at x = 16 = the first cut of 4 slabs) and turbine (C5: ALM
+    rotor + IBM nacelle and tower) boxes: Lagrangian points next to a cut are known to both sub-domains"""
+    from oracle import binding as ob
+    w = wl.by_name(name, small=True)
+    for world in range(2, 9):                                 # the first decomposition that cuts through the body
+        d = slab.SlabDecomposition(w.cfg, world)
+        cuts = w.cfg.origin[0] + d.x_lo[1:-1] * w.cfg.spacing[0]
+        if np.abs(w.ibm[0][:, :1] - cuts[None, :]).min() < 0.5 * w.cfg.spacing[0]:
+            break
+    shared = sum(len(d.ibm_points(r, *w.ibm)[0]) for r in range(world)) - len(w.ibm[0])
+    assert shared > 0                                         # the case does exercise the cut
+    Ws, W1 = run_slabs(w, world, 3), run_single(w, 3)
+    assert rel_linf(Ws, W1) <= 1e-13                          # fp64 atomics of the spreading: order only
+    o = ob.Oracle(w.cfg)
+    o.ibm_set_points(*w.ibm)
+    o.set_state(w.W0)
+    for k in range(3):
+        if w.alm is not None:
+            o.alm_set_points(*w.alm(k))
         o.step(w.dt)
     assert rel_linf(Ws, o.get_state()) <= 3e-11
     o.close()

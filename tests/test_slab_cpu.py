@@ -133,3 +133,23 @@ def test_dist_transport_over_gloo(world, periodic):
     for p in procs:
         p.join(timeout=60)
     assert res == {r: "ok" for r in range(world)}, res
+
+
+def test_ibm_points_are_shared_across_cuts_and_wrapped_on_a_periodic_axis():
+    h = 0.1
+    cfg = GridConfig(n=(24, 8, 8), spacing=(h, h, h), bc=(wl.BC_INFLOW, wl.BC_EXTRAPOLATE, 0, 0, 0, 0))
+    d = slab.SlabDecomposition(cfg, 2)                                  # cut at x = 1.2
+    pos = np.array([[0.05, .4, .4], [1.10, .4, .4], [1.26, .4, .4], [1.40, .4, .4], [2.35, .4, .4]])
+    vol = np.arange(5.0)
+    p0, v0 = d.ibm_points(0, pos, vol)
+    p1, v1 = d.ibm_points(1, pos, vol)
+    assert list(v0) == [0, 1, 2] and list(v1) == [1, 2, 3, 4]           # 1.10 and 1.26 are within 1.5 h of the cut
+    assert np.array_equal(p0, pos[:3]) and np.array_equal(p1, pos[1:])
+    per = GridConfig(n=(24, 8, 8), spacing=(h, h, h), bc=(0,) * 6)
+    d = slab.SlabDecomposition(per, 2)
+    p0, v0 = d.ibm_points(0, pos, vol)
+    p1, v1 = d.ibm_points(1, pos, vol)
+    # across the periodic seam: the point at 2.35 is also seen by slab 0 at x = -0.05, the one at 0.05 by slab 1 at 2.45
+    assert sorted(v0) == [0, 1, 2, 4] and sorted(v1) == [0, 1, 2, 3, 4]
+    assert p0[list(v0).index(4), 0] == pytest.approx(-0.05) and p1[list(v1).index(0), 0] == pytest.approx(2.45)
+    assert slab.SlabDecomposition(per, 1).ibm_points(0, pos, vol)[0].shape == pos.shape
