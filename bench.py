@@ -145,6 +145,9 @@ def main():
     ap.add_argument("--sweep", type=int, default=0, help="0 fused (production), 1 unfused cross-check kernels")
     ap.add_argument("--variant", default="weno", choices=["weno", "linear"],
                     help="weno: the scheme as read from the paper (default, the metric); linear: linear-weight tangential passes")
+    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: replicas = N independent copies of the workload (default, weak scaling); slab = ONE\n"
+                         "workload cut into N x-slabs with halo exchange over NCCL (strong scaling, PAPER.md:193-197)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
     args = ap.parse_args()
@@ -171,7 +174,21 @@ def main():
         torch.cuda.synchronize()
 
     w = wl.by_name(args.workload)
+    slab_mode = args.decomp == "slab" and world > 1
+    stepper = None
+    if slab_mode:
+        # one workload, N x-slabs: this rank owns one sub-domain; halos move over NCCL (paper_2603_11102_b200/slab.py)
+        from dataclasses import replace as dc_replace
+        from paper_2603_11102_b200 import slab
+        if w.bulk_flux is not None:
+            raise SystemExit("--decomp slab: the bulk-flux forcing needs a global sum (not built)")
+        dec = slab.SlabDecomposition(w.cfg, world)
+        ibm_local = dec.ibm_points(rank, *w.ibm) if w.ibm is not None else None
+        w_global = w
+        w = dc_replace(w, cfg=dec.local_cfg(rank), W0=dec.scatter(w.W0, rank), ibm=ibm_local)
     g = setup_solver(w, gks, device)
+    if slab_mode:
+        stepper = slab.SlabStepper(slab.DistTransport(dec, rank), g, slab.BufferPool(device))
     g.debug_set_sweep(args.sweep)
     if args.variant == "linear":
         g.set_reconstruction(1)
@@ -185,7 +202,10 @@ def main():
     def one_step():
         if w.alm is not None:
             g.alm_set_points(*w.alm(step_no[0]))
-        g.step(w.dt)
+        if stepper is not None:
+            stepper.step(w.dt, ibm=w_global.ibm is not None)
+        else:
+            g.step(w.dt)
         step_no[0] += 1
 
     for _ in range(max(args.warmup, 3)):
@@ -218,14 +238,20 @@ def main():
     Hin = torch.from_numpy(w.W0.copy()).pin_memory()
     Hout = torch.empty_like(Hin).pin_memory()
     nbytes = Hin.numel() * 8
+    def plain_step():
+        if stepper is not None:
+            stepper.step(w.dt, ibm=w_global.ibm is not None)
+        else:
+            g.step(w.dt)
+
     g.set_state(Hin)
-    g.step(w.dt)
+    plain_step()
     g.get_state(Hout)
     barrier()
     t0 = time.perf_counter()
     for _ in range(args.e2e_steps):
         g.set_state(Hin)
-        g.step(w.dt)
+        plain_step()
         g.get_state(Hout)          # synchronises
         Hin, Hout = Hout, Hin
     barrier()
@@ -237,8 +263,10 @@ def main():
     ms, e2e_ms = t.tolist()
     if rank == 0:
         peaks, peak_src = read_peaks()
-        value = cells * world * args.steps / (ms * 1e-3) / 1e6
-        e2e_value = cells * world * args.e2e_steps / (e2e_ms * 1e-3) / 1e6
+        # replicas: every rank steps its own copy of the workload; slab: the ranks share ONE workload
+        total_cells = w_global.cfg.cells if slab_mode else cells * world
+        value = total_cells * args.steps / (ms * 1e-3) / 1e6
+        e2e_value = total_cells * args.e2e_steps / (e2e_ms * 1e-3) / 1e6
         sweep_ms = sum(prof[k][0] for k in ("sweep_x", "sweep_y", "sweep_z"))
         sweep_n = sum(prof[k][1] for k in ("sweep_x", "sweep_y", "sweep_z"))
         faces = cells  # one face per cell and direction (+ one boundary plane, < 0.5 %)
@@ -255,10 +283,10 @@ def main():
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "%s %s %dx%dx%d" % (args.workload, w.name, *w.cfg.n),
+            "scaling": "strong" if slab_mode else "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "%s %s %dx%dx%d" % (args.workload, w.name, *(w_global if slab_mode else w).cfg.n),
                        "sweep": "fused" if args.sweep == 0 else "unfused", "variant": args.variant,
-                       "multi_gpu": "replicas only" if world > 1 else "single GPU",
+                       "multi_gpu": ("x-slabs with halo exchange" if slab_mode else "replicas only") if world > 1 else "single GPU",
                        "l2": "inputs larger than L2 (state %.0f MB per field set)" % (cells * 32 / 1e6)},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,

@@ -110,9 +110,11 @@ class LocalTransport:
 
     def exchange(self, solvers, which, new_buffer):
         packed = {}
+        for s in solvers:                         # persistent buffers: the previous unpacks have finished
+            s.synchronize()
         for r, s in enumerate(solvers):
             for face, dst, dst_face in self.d.schedule(r):
-                buf = new_buffer(s, face)
+                buf = new_buffer(s, face, "send")
                 s.halo_pack(which, face, buf)
                 packed[(dst, dst_face)] = buf
         for s in solvers:                         # every solver has its own stream: packs before unpacks
@@ -129,35 +131,56 @@ class DistTransport:
         self.d, self.rank, self.dist, self.group = decomposition, rank, dist, group
 
     def exchange(self, solver, which, new_buffer):
+        import contextlib
+        import torch
         dist = self.dist
         sched = self.d.schedule(self.rank)
-        sends, recvs, ops = [], [], []
+        recvs, ops = [], []
+        cuda = False
         for face, dst, dst_face in sched:                       # sends in the order of the packed face
-            sbuf = new_buffer(solver, face)
+            sbuf = new_buffer(solver, face, "send")
+            cuda = cuda or sbuf.is_cuda
             solver.halo_pack(which, face, sbuf)
-            sends.append(sbuf)
             ops.append(dist.P2POp(dist.isend, sbuf, dst, group=self.group, tag=face))
         # what arrives for my face `face` was packed by `dst` at its face `dst_face`.  NCCL matches the messages
         # of a pair of ranks by order, not by tag: receives are posted in the order of the SENDER's packed face
         # (this matters when both neighbours are the same rank: two slabs on a periodic axis)
         for face, dst, dst_face in sorted(sched, key=lambda e: e[2]):
-            rbuf = new_buffer(solver, face)
+            rbuf = new_buffer(solver, face, "recv")
             recvs.append((face, rbuf))
             ops.append(dist.P2POp(dist.irecv, rbuf, dst, group=self.group, tag=dst_face))
         if ops:
-            solver.synchronize()                  # the packs are on the solver's stream
-            for req in dist.batch_isend_irecv(ops):
-                req.wait()
+            # device buffers (NCCL): issue on the solver's stream, so that the packs before and the unpacks after
+            # are ordered with the transfers without a host synchronisation; host buffers (gloo): the packs have
+            # synchronised already
+            with (torch.cuda.stream(solver.stream) if cuda else contextlib.nullcontext()):
+                for req in dist.batch_isend_irecv(ops):
+                    req.wait()
         for face, rbuf in recvs:
             solver.halo_unpack(which, face, rbuf)
+
+
+class BufferPool:
+    """persistent halo buffers, one per (solver, face, role): nothing is allocated inside a step"""
+
+    def __init__(self, device):
+        self.device, self.bufs = device, {}
+
+    def __call__(self, solver, face, role):
+        import torch
+        key = (id(solver), face, role)
+        if key not in self.bufs:
+            self.bufs[key] = torch.empty(solver.halo_doubles(face), dtype=torch.float64, device=self.device)
+        return self.bufs[key]
 
 
 class SlabStepper:
     """The step of include/gks.h "Domain decomposition" for the sub-domain(s) of this process.
 
     solvers: the list of all sub-domain solvers (LocalTransport) or the single solver of this rank
-    (DistTransport).  new_buffer(solver, face) -> a contiguous float64 torch tensor of solver.halo_doubles(face)
-    elements on the device the transport moves (CUDA for nccl / local, CPU for gloo)."""
+    (DistTransport).  new_buffer(solver, face, role) -> a contiguous float64 torch tensor of
+    solver.halo_doubles(face) elements on the device the transport moves (CUDA for nccl / local, CPU for gloo);
+    role is "send" or "recv" (`BufferPool` keeps one persistent buffer per solver, face and role)."""
 
     def __init__(self, transport, solvers, new_buffer):
         self.t, self.solvers, self.new_buffer = transport, solvers, new_buffer

@@ -21,7 +21,7 @@ def run_slabs(w, world, steps, linear=False):
         if w.ibm is not None:
             s.ibm_set_points(*d.ibm_points(r, *w.ibm))
         s.set_state(d.scatter(w.W0, r))
-    newbuf = lambda s, face: torch.empty(s.halo_doubles(face), dtype=torch.float64, device="cuda:0")
+    newbuf = slab.BufferPool("cuda:0")
     stepper = slab.SlabStepper(slab.LocalTransport(d), solvers, newbuf)
     for k in range(steps):
         pts = w.alm(k) if w.alm is not None else None

@@ -90,7 +90,7 @@ def test_local_transport_moves_the_right_planes(world, periodic):
     d = slab.SlabDecomposition(cfg, world)
     solvers = [FakeSolver(d.local_cfg(r), d.scatter(W, r)) for r in range(world)]
     t = slab.LocalTransport(d)
-    newbuf = lambda s, face: torch.empty(s.halo_doubles(face), dtype=torch.float64)
+    newbuf = slab.BufferPool("cpu")
     t.exchange(solvers, 0, newbuf)
     for r, s in enumerate(solvers):
         _check_ghosts(d, r, s, W, 0)
@@ -106,7 +106,7 @@ def _dist_worker(rank, world, port, periodic, W, q):
         s = FakeSolver(d.local_cfg(rank), d.scatter(W, rank))
         s.Ws[..., NG:-NG] *= 2.0                               # a different field for which = 1
         t = slab.DistTransport(d, rank)
-        newbuf = lambda sv, face: torch.empty(sv.halo_doubles(face), dtype=torch.float64)
+        newbuf = slab.BufferPool("cpu")
         t.exchange(s, 0, newbuf)
         t.exchange(s, 1, newbuf)
         _check_ghosts(d, rank, s, W, 0)
