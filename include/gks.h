@@ -99,7 +99,7 @@ gks_status gks_get_state(gks_ctx *ctx, double *W);
 gks_status gks_step(gks_ctx *ctx, double dt);
 
 /* Domain decomposition (x-slabs over several GPUs).  A sub-domain is an
- * ordinary context whose cut faces carry GKS_BC_HALO.  Such a face must lie on a uniform axis; a convective
+ * ordinary context whose cut faces carry GKS_BC_HALO.  Only x faces may (x-slabs), on a uniform x axis; a convective
  * outflow may then only sit on that same axis; gks_set_bulk_flux is refused (it needs a global sum).
  * The ghost fill leaves HALO ghosts alone; the driver moves them:
  *   gks_halo_pack(ctx, which, face, buf)   copies the 3 interior planes next to `face` (0..5 = xlo,xhi,ylo,...)

@@ -52,6 +52,7 @@ const char *validate(const gks_config *c) {
   for (int a = 0; a < 3; ++a) {
     const int lo = c->bc[2 * a], hi = c->bc[2 * a + 1];
     if (lo < 0 || lo > 6 || hi < 0 || hi > 6) return "unknown boundary kind";
+    if ((lo == GKS_BC_HALO || hi == GKS_BC_HALO) && a != 0) return "HALO faces are built for x-slabs: x faces only";
     if ((lo == GKS_BC_HALO || hi == GKS_BC_HALO) && f[a]) return "a HALO face needs a uniform axis";
     if (lo == GKS_BC_HALO || hi == GKS_BC_HALO)
       for (int b = 0; b < 3; ++b)
