@@ -160,6 +160,14 @@ gks_status alm_set_rotor(gks_ctx *ctx, const alm_rotor *rotor);
  * points for the CURRENT state and rotor clock; synchronises the stream. */
 gks_status alm_rotor_eval(gks_ctx *ctx, double *pos, double *force);
 
+/* The same front half without state in the context: positions and forces ON THE FLUID of the actuator points of
+ * `rotor` at rotor time t, sampled from the CURRENT state (between gks_step_finish and gks_step_force: the
+ * un-forced W^{n+1}).  For drivers that own the rotor clock - the x-slab driver evaluates the rotor on the
+ * sub-domain that contains the disc (sampling reads the first HALO ghost layer), broadcasts the forces and hands
+ * them to every sub-domain with alm_set_points.  pos, force: nblades*npts*3 doubles each, host (the call then
+ * synchronises) or device.  GKS_ERR_STATE while a rotor is set with alm_set_rotor. */
+gks_status alm_rotor_points(gks_ctx *ctx, const alm_rotor *rotor, double t, double *pos, double *force);
+
 /* IBM: n Lagrangian points; pos n*3 doubles, weights n doubles = V_p = dx*dS
  * (PAPER.md:155); host or device.  Velocities default to 0 (stationary body).
  * Each point must lie inside the domain and the grid must be locally uniform over its 3x3x3

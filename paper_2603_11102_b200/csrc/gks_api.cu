@@ -73,7 +73,7 @@ struct Layout {
   int P[3];
   size_t FS;       /* doubles per padded field */
   size_t off_Wn, off_Ws, off_P, off_flux[3], off_tmpN, off_tmpT, off_coords, off_red, off_alm_pos,
-      off_alm_force, off_rotor, off_ibm_pos, off_ibm_vol, off_ibm_vel, off_ibm_coef, total;
+      off_alm_force, off_rotor, off_rotor_out, off_ibm_pos, off_ibm_vol, off_ibm_vel, off_ibm_coef, total;
   size_t coords_doubles;
   int ibm_capacity;
 };
@@ -105,6 +105,7 @@ Layout make_layout(const gks_config *c) {
   L.off_alm_pos = take(3 * (size_t)GKS_MAX_ALM_POINTS);
   L.off_alm_force = take(3 * (size_t)GKS_MAX_ALM_POINTS);
   L.off_rotor = take(2 * (size_t)GKS_MAX_ROTOR_STATIONS + 3 * (size_t)GKS_MAX_POLAR);
+  L.off_rotor_out = take(6 * (size_t)GKS_MAX_ALM_POINTS);
   /* IBM capacity: one point per 8 cells, at least 65536, at most GKS_MAX_IBM_POINTS */
   size_t cap = (size_t)c->nx * c->ny * c->nz / 8;
   if (cap < 65536) cap = 65536;
@@ -217,6 +218,7 @@ gks_status gks_create(const gks_config *cfg, void *workspace, size_t workspace_b
   ctx->alm_pos = (double *)(base + L.off_alm_pos);
   ctx->alm_force = (double *)(base + L.off_alm_force);
   ctx->rotor_tab = (double *)(base + L.off_rotor);
+  ctx->rotor_out = (double *)(base + L.off_rotor_out);
   ctx->ibm_pos = (double *)(base + L.off_ibm_pos);
   ctx->ibm_vol = (double *)(base + L.off_ibm_vol);
   ctx->ibm_vel = (double *)(base + L.off_ibm_vel);

@@ -305,13 +305,9 @@ gks_status alm_set_points(gks_ctx *ctx, int n, const double *pos, const double *
   return GKS_OK;
 }
 
-gks_status alm_set_rotor(gks_ctx *ctx, const alm_rotor *r) {
-  if (!ctx) return GKS_ERR_INVALID_ARG;
-  if (!r) {
-    ctx->rotor_on = 0;
-    ctx->n_alm = 0;
-    return GKS_OK;
-  }
+namespace {
+/* validate a rotor description, copy its tables to the device and fill the kernel's view of it */
+gks_status upload_rotor(gks_ctx *ctx, const alm_rotor *r, GksRotor &R) {
   if (r->nblades < 1 || r->npts < 1 || r->npts > GKS_MAX_ROTOR_STATIONS || r->npolar < 2 || r->npolar > GKS_MAX_POLAR ||
       (long long)r->nblades * r->npts > GKS_MAX_ALM_POINTS)
     return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "rotor: sizes out of range");
@@ -328,24 +324,38 @@ gks_status alm_set_rotor(gks_ctx *ctx, const alm_rotor *r) {
     if (gks_status st = fetch_host(ctx, src[q], cnt5[q], t[q])) return st;
   for (int m = 1; m < r->npolar; ++m)
     if (!(t[2][m] > t[2][m - 1])) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "rotor: polar angles must increase");
-  /* the blades sweep the disc of radius R about the hub in the plane x = hub[0]: its bounding box is constant */
-  const double pmin[3] = {r->hub[0], r->hub[1] - r->R, r->hub[2] - r->R};
-  const double pmax[3] = {r->hub[0], r->hub[1] + r->R, r->hub[2] + r->R};
-  int lo[3], cnt[3];
-  if (gks_status st = alm_bbox(ctx, pmin, pmax, r->eps, lo, cnt)) return st;
   const size_t off[5] = {0, GKS_MAX_ROTOR_STATIONS, 2 * GKS_MAX_ROTOR_STATIONS, 2 * GKS_MAX_ROTOR_STATIONS + GKS_MAX_POLAR,
                          2 * GKS_MAX_ROTOR_STATIONS + 2 * GKS_MAX_POLAR};
   for (int q = 0; q < 5; ++q)
     CUDA_TRY(ctx, cudaMemcpyAsync(ctx->rotor_tab + off[q], t[q].data(), cnt5[q] * sizeof(double), cudaMemcpyHostToDevice,
                                   ctx->stream));
   CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));   /* the staging vectors go out of scope */
-  GksRotor &R = ctx->rotor;
   R.nb = r->nblades; R.np = r->npts; R.npolar = r->npolar;
   R.fs_corr = r->freestream_correction != 0; R.tip_corr = r->tip_correction != 0;
   for (int a = 0; a < 3; ++a) R.hub[a] = r->hub[a];
   R.R = r->R; R.rhub = r->r_hub; R.omega = r->omega; R.theta0 = r->theta0; R.uref = r->u_ref;
   R.chord = ctx->rotor_tab + off[0]; R.twist = ctx->rotor_tab + off[1]; R.alpha = ctx->rotor_tab + off[2];
   R.cl = ctx->rotor_tab + off[3]; R.cd = ctx->rotor_tab + off[4];
+  return GKS_OK;
+}
+} /* namespace */
+
+gks_status alm_set_rotor(gks_ctx *ctx, const alm_rotor *r) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (!r) {
+    ctx->rotor_on = 0;
+    ctx->n_alm = 0;
+    return GKS_OK;
+  }
+  /* the blades sweep the disc of radius R about the hub in the plane x = hub[0]: its bounding box is constant */
+  const double pmin[3] = {r->hub[0], r->hub[1] - r->R, r->hub[2] - r->R};
+  const double pmax[3] = {r->hub[0], r->hub[1] + r->R, r->hub[2] + r->R};
+  int lo[3], cnt[3];
+  if (!(r->eps > 0) || !std::isfinite(r->R)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "rotor: need eps > 0 and a finite R");
+  if (gks_status st = alm_bbox(ctx, pmin, pmax, r->eps, lo, cnt)) return st;
+  GksRotor R;
+  if (gks_status st = upload_rotor(ctx, r, R)) return st;
+  ctx->rotor = R;
   for (int a = 0; a < 3; ++a) {
     ctx->alm_lo[a] = lo[a];
     ctx->alm_cnt[a] = cnt[a];
@@ -354,6 +364,24 @@ gks_status alm_set_rotor(gks_ctx *ctx, const alm_rotor *r) {
   ctx->n_alm = 0;
   ctx->rotor_on = 1;
   ctx->rotor_time = 0.0;
+  return GKS_OK;
+}
+
+gks_status alm_rotor_points(gks_ctx *ctx, const alm_rotor *r, double t, double *pos, double *force) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (!r || !pos || !force) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "rotor/pos/force is NULL");
+  if (!std::isfinite(t)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "t must be finite");
+  if (!ctx->have_state) return gks_set_err(ctx, GKS_ERR_STATE, "alm_rotor_points before gks_set_state");
+  if (ctx->rotor_on) return gks_set_err(ctx, GKS_ERR_STATE, "a rotor is set with alm_set_rotor: clear it first");
+  GksRotor R;
+  if (gks_status st = upload_rotor(ctx, r, R)) return st;
+  const size_t n3 = 3 * (size_t)R.nb * R.np;
+  double *dp = gks_is_device_ptr(pos) ? pos : ctx->rotor_out, *df = gks_is_device_ptr(force) ? force : ctx->rotor_out + n3;
+  ctx->launches += gks_launch_rotor_forces(ctx->g, ctx->Wn, R, t, r->eps, dp, df, ctx->stream);
+  CUDA_TRY(ctx, cudaGetLastError());
+  if (dp != pos) CUDA_TRY(ctx, cudaMemcpyAsync(pos, dp, n3 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+  if (df != force) CUDA_TRY(ctx, cudaMemcpyAsync(force, df, n3 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+  if (dp != pos || df != force) CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
   return GKS_OK;
 }
 

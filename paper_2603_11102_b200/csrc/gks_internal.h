@@ -91,6 +91,7 @@ struct gks_ctx {
   GksRotor rotor;              /* valid when rotor_on */
   int rotor_on;
   double rotor_time;           /* rotor clock: 0 at alm_set_rotor, + dt per step */
+  double *rotor_out;           /* device scratch of alm_rotor_points: pos, force (GKS_MAX_ALM_POINTS*3 each) */
   double *rotor_tab;           /* device: chord, twist (GKS_MAX_ROTOR_STATIONS each), alpha, cl, cd (GKS_MAX_POLAR each) */
   int n_ibm;
   int ibm_maxit;               /* multi-direct-forcing passes per step (1 = single pass) */

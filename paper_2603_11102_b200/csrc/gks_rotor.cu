@@ -50,9 +50,9 @@ __device__ void sample_trilinear(const GksGrid &g, const double *__restrict__ W,
     if (g.periodic[a]) {
       i0[a] = (lo + n) % n;
       i1[a] = (lo + 1) % n;
-    } else {
-      i0[a] = min(max(lo, 0), n - 1);
-      i1[a] = min(max(lo + 1, 0), n - 1);
+    } else { /* the first ghost layer of a HALO face holds the neighbouring sub-domain's cell */
+      i0[a] = min(max(lo, g.halo[2 * a] ? -1 : 0), n - 1);
+      i1[a] = min(max(lo + 1, 0), g.halo[2 * a + 1] ? n : n - 1);
     }
   }
   out[0] = out[1] = out[2] = out[3] = 0.0;

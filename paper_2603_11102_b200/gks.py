@@ -18,7 +18,7 @@ STATUS = {0: "GKS_OK", 1: "GKS_ERR_INVALID_ARG", 2: "GKS_ERR_WORKSPACE", 3: "GKS
           4: "GKS_ERR_STATE", 5: "GKS_ERR_NONFINITE"}
 
 EXPORTS = ["gks_workspace_bytes", "gks_create", "gks_destroy", "gks_set_state", "gks_get_state", "gks_step",
-           "gks_set_body_force", "gks_set_bulk_flux", "alm_set_points", "ibm_set_points", "ibm_set_velocities", "ibm_set_iterations", "gks_cfl_dt", "alm_set_rotor", "alm_rotor_eval", "gks_set_reconstruction", "gks_halo_doubles", "gks_halo_pack", "gks_halo_unpack", "gks_step_begin",
+           "gks_set_body_force", "gks_set_bulk_flux", "alm_set_points", "ibm_set_points", "ibm_set_velocities", "ibm_set_iterations", "gks_cfl_dt", "alm_set_rotor", "alm_rotor_eval", "alm_rotor_points", "gks_set_reconstruction", "gks_halo_doubles", "gks_halo_pack", "gks_halo_unpack", "gks_step_begin",
            "gks_step_finish", "gks_step_force",
            "gks_debug_eval_flux", "gks_debug_set_sweep", "gks_debug_fp64_peak",
            "gks_profile_enable", "gks_profile_read", "gks_check_finite", "gks_launch_count", "gks_last_error"]
@@ -72,6 +72,7 @@ def lib():
         L.gks_cfl_dt.argtypes = [vp, C.c_double, vp]
         L.alm_set_rotor.argtypes = [vp, C.POINTER(AlmRotor)]
         L.alm_rotor_eval.argtypes = [vp, vp, vp]
+        L.alm_rotor_points.argtypes = [vp, C.POINTER(AlmRotor), C.c_double, vp, vp]
         L.gks_set_reconstruction.argtypes = [vp, C.c_int]
         L.gks_halo_doubles.argtypes = [vp, C.c_int]
         L.gks_halo_doubles.restype = C.c_size_t
@@ -217,12 +218,8 @@ class Gks:
         self._check(lib().ibm_set_points(self._h, n, pp, pw))
         self.n_ibm = n
 
-    def alm_set_rotor(self, r):
-        """r: workloads.Rotor (duck-typed) or None to clear; tables are copied by the library during the call"""
-        if r is None:
-            self._check(lib().alm_set_rotor(self._h, None))
-            self._rotor_n = 0
-            return
+    @staticmethod
+    def _rotor_struct(r):
         keep = [np.ascontiguousarray(np.asarray(x, dtype=np.float64)) for x in (r.chord, r.twist, r.alpha, r.cl, r.cd)]
         c = AlmRotor()
         c.nblades, c.npts = r.nblades, r.npts
@@ -231,8 +228,30 @@ class Gks:
         c.chord, c.twist, c.alpha, c.cl, c.cd = [x.ctypes.data_as(_dp) for x in keep]
         c.npolar = len(keep[2])
         c.freestream_correction, c.tip_correction = int(r.freestream_correction), int(r.tip_correction)
+        return c, keep
+
+    def alm_set_rotor(self, r):
+        """r: workloads.Rotor (duck-typed) or None to clear; tables are copied by the library during the call"""
+        if r is None:
+            self._check(lib().alm_set_rotor(self._h, None))
+            self._rotor_n = 0
+            return
+        c, _keep = self._rotor_struct(r)
         self._check(lib().alm_set_rotor(self._h, C.byref(c)))
         self._rotor_n = r.nblades * r.npts
+
+    def alm_rotor_points(self, r, t, pos=None, force=None):
+        """stateless front half at rotor time t on the current state; pos / force: torch CUDA tensors (n, 3) to
+        fill asynchronously, or None for host numpy arrays"""
+        c, _keep = self._rotor_struct(r)
+        n = r.nblades * r.npts
+        if pos is None:
+            pos, force = np.empty((n, 3)), np.empty((n, 3))
+            self._check(lib().alm_rotor_points(self._h, C.byref(c), float(t), pos.ctypes.data, force.ctypes.data))
+        else:
+            assert pos.is_contiguous() and force.is_contiguous() and pos.numel() == 3 * n == force.numel()
+            self._check(lib().alm_rotor_points(self._h, C.byref(c), float(t), pos.data_ptr(), force.data_ptr()))
+        return pos, force
 
     def alm_rotor_eval(self):
         pos, force = np.empty((self._rotor_n, 3)), np.empty((self._rotor_n, 3))

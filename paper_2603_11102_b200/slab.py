@@ -15,7 +15,8 @@ This module holds host logic only (who owns what, who talks to whom, in which or
     CPU tensors in the CPU tests of the plumbing).
 IBM points within 1.5 cells of a cut are given to both sub-domains (`SlabDecomposition.ibm_points`); both
 interpolate the same U_p after a third exchange (the un-forced W^{n+1}) and each adds to the cells it owns.
-Not covered yet: more than one IBM pass, the on-line rotor (it samples across cuts), bulk-flux forcing.
+The on-line rotor is evaluated by the sub-domain that contains the disc and broadcast (`RotorDriver`).
+Not covered yet: more than one IBM pass (an exchange per pass), bulk-flux forcing (a scalar all-reduce).
 """
 from dataclasses import replace
 
@@ -159,6 +160,47 @@ class DistTransport:
         for face, rbuf in recvs:
             solver.halo_unpack(which, face, rbuf)
 
+    def broadcast(self, solver, src, tensors):
+        import contextlib
+        import torch
+        with (torch.cuda.stream(solver.stream) if tensors[0].is_cuda else contextlib.nullcontext()):
+            for t in tensors:
+                self.dist.broadcast(t, src=src, group=self.group)
+
+
+class RotorDriver:
+    """The on-line actuator-line rotor on sub-domains: the disc x = hub_x lies in ONE slab (its owner), which
+    evaluates the blade-element forces of all points from the un-forced field (trilinear sampling reads the first
+    HALO ghost layer when the disc sits within half a cell of a cut); the (tiny) position and force arrays are
+    broadcast and every sub-domain spreads them onto the cells it owns."""
+
+    def __init__(self, decomposition, rotor, device):
+        import torch
+        self.d, self.r, self.t = decomposition, rotor, 0.0
+        i = int(np.floor((rotor.hub[0] - decomposition.cfg.origin[0]) / decomposition.cfg.spacing[0]))
+        i = min(max(i, 0), decomposition.cfg.n[0] - 1)
+        self.owner = int(np.searchsorted(decomposition.x_lo, i, side="right") - 1)
+        n = rotor.nblades * rotor.npts
+        self.pos = torch.zeros((n, 3), dtype=torch.float64, device=device)
+        self.force = torch.zeros((n, 3), dtype=torch.float64, device=device)
+
+    def evaluate(self, transport, solvers, many):
+        """between step_finish (+ exchange of the un-forced field) and step_force"""
+        if many:                                   # all sub-domains in this process: the owner's arrays are everyone's
+            solvers[self.owner].alm_rotor_points(self.r, self.t, self.pos, self.force)
+            solvers[self.owner].synchronize()
+            targets = solvers
+        else:
+            if transport.rank == self.owner:
+                solvers.alm_rotor_points(self.r, self.t, self.pos, self.force)
+            transport.broadcast(solvers, self.owner, [self.pos, self.force])
+            targets = [solvers]
+        for s in targets:
+            s.alm_set_points(self.pos, self.force, self.r.eps)
+
+    def advance(self, dt):
+        self.t += dt
+
 
 class BufferPool:
     """persistent halo buffers, one per (solver, face, role): nothing is allocated inside a step"""
@@ -190,15 +232,20 @@ class SlabStepper:
         for s in (self.solvers if self.many else [self.solvers]):
             fn(s)
 
-    def step(self, dt, before_forcing=None, ibm=False):
+    def step(self, dt, before_forcing=None, ibm=False, rotor=None):
         """before_forcing(solver): e.g. alm_set_points for this step (replicated point list);
-        ibm: Lagrangian points are set (on any rank): the un-forced W^{n+1} is exchanged before the forcing"""
+        ibm: Lagrangian points are set (on any rank): the un-forced W^{n+1} is exchanged before the forcing;
+        rotor: a RotorDriver (on-line actuator lines), evaluated on the un-forced W^{n+1} as well"""
         if before_forcing is not None:
             self._each(before_forcing)
         self.t.exchange(self.solvers, 0, self.new_buffer)      # ghosts of W^n
         self._each(lambda s: s.step_begin(dt))
         self.t.exchange(self.solvers, 1, self.new_buffer)      # ghosts of W*
         self._each(lambda s: s.step_finish(dt))
-        if ibm:
+        if ibm or rotor is not None:
             self.t.exchange(self.solvers, 0, self.new_buffer)  # ghosts of the un-forced W^{n+1}
+        if rotor is not None:
+            rotor.evaluate(self.t, self.solvers, self.many)
         self._each(lambda s: s.step_force(dt))
+        if rotor is not None:
+            rotor.advance(dt)

@@ -104,6 +104,50 @@ def test_ibm_bodies_across_cuts(name):
     o.close()
 
 
+@pytest.mark.parametrize("name,switches", [("C4", {}), ("C5", {"freestream_correction": True, "tip_correction": True})])
+def test_online_rotor_on_slabs(name, switches):
+    """the on-line rotor with the disc ON a cut (hub at cell 24 of 96 = the first cut of 4 slabs: the sampling of
+    the owner reads its HALO ghosts), with IBM bodies for the turbine: the decomposed run reproduces the
+    single-domain run with alm_set_rotor, and the oracle"""
+    from oracle import binding as ob
+    from paper_2603_11102_b200 import gks
+    w = wl.by_name(name, small=True)
+    pos0, _, eps = w.alm(0)
+    hub = pos0.reshape(3, -1, 3).mean(axis=(0, 1))
+    r = wl.synthetic_rotor(hub=hub, R=float(np.linalg.norm(pos0 - hub, axis=1).max() * 64.5 / 64.0), eps=eps, npts=40,
+                           **switches)
+    world, steps = 4, 3
+    d = slab.SlabDecomposition(w.cfg, world)
+    assert abs(hub[0] / w.cfg.spacing[0] - d.owned(1)[0]) < 0.5
+    solvers = [gks.Gks(d.local_cfg(k)) for k in range(world)]
+    for k, s in enumerate(solvers):
+        if w.ibm is not None:
+            s.ibm_set_points(*d.ibm_points(k, *w.ibm))
+        s.set_state(d.scatter(w.W0, k))
+    stepper = slab.SlabStepper(slab.LocalTransport(d), solvers, slab.BufferPool("cuda:0"))
+    rot = slab.RotorDriver(d, r, "cuda:0")
+    assert rot.owner == 1
+    for _ in range(steps):
+        stepper.step(w.dt, ibm=w.ibm is not None, rotor=rot)
+    Ws = d.gather([s.get_state() for s in solvers])
+    for s in solvers:
+        s.close()
+    o, g = ob.Oracle(w.cfg), gks.Gks(w.cfg)
+    for s in (o, g):
+        if w.ibm is not None:
+            s.ibm_set_points(*w.ibm)
+        s.set_state(w.W0)
+        s.alm_set_rotor(r)
+        for _ in range(steps):
+            s.step(w.dt)
+    assert rel_linf(Ws, g.get_state()) <= 1e-13
+    assert rel_linf(Ws, o.get_state()) <= 3e-11
+    with pytest.raises(gks.GksError):
+        g.alm_rotor_points(r, 0.0)                           # refused while a rotor is set
+    g.close()
+    o.close()
+
+
 def test_linear_variant_and_error_paths():
     from paper_2603_11102_b200 import gks
     w = wl.by_name("C1")

@@ -111,6 +111,10 @@ def _dist_worker(rank, world, port, periodic, W, q):
         t.exchange(s, 1, newbuf)
         _check_ghosts(d, rank, s, W, 0)
         _check_ghosts(d, rank, s, 2.0 * W, 1)
+        # the rotor driver's broadcast: the owner's arrays arrive everywhere
+        a = torch.full((5, 3), float(rank)) if rank == world - 1 else torch.zeros((5, 3))
+        t.broadcast(s, world - 1, [a])
+        assert torch.equal(a, torch.full((5, 3), float(world - 1)))
         q.put((rank, "ok"))
     except Exception as e:                                      # noqa: BLE001 - reported to the parent
         q.put((rank, repr(e)))
@@ -153,3 +157,12 @@ def test_ibm_points_are_shared_across_cuts_and_wrapped_on_a_periodic_axis():
     assert sorted(v0) == [0, 1, 2, 4] and sorted(v1) == [0, 1, 2, 3, 4]
     assert p0[list(v0).index(4), 0] == pytest.approx(-0.05) and p1[list(v1).index(0), 0] == pytest.approx(2.45)
     assert slab.SlabDecomposition(per, 1).ibm_points(0, pos, vol)[0].shape == pos.shape
+
+
+def test_rotor_driver_owner_is_the_slab_that_contains_the_disc():
+    w = wl.by_name("C4", small=True)                                    # 96 cells along x, hub at x = 3 = cell 24
+    r = wl.synthetic_rotor(hub=(3.0, 3.0, 3.0), R=1.0, eps=0.25)
+    for world, owner in ((1, 0), (2, 0), (4, 1), (5, 1)):
+        assert slab.RotorDriver(slab.SlabDecomposition(w.cfg, world), r, "cpu").owner == owner
+    r2 = wl.synthetic_rotor(hub=(2.99, 3.0, 3.0), R=1.0, eps=0.25)
+    assert slab.RotorDriver(slab.SlabDecomposition(w.cfg, 4), r2, "cpu").owner == 0
