@@ -180,8 +180,6 @@ def main():
         # one workload, N x-slabs: this rank owns one sub-domain; halos move over NCCL (paper_2603_11102_b200/slab.py)
         from dataclasses import replace as dc_replace
         from paper_2603_11102_b200 import slab
-        if w.bulk_flux is not None:
-            raise SystemExit("--decomp slab: the bulk-flux forcing needs a global sum (not built)")
         dec = slab.SlabDecomposition(w.cfg, world)
         ibm_local = dec.ibm_points(rank, *w.ibm) if w.ibm is not None else None
         w_global = w
@@ -203,7 +201,7 @@ def main():
         if w.alm is not None:
             g.alm_set_points(*w.alm(step_no[0]))
         if stepper is not None:
-            stepper.step(w.dt, ibm=w_global.ibm is not None)
+            stepper.step(w.dt, ibm=w_global.ibm is not None, bulk=w.bulk_flux is not None)
         else:
             g.step(w.dt)
         step_no[0] += 1
@@ -240,7 +238,7 @@ def main():
     nbytes = Hin.numel() * 8
     def plain_step():
         if stepper is not None:
-            stepper.step(w.dt, ibm=w_global.ibm is not None)
+            stepper.step(w.dt, ibm=w_global.ibm is not None, bulk=w.bulk_flux is not None)
         else:
             g.step(w.dt)
 

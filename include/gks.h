@@ -100,7 +100,7 @@ gks_status gks_step(gks_ctx *ctx, double dt);
 
 /* Domain decomposition (x-slabs over several GPUs).  A sub-domain is an
  * ordinary context whose cut faces carry GKS_BC_HALO.  Only x faces may (x-slabs), on a uniform x axis; a convective
- * outflow may then only sit on that same axis; gks_set_bulk_flux is refused (it needs a global sum).
+ * outflow may then only sit on that same axis.
  * The ghost fill leaves HALO ghosts alone; the driver moves them:
  *   gks_halo_pack(ctx, which, face, buf)   copies the 3 interior planes next to `face` (0..5 = xlo,xhi,ylo,...)
  *       of state `which` (0: W^n / W^{n+1}, 1: the first-stage state W*) to buf, a DEVICE or host array of
@@ -114,8 +114,11 @@ gks_status gks_step(gks_ctx *ctx, double dt);
  *   gks_step_force(ctx, dt)   forcing of Eq. 13.  IBM points within 1.5 cells of a cut read across it: with IBM
  *       the HALO ghosts of the un-forced W^{n+1} (which = 0) must be in place.  Every sub-domain is given the
  *       Lagrangian points that lie inside it or at most 2 cells beyond a HALO face, interpolates U_p from the
- *       same cells as its neighbour, and adds only to the cells it owns.  Not available on a sub-domain:
- *       more than one IBM pass, the on-line rotor, the bulk-flux forcing (GKS_ERR_INVALID_ARG).
+ *       same cells as its neighbour, and adds only to the cells it owns.  The bulk-flux forcing needs the
+ *       global sum: between finish and force every sub-domain calls gks_bulk_partial (its sum of
+ *       m_axis |Omega| over the un-forced field and its volume), the driver adds them up (one scalar
+ *       all-reduce) and returns the totals with gks_bulk_set_global (sum: host or device pointer).
+ *       Not available on a sub-domain: more than one IBM pass, alm_set_rotor (use alm_rotor_points).
  * gks_step = begin + finish + force.  Errors: GKS_ERR_INVALID_ARG (face without HALO, NULL), GKS_ERR_STATE
  * (order of the calls). */
 size_t gks_halo_doubles(const gks_ctx *ctx, int face);
@@ -124,6 +127,8 @@ gks_status gks_halo_unpack(gks_ctx *ctx, int which, int face, const double *buf)
 gks_status gks_step_begin(gks_ctx *ctx, double dt);
 gks_status gks_step_finish(gks_ctx *ctx, double dt);
 gks_status gks_step_force(gks_ctx *ctx, double dt);
+gks_status gks_bulk_partial(gks_ctx *ctx, double *sum, double *volume /* host, may be NULL */);
+gks_status gks_bulk_set_global(gks_ctx *ctx, const double *sum, double volume);
 
 /* Uniform acceleration g: momentum += dt * rho * g each step.  (0,0,0) disables. */
 gks_status gks_set_body_force(gks_ctx *ctx, double gx, double gy, double gz);

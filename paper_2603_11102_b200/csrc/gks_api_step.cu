@@ -167,6 +167,8 @@ gks_status gks_step_force(gks_ctx *ctx, double dt) {
   for (int f = 0; f < 6; ++f) any_halo = any_halo || g.halo[f];
   if (any_halo && ctx->n_ibm > 0 && ctx->ibm_maxit > 1)
     return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "IBM passes > 1 need an exchange per pass: not available on a sub-domain");
+  if (any_halo && ctx->bulk_axis >= 0 && !ctx->bulk_external)
+    return gks_set_err(ctx, GKS_ERR_STATE, "bulk-flux forcing on a sub-domain: gks_bulk_set_global must supply the global sum first");
   if (any_halo && ctx->rotor_on)
     return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "the on-line rotor samples across cuts: not available on a sub-domain");
   ctx->mid_step = 0;
@@ -179,7 +181,9 @@ gks_status gks_step_force(gks_ctx *ctx, double dt) {
     ctx->n_alm = ctx->rotor.nb * ctx->rotor.np;
     ctx->rotor_time += dt;
   }
-  if (ctx->bulk_axis >= 0) ctx->launches += gks_launch_bulk_reduce(g, ctx->Wn, ctx->bulk_axis, ctx->red, s);
+  const bool ext = ctx->bulk_external != 0;       /* sub-domain: the global sum is already in place */
+  ctx->bulk_external = 0;
+  if (ctx->bulk_axis >= 0 && !ext) ctx->launches += gks_launch_bulk_reduce(g, ctx->Wn, ctx->bulk_axis, ctx->red, s);
   if (ctx->n_ibm > 0) {
     /* multi-direct-forcing passes (Eq. 11-12): pass k interpolates from the un-forced field plus the IBM
        increments of the passes before it, in place; nothing else has touched the momentum yet (S12) */
@@ -195,7 +199,7 @@ gks_status gks_step_force(gks_ctx *ctx, double dt) {
   }
   if (uniform || ctx->bulk_axis >= 0)
     ctx->launches += gks_launch_uniform_force(g, ctx->Wn, dt, ctx->gacc, ctx->bulk_axis, ctx->bulk_target,
-                                              ctx->total_volume, ctx->red, s);
+                                              ext ? ctx->bulk_volume_ext : ctx->total_volume, ctx->red, s);
   if (ctx->n_alm > 0)
     ctx->launches += gks_launch_alm(g, ctx->Wn, ctx->n_alm, ctx->alm_pos, ctx->alm_force, ctx->alm_eps, dt,
                                     ctx->alm_lo, ctx->alm_cnt, s);
@@ -260,11 +264,39 @@ gks_status gks_set_body_force(gks_ctx *ctx, double gx, double gy, double gz) {
 gks_status gks_set_bulk_flux(gks_ctx *ctx, int axis, double target) {
   if (!ctx) return GKS_ERR_INVALID_ARG;
   if (axis > 2) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "axis must be 0, 1, 2 or negative");
-  for (int f = 0; f < 6; ++f)
-    if (axis >= 0 && ctx->ph.bc[f] == GKS_BC_HALO)
-      return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "the bulk-flux forcing needs a global sum: not available on a sub-domain");
+
   ctx->bulk_axis = axis < 0 ? -1 : axis;
   ctx->bulk_target = target;
+  return GKS_OK;
+}
+
+gks_status gks_bulk_partial(gks_ctx *ctx, double *sum, double *volume) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (!sum) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "sum is NULL");
+  if (ctx->bulk_axis < 0) return gks_set_err(ctx, GKS_ERR_STATE, "no bulk-flux forcing set");
+  if (ctx->mid_step != 2) return gks_set_err(ctx, GKS_ERR_STATE, "gks_bulk_partial belongs between gks_step_finish and gks_step_force");
+  ctx->launches += gks_launch_bulk_reduce(ctx->g, ctx->Wn, ctx->bulk_axis, ctx->red, ctx->stream);
+  CUDA_TRY(ctx, cudaGetLastError());
+  if (volume) *volume = ctx->total_volume;
+  if (gks_is_device_ptr(sum)) {
+    CUDA_TRY(ctx, cudaMemcpyAsync(sum, ctx->red + GKS_RED_BULK_SUM, sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
+  } else {
+    CUDA_TRY(ctx, cudaMemcpyAsync(sum, ctx->red + GKS_RED_BULK_SUM, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+  }
+  return GKS_OK;
+}
+
+gks_status gks_bulk_set_global(gks_ctx *ctx, const double *sum, double volume) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (!sum || !(volume > 0) || !std::isfinite(volume)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "sum is NULL or volume is not > 0");
+  if (ctx->bulk_axis < 0) return gks_set_err(ctx, GKS_ERR_STATE, "no bulk-flux forcing set");
+  if (ctx->mid_step != 2) return gks_set_err(ctx, GKS_ERR_STATE, "gks_bulk_set_global belongs between gks_step_finish and gks_step_force");
+  const cudaMemcpyKind k = gks_is_device_ptr(sum) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  CUDA_TRY(ctx, cudaMemcpyAsync(ctx->red + GKS_RED_BULK_SUM, sum, sizeof(double), k, ctx->stream));
+  if (k == cudaMemcpyHostToDevice) CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+  ctx->bulk_external = 1;
+  ctx->bulk_volume_ext = volume;
   return GKS_OK;
 }
 

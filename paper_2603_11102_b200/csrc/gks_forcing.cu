@@ -12,7 +12,7 @@
 
 namespace {
 
-constexpr int RED_BLOCKS = 1024;
+constexpr int RED_BLOCKS = GKS_RED_BULK_SUM;
 
 /* ---- bulk momentum: deterministic two-level sum of m_axis * |Omega| over the interior ---- */
 __global__ void __launch_bounds__(256) k_bulk_partial(GksGrid g, const double *__restrict__ W, int axis,

@@ -84,6 +84,8 @@ struct gks_ctx {
   double gacc[3];
   int bulk_axis;
   double bulk_target, total_volume;
+  int bulk_external;           /* sub-domain: the global sum was supplied with gks_bulk_set_global for this step */
+  double bulk_volume_ext;      /* and the global volume */
   double dmin;                 /* smallest cell width of the grid (CFL condition) */
   int n_alm;
   double alm_eps;
@@ -107,6 +109,7 @@ struct gks_ctx {
   int *prof_cat;
 };
 #define GKS_IBM_MAX_PASSES 64
+#define GKS_RED_BULK_SUM 1024  /* ctx->red + this: sum of m_axis |Omega| (gks_forcing.cu: RED_BLOCKS partials before it) */
 #define GKS_RED_CFL 1680       /* ctx->red + this: |U|_max bits, dt */
 #define GKS_RED_IBM_RES 1600   /* ctx->red + this: GKS_IBM_MAX_PASSES residual slots (bit patterns) */
 #define GKS_PROF_MAX 4096

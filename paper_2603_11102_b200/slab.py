@@ -16,7 +16,8 @@ This module holds host logic only (who owns what, who talks to whom, in which or
 IBM points within 1.5 cells of a cut are given to both sub-domains (`SlabDecomposition.ibm_points`); both
 interpolate the same U_p after a third exchange (the un-forced W^{n+1}) and each adds to the cells it owns.
 The on-line rotor is evaluated by the sub-domain that contains the disc and broadcast (`RotorDriver`).
-Not covered yet: more than one IBM pass (an exchange per pass), bulk-flux forcing (a scalar all-reduce).
+The bulk-flux forcing adds the sub-domains' partial sums up with one scalar all-reduce.
+Not covered yet: more than one IBM pass (an exchange per pass).
 """
 from dataclasses import replace
 
@@ -160,6 +161,17 @@ class DistTransport:
         for face, rbuf in recvs:
             solver.halo_unpack(which, face, rbuf)
 
+    def all_reduce_sum(self, solver, scalar, volume):
+        """(sum over ranks of a 1-element tensor, sum of the host number `volume`)"""
+        import contextlib
+        import torch
+        pair = torch.stack([scalar.reshape(()), torch.tensor(volume, dtype=torch.float64, device=scalar.device)])
+        with (torch.cuda.stream(solver.stream) if scalar.is_cuda else contextlib.nullcontext()):
+            self.dist.all_reduce(pair, group=self.group)
+        if scalar.is_cuda:
+            solver.synchronize()
+        return pair[:1].contiguous(), float(pair[1])
+
     def broadcast(self, solver, src, tensors):
         import contextlib
         import torch
@@ -232,10 +244,29 @@ class SlabStepper:
         for s in (self.solvers if self.many else [self.solvers]):
             fn(s)
 
-    def step(self, dt, before_forcing=None, ibm=False, rotor=None):
+    def _bulk(self):
+        """global sum of the bulk momentum: partial sums of the sub-domains, one scalar all-reduce"""
+        import torch
+        sols = self.solvers if self.many else [self.solvers]
+        dev = self.new_buffer.device if hasattr(self.new_buffer, "device") else "cpu"
+        parts = [torch.zeros(1, dtype=torch.float64, device=dev) for _ in sols]
+        vols = [s.bulk_partial(p) for s, p in zip(sols, parts)]
+        if self.many:
+            for s in sols:
+                s.synchronize()
+            total, volume = torch.stack(parts).sum(0), float(sum(vols))
+            if total.is_cuda:
+                torch.cuda.current_stream().synchronize()   # the solvers copy it on their own streams
+        else:
+            total, volume = self.t.all_reduce_sum(sols[0], parts[0], vols[0])
+        for s in sols:
+            s.bulk_set_global(total, volume)
+
+    def step(self, dt, before_forcing=None, ibm=False, rotor=None, bulk=False):
         """before_forcing(solver): e.g. alm_set_points for this step (replicated point list);
         ibm: Lagrangian points are set (on any rank): the un-forced W^{n+1} is exchanged before the forcing;
-        rotor: a RotorDriver (on-line actuator lines), evaluated on the un-forced W^{n+1} as well"""
+        rotor: a RotorDriver (on-line actuator lines), evaluated on the un-forced W^{n+1} as well;
+        bulk: the bulk-flux forcing is set: its global sum is assembled before the forcing"""
         if before_forcing is not None:
             self._each(before_forcing)
         self.t.exchange(self.solvers, 0, self.new_buffer)      # ghosts of W^n
@@ -246,6 +277,8 @@ class SlabStepper:
             self.t.exchange(self.solvers, 0, self.new_buffer)  # ghosts of the un-forced W^{n+1}
         if rotor is not None:
             rotor.evaluate(self.t, self.solvers, self.many)
+        if bulk:
+            self._bulk()
         self._each(lambda s: s.step_force(dt))
         if rotor is not None:
             rotor.advance(dt)

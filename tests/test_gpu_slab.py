@@ -20,13 +20,15 @@ def run_slabs(w, world, steps, linear=False):
             s.set_reconstruction(1)
         if w.ibm is not None:
             s.ibm_set_points(*d.ibm_points(r, *w.ibm))
+        if w.bulk_flux is not None:
+            s.set_bulk_flux(*w.bulk_flux)
         s.set_state(d.scatter(w.W0, r))
     newbuf = slab.BufferPool("cuda:0")
     stepper = slab.SlabStepper(slab.LocalTransport(d), solvers, newbuf)
     for k in range(steps):
         pts = w.alm(k) if w.alm is not None else None
         stepper.step(w.dt, before_forcing=(lambda s: s.alm_set_points(*pts)) if pts is not None else None,
-                     ibm=w.ibm is not None)
+                     ibm=w.ibm is not None, bulk=w.bulk_flux is not None)
     W = d.gather([s.get_state() for s in solvers])
     for s in solvers:
         s.close()
@@ -40,6 +42,8 @@ def run_single(w, steps, linear=False):
         g.set_reconstruction(1)
     if w.ibm is not None:
         g.ibm_set_points(*w.ibm)
+    if w.bulk_flux is not None:
+        g.set_bulk_flux(*w.bulk_flux)
     g.set_state(w.W0)
     for k in range(steps):
         if w.alm is not None:
@@ -57,6 +61,25 @@ def test_periodic_box_in_slabs_equals_the_single_domain(world):
     # same arithmetic per cell up to the warp-uniform choice of the erf/exp series length, which depends on the
     # other faces of the tile (8 terms if all have z^2 <= 1/64, else 12/14): both are exact to 1e-17
     assert rel_linf(Ws, W1) <= 1e-13
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_channel_with_bulk_flux_forcing_in_slabs(world):
+    """small C2: periodic x, stretched no-slip y, bulk-flux forcing = one global sum per step, assembled from the
+    sub-domains' partial sums"""
+    from oracle import binding as ob
+    w = wl.by_name("C2", small=True)
+    Ws, W1 = run_slabs(w, world, 3), run_single(w, 3)
+    assert rel_linf(Ws, W1) <= 1e-13
+    o = ob.Oracle(w.cfg)
+    o.set_bulk_flux(*w.bulk_flux)
+    o.set_state(w.W0)
+    for _ in range(3):
+        o.step(w.dt)
+    assert rel_linf(Ws, o.get_state()) <= 3e-11
+    vol = np.einsum("k,j,i->kji", w.cfg.widths(2), w.cfg.widths(1), w.cfg.widths(0))
+    assert (Ws[1] * vol).sum() / vol.sum() == pytest.approx(w.bulk_flux[1], rel=1e-12)
+    o.close()
 
 
 def test_rotor_box_in_four_slabs_with_the_rotor_on_a_cut():
@@ -162,8 +185,16 @@ def test_linear_variant_and_error_paths():
         g.halo_pack(1, 0, buf)                               # W* only exists inside a step
     with pytest.raises(gks.GksError):
         g.step_finish(w.dt)                                  # without begin
+    g.set_bulk_flux(0, 0.1)
+    g.step_begin(w.dt)
+    g.step_finish(w.dt)
     with pytest.raises(gks.GksError):
-        g.set_bulk_flux(0, 0.1)                              # needs a global sum
+        g.step_force(w.dt)                                   # the global bulk sum was not supplied
+    part = torch.zeros(1, dtype=torch.float64, device="cuda:0")
+    vol = g.bulk_partial(part)
+    g.bulk_set_global(part, vol)
+    g.step_force(w.dt)
+    g.set_bulk_flux(-1, 0.0)
     g.halo_pack(0, 0, buf)
     host = torch.empty(g.halo_doubles(1), dtype=torch.float64)
     g.halo_pack(0, 1, host)                                  # host buffers are accepted too

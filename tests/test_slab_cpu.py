@@ -115,6 +115,8 @@ def _dist_worker(rank, world, port, periodic, W, q):
         a = torch.full((5, 3), float(rank)) if rank == world - 1 else torch.zeros((5, 3))
         t.broadcast(s, world - 1, [a])
         assert torch.equal(a, torch.full((5, 3), float(world - 1)))
+        tot, vol = t.all_reduce_sum(s, torch.tensor([float(rank + 1)], dtype=torch.float64), 0.5 * (rank + 1))
+        assert float(tot) == world * (world + 1) / 2 and vol == pytest.approx(0.25 * world * (world + 1))
         q.put((rank, "ok"))
     except Exception as e:                                      # noqa: BLE001 - reported to the parent
         q.put((rank, repr(e)))
