@@ -93,7 +93,14 @@ struct Tile {
                                                        cell a0-3: TMA needs a 16-byte aligned box start (even index) */
   static constexpr int CB = NA ? T1 + 4 : TN + 5;
   static constexpr int EA = (CA + 1) & ~1;          /* TMA box: inner extent even (16-byte rows) */
-  static constexpr int EB = CB;
+  /* rows of the box: padded until the component stride EB*EA is 4 or 12 (mod 16 doubles), which makes the
+     (component, cell) lanes of stage A hit 16 different bank pairs */
+  static constexpr int eb_pad(int cb, int ea) {
+    int eb = cb;
+    while ((eb * ea) % 16 != 4 && (eb * ea) % 16 != 12) ++eb;
+    return eb;
+  }
+  static constexpr int EB = eb_pad(CB, EA);
   static constexpr int HA = NA ? TN : T1 + 4;       /* halo-face box (faces needed by pass 1) */
   static constexpr int HB = NA ? T1 + 4 : TN;
   static constexpr int FH = HA * HB;
@@ -106,7 +113,9 @@ struct Tile {
   static constexpr int WSLAB_PAD = (WSLAB + 15) & ~15;
   /* shared memory carve (doubles) */
   static constexpr int OFF_W = 0;                          /* 2 slabs (TMA destinations) */
-  static constexpr int SBUF = 3 * FH * 4;                  /* one stage buffer: QL->Q0 | QR | Dn, each [FH][4] */
+  static constexpr int SBUF = 3 * FH * 4 + 8;              /* one stage buffer: QL->Q0 | QR | Dn, each [FH][4]; QR and Dn
+                                                              are shifted by 2 and 4 doubles against bank conflicts
+                                                              between the QL and QR rows of a face (stage BC) */
   static constexpr int OFF_S = OFF_W + 2 * WSLAB_PAD;      /* 3 stage buffers (plane j lives in buffer j % 3) */
   static constexpr int OFF_XB = OFF_S + 3 * SBUF;          /* transpose buffer, 64 doubles per face, XOR-swizzled */
   static constexpr int OFF_RING = OFF_XB + NF * 64;        /* 4-plane ring of pass-1 results [4][6][NF][4] */
@@ -251,7 +260,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
 #pragma unroll
   for (int cc = 0; cc < 4; ++cc) ro[cc] = 4 * (cc ^ (fid & 3)) + (c ^ cc);
   constexpr int sn = T::NA ? 1 : EA;            /* slab stride along the normal */
-  constexpr int QLo = 0, QRo = FH * 4, DNo = 2 * FH * 4;   /* offsets inside a stage buffer */
+  constexpr int QLo = 0, QRo = FH * 4 + 2, DNo = 2 * FH * 4 + 4;   /* offsets inside a stage buffer */
 
   for (int i = 0; i < J + 2; ++i) {
     if (i > 0) mbar_wait(&bar[2], (i - 1) & 1);   /* every warp has finished A, BC, D of iteration i-1 */
@@ -438,8 +447,8 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
       __syncwarp();                               /* every lane has consumed its reads: the buffer is reusable */
       /* face average: the 4 lanes of a face (one Gauss point each) leave their F, dF in the warp-private
          buffer, lane c sums component c in the order (g0+g1)+(g2+g3).  Row v of face fid sits at
-         ((v ^ (fid&3)) * 4 + gp), faces of a pair are offset by 2 doubles: conflict-free stores, 128-bit loads */
-      double *const xs = XBuf + fid * 64 + 2 * (fid & 1);
+         ((v ^ (fid&3)) * 4 + gp): conflict-free 64-bit stores and loads */
+      double *const xs = XBuf + fid * 64;
       const int f3 = fid & 3;
 #pragma unroll
       for (int v = 0; v < 4; ++v) {
@@ -449,13 +458,9 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
       __syncwarp();
       double fsel = 0.0, dsel;
       {
-        const double2 *r = reinterpret_cast<const double2 *>(xs + (c ^ f3) * 4);
-        if (NEED_F) {
-          const double2 u0 = r[0], u1 = r[1];
-          fsel = (u0.x + u0.y) + (u1.x + u1.y);
-        }
-        const double2 w0 = r[8], w1 = r[9];
-        dsel = (w0.x + w0.y) + (w1.x + w1.y);
+        const double *r = xs + (c ^ f3) * 4;
+        if (NEED_F) fsel = (r[0] + r[1]) + (r[2] + r[3]);
+        dsel = (r[16] + r[17]) + (r[18] + r[19]);
       }
       __syncwarp();                               /* pass 2 of the next plane writes the buffer again */
       if (face_ok) {
