@@ -118,7 +118,12 @@ gks_status gks_step(gks_ctx *ctx, double dt);
  *       global sum: between finish and force every sub-domain calls gks_bulk_partial (its sum of
  *       m_axis |Omega| over the un-forced field and its volume), the driver adds them up (one scalar
  *       all-reduce) and returns the totals with gks_bulk_set_global (sum: host or device pointer).
- *       Not available on a sub-domain: more than one IBM pass, alm_set_rotor (use alm_rotor_points).
+ *       More than one IBM pass (ibm_set_iterations) needs the neighbours' increments between the passes and a
+ *       common stop decision: between finish and force the driver runs, for pass k = 0 .. max_iter-1,
+ *       [k > 0: exchange of the HALO ghosts, which = 0]  gks_ibm_pass(ctx, k, 0) (interpolate; records this
+ *       sub-domain's max slip)  [k > 0: gks_ibm_residual get -> MAX over the sub-domains -> set]
+ *       gks_ibm_pass(ctx, k, 1) (spread; skipped on the device once the slip fell below tol); gks_step_force
+ *       then leaves the IBM alone.  Not available on a sub-domain: alm_set_rotor (use alm_rotor_points).
  * gks_step = begin + finish + force.  Errors: GKS_ERR_INVALID_ARG (face without HALO, NULL), GKS_ERR_STATE
  * (order of the calls). */
 size_t gks_halo_doubles(const gks_ctx *ctx, int face);
@@ -127,6 +132,8 @@ gks_status gks_halo_unpack(gks_ctx *ctx, int which, int face, const double *buf)
 gks_status gks_step_begin(gks_ctx *ctx, double dt);
 gks_status gks_step_finish(gks_ctx *ctx, double dt);
 gks_status gks_step_force(gks_ctx *ctx, double dt);
+gks_status gks_ibm_pass(gks_ctx *ctx, int pass, int phase /* 0 interpolate, 1 spread */);
+gks_status gks_ibm_residual(gks_ctx *ctx, int pass, double *value /* host or device */, int set /* 0 get, 1 set */);
 gks_status gks_bulk_partial(gks_ctx *ctx, double *sum, double *volume /* host, may be NULL */);
 gks_status gks_bulk_set_global(gks_ctx *ctx, const double *sum, double volume);
 

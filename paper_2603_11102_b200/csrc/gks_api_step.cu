@@ -165,8 +165,8 @@ gks_status gks_step_force(gks_ctx *ctx, double dt) {
   cudaStream_t s = ctx->stream;
   bool any_halo = false;
   for (int f = 0; f < 6; ++f) any_halo = any_halo || g.halo[f];
-  if (any_halo && ctx->n_ibm > 0 && ctx->ibm_maxit > 1)
-    return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "IBM passes > 1 need an exchange per pass: not available on a sub-domain");
+  if (any_halo && ctx->n_ibm > 0 && ctx->ibm_maxit > 1 && !ctx->ibm_external)
+    return gks_set_err(ctx, GKS_ERR_STATE, "IBM passes > 1 on a sub-domain need an exchange per pass: drive them with gks_ibm_pass");
   if (any_halo && ctx->bulk_axis >= 0 && !ctx->bulk_external)
     return gks_set_err(ctx, GKS_ERR_STATE, "bulk-flux forcing on a sub-domain: gks_bulk_set_global must supply the global sum first");
   if (any_halo && ctx->rotor_on)
@@ -184,7 +184,9 @@ gks_status gks_step_force(gks_ctx *ctx, double dt) {
   const bool ext = ctx->bulk_external != 0;       /* sub-domain: the global sum is already in place */
   ctx->bulk_external = 0;
   if (ctx->bulk_axis >= 0 && !ext) ctx->launches += gks_launch_bulk_reduce(g, ctx->Wn, ctx->bulk_axis, ctx->red, s);
-  if (ctx->n_ibm > 0) {
+  const bool ibm_done = ctx->ibm_external != 0;   /* sub-domain: the passes were driven with gks_ibm_pass */
+  ctx->ibm_external = 0;
+  if (ctx->n_ibm > 0 && !ibm_done) {
     /* multi-direct-forcing passes (Eq. 11-12): pass k interpolates from the un-forced field plus the IBM
        increments of the passes before it, in place; nothing else has touched the momentum yet (S12) */
     unsigned long long *res = reinterpret_cast<unsigned long long *>(ctx->red + GKS_RED_IBM_RES);
@@ -267,6 +269,38 @@ gks_status gks_set_bulk_flux(gks_ctx *ctx, int axis, double target) {
 
   ctx->bulk_axis = axis < 0 ? -1 : axis;
   ctx->bulk_target = target;
+  return GKS_OK;
+}
+
+gks_status gks_ibm_pass(gks_ctx *ctx, int pass, int phase) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (pass < 0 || pass >= ctx->ibm_maxit || (phase != 0 && phase != 1))
+    return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "pass must be in [0, max_iter) and phase 0 (interpolate) or 1 (spread)");
+  if (ctx->mid_step != 2) return gks_set_err(ctx, GKS_ERR_STATE, "gks_ibm_pass belongs between gks_step_finish and gks_step_force");
+  unsigned long long *res = reinterpret_cast<unsigned long long *>(ctx->red + GKS_RED_IBM_RES);
+  if (pass == 0 && phase == 0)
+    CUDA_TRY(ctx, cudaMemsetAsync(res, 0, GKS_IBM_MAX_PASSES * sizeof(unsigned long long), ctx->stream));
+  ctx->ibm_external = 1;
+  if (ctx->n_ibm > 0) {
+    if (phase == 0)
+      ctx->launches += gks_launch_ibm_interp(ctx->g, ctx->Wn, ctx->n_ibm, ctx->ibm_pos, ctx->ibm_vol, ctx->ibm_vel,
+                                             ctx->ibm_coef, pass, ctx->ibm_tol, res, ctx->stream);
+    else
+      ctx->launches += gks_launch_ibm_spread(ctx->g, ctx->Wn, ctx->n_ibm, ctx->ibm_pos, ctx->ibm_coef, pass, ctx->ibm_tol,
+                                             res, ctx->stream);
+    CUDA_TRY(ctx, cudaGetLastError());
+  }
+  return GKS_OK;
+}
+
+gks_status gks_ibm_residual(gks_ctx *ctx, int pass, double *value, int set) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (!value || pass < 0 || pass >= GKS_IBM_MAX_PASSES) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "value is NULL or pass out of range");
+  double *slot = ctx->red + GKS_RED_IBM_RES + pass;   /* a non-negative double (its bit pattern orders like an integer) */
+  const bool dev = gks_is_device_ptr(value);
+  if (set) CUDA_TRY(ctx, cudaMemcpyAsync(slot, value, sizeof(double), dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, ctx->stream));
+  else CUDA_TRY(ctx, cudaMemcpyAsync(value, slot, sizeof(double), dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream));
+  if (!dev) CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
   return GKS_OK;
 }
 

@@ -84,6 +84,7 @@ struct gks_ctx {
   double gacc[3];
   int bulk_axis;
   double bulk_target, total_volume;
+  int ibm_external;            /* sub-domain: this step's IBM passes were driven with gks_ibm_pass */
   int bulk_external;           /* sub-domain: the global sum was supplied with gks_bulk_set_global for this step */
   double bulk_volume_ext;      /* and the global volume */
   double dmin;                 /* smallest cell width of the grid (CFL condition) */

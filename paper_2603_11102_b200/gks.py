@@ -19,7 +19,7 @@ STATUS = {0: "GKS_OK", 1: "GKS_ERR_INVALID_ARG", 2: "GKS_ERR_WORKSPACE", 3: "GKS
 
 EXPORTS = ["gks_workspace_bytes", "gks_create", "gks_destroy", "gks_set_state", "gks_get_state", "gks_step",
            "gks_set_body_force", "gks_set_bulk_flux", "alm_set_points", "ibm_set_points", "ibm_set_velocities", "ibm_set_iterations", "gks_cfl_dt", "alm_set_rotor", "alm_rotor_eval", "alm_rotor_points", "gks_set_reconstruction", "gks_halo_doubles", "gks_halo_pack", "gks_halo_unpack", "gks_step_begin",
-           "gks_step_finish", "gks_step_force", "gks_bulk_partial", "gks_bulk_set_global",
+           "gks_step_finish", "gks_step_force", "gks_bulk_partial", "gks_bulk_set_global", "gks_ibm_pass", "gks_ibm_residual",
            "gks_debug_eval_flux", "gks_debug_set_sweep", "gks_debug_fp64_peak",
            "gks_profile_enable", "gks_profile_read", "gks_check_finite", "gks_launch_count", "gks_last_error"]
 
@@ -83,6 +83,8 @@ def lib():
         L.gks_step_force.argtypes = [vp, C.c_double]
         L.gks_bulk_partial.argtypes = [vp, vp, C.POINTER(C.c_double)]
         L.gks_bulk_set_global.argtypes = [vp, vp, C.c_double]
+        L.gks_ibm_pass.argtypes = [vp, C.c_int, C.c_int]
+        L.gks_ibm_residual.argtypes = [vp, C.c_int, vp, C.c_int]
         L.gks_debug_eval_flux.argtypes = [vp, C.c_int, vp, vp]
         L.gks_debug_set_sweep.argtypes = [vp, C.c_int]
         L.gks_check_finite.argtypes = [vp]
@@ -268,6 +270,13 @@ class Gks:
 
     def step_force(self, dt):
         self._check(lib().gks_step_force(self._h, float(dt)))
+
+    def ibm_pass(self, k, phase):
+        self._check(lib().gks_ibm_pass(self._h, int(k), int(phase)))
+
+    def ibm_residual(self, k, tensor, set=False):
+        """get / set the max slip recorded by pass k (1-element float64 torch tensor, CUDA or CPU)"""
+        self._check(lib().gks_ibm_residual(self._h, int(k), tensor.data_ptr(), 1 if set else 0))
 
     def bulk_partial(self, out):
         """out: 1-element float64 torch tensor (CUDA or CPU) receiving this sub-domain's sum of m_axis |Omega|;

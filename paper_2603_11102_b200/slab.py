@@ -16,8 +16,8 @@ This module holds host logic only (who owns what, who talks to whom, in which or
 IBM points within 1.5 cells of a cut are given to both sub-domains (`SlabDecomposition.ibm_points`); both
 interpolate the same U_p after a third exchange (the un-forced W^{n+1}) and each adds to the cells it owns.
 The on-line rotor is evaluated by the sub-domain that contains the disc and broadcast (`RotorDriver`).
-The bulk-flux forcing adds the sub-domains' partial sums up with one scalar all-reduce.
-Not covered yet: more than one IBM pass (an exchange per pass).
+The bulk-flux forcing adds the sub-domains' partial sums up with one scalar all-reduce; IBM passes > 1 exchange
+the halo between the passes and take the MAX of the sub-domains' slips for the common stop decision.
 """
 from dataclasses import replace
 
@@ -172,6 +172,13 @@ class DistTransport:
             solver.synchronize()
         return pair[:1].contiguous(), float(pair[1])
 
+    def all_reduce_max(self, solver, scalar):
+        import contextlib
+        import torch
+        with (torch.cuda.stream(solver.stream) if scalar.is_cuda else contextlib.nullcontext()):
+            self.dist.all_reduce(scalar, op=self.dist.ReduceOp.MAX, group=self.group)
+        return scalar
+
     def broadcast(self, solver, src, tensors):
         import contextlib
         import torch
@@ -262,11 +269,40 @@ class SlabStepper:
         for s in sols:
             s.bulk_set_global(total, volume)
 
-    def step(self, dt, before_forcing=None, ibm=False, rotor=None, bulk=False):
+    def _ibm_passes(self, passes):
+        """multi-direct-forcing passes on sub-domains: the neighbours' increments travel between the passes and
+        the stop decision is common (MAX of the sub-domains' slips)"""
+        import torch
+        sols = self.solvers if self.many else [self.solvers]
+        dev = self.new_buffer.device if hasattr(self.new_buffer, "device") else "cpu"
+        for k in range(passes):
+            if k > 0:
+                self.t.exchange(self.solvers, 0, self.new_buffer)
+            for s in sols:
+                s.ibm_pass(k, 0)
+            if k > 0:
+                slips = [torch.zeros(1, dtype=torch.float64, device=dev) for _ in sols]
+                for s, r in zip(sols, slips):
+                    s.ibm_residual(k, r)
+                if self.many:
+                    for s in sols:
+                        s.synchronize()
+                    top = torch.stack(slips).max(0).values
+                    if top.is_cuda:
+                        torch.cuda.current_stream().synchronize()
+                else:
+                    top = self.t.all_reduce_max(sols[0], slips[0])
+                for s in sols:
+                    s.ibm_residual(k, top, set=True)
+            for s in sols:
+                s.ibm_pass(k, 1)
+
+    def step(self, dt, before_forcing=None, ibm=False, rotor=None, bulk=False, ibm_passes=1):
         """before_forcing(solver): e.g. alm_set_points for this step (replicated point list);
         ibm: Lagrangian points are set (on any rank): the un-forced W^{n+1} is exchanged before the forcing;
         rotor: a RotorDriver (on-line actuator lines), evaluated on the un-forced W^{n+1} as well;
-        bulk: the bulk-flux forcing is set: its global sum is assembled before the forcing"""
+        bulk: the bulk-flux forcing is set: its global sum is assembled before the forcing;
+        ibm_passes: the max_iter given to ibm_set_iterations on every sub-domain, when > 1"""
         if before_forcing is not None:
             self._each(before_forcing)
         self.t.exchange(self.solvers, 0, self.new_buffer)      # ghosts of W^n
@@ -279,6 +315,8 @@ class SlabStepper:
             rotor.evaluate(self.t, self.solvers, self.many)
         if bulk:
             self._bulk()
+        if ibm and ibm_passes > 1:
+            self._ibm_passes(ibm_passes)
         self._each(lambda s: s.step_force(dt))
         if rotor is not None:
             rotor.advance(dt)

@@ -171,6 +171,72 @@ def test_online_rotor_on_slabs(name, switches):
     o.close()
 
 
+@pytest.mark.parametrize("name", ["C3", "C5"])
+def test_ibm_passes_on_slabs(name):
+    """multi-direct-forcing passes with the body cut through: a fixed number of passes, and the stop rule with a
+    tolerance that ends the passes early - the decision is taken from the MAX of the sub-domains' slips"""
+    from paper_2603_11102_b200 import gks
+    w = wl.by_name(name, small=True)
+    for world in range(2, 9):
+        d = slab.SlabDecomposition(w.cfg, world)
+        cuts = w.cfg.origin[0] + d.x_lo[1:-1] * w.cfg.spacing[0]
+        if np.abs(w.ibm[0][:, :1] - cuts[None, :]).min() < 0.5 * w.cfg.spacing[0]:
+            break
+
+    def single(passes, tol):
+        g = gks.Gks(w.cfg)
+        g.ibm_set_points(*w.ibm)
+        g.ibm_set_iterations(passes, tol)
+        g.set_state(w.W0)
+        for k in range(2):
+            if w.alm is not None:
+                g.alm_set_points(*w.alm(k))
+            g.step(w.dt)
+        W = g.get_state()
+        g.close()
+        return W
+
+    def slabs(passes, tol):
+        solvers = [gks.Gks(d.local_cfg(r)) for r in range(world)]
+        for r, s in enumerate(solvers):
+            s.ibm_set_points(*d.ibm_points(r, *w.ibm))
+            s.ibm_set_iterations(passes, tol)
+            s.set_state(d.scatter(w.W0, r))
+        st = slab.SlabStepper(slab.LocalTransport(d), solvers, slab.BufferPool("cuda:0"))
+        for k in range(2):
+            pts = w.alm(k) if w.alm is not None else None
+            st.step(w.dt, before_forcing=(lambda s: s.alm_set_points(*pts)) if pts is not None else None, ibm=True,
+                    ibm_passes=passes)
+        W = d.gather([s.get_state() for s in solvers])
+        for s in solvers:
+            s.close()
+        return W
+
+    W1, W3, W8 = single(1, 0.0), single(3, 0.0), single(8, 0.0)
+    assert rel_linf(slabs(3, 0.0), W3) <= 1e-13
+    # a tolerance between the slips that stop after 3 passes: the result equals the 3-pass one, not the 8-pass one
+    o_slip = []
+    for k in (2, 3):
+        g = gks.Gks(w.cfg)
+        g.ibm_set_points(*w.ibm)
+        g.ibm_set_iterations(k, 0.0)
+        g.set_state(w.W0)
+        if w.alm is not None:
+            g.alm_set_points(np.zeros((0, 3)), np.zeros((0, 3)), 1.0)
+        g.step(w.dt)
+        from oracle import binding as ob
+        o = ob.Oracle(w.cfg)
+        o.ibm_set_points(*w.ibm)
+        o.set_state(g.get_state())
+        o_slip.append(np.linalg.norm(o.ibm_interpolate(), axis=1).max())
+        o.close()
+        g.close()
+    tol = 0.5 * (o_slip[0] + o_slip[1])
+    Wt = slabs(8, tol)
+    assert rel_linf(Wt, single(8, tol)) <= 1e-13
+    assert rel_linf(Wt, W8) > 1e-9 and rel_linf(W3, W1) > 1e-9
+
+
 def test_linear_variant_and_error_paths():
     from paper_2603_11102_b200 import gks
     w = wl.by_name("C1")

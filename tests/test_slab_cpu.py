@@ -117,6 +117,8 @@ def _dist_worker(rank, world, port, periodic, W, q):
         assert torch.equal(a, torch.full((5, 3), float(world - 1)))
         tot, vol = t.all_reduce_sum(s, torch.tensor([float(rank + 1)], dtype=torch.float64), 0.5 * (rank + 1))
         assert float(tot) == world * (world + 1) / 2 and vol == pytest.approx(0.25 * world * (world + 1))
+        top = t.all_reduce_max(s, torch.tensor([0.1 * (rank + 1)], dtype=torch.float64))
+        assert float(top) == pytest.approx(0.1 * world)
         q.put((rank, "ok"))
     except Exception as e:                                      # noqa: BLE001 - reported to the parent
         q.put((rank, repr(e)))
