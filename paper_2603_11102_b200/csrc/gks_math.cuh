@@ -348,14 +348,19 @@ __device__ __forceinline__ void erf_expm2_warp(double z, double &erfz, double &e
 }
 
 /* one of the two functions per lane: func = 0 -> erf(z), func = 1 -> exp(-z^2); the lanes of a warp run the
- * same Horner recurrence on their own coefficient set (series length chosen warp-uniformly as above) */
-__device__ __forceinline__ double erf_or_expm2_warp(double z, int func) {
+ * same Horner recurrence on their own coefficient set cf[n] = func ? GK_EXP[n] : GK_ERF[n], chosen once per thread
+ * (series length chosen warp-uniformly as above) */
+__device__ __forceinline__ void series_coefficients(int func, double (&cf)[8]) {
+#pragma unroll
+  for (int n = 0; n < 8; ++n) cf[n] = func ? GK_EXP[n] : GK_ERF[n];
+}
+__device__ __forceinline__ double erf_or_expm2_warp(double z, int func, const double (&cf)[8]) {
   const double w = z * z;
   const bool small = !(w > 1.0 / 64.0);
   if (__all_sync(0xffffffffu, small)) {
-    double p = func ? GK_EXP[7] : GK_ERF[7];
+    double p = cf[7];
 #pragma unroll
-    for (int n = 6; n >= 0; --n) p = fma(p, w, func ? GK_EXP[n] : GK_ERF[n]);
+    for (int n = 6; n >= 0; --n) p = fma(p, w, cf[n]);
     return func ? p : p * z;
   }
   double erfz, ex;

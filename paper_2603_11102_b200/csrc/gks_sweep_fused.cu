@@ -260,6 +260,8 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
 #pragma unroll
   for (int cc = 0; cc < 4; ++cc) ro[cc] = 4 * (cc ^ (fid & 3)) + (c ^ cc);
   constexpr int sn = T::NA ? 1 : EA;            /* slab stride along the normal */
+  double bcf[8];                                /* stage BC: this lane's series (its items all have cc = tid & 3) */
+  gksd::series_coefficients((tid & 3) >> 1, bcf);
   constexpr int QLo = 0, QRo = FH * 4 + 2, DNo = 2 * FH * 4 + 4;   /* offsets inside a stage buffer */
 
   for (int i = 0; i < J + 2; ++i) {
@@ -348,7 +350,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
         const double rho = qs[0];
         const double z = ph.theta * (qs[1 + DIR] * gksd::fast_rcp3(rho));
         /* lane (side, func): func 0 -> erfc(-+z)/2 of that side, func 1 -> rho exp(-z^2) / (2 sqrt(pi lambda)) */
-        const double v = gksd::erf_or_expm2_warp(z, func);
+        const double v = gksd::erf_or_expm2_warp(z, func, bcf);
         const double r = func ? rho * (ph.cx * v) : fma(side ? -0.5 : 0.5, v, 0.5);
         const double el = __shfl_sync(0xffffffffu, r, gl), er = __shfl_sync(0xffffffffu, r, gl + 1);
         const double xl = __shfl_sync(0xffffffffu, r, gl + 2), xr = __shfl_sync(0xffffffffu, r, gl + 3);
