@@ -9,20 +9,21 @@
  *     DIR 0 (x-faces): a = x = normal, b = y = t1, march z = t2
  *     DIR 1 (y-faces): a = x = t1,     b = y = normal, march z = t2
  *     DIR 2 (z-faces): a = x = t1,     b = z = normal, march y = t2
- * Per marched plane p the CTA
- *   A  reconstructs both edge values of every cell (one smoothness-indicator set per cell serves
- *      the face on either side) from the W halo slab that TMA staged in shared memory,
- *   B  evaluates the collision factors (erfc/exp) once per face,
- *   C  forms Q0 and the normal slope Dn on the TN x (T1+4) halo faces,
- *   D  runs tangential pass 1 (along t1) and pushes 24 doubles per face into a 5-plane ring in
- *      shared memory,
- *   E  runs tangential pass 2 (along t2) for plane p-2 out of the ring,
- *   F  evaluates the four Gauss-point fluxes and writes the face average F, dF/dt to HBM.
- * Thread mapping: 4 threads per face.  In A-E thread (face, c) owns component c (WENO is
- * component-wise); in F thread (face, g) owns Gauss point g (the flux couples all components);
- * the 4x4 transpose goes through shared memory and needs only __syncwarp.
- * The W slab of plane p+2 is fetched by TMA (cp.async.bulk.tensor, mbarrier completion) while plane
- * p is processed: 2-stage pipeline, one elected thread issues.
+ * Per marched plane the CTA runs the stages
+ *   A   both WENO5 edge values of every cell (one smoothness-indicator set per cell serves the face on
+ *       either side) and the normal slope Dn, from the W halo slab that TMA staged in shared memory,
+ *   BC  the collision Q0(QL, QR) on the TN x (T1+4) halo faces (four lanes per face split sides and series),
+ *   D   tangential pass 1 (along t1): 6 values per (face, component),
+ *   EF  tangential pass 2 (along t2) for the plane two behind, out of a thread-private 4-plane ring in shared
+ *       memory (the newest plane comes from D's registers), the four Gauss-point fluxes, the face average
+ *       F, dF/dt to HBM,
+ * software-pipelined over three planes per iteration (k_sweep_fused's comment has the schedule, the
+ * persistent wave-major work distribution and the single split mbarrier hand-over per iteration).
+ * Thread mapping: 4 threads per face.  In A-E thread (face, c) owns component c (WENO is component-wise);
+ * in F thread (face, g) owns Gauss point g (the flux couples all components); the 4x4 transpose goes
+ * through a swizzled warp-private buffer and needs only __syncwarp.
+ * The W slab of the next plane is fetched by TMA (cp.async.bulk.tensor, mbarrier completion) one iteration
+ * ahead: 2 slab buffers, one elected thread issues.
  *
  * Roofline: fp64-ALU bound (about 4.7 kflop per face against 32 B read + 64 B written per face).
  */
