@@ -311,3 +311,38 @@ def test_linear_tangential_variant_matches_the_oracle(sweep):
             with pytest.raises(gks.GksError):
                 g.set_reconstruction(3)
         g.close()
+
+
+def test_split_step_equals_gks_step_and_enforces_the_call_order():
+    """gks_step = gks_step_begin + gks_step_finish + gks_step_force (the form the x-slab driver uses), bit for bit on
+    the small turbine box (IBM atomics aside: compared to 1e-14), and the calls refuse a wrong order"""
+    from paper_2603_11102_b200 import gks
+    w = wl.by_name("C5", small=True)
+    res = []
+    for split in (False, True):
+        g = gks.Gks(w.cfg)
+        g.ibm_set_points(*w.ibm)
+        g.set_state(w.W0)
+        for k in range(3):
+            g.alm_set_points(*w.alm(k))
+            if split:
+                g.step_begin(w.dt)
+                g.step_finish(w.dt)
+                g.step_force(w.dt)
+            else:
+                g.step(w.dt)
+        res.append(g.get_state())
+        if split:
+            with pytest.raises(gks.GksError):
+                g.step_force(w.dt)
+            g.step_begin(w.dt)
+            with pytest.raises(gks.GksError):
+                g.step_begin(w.dt)
+            with pytest.raises(gks.GksError):
+                g.step(w.dt)
+            with pytest.raises(gks.GksError):
+                g.step_force(w.dt)
+            g.step_finish(w.dt)
+            g.step_force(w.dt)
+        g.close()
+    assert rel_linf(res[1], res[0]) <= 1e-14
