@@ -16,14 +16,21 @@
  *   Eq. 10  ALM Gaussian projection, cut at 3 eps
  *   Eq. 11-12 IBM direct forcing
  *   Eq. 13  momentum update with body force
- * Readings S1..S24 (where the paper is silent) are those of DESIGN.md / SURVEY.md §8(c).
+ *   multi-direct-forcing passes of the IBM, stop rule
+ *   ALM front half: trilinear sampling, Eq. 9, free-stream correction
+ *   Eq. 14  tip correction
+ *   CFL time step
+ * Readings S1..S27 (where the paper is silent) are those of DESIGN.md / SURVEY.md §8(c).
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): moment recursion vs quadrature (P1), polynomial
  * exactness of every reconstruction operator (P2), Appendix solve (P3), collision special cases
  * (P4), Navier-Stokes flux identity + brute-force velocity-space quadrature (P5, P13), free-stream
  * preservation (P6), conservation (P7), order of accuracy on an exact simple wave (P8), viscous
  * decay (P9), acoustic speed (P10), ALM integral (P11), IBM delta identities (P12), axis
- * permutation symmetry (P14).
+ * permutation symmetry (P14), IBM passes: closed-form contraction of an isolated point (P15), CFL time step:
+ * hand-worked numbers (P16), ALM front half: geometry, exact sampling of trilinear fields, lift normal / drag
+ * parallel to the relative flow, correction identities, a worked tip factor (P17), linear-weight tangential
+ * variant: SURVEY's value row, exactness for quartics, order of accuracy (P18).
  * PARITY UNPINNED (no independent check exists in the paper): the stretched-grid metric choice
  * (S10), the convective-outflow ghost update (S20), the Riemann-invariant inflow density (S19).
  */

@@ -8,7 +8,8 @@
  *
  * The oracle is the algorithm of arxiv/paper_2603_11102 written out step by step, slowly, in fp64:
  * PAPER.md §2 (:41-93), Appendix (:501-558), §3.1 Eq. 10 (:135-139, :293), §3.2 (:141-175),
- * §3.3 (:177-191), with the readings S1..S24 of DESIGN.md where the paper is silent.
+ * §3.3 (:177-191), the ALM front half (:101-127, Eq. 14 :388-399), the CFL condition (:91), with the readings
+ * S1..S27 of DESIGN.md where the paper is silent.
  *
  * All pointers are HOST pointers.  Layouts: W[c][k][j][i] interior cells only, c in
  * {rho, rhoU, rhoV, rhoW}.  Return value 0 = ok, non-zero = error (gkso_last_error()).
