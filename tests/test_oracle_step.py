@@ -3,6 +3,7 @@
 CPU only.  Sizes are chosen so that the file runs in about a minute.
 """
 import math
+import os
 
 import numpy as np
 import pytest
@@ -545,10 +546,18 @@ def test_P17_corrections():
         assert f[rad < 0.2].min() > 0.99 and f[-1] < 0.2
     assert np.abs(f_ax - f_tan).max() > 1e-3
     # worked value: N = 3, lambda = 7, r = 0.9 R, phi from a uniform wind: f = 2/pi acos(exp(-g1 N (R-r)/(2 r sin phi)))
+    # with the constants the paper prints (tests/golden/paper_constants.txt), axial and tangential
+    gold = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "paper_constants.txt")) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                gold[line.split()[0]] = float(line.split()[1])
     i = np.argmin(np.abs(rad - 0.9))
     sphi = math.sin(math.atan2(0.1, 0.7 * rad[i]))
-    g1 = math.exp(-0.1219 * (3 * 7.0 - 21.52)) + 0.1
-    assert f_ax[i] == pytest.approx(2 / math.pi * math.acos(math.exp(-g1 * 3 * (1.0 - rad[i]) / (2 * rad[i] * sphi))), rel=1e-10)
+    for f_meas, kind in ((f_ax, "axial"), (f_tan, "tangential")):
+        g1 = math.exp(-gold["tip_c1_" + kind] * (3 * 7.0 - gold["tip_c2_" + kind])) + 0.1
+        want = 2 / math.pi * math.acos(math.exp(-g1 * 3 * (1.0 - rad[i]) / (2 * rad[i] * sphi)))
+        assert f_meas[i] == pytest.approx(want, rel=1e-10)
     with pytest.raises(ob.OracleError):
         bad = mk(tip_correction=True)
         bad.u_ref = 0.0
