@@ -30,9 +30,11 @@
  * permutation symmetry (P14), IBM passes: closed-form contraction of an isolated point (P15), CFL time step:
  * hand-worked numbers (P16), ALM front half: geometry, exact sampling of trilinear fields, lift normal / drag
  * parallel to the relative flow, correction identities, a worked tip factor (P17), linear-weight tangential
- * variant: SURVEY's value row, exactness for quartics, order of accuracy (P18).
- * PARITY UNPINNED (no independent check exists in the paper): the stretched-grid metric choice
- * (S10), the convective-outflow ghost update (S20), the Riemann-invariant inflow density (S19).
+ * variant: SURVEY's value row, exactness for quartics, order of accuracy (P18), stretched-grid metrics (S10):
+ * the Couette stress -mu a through every face family and the decay rate of a wall-bounded vortex, both second
+ * order under refinement (P19), inflow density (S19): the Rankine-Hugoniot plateau, velocity and injected mass of
+ * the piston problem (P20), convective outflow (S20): an exactly advected vortical pulse leaves without reflection
+ * (P21).  The paper prints no numbers for S10, S19, S20; the pins are exact solutions of the equations it solves.
  */
 #include "gks_oracle.h"
 

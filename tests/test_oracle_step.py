@@ -1,6 +1,6 @@
-"""Pins of the oracle's whole step against invariants, exact solutions and closed forms (P6-P12, P14).
+"""Pins of the oracle's whole step against invariants, exact solutions and closed forms (P6-P12, P14-P21).
 
-CPU only.  Sizes are chosen so that the file runs in about a minute.
+CPU only.  Sizes are chosen so that the file runs in about two minutes.
 """
 import math
 import os
@@ -625,3 +625,161 @@ def test_P18_linear_tangential_variant():
     assert math.log2(e16 / e32) >= 3.5 and e32 < 2e-6
     with pytest.raises(ob.OracleError):
         ob.Oracle(cfg).set_reconstruction(2)
+
+
+# ---------------------------------------------------------------- P19 stretched-grid metrics (reading S10)
+def exp_faces(N, ratio=3.0):
+    """smooth one-sided stretching of [0, 1]: the last cell is `ratio` times as wide as the first; one-sided, so that
+    a first-order metric error cannot cancel between the two ends"""
+    b = math.log(ratio)
+    return (np.exp(b * np.arange(N + 1) / N) - 1.0) / (math.exp(b) - 1.0)
+
+
+def couette_stress_errors(N, s, m, nu=0.05, a=0.02):
+    """rho = 1, velocity component m = a x_s (plane Couette flow), axis s stretched.  Navier-Stokes: the flux of
+    momentum m through faces normal to s and the flux of momentum s through faces normal to m are both -mu a,
+    everywhere.  Returns the two relative errors away from the (non-linear) boundary ghosts."""
+    sf = exp_faces(N)
+    n = [6, 6, 6]
+    n[s] = N
+    faces = [None, None, None]
+    faces[s] = sf
+    bc = [P] * 6
+    bc[2 * s] = bc[2 * s + 1] = EX
+    cfg = GridConfig(n=tuple(n), faces=tuple(faces), spacing=(0.1, 0.1, 0.1), RT=1.0, nu=nu, bc=tuple(bc))
+    W0 = const_state(n, (1.0, 0.0, 0.0, 0.0))
+    shape = [1, 1, 1]
+    shape[2 - s] = N
+    W0[1 + m] = a * (0.5 * (sf[1:] + sf[:-1])).reshape(shape)      # the cell average of a linear profile
+    o = ob.Oracle(cfg)
+    o.set_state(W0)
+    Fs, _ = o.eval_flux(s)
+    Fm, _ = o.eval_flux(m)
+    o.close()
+    core = [slice(None)] * 3
+    core[2 - s] = slice(4, N - 4)
+    core = tuple(core)
+    return np.abs(Fs[1 + m][core] / (-nu * a) - 1).max(), np.abs(Fm[1 + s][core] / (-nu * a) - 1).max()
+
+
+@pytest.mark.parametrize("s,m", [(0, 1), (0, 2), (1, 0), (1, 2), (2, 0), (2, 1)])
+def test_P19_couette_stress_on_a_stretched_axis_is_second_order(s, m):
+    """S10 divides index-space slopes by the centre distance (normal) or the cell width (tangential, both passes).
+    Either is a second-order approximation of the metric; taking the other one is first order (3 % at 16 cells).
+    The six (s, m) pairs reach the normal slope of every sweep and the t1 and t2 slopes of every sweep."""
+    n16, t16 = couette_stress_errors(16, s, m)
+    n32, t32 = couette_stress_errors(32, s, m)
+    assert n32 < 1.5e-4 and t32 < 1.5e-4
+    assert n16 / n32 > 3.5 and t16 / t32 > 3.5
+
+
+def vortex_decay_rate_error(N, nu=0.05, U0=0.01, T=0.1):
+    """u = U0 sin(kx) cos(ky), v = -U0 cos(kx) sin(ky) between slip walls at y = 0, 1 (k = pi) decays at 2 nu k^2
+    (incompressible Navier-Stokes; the compressible correction is O(Ma^2) = 1e-4); x uniform, y stretched"""
+    k = math.pi
+    yf, xf = exp_faces(N), 2.0 * np.arange(N + 1) / N
+    avg = lambda F, f: (F(f[1:]) - F(f[:-1])) / np.diff(f)
+    sx, cx = avg(lambda x: -np.cos(k * x) / k, xf), avg(lambda x: np.sin(k * x) / k, xf)
+    sy, cy = avg(lambda y: -np.cos(k * y) / k, yf), avg(lambda y: np.sin(k * y) / k, yf)
+    cfg = GridConfig(n=(N, N, 6), faces=(None, yf, None), spacing=(2.0 / N, 1.0, 0.1), RT=1.0, nu=nu,
+                     bc=(P, P, SL, SL, P, P))
+    W0 = const_state((N, N, 6), (1.0, 0.0, 0.0, 0.0))
+    W0[1] = U0 * (cy[:, None] * sx[None, :])[None]
+    W0[2] = -U0 * (sy[:, None] * cx[None, :])[None]
+    hmin = min(np.diff(yf).min(), 2.0 / N)
+    steps = math.ceil(T / min(0.3 * hmin, 0.15 * hmin ** 2 / nu))
+    W = run(cfg, W0, T / steps, steps)
+    wy, mode = np.diff(yf), cy[:, None] * sx[None, :]
+    amp = (W[1].mean(0) * mode * wy[:, None]).sum() / (mode ** 2 * wy[:, None]).sum() / U0
+    return -math.log(amp) / T / (2 * nu * k * k) - 1.0
+
+
+def test_P19_vortex_between_slip_walls_on_a_stretched_axis_decays_at_2_nu_k2():
+    """the whole step on a stretched axis: normal slope / centre distance, flux difference / cell width, mirrored
+    ghost widths at the walls.  A metric that is off by one cell is first order: 1.4 % at 32 cells"""
+    e16, e32 = vortex_decay_rate_error(16), vortex_decay_rate_error(32)
+    assert abs(e32) < 1.5e-3 and abs(e16 / e32) > 3.0
+
+
+# ---------------------------------------------------------------- P20 inflow (reading S19): the piston problem
+@pytest.mark.parametrize("axis,side", [(0, 0), (1, 1)])
+def test_P20_impulsive_inflow_drives_the_rankine_hugoniot_shock(axis, side):
+    """Gas at rest, inflow face switched on at U_b = 0.1 c_s: a piston.  Exact solution of the isothermal Euler
+    equations: a shock with (r - 1)^2 = r M^2, r = rho_1 / rho_0, M = U_b / c_s, speed r U_b / (r - 1); behind it
+    rho_1 and U_b; the mass that entered is rho_1 U_b t.  The ghost density of S19 (outgoing invariant) meets all
+    three; its sign flipped, a Dirichlet density or a zero-gradient density each miss at least one by > 5x."""
+    N, M, RT, T = 200, 0.1, 1.0, 0.8
+    cs = math.sqrt(RT)
+    Ub, h = M * cs, 2.0 / N
+    n = [6, 6, 6]
+    n[axis] = N
+    bc = [P] * 6
+    bc[2 * axis + side], bc[2 * axis + 1 - side] = IN, EX
+    inflow = [1.0, 0.0, 0.0, 0.0]
+    inflow[1 + axis] = Ub if side == 0 else -Ub
+    cfg = GridConfig(n=tuple(n), spacing=(h, h, h), RT=RT, nu=0.0, bc=tuple(bc), inflow=tuple(inflow))
+    steps = math.ceil(T / (0.3 * h / (cs + Ub)))
+    W = run(cfg, const_state(n, (1.0, 0.0, 0.0, 0.0)), T / steps, steps)
+    line = [0, 0, 0]
+    line[2 - axis] = slice(None)
+    rho, mom = W[0][tuple(line)], W[1 + axis][tuple(line)]
+    if side == 1:
+        rho, mom = rho[::-1], -mom[::-1]
+    r = 1 + M * M / 2 + M * math.sqrt(1 + M * M / 4)
+    assert (r - 1) ** 2 == pytest.approx(r * M * M, rel=1e-12)
+    speed = r * Ub / (r - 1)
+    x = (np.arange(N) + 0.5) * h
+    plateau = (x > 0.1) & (x < speed * T - 0.15)
+    assert plateau.sum() > 50
+    assert np.abs(rho[plateau] - r).max() < 3e-4                       # the jump itself is 0.105
+    assert np.abs(mom[plateau] / rho[plateau] - Ub).max() < 2e-3 * Ub
+    assert (rho - 1).sum() * h == pytest.approx(r * Ub * T, rel=1e-3)  # mass through the inflow face
+    ahead = x > speed * T + 0.15
+    assert np.abs(rho[ahead] - 1).max() < 1e-5                          # nothing outruns the shock
+
+
+# ---------------------------------------------------------------- P21 convective outflow (reading S20)
+@pytest.mark.parametrize("axis,side", [(0, 1), (1, 0)])
+def test_P21_vortical_pulse_leaves_through_the_convective_outflow(axis, side):
+    """rho = 1, normal velocity U0, a transverse velocity A exp(-(x - x0 - U0 t)^2 / 2 sigma^2): an exact solution of
+    the isothermal Euler equations (rho and the normal velocity stay uniform, the transverse momentum is advected).
+    The pulse crosses the outflow face at t = 4/3; the interior must follow the exact solution while it leaves and
+    be quiet afterwards.  S20's ghost update does (0.9 % of A at 4 cells per sigma); frozen ghosts give 18 % and more,
+    the sign of C flipped blows up, C doubled gives 3.4 %."""
+    N, U0, A, sig, x0 = 40, 0.3, 0.01, 0.1, 0.6
+    h = 1.0 / N
+    t_axis = (axis + 1) % 3                     # direction of the transverse velocity
+    n = [6, 6, 6]
+    n[axis] = N
+    bc = [P] * 6
+    bc[2 * axis + side], bc[2 * axis + 1 - side] = OUT, IN
+    inflow = [1.0, 0.0, 0.0, 0.0]
+    inflow[1 + axis] = U0 if side == 1 else -U0
+    cfg = GridConfig(n=tuple(n), spacing=(h, h, h), RT=1.0, nu=0.0, bc=tuple(bc), inflow=tuple(inflow))
+    xf = np.arange(N + 1) * h
+
+    def exact(t):                               # cell averages, in the coordinate that runs towards the outflow
+        F = A * sig * math.sqrt(math.pi / 2) * np.array([math.erf((v - x0 - U0 * t) / (sig * math.sqrt(2))) for v in xf])
+        return np.diff(F) / h
+
+    def along(v):                               # lay a 1-D profile along `axis`, flipped if the flow runs down the axis
+        shape = [1, 1, 1]
+        shape[2 - axis] = N
+        return (v if side == 1 else v[::-1]).reshape(shape)
+
+    W0 = const_state(n, inflow)
+    W0[1 + t_axis] = along(exact(0.0))
+    o = ob.Oracle(cfg)
+    o.set_state(W0)
+    t, dt = 0.0, 0.3 * h / (1.0 + U0)
+    for T in (1.1, 4.0 / 3.0, 1.6, 2.8):
+        steps = math.ceil((T - t) / dt - 1e-9)
+        for _ in range(steps):
+            o.step((T - t) / steps)
+        t = T
+        W = o.get_state()
+        err = np.abs(W[1 + t_axis] - along(exact(T))).max() / A
+        assert err < 0.015, T
+        assert np.abs(W[0] - 1).max() < 1e-12 and np.abs(W[1 + axis] - inflow[1 + axis]).max() < 1e-12
+    o.close()
+    assert np.abs(exact(2.8)).max() < 1e-4 * A   # by then the pulse is gone
