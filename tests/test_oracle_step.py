@@ -1,4 +1,4 @@
-"""Pins of the oracle's whole step against invariants, exact solutions and closed forms (P6-P12, P14-P21).
+"""Pins of the oracle's whole step against invariants, exact solutions and closed forms (P6-P12, P14-P22).
 
 CPU only.  Sizes are chosen so that the file runs in about two minutes.
 """
@@ -783,3 +783,60 @@ def test_P21_vortical_pulse_leaves_through_the_convective_outflow(axis, side):
         assert np.abs(W[0] - 1).max() < 1e-12 and np.abs(W[1 + axis] - inflow[1 + axis]).max() < 1e-12
     o.close()
     assert np.abs(exact(2.8)).max() < 1e-4 * A   # by then the pulse is gone
+
+
+# ---------------------------------------------------------------- P22 no-slip wall (reading S17) and the uniform body force
+def wall_channel(N, axis):
+    """6 x N x 6 cells (N along `axis`) between no-slip walls at 0 and 1, flow along the next axis"""
+    h = 1.0 / N
+    n = [6, 6, 6]
+    n[axis] = N
+    bc = [P] * 6
+    bc[2 * axis] = bc[2 * axis + 1] = NS
+    shape = [1, 1, 1]
+    shape[2 - axis] = N
+    other = tuple(i for i in range(3) if i != 2 - axis)
+    return h, n, tuple(bc), (axis + 1) % 3, shape, other
+
+
+@pytest.mark.parametrize("axis", [1, 2])
+def test_P22_shear_mode_between_noslip_walls_decays_at_nu_k2(axis):
+    """u = U0 sin(pi y) exp(-nu pi^2 t) vanishes on both walls: exact.  The mirror ghosts of S17 put the wall on the
+    face to second order; a slip wall or a wall half a cell off would change the rate by O(1) / O(h)."""
+    nu, U0, T, k = 0.05, 0.01, 0.2, math.pi
+    err = []
+    for N in (12, 24):
+        h, n, bc, m, shape, other = wall_channel(N, axis)
+        yf = np.arange(N + 1) * h
+        savg = (np.cos(k * yf[:-1]) - np.cos(k * yf[1:])) / (k * h)
+        cfg = GridConfig(n=tuple(n), spacing=(h, h, h), RT=1.0, nu=nu, bc=bc)
+        W0 = const_state(n, (1.0, 0.0, 0.0, 0.0))
+        W0[1 + m] = U0 * savg.reshape(shape)
+        steps = math.ceil(T / min(0.3 * h, 0.15 * h * h / nu))
+        u = run(cfg, W0, T / steps, steps)[1 + m].mean(axis=other)
+        amp = (u * savg).sum() / (savg ** 2).sum() / U0
+        assert np.abs(u / U0 - amp * savg).max() < 1e-6            # it stays the mode it was
+        err.append(-math.log(amp) / T / (nu * k * k) - 1.0)
+    assert abs(err[1]) < 2e-3 and err[0] / err[1] > 3.5
+
+
+def test_P22_poiseuille_profile_is_steady_under_the_body_force():
+    """g y (1 - y) / (2 nu) between no-slip walls balances the uniform acceleration g exactly (Navier-Stokes); started
+    from its cell averages the step must keep it: the drift after half a viscous time is second order in h"""
+    nu, g = 0.05, 0.01
+    drift = []
+    for N in (12, 24):
+        h, n, bc, m, shape, other = wall_channel(N, 1)
+        yf = np.arange(N + 1) * h
+        uavg = np.diff(g / (2 * nu) * (yf ** 2 / 2 - yf ** 3 / 3)) / h
+        cfg = GridConfig(n=tuple(n), spacing=(h, h, h), RT=1.0, nu=nu, bc=bc)
+        W0 = const_state(n, (1.0, 0.0, 0.0, 0.0))
+        W0[1 + m] = uavg.reshape(shape)
+        acc = [0.0, 0.0, 0.0]
+        acc[m] = g
+        T = 0.5 / (nu * math.pi ** 2)
+        steps = math.ceil(T / min(0.3 * h, 0.15 * h * h / nu))
+        W = run(cfg, W0, T / steps, steps, setup=lambda o: o.set_body_force(*acc))
+        drift.append(np.abs(W[1 + m].mean(axis=other) - uavg).max() / uavg.max())
+        assert np.abs(W[0] - 1).max() < 1e-9
+    assert drift[1] < 2e-3 and drift[0] / drift[1] > 3.5
