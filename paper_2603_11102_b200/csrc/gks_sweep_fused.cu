@@ -54,6 +54,10 @@ __device__ __forceinline__ void fence_barrier_init() {
 __device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+/* raises the transaction count of the current phase without arriving */
+__device__ __forceinline__ void mbar_expect_tx_only(uint64_t *bar, uint32_t bytes) {
+  asm volatile("mbarrier.expect_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
   /* try_wait suspends the warp in hardware up to the time hint (ns) instead of spinning on issue slots */
   asm volatile(
@@ -120,7 +124,7 @@ struct Tile {
   static constexpr int OFF_XB = OFF_S + 3 * SBUF;          /* transpose buffer, 64 doubles per face, XOR-swizzled */
   static constexpr int OFF_RING = OFF_XB + NF * 64;        /* 4-plane ring of pass-1 results [4][6][NF][4] */
   static constexpr int RING = 4 * 6 * NF * 4;
-  static constexpr int OFF_BAR = OFF_RING + RING;          /* mbarriers: 2 TMA + 1 iteration barrier */
+  static constexpr int OFF_BAR = OFF_RING + RING;          /* mbarriers: [0] first slab, [2] iteration barrier */
   static constexpr size_t SMEM_BYTES = (size_t)(OFF_BAR + 4) * 8;
   static_assert(SMEM_BYTES + 1024 <= 233472, "the CTA must fit in shared memory");
   static_assert(NT <= 1024 && NT % 32 == 0 && (NT & (NT - 1)) == 0, "whole warps, power of two");
@@ -160,7 +164,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
   double *const Sb = sm + T::OFF_S;            /* [3][3][FH][4] */
   double *const XBuf = sm + T::OFF_XB;
   double *const ring = sm + T::OFF_RING;       /* [4][6][NF][4] */
-  uint64_t *const bar = reinterpret_cast<uint64_t *>(sm + T::OFF_BAR);   /* [0],[1] TMA slabs; [2] iteration */
+  uint64_t *const bar = reinterpret_cast<uint64_t *>(sm + T::OFF_BAR);   /* [0] slab of plane 0; [2] iteration hand-over + slabs */
 
   const int tid = threadIdx.x;
   const int n2 = g.n[T::AXM];
@@ -222,18 +226,18 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
 
   if (tid == 0) {
     mbar_init(&bar[0], 1);
-    mbar_init(&bar[1], 1);
     mbar_init(&bar[2], T::NW);
     fence_barrier_init();
   }
   __syncthreads();
 
   auto issue = [&](const Cur &c, int j) {       /* request staged plane j (described by cursor c) */
-    uint64_t *b = &bar[j & 1];
+    uint64_t *b = j == 0 ? &bar[0] : &bar[2];     /* see the hand-over at the top of the loop */
     double *dst = Wp + (j & 1) * T::WSLAB_PAD;
     const int pm = c.s.p0 + c.it + GKS_NG;      /* padded index space: cell -3 <-> 0 */
     const int ca0 = c.s.a0, cb0 = T::NA ? c.s.b0 + 1 : c.s.b0;
-    mbar_expect_tx(b, T::WSLAB * 8);
+    if (j == 0) mbar_expect_tx(b, T::WSLAB * 8);
+    else mbar_expect_tx_only(b, T::WSLAB * 8);
     if (DIR == 2) tma_load_4d(dst, &tmap, b, ca0, pm, cb0, 0);
     else tma_load_4d(dst, &tmap, b, ca0, cb0, pm, 0);
   };
@@ -265,7 +269,12 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
   constexpr int QLo = 0, QRo = FH * 4 + 2, DNo = 2 * FH * 4 + 4;   /* offsets inside a stage buffer */
 
   for (int i = 0; i < J + 2; ++i) {
-    if (i > 0) mbar_wait(&bar[2], (i - 1) & 1);   /* every warp has finished A, BC, D of iteration i-1 */
+    /* ONE hand-over per iteration: phase i-1 of the iteration barrier completes when every warp has finished
+       A, BC, D of iteration i-1 AND the slab of plane i has landed - its TMA was issued at the top of iteration
+       i-1, inside that phase, with its bytes expected on the same barrier (thread 0 arrives after it has issued,
+       so the phase cannot complete before the expectation is registered).  Plane 0 has a barrier of its own. */
+    if (i > 0) mbar_wait(&bar[2], (i - 1) & 1);
+    else mbar_wait(&bar[0], 0);
     if (i + 1 < J) {
       if (tid == 0) issue(cT, i + 1);             /* slab (i+1)&1 was last read by stage A of iteration i-1 */
       cur_next(cT);
@@ -277,7 +286,6 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
     if (i < J) {
       const double *W = Wp + (i & 1) * T::WSLAB_PAD;
       double *const S = Sb + (i % 3) * T::SBUF;
-      mbar_wait(&bar[i & 1], (i >> 1) & 1);
       constexpr int NITEM = T::NCA * T::NCB * 4;
       const int n0 = T::NA ? cA.s.a0 : cA.s.b0;   /* global index of normal face 0 of the tile */
       auto locate = [&](int item, const double *&w, int &cn, int &ct, int &cc) {
