@@ -15,8 +15,14 @@ from paper_2603_11102_b200.workloads import GridConfig
 P, NS, SL, IN, OUT, EX = range(6)
 
 
+def new_solver(cfg):
+    """the solver under test: the oracle here; tests/test_gpu_physics.py swaps in the CUDA library and runs the
+    same exact-solution checks on it"""
+    return ob.Oracle(cfg)
+
+
 def run(cfg, W0, dt, steps, setup=None):
-    o = ob.Oracle(cfg)
+    o = new_solver(cfg)
     if setup:
         setup(o)
     o.set_state(W0)
@@ -651,7 +657,7 @@ def couette_stress_errors(N, s, m, nu=0.05, a=0.02):
     shape = [1, 1, 1]
     shape[2 - s] = N
     W0[1 + m] = a * (0.5 * (sf[1:] + sf[:-1])).reshape(shape)      # the cell average of a linear profile
-    o = ob.Oracle(cfg)
+    o = new_solver(cfg)
     o.set_state(W0)
     Fs, _ = o.eval_flux(s)
     Fm, _ = o.eval_flux(m)
@@ -769,7 +775,7 @@ def test_P21_vortical_pulse_leaves_through_the_convective_outflow(axis, side):
 
     W0 = const_state(n, inflow)
     W0[1 + t_axis] = along(exact(0.0))
-    o = ob.Oracle(cfg)
+    o = new_solver(cfg)
     o.set_state(W0)
     t, dt = 0.0, 0.3 * h / (1.0 + U0)
     for T in (1.1, 4.0 / 3.0, 1.6, 2.8):
