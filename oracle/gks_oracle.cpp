@@ -399,7 +399,7 @@ namespace {
  * Ghost fill (readings S17-S21).  Pass x covers interior (j,k); pass y covers all i (ghosts
  * included) and interior k; pass z covers all (i,j): edges and corners end up defined.
  * ------------------------------------------------------------------------------------------ */
-void fill_ghost_line(const gkso_ctx &s, std::vector<double> &W, int a, int p[3], bool tang_interior) {
+void fill_ghost_line(const gkso_ctx &s, std::vector<double> &W, int a, int p[3]) {
   const int n = s.n[a];
   const double cs = std::sqrt(s.RT);
   for (int side = 0; side < 2; ++side) {
@@ -438,9 +438,8 @@ void fill_ghost_line(const gkso_ctx &s, std::vector<double> &W, int a, int p[3],
           for (int c = 1; c < 4; ++c) q[c] = rhob * s.inflow[c];
           break;
         }
-        case BC_OUTFLOW: /* S20: ghosts are state on tangentially interior lines; zero gradient elsewhere */
-          if (tang_interior) continue;
-          /* fall through */
+        case BC_OUTFLOW: /* S20: ghosts are state, on every line this pass covers */
+          continue;
         case BC_EXTRAP: /* S21 */
         default:
           pm[a] = first;
@@ -452,19 +451,25 @@ void fill_ghost_line(const gkso_ctx &s, std::vector<double> &W, int a, int p[3],
   }
 }
 
-void fill_ghosts(const gkso_ctx &s, std::vector<double> &W) {
+/* the lines pass a covers: x interior (j,k); y all i, interior k; z all (i,j).  f(p) is called with p[a] = 0 */
+template <class F>
+void for_lines_of_pass(const gkso_ctx &s, int a, F f) {
+  const int t1 = a == 0 ? 1 : 0, t2 = a == 2 ? 1 : 2;
+  /* a tangential axis is covered with its ghosts when its own pass ran before this one */
+  const int lo1 = t1 < a ? -NG : 0, hi1 = t1 < a ? s.n[t1] + NG : s.n[t1];
+  const int lo2 = t2 < a ? -NG : 0, hi2 = t2 < a ? s.n[t2] + NG : s.n[t2];
   int p[3];
-  /* x pass */
-  for (p[2] = 0; p[2] < s.n[2]; ++p[2])
-    for (p[1] = 0; p[1] < s.n[1]; ++p[1]) fill_ghost_line(s, W, 0, p, true);
-  /* y pass */
-  for (p[2] = 0; p[2] < s.n[2]; ++p[2])
-    for (p[0] = -NG; p[0] < s.n[0] + NG; ++p[0])
-      fill_ghost_line(s, W, 1, p, p[0] >= 0 && p[0] < s.n[0]);
-  /* z pass */
-  for (p[1] = -NG; p[1] < s.n[1] + NG; ++p[1])
-    for (p[0] = -NG; p[0] < s.n[0] + NG; ++p[0])
-      fill_ghost_line(s, W, 2, p, p[0] >= 0 && p[0] < s.n[0] && p[1] >= 0 && p[1] < s.n[1]);
+  p[a] = 0;
+  for (p[t2] = lo2; p[t2] < hi2; ++p[t2])
+    for (p[t1] = lo1; p[t1] < hi1; ++p[t1]) f(p);
+}
+
+void fill_pass(const gkso_ctx &s, std::vector<double> &W, int a) {
+  for_lines_of_pass(s, a, [&](int p[3]) { fill_ghost_line(s, W, a, p); });
+}
+
+void fill_ghosts(const gkso_ctx &s, std::vector<double> &W) {
+  for (int a = 0; a < 3; ++a) fill_pass(s, W, a);
 }
 
 /* ------------------------------------------------------------------------------------------
@@ -874,27 +879,42 @@ void eval_forcing(const gkso_ctx &s, const std::vector<double> &Wp, double dt, s
   }
 }
 
-/* S20: advance the convective-outflow ghost state after the step */
-void advance_outflow(gkso_ctx &s, std::vector<double> &W, double dt) {
-  for (int a = 0; a < 3; ++a)
-    for (int side = 0; side < 2; ++side) {
-      if (s.bc[2 * a + side] != BC_OUTFLOW) continue;
-      const int t1 = a == 0 ? 1 : 0, t2 = a == 2 ? 1 : 2;
-      const double Uc = std::fabs(s.inflow[1 + a]);
-      for (int i2 = 0; i2 < s.n[t2]; ++i2)
-        for (int i1 = 0; i1 < s.n[t1]; ++i1)
-          for (int c = 0; c < 4; ++c)
-            for (int g = 1; g <= NG; ++g) {
-              int pg[3], pm[3];
-              pg[t1] = pm[t1] = i1;
-              pg[t2] = pm[t2] = i2;
-              pg[a] = side == 0 ? -g : s.n[a] - 1 + g;
-              pm[a] = side == 0 ? -g + 1 : s.n[a] - 2 + g; /* g-1: one cell closer to the interior */
-              const double C = Uc * dt / std::fabs(s.ax[a].xc(pg[a]) - s.ax[a].xc(pm[a]));
-              double &phi = W[s.idp(c, pg)];
-              phi = phi - C * (phi - W[s.idp(c, pm)]);
-            }
-    }
+/* S20: the convective-outflow ghost state of axis a, on every line pass a covers (the ghosts of the tangential
+ * axes that pass a reads must be current: call after the passes of the lower axes).
+ * dt < 0: start from the last interior value; dt >= 0: phi_g -= C (phi_g - phi_{g-1}), g = 1,2,3 in order */
+void outflow_state_of_axis(const gkso_ctx &s, std::vector<double> &W, int a, double dt) {
+  for (int side = 0; side < 2; ++side) {
+    if (s.bc[2 * a + side] != BC_OUTFLOW) continue;
+    const double Uc = std::fabs(s.inflow[1 + a]);
+    for_lines_of_pass(s, a, [&](int p[3]) {
+      for (int c = 0; c < 4; ++c)
+        for (int g = 1; g <= NG; ++g) {
+          int pg[3] = {p[0], p[1], p[2]}, pm[3] = {p[0], p[1], p[2]};
+          pg[a] = side == 0 ? -g : s.n[a] - 1 + g;
+          if (dt < 0) {
+            pm[a] = side == 0 ? 0 : s.n[a] - 1;
+            W[s.idp(c, pg)] = W[s.idp(c, pm)];
+          } else {
+            pm[a] = side == 0 ? -g + 1 : s.n[a] - 2 + g; /* g-1: one cell closer to the interior */
+            const double C = Uc * dt / std::fabs(s.ax[a].xc(pg[a]) - s.ax[a].xc(pm[a]));
+            double &phi = W[s.idp(c, pg)];
+            phi = phi - C * (phi - W[s.idp(c, pm)]);
+          }
+        }
+    });
+  }
+}
+
+/* initialise (dt < 0) or advance the outflow ghost state of every axis; the passes of the lower axes run in
+ * between so that the lines through their ghosts see current values */
+void outflow_state(const gkso_ctx &s, std::vector<double> &W, double dt) {
+  bool any = false;
+  for (int f = 0; f < 6; ++f) any = any || s.bc[f] == BC_OUTFLOW;
+  if (!any) return;
+  for (int a = 0; a < 3; ++a) {
+    outflow_state_of_axis(s, W, a, dt);
+    fill_pass(s, W, a);
+  }
 }
 
 int validate(const gkso_config &c) {
@@ -955,22 +975,7 @@ int gkso_set_state(gkso_ctx *s, const double *Win) {
       for (int j = 0; j < s->n[1]; ++j)
         for (int i = 0; i < s->n[0]; ++i) s->W[s->id(c, i, j, k)] = Win[s->ii(c, i, j, k)];
   /* S20: convective-outflow ghosts start from the last interior value */
-  for (int a = 0; a < 3; ++a)
-    for (int side = 0; side < 2; ++side) {
-      if (s->bc[2 * a + side] != BC_OUTFLOW) continue;
-      const int t1 = a == 0 ? 1 : 0, t2 = a == 2 ? 1 : 2;
-      for (int i2 = 0; i2 < s->n[t2]; ++i2)
-        for (int i1 = 0; i1 < s->n[t1]; ++i1)
-          for (int c = 0; c < 4; ++c)
-            for (int g = 1; g <= NG; ++g) {
-              int pg[3], pm[3];
-              pg[t1] = pm[t1] = i1;
-              pg[t2] = pm[t2] = i2;
-              pg[a] = side == 0 ? -g : s->n[a] - 1 + g;
-              pm[a] = side == 0 ? 0 : s->n[a] - 1;
-              s->W[s->idp(c, pg)] = s->W[s->idp(c, pm)];
-            }
-    }
+  outflow_state(*s, s->W, -1.0);
   s->have_state = true;
   return 0;
 }
@@ -1031,7 +1036,7 @@ int gkso_step(gkso_ctx *s, double dt) {
       for (int j = 0; j < s->n[1]; ++j)
         for (int i = 0; i < s->n[0]; ++i) Wnew[s->id(1 + c, i, j, k)] += dM[s->ii(c, i, j, k)];
   /* 7: convective-outflow ghosts */
-  advance_outflow(*s, Wnew, dt);
+  outflow_state(*s, Wnew, dt);
   (void)N;
   s->W.swap(Wnew);
   return 0;

@@ -239,9 +239,9 @@ gks_status gks_create(const gks_config *cfg, void *workspace, size_t workspace_b
     g.halo[2 * a] = cfg->bc[2 * a] == GKS_BC_HALO;
     g.halo[2 * a + 1] = cfg->bc[2 * a + 1] == GKS_BC_HALO;
   }
-  /* On a periodic axis face n is face 0, cell for cell, unless another axis carries convective-outflow
-     ghosts: those are state on interior lines but zero-gradient on tangential-ghost lines (S20),
-     which breaks the identity.  Where it holds, the fused sweep stores n faces and readers wrap. */
+  /* On a periodic axis face n is face 0, cell for cell: the fused sweep stores n faces and readers wrap.
+     Conservatively switched off when another axis carries convective-outflow ghost state (S20):
+     the state on this axis' ghost lines is advanced on its own there, all n+1 faces are computed. */
   for (int a = 0; a < 3; ++a) {
     bool other_outflow = false;
     for (int b = 0; b < 3; ++b)

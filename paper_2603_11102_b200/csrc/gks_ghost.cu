@@ -5,6 +5,9 @@
  *
  * Pass order x, y, z; pass y also covers the i-ghosts, pass z covers i- and j-ghosts, so edges and
  * corners are defined.  One thread fills the 3 ghosts x 4 components of one line end.
+ * The convective-outflow ghosts of an axis are state on EVERY line its pass covers (also the lines through
+ * the ghosts of the lower axes): initialised and advanced per axis, with the passes of the lower axes run in
+ * between, so that a periodic / mirrored tangential ghost line carries the image of the ghost state.
  */
 #include "gks_internal.h"
 
@@ -26,7 +29,6 @@ __global__ void __launch_bounds__(128) k_ghost(GksGrid g, GksPhys ph, double *W,
   p[UA] = ulo + iu;
   p[VA] = vlo + iv;
   p[AX] = 0;
-  const bool tang_interior = p[UA] >= 0 && p[UA] < g.n[UA] && p[VA] >= 0 && p[VA] < g.n[VA];
   const long long base = g.idx(p[0], p[1], p[2]); /* cell 0 of the line */
   const long long sa = g.st[AX];
   const int n = g.n[AX];
@@ -60,9 +62,7 @@ __global__ void __launch_bounds__(128) k_ghost(GksGrid g, GksPhys ph, double *W,
         case BC_NOSLIP: q = c == 0 ? w[mirror * sa] : -w[mirror * sa]; break;
         case BC_SLIP: q = c == 1 + AX ? -w[mirror * sa] : w[mirror * sa]; break;
         case BC_INFLOW: q = qin[c]; break;
-        case BC_OUTFLOW:
-          q = tang_interior ? Wstate[c * g.FS + base + ghost * sa] : w[first * sa];
-          break;
+        case BC_OUTFLOW: q = Wstate[c * g.FS + base + ghost * sa]; break;
         default: q = w[first * sa]; break;
       }
       w[ghost * sa] = q;
@@ -72,17 +72,18 @@ __global__ void __launch_bounds__(128) k_ghost(GksGrid g, GksPhys ph, double *W,
 
 /* S20: initialise (dt < 0) or advance (dt >= 0) the convective-outflow ghost state of axis AX */
 template <int AX>
-__global__ void __launch_bounds__(128) k_outflow(GksGrid g, GksPhys ph, double *__restrict__ W, double dt) {
+__global__ void __launch_bounds__(128) k_outflow(GksGrid g, GksPhys ph, double *__restrict__ W, double dt, int ulo,
+                                                 int ucnt, int vlo, int vcnt) {
   constexpr int UA = AX == 0 ? 1 : 0, VA = AX == 2 ? 1 : 2;
   const int iu = blockIdx.x * blockDim.x + threadIdx.x;
   const int iv = blockIdx.y;
   const int side = blockIdx.z & 1;
   const int c = blockIdx.z >> 1;
-  if (iu >= g.n[UA] || iv >= g.n[VA]) return;
+  if (iu >= ucnt || iv >= vcnt) return;
   if (ph.bc[2 * AX + side] != BC_OUTFLOW) return;
   int p[3];
-  p[UA] = iu;
-  p[VA] = iv;
+  p[UA] = ulo + iu;
+  p[VA] = vlo + iv;
   p[AX] = 0;
   double *w = W + c * g.FS + g.idx(p[0], p[1], p[2]);
   const long long sa = g.st[AX];
@@ -158,23 +159,48 @@ __global__ void __launch_bounds__(256) k_check_finite(GksGrid g, const double *_
   if (bad) atomicOr(flag, 1);
 }
 
+/* lines of pass AX: x pass: interior (j,k); y pass: all i, interior k; z pass: all i, all j */
+template <int AX>
+struct PassLines {
+  static constexpr int UA = AX == 0 ? 1 : 0, VA = AX == 2 ? 1 : 2;
+  int ulo, ucnt, vlo, vcnt;
+  explicit PassLines(const GksGrid &g)
+      : ulo(AX == 0 ? 0 : -GKS_NG), ucnt(AX == 0 ? g.n[UA] : g.n[UA] + 2 * GKS_NG), vlo(AX == 2 ? -GKS_NG : 0),
+        vcnt(AX == 2 ? g.n[VA] + 2 * GKS_NG : g.n[VA]) {}
+};
+
 template <int AX>
 void launch_ghost_axis(const GksGrid &g, const GksPhys &ph, double *W, const double *Wstate, cudaStream_t s) {
-  constexpr int UA = AX == 0 ? 1 : 0, VA = AX == 2 ? 1 : 2;
-  /* x pass: interior (j,k); y pass: all i, interior k; z pass: all i, all j */
-  const int ulo = (AX == 0) ? 0 : -GKS_NG, ucnt = (AX == 0) ? g.n[UA] : g.n[UA] + 2 * GKS_NG;
-  const int vlo = (AX == 2) ? -GKS_NG : 0, vcnt = (AX == 2) ? g.n[VA] + 2 * GKS_NG : g.n[VA];
-  dim3 grid((ucnt + 127) / 128, vcnt, 2);
-  k_ghost<AX><<<grid, 128, 0, s>>>(g, ph, W, Wstate, ulo, ucnt, vlo, vcnt);
+  const PassLines<AX> L(g);
+  dim3 grid((L.ucnt + 127) / 128, L.vcnt, 2);
+  k_ghost<AX><<<grid, 128, 0, s>>>(g, ph, W, Wstate, L.ulo, L.ucnt, L.vlo, L.vcnt);
+}
+
+static bool outflow_on(const GksPhys &ph, int ax) {
+  return ph.bc[2 * ax] == BC_OUTFLOW || ph.bc[2 * ax + 1] == BC_OUTFLOW;
 }
 
 template <int AX>
 int launch_outflow_axis(const GksGrid &g, const GksPhys &ph, double *W, double dt, cudaStream_t s) {
-  if (ph.bc[2 * AX] != BC_OUTFLOW && ph.bc[2 * AX + 1] != BC_OUTFLOW) return 0;
-  constexpr int UA = AX == 0 ? 1 : 0, VA = AX == 2 ? 1 : 2;
-  dim3 grid((g.n[UA] + 127) / 128, g.n[VA], 8);
-  k_outflow<AX><<<grid, 128, 0, s>>>(g, ph, W, dt);
+  if (!outflow_on(ph, AX)) return 0;
+  const PassLines<AX> L(g);
+  dim3 grid((L.ucnt + 127) / 128, L.vcnt, 8);
+  k_outflow<AX><<<grid, 128, 0, s>>>(g, ph, W, dt, L.ulo, L.ucnt, L.vlo, L.vcnt);
   return 1;
+}
+
+/* initialise (dt < 0) or advance the outflow ghost state of every axis that has some.  The state of the y (z)
+ * axis also lives on the lines through the x (x and y) ghosts: those must be current first, so the passes of
+ * the lower axes run in between - only when there IS an outflow face on y or z (the paper's cases have theirs on x) */
+int outflow_state(const GksGrid &g, const GksPhys &ph, double *W, double dt, cudaStream_t s) {
+  int n = launch_outflow_axis<0>(g, ph, W, dt, s);
+  if (!outflow_on(ph, 1) && !outflow_on(ph, 2)) return n;
+  launch_ghost_axis<0>(g, ph, W, W, s);
+  n += 1 + launch_outflow_axis<1>(g, ph, W, dt, s);
+  if (!outflow_on(ph, 2)) return n;
+  launch_ghost_axis<1>(g, ph, W, W, s);
+  n += 1 + launch_outflow_axis<2>(g, ph, W, dt, s);
+  return n;
 }
 
 } /* namespace */
@@ -187,13 +213,11 @@ int gks_launch_ghost_fill(const GksGrid &g, const GksPhys &ph, double *W, const 
 }
 
 int gks_launch_outflow_init(const GksGrid &g, const GksPhys &ph, double *W, cudaStream_t s) {
-  return launch_outflow_axis<0>(g, ph, W, -1.0, s) + launch_outflow_axis<1>(g, ph, W, -1.0, s) +
-         launch_outflow_axis<2>(g, ph, W, -1.0, s);
+  return outflow_state(g, ph, W, -1.0, s);
 }
 
 int gks_launch_outflow_advance(const GksGrid &g, const GksPhys &ph, double *W, double dt, cudaStream_t s) {
-  return launch_outflow_axis<0>(g, ph, W, dt, s) + launch_outflow_axis<1>(g, ph, W, dt, s) +
-         launch_outflow_axis<2>(g, ph, W, dt, s);
+  return outflow_state(g, ph, W, dt, s);
 }
 
 static dim3 grid2d(int nx, int ny, int nz) { return dim3((nx + 63) / 64, (ny + 3) / 4, nz); }

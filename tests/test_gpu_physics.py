@@ -68,10 +68,8 @@ def test_piston_problem(axis, side):
     tos.test_P20_impulsive_inflow_drives_the_rankine_hugoniot_shock(axis, side)
 
 
-@pytest.mark.parametrize("axis,side", [(0, 1), (0, 0), (1, 0)])
+@pytest.mark.parametrize("axis,side", [(0, 1), (0, 0), (1, 0), (1, 1), (2, 0), (2, 1)])
 def test_pulse_through_the_convective_outflow(axis, side):
-    """(an outflow face on the z axis shows the corner-ghost artefact DESIGN.md lists under S20; the paper's cases
-    put the outflow on x)"""
     tos.test_P21_vortical_pulse_leaves_through_the_convective_outflow(axis, side)
 
 

@@ -745,7 +745,7 @@ def test_P20_impulsive_inflow_drives_the_rankine_hugoniot_shock(axis, side):
 
 
 # ---------------------------------------------------------------- P21 convective outflow (reading S20)
-@pytest.mark.parametrize("axis,side", [(0, 1), (1, 0)])
+@pytest.mark.parametrize("axis,side", [(0, 1), (1, 0), (2, 1)])
 def test_P21_vortical_pulse_leaves_through_the_convective_outflow(axis, side):
     """rho = 1, normal velocity U0, a transverse velocity A exp(-(x - x0 - U0 t)^2 / 2 sigma^2): an exact solution of
     the isothermal Euler equations (rho and the normal velocity stay uniform, the transverse momentum is advected).
