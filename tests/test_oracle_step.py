@@ -389,6 +389,48 @@ def test_P14_axis_permutation_commutes_up_to_the_pass_order():
     assert diff < 1e-6                       # only S9 (order of the tangential WENO passes) differs: O(h^5)
 
 
+@pytest.mark.parametrize("lo,hi", [(NS, NS), (SL, SL), (IN, OUT), (OUT, IN), (EX, EX), (IN, EX), (NS, SL)])
+@pytest.mark.parametrize("stretched", [False, True])
+def test_P14_every_boundary_kind_treats_the_three_axes_alike(lo, hi, stretched):
+    """data that vary along ONE axis only, between any pair of boundary kinds, on a uniform or a stretched axis: the
+    same numbers whichever axis it is (to round-off: only the order of the tangential passes differs, and they act
+    on constants), and exactly uniform along the two periodic axes afterwards.  This is what caught the
+    zero-gradient corner ghosts of the first form of S20."""
+    N = 14
+    x = (np.arange(N) + 0.5) / N
+    rho, un, ut = 1 + 0.02 * np.sin(2 * np.pi * x + 0.3), 0.1 + 0.01 * np.cos(2 * np.pi * x), 0.02 * np.sin(4 * np.pi * x)
+    sf = np.cumsum(np.r_[0.0, np.linspace(0.8, 1.3, N)]) * 0.1
+    lines = []
+    for a in range(3):
+        n = [6, 6, 6]
+        n[a] = N
+        bc = [P] * 6
+        bc[2 * a], bc[2 * a + 1] = lo, hi
+        inflow = [1.0, 0.0, 0.0, 0.0]
+        inflow[1 + a] = 0.1
+        faces = [None] * 3
+        if stretched:
+            faces[a] = sf
+        cfg = GridConfig(n=tuple(n), faces=tuple(faces), spacing=(0.1, 0.1, 0.1), nu=2e-3, bc=tuple(bc),
+                         inflow=tuple(inflow))
+        shape = [1, 1, 1]
+        shape[2 - a] = N
+        t = (a + 1) % 3
+        W0 = np.zeros((4, n[2], n[1], n[0]))
+        W0[0] = rho.reshape(shape)
+        W0[1 + a] = (rho * un).reshape(shape)
+        W0[1 + t] = (rho * ut).reshape(shape)
+        W = run(cfg, W0, 0.02, 4)
+        other = tuple(i for i in range(3) if i != 2 - a)
+        assert max(np.ptp(W[c], axis=other).max() for c in range(4)) == 0.0
+        pick = [0, 0, 0]
+        pick[2 - a] = slice(None)
+        pick = tuple(pick)
+        lines.append(np.stack([W[0][pick], W[1 + a][pick], W[1 + t][pick], W[1 + (a + 2) % 3][pick]]))
+        assert np.abs(lines[-1] - np.stack([rho, rho * un, rho * ut, 0 * rho])).max() > 1e-6      # it moved
+    assert np.abs(lines[0] - lines[1]).max() < 1e-15 and np.abs(lines[0] - lines[2]).max() < 1e-15
+
+
 # ---------------------------------------------------------------- P16 CFL time step (PAPER.md:91)
 def test_P16_cfl_dt_closed_forms_and_invariants():
     """dt = CFL min(dx,dy,dz)/(|U|max + sqrt(RT)): numbers worked by hand on a uniform state, the global minimum
