@@ -34,7 +34,8 @@
  * the Couette stress -mu a through every face family and the decay rate of a wall-bounded vortex, both second
  * order under refinement (P19), inflow density (S19): the Rankine-Hugoniot plateau, velocity and injected mass of
  * the piston problem (P20), convective outflow (S20): an exactly advected vortical pulse leaves without reflection
- * (P21), no-slip wall (S17) and body force: decaying shear mode and steady Poiseuille profile between walls (P22).
+ * (P21), no-slip wall (S17) and body force: decaying shear mode and steady Poiseuille profile between walls (P22),
+ * mirror symmetry of the whole step with every boundary kind, ALM and IBM (P23).
  * The paper prints no numbers for S10, S17, S19, S20; the pins are exact solutions of the equations it solves.
  */
 #include "gks_oracle.h"

@@ -1,4 +1,4 @@
-"""Pins of the oracle's whole step against invariants, exact solutions and closed forms (P6-P12, P14-P22).
+"""Pins of the oracle's whole step against invariants, exact solutions and closed forms (P6-P12, P14-P23).
 
 CPU only.  Sizes are chosen so that the file runs in about two minutes.
 """
@@ -888,3 +888,54 @@ def test_P22_poiseuille_profile_is_steady_under_the_body_force():
         drift.append(np.abs(W[1 + m].mean(axis=other) - uavg).max() / uavg.max())
         assert np.abs(W[0] - 1).max() < 1e-9
     assert drift[1] < 2e-3 and drift[0] / drift[1] > 3.5
+
+
+# ---------------------------------------------------------------- P23 mirror symmetry (low side / high side of every boundary kind)
+@pytest.mark.parametrize("bc", [(IN, OUT, P, P, SL, NS), (NS, SL, IN, OUT, P, P), (P, P, EX, NS, OUT, IN),
+                                (EX, IN, SL, SL, NS, EX)])
+@pytest.mark.parametrize("with_ibm", [False, True])
+def test_P23_the_mirrored_problem_gives_the_mirrored_result(bc, with_ibm):
+    """reflect the grid, the state, the boundary kinds, the inflow velocity and the actuator / immersed points about
+    the mid-plane of an axis: the step must return the reflection (WENO, the collision and both forcing kernels are
+    mirror-symmetric; round-off only).  Catches anything that treats the low and the high side of an axis
+    differently.  Without IBM points the y axis is stretched."""
+    n, sp = (10, 9, 8), (0.1, 0.1, 0.12)
+    z, y, x = np.meshgrid(*[(np.arange(m) + 0.5) / m for m in (n[2], n[1], n[0])], indexing="ij")
+    W0 = np.zeros((4,) + x.shape)
+    W0[0] = 1 + 0.02 * np.sin(2 * np.pi * x + 1) * np.cos(2 * np.pi * y) + 0.01 * np.sin(2 * np.pi * z + 0.5)
+    W0[1] = W0[0] * (0.1 + 0.02 * np.cos(2 * np.pi * y + 0.3) * np.sin(2 * np.pi * z))
+    W0[2] = W0[0] * (0.03 * np.sin(2 * np.pi * x + 0.2) + 0.01 * np.cos(2 * np.pi * z))
+    W0[3] = W0[0] * (0.02 * np.cos(2 * np.pi * x) * np.sin(2 * np.pi * y + 0.7))
+    inflow = [1.0, 0.0, 0.0, 0.0]
+    for ax in range(3):
+        if IN in bc[2 * ax:2 * ax + 2]:
+            inflow[1 + ax] = 0.1 if bc[2 * ax] == IN else -0.1
+    yf = np.arange(n[1] + 1) * sp[1] if with_ibm else np.cumsum(np.r_[0.0, np.linspace(0.7, 1.4, n[1])]) * 0.1
+    length = [n[0] * sp[0], yf[-1], n[2] * sp[2]]
+    alm_pos = np.array([[0.42, 0.40, 0.5], [0.61, 0.33, 0.41]])
+    alm_force = np.array([[0.01, 0.02, -0.01], [-0.02, 0.0, 0.01]])
+    ibm_pos = np.array([[0.5, 0.45, 0.48], [0.52, 0.47, 0.5], [0.3, 0.6, 0.36]])
+    ibm_vol = np.full(3, 0.5 * sp[0] * sp[1] * sp[2])
+
+    def solve(faces_y, bcs, infl, state, apos, aforce, ipos):
+        def setup(o):
+            o.alm_set_points(apos, aforce, 0.12)
+            if with_ibm:
+                o.ibm_set_points(ipos, ibm_vol)
+        cfg = GridConfig(n=n, faces=(None, faces_y, None), spacing=sp, nu=2e-3, bc=tuple(bcs), inflow=tuple(infl))
+        return run(cfg, state, 0.01, 3, setup=setup)
+
+    Wa = solve(yf, bc, inflow, W0, alm_pos, alm_force, ibm_pos)
+    assert np.abs(Wa - W0).max() > 1e-4
+    for a in range(3):
+        sign = np.ones(4)
+        sign[1 + a] = -1.0
+        flip = lambda W: np.ascontiguousarray(np.flip(W, axis=3 - a) * sign[:, None, None, None])
+        bcm = list(bc)
+        bcm[2 * a], bcm[2 * a + 1] = bc[2 * a + 1], bc[2 * a]
+        inflm = list(inflow)
+        inflm[1 + a] = -inflow[1 + a]
+        mirror = lambda pts: np.where(np.arange(3) == a, length[a] - pts, pts)
+        Wb = flip(solve((yf[-1] - yf)[::-1] if a == 1 else yf, bcm, inflm, flip(W0), mirror(alm_pos),
+                        alm_force * sign[1:], mirror(ibm_pos)))
+        assert np.abs(Wa - Wb).max() < 5e-15, a
