@@ -42,6 +42,11 @@
 
 namespace {
 
+#ifndef GKS_FUSE_BCD
+#define GKS_FUSE_BCD 1   /* 0: stages separate; 1: BC + D one straight-line block; 2: that for y- and z-faces only;
+                            3: A + BC + D one block */
+#endif
+
 /* ---------------- PTX helpers: mbarrier + TMA ---------------- */
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -159,6 +164,8 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
                   int ncol_a, int nfull, long long rem, long long PPC) {
   using T = Tile<DIR, TA, TB>;
   constexpr int TN = T::TN, NF = T::NF, NT = T::NT, EA = T::EA, EB = T::EB, HA = T::HA, FH = T::FH;
+  constexpr bool FUSE_BCD = GKS_FUSE_BCD == 1 || GKS_FUSE_BCD == 3 || (GKS_FUSE_BCD == 2 && DIR != 0);
+  constexpr bool FUSE_A = GKS_FUSE_BCD == 3;
   extern __shared__ __align__(128) double sm[];
   double *const Wp = sm + T::OFF_W;
   double *const Sb = sm + T::OFF_S;            /* [3][3][FH][4] */
@@ -282,37 +289,61 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
 
     /* ================= stage A: plane i =================
      * both WENO5 edge values of each cell, per component (one smoothness-indicator set serves the face on
-     * either side), and the normal slope at the cell's right face; two cells at a time where a thread owns two */
-    if (i < J) {
-      const double *W = Wp + (i & 1) * T::WSLAB_PAD;
-      double *const S = Sb + (i % 3) * T::SBUF;
-      constexpr int NITEM = T::NCA * T::NCB * 4;
-      const int n0 = T::NA ? cA.s.a0 : cA.s.b0;   /* global index of normal face 0 of the tile */
-      auto locate = [&](int item, const double *&w, int &cn, int &ct, int &cc) {
-        cc = item & 3;
-        const int cell = item >> 2;
-        const int xa = cell % T::NCA, xb = cell / T::NCA;
-        const int sa = T::NA ? xa + 2 : xa + 1, sb = T::NA ? xb : xb + 2;
-        w = W + (cc * EB + sb) * EA + sa;
-        cn = T::NA ? xa : xb; /* cell along the normal: global f0-1+cn */
-        ct = T::NA ? xb : xa; /* halo index along t1 */
-      };
-      auto store = [&](int cn, int ct, int cc, double vl, double vr, double dn) {
-        if (cn >= 1) { /* left edge = face cn-1: Qr */
-          const int fh = T::NA ? ct * HA + (cn - 1) : (cn - 1) * HA + ct;
-          S[QRo + fh * 4 + cc] = vl;
-        }
-        if (cn < TN) { /* right edge = face cn: Ql, and the slope at that face */
-          const int fh = T::NA ? ct * HA + cn : cn * HA + ct;
-          S[QLo + fh * 4 + cc] = vr;
-          S[DNo + fh * 4 + cc] = dn * g.inv_hn[DIR][min(n0 + cn, g.n[DIR]) + GKS_NG];
-        }
-      };
-      /* every thread owns item tid; the NITEM - NT extra items go to a window of warps that rotates with
-         the iteration, so that no warp is systematically the slowest */
-      constexpr int NXA = NITEM - NT;
-      static_assert(NXA >= 0 && NXA <= NT / 2, "stage A: at most two items per thread, extras on half the CTA");
-      const int xa_id = (tid - 32 * ((i * 5) % T::NW)) & (NT - 1);
+     * either side), and the normal slope at the cell's right face.  Every thread owns item tid; the NITEM - NT
+     * extra items go to a window of warps that rotates with the iteration, so that no warp is systematically
+     * the slowest.  Without FUSE_A a thread with two items evaluates them together, statement-interleaved; with
+     * FUSE_A the thread's own item is computed here unconditionally (stale slab in the draining iterations,
+     * result dropped) as the head of the straight-line block that continues through BC and D below, and the
+     * stores and the extra item follow that block. */
+    const bool okA = i < J;
+    const double *const W = Wp + (i & 1) * T::WSLAB_PAD;
+    double *const SA = Sb + (i % 3) * T::SBUF;
+    constexpr int NITEM = T::NCA * T::NCB * 4;
+    const int n0 = T::NA ? cA.s.a0 : cA.s.b0;     /* global index of normal face 0 of the tile */
+    auto locate = [&](int item, const double *&w, int &cn, int &ct, int &cc) {
+      cc = item & 3;
+      const int cell = item >> 2;
+      const int xa = cell % T::NCA, xb = cell / T::NCA;
+      const int sa = T::NA ? xa + 2 : xa + 1, sb = T::NA ? xb : xb + 2;
+      w = W + (cc * EB + sb) * EA + sa;
+      cn = T::NA ? xa : xb; /* cell along the normal: global f0-1+cn */
+      ct = T::NA ? xb : xa; /* halo index along t1 */
+    };
+    auto store = [&](int cn, int ct, int cc, double vl, double vr, double dn) {
+      if (cn >= 1) { /* left edge = face cn-1: Qr */
+        const int fh = T::NA ? ct * HA + (cn - 1) : (cn - 1) * HA + ct;
+        SA[QRo + fh * 4 + cc] = vl;
+      }
+      if (cn < TN) { /* right edge = face cn: Ql, and the slope at that face */
+        const int fh = T::NA ? ct * HA + cn : cn * HA + ct;
+        SA[QLo + fh * 4 + cc] = vr;
+        SA[DNo + fh * 4 + cc] = dn * g.inv_hn[DIR][min(n0 + cn, g.n[DIR]) + GKS_NG];
+      }
+    };
+    auto edges_of_one = [&](int item) {
+      double q[5][1], vl[1], vr[1];
+      int cn, ct, cc;
+      const double *w;
+      locate(item, w, cn, ct, cc);
+#pragma unroll
+      for (int k = 0; k < 5; ++k) q[k][0] = w[(k - 2) * sn];
+      gksd::weno5_edges_v<1>(q, eps, vl, vr);
+      store(cn, ct, cc, vl[0], vr[0], gksd::normal_slope(q[1][0], q[2][0], q[3][0], q[4][0]));
+    };
+    constexpr int NXA = NITEM - NT;
+    static_assert(NXA >= 0 && NXA <= NT / 2, "stage A: at most two items per thread, extras on half the CTA");
+    const int xa_id = (tid - 32 * ((i * 5) % T::NW)) & (NT - 1);
+    double a_vl[1], a_vr[1], a_dn = 0.0;
+    int a_cn = 0, a_ct = 0, a_cc = 0;
+    if (FUSE_A) {
+      double q[5][1];
+      const double *w;
+      locate(tid, w, a_cn, a_ct, a_cc);
+#pragma unroll
+      for (int k = 0; k < 5; ++k) q[k][0] = w[(k - 2) * sn];
+      gksd::weno5_edges_v<1>(q, eps, a_vl, a_vr);
+      a_dn = gksd::normal_slope(q[1][0], q[2][0], q[3][0], q[4][0]);
+    } else if (okA) {
       if (xa_id < NXA) {
         double q[5][2], vl[2], vr[2];
         int cnv[2], ctv[2], ccv[2];
@@ -328,31 +359,32 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
         for (int u = 0; u < 2; ++u)
           store(cnv[u], ctv[u], ccv[u], vl[u], vr[u], gksd::normal_slope(q[1][u], q[2][u], q[3][u], q[4][u]));
       } else {
-        double q[5][1], vl[1], vr[1];
-        int cn, ct, cc;
-        const double *w;
-        locate(tid, w, cn, ct, cc);
-#pragma unroll
-        for (int k = 0; k < 5; ++k) q[k][0] = w[(k - 2) * sn];
-        gksd::weno5_edges_v<1>(q, eps, vl, vr);
-        store(cn, ct, cc, vl[0], vr[0], gksd::normal_slope(q[1][0], q[2][0], q[3][0], q[4][0]));
+        edges_of_one(tid);
       }
       cur_next(cA);
     }
 
-    /* ================= stage BC: plane i-1 =================
-     * collision (S4): the 4 lanes of a halo face split the four half-Maxwellian factors (left / right side,
-     * erf / exp series), exchange them by shuffle, and every lane forms its component of Q0 in place of QL */
-    if (i >= 1 && i - 1 < J) {
-      double *const S = Sb + ((i - 1) % 3) * T::SBUF;
+    /* ================= stages BC (plane i-1) and D (plane i-2) =================
+     * BC, collision (S4): the 4 lanes of a halo face split the four half-Maxwellian factors (left / right side,
+     * erf / exp series), exchange them by shuffle, and every lane forms its component of Q0 in place of QL.
+     * D, tangential pass 1 (along t1) on Q0 and Dn of the plane before.
+     * The two touch different stage buffers.  With FUSE_BCD every thread's own BC item and its D item form ONE
+     * straight-line block - loads, the short series unconditionally, two WENO5 Gauss-point evaluations, shuffles -
+     * so that BC's serial chain (reciprocal, Horner, shuffles) issues in the shadow of D's dense arithmetic; in
+     * the priming / draining iterations a stage works on stale shared memory and its result is dropped; a warp
+     * that needs the long series (rare: |z| > 1/8) redoes its item afterwards. */
+    const bool okB = i >= 1 && i - 1 < J;
+    const bool have = i >= 2;
+    double d6[6];
+    int ga = 0, gb = 0;
+    {
+      double *const S = Sb + ((i + 2) % 3) * T::SBUF;               /* plane i-1 */
       static_assert((FH * 4) % 32 == 0, "whole warps in the collision stage");
       const int gl = (tid & 31) & ~3;               /* first lane of this face group */
       constexpr int NXB = FH * 4 - NT;              /* extra items: a rotating window of whole warps, disjoint from A's */
       static_assert(NXB >= 0 && NXB <= NT / 4 && NXB % 32 == 0, "stage BC: extras on whole warps");
       const int xb_id = (tid - 32 * ((i * 5 + T::NW / 2) % T::NW)) & (NT - 1);
-      const int nitem = xb_id < NXB ? 2 : 1;
-      for (int u = 0; u < nitem; ++u) {
-        const int item = u ? NT + xb_id : tid;
+      auto collide = [&](int item) {
         const int cc = item & 3, fh = item >> 2, side = cc & 1, func = cc >> 1;
         const double *qs = S + (side ? QRo : QLo) + fh * 4;
         const double rho = qs[0];
@@ -365,33 +397,60 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
         double q0 = S[QLo + item] * el + S[QRo + item] * er;
         if (cc == 1 + DIR) q0 += xl - xr;
         S[QLo + item] = q0;
-      }
-    }
-
-    /* ================= stage D: plane i-2, tangential pass 1 (along t1) on Q0 and Dn ================= */
-    const bool have = i >= 2;
-    double d6[6];
-    int ga = 0, gb = 0;
-    if (have) {
-      ga = cD.s.a0 + fa;
-      gb = cD.s.b0 + fb;
-      const int t1_glob = T::NA ? gb : ga;
-      const double iw1 = g.inv_w[T::AXT1][min(t1_glob, g.n[T::AXT1] - 1) + GKS_NG];
-      const double *q = Sb + ((i - 2) % 3) * T::SBUF + QLo + fh0 * 4 + c; /* Q0 */
-      const double *d = q + DNo;                                          /* Dn */
-      double qq[5][2], vm[2], vp[2], sm_[2], sp_[2];
+      };
+      auto pass1 = [&]() {
+        ga = cD.s.a0 + fa;
+        gb = cD.s.b0 + fb;
+        const int t1_glob = T::NA ? gb : ga;
+        const double iw1 = g.inv_w[T::AXT1][min(t1_glob, g.n[T::AXT1] - 1) + GKS_NG];
+        const double *q = Sb + ((i + 1) % 3) * T::SBUF + QLo + fh0 * 4 + c; /* Q0 of plane i-2 */
+        const double *d = q + DNo;                                          /* Dn */
+        double qq[5][2], vm[2], vp[2], sm_[2], sp_[2];
 #pragma unroll
-      for (int k = 0; k < 5; ++k) {
-        qq[k][0] = q[(k - 2) * s1 * 4];
-        qq[k][1] = d[(k - 2) * s1 * 4];
+        for (int k = 0; k < 5; ++k) {
+          qq[k][0] = q[(k - 2) * s1 * 4];
+          qq[k][1] = d[(k - 2) * s1 * 4];
+        }
+        gksd::weno5_gauss_v<2, LIN>(qq, eps, vm, vp, sm_, sp_);
+        d6[0] = vm[0];
+        d6[1] = vp[0];
+        d6[2] = vm[1];
+        d6[3] = vp[1];
+        d6[4] = sm_[0] * iw1;
+        d6[5] = sp_[0] * iw1;
+      };
+      if (FUSE_BCD) {
+        const int side = c & 1, func = c >> 1;
+        const double *qs = S + (side ? QRo : QLo) + (tid & ~3);
+        const double rho = qs[0], mn = qs[1 + DIR];
+        const double ql = S[QLo + tid], qr = S[QRo + tid];
+        const double z = ph.theta * (mn * gksd::fast_rcp3(rho));
+        const double w = z * z;
+        const bool all_small = __all_sync(0xffffffffu, !(w > 1.0 / 64.0));
+        double p = bcf[7];
+#pragma unroll
+        for (int n = 6; n >= 0; --n) p = fma(p, w, bcf[n]);
+        const double v = func ? p : p * z;
+        const double r = func ? rho * (ph.cx * v) : fma(side ? -0.5 : 0.5, v, 0.5);
+        const double el = __shfl_sync(0xffffffffu, r, gl), er = __shfl_sync(0xffffffffu, r, gl + 1);
+        const double xl = __shfl_sync(0xffffffffu, r, gl + 2), xr = __shfl_sync(0xffffffffu, r, gl + 3);
+        double q0 = ql * el + qr * er;
+        if (c == 1 + DIR) q0 += xl - xr;
+        pass1();
+        if (okB) {
+          if (all_small) S[QLo + tid] = q0;
+          else collide(tid);
+        }
+      } else {
+        if (okB) collide(tid);
+        if (have) pass1();
       }
-      gksd::weno5_gauss_v<2, LIN>(qq, eps, vm, vp, sm_, sp_);
-      d6[0] = vm[0];
-      d6[1] = vp[0];
-      d6[2] = vm[1];
-      d6[3] = vp[1];
-      d6[4] = sm_[0] * iw1;
-      d6[5] = sp_[0] * iw1;
+      if (okB && xb_id < NXB) collide(NT + xb_id);
+    }
+    if (FUSE_A && okA) {
+      store(a_cn, a_ct, a_cc, a_vl[0], a_vr[0], a_dn);
+      if (xa_id < NXA) edges_of_one(NT + xa_id);
+      cur_next(cA);
     }
     /* this warp is done with the shared stage buffers of iteration i */
     __syncwarp();
