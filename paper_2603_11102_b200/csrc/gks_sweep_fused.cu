@@ -166,6 +166,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
   constexpr int TN = T::TN, NF = T::NF, NT = T::NT, EA = T::EA, EB = T::EB, HA = T::HA, FH = T::FH;
   constexpr bool FUSE_BCD = GKS_FUSE_BCD == 1 || GKS_FUSE_BCD == 3 || (GKS_FUSE_BCD == 2 && DIR != 0);
   constexpr bool FUSE_A = GKS_FUSE_BCD == 3;
+  constexpr bool D_FIRST = DIR == 0;   /* source order of D and BC inside the fused block: measured, x-faces 0.7 % */
   extern __shared__ __align__(128) double sm[];
   double *const Wp = sm + T::OFF_W;
   double *const Sb = sm + T::OFF_S;            /* [3][3][FH][4] */
@@ -420,6 +421,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
         d6[5] = sp_[0] * iw1;
       };
       if (FUSE_BCD) {
+        if (D_FIRST) pass1();
         const int side = c & 1, func = c >> 1;
         const double *qs = S + (side ? QRo : QLo) + (tid & ~3);
         const double rho = qs[0], mn = qs[1 + DIR];
@@ -436,7 +438,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
         const double xl = __shfl_sync(0xffffffffu, r, gl + 2), xr = __shfl_sync(0xffffffffu, r, gl + 3);
         double q0 = ql * el + qr * er;
         if (c == 1 + DIR) q0 += xl - xr;
-        pass1();
+        if (!D_FIRST) pass1();
         if (okB) {
           if (all_small) S[QLo + tid] = q0;
           else collide(tid);
