@@ -569,7 +569,7 @@ bool encode_dir(encode_fn_t enc, const GksGrid &g, double *base, CUtensorMap *ou
   const cuuint32_t es[4] = {1, 1, 1, 1};
   return enc(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NAN_REQUEST_ZERO_FMA) == CUDA_SUCCESS;
 }
 
 template <int DIR, bool NEED_F, bool LIN>
