@@ -240,15 +240,9 @@ gks_status gks_create(const gks_config *cfg, void *workspace, size_t workspace_b
     g.halo[2 * a + 1] = cfg->bc[2 * a + 1] == GKS_BC_HALO;
   }
   /* On a periodic axis face n is face 0, cell for cell: the fused sweep stores n faces and readers wrap.
-     Conservatively switched off when another axis carries convective-outflow ghost state (S20):
-     the state on this axis' ghost lines is advanced on its own there, all n+1 faces are computed. */
-  for (int a = 0; a < 3; ++a) {
-    bool other_outflow = false;
-    for (int b = 0; b < 3; ++b)
-      if (b != a && (cfg->bc[2 * b] == GKS_BC_OUTFLOW_CONVECTIVE || cfg->bc[2 * b + 1] == GKS_BC_OUTFLOW_CONVECTIVE))
-        other_outflow = true;
-    g.wrapf[a] = g.periodic[a] && !other_outflow;
-  }
+     (Holds next to a convective-outflow face of another axis too, since the ghost state of that axis is carried on
+     this axis' ghost lines as the image of the interior lines' state, S20.) */
+  for (int a = 0; a < 3; ++a) g.wrapf[a] = g.periodic[a];
   g.st[0] = 1;
   g.st[1] = g.P[0];
   g.st[2] = (long long)g.P[0] * g.P[1];
