@@ -22,8 +22,10 @@
  * Thread mapping: 4 threads per face.  In A-E thread (face, c) owns component c (WENO is component-wise);
  * in F thread (face, g) owns Gauss point g (the flux couples all components); the 4x4 transpose goes
  * through a swizzled warp-private buffer and needs only __syncwarp.
- * The W slab of the next plane is fetched by TMA (cp.async.bulk.tensor, mbarrier completion) one iteration
- * ahead: 2 slab buffers, one elected thread issues.
+ * The W slab of the next plane is fetched by TMA (cp.async.bulk.tensor) one iteration ahead: 2 slab buffers,
+ * one elected thread issues, the bytes are expected on the iteration barrier itself (one wait per iteration);
+ * cells beyond the padded array (overhanging tiles) are filled with NaN, which takes the short path
+ * everywhere and is never stored.
  *
  * Roofline: fp64-ALU bound (about 4.7 kflop per face against 32 B read + 64 B written per face).
  */
@@ -156,7 +158,8 @@ struct Seg {
  * A, BC and D touch three different buffers, so an iteration needs ONE CTA-wide hand-over, and that one
  * is split: a warp arrives on the iteration mbarrier after A, BC, D and waits for it only at the top of
  * the next iteration, after its EF (about half of the iteration's arithmetic) - warps may drift by half
- * an iteration without anyone waiting.
+ * an iteration without anyone waiting.  A thread's own BC item and its D item are written as one
+ * straight-line block (GKS_FUSE_BCD): BC's serial chain issues in the shadow of D's arithmetic.
  */
 template <int DIR, bool NEED_F, bool LIN, int TA, int TB>
 __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
