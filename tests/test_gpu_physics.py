@@ -31,6 +31,8 @@ class CudaSolver:
 @pytest.fixture(autouse=True)
 def cuda_solver(monkeypatch):
     monkeypatch.setattr(tos, "new_solver", CudaSolver)
+    monkeypatch.setattr(tos, "TOL_SYMMETRY", 1e-13)
+    monkeypatch.setattr(tos, "TOL_UNIFORM", 1e-13)
 
 
 def test_order_of_accuracy_on_the_exact_simple_wave_up_to_64_cubed():
@@ -100,3 +102,18 @@ def test_taylor_green_kinetic_energy_decays_at_2_nu_k2_on_the_metric_box_shape()
     amp = (W[1] * mode).sum() / (mode ** 2).sum() / N / U0
     assert -math.log(amp) / T == pytest.approx(2 * nu * k * k, rel=2e-3)   # O(Ma^2) = 4e-4 compressibility
     assert np.abs(W[3]).max() < 1e-12
+
+
+@pytest.mark.parametrize("lo,hi", [(tos.NS, tos.SL), (tos.IN, tos.OUT), (tos.OUT, tos.IN), (tos.EX, tos.EX)])
+@pytest.mark.parametrize("stretched", [False, True])
+def test_every_boundary_kind_treats_the_three_axes_alike(lo, hi, stretched):
+    """P14 on the CUDA path: three different sweep kernels (x-, y-, z-faces) and three ghost passes must agree"""
+    tos.test_P14_every_boundary_kind_treats_the_three_axes_alike(lo, hi, stretched)
+
+
+@pytest.mark.parametrize("bc", [(tos.IN, tos.OUT, tos.P, tos.P, tos.SL, tos.NS), (tos.P, tos.P, tos.EX, tos.NS, tos.OUT, tos.IN),
+                                (tos.EX, tos.IN, tos.SL, tos.SL, tos.NS, tos.EX)])
+@pytest.mark.parametrize("with_ibm", [False, True])
+def test_the_mirrored_problem_gives_the_mirrored_result(bc, with_ibm):
+    """P23 on the CUDA path: low and high side of every boundary kind, of the tiles' ragged edges, of IBM and ALM"""
+    tos.test_P23_the_mirrored_problem_gives_the_mirrored_result(bc, with_ibm)

@@ -15,6 +15,12 @@ from paper_2603_11102_b200.workloads import GridConfig
 P, NS, SL, IN, OUT, EX = range(6)
 
 
+# round-off bounds of the symmetry pins (P14, P23); tests/test_gpu_physics.py widens them for the CUDA path, whose
+# warps pick the series length of the collision stage per warp
+TOL_SYMMETRY = 5e-15
+TOL_UNIFORM = 0.0
+
+
 def new_solver(cfg):
     """the solver under test: the oracle here; tests/test_gpu_physics.py swaps in the CUDA library and runs the
     same exact-solution checks on it"""
@@ -422,13 +428,13 @@ def test_P14_every_boundary_kind_treats_the_three_axes_alike(lo, hi, stretched):
         W0[1 + t] = (rho * ut).reshape(shape)
         W = run(cfg, W0, 0.02, 4)
         other = tuple(i for i in range(3) if i != 2 - a)
-        assert max(np.ptp(W[c], axis=other).max() for c in range(4)) == 0.0
+        assert max(np.ptp(W[c], axis=other).max() for c in range(4)) <= TOL_UNIFORM
         pick = [0, 0, 0]
         pick[2 - a] = slice(None)
         pick = tuple(pick)
         lines.append(np.stack([W[0][pick], W[1 + a][pick], W[1 + t][pick], W[1 + (a + 2) % 3][pick]]))
         assert np.abs(lines[-1] - np.stack([rho, rho * un, rho * ut, 0 * rho])).max() > 1e-6      # it moved
-    assert np.abs(lines[0] - lines[1]).max() < 1e-15 and np.abs(lines[0] - lines[2]).max() < 1e-15
+    assert np.abs(lines[0] - lines[1]).max() < TOL_SYMMETRY and np.abs(lines[0] - lines[2]).max() < TOL_SYMMETRY
 
 
 # ---------------------------------------------------------------- P16 CFL time step
@@ -919,7 +925,7 @@ def test_P23_the_mirrored_problem_gives_the_mirrored_result(bc, with_ibm):
 
     def solve(faces_y, bcs, infl, state, apos, aforce, ipos):
         def setup(o):
-            o.alm_set_points(apos, aforce, 0.12)
+            o.alm_set_points(apos, aforce, 0.08)
             if with_ibm:
                 o.ibm_set_points(ipos, ibm_vol)
         cfg = GridConfig(n=n, faces=(None, faces_y, None), spacing=sp, nu=2e-3, bc=tuple(bcs), inflow=tuple(infl))
@@ -938,4 +944,4 @@ def test_P23_the_mirrored_problem_gives_the_mirrored_result(bc, with_ibm):
         mirror = lambda pts: np.where(np.arange(3) == a, length[a] - pts, pts)
         Wb = flip(solve((yf[-1] - yf)[::-1] if a == 1 else yf, bcm, inflm, flip(W0), mirror(alm_pos),
                         alm_force * sign[1:], mirror(ibm_pos)))
-        assert np.abs(Wa - Wb).max() < 5e-15, a
+        assert np.abs(Wa - Wb).max() < TOL_SYMMETRY, a
