@@ -145,7 +145,10 @@ gks_status gks_set_bulk_flux(gks_ctx *ctx, int axis, double target_bulk_momentum
 
 /* ALM (Eq. 10): n actuator points; pos and force are n*3 doubles (x,y,z per point),
  * host or device; force = point force ON THE FLUID; eps > 0 is the Gaussian width; the kernel is
- * sampled at cell centres and cut at r <= 3 eps.  n = 0 clears.  n <= GKS_MAX_ALM_POINTS. */
+ * sampled at cell centres and cut at r <= 3 eps.  n = 0 clears.  n <= GKS_MAX_ALM_POINTS.
+ * Points may lie anywhere along a periodic axis (they act through their images); 6 eps must be smaller than every
+ * periodic axis length (GKS_ERR_INVALID_ARG otherwise).  On a non-periodic axis the part of a support beyond the
+ * domain is lost. */
 gks_status alm_set_points(gks_ctx *ctx, int n, const double *pos, const double *force, double eps);
 
 /* On-line actuator-line rotor (Eq. 9, Eq. 14; S26-S27): instead of prescribed point

@@ -66,7 +66,10 @@ gks_status alm_bbox(gks_ctx *ctx, const double pmin[3], const double pmax[3], do
     long long l = cell_of(pmin[a] - R) - 1, h = cell_of(pmax[a] + R) + 1;
     if (ctx->g.periodic[a]) {
       if (2.0 * R >= L) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "alm: 6 eps must be smaller than a periodic axis");
-      if (h - l + 1 > nn) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "alm: point cloud + support wider than a periodic axis");
+      if (h - l + 1 > nn) { /* the whole axis: k_alm takes the nearest image of every point along it */
+        l = 0;
+        h = nn - 1;
+      }
     } else {
       if (l < 0) l = 0;
       if (h > nn - 1) h = nn - 1;

@@ -219,6 +219,15 @@ __global__ void __launch_bounds__(128) k_alm(GksGrid g, double *__restrict__ W, 
   int iu[3] = {0, 0, 0};
   double xc[3] = {0, 0, 0};
   long long id = 0;
+  /* a box that covers a whole periodic axis (point cloud + support wider than the axis) visits every cell once and
+     takes the nearest image of each point along that axis; 6 eps < L (checked by the host) leaves only one in range */
+  double Lmi[3];
+  {
+    const int cc[3] = {c0, c1, c2};
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+      Lmi[a] = (g.periodic[a] && cc[a] == g.n[a]) ? g.xf[a][g.n[a] + GKS_NG] - g.xf[a][GKS_NG] : 0.0;
+  }
   if (active) {
     iu[0] = lo0 + (int)(t % c0);
     iu[1] = lo1 + (int)((t / c0) % c1);
@@ -249,7 +258,10 @@ __global__ void __launch_bounds__(128) k_alm(GksGrid g, double *__restrict__ W, 
     __syncthreads();
     if (active) {
       for (int q = 0; q < cnt; ++q) {
-        const double rx = xc[0] - sp[3 * q], ry = xc[1] - sp[3 * q + 1], rz = xc[2] - sp[3 * q + 2];
+        double rx = xc[0] - sp[3 * q], ry = xc[1] - sp[3 * q + 1], rz = xc[2] - sp[3 * q + 2];
+        if (Lmi[0] > 0.0) rx -= Lmi[0] * rint(rx / Lmi[0]);
+        if (Lmi[1] > 0.0) ry -= Lmi[1] * rint(ry / Lmi[1]);
+        if (Lmi[2] > 0.0) rz -= Lmi[2] * rint(rz / Lmi[2]);
         const double r2 = rx * rx + ry * ry + rz * rz;
         if (r2 <= R2) {
           const double kern = norm * exp(-r2 * ie2);

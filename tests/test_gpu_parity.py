@@ -146,6 +146,39 @@ def test_error_paths_on_the_device():
     g.close()
 
 
+def test_alm_cloud_wider_than_a_periodic_axis():
+    """actuator points spread over more than a period of y and z (a rotor in a narrow periodic box): the gather box
+    covers the whole axis once and takes the nearest image of every point; points outside [0, L) wrap"""
+    from oracle import binding as ob
+    from paper_2603_11102_b200 import gks
+    n, h = (16, 10, 12), 0.1
+    cfg = GridConfig(n=n, spacing=(h, h, h), nu=1e-3, bc=(EX, EX, P, P, P, P))
+    rng = np.random.default_rng(11)
+    W0 = np.zeros((4, n[2], n[1], n[0]))
+    W0[0] = 1.0 + 0.01 * rng.standard_normal(W0[0].shape)
+    W0[1] = 0.1 * W0[0]
+    pos = np.column_stack([rng.uniform(0.5, 1.1, 40), rng.uniform(-0.3, 1.4, 40), rng.uniform(-0.2, 1.5, 40)])
+    force = 0.05 * rng.standard_normal((40, 3))
+    eps = 0.15                                       # 6 eps = 0.9 < 1.0 = the y period
+    o = ob.Oracle(cfg)
+    o.alm_set_points(pos, force, eps)
+    o.set_state(W0)
+    o.step(0.02)
+    g = gks.Gks(cfg)
+    g.alm_set_points(pos, force, eps)
+    g.set_state(W0)
+    g.step(0.02)
+    Wg, Wo = g.get_state(), o.get_state()
+    g.close()
+    o.close()
+    assert rel_linf(Wg, Wo) <= TOL1
+    free = ob.Oracle(cfg)
+    free.set_state(W0)
+    free.step(0.02)
+    assert np.abs(Wo - free.get_state()).max() > 1e-5          # the forcing is there
+    free.close()
+
+
 @pytest.mark.parametrize("passes,tol", [(3, 0.0), (8, 0.0), (20, None)])
 def test_ibm_multi_direct_forcing_passes(passes, tol):
     """IBM passes (Eq. 11-12, S25) on the small cylinder and turbine cases: a fixed number of passes, and the
