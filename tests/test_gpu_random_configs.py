@@ -1,0 +1,95 @@
+"""Parity of the CUDA path with the oracle on SEEDED RANDOM configurations: sizes 6..29 per axis (ragged against every
+tile shape), any pair of boundary kinds per axis, stretched non-periodic axes, both RT, three viscosities, and any
+mix of ALM points, IBM points, body force and bulk-flux forcing.  Two steps, north_star tolerance 1e-11.
+Whatever the oracle accepts the library must accept, and the other way round."""
+import numpy as np
+import pytest
+
+from conftest import rel_linf
+from paper_2603_11102_b200.workloads import GridConfig
+
+pytestmark = pytest.mark.gpu
+
+P, NS, SL, IN, OUT, EX = range(6)
+KINDS = [(P, P), (NS, NS), (SL, SL), (NS, SL), (EX, EX), (IN, OUT), (OUT, IN), (IN, EX), (EX, NS), (SL, EX)]
+
+
+def random_case(seed):
+    rng = np.random.default_rng(seed)
+    n = tuple(int(v) for v in rng.integers(6, 30, 3))
+    bc, inflow = [], [1.0, 0.0, 0.0, 0.0]
+    for a in range(3):
+        lo, hi = KINDS[rng.integers(len(KINDS))]
+        bc += [lo, hi]
+        if IN in (lo, hi) or OUT in (lo, hi):
+            inflow[1 + a] = 0.1 if (lo == IN or hi == OUT) else -0.1
+    sp = tuple(float(v) for v in rng.uniform(0.05, 0.15, 3))
+    faces = [None] * 3
+    for a in range(3):
+        if bc[2 * a] != P and rng.random() < 0.4:
+            faces[a] = np.cumsum(np.r_[0.0, rng.uniform(0.7, 1.3, n[a])]) * sp[a]
+    cfg = GridConfig(n=n, faces=tuple(faces), spacing=sp, nu=float(rng.choice([0.0, 1e-3, 1e-2])), bc=tuple(bc),
+                     inflow=tuple(inflow), RT=float(rng.choice([1.0, 0.7])))
+    W0 = np.zeros((4, n[2], n[1], n[0]))
+    W0[0] = 1 + 0.02 * rng.standard_normal(W0[0].shape)
+    for c in range(3):
+        W0[1 + c] = W0[0] * (inflow[1 + c] + 0.02 * rng.standard_normal(W0[0].shape))
+    x0 = [cfg.face_coords(a)[0] for a in range(3)]
+    length = [cfg.face_coords(a)[-1] - x0[a] for a in range(3)]
+    alm = ibm = body = bulk = None
+    if rng.random() < 0.6:
+        k = int(rng.integers(1, 12))
+        eps = float(rng.uniform(1.0, 2.0) * max(sp))
+        if all(6 * eps < length[a] for a in range(3) if bc[2 * a] == P):
+            pos = np.column_stack([x0[a] + rng.uniform(-0.2, 1.2, k) * length[a] if bc[2 * a] == P
+                                   else x0[a] + rng.uniform(0.1, 0.9, k) * length[a] for a in range(3)])
+            alm = (pos, 0.05 * rng.standard_normal((k, 3)), eps)
+    if all(f is None for f in faces) and rng.random() < 0.6:
+        k = int(rng.integers(1, 30))
+        pos = np.column_stack([x0[a] + rng.uniform(0.3, 0.7, k) * length[a] for a in range(3)])
+        ibm = (pos, np.full(k, sp[0] * sp[1] * sp[2]) * rng.uniform(0.3, 1.0, k))
+    if rng.random() < 0.3:
+        body = tuple(0.01 * rng.standard_normal(3))
+    if rng.random() < 0.2:
+        bulk = (int(rng.integers(3)), 0.1)
+    dt = 0.3 * min(cfg.widths(a).min() for a in range(3)) / 1.3
+    return cfg, W0, alm, ibm, body, bulk, dt
+
+
+def two_steps(solver, cfg, W0, alm, ibm, body, bulk, dt):
+    s = solver(cfg)
+    try:
+        if alm:
+            s.alm_set_points(*alm)
+        if ibm:
+            s.ibm_set_points(*ibm)
+        if body:
+            s.set_body_force(*body)
+        if bulk:
+            s.set_bulk_flux(*bulk)
+        s.set_state(W0)
+        for _ in range(2):
+            s.step(dt)
+        return s.get_state()
+    finally:
+        s.close()
+
+
+@pytest.mark.parametrize("first", [0, 20, 40, 60, 80])
+def test_twenty_random_configurations(first):
+    from oracle import binding as ob
+    from paper_2603_11102_b200 import gks
+    forced = 0
+    for seed in range(first, first + 20):
+        case = random_case(seed)
+        try:
+            Wo = two_steps(ob.Oracle, *case)
+        except ob.OracleError:
+            with pytest.raises(gks.GksError):
+                two_steps(gks.Gks, *case)
+            continue
+        Wg = two_steps(gks.Gks, *case)
+        err = rel_linf(Wg, Wo)
+        assert err <= 1e-11, (seed, case[0].n, case[0].bc, err)
+        forced += any(c is not None for c in case[2:6])
+    assert forced >= 5
