@@ -1,12 +1,13 @@
 """Parity of the CUDA path with the oracle on SEEDED RANDOM configurations: sizes 6..29 per axis (ragged against every
 tile shape), any pair of boundary kinds per axis, stretched non-periodic axes, both RT, three viscosities, and any
-mix of ALM points, IBM points, body force and bulk-flux forcing.  Two steps, north_star tolerance 1e-11.
+mix of ALM points or an on-line rotor, IBM points with one or several forcing passes, body force, bulk-flux forcing
+and the linear-weight tangential variant.  Two steps, north_star tolerance 1e-11.
 Whatever the oracle accepts the library must accept, and the other way round."""
 import numpy as np
 import pytest
 
 from conftest import rel_linf
-from paper_2603_11102_b200.workloads import GridConfig
+from paper_2603_11102_b200.workloads import GridConfig, synthetic_rotor
 
 pytestmark = pytest.mark.gpu
 
@@ -53,16 +54,32 @@ def random_case(seed):
     if rng.random() < 0.2:
         bulk = (int(rng.integers(3)), 0.1)
     dt = 0.3 * min(cfg.widths(a).min() for a in range(3)) / 1.3
-    return cfg, W0, alm, ibm, body, bulk, dt
+    extras = {"linear": rng.random() < 0.25, "passes": int(rng.integers(2, 6)) if ibm and rng.random() < 0.4 else 0,
+              "rotor": None}
+    if alm is None and rng.random() < 0.5:          # a small rotor about the middle of the box, axis +x
+        R = 0.3 * min(length[1], length[2])
+        eps = float(1.5 * max(sp))
+        if all(6 * eps < length[a] for a in range(3) if bc[2 * a] == P):
+            hub = tuple(x0[a] + 0.5 * length[a] for a in range(3))
+            extras["rotor"] = synthetic_rotor(hub, R, eps, u_ref=0.1, tsr=5.0, nblades=int(rng.integers(2, 4)), npts=8,
+                                              seed=seed, freestream_correction=bool(rng.integers(2)),
+                                              tip_correction=bool(rng.integers(2)))
+    return cfg, W0, alm, ibm, body, bulk, dt, extras
 
 
-def two_steps(solver, cfg, W0, alm, ibm, body, bulk, dt):
+def two_steps(solver, cfg, W0, alm, ibm, body, bulk, dt, extras):
     s = solver(cfg)
     try:
+        if extras["linear"]:
+            s.set_reconstruction(1)
         if alm:
             s.alm_set_points(*alm)
+        if extras["rotor"] is not None:
+            s.alm_set_rotor(extras["rotor"])
         if ibm:
             s.ibm_set_points(*ibm)
+            if extras["passes"]:
+                s.ibm_set_iterations(extras["passes"], 0.0)
         if body:
             s.set_body_force(*body)
         if bulk:
@@ -91,5 +108,5 @@ def test_twenty_random_configurations(first):
         Wg = two_steps(gks.Gks, *case)
         err = rel_linf(Wg, Wo)
         assert err <= 1e-11, (seed, case[0].n, case[0].bc, err)
-        forced += any(c is not None for c in case[2:6])
+        forced += any(c is not None for c in case[2:6]) or case[7]["rotor"] is not None
     assert forced >= 5
