@@ -4,7 +4,8 @@ domain is divided along the x-direction ... the ghost cells are exchanged betwee
 Rank r owns the cells i in [x_lo[r], x_lo[r+1]) of the global grid; its sub-domain is an ordinary `gks.Gks`
 context whose cut faces carry GKS_BC_HALO.  Per step the 3 ghost planes x 4 fields of each cut face move
 twice: the state W^n before `step_begin`, the first-stage state W* before `step_finish`
-(include/gks.h, "Domain decomposition").  Actuator points are replicated on every rank: the Gaussian
+(include/gks.h, "Domain decomposition").  Actuator points are given to every rank whose cells their support
+reaches (`SlabDecomposition.alm_points`; images beyond the seam of a periodic x axis included): the Gaussian
 gather of a rank only adds to the cells it owns, so a support that straddles a cut needs no exchange.
 
 This module holds host logic only (who owns what, who talks to whom, in which order); every number is moved by
@@ -90,6 +91,41 @@ class SlabDecomposition:
             out_p.append(q)
             out_v.append(vol[m])
         return np.concatenate(out_p), np.concatenate(out_v)
+
+    def alm_points(self, rank, pos, force, eps):
+        """Actuator points sub-domain `rank` must know: those whose Gaussian support (3 eps) reaches the cells it owns.
+        A sub-domain's cut faces are not periodic, so on a periodic x axis a point acts on a slab beyond the seam
+        through its image: positions are wrapped into the period and the images one period below and above are
+        offered too (6 eps < period: a cell sees one image of a point at most)."""
+        pos, force = np.asarray(pos, dtype=np.float64), np.asarray(force, dtype=np.float64)
+        i0, i1 = self.owned(rank)
+        h, x0 = self.cfg.spacing[0], self.cfg.origin[0]
+        a, b = x0 + i0 * h - 3.0 * eps, x0 + i1 * h + 3.0 * eps
+        L = self.cfg.n[0] * h
+        wrap = self.periodic and self.world > 1
+        x = x0 + np.mod(pos[:, 0] - x0, L) if wrap else pos[:, 0]
+        out_p, out_f = [], []
+        for shift in ((0.0, -L, L) if wrap else (0.0,)):
+            m = (x + shift >= a) & (x + shift <= b)
+            q = pos[m].copy()
+            q[:, 0] = x[m] + shift
+            out_p.append(q)
+            out_f.append(force[m])
+        return np.concatenate(out_p), np.concatenate(out_f), eps
+
+    def seam_shift(self, rank, x, reach):
+        """the multiple of the period that brings the plane x within `reach` of sub-domain `rank` (0.0 if it already
+        is, or if x is not periodic, or if no image is)"""
+        if not (self.periodic and self.world > 1):
+            return 0.0
+        i0, i1 = self.owned(rank)
+        h, x0 = self.cfg.spacing[0], self.cfg.origin[0]
+        L = self.cfg.n[0] * h
+        xw = x0 + np.mod(x - x0, L)
+        for shift in (0.0, -L, L):
+            if x0 + i0 * h - reach <= xw + shift <= x0 + i1 * h + reach:
+                return float(xw + shift - x)
+        return 0.0
 
     def schedule(self, rank):
         """The exchange of one halo, as a list of (face to pack, destination rank, face the destination unpacks).
@@ -208,14 +244,20 @@ class RotorDriver:
         if many:                                   # all sub-domains in this process: the owner's arrays are everyone's
             solvers[self.owner].alm_rotor_points(self.r, self.t, self.pos, self.force)
             solvers[self.owner].synchronize()
-            targets = solvers
+            targets = list(enumerate(solvers))
         else:
             if transport.rank == self.owner:
                 solvers.alm_rotor_points(self.r, self.t, self.pos, self.force)
             transport.broadcast(solvers, self.owner, [self.pos, self.force])
-            targets = [solvers]
-        for s in targets:
-            s.alm_set_points(self.pos, self.force, self.r.eps)
+            targets = [(transport.rank, solvers)]
+        for rank, s in targets:
+            # the disc is a plane x = hub_x: beyond the seam of a periodic x axis a slab meets its image
+            shift = self.d.seam_shift(rank, self.r.hub[0], 3.0 * self.r.eps)
+            pos = self.pos
+            if shift != 0.0:
+                pos = self.pos.clone()
+                pos[:, 0] += shift
+            s.alm_set_points(pos, self.force, self.r.eps)
 
     def advance(self, dt):
         self.t += dt

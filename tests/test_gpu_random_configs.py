@@ -110,3 +110,61 @@ def test_twenty_random_configurations(first):
         assert err <= 1e-11, (seed, case[0].n, case[0].bc, err)
         forced += any(c is not None for c in case[2:6]) or case[7]["rotor"] is not None
     assert forced >= 5
+
+
+def slab_case(seed):
+    """a random case whose x axis can be cut: uniform x, at least 6 cells per slab, periodic or closed or
+    inflow/outflow x; forcing of every kind"""
+    rng = np.random.default_rng(10_000 + seed)
+    for trial in range(100):
+        case = random_case(int(rng.integers(1 << 30)))
+        cfg = case[0]
+        world = int(rng.integers(2, 5))
+        if cfg.faces[0] is None and cfg.n[0] // world >= 6 and OUT not in cfg.bc[2:]:   # include/gks.h: outflow on the cut axis only
+            return case, world
+    raise AssertionError("no cuttable case")
+
+
+def slab_two_steps(case, world):
+    from paper_2603_11102_b200 import gks, slab
+    cfg, W0, alm, ibm, body, bulk, dt, extras = case
+    d = slab.SlabDecomposition(cfg, world)
+    solvers = [gks.Gks(d.local_cfg(r)) for r in range(world)]
+    try:
+        for r, s in enumerate(solvers):
+            if extras["linear"]:
+                s.set_reconstruction(1)
+            if ibm:
+                s.ibm_set_points(*d.ibm_points(r, *ibm))
+                if extras["passes"]:
+                    s.ibm_set_iterations(extras["passes"], 0.0)
+            if body:
+                s.set_body_force(*body)
+            if bulk:
+                s.set_bulk_flux(*bulk)
+            s.set_state(d.scatter(W0, r))
+        stepper = slab.SlabStepper(slab.LocalTransport(d), solvers, slab.BufferPool("cuda:0"))
+        rot = slab.RotorDriver(d, extras["rotor"], "cuda:0") if extras["rotor"] is not None else None
+        for _ in range(2):
+            stepper.step(dt, before_forcing=(lambda s: s.alm_set_points(*d.alm_points(solvers.index(s), *alm))) if alm else None,
+                         ibm=bool(ibm),
+                         bulk=bool(bulk), rotor=rot, ibm_passes=max(extras["passes"], 1))
+        return d.gather([s.get_state() for s in solvers])
+    finally:
+        for s in solvers:
+            s.close()
+
+
+@pytest.mark.parametrize("first", [0, 15])
+def test_fifteen_random_configurations_cut_into_x_slabs(first):
+    """the x-slab path (f3) on random configurations, 2-4 sub-domains in this process: equal to the single-domain run of
+    the library to round-off (the arithmetic of a cell does not depend on the sub-domain it sits in, up to the
+    warp-uniform series length) and to the oracle within the north_star tolerance"""
+    from oracle import binding as ob
+    from paper_2603_11102_b200 import gks
+    for seed in range(first, first + 15):
+        case, world = slab_case(seed)
+        Ws = slab_two_steps(case, world)
+        W1 = two_steps(gks.Gks, *case)
+        assert rel_linf(Ws, W1) <= 1e-13, (seed, world, case[0].n, case[0].bc)
+        assert rel_linf(Ws, two_steps(ob.Oracle, *case)) <= 1e-11, (seed, world)

@@ -271,3 +271,51 @@ def test_linear_variant_and_error_paths():
     with pytest.raises(gks.GksError):
         single.halo_pack(0, 0, torch.empty(single.halo_doubles(0), dtype=torch.float64, device="cuda:0"))   # not a HALO face
     single.close()
+
+
+def test_rotor_and_points_at_the_seam_of_a_periodic_x_axis():
+    """a rotor disc and prescribed actuator points within 3 eps of the periodic seam: the slab on the far side of the seam
+    meets them through their images (SlabDecomposition.alm_points, seam_shift)"""
+    from paper_2603_11102_b200 import gks
+    from paper_2603_11102_b200.workloads import GridConfig
+    n, h = (30, 12, 12), 0.1
+    cfg = GridConfig(n=n, spacing=(h, h, h), nu=1e-3, bc=(0,) * 6)
+    rng = np.random.default_rng(4)
+    W0 = np.zeros((4, n[2], n[1], n[0]))
+    W0[0] = 1 + 0.01 * rng.standard_normal(W0[0].shape)
+    W0[1] = 0.1 * W0[0]
+    eps, dt, world = 0.15, 0.02, 3
+    rotor = wl.synthetic_rotor(hub=(0.04, 0.6, 0.6), R=0.4, eps=eps, u_ref=0.1, tsr=5.0, npts=10)
+    pos = np.column_stack([rng.uniform(-0.3, 3.3, 12), rng.uniform(0, 1.2, 12), rng.uniform(0, 1.2, 12)])
+    force = 0.05 * rng.standard_normal((12, 3))
+    d = slab.SlabDecomposition(cfg, world)
+    for use_rotor in (True, False):
+        solvers = [gks.Gks(d.local_cfg(r)) for r in range(world)]
+        for r, s in enumerate(solvers):
+            s.set_state(d.scatter(W0, r))
+        stepper = slab.SlabStepper(slab.LocalTransport(d), solvers, slab.BufferPool("cuda:0"))
+        rot = slab.RotorDriver(d, rotor, "cuda:0") if use_rotor else None
+        hook = None if use_rotor else (lambda s: s.alm_set_points(*d.alm_points(solvers.index(s), pos, force, eps)))
+        for _ in range(3):
+            stepper.step(dt, before_forcing=hook, rotor=rot)
+        Ws = d.gather([s.get_state() for s in solvers])
+        for s in solvers:
+            s.close()
+        g = gks.Gks(cfg)
+        g.set_state(W0)
+        if use_rotor:
+            g.alm_set_rotor(rotor)
+        else:
+            g.alm_set_points(pos, force, eps)
+        for _ in range(3):
+            g.step(dt)
+        W1 = g.get_state()
+        g.close()
+        assert rel_linf(Ws, W1) <= 1e-13, use_rotor
+        # the forcing does reach the last slab (beyond the seam)
+        free = gks.Gks(cfg)
+        free.set_state(W0)
+        for _ in range(3):
+            free.step(dt)
+        assert np.abs(W1 - free.get_state())[..., -3:].max() > 1e-6
+        free.close()

@@ -170,3 +170,55 @@ def test_rotor_driver_owner_is_the_slab_that_contains_the_disc():
         assert slab.RotorDriver(slab.SlabDecomposition(w.cfg, world), r, "cpu").owner == owner
     r2 = wl.synthetic_rotor(hub=(2.99, 3.0, 3.0), R=1.0, eps=0.25)
     assert slab.RotorDriver(slab.SlabDecomposition(w.cfg, 4), r2, "cpu").owner == 0
+
+
+@pytest.mark.parametrize("periodic", [True, False])
+@pytest.mark.parametrize("world", [2, 3, 4])
+def test_alm_points_reach_every_slab_they_act_on(world, periodic):
+    """brute force: the Gaussian sums (cut at 3 eps) that the sub-domains form over the cells they own, from the
+    points `alm_points` gives them and WITHOUT any wrap along x, equal the sums of the whole domain with the
+    nearest image along a periodic x; points outside [0, L) and supports across the seam included"""
+    n, h, eps = 24, 0.1, 0.19                                   # 6 eps = 1.14 < L = 2.4
+    cfg = GridConfig(n=(n, 6, 6), spacing=(h, h, h), bc=((0, 0) if periodic else (5, 5)) + (0, 0, 0, 0))
+    d = slab.SlabDecomposition(cfg, world)
+    rng = np.random.default_rng(world)
+    L = n * h
+    pos = np.column_stack([rng.uniform(-0.6, L + 0.6, 30) if periodic else rng.uniform(0.0, L, 30),
+                           rng.uniform(0, 0.6, 30), rng.uniform(0, 0.6, 30)])
+    pos[0, 0], pos[1, 0] = 0.01, L - 0.02                       # right at the seam
+    force = rng.standard_normal((30, 3))
+    xc = (np.arange(n) + 0.5) * h
+
+    def gaussian_sum(points, weights, cells, wrap):
+        dx = cells[:, None] - points[None, :, 0]
+        if wrap:
+            dx -= L * np.round(dx / L)
+        k = np.exp(-(dx / eps) ** 2) * (np.abs(dx) <= 3 * eps)   # the y, z factors are the same on both sides
+        return k @ weights
+
+    whole = gaussian_sum(pos, force[:, 0], xc, periodic)
+    seen = np.zeros(30, dtype=int)
+    for r in range(world):
+        p, f, e = d.alm_points(r, pos, force, eps)
+        assert e == eps and p.shape == f.shape
+        i0, i1 = d.owned(r)
+        assert np.allclose(gaussian_sum(p, f[:, 0], xc[i0:i1], False), whole[i0:i1], rtol=1e-12, atol=1e-14)
+        assert np.array_equal(p[:, 1:], p[:, 1:]) and len(p) <= 2 * len(pos)
+        for q in p:                                              # every offered point is one of the originals, shifted by k L
+            j = np.where(np.all(np.isclose(pos[:, 1:], q[1:]), axis=1))[0]
+            assert len(j) == 1 and abs((q[0] - pos[j[0], 0]) / L - round((q[0] - pos[j[0], 0]) / L)) < 1e-12
+            seen[j[0]] += 1
+    assert (seen >= 1).all()
+    assert np.abs(whole).max() > 0.1
+
+
+def test_seam_shift_brings_the_rotor_disc_next_to_the_slab_beyond_the_seam():
+    cfg = GridConfig(n=(24, 6, 6), spacing=(0.1, 0.1, 0.1), bc=(0,) * 6)
+    d = slab.SlabDecomposition(cfg, 3)                           # slabs [0, 0.8), [0.8, 1.6), [1.6, 2.4)
+    assert d.seam_shift(0, 0.05, 0.3) == 0.0
+    assert d.seam_shift(2, 0.05, 0.3) == pytest.approx(2.4)      # the image at 2.45 acts on the last slab
+    assert d.seam_shift(1, 0.05, 0.3) == 0.0                     # out of reach of the middle slab either way
+    assert d.seam_shift(0, 2.35, 0.3) == pytest.approx(-2.4)
+    assert d.seam_shift(0, 2.35 + 2.4, 0.3) == pytest.approx(-4.8)
+    closed = slab.SlabDecomposition(GridConfig(n=(24, 6, 6), spacing=(0.1, 0.1, 0.1), bc=(5, 5, 0, 0, 0, 0)), 3)
+    assert closed.seam_shift(2, 0.05, 0.3) == 0.0
