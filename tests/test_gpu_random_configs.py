@@ -15,9 +15,12 @@ P, NS, SL, IN, OUT, EX = range(6)
 KINDS = [(P, P), (NS, NS), (SL, SL), (NS, SL), (EX, EX), (IN, OUT), (OUT, IN), (IN, EX), (EX, NS), (SL, EX)]
 
 
-def random_case(seed):
+def random_case(seed, wide=False):
     rng = np.random.default_rng(seed)
     n = tuple(int(v) for v in rng.integers(6, 30, 3))
+    if wide:        # two long axes and a short one: more tile columns than SMs, so whole-column waves AND a remainder
+        n = [int(rng.integers(120, 200)), int(rng.integers(120, 200)), int(rng.integers(6, 12))]
+        n = tuple(n[i] for i in rng.permutation(3))
     bc, inflow = [], [1.0, 0.0, 0.0, 0.0]
     for a in range(3):
         lo, hi = KINDS[rng.integers(len(KINDS))]
@@ -168,3 +171,14 @@ def test_fifteen_random_configurations_cut_into_x_slabs(first):
         W1 = two_steps(gks.Gks, *case)
         assert rel_linf(Ws, W1) <= 1e-13, (seed, world, case[0].n, case[0].bc)
         assert rel_linf(Ws, two_steps(ob.Oracle, *case)) <= 1e-11, (seed, world)
+
+
+@pytest.mark.parametrize("seed", [1, 2, 3, 4, 5, 6])
+def test_wide_random_configurations_fill_whole_waves_of_the_persistent_kernel(seed):
+    """about 200 tile columns on 148 SMs for the sweeps whose tile lies in the two long axes (whole-column waves plus an
+    evenly cut remainder) and a few long columns for the others"""
+    from oracle import binding as ob
+    from paper_2603_11102_b200 import gks
+    case = random_case(1000 + seed, wide=True)
+    err = rel_linf(two_steps(gks.Gks, *case), two_steps(ob.Oracle, *case))
+    assert err <= 1e-11, (case[0].n, case[0].bc, err)
