@@ -3,6 +3,8 @@ tile shape), any pair of boundary kinds per axis, stretched non-periodic axes, b
 mix of ALM points or an on-line rotor, IBM points with one or several forcing passes, body force, bulk-flux forcing
 and the linear-weight tangential variant.  Two steps, north_star tolerance 1e-11.
 Whatever the oracle accepts the library must accept, and the other way round."""
+from dataclasses import replace
+
 import numpy as np
 import pytest
 
@@ -182,3 +184,92 @@ def test_wide_random_configurations_fill_whole_waves_of_the_persistent_kernel(se
     case = random_case(1000 + seed, wide=True)
     err = rel_linf(two_steps(gks.Gks, *case), two_steps(ob.Oracle, *case))
     assert err <= 1e-11, (case[0].n, case[0].bc, err)
+
+
+# ---------------------------------------------------------------- invalid input: refusal parity
+def attempt(solver, cfg, W0, actions, dt):
+    """'ok', or where it was refused and why"""
+    try:
+        s = solver(cfg)
+    except Exception as e:
+        return "create: " + str(e)[:70]
+    try:
+        for name, args in actions:
+            getattr(s, name)(*args)
+        s.set_state(W0)
+        s.step(dt)
+        return "ok" if np.isfinite(s.get_state()).all() else "nonfinite"
+    except Exception as e:
+        return "call: " + str(e)[:70]
+    finally:
+        s.close()
+
+
+def defective_case(seed):
+    """a random case with one random defect (or borderline value) in the configuration, the time step or a call"""
+    rng = np.random.default_rng(50_000 + seed)
+    cfg, W0, _, _, _, _, dt, _ = random_case(int(rng.integers(1 << 30)))
+    x0 = [cfg.face_coords(a)[0] for a in range(3)]
+    length = [cfg.face_coords(a)[-1] - x0[a] for a in range(3)]
+    centre = np.array([[x0[a] + 0.5 * length[a] for a in range(3)]])
+    actions = []
+    defect, a = int(rng.integers(12)), int(rng.integers(3))
+    if defect == 0:       # ALM width: zero, negative, just above / below a sixth of the shortest axis
+        eps = float(rng.choice([0.0, -1.0, min(length) / 5.9, min(length) / 6.1]))
+        actions.append(("alm_set_points", (centre, np.ones((1, 3)), eps)))
+    elif defect == 1:     # ALM point outside the domain along axis a
+        p = centre.copy()
+        p[0, a] = x0[a] + float(rng.choice([-0.05, 1.05, -3.0, 4.0])) * length[a]
+        actions.append(("alm_set_points", (p, np.ones((1, 3)), 1.2 * max(cfg.spacing))))
+    elif defect == 2:     # IBM point near, on or beyond a boundary face of axis a
+        p = centre.copy()
+        p[0, a] = x0[a] + float(rng.choice([-0.01, 0.0, 0.01, 0.5, 0.99, 1.0, 1.01])) * length[a]
+        actions.append(("ibm_set_points", (p, np.array([1e-3]))))
+    elif defect == 3:     # IBM points on whatever grid the case has (stretched axes are refused)
+        p = np.column_stack([x0[b] + rng.uniform(0.05, 0.95, 5) * length[b] for b in range(3)])
+        actions.append(("ibm_set_points", (p, np.full(5, 1e-3))))
+    elif defect == 4:     # periodic on one side only
+        bc = list(cfg.bc)
+        bc[2 * a], bc[2 * a + 1] = P, int(rng.choice([NS, EX, P]))
+        cfg = replace(cfg, bc=tuple(bc), faces=(None, None, None))
+    elif defect == 5:     # 1..6 cells along axis a
+        n = list(cfg.n)
+        n[a] = int(rng.integers(1, 7))
+        cfg = replace(cfg, n=tuple(n), faces=(None, None, None))
+        W0 = np.ones((4, n[2], n[1], n[0]))
+        W0[1:] = 0.0
+    elif defect == 6:
+        dt = float(rng.choice([0.0, -1e-3, np.nan]))
+    elif defect == 7:
+        cfg = replace(cfg, RT=float(rng.choice([0.0, -1.0, 1.0])), nu=float(rng.choice([-1e-3, 0.0])))
+    elif defect == 8:     # face coordinates that do not increase
+        f = np.cumsum(np.r_[0.0, np.full(cfg.n[a], cfg.spacing[a])])
+        f[3] = f[2] if rng.random() < 0.5 else f[1]
+        faces, bc = list(cfg.faces), list(cfg.bc)
+        faces[a] = f
+        if bc[2 * a] == P:
+            bc[2 * a] = bc[2 * a + 1] = EX
+        cfg = replace(cfg, faces=tuple(faces), bc=tuple(bc))
+    elif defect == 9:
+        actions.append(("set_bulk_flux", (int(rng.choice([-1, 0, 2, 3, 7])), 0.1)))
+    elif defect == 10:    # (more than 64 passes is a limit of the library only, include/gks.h)
+        actions.append(("ibm_set_iterations", (int(rng.choice([0, -1, 1, 64])), float(rng.choice([0.0, -1.0, 1e-3])))))
+    else:
+        actions.append(("set_reconstruction", (int(rng.choice([-1, 0, 1, 2])),)))
+    return cfg, W0, actions, dt
+
+
+@pytest.mark.parametrize("first", [0, 50, 100])
+def test_what_the_oracle_refuses_the_library_refuses(first):
+    """ALM width against the periodic axes, points outside or on the boundary, IBM on stretched grids, unpaired
+    periodic faces, fewer than 6 cells, dt <= 0 or NaN, RT <= 0, nu < 0, non-increasing faces, bad axis / pass count /
+    variant arguments: the same accept-or-refuse decision on both sides, and a finite state wherever both accept"""
+    from oracle import binding as ob
+    from paper_2603_11102_b200 import gks
+    refused = 0
+    for seed in range(first, first + 50):
+        cfg, W0, actions, dt = defective_case(seed)
+        ro, rg = attempt(ob.Oracle, cfg, W0, actions, dt), attempt(gks.Gks, cfg, W0, actions, dt)
+        assert (ro == "ok") == (rg == "ok"), (seed, ro, rg)
+        refused += ro != "ok"
+    assert 5 <= refused <= 45
