@@ -92,7 +92,7 @@ def two_steps(solver, cfg, W0, alm, ibm, body, bulk, dt, extras):
         s.set_state(W0)
         for _ in range(2):
             s.step(dt)
-        return s.get_state()
+        return s.get_state(), s.cfl_dt(0.4)
     finally:
         s.close()
 
@@ -105,14 +105,15 @@ def test_twenty_random_configurations(first):
     for seed in range(first, first + 20):
         case = random_case(seed)
         try:
-            Wo = two_steps(ob.Oracle, *case)
+            Wo, dto = two_steps(ob.Oracle, *case)
         except ob.OracleError:
             with pytest.raises(gks.GksError):
                 two_steps(gks.Gks, *case)
             continue
-        Wg = two_steps(gks.Gks, *case)
+        Wg, dtg = two_steps(gks.Gks, *case)
         err = rel_linf(Wg, Wo)
         assert err <= 1e-11, (seed, case[0].n, case[0].bc, err)
+        assert dtg == pytest.approx(dto, rel=1e-12)          # the CFL time step of the state after the two steps
         forced += any(c is not None for c in case[2:6]) or case[7]["rotor"] is not None
     assert forced >= 5
 
@@ -170,9 +171,9 @@ def test_fifteen_random_configurations_cut_into_x_slabs(first):
     for seed in range(first, first + 15):
         case, world = slab_case(seed)
         Ws = slab_two_steps(case, world)
-        W1 = two_steps(gks.Gks, *case)
+        W1 = two_steps(gks.Gks, *case)[0]
         assert rel_linf(Ws, W1) <= 1e-13, (seed, world, case[0].n, case[0].bc)
-        assert rel_linf(Ws, two_steps(ob.Oracle, *case)) <= 1e-11, (seed, world)
+        assert rel_linf(Ws, two_steps(ob.Oracle, *case)[0]) <= 1e-11, (seed, world)
 
 
 @pytest.mark.parametrize("seed", [1, 2, 3, 4, 5, 6])
@@ -182,7 +183,7 @@ def test_wide_random_configurations_fill_whole_waves_of_the_persistent_kernel(se
     from oracle import binding as ob
     from paper_2603_11102_b200 import gks
     case = random_case(1000 + seed, wide=True)
-    err = rel_linf(two_steps(gks.Gks, *case), two_steps(ob.Oracle, *case))
+    err = rel_linf(two_steps(gks.Gks, *case)[0], two_steps(ob.Oracle, *case)[0])
     assert err <= 1e-11, (case[0].n, case[0].bc, err)
 
 
