@@ -560,7 +560,15 @@ typedef CUresult (*encode_fn_t)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, 
                                 CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 /* tile shapes: 128 faces per CTA; x-faces 8 (normal, along a) x 16 (t1), y/z-faces 16 (t1, along a) x 8 (normal) */
-template <int DIR> struct Shape { static constexpr int TA = DIR == 0 ? 8 : 16, TB = DIR == 0 ? 16 : 8; };
+#ifndef GKS_TILE_YZ_A
+#define GKS_TILE_YZ_A 32
+#endif
+#ifndef GKS_TILE_X_A
+#define GKS_TILE_X_A 8
+#endif
+template <int DIR> struct Shape {
+  static constexpr int TA = DIR == 0 ? GKS_TILE_X_A : GKS_TILE_YZ_A, TB = 128 / TA;
+};
 
 template <int DIR>
 bool encode_dir(encode_fn_t enc, const GksGrid &g, double *base, CUtensorMap *out) {
