@@ -559,7 +559,7 @@ typedef CUresult (*encode_fn_t)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, 
                                 const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
                                 CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-/* tile shapes: 128 faces per CTA; x-faces 8 (normal, along a) x 16 (t1), y/z-faces 16 (t1, along a) x 8 (normal) */
+/* tile shapes: 128 faces per CTA; x-faces 8 (normal, along a) x 16 (t1), y/z-faces 32 (t1, along a) x 4 (normal): measured */
 #ifndef GKS_TILE_YZ_A
 #define GKS_TILE_YZ_A 32
 #endif
