@@ -117,3 +117,27 @@ def test_every_boundary_kind_treats_the_three_axes_alike(lo, hi, stretched):
 def test_the_mirrored_problem_gives_the_mirrored_result(bc, with_ibm):
     """P23 on the CUDA path: low and high side of every boundary kind, of the tiles' ragged edges, of IBM and ALM"""
     tos.test_P23_the_mirrored_problem_gives_the_mirrored_result(bc, with_ibm)
+
+
+def test_three_hundred_steps_of_the_taylor_green_vortex_stay_conservative_and_dissipative():
+    """the metric box's flow at 128^3, 300 steps (a long run for a test, a blink for the GPU): mass and momentum are
+    conserved to round-off, the kinetic energy never grows (Re = 1600, early times: slow viscous decay), all finite"""
+    from paper_2603_11102_b200 import gks, workloads as wl
+    w = wl.taylor_green(128)
+    g = gks.Gks(w.cfg)
+    g.set_state(w.W0)
+    ke = lambda W: 0.5 * ((W[1:] ** 2).sum(0) / W[0]).sum(dtype=np.longdouble)
+    energy, sums0 = [ke(w.W0)], [w.W0[c].sum(dtype=np.longdouble) for c in range(4)]
+    scale = np.abs(w.W0[1:]).sum(dtype=np.longdouble)
+    for chunk in range(6):
+        for _ in range(50):
+            g.step(w.dt)
+        W = g.get_state()
+        g.check_finite()
+        energy.append(ke(W))
+        assert abs(W[0].sum(dtype=np.longdouble) - sums0[0]) <= 1e-12 * abs(sums0[0])
+        for c in range(1, 4):
+            assert abs(W[c].sum(dtype=np.longdouble) - sums0[c]) <= 1e-12 * scale
+    g.close()
+    drops = -np.diff(np.array(energy, dtype=np.float64))
+    assert (drops > 0).all() and drops.sum() < 0.05 * float(energy[0]), energy
