@@ -17,7 +17,7 @@ P, NS, SL, IN, OUT, EX = range(6)
 KINDS = [(P, P), (NS, NS), (SL, SL), (NS, SL), (EX, EX), (IN, OUT), (OUT, IN), (IN, EX), (EX, NS), (SL, EX)]
 
 
-def random_case(seed, wide=False):
+def random_case(seed, wide=False, anywhere=False):
     rng = np.random.default_rng(seed)
     n = tuple(int(v) for v in rng.integers(6, 30, 3))
     if wide:        # two long axes and a short one: more tile columns than SMs, so whole-column waves AND a remainder
@@ -47,12 +47,14 @@ def random_case(seed, wide=False):
         k = int(rng.integers(1, 12))
         eps = float(rng.uniform(1.0, 2.0) * max(sp))
         if all(6 * eps < length[a] for a in range(3) if bc[2 * a] == P):
+            inside = (0.0, 1.0) if anywhere else (0.1, 0.9)       # anywhere: supports cut by walls and faces
             pos = np.column_stack([x0[a] + rng.uniform(-0.2, 1.2, k) * length[a] if bc[2 * a] == P
-                                   else x0[a] + rng.uniform(0.1, 0.9, k) * length[a] for a in range(3)])
+                                   else x0[a] + rng.uniform(*inside, k) * length[a] for a in range(3)])
             alm = (pos, 0.05 * rng.standard_normal((k, 3)), eps)
     if all(f is None for f in faces) and rng.random() < 0.6:
         k = int(rng.integers(1, 30))
-        pos = np.column_stack([x0[a] + rng.uniform(0.3, 0.7, k) * length[a] for a in range(3)])
+        inside = (0.0, 1.0) if anywhere else (0.3, 0.7)       # anywhere: next to walls, across periodic seams
+        pos = np.column_stack([x0[a] + rng.uniform(*inside, k) * length[a] for a in range(3)])
         ibm = (pos, np.full(k, sp[0] * sp[1] * sp[2]) * rng.uniform(0.3, 1.0, k))
     if rng.random() < 0.3:
         body = tuple(0.01 * rng.standard_normal(3))
@@ -174,6 +176,21 @@ def test_fifteen_random_configurations_cut_into_x_slabs(first):
         W1 = two_steps(gks.Gks, *case)[0]
         assert rel_linf(Ws, W1) <= 1e-13, (seed, world, case[0].n, case[0].bc)
         assert rel_linf(Ws, two_steps(ob.Oracle, *case)[0]) <= 1e-11, (seed, world)
+
+
+def test_forty_random_configurations_with_points_anywhere_in_the_domain():
+    """Lagrangian and actuator points up to the boundary faces: supports cut by walls (dropped beyond them, include/gks.h),
+    wrapped across periodic seams, sitting on cell faces"""
+    from oracle import binding as ob
+    from paper_2603_11102_b200 import gks
+    with_points = 0
+    for seed in range(2000, 2040):
+        case = random_case(seed, anywhere=True)
+        Wo, _ = two_steps(ob.Oracle, *case)
+        Wg, _ = two_steps(gks.Gks, *case)
+        assert rel_linf(Wg, Wo) <= 1e-11, (seed, case[0].n, case[0].bc)
+        with_points += case[2] is not None or case[3] is not None
+    assert with_points >= 15
 
 
 @pytest.mark.parametrize("seed", [1, 2, 3, 4, 5, 6])
