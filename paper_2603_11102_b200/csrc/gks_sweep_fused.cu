@@ -39,7 +39,7 @@
 #include "gks_math.cuh"
 
 #ifndef GKS_E_WIDTH
-#define GKS_E_WIDTH 0   /* pass-2 evaluations written side by side: 2, 3 or 6; 0 = the measured best per direction */
+#define GKS_E_WIDTH 3   /* pass-2 evaluations written side by side: 2, 3 or 6 (measured: 3 is best for all three tile shapes) */
 #endif
 
 namespace {
@@ -481,7 +481,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
 #pragma unroll
     for (int k = 0; k < 4; ++k) rs[k] = rg + ((it + k) & 3) * RS;
     /* the six evaluations (field Q0, Dn, Dt1) x (g1 = -, +) run EW at a time, statement-interleaved */
-    constexpr int EW = GKS_E_WIDTH ? GKS_E_WIDTH : (DIR == 1 ? 2 : 3);   /* x- and z-faces 1 % faster 3 wide, y-faces 2 % slower */
+    constexpr int EW = GKS_E_WIDTH;
     static_assert(6 % EW == 0, "E width");
 #pragma unroll
     for (int e0 = 0; e0 < 6; e0 += EW) {
