@@ -302,9 +302,9 @@ def main():
             "kernel_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()},
         }
         if not args.no_cpu_baseline and world == 1:
-            rate, secs, cores = oracle_rate(64, 2)
+            rate, secs, cores = oracle_rate(128, 3, warmup=1)
             line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                    "sample": "2 steps of the 64^3 Taylor-Green box (same workload, reduced n)",
+                                    "sample": "3 steps (after 1 untimed) of the 128^3 Taylor-Green box (same workload, reduced n)",
                                     "seconds": secs}
         print(json.dumps(line), flush=True)
     g.close()
