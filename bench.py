@@ -173,6 +173,12 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    # the library is built in-tree (git ignores the .so): a fresh checkout compiles it once, rank 0 only
+    if rank == 0:
+        from paper_2603_11102_b200 import build as gks_build
+        gks_build.build()
+    barrier()
+
     w = wl.by_name(args.workload)
     slab_mode = args.decomp == "slab" and world > 1
     stepper = None

@@ -13,6 +13,17 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "slow: longer CPU test")
 
 
+def pytest_collection_modifyitems(config, items):
+    """The CUDA library is built in-tree and git ignores the .so: a fresh checkout compiles it (nvcc, seconds)
+    before the first GPU test; a failed build fails those tests loudly at load time (there is no CPU fallback)."""
+    if any(it.get_closest_marker("gpu") for it in items):
+        try:
+            from paper_2603_11102_b200 import build
+            build.build()
+        except Exception as e:  # the tests themselves report the missing library
+            sys.stderr.write("conftest: building libgks_b200.so failed: %s\n" % e)
+
+
 def rel_linf(a, b):
     """Error norm S24: density and momentum normalised separately; momentum components
     jointly by the largest momentum magnitude.  a = tested, b = oracle; shape (4, nz, ny, nx)."""
