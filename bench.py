@@ -27,6 +27,8 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "S2O4 GKS Mcell-steps/s (fp64)"
+# nominal fp64 FMA peak: 148 SMs x 64 DFMA lanes x 2 flop x 1.965 GHz
+FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 UNIT = "Mcell-steps/s"
 # Algorithmic fp64 flops of one cell-step (plain count of +,-,*,/ and one per
 # erfc/exp/sqrt, smoothness indicators shared between the two points of a cell, Navier-Stokes closed
@@ -300,6 +302,8 @@ def main():
                          "achieved": ach, "peak": fp64_peak, "unit": "TFLOP/s",
                          "frac": (ach / fp64_peak) if (ach and fp64_peak) else None, "traffic": traffic,
                          "peak_source": "fp64 DFMA microbenchmark in this run (gks_debug_fp64_peak)",
+                         "peak_nominal": FP64_NOMINAL_TFLOPS,
+                         "frac_nominal": (ach / FP64_NOMINAL_TFLOPS) if ach else None,
                          "flops_per_launch": flops_per_launch,
                          "share_of_step": sweep_ms / ms if ms > 0 else None},
             "hbm": {"bytes_per_cell_step_algorithmic": 192,
