@@ -589,10 +589,12 @@ int launch_dir(gks_ctx *ctx, const CUtensorMap &map, double *flux) {
   using T = Tile<DIR, TA, TB>;
   const GksGrid &g = ctx->g;
   auto kern = k_sweep_fused<DIR, NEED_F, LIN, TA, TB>;
-  static bool attr_done = false;
-  if (!attr_done) {
+  static bool attr_done[64] = {};                /* the attribute is per device: one process may hold contexts on several */
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (dev < 0 || dev >= 64 || !attr_done[dev]) {
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES);
-    attr_done = true;
+    if (dev >= 0 && dev < 64) attr_done[dev] = true;
   }
   const int ext_a = g.n[0] + (T::NA && !g.wrapf[0] ? 1 : 0), ext_b = g.n[T::AXB] + (!T::NA && !g.wrapf[T::AXB] ? 1 : 0);
   const int n2 = g.n[T::AXM];
