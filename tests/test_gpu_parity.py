@@ -379,3 +379,27 @@ def test_split_step_equals_gks_step_and_enforces_the_call_order():
             g.step_force(w.dt)
         g.close()
     assert rel_linf(res[1], res[0]) <= 1e-14
+
+
+def test_two_contexts_on_their_own_streams_do_not_interfere():
+    """include/gks.h: a context owns all of its state (workspace, stream, point sets); two contexts of different
+    shape and forcing, stepped alternately on their own streams with no synchronisation in between, give what
+    each gives alone - bit for bit on the periodic box, to round-off where the IBM spreading adds with atomics."""
+    from paper_2603_11102_b200 import gks
+    wa, wb = wl.by_name("C1"), wl.by_name("C5", small=True)
+    steps = 3
+    alone = [gks.run_workload(w, steps=steps) for w in (wa, wb)]
+    ga, gb = gks.Gks(wa.cfg), gks.Gks(wb.cfg)
+    assert ga.stream.cuda_stream != gb.stream.cuda_stream
+    gb.ibm_set_points(*wb.ibm)
+    ga.set_state(wa.W0)
+    gb.set_state(wb.W0)
+    for s in range(steps):
+        gb.alm_set_points(*wb.alm(s))
+        ga.step(wa.dt)
+        gb.step(wb.dt)
+    Wb, Wa = gb.get_state(), ga.get_state()
+    ga.close()
+    gb.close()
+    assert np.array_equal(Wa, alone[0])
+    assert rel_linf(Wb, alone[1]) <= 1e-13
