@@ -46,9 +46,10 @@ def build(force=False, verbose=False):
     if verbose:
         for l in logs:
             sys.stderr.write(l)
-    if force or jobs or _newer(LIB, objs):
+    if force or jobs or _newer(LIB, objs + [os.path.join(CSRC, "gks_exports.map")]):
         run([NVCC, "-shared", "-o", LIB] + objs + ["-gencode", "arch=compute_100a,code=sm_100a",
-                                                   "-ccbin", "/usr/bin/g++"])
+                                                   "-ccbin", "/usr/bin/g++", "-Xlinker",
+                                                   "--version-script=" + os.path.join(CSRC, "gks_exports.map")])
     return LIB
 
 
