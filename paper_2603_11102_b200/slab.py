@@ -201,12 +201,15 @@ class DistTransport:
         """(sum over ranks of a 1-element tensor, sum of the host number `volume`)"""
         import contextlib
         import torch
-        pair = torch.stack([scalar.reshape(()), torch.tensor(volume, dtype=torch.float64, device=scalar.device)])
+        # on the solver's stream throughout: `scalar` was written there (gks_bulk_partial) and torch's current
+        # stream is not ordered against it
         with (torch.cuda.stream(solver.stream) if scalar.is_cuda else contextlib.nullcontext()):
+            pair = torch.stack([scalar.reshape(()), torch.tensor(volume, dtype=torch.float64).to(scalar.device)])
             self.dist.all_reduce(pair, group=self.group)
+            total = pair[:1].contiguous()
         if scalar.is_cuda:
             solver.synchronize()
-        return pair[:1].contiguous(), float(pair[1])
+        return total, float(pair[1])
 
     def all_reduce_max(self, solver, scalar):
         import contextlib
@@ -255,8 +258,13 @@ class RotorDriver:
             shift = self.d.seam_shift(rank, self.r.hub[0], 3.0 * self.r.eps)
             pos = self.pos
             if shift != 0.0:
-                pos = self.pos.clone()
-                pos[:, 0] += shift
+                import contextlib
+                import torch
+                # on the solver's stream: ordered after the broadcast and before the library's copy, and the
+                # caching allocator reuses the block only behind that copy
+                with (torch.cuda.stream(s.stream) if self.pos.is_cuda else contextlib.nullcontext()):
+                    pos = self.pos.clone()
+                    pos[:, 0] += shift
             s.alm_set_points(pos, self.force, self.r.eps)
 
     def advance(self, dt):
@@ -288,6 +296,20 @@ class SlabStepper:
     def __init__(self, transport, solvers, new_buffer):
         self.t, self.solvers, self.new_buffer = transport, solvers, new_buffer
         self.many = isinstance(solvers, (list, tuple))
+        self._scr, self._keep = {}, []
+
+    def _scratch(self, name, n, dev):
+        """n persistent 1-element tensors.  The solvers write and read them on their OWN streams, which are not
+        ordered against torch's current stream: a fresh `torch.zeros` per step would race its fill against those
+        writes, and a temporary freed at return could be reused while a solver's copy from it is still queued.
+        Allocated once, filled once, with a device-wide synchronisation at that point only."""
+        import torch
+        key = (name, n)
+        if key not in self._scr:
+            self._scr[key] = [torch.zeros(1, dtype=torch.float64, device=dev) for _ in range(n)]
+            if self._scr[key][0].is_cuda:
+                torch.cuda.synchronize()
+        return self._scr[key]
 
     def _each(self, fn):
         for s in (self.solvers if self.many else [self.solvers]):
@@ -298,16 +320,19 @@ class SlabStepper:
         import torch
         sols = self.solvers if self.many else [self.solvers]
         dev = self.new_buffer.device if hasattr(self.new_buffer, "device") else "cpu"
-        parts = [torch.zeros(1, dtype=torch.float64, device=dev) for _ in sols]
+        parts = self._scratch("bulk", len(sols), dev)
         vols = [s.bulk_partial(p) for s, p in zip(sols, parts)]
         if self.many:
             for s in sols:
                 s.synchronize()
+            self._keep.clear()          # every solver stream is idle: nothing reads last step's totals any more
             total, volume = torch.stack(parts).sum(0), float(sum(vols))
             if total.is_cuda:
                 torch.cuda.current_stream().synchronize()   # the solvers copy it on their own streams
         else:
-            total, volume = self.t.all_reduce_sum(sols[0], parts[0], vols[0])
+            total, volume = self.t.all_reduce_sum(sols[0], parts[0], vols[0])   # synchronises the solver
+            self._keep.clear()
+        self._keep.append(total)        # the solvers copy from it asynchronously: alive until they were synchronised
         for s in sols:
             s.bulk_set_global(total, volume)
 
@@ -323,15 +348,17 @@ class SlabStepper:
             for s in sols:
                 s.ibm_pass(k, 0)
             if k > 0:
-                slips = [torch.zeros(1, dtype=torch.float64, device=dev) for _ in sols]
+                slips = self._scratch("slip%d" % k, len(sols), dev)
                 for s, r in zip(sols, slips):
                     s.ibm_residual(k, r)
                 if self.many:
                     for s in sols:
                         s.synchronize()
+                    self._keep.clear()          # safe point: every solver stream is idle
                     top = torch.stack(slips).max(0).values
                     if top.is_cuda:
                         torch.cuda.current_stream().synchronize()
+                    self._keep.append(top)      # copied by the solvers on their own streams after this returns
                 else:
                     top = self.t.all_reduce_max(sols[0], slips[0])
                 for s in sols:
