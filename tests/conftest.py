@@ -13,6 +13,34 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "slow: longer CPU test")
 
 
+def pytest_addoption(parser):
+    parser.addoption("--poison", action="store_true", default=False,
+                     help="fill every device buffer torch.empty hands out (solver workspaces, halo buffers) with NaN "
+                          "bit patterns first: a read of memory the library never wrote turns into a failed parity")
+
+
+@pytest.fixture(scope="session", autouse=True)
+def _poison_device_buffers(request):
+    """compute-sanitizer is not available on the GPU pool; this is the suite's own check for reads of
+    uninitialised workspace memory (`pytest -m gpu --poison`)."""
+    if not request.config.getoption("--poison"):
+        yield
+        return
+    import torch
+    orig = torch.empty
+
+    def empty(*a, **k):
+        t = orig(*a, **k)
+        if t.is_cuda and t.dtype in (torch.uint8, torch.float64):
+            t.fill_(255 if t.dtype == torch.uint8 else float("nan"))
+            torch.cuda.synchronize()        # the fill runs on torch's stream, the solvers on their own
+        return t
+
+    torch.empty = empty
+    yield
+    torch.empty = orig
+
+
 def pytest_collection_modifyitems(config, items):
     """The CUDA library is built in-tree and git ignores the .so: a fresh checkout compiles it (nvcc, seconds)
     before the first GPU test; a failed build fails those tests loudly at load time (there is no CPU fallback)."""

@@ -252,11 +252,22 @@ def test_linear_variant_and_error_paths():
     with pytest.raises(gks.GksError):
         g.step_finish(w.dt)                                  # without begin
     g.set_bulk_flux(0, 0.1)
+
+    def fill_halo_ghosts(which):
+        # the contract of gks_step_begin / gks_step_finish: HALO ghosts in place.  Any finite data will do here:
+        # the sub-domain is its own neighbour (what it packs at one face it unpacks beyond the other)
+        for src, dst in ((0, 1), (1, 0)):
+            g.halo_pack(which, src, buf)
+            g.halo_unpack(which, dst, buf)
+
+    fill_halo_ghosts(0)
     g.step_begin(w.dt)
+    fill_halo_ghosts(1)
     g.step_finish(w.dt)
     with pytest.raises(gks.GksError):
         g.step_force(w.dt)                                   # the global bulk sum was not supplied
     part = torch.zeros(1, dtype=torch.float64, device="cuda:0")
+    torch.cuda.synchronize()                                 # the fill runs on torch's stream, the solver on its own
     vol = g.bulk_partial(part)
     g.bulk_set_global(part, vol)
     g.step_force(w.dt)
