@@ -23,6 +23,9 @@
  *   - Pointers marked "host or device" are classified with cudaPointerGetAttributes; the copy is
  *     enqueued on the context's stream.  The caller owns every array it passes; the library copies
  *     what it needs during the call and never retains a caller pointer, except `workspace`.
+ *     A DEVICE array is read or written asynchronously ON THE CONTEXT'S STREAM: the caller orders its own
+ *     streams against that one (what another stream wrote must be complete before the call; the array must
+ *     stay allocated, and untouched by other streams, until the context's stream has passed the copy).
  *   - `workspace` is DEVICE memory owned by the caller (e.g. a torch tensor), at least
  *     gks_workspace_bytes(cfg) bytes, 256-byte aligned, kept alive until gks_destroy.  No call
  *     allocates device memory.  All kernels are enqueued on `cuda_stream` (a cudaStream_t; NULL = the
