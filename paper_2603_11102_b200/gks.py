@@ -138,6 +138,7 @@ class Gks:
             raise RuntimeError("no CUDA device: the gas-kinetic step has no CPU fallback")
         L = lib()
         self._torch = torch
+        self._sync_back = False
         self.device = torch.device(device)
         self.n = tuple(cfg.n)
         c, keep = make_config(cfg)
@@ -161,7 +162,24 @@ class Gks:
         self.n_ibm = 0
 
     # -- helpers
+    def _p(self, x):
+        """_ptr, plus the ordering include/gks.h asks of the caller when x is a device tensor that torch's current
+        stream produced or will consume: the solver's stream waits for torch's before the call, torch's waits for
+        the solver's after it (in _check), and the caching allocator keeps the block until the solver has passed."""
+        p, keep = _ptr(x)
+        t = self._torch
+        if isinstance(x, t.Tensor) and x.is_cuda:
+            cur = t.cuda.current_stream(x.device)
+            if cur != self.stream:
+                self.stream.wait_stream(cur)
+                x.record_stream(self.stream)
+                self._sync_back = True
+        return p, keep
+
     def _check(self, st):
+        if self._sync_back:
+            self._sync_back = False
+            self._torch.cuda.current_stream(self.device).wait_stream(self.stream)
         if st != GKS_OK:
             raise GksError(st, lib().gks_last_error(self._h).decode())
 
@@ -187,7 +205,7 @@ class Gks:
 
     # -- the C ABI, same names
     def set_state(self, W):
-        p, keep = _ptr(W)
+        p, keep = self._p(W)
         self._check(lib().gks_set_state(self._h, p))
         if isinstance(keep, np.ndarray):
             self.synchronize()      # pageable host source: be safe before the caller frees it
@@ -196,7 +214,7 @@ class Gks:
         """Returns a host numpy array, or fills `out` (numpy array or torch tensor, host or device)."""
         if out is None:
             out = np.empty(self.shape)
-        p, _ = _ptr(out)
+        p, _ = self._p(out)
         self._check(lib().gks_get_state(self._h, p))
         return out
 
@@ -211,14 +229,14 @@ class Gks:
 
     def alm_set_points(self, pos, force, eps):
         n = 0 if pos is None else (pos.shape[0] if hasattr(pos, "shape") else len(pos))
-        pp, k1 = _ptr(pos)
-        pf, k2 = _ptr(force)
+        pp, k1 = self._p(pos)
+        pf, k2 = self._p(force)
         self._check(lib().alm_set_points(self._h, n, pp, pf, float(eps)))
 
     def ibm_set_points(self, pos, weights):
         n = 0 if pos is None else (pos.shape[0] if hasattr(pos, "shape") else len(pos))
-        pp, k1 = _ptr(pos)
-        pw, k2 = _ptr(weights)
+        pp, k1 = self._p(pos)
+        pw, k2 = self._p(weights)
         self._check(lib().ibm_set_points(self._h, n, pp, pw))
         self.n_ibm = n
 
@@ -316,7 +334,7 @@ class Gks:
         self._check(lib().ibm_set_iterations(self._h, int(max_iter), float(tol)))
 
     def ibm_set_velocities(self, vel):
-        pv, k = _ptr(vel)
+        pv, k = self._p(vel)
         self._check(lib().ibm_set_velocities(self._h, pv))
 
     def debug_eval_flux(self, d):
