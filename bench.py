@@ -7,8 +7,11 @@ A "step" is one pass of the whole hot path (ghost fill, three fused sweeps, stag
 forcing) over the whole grid.  Prints ONE JSON line (rank 0).  See DESIGN.md §Measurement for the
 definitions of `roofline`, `e2e` and `cpu_baseline`.
 
-Multi-GPU: the path is built for one GPU (BASELINE.json north_star: no sharding, no collectives), so
---gpus N runs N independent replicas, one per rank ("replicas only", weak scaling).
+Multi-GPU: the metric is built for one GPU (BASELINE.json north_star: no sharding, no collectives), so by default
+--gpus N runs N independent replicas, one per rank ("replicas only", weak scaling).  `--decomp slab` instead cuts ONE
+workload into N x-slabs with halo exchange over NCCL (paper_2603_11102_b200/slab.py; strong
+scaling); that path is validated on one GPU and over gloo only - its NCCL numbers are UNVERIFIED until a box with two
+or more GPUs has run it, and the JSON line says so.
 """
 import argparse
 import csv
@@ -101,9 +104,10 @@ def setup_solver(w, gks, device):
 
 
 def oracle_rate(sample_n, steps, warmup=0):
-    """Mcell-steps/s of the CPU oracle, as it stands, on a Taylor-Green box of sample_n^3 cells."""
+    """Mcell-steps/s of the CPU oracle, as it stands, on a Taylor-Green box of sample_n^3 cells (256 = M0 itself)."""
     from oracle import binding as ob
     from paper_2603_11102_b200 import workloads as wl
+    ob.build()
     w = wl.taylor_green(sample_n)
     o = ob.Oracle(w.cfg)
     o.set_state(w.W0)
@@ -119,22 +123,66 @@ def oracle_rate(sample_n, steps, warmup=0):
 
 
 def run_reference(args, rank, world):
-    """--impl reference: the CPU oracle (the only reference this tier has), timed as it stands on the
-    host cores; each step is one oracle step on a bounded sample (64^3 box of the same workload)."""
+    """--impl reference: the CPU oracle (the only reference this tier has), timed as it stands on the host cores ON
+    THE METRIC BOX ITSELF (M0, 256^3).  One oracle step of 256^3 takes about 25 s on 16 cores, so the sample is
+    bounded: min(K, 2) timed steps, no warm-up steps (the oracle has no caches to warm: its first step costs what
+    every step costs); ms_per_step is the mean of the steps that were timed."""
     if rank != 0:
         return
-    sample = 64
-    rate, secs, cores = oracle_rate(sample, args.steps, args.warmup)
+    if args.workload != "M0":
+        raise SystemExit("--impl reference times the metric workload M0")
+    n = args.ref_box                      # 256 = M0 itself; smaller only for the CPU test of this arm's plumbing
+    timed = max(1, min(args.steps, 2))
+    rate, secs, cores = oracle_rate(n, timed, 0)
+    sample = "%d of the %d steps timed (no warm-up), each one oracle step of the whole %d^3 box" % (timed, args.steps, n)
     line = {"impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": secs / args.steps * 1e3,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": secs / timed * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
-            "config": {"workload": "M0 periodic Taylor-Green 256^3 (oracle timed on a %d^3 sample)" % sample},
-            "cpu_baseline": {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
-                             "sample": "%d step(s) of the %d^3 Taylor-Green box" % (args.steps, sample)},
+            "config": {"workload": "M0 taylor_green_%d %dx%dx%d" % (n, n, n, n), "sample": sample, "steps_timed": timed},
+            "cpu_baseline": {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
+
+
+def time_workload(gks, wl, name, device, steps, warmup=3, variant="weno"):
+    """Mcell-steps/s and per-class kernel times of one of the paper-shaped workloads, device-resident state,
+    CUDA events on the solver's stream (the same procedure as the headline number, fewer steps)."""
+    import torch
+    w = wl.by_name(name)
+    g = setup_solver(w, gks, device)
+    if variant == "linear":
+        g.set_reconstruction(1)
+    g.set_state(w.W0)
+    k = [0]
+
+    def one():
+        if w.alm is not None:
+            g.alm_set_points(*w.alm(k[0]))
+        g.step(w.dt)
+        k[0] += 1
+
+    for _ in range(warmup):
+        one()
+    g.synchronize()
+    g.profile_enable(True)
+    g.profile_read()
+    l0 = g.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(g.stream)
+    for _ in range(steps):
+        one()
+    e1.record(g.stream)
+    g.synchronize()
+    ms = e0.elapsed_time(e1)
+    prof = g.profile_read()
+    launches = g.launch_count - l0
+    g.check_finite()
+    g.close()
+    return {"workload": "%s %s %dx%dx%d" % (name, w.name, *w.cfg.n), "value": w.cfg.cells * steps / (ms * 1e-3) / 1e6,
+            "unit": UNIT, "steps": steps, "ms_per_step": ms / steps, "gpu_launches_per_step": launches / steps,
+            "kernel_ms_per_step": {c: v[0] / steps for c, v in prof.items()}}
 
 
 def main():
@@ -151,6 +199,10 @@ def main():
                     help="N > 1: replicas = N independent copies of the workload (default, weak scaling); slab = ONE\n"
                          "workload cut into N x-slabs with halo exchange over NCCL (strong scaling, PAPER.md:193-197)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ref-box", type=int, default=256,
+                    help="--impl reference: cells per axis of the Taylor-Green box the oracle is timed on (256 = M0)")
+    ap.add_argument("--no-configs", action="store_true", help="skip the C1..C5 throughput block of the JSON line")
+    ap.add_argument("--ibm-passes", type=int, default=1, help="IBM multi-direct-forcing passes per step (workloads with IBM)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -192,10 +244,19 @@ def main():
         ibm_local = dec.ibm_points(rank, *w.ibm) if w.ibm is not None else None
         w_global = w
         w = dc_replace(w, cfg=dec.local_cfg(rank), W0=dec.scatter(w.W0, rank), ibm=ibm_local)
-    g = setup_solver(w, gks, device)
+    if args.sweep == 1:                  # the unfused cross-check kernels exist in the debug library only
+        g = gks.Gks(w.cfg, device=device, debug=True)
+        if w.bulk_flux is not None:
+            g.set_bulk_flux(*w.bulk_flux)
+        if w.ibm is not None:
+            g.ibm_set_points(*w.ibm)
+        g.debug_set_sweep(1)
+    else:
+        g = setup_solver(w, gks, device)
+    if args.ibm_passes > 1 and w.ibm is not None:
+        g.ibm_set_iterations(args.ibm_passes, 0.0)
     if slab_mode:
         stepper = slab.SlabStepper(slab.DistTransport(dec, rank), g, slab.BufferPool(device))
-    g.debug_set_sweep(args.sweep)
     if args.variant == "linear":
         g.set_reconstruction(1)
     cells = w.cfg.cells
@@ -205,19 +266,26 @@ def main():
     g.set_state(Wd)
     step_no = [0]
 
+    def slab_step(k):
+        # actuator points reach a slab through dec.alm_points (supports across cuts, images beyond a periodic seam)
+        hook = (lambda s: s.alm_set_points(*dec.alm_points(rank, *w.alm(k)))) if w.alm is not None else None
+        stepper.step(w.dt, before_forcing=hook, ibm=w_global.ibm is not None, bulk=w.bulk_flux is not None,
+                     ibm_passes=args.ibm_passes)
+
     def one_step():
-        if w.alm is not None:
-            g.alm_set_points(*w.alm(step_no[0]))
         if stepper is not None:
-            stepper.step(w.dt, ibm=w_global.ibm is not None, bulk=w.bulk_flux is not None)
+            slab_step(step_no[0])
         else:
+            if w.alm is not None:
+                g.alm_set_points(*w.alm(step_no[0]))
             g.step(w.dt)
         step_no[0] += 1
 
     for _ in range(max(args.warmup, 3)):
         one_step()
     g.synchronize()
-    fp64_peak = g.debug_fp64_peak() if rank == 0 else None
+    # context figure only (the headline fraction is against the nominal unit count): DFMA throughput of this GPU
+    fp64_peak = gks.fp64_peak(device) if rank == 0 else None
 
     # ---- timed region: exactly K steps, device-resident state, CUDA events on the solver's stream
     g.profile_enable(True)
@@ -246,7 +314,7 @@ def main():
     nbytes = Hin.numel() * 8
     def plain_step():
         if stepper is not None:
-            stepper.step(w.dt, ibm=w_global.ibm is not None, bulk=w.bulk_flux is not None)
+            slab_step(step_no[0])
         else:
             g.step(w.dt)
 
@@ -279,13 +347,15 @@ def main():
         fpf = FLOPS_PER_FACE_LINEAR if args.variant == "linear" else FLOPS_PER_FACE
         flops_per_launch = 0.5 * (fpf[True] + fpf[False]) * faces
         ach = flops_per_launch / (sweep_ms / max(sweep_n, 1) * 1e-3) / 1e12 if sweep_ms > 0 else None
-        traffic = None
+        traffic, frac_pipe = None, None
         tps = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_traffic.csv")))
         if tps and args.workload == "M0" and args.sweep == 0 and args.variant == "weno":
             with open(tps[-1]) as f:      # latest round's ncu --set full capture (text summary, not executed)
                 for row in csv.DictReader(f):
                     if row["kernel"] == "sweep_mean_of_6":
                         traffic = float(row["dram_bytes_per_launch"])
+                        if row.get("fp64_pipe_active_pct"):
+                            frac_pipe = float(row["fp64_pipe_active_pct"]) / 100.0
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
@@ -298,12 +368,19 @@ def main():
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
                     "steps": args.e2e_steps},
             "gpu_launches": int(launches),
+            # headline fraction: against the NOMINAL fp64 rate (unit count x clock; neither MEASURED_PEAKS.json nor the
+            # profiling guide carries an fp64 figure).  frac_pipe: ncu "fp64 pipe active" of the same kernels from the
+            # committed capture (profiles/), the honest utilisation figure: `achieved` counts unfused +,-,* as one flop
+            # each while the peak counts two per DFMA.  peak_dfma_measured: this run's own DFMA calibration (context).
             "roofline": {"bound": "alu", "kernel": "sweep (reconstruction + flux), mean of 6 launches per step",
-                         "achieved": ach, "peak": fp64_peak, "unit": "TFLOP/s",
-                         "frac": (ach / fp64_peak) if (ach and fp64_peak) else None, "traffic": traffic,
-                         "peak_source": "fp64 DFMA microbenchmark in this run (gks_debug_fp64_peak)",
-                         "peak_nominal": FP64_NOMINAL_TFLOPS,
+                         "achieved": ach, "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s",
+                         "frac": (ach / FP64_NOMINAL_TFLOPS) if ach else None, "traffic": traffic,
+                         "peak_source": "nominal: 148 SMs x 64 fp64 FMA lanes x 2 flop x 1.965 GHz (DESIGN.md section 8)",
                          "frac_nominal": (ach / FP64_NOMINAL_TFLOPS) if ach else None,
+                         "frac_pipe": frac_pipe,
+                         "frac_pipe_source": os.path.relpath(tps[-1], ROOT) if (tps and frac_pipe is not None) else None,
+                         "peak_dfma_measured": fp64_peak,
+                         "frac_dfma_measured": (ach / fp64_peak) if (ach and fp64_peak) else None,
                          "flops_per_launch": flops_per_launch,
                          "share_of_step": sweep_ms / ms if ms > 0 else None},
             "hbm": {"bytes_per_cell_step_algorithmic": 192,
@@ -311,13 +388,24 @@ def main():
                     "peak_gbs": peaks.get("hbm_gbs"), "peak_source": peak_src},
             "kernel_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()},
         }
+        if slab_mode:
+            line["config"]["note"] = "x-slab numbers over NCCL are UNVERIFIED: validated on one GPU and over gloo only"
+    g.close()
+    if rank == 0:
+        if not args.no_configs and world == 1 and args.workload == "M0" and args.sweep == 0:
+            # north_star: throughput on the five paper-shaped workloads, same run, same procedure, 5 timed steps each
+            line["configs"] = {nm: time_workload(gks, wl, nm, device, steps=5, variant=args.variant)
+                               for nm in ("C1", "C2", "C3", "C4", "C5")}
         if not args.no_cpu_baseline and world == 1:
-            rate, secs, cores = oracle_rate(128, 3, warmup=1)
-            line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                    "sample": "3 steps (after 1 untimed) of the 128^3 Taylor-Green box (same workload, reduced n)",
+            if args.workload == "M0":       # the metric box itself: one oracle step of 256^3 (about 25 s on 16 cores)
+                rate, secs, cores = oracle_rate(256, 1, warmup=0)
+                sample = "1 oracle step of the whole 256^3 Taylor-Green box (the workload of `value`)"
+            else:
+                rate, secs, cores = oracle_rate(128, 3, warmup=1)
+                sample = "3 steps (after 1 untimed) of the 128^3 Taylor-Green box"
+            line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
                                     "seconds": secs}
         print(json.dumps(line), flush=True)
-    g.close()
     if world > 1:
         dist.destroy_process_group()
 

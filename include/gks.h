@@ -33,6 +33,8 @@
  *     the destination is host memory.
  *   - Every call returns a gks_status, never throws or aborts.  On error the context is unchanged
  *     and gks_last_error(ctx) (or gks_last_error(NULL) for gks_create failures) holds a message.
+ *   - A context belongs to the CUDA device that is current at gks_create (the workspace must live there); every
+ *     later call must find that device current, else GKS_ERR_STATE.
  *   - A context is not thread-safe.
  *   - There is no CPU fallback: without a CUDA device gks_create returns GKS_ERR_CUDA.
  */
@@ -79,7 +81,7 @@ typedef struct {
   int bc[6];                    /* gks_bc for xlo, xhi, ylo, yhi, zlo, zhi; periodic must be paired */
   double inflow[4];             /* rho, U, V, W for GKS_BC_INFLOW; |velocity normal to an outflow face| is
                                    the convective speed of GKS_BC_OUTFLOW_CONVECTIVE */
-  double weno_eps;              /* WENO-JS epsilon; 0 => 1e-6 */
+  double weno_eps;              /* WENO-JS epsilon; 0 => 1e-6; otherwise >= 1e-30 */
 } gks_config;
 
 /* Bytes of device workspace gks_create needs for this configuration (0 if cfg is invalid). */
@@ -91,7 +93,9 @@ gks_status gks_create(const gks_config *cfg, void *workspace, size_t workspace_b
 gks_status gks_destroy(gks_ctx *ctx);
 
 /* W: host or device, 4*nz*ny*nx doubles, W[c][k][j][i].  set_state also initialises the
- * convective-outflow ghost state (S20).  get_state synchronises for host destinations. */
+ * convective-outflow ghost state (S20).  get_state synchronises for host destinations.
+ * Inside a split step (between gks_step_begin and gks_step_force) gks_set_state returns GKS_ERR_STATE; gks_get_state
+ * is allowed there and reads W^n after gks_step_begin, the un-forced W^{n+1} after gks_step_finish. */
 gks_status gks_set_state(gks_ctx *ctx, const double *W);
 gks_status gks_get_state(gks_ctx *ctx, double *W);
 
@@ -127,7 +131,8 @@ gks_status gks_step(gks_ctx *ctx, double dt);
  *       sub-domain's max slip)  [k > 0: gks_ibm_residual get -> MAX over the sub-domains -> set]
  *       gks_ibm_pass(ctx, k, 1) (spread; skipped on the device once the slip fell below tol); gks_step_force
  *       then leaves the IBM alone.  Not available on a sub-domain: alm_set_rotor (use alm_rotor_points).
- * gks_step = begin + finish + force.  Errors: GKS_ERR_INVALID_ARG (face without HALO, NULL), GKS_ERR_STATE
+ * gks_step = begin + finish + force.  The three parts of one step must be given the same dt.
+ * Errors: GKS_ERR_INVALID_ARG (face without HALO, NULL, a dt that differs from gks_step_begin's), GKS_ERR_STATE
  * (order of the calls). */
 size_t gks_halo_doubles(const gks_ctx *ctx, int face);
 gks_status gks_halo_pack(gks_ctx *ctx, int which, int face, double *buf);
@@ -175,8 +180,18 @@ typedef struct {
 } alm_rotor;
 gks_status alm_set_rotor(gks_ctx *ctx, const alm_rotor *rotor);
 /* Test hook: positions and forces ON THE FLUID (nblades*npts*3 doubles each, host or device) of the actuator
- * points for the CURRENT state and rotor clock; synchronises the stream. */
+ * points for the CURRENT state and rotor clock; synchronises the stream unless both pointers are device memory. */
 gks_status alm_rotor_eval(gks_ctx *ctx, double *pos, double *force);
+
+/* The on-line rotor on a sub-domain (x-slab decomposition).  alm_set_rotor is accepted on every sub-domain: each
+ * keeps the rotor description and the rotor clock (advanced by dt in every gks_step_force, so all clocks agree), but
+ * the sampling reads across cuts, so a sub-domain does not evaluate the blade forces inside gks_step_force.  Between
+ * gks_step_finish and gks_step_force the driver (i) has the sub-domain that contains the disc evaluate them with
+ * alm_rotor_eval (device pointers: asynchronous), (ii) broadcasts the two small arrays and (iii) hands them to every
+ * sub-domain with alm_rotor_supply(ctx, pos, force, x_shift): nblades*npts*3 doubles each, host or device; x_shift is
+ * added to every x coordinate (a slab beyond the seam of a periodic x axis meets the disc through its image; else 0).
+ * gks_step_force on a sub-domain with a rotor set and nothing supplied for the step: GKS_ERR_STATE. */
+gks_status alm_rotor_supply(gks_ctx *ctx, const double *pos, const double *force, double x_shift);
 
 /* The same front half without state in the context: positions and forces ON THE FLUID of the actuator points of
  * `rotor` at rotor time t, sampled from the CURRENT state (between gks_step_finish and gks_step_force: the
@@ -215,13 +230,8 @@ gks_status gks_cfl_dt(gks_ctx *ctx, double cfl, double *dt);
 /* Test hook: fill ghosts of the CURRENT state and evaluate the face-averaged flux F and its
  * time derivative dF/dt (Eq. 6-7) for sweep direction dir in {0,1,2}.  Output (host or device):
  * 4 * (faces) doubles each, faces laid out like cells but with n_dir+1 entries along `dir`,
- * component-major: F[c][k][j][i].  Does not modify the state. */
+ * component-major: F[c][k][j][i].  Does not modify the state.  GKS_ERR_STATE inside a split step. */
 gks_status gks_debug_eval_flux(gks_ctx *ctx, int dir, double *F, double *dFdt);
-
-/* Test hook: choose the sweep implementation.  0 (default) = fused production kernels
- * (reconstruction + flux in one kernel per direction, slabs staged through shared memory by TMA);
- * 1 = unfused cross-check kernels (three kernels per direction, intermediates in HBM). */
-gks_status gks_debug_set_sweep(gks_ctx *ctx, int mode);
 
 /* Synchronising check of the current state; GKS_ERR_NONFINITE if any interior value is NaN/Inf. */
 gks_status gks_check_finite(gks_ctx *ctx);
@@ -235,10 +245,6 @@ enum { GKS_PROF_GHOST = 0, GKS_PROF_SWEEP_X = 1, GKS_PROF_SWEEP_Y = 2, GKS_PROF_
        GKS_PROF_UPDATE = 4, GKS_PROF_FORCING = 5, GKS_PROF_N = 6 };
 gks_status gks_profile_enable(gks_ctx *ctx, int on);
 gks_status gks_profile_read(gks_ctx *ctx, double *ms, long long *count);
-
-/* Calibration: sustained fp64 FMA throughput of this GPU in TFLOP/s (2 flop per DFMA), measured with
- * a register-resident DFMA kernel on the context's stream (about 50 ms).  Synchronises. */
-gks_status gks_debug_fp64_peak(gks_ctx *ctx, double *tflops);
 
 /* Number of kernels this context has launched since gks_create (for bench.py's gpu_launches). */
 long long gks_launch_count(const gks_ctx *ctx);

@@ -45,7 +45,8 @@ const char *validate(const gks_config *c) {
   if (!(c->RT > 0)) return "RT must be > 0";
   if (!(c->nu >= 0)) return "nu must be >= 0";
   if (!(c->rho_ref > 0)) return "rho_ref must be > 0";
-  if (c->weno_eps < 0) return "weno_eps must be >= 0";
+  /* the common-denominator WENO weights carry products of about eps^8: below 1e-30 they leave the fp64 range */
+  if (c->weno_eps < 0 || (c->weno_eps > 0 && c->weno_eps < 1e-30)) return "weno_eps must be 0 (default 1e-6) or >= 1e-30";
   const int n[3] = {c->nx, c->ny, c->nz};
   const double *f[3] = {c->xf, c->yf, c->zf};
   const double d[3] = {c->dx, c->dy, c->dz};
@@ -72,10 +73,13 @@ const char *validate(const gks_config *c) {
 struct Layout {
   int P[3];
   size_t FS;       /* doubles per padded field */
-  size_t off_Wn, off_Ws, off_P, off_flux[3], off_tmpN, off_tmpT, off_coords, off_red, off_alm_pos,
+  size_t off_Wn, off_Ws, off_P, off_flux[3], off_coords, off_red, off_alm_pos,
       off_alm_force, off_rotor, off_rotor_out, off_ibm_pos, off_ibm_vol, off_ibm_vel, off_ibm_coef, total;
   size_t coords_doubles;
   int ibm_capacity;
+#ifdef GKS_DEBUG
+  size_t off_tmpN, off_tmpT;   /* intermediates of the unfused cross-check sweep: debug library only */
+#endif
 };
 
 Layout make_layout(const gks_config *c) {
@@ -94,8 +98,10 @@ Layout make_layout(const gks_config *c) {
   L.off_Ws = take(4 * L.FS);
   L.off_P = take(4 * L.FS);
   for (int d = 0; d < 3; ++d) L.off_flux[d] = take(8 * L.FS);
+#ifdef GKS_DEBUG
   L.off_tmpN = take(8 * L.FS);
   L.off_tmpT = take(24 * L.FS);
+#endif
   /* per axis: xf (n+7), xc, w, inv_w, inv_hn (n+6 each) */
   L.coords_doubles = 0;
   const int n[3] = {c->nx, c->ny, c->nz};
@@ -158,6 +164,13 @@ bool gks_is_device_ptr(const void *p) {
   return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
 }
 
+gks_status gks_check_device(gks_ctx *ctx) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev != ctx->device)
+    return gks_set_err(ctx, GKS_ERR_STATE, "the context was created on CUDA device %d but device %d is current", ctx->device, dev);
+  return GKS_OK;
+}
+
 int gks_host_find_cell(const gks_ctx *ctx, int a, double x) {
   const int n = ctx->g.n[a];
   const double *xf = ctx->h_xf[a] + GKS_NG;
@@ -197,6 +210,15 @@ gks_status gks_create(const gks_config *cfg, void *workspace, size_t workspace_b
   if (workspace_bytes < L.total)
     return set_err(nullptr, GKS_ERR_WORKSPACE, "workspace too small: %zu < %zu bytes", workspace_bytes, L.total);
   if (!is_device_ptr(workspace)) return set_err(nullptr, GKS_ERR_WORKSPACE, "workspace is not device memory");
+  /* kernels, tensor maps and the SM count are those of the CURRENT device: it must be the workspace's */
+  int cur_dev = -1;
+  cudaPointerAttributes wat;
+  if (cudaGetDevice(&cur_dev) != cudaSuccess || cudaPointerGetAttributes(&wat, workspace) != cudaSuccess) {
+    cudaGetLastError();
+    return set_err(nullptr, GKS_ERR_CUDA, "cannot query the current device");
+  }
+  if (wat.type == cudaMemoryTypeDevice && wat.device != cur_dev)
+    return set_err(nullptr, GKS_ERR_WORKSPACE, "workspace lives on CUDA device %d but device %d is current", wat.device, cur_dev);
 
   gks_ctx *ctx = new (std::nothrow) gks_ctx();
   if (!ctx) return set_err(nullptr, GKS_ERR_INVALID_ARG, "out of host memory");
@@ -204,6 +226,7 @@ gks_status gks_create(const gks_config *cfg, void *workspace, size_t workspace_b
   ctx->cfg = *cfg;
   ctx->cfg.xf = ctx->cfg.yf = ctx->cfg.zf = nullptr; /* caller pointers are not retained */
   ctx->stream = (cudaStream_t)cuda_stream;
+  ctx->device = cur_dev;         /* workspace, stream and tensor maps belong to the device that is current now */
   ctx->bulk_axis = -1;
   ctx->ibm_maxit = 1;
   char *base = (char *)workspace;
@@ -211,8 +234,10 @@ gks_status gks_create(const gks_config *cfg, void *workspace, size_t workspace_b
   ctx->Ws = (double *)(base + L.off_Ws);
   ctx->Pbuf = (double *)(base + L.off_P);
   for (int d = 0; d < 3; ++d) ctx->flux[d] = (double *)(base + L.off_flux[d]);
+#ifdef GKS_DEBUG
   ctx->tmpN = (double *)(base + L.off_tmpN);
   ctx->tmpT = (double *)(base + L.off_tmpT);
+#endif
   ctx->coords = (double *)(base + L.off_coords);
   ctx->red = (double *)(base + L.off_red);
   ctx->alm_pos = (double *)(base + L.off_alm_pos);

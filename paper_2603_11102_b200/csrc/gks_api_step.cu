@@ -34,11 +34,13 @@ gks_status fetch_host(gks_ctx *ctx, const double *src, size_t count, std::vector
 void sweeps(gks_ctx *ctx, const double *W, bool need_F) {
   for (int d = 0; d < 3; ++d) {
     gks_prof_begin(ctx, GKS_PROF_SWEEP_X + d);
-    if (ctx->sweep_mode == 0)
-      ctx->launches += gks_launch_sweep_fused(ctx, d, W == ctx->Wn ? 0 : 1, ctx->flux[d], need_F);
-    else
+#ifdef GKS_DEBUG
+    if (ctx->sweep_mode == 1)
       ctx->launches += gks_launch_sweep_unfused(ctx->g, ctx->ph, d, W, ctx->tmpN, ctx->tmpT, ctx->flux[d], need_F,
                                                 ctx->stream);
+    else
+#endif
+      ctx->launches += gks_launch_sweep_fused(ctx, d, W == ctx->Wn ? 0 : 1, ctx->flux[d], need_F);
     gks_prof_end(ctx);
   }
 }
@@ -88,11 +90,13 @@ extern "C" {
 gks_status gks_set_state(gks_ctx *ctx, const double *W) {
   if (!ctx) return GKS_ERR_INVALID_ARG;
   if (!W) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "W is NULL");
+  if (gks_status st = gks_check_device(ctx)) return st;
+  if (ctx->mid_step) return gks_set_err(ctx, GKS_ERR_STATE, "gks_set_state inside an unfinished step (between gks_step_begin and gks_step_force)");
   const double *src = W;
-  if (!gks_is_device_ptr(W)) { /* host: stage through Pbuf (free between steps) */
-    CUDA_TRY(ctx, cudaMemcpyAsync(ctx->Pbuf, W, interior_doubles(ctx) * sizeof(double), cudaMemcpyHostToDevice,
+  if (!gks_is_device_ptr(W)) { /* host: stage through the flux buffer of the x-sweep (idle between the kernels of a step) */
+    CUDA_TRY(ctx, cudaMemcpyAsync(ctx->flux[0], W, interior_doubles(ctx) * sizeof(double), cudaMemcpyHostToDevice,
                                   ctx->stream));
-    src = ctx->Pbuf;
+    src = ctx->flux[0];
   }
   ctx->launches += gks_launch_pack(ctx->g, src, ctx->Wn, ctx->stream);
   ctx->launches += gks_launch_outflow_init(ctx->g, ctx->ph, ctx->Wn, ctx->stream);
@@ -105,13 +109,18 @@ gks_status gks_get_state(gks_ctx *ctx, double *W) {
   if (!ctx) return GKS_ERR_INVALID_ARG;
   if (!W) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "W is NULL");
   if (!ctx->have_state) return gks_set_err(ctx, GKS_ERR_STATE, "gks_get_state before gks_set_state");
+  if (gks_status st = gks_check_device(ctx)) return st;
   if (gks_is_device_ptr(W)) {
     ctx->launches += gks_launch_unpack(ctx->g, ctx->Wn, W, ctx->stream);
     CUDA_TRY(ctx, cudaGetLastError());
   } else {
-    ctx->launches += gks_launch_unpack(ctx->g, ctx->Wn, ctx->Pbuf, ctx->stream);
+    /* staged through the flux buffer of the x-sweep: free whenever no kernel of a step is in flight ahead of this
+       call on the stream - also inside a split step, where Pbuf holds the predictor P (the state read is then W^n
+       after gks_step_begin, the un-forced W^{n+1} after gks_step_finish) */
+    double *stage = ctx->flux[0];
+    ctx->launches += gks_launch_unpack(ctx->g, ctx->Wn, stage, ctx->stream);
     CUDA_TRY(ctx, cudaGetLastError());
-    CUDA_TRY(ctx, cudaMemcpyAsync(W, ctx->Pbuf, interior_doubles(ctx) * sizeof(double), cudaMemcpyDeviceToHost,
+    CUDA_TRY(ctx, cudaMemcpyAsync(W, stage, interior_doubles(ctx) * sizeof(double), cudaMemcpyDeviceToHost,
                                   ctx->stream));
     CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
   }
@@ -123,6 +132,8 @@ gks_status gks_step_begin(gks_ctx *ctx, double dt) {
   if (!ctx->have_state) return gks_set_err(ctx, GKS_ERR_STATE, "gks_step before gks_set_state");
   if (!(dt > 0) || !std::isfinite(dt)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "dt must be > 0");
   if (ctx->mid_step) return gks_set_err(ctx, GKS_ERR_STATE, "gks_step_begin inside an unfinished step");
+  if (gks_status st = gks_check_device(ctx)) return st;
+  ctx->step_dt = dt;
   const GksGrid &g = ctx->g;
   const GksPhys &ph = ctx->ph;
   cudaStream_t s = ctx->stream;
@@ -143,6 +154,8 @@ gks_status gks_step_finish(gks_ctx *ctx, double dt) {
   if (!ctx) return GKS_ERR_INVALID_ARG;
   if (ctx->mid_step != 1) return gks_set_err(ctx, GKS_ERR_STATE, "gks_step_finish without gks_step_begin");
   if (!(dt > 0) || !std::isfinite(dt)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "dt must be > 0");
+  if (dt != ctx->step_dt) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "gks_step_finish: dt = %.17g differs from the dt = %.17g of gks_step_begin", dt, ctx->step_dt);
+  if (gks_status st = gks_check_device(ctx)) return st;
   const GksGrid &g = ctx->g;
   const GksPhys &ph = ctx->ph;
   cudaStream_t s = ctx->stream;
@@ -163,6 +176,8 @@ gks_status gks_step_force(gks_ctx *ctx, double dt) {
   if (!ctx) return GKS_ERR_INVALID_ARG;
   if (ctx->mid_step != 2) return gks_set_err(ctx, GKS_ERR_STATE, "gks_step_force without gks_step_finish");
   if (!(dt > 0) || !std::isfinite(dt)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "dt must be > 0");
+  if (dt != ctx->step_dt) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "gks_step_force: dt = %.17g differs from the dt = %.17g of gks_step_begin", dt, ctx->step_dt);
+  if (gks_status st = gks_check_device(ctx)) return st;
   const GksGrid &g = ctx->g;
   const GksPhys &ph = ctx->ph;
   cudaStream_t s = ctx->stream;
@@ -172,15 +187,17 @@ gks_status gks_step_force(gks_ctx *ctx, double dt) {
     return gks_set_err(ctx, GKS_ERR_STATE, "IBM passes > 1 on a sub-domain need an exchange per pass: drive them with gks_ibm_pass");
   if (any_halo && ctx->bulk_axis >= 0 && !ctx->bulk_external)
     return gks_set_err(ctx, GKS_ERR_STATE, "bulk-flux forcing on a sub-domain: gks_bulk_set_global must supply the global sum first");
-  if (any_halo && ctx->rotor_on)
-    return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "the on-line rotor samples across cuts: not available on a sub-domain");
+  if (any_halo && ctx->rotor_on && !ctx->rotor_external)
+    return gks_set_err(ctx, GKS_ERR_STATE, "the on-line rotor samples across cuts: on a sub-domain this step's points must be supplied with alm_rotor_supply");
   ctx->mid_step = 0;
   gks_prof_begin(ctx, GKS_PROF_FORCING);
   /* forcing (Eq. 13), every increment from the un-forced field: read-only kernels first */
   const bool uniform = ctx->gacc[0] != 0.0 || ctx->gacc[1] != 0.0 || ctx->gacc[2] != 0.0;
   if (ctx->rotor_on) { /* ALM front half on the un-forced field at the rotor clock t^n (S12, S26) */
-    ctx->launches += gks_launch_rotor_forces(g, ctx->Wn, ctx->rotor, ctx->rotor_time, ctx->alm_eps, ctx->alm_pos,
-                                             ctx->alm_force, s);
+    if (!ctx->rotor_external)                     /* sub-domain: evaluated by the slab that holds the disc and supplied */
+      ctx->launches += gks_launch_rotor_forces(g, ctx->Wn, ctx->rotor, ctx->rotor_time, ctx->alm_eps, ctx->alm_pos,
+                                               ctx->alm_force, s);
+    ctx->rotor_external = 0;
     ctx->n_alm = ctx->rotor.nb * ctx->rotor.np;
     ctx->rotor_time += dt;
   }
@@ -239,8 +256,8 @@ gks_status halo_move(gks_ctx *ctx, int which, int face, double *buf, int unpack)
   const size_t bytes = gks_halo_doubles(ctx, face) * sizeof(double);
   if (gks_is_device_ptr(buf)) {
     ctx->launches += gks_launch_halo(ctx->g, W, buf, face, unpack, ctx->stream);
-  } else { /* host buffer: stage through the tangential-pass scratch of the unfused sweep (idle here) */
-    double *stage = ctx->tmpT;
+  } else { /* host buffer: stage through the flux buffer of the y-sweep (idle at every point a halo may move) */
+    double *stage = ctx->flux[1];
     if (unpack) CUDA_TRY(ctx, cudaMemcpyAsync(stage, buf, bytes, cudaMemcpyHostToDevice, ctx->stream));
     ctx->launches += gks_launch_halo(ctx->g, W, stage, face, unpack, ctx->stream);
     if (!unpack) CUDA_TRY(ctx, cudaMemcpyAsync(buf, stage, bytes, cudaMemcpyDeviceToHost, ctx->stream));
@@ -341,6 +358,7 @@ gks_status alm_set_points(gks_ctx *ctx, int n, const double *pos, const double *
   if (!ctx) return GKS_ERR_INVALID_ARG;
   if (n < 0 || n > GKS_MAX_ALM_POINTS) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "n out of range");
   ctx->rotor_on = 0;   /* prescribed points replace an on-line rotor */
+  ctx->rotor_external = 0;
   if (n == 0) {
     ctx->n_alm = 0;
     return GKS_OK;
@@ -432,7 +450,35 @@ gks_status alm_set_rotor(gks_ctx *ctx, const alm_rotor *r) {
   ctx->alm_eps = r->eps;
   ctx->n_alm = 0;
   ctx->rotor_on = 1;
+  ctx->rotor_external = 0;
   ctx->rotor_time = 0.0;
+  return GKS_OK;
+}
+
+gks_status alm_rotor_supply(gks_ctx *ctx, const double *pos, const double *force, double x_shift) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (!pos || !force || !std::isfinite(x_shift)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "pos/force is NULL or x_shift is not finite");
+  if (!ctx->rotor_on) return gks_set_err(ctx, GKS_ERR_STATE, "no rotor set");
+  if (ctx->mid_step != 2) return gks_set_err(ctx, GKS_ERR_STATE, "alm_rotor_supply belongs between gks_step_finish and gks_step_force");
+  /* the gather box of the disc as this sub-domain meets it (beyond the seam of a periodic x axis: its image) */
+  const GksRotor &R = ctx->rotor;
+  const double pmin[3] = {R.hub[0] + x_shift, R.hub[1] - R.R, R.hub[2] - R.R};
+  const double pmax[3] = {R.hub[0] + x_shift, R.hub[1] + R.R, R.hub[2] + R.R};
+  int lo[3], cnt[3];
+  if (gks_status st = alm_bbox(ctx, pmin, pmax, ctx->alm_eps, lo, cnt)) return st;
+  const size_t bytes = 3 * (size_t)R.nb * R.np * sizeof(double);
+  const cudaMemcpyKind kp = gks_is_device_ptr(pos) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  const cudaMemcpyKind kf = gks_is_device_ptr(force) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  CUDA_TRY(ctx, cudaMemcpyAsync(ctx->alm_pos, pos, bytes, kp, ctx->stream));
+  CUDA_TRY(ctx, cudaMemcpyAsync(ctx->alm_force, force, bytes, kf, ctx->stream));
+  if (x_shift != 0.0) ctx->launches += gks_launch_shift_x(ctx->alm_pos, R.nb * R.np, x_shift, ctx->stream);
+  if (kp == cudaMemcpyHostToDevice || kf == cudaMemcpyHostToDevice) CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+  CUDA_TRY(ctx, cudaGetLastError());
+  for (int a = 0; a < 3; ++a) {
+    ctx->alm_lo[a] = lo[a];
+    ctx->alm_cnt[a] = cnt[a];
+  }
+  ctx->rotor_external = 1;
   return GKS_OK;
 }
 
@@ -467,7 +513,7 @@ gks_status alm_rotor_eval(gks_ctx *ctx, double *pos, double *force) {
   const cudaMemcpyKind kf = gks_is_device_ptr(force) ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
   CUDA_TRY(ctx, cudaMemcpyAsync(pos, ctx->alm_pos, 3 * (size_t)n * sizeof(double), kp, ctx->stream));
   CUDA_TRY(ctx, cudaMemcpyAsync(force, ctx->alm_force, 3 * (size_t)n * sizeof(double), kf, ctx->stream));
-  CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+  if (kp == cudaMemcpyDeviceToHost || kf == cudaMemcpyDeviceToHost) CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
   return GKS_OK;
 }
 
@@ -545,13 +591,17 @@ gks_status gks_debug_eval_flux(gks_ctx *ctx, int dir, double *F, double *dFdt) {
   if (!ctx) return GKS_ERR_INVALID_ARG;
   if (dir < 0 || dir > 2 || !F || !dFdt) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "bad dir or NULL output");
   if (!ctx->have_state) return gks_set_err(ctx, GKS_ERR_STATE, "gks_debug_eval_flux before gks_set_state");
+  if (ctx->mid_step) return gks_set_err(ctx, GKS_ERR_STATE, "gks_debug_eval_flux inside an unfinished step (it refills ghosts and flux buffers)");
+  if (gks_status st = gks_check_device(ctx)) return st;
   const GksGrid &g = ctx->g;
   ctx->launches += gks_launch_ghost_fill(g, ctx->ph, ctx->Wn, ctx->Wn, ctx->stream);
-  if (ctx->sweep_mode == 0)
-    ctx->launches += gks_launch_sweep_fused(ctx, dir, 0, ctx->flux[dir], true);
-  else
+#ifdef GKS_DEBUG
+  if (ctx->sweep_mode == 1)
     ctx->launches += gks_launch_sweep_unfused(g, ctx->ph, dir, ctx->Wn, ctx->tmpN, ctx->tmpT, ctx->flux[dir], true,
                                               ctx->stream);
+  else
+#endif
+    ctx->launches += gks_launch_sweep_fused(ctx, dir, 0, ctx->flux[dir], true);
   const size_t nf = 4 * (size_t)(g.n[0] + (dir == 0)) * (g.n[1] + (dir == 1)) * (g.n[2] + (dir == 2));
   double *outs[2] = {F, dFdt};
   for (int h = 0; h < 2; ++h) {
@@ -586,12 +636,15 @@ gks_status gks_cfl_dt(gks_ctx *ctx, double cfl, double *dt) {
   return GKS_OK;
 }
 
+#ifdef GKS_DEBUG
 gks_status gks_debug_set_sweep(gks_ctx *ctx, int mode) {
   if (!ctx) return GKS_ERR_INVALID_ARG;
   if (mode != 0 && mode != 1) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "mode must be 0 or 1");
+  if (ctx->mid_step) return gks_set_err(ctx, GKS_ERR_STATE, "gks_debug_set_sweep inside an unfinished step");
   ctx->sweep_mode = mode;
   return GKS_OK;
 }
+#endif
 
 gks_status gks_check_finite(gks_ctx *ctx) {
   if (!ctx) return GKS_ERR_INVALID_ARG;

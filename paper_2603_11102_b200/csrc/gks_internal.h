@@ -14,6 +14,9 @@
 #include <stddef.h>
 
 #include "../../include/gks.h"
+#ifdef GKS_DEBUG
+#include "../../include/gks_debug.h"
+#endif
 
 #define GKS_NG 3
 
@@ -63,14 +66,17 @@ struct gks_ctx {
   cudaStream_t stream;
   bool have_state;
   int mid_step;               /* 0 idle, 1 after gks_step_begin, 2 after gks_step_finish (forcing pending) */
-  int sweep_mode;             /* 0 fused, 1 unfused */
+  double step_dt;             /* dt of the step in flight (gks_step_begin): finish and force must be given the same */
+  int device;                 /* CUDA device of the workspace and stream: every call must find it current */
+  int sweep_mode;             /* 0 fused, 1 unfused (GKS_DEBUG builds only) */
   long long launches;
   char err[512];
 
   /* workspace carve (device) */
   double *Wn, *Ws, *Pbuf;      /* padded 4-field states; Pbuf doubles as staging between steps */
   double *flux[3];             /* per direction: F[4] then dF[4], padded index space */
-  double *tmpN, *tmpT;         /* unfused sweep intermediates: 8 and 24 padded fields */
+  double *tmpN, *tmpT;         /* unfused cross-check sweep: 8 and 24 padded fields of intermediates; NULL unless
+                                  GKS_DEBUG (the struct layout does not depend on the macro: objects are shared) */
   double *coords;              /* coordinate tables */
   double *red;                 /* reduction scratch (partials + result) */
   double *alm_pos, *alm_force; /* GKS_MAX_ALM_POINTS*3 each */
@@ -93,6 +99,7 @@ struct gks_ctx {
   int alm_lo[3], alm_cnt[3];   /* bounding box of the ALM support in (unwrapped) cell indices */
   GksRotor rotor;              /* valid when rotor_on */
   int rotor_on;
+  int rotor_external;          /* sub-domain: this step's actuator points were supplied with alm_rotor_supply */
   double rotor_time;           /* rotor clock: 0 at alm_set_rotor, + dt per step */
   double *rotor_out;           /* device scratch of alm_rotor_points: pos, force (GKS_MAX_ALM_POINTS*3 each) */
   double *rotor_tab;           /* device: chord, twist (GKS_MAX_ROTOR_STATIONS each), alpha, cl, cd (GKS_MAX_POLAR each) */
@@ -120,6 +127,7 @@ void gks_prof_free(gks_ctx *ctx);
 
 /* ---- host helpers shared by the API translation units ---- */
 gks_status gks_set_err(gks_ctx *ctx, gks_status st, const char *fmt, ...);
+gks_status gks_check_device(gks_ctx *ctx);   /* GKS_ERR_STATE unless the context's device is the current one */
 bool gks_is_device_ptr(const void *p);
 int gks_host_find_cell(const gks_ctx *ctx, int a, double x); /* interior cell containing x, or -1 */
 
@@ -132,9 +140,11 @@ int gks_launch_unpack(const GksGrid &g, const double *Wpad, double *Wint, cudaSt
 int gks_launch_halo(const GksGrid &g, double *W, double *buf, int face, int unpack, cudaStream_t s);
 int gks_launch_unpack_faces(const GksGrid &g, int dir, const double *Fpad, double *Fout, cudaStream_t s);
 
-/* sweep of one direction: fills flux[dir] (F and dF; stage 2 needs only dF) */
+#ifdef GKS_DEBUG
+/* unfused cross-check sweep of one direction: fills flux[dir] (F and dF; stage 2 needs only dF) */
 int gks_launch_sweep_unfused(const GksGrid &g, const GksPhys &ph, int dir, const double *W, double *tmpN,
                              double *tmpT, double *flux, bool need_F, cudaStream_t s);
+#endif
 
 /* fused sweep (gks_sweep_fused.cu); which = 0 reads Wn, 1 reads Ws */
 bool gks_fused_init(gks_ctx *ctx);
@@ -157,6 +167,7 @@ int gks_launch_alm(const GksGrid &g, double *W, int n, const double *pos, const 
                    double dt, const int lo[3], const int cnt[3], cudaStream_t s);
 int gks_launch_cfl_dt(const GksGrid &g, const double *W, double cfl, double dmin, double cs, double *scratch,
                       cudaStream_t s);
+int gks_launch_shift_x(double *pos, int n, double shift, cudaStream_t s);
 int gks_launch_rotor_forces(const GksGrid &g, const double *W, const GksRotor &r, double time, double eps,
                             double *pos, double *force, cudaStream_t s);
 int gks_launch_check_finite(const GksGrid &g, const double *W, int *flag, cudaStream_t s);

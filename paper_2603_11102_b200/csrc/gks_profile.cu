@@ -1,7 +1,7 @@
 /*
  * gks_profile.cu — measurement helpers of the C ABI: per-kernel-class CUDA-event timing on the
- * context's stream and an fp64 FMA throughput calibration kernel (the denominator of the "alu"
- * roofline bench.py reports).
+ * context's stream and, in the GKS_DEBUG library only, an fp64 FMA throughput calibration kernel (context
+ * for the "alu" roofline bench.py reports).
  */
 #include <cstdlib>
 
@@ -29,6 +29,7 @@ void gks_prof_free(gks_ctx *ctx) {
   }
 }
 
+#ifdef GKS_DEBUG
 namespace {
 
 /* 8 independent DFMA chains per thread, all in registers */
@@ -45,6 +46,7 @@ __global__ void __launch_bounds__(256) k_dfma(double *out, int iters, double a, 
 }
 
 } /* namespace */
+#endif
 
 extern "C" {
 
@@ -78,6 +80,7 @@ gks_status gks_profile_read(gks_ctx *ctx, double *ms, long long *count) {
   return GKS_OK;
 }
 
+#ifdef GKS_DEBUG
 gks_status gks_debug_fp64_peak(gks_ctx *ctx, double *tflops) {
   if (!ctx || !tflops) return GKS_ERR_INVALID_ARG;
   cudaDeviceProp prop;
@@ -107,5 +110,6 @@ gks_status gks_debug_fp64_peak(gks_ctx *ctx, double *tflops) {
   *tflops = best;
   return GKS_OK;
 }
+#endif
 
 } /* extern "C" */

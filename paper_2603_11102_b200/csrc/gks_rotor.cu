@@ -140,6 +140,19 @@ __global__ void __launch_bounds__(128) k_rotor_forces(GksGrid g, const double *_
 
 } /* namespace */
 
+namespace {
+/* x -> x + shift for n points (pos[3 p]): the image of a rotor beyond the seam of a periodic x axis */
+__global__ void k_shift_x(double *pos, int n, double shift) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p < n) pos[3 * p] += shift;
+}
+} /* namespace */
+
+int gks_launch_shift_x(double *pos, int n, double shift, cudaStream_t s) {
+  k_shift_x<<<(n + 127) / 128, 128, 0, s>>>(pos, n, shift);
+  return 1;
+}
+
 int gks_launch_rotor_forces(const GksGrid &g, const double *W, const GksRotor &r, double time, double eps,
                             double *pos, double *force, cudaStream_t s) {
   const int n = r.nb * r.np;

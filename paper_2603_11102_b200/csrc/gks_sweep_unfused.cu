@@ -7,6 +7,7 @@
  * Intermediates live in HBM in the padded cell index space (gks_internal.h).
  * PAPER.md:68-89 (Eq. 6-8), Appendix :501-558; readings S1-S11.
  */
+#ifdef GKS_DEBUG   /* cross-check path: compiled into libgks_b200_debug.so only (include/gks_debug.h) */
 #include "gks_internal.h"
 #include "gks_math.cuh"
 
@@ -164,3 +165,5 @@ int gks_launch_sweep_unfused(const GksGrid &g, const GksPhys &ph, int dir, const
     default: return sweep_dir<2>(g, ph, W, tmpN, tmpT, flux, need_F, s);
   }
 }
+
+#endif /* GKS_DEBUG */

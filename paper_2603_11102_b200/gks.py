@@ -10,7 +10,8 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libgks_b200.so")
-_LIB = None
+_LIB_DEBUG_PATH = os.path.join(_HERE, "libgks_b200_debug.so")     # same sources with -DGKS_DEBUG (include/gks_debug.h)
+_LIBS = {}
 _dp = C.POINTER(C.c_double)
 
 GKS_OK = 0
@@ -20,8 +21,9 @@ STATUS = {0: "GKS_OK", 1: "GKS_ERR_INVALID_ARG", 2: "GKS_ERR_WORKSPACE", 3: "GKS
 EXPORTS = ["gks_workspace_bytes", "gks_create", "gks_destroy", "gks_set_state", "gks_get_state", "gks_step",
            "gks_set_body_force", "gks_set_bulk_flux", "alm_set_points", "ibm_set_points", "ibm_set_velocities", "ibm_set_iterations", "gks_cfl_dt", "alm_set_rotor", "alm_rotor_eval", "alm_rotor_points", "gks_set_reconstruction", "gks_halo_doubles", "gks_halo_pack", "gks_halo_unpack", "gks_step_begin",
            "gks_step_finish", "gks_step_force", "gks_bulk_partial", "gks_bulk_set_global", "gks_ibm_pass", "gks_ibm_residual",
-           "gks_debug_eval_flux", "gks_debug_set_sweep", "gks_debug_fp64_peak",
+           "gks_debug_eval_flux", "alm_rotor_supply",
            "gks_profile_enable", "gks_profile_read", "gks_check_finite", "gks_launch_count", "gks_last_error"]
+DEBUG_EXPORTS = ["gks_debug_set_sweep", "gks_debug_fp64_peak"]    # include/gks_debug.h: libgks_b200_debug.so only
 
 
 class AlmRotor(C.Structure):
@@ -47,14 +49,15 @@ class GksError(RuntimeError):
         self.status = status
 
 
-def lib():
-    """Load libgks_b200.so (built in-tree by paper_2603_11102_b200/build.py).  Fails loudly if absent."""
-    global _LIB
-    if _LIB is None:
-        if not os.path.exists(_LIB_PATH):
-            raise ImportError("libgks_b200.so is not built (run `python -m paper_2603_11102_b200.build`); "
-                              "there is no CPU fallback")
-        L = C.CDLL(_LIB_PATH)
+def lib(debug=False):
+    """Load libgks_b200.so - or, debug=True, libgks_b200_debug.so, the same sources with the test hooks of
+    include/gks_debug.h - built in-tree by paper_2603_11102_b200/build.py.  Fails loudly if absent."""
+    if debug not in _LIBS:
+        path = _LIB_DEBUG_PATH if debug else _LIB_PATH
+        if not os.path.exists(path):
+            raise ImportError("%s is not built (run `python -m paper_2603_11102_b200.build`); "
+                              "there is no CPU fallback" % os.path.basename(path))
+        L = C.CDLL(path)
         vp = C.c_void_p
         L.gks_workspace_bytes.argtypes = [C.POINTER(GksConfig)]
         L.gks_workspace_bytes.restype = C.c_size_t
@@ -86,17 +89,19 @@ def lib():
         L.gks_ibm_pass.argtypes = [vp, C.c_int, C.c_int]
         L.gks_ibm_residual.argtypes = [vp, C.c_int, vp, C.c_int]
         L.gks_debug_eval_flux.argtypes = [vp, C.c_int, vp, vp]
-        L.gks_debug_set_sweep.argtypes = [vp, C.c_int]
+        L.alm_rotor_supply.argtypes = [vp, vp, vp, C.c_double]
         L.gks_check_finite.argtypes = [vp]
         L.gks_profile_enable.argtypes = [vp, C.c_int]
         L.gks_profile_read.argtypes = [vp, _dp, C.POINTER(C.c_longlong)]
-        L.gks_debug_fp64_peak.argtypes = [vp, _dp]
+        if debug:
+            L.gks_debug_set_sweep.argtypes = [vp, C.c_int]
+            L.gks_debug_fp64_peak.argtypes = [vp, _dp]
         L.gks_launch_count.argtypes = [vp]
         L.gks_launch_count.restype = C.c_longlong
         L.gks_last_error.argtypes = [vp]
         L.gks_last_error.restype = C.c_char_p
-        _LIB = L
-    return _LIB
+        _LIBS[debug] = L
+    return _LIBS[debug]
 
 
 def make_config(cfg):
@@ -130,13 +135,15 @@ def _ptr(x):
 
 
 class Gks:
-    """One solver context on the current CUDA device.  `stream` is a torch.cuda.Stream (default: a new one)."""
+    """One solver context on `device`.  `stream` is a torch.cuda.Stream of that device (default: a new one).
+    debug=True binds libgks_b200_debug.so, which adds the hooks of include/gks_debug.h (and their workspace)."""
 
-    def __init__(self, cfg, stream=None, device="cuda:0"):
+    def __init__(self, cfg, stream=None, device="cuda:0", debug=False):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("no CUDA device: the gas-kinetic step has no CPU fallback")
-        L = lib()
+        L = lib(debug)
+        self._L, self.debug = L, bool(debug)
         self._torch = torch
         self._sync_back = False
         self.device = torch.device(device)
@@ -147,19 +154,22 @@ class Gks:
             h = C.c_void_p()
             st = L.gks_create(C.byref(c), None, 0, None, C.byref(h))
             raise GksError(st, L.gks_last_error(None).decode())
+        # the library works on the CURRENT device (SM count, kernel attributes, launches): every call below is made
+        # with this context's device current (`_c`)
         with torch.cuda.device(self.device):
             self.stream = stream if stream is not None else torch.cuda.Stream(device=self.device)
             self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
-        base = self.workspace.data_ptr()
-        aligned = (base + 255) // 256 * 256
-        self.workspace_bytes = nbytes
-        self._h = C.c_void_p()
-        st = L.gks_create(C.byref(c), C.c_void_p(aligned), nbytes, C.c_void_p(self.stream.cuda_stream),
-                          C.byref(self._h))
+            base = self.workspace.data_ptr()
+            aligned = (base + 255) // 256 * 256
+            self.workspace_bytes = nbytes
+            self._h = C.c_void_p()
+            st = L.gks_create(C.byref(c), C.c_void_p(aligned), nbytes, C.c_void_p(self.stream.cuda_stream),
+                              C.byref(self._h))
         if st != GKS_OK:
             self._h = None
             raise GksError(st, L.gks_last_error(None).decode())
         self.n_ibm = 0
+        self._rotor_n = 0
 
     # -- helpers
     def _p(self, x):
@@ -181,11 +191,18 @@ class Gks:
             self._sync_back = False
             self._torch.cuda.current_stream(self.device).wait_stream(self.stream)
         if st != GKS_OK:
-            raise GksError(st, lib().gks_last_error(self._h).decode())
+            raise GksError(st, self._L.gks_last_error(self._h).decode())
+
+    def _c(self, name, *args):
+        """call `name`(ctx, *args) of the C ABI with this context's device current, raise on a status other than OK"""
+        with self._torch.cuda.device(self.device):
+            st = getattr(self._L, name)(self._h, *args)
+        self._check(st)
 
     def close(self):
         if getattr(self, "_h", None):
-            lib().gks_destroy(self._h)
+            with self._torch.cuda.device(self.device):
+                self._L.gks_destroy(self._h)
             self._h = None
 
     def __del__(self):
@@ -206,7 +223,7 @@ class Gks:
     # -- the C ABI, same names
     def set_state(self, W):
         p, keep = self._p(W)
-        self._check(lib().gks_set_state(self._h, p))
+        self._c("gks_set_state", p)
         if isinstance(keep, np.ndarray):
             self.synchronize()      # pageable host source: be safe before the caller frees it
 
@@ -215,29 +232,29 @@ class Gks:
         if out is None:
             out = np.empty(self.shape)
         p, _ = self._p(out)
-        self._check(lib().gks_get_state(self._h, p))
+        self._c("gks_get_state", p)
         return out
 
     def step(self, dt):
-        self._check(lib().gks_step(self._h, float(dt)))
+        self._c("gks_step", float(dt))
 
     def set_body_force(self, gx, gy, gz):
-        self._check(lib().gks_set_body_force(self._h, gx, gy, gz))
+        self._c("gks_set_body_force", gx, gy, gz)
 
     def set_bulk_flux(self, axis, target):
-        self._check(lib().gks_set_bulk_flux(self._h, int(axis), float(target)))
+        self._c("gks_set_bulk_flux", int(axis), float(target))
 
     def alm_set_points(self, pos, force, eps):
         n = 0 if pos is None else (pos.shape[0] if hasattr(pos, "shape") else len(pos))
         pp, k1 = self._p(pos)
         pf, k2 = self._p(force)
-        self._check(lib().alm_set_points(self._h, n, pp, pf, float(eps)))
+        self._c("alm_set_points", n, pp, pf, float(eps))
 
     def ibm_set_points(self, pos, weights):
         n = 0 if pos is None else (pos.shape[0] if hasattr(pos, "shape") else len(pos))
         pp, k1 = self._p(pos)
         pw, k2 = self._p(weights)
-        self._check(lib().ibm_set_points(self._h, n, pp, pw))
+        self._c("ibm_set_points", n, pp, pw)
         self.n_ibm = n
 
     @staticmethod
@@ -255,11 +272,11 @@ class Gks:
     def alm_set_rotor(self, r):
         """r: workloads.Rotor (duck-typed) or None to clear; tables are copied by the library during the call"""
         if r is None:
-            self._check(lib().alm_set_rotor(self._h, None))
+            self._c("alm_set_rotor", None)
             self._rotor_n = 0
             return
         c, _keep = self._rotor_struct(r)
-        self._check(lib().alm_set_rotor(self._h, C.byref(c)))
+        self._c("alm_set_rotor", C.byref(c))
         self._rotor_n = r.nblades * r.npts
 
     def alm_rotor_points(self, r, t, pos=None, force=None):
@@ -269,114 +286,142 @@ class Gks:
         n = r.nblades * r.npts
         if pos is None:
             pos, force = np.empty((n, 3)), np.empty((n, 3))
-            self._check(lib().alm_rotor_points(self._h, C.byref(c), float(t), pos.ctypes.data, force.ctypes.data))
+            self._c("alm_rotor_points", C.byref(c), float(t), pos.ctypes.data, force.ctypes.data)
         else:
             assert pos.is_contiguous() and force.is_contiguous() and pos.numel() == 3 * n == force.numel()
-            self._check(lib().alm_rotor_points(self._h, C.byref(c), float(t), pos.data_ptr(), force.data_ptr()))
+            self._c("alm_rotor_points", C.byref(c), float(t), pos.data_ptr(), force.data_ptr())
         return pos, force
 
-    def alm_rotor_eval(self):
-        pos, force = np.empty((self._rotor_n, 3)), np.empty((self._rotor_n, 3))
-        self._check(lib().alm_rotor_eval(self._h, pos.ctypes.data, force.ctypes.data))
+    def alm_rotor_eval(self, pos=None, force=None):
+        """positions and forces of the rotor set with alm_set_rotor at the context's rotor clock, from the current
+        state: host numpy arrays (synchronises), or fills the given torch CUDA tensors asynchronously"""
+        n = self._rotor_n
+        if pos is None:
+            pos, force = np.empty((n, 3)), np.empty((n, 3))
+            self._c("alm_rotor_eval", pos.ctypes.data, force.ctypes.data)
+        else:
+            assert pos.is_contiguous() and force.is_contiguous() and pos.numel() == 3 * n == force.numel()
+            self._c("alm_rotor_eval", pos.data_ptr(), force.data_ptr())
         return pos, force
+
+    def alm_rotor_supply(self, pos, force, x_shift=0.0):
+        """sub-domain: this step's actuator points of the rotor set with alm_set_rotor (torch tensors, CUDA or CPU)"""
+        assert pos.is_contiguous() and force.is_contiguous() and pos.numel() == 3 * self._rotor_n == force.numel()
+        self._c("alm_rotor_supply", pos.data_ptr(), force.data_ptr(), float(x_shift))
 
     def step_begin(self, dt):
-        self._check(lib().gks_step_begin(self._h, float(dt)))
+        self._c("gks_step_begin", float(dt))
 
     def step_finish(self, dt):
-        self._check(lib().gks_step_finish(self._h, float(dt)))
+        self._c("gks_step_finish", float(dt))
 
     def step_force(self, dt):
-        self._check(lib().gks_step_force(self._h, float(dt)))
+        self._c("gks_step_force", float(dt))
 
     def ibm_pass(self, k, phase):
-        self._check(lib().gks_ibm_pass(self._h, int(k), int(phase)))
+        self._c("gks_ibm_pass", int(k), int(phase))
 
     def ibm_residual(self, k, tensor, set=False):
         """get / set the max slip recorded by pass k (1-element float64 torch tensor, CUDA or CPU)"""
-        self._check(lib().gks_ibm_residual(self._h, int(k), tensor.data_ptr(), 1 if set else 0))
+        self._c("gks_ibm_residual", int(k), tensor.data_ptr(), 1 if set else 0)
 
     def bulk_partial(self, out):
         """out: 1-element float64 torch tensor (CUDA or CPU) receiving this sub-domain's sum of m_axis |Omega|;
         returns the sub-domain's volume"""
         vol = C.c_double(0.0)
-        self._check(lib().gks_bulk_partial(self._h, out.data_ptr(), C.byref(vol)))
+        self._c("gks_bulk_partial", out.data_ptr(), C.byref(vol))
         return vol.value
 
     def bulk_set_global(self, total, volume):
-        self._check(lib().gks_bulk_set_global(self._h, total.data_ptr(), float(volume)))
+        self._c("gks_bulk_set_global", total.data_ptr(), float(volume))
 
     def halo_doubles(self, face):
-        return int(lib().gks_halo_doubles(self._h, int(face)))
+        return int(self._L.gks_halo_doubles(self._h, int(face)))
 
     def halo_pack(self, which, face, buf):
         """buf: torch tensor (CUDA or CPU, float64, contiguous) of halo_doubles(face) elements"""
         assert buf.is_contiguous() and buf.numel() == self.halo_doubles(face)
-        self._check(lib().gks_halo_pack(self._h, int(which), int(face), buf.data_ptr()))
+        self._c("gks_halo_pack", int(which), int(face), buf.data_ptr())
 
     def halo_unpack(self, which, face, buf):
         assert buf.is_contiguous() and buf.numel() == self.halo_doubles(face)
-        self._check(lib().gks_halo_unpack(self._h, int(which), int(face), buf.data_ptr()))
+        self._c("gks_halo_unpack", int(which), int(face), buf.data_ptr())
 
     def set_reconstruction(self, tangential_linear):
-        self._check(lib().gks_set_reconstruction(self._h, int(tangential_linear)))
+        self._c("gks_set_reconstruction", int(tangential_linear))
 
     def cfl_dt(self, cfl, out=None):
         """dt of PAPER.md:91 for the current state; out = a 1-element torch CUDA tensor keeps the call asynchronous"""
         if out is not None:
-            self._check(lib().gks_cfl_dt(self._h, float(cfl), out.data_ptr()))
+            self._c("gks_cfl_dt", float(cfl), out.data_ptr())
             return out
         host = np.zeros(1)
-        self._check(lib().gks_cfl_dt(self._h, float(cfl), host.ctypes.data))
+        self._c("gks_cfl_dt", float(cfl), host.ctypes.data)
         return float(host[0])
 
     def ibm_set_iterations(self, max_iter, tol=0.0):
-        self._check(lib().ibm_set_iterations(self._h, int(max_iter), float(tol)))
+        self._c("ibm_set_iterations", int(max_iter), float(tol))
 
     def ibm_set_velocities(self, vel):
         pv, k = self._p(vel)
-        self._check(lib().ibm_set_velocities(self._h, pv))
+        self._c("ibm_set_velocities", pv)
 
     def debug_eval_flux(self, d):
         F, dF = np.empty(self.face_shape(d)), np.empty(self.face_shape(d))
-        self._check(lib().gks_debug_eval_flux(self._h, d, F.ctypes.data, dF.ctypes.data))
+        self._c("gks_debug_eval_flux", d, F.ctypes.data, dF.ctypes.data)
         return F, dF
 
     def debug_set_sweep(self, mode):
-        """0 = fused production kernels, 1 = unfused cross-check kernels"""
-        self._check(lib().gks_debug_set_sweep(self._h, int(mode)))
+        """0 = fused production kernels, 1 = unfused cross-check kernels (debug library only: include/gks_debug.h)"""
+        if not self.debug:
+            raise RuntimeError("gks_debug_set_sweep is not part of libgks_b200.so: create the context with debug=True")
+        self._c("gks_debug_set_sweep", int(mode))
 
     PROF_NAMES = ("ghost", "sweep_x", "sweep_y", "sweep_z", "update", "forcing")
 
     def profile_enable(self, on=True):
-        self._check(lib().gks_profile_enable(self._h, int(on)))
+        self._c("gks_profile_enable", int(on))
 
     def profile_read(self):
         """{class: (milliseconds, intervals)} accumulated since the last read; synchronises"""
         ms = (C.c_double * 6)()
         cnt = (C.c_longlong * 6)()
-        self._check(lib().gks_profile_read(self._h, ms, cnt))
+        self._c("gks_profile_read", ms, cnt)
         return {n: (ms[i], cnt[i]) for i, n in enumerate(self.PROF_NAMES)}
 
     def debug_fp64_peak(self):
+        if not self.debug:
+            raise RuntimeError("gks_debug_fp64_peak is not part of libgks_b200.so: create the context with debug=True")
         v = C.c_double()
-        self._check(lib().gks_debug_fp64_peak(self._h, C.byref(v)))
+        self._c("gks_debug_fp64_peak", C.byref(v))
         return v.value
 
     def check_finite(self):
-        self._check(lib().gks_check_finite(self._h))
+        self._c("gks_check_finite")
 
     @property
     def launch_count(self):
-        return lib().gks_launch_count(self._h)
+        return self._L.gks_launch_count(self._h)
 
     def synchronize(self):
         self.stream.synchronize()
 
 
+def fp64_peak(device="cuda:0"):
+    """sustained fp64 FMA throughput [TFLOP/s] of `device`, measured by the debug library's calibration kernel on a
+    throw-away context (context for bench.py's roofline; the product library does not carry the kernel)"""
+    from .workloads import GridConfig
+    g = Gks(GridConfig(n=(8, 8, 8), spacing=(1.0, 1.0, 1.0)), device=device, debug=True)
+    try:
+        return g.debug_fp64_peak()
+    finally:
+        g.close()
+
+
 def run_workload(w, steps=None, sweep=None):
-    """Run a workloads.Workload through the C ABI; returns the final state (host numpy array)."""
-    g = Gks(w.cfg)
+    """Run a workloads.Workload through the C ABI; returns the final state (host numpy array).
+    sweep = 1 selects the unfused cross-check kernels (debug library)."""
+    g = Gks(w.cfg, debug=sweep is not None)
     if sweep is not None:
         g.debug_set_sweep(sweep)
     if w.bulk_flux is not None:

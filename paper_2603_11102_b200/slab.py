@@ -70,27 +70,39 @@ class SlabDecomposition:
     def gather(self, parts):
         return np.concatenate(parts, axis=-1)
 
-    def ibm_points(self, rank, pos, vol):
-        """Lagrangian points sub-domain `rank` must know: those inside it and those of a neighbour whose 3-point
-        support (1.5 cells) reaches across a cut.  On a periodic x axis the images beyond the seam are shifted by
-        the period so that they sit next to the slab."""
+    def ibm_select(self, rank, pos):
+        """(indices into the global point list, x shifts) of the Lagrangian points sub-domain `rank` must know:
+        those inside it and those of a neighbour whose 3-point support (1.5 cells) reaches across a cut.  On a
+        periodic x axis the images beyond the seam are shifted by the period so that they sit next to the slab.
+        Per-point data of the global list (volumes, velocities) are taken with the same indices."""
         i0, i1 = self.owned(rank)
         h, x0 = self.cfg.spacing[0], self.cfg.origin[0]
         lo, hi = self.neighbours(rank)
         a = x0 + i0 * h - (1.5 * h if lo is not None else 0.0)
         b = x0 + i1 * h + (1.5 * h if hi is not None else 0.0)
         L = self.cfg.n[0] * h
-        out_p, out_v = [], []
+        idx, shifts = [], []
         for shift in ((0.0, -L, L) if (self.periodic and self.world > 1) else (0.0,)):
             x = pos[:, 0] + shift
             m = (x >= a) & (x <= b)
             if shift != 0.0:                      # images only where they are NOT already inside the slab proper
                 m &= (x < x0 + i0 * h) | (x > x0 + i1 * h)
-            q = pos[m].copy()
-            q[:, 0] += shift
-            out_p.append(q)
-            out_v.append(vol[m])
-        return np.concatenate(out_p), np.concatenate(out_v)
+            k = np.nonzero(m)[0]
+            idx.append(k)
+            shifts.append(np.full(len(k), shift))
+        return np.concatenate(idx), np.concatenate(shifts)
+
+    def ibm_points(self, rank, pos, vol):
+        """(positions, volumes) of the Lagrangian points of `ibm_select(rank, pos)`"""
+        idx, shifts = self.ibm_select(rank, pos)
+        q = pos[idx].copy()
+        q[:, 0] += shifts
+        return q, vol[idx]
+
+    def ibm_velocities(self, rank, pos, vel):
+        """the velocities v_p of the same points, in the same order (gks `ibm_set_velocities`)"""
+        idx, _ = self.ibm_select(rank, pos)
+        return np.ascontiguousarray(np.asarray(vel, dtype=np.float64)[idx])
 
     def alm_points(self, rank, pos, force, eps):
         """Actuator points sub-domain `rank` must know: those whose Gaussian support (3 eps) reaches the cells it owns.
@@ -227,48 +239,45 @@ class DistTransport:
 
 
 class RotorDriver:
-    """The on-line actuator-line rotor on sub-domains: the disc x = hub_x lies in ONE slab (its owner), which
-    evaluates the blade-element forces of all points from the un-forced field (trilinear sampling reads the first
-    HALO ghost layer when the disc sits within half a cell of a cut); the (tiny) position and force arrays are
-    broadcast and every sub-domain spreads them onto the cells it owns."""
+    """The on-line actuator-line rotor on sub-domains: every sub-domain is given the rotor with `alm_set_rotor` and
+    keeps its clock in the library (advanced by dt in every `gks_step_force`); the disc x = hub_x lies in ONE slab
+    (its owner), which evaluates the blade-element forces of all points from the un-forced field with
+    `alm_rotor_eval` (trilinear sampling reads the first HALO ghost layer when the disc sits within half a cell of a
+    cut); the (tiny) position and force arrays are broadcast and handed to every sub-domain with `alm_rotor_supply`,
+    which spreads them onto the cells it owns."""
 
     def __init__(self, decomposition, rotor, device):
         import torch
-        self.d, self.r, self.t = decomposition, rotor, 0.0
+        self.d, self.r = decomposition, rotor
         i = int(np.floor((rotor.hub[0] - decomposition.cfg.origin[0]) / decomposition.cfg.spacing[0]))
         i = min(max(i, 0), decomposition.cfg.n[0] - 1)
         self.owner = int(np.searchsorted(decomposition.x_lo, i, side="right") - 1)
         n = rotor.nblades * rotor.npts
         self.pos = torch.zeros((n, 3), dtype=torch.float64, device=device)
         self.force = torch.zeros((n, 3), dtype=torch.float64, device=device)
+        if self.pos.is_cuda:
+            torch.cuda.synchronize()               # the fills ran on torch's stream, the solvers write on their own
+        self._attached = False
 
     def evaluate(self, transport, solvers, many):
         """between step_finish (+ exchange of the un-forced field) and step_force"""
+        sols = solvers if many else [solvers]
+        if not self._attached:                     # rotor description and clock (t = 0 now) live in every context
+            for s in sols:
+                s.alm_set_rotor(self.r)
+            self._attached = True
         if many:                                   # all sub-domains in this process: the owner's arrays are everyone's
-            solvers[self.owner].alm_rotor_points(self.r, self.t, self.pos, self.force)
+            solvers[self.owner].alm_rotor_eval(self.pos, self.force)
             solvers[self.owner].synchronize()
             targets = list(enumerate(solvers))
         else:
             if transport.rank == self.owner:
-                solvers.alm_rotor_points(self.r, self.t, self.pos, self.force)
+                solvers.alm_rotor_eval(self.pos, self.force)
             transport.broadcast(solvers, self.owner, [self.pos, self.force])
             targets = [(transport.rank, solvers)]
         for rank, s in targets:
             # the disc is a plane x = hub_x: beyond the seam of a periodic x axis a slab meets its image
-            shift = self.d.seam_shift(rank, self.r.hub[0], 3.0 * self.r.eps)
-            pos = self.pos
-            if shift != 0.0:
-                import contextlib
-                import torch
-                # on the solver's stream: ordered after the broadcast and before the library's copy, and the
-                # caching allocator reuses the block only behind that copy
-                with (torch.cuda.stream(s.stream) if self.pos.is_cuda else contextlib.nullcontext()):
-                    pos = self.pos.clone()
-                    pos[:, 0] += shift
-            s.alm_set_points(pos, self.force, self.r.eps)
-
-    def advance(self, dt):
-        self.t += dt
+            s.alm_rotor_supply(self.pos, self.force, self.d.seam_shift(rank, self.r.hub[0], 3.0 * self.r.eps))
 
 
 class BufferPool:
@@ -387,5 +396,3 @@ class SlabStepper:
         if ibm and ibm_passes > 1:
             self._ibm_passes(ibm_passes)
         self._each(lambda s: s.step_force(dt))
-        if rotor is not None:
-            rotor.advance(dt)

@@ -3,6 +3,7 @@ declares, and the host logic that needs no GPU (validation) answers as documente
 import ctypes as C
 import os
 import re
+import subprocess
 
 import numpy as np
 import pytest
@@ -12,13 +13,19 @@ from paper_2603_11102_b200 import gks, workloads as wl
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def declared_functions():
-    src = open(os.path.join(ROOT, "include", "gks.h")).read()
+def declared_functions(header="gks.h"):
+    src = open(os.path.join(ROOT, "include", header)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b((?:gks|alm|ibm)_[a-z0-9_]+)\s*\(", src)))
 
 
+def exported_functions(path):
+    out = subprocess.run(["nm", "-D", "--defined-only", path], capture_output=True, text=True, check=True).stdout
+    return sorted(ln.split()[-1] for ln in out.splitlines() if " T " in ln)
+
+
 def test_library_exports_every_declared_symbol():
+    """the product library exports include/gks.h and nothing else; the debug library adds include/gks_debug.h"""
     from paper_2603_11102_b200 import build
     build.build()
     L = C.CDLL(gks._LIB_PATH)
@@ -27,6 +34,24 @@ def test_library_exports_every_declared_symbol():
     for n in names:
         assert hasattr(L, n), n
     assert sorted(gks.EXPORTS) == names
+    assert exported_functions(gks._LIB_PATH) == names
+    dbg = declared_functions("gks_debug.h")
+    assert dbg == sorted(gks.DEBUG_EXPORTS) and len(dbg) >= 2
+    assert exported_functions(gks._LIB_DEBUG_PATH) == sorted(names + dbg)
+    for n in dbg:                           # the test hooks and their kernels do not ship in the product
+        assert not hasattr(L, n), n
+
+
+def test_product_workspace_does_not_carry_the_cross_check_buffers():
+    """gks_workspace_bytes of the product: 3 states + 3 x 8 flux fields = 36 padded fields (+ tables, point arrays);
+    the debug library adds the 32 fields of intermediates of the unfused sweep"""
+    w = wl.taylor_green(64)
+    c, keep = gks.make_config(w.cfg)
+    padded = 72 * 70 * 70 * 8
+    prod = gks.lib().gks_workspace_bytes(C.byref(c))
+    dbg = gks.lib(True).gks_workspace_bytes(C.byref(c))
+    assert 36 * padded <= prod <= 36 * padded + (12 << 20)
+    assert dbg - prod >= 32 * padded
 
 
 def test_workspace_bytes_and_validation_without_gpu():
@@ -35,7 +60,7 @@ def test_workspace_bytes_and_validation_without_gpu():
     c, keep = gks.make_config(w.cfg)
     nbytes = L.gks_workspace_bytes(C.byref(c))
     padded = 40 * 38 * 38              # pitch rounded up to 4
-    assert nbytes >= 68 * 8 * padded and nbytes % 256 == 0
+    assert nbytes >= 36 * 8 * padded and nbytes % 256 == 0
     c.nx = 5                           # too small for the 5-cell stencils and 3 ghost layers
     assert L.gks_workspace_bytes(C.byref(c)) == 0
     c.nx = 32

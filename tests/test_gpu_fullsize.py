@@ -162,3 +162,58 @@ def test_C5_turbine_512x256x256_sampled():
     boxes = [(116, 114, 86), (124, 114, 40), (122, 114, 0), (116, 114, 120), (300, 100, 100), (0, 120, 90),
              (484, 120, 90), (250, -14, 228)]
     check_samples(w, Wg, boxes, need=[("alm", "ibm"), ("ibm",), ("ibm",), ("alm",)])
+
+
+@pytest.mark.parametrize("name", ["C2", "C3"])
+def test_full_channel_and_cylinder_ten_steps(name):
+    """north_star's second bar (1e-9 after ten steps) at the stated sizes of configs 2 and 3, whole grid, cell for cell"""
+    from oracle import binding as ob
+    from paper_2603_11102_b200 import gks
+    w = wl.by_name(name)
+    Wg = gks.run_workload(w, steps=10)
+    o = ob.Oracle(w.cfg)
+    if w.bulk_flux is not None:
+        o.set_bulk_flux(*w.bulk_flux)
+    if w.ibm is not None:
+        o.ibm_set_points(*w.ibm)
+    o.set_state(w.W0)
+    for _ in range(10):
+        o.step(w.dt)
+    err = rel_linf(Wg, o.get_state())
+    o.close()
+    assert err <= 1e-9, err
+
+
+def test_C4_rotor_ten_steps_sampled():
+    """config 4 at 384x192x192, ten steps with the blades turning (`alm_set_points` re-issued every step on both
+    sides): the oracle runs a 144^3 sub-box that holds the whole rotor disc; its trusted core (64 cells from every
+    cut: 6 per step and a margin) is the 16^3 cells around the inner half of blade 0 in the rotor plane"""
+    from paper_2603_11102_b200 import gks
+    w = wl.by_name("C4")
+    Wg = gks.run_workload(w, steps=10)
+    lo, size = (24, 34, 26), (144, 144, 144)
+    for s in (0, 9):                                   # every actuator point acts inside the sub-box, at both ends of the run
+        p = w.alm(s)[0] / w.cfg.spacing[0]
+        assert all((p[:, a] > lo[a] + 8).all() and (p[:, a] < lo[a] + size[a] - 8).all() for a in range(3))
+        r0 = p[4:36]                                   # stations of blade 0 at 2.25 .. 17.75 cells from the hub: inside the core
+        assert all((r0[:, a] > lo[a] + 64).all() and (r0[:, a] < lo[a] + size[a] - 64).all() for a in range(3))
+    check_samples(w, Wg, [lo], size=size, need=[("alm",)], steps=10, tol=1e-9, margin=64)
+
+
+def test_C5_turbine_ten_steps_sampled():
+    """config 5 at 512x256x256, ten steps, rotor turning: a 152 x 152 x 172 sub-box standing on the ground (the slip wall
+    keeps its boundary condition, margin 0 there) that holds the rotor disc, the nacelle and the whole tower; trusted core
+    = 24 x 24 cells around the tower axis from the ground up to the nacelle (z < 108).  The cuts are 64 cells from the
+    core and more than 60 from the body: in ten steps their influence (6 cells per step) reaches neither, so the IBM
+    (which couples cells 3 apart through a Lagrangian point) cannot carry it further"""
+    from paper_2603_11102_b200 import gks
+    w = wl.by_name("C5")
+    Wg = gks.run_workload(w, steps=10)
+    lo, size = (60, 52, 0), (152, 152, 172)
+    q = w.ibm[0] / w.cfg.spacing[0]
+    for a in range(3):                                 # the whole body is further than 60 + 3 cells from every cut
+        assert (q[:, a] > lo[a] + (64 if lo[a] > 0 else 0)).all() and (q[:, a] < lo[a] + size[a] - 64).all()
+    for s in (0, 9):
+        p = w.alm(s)[0] / w.cfg.spacing[0]
+        assert all((p[:, a] > lo[a] + 8).all() and (p[:, a] < lo[a] + size[a] - 8).all() for a in range(3))
+    check_samples(w, Wg, [lo], size=size, need=[("alm", "ibm")], steps=10, tol=1e-9, margin=64)

@@ -54,7 +54,7 @@ def test_face_fluxes_match_the_oracle(d, sweep):
     o = ob.Oracle(w.cfg)
     o.set_state(w.W0)
     Fo, dFo = o.eval_flux(d)
-    g = gks.Gks(w.cfg)
+    g = gks.Gks(w.cfg, debug=True)
     g.debug_set_sweep(sweep)
     g.set_state(w.W0)
     Fg, dFg = g.debug_eval_flux(d)
@@ -322,7 +322,7 @@ def test_linear_tangential_variant_matches_the_oracle(sweep):
     cases = [(wl.by_name("C1"), 1, TOL1), (wl.by_name("C1"), 10, TOL10), (wl.by_name("C2", small=True), 3, 10 * TOL1),
              (wl.Workload("ragged", cfg, W0, wl.cfl_dt(cfg, W0), 3), 3, 10 * TOL1)]
     for w, steps, tol in cases:
-        o, g = ob.Oracle(w.cfg), gks.Gks(w.cfg)
+        o, g = ob.Oracle(w.cfg), gks.Gks(w.cfg, debug=True)
         g.debug_set_sweep(sweep)
         for s in (o, g):
             s.set_reconstruction(1)
@@ -379,6 +379,47 @@ def test_split_step_equals_gks_step_and_enforces_the_call_order():
             g.step_force(w.dt)
         g.close()
     assert rel_linf(res[1], res[0]) <= 1e-14
+
+
+def test_calls_inside_a_split_step_cannot_corrupt_it():
+    """between gks_step_begin and gks_step_force the predictor P and the flux buffers are live: gks_set_state and
+    gks_debug_eval_flux are refused (GKS_ERR_STATE), a diagnostic gks_get_state to HOST memory is allowed, reads W^n /
+    the un-forced W^{n+1} and leaves the step untouched; the three parts of a step must be given the same dt"""
+    from paper_2603_11102_b200 import gks
+    w = wl.by_name("C5", small=True)
+    ref = gks.Gks(w.cfg)
+    ref.ibm_set_points(*w.ibm)
+    ref.set_state(w.W0)
+    ref.alm_set_points(*w.alm(0))
+    ref.step(w.dt)
+    Wref = ref.get_state()
+    ref.close()
+    g = gks.Gks(w.cfg)
+    g.ibm_set_points(*w.ibm)
+    g.set_state(w.W0)
+    g.alm_set_points(*w.alm(0))
+    g.step_begin(w.dt)
+    for call in (lambda: g.set_state(w.W0), lambda: g.debug_eval_flux(0)):
+        with pytest.raises(gks.GksError) as e:
+            call()
+        assert e.value.status == 4
+    assert np.array_equal(g.get_state(), w.W0)                # W^n, staged through a buffer that is free here
+    with pytest.raises(gks.GksError) as e:
+        g.step_finish(w.dt * (1 + 1e-12))                     # a driver that recomputed dt between the halves
+    assert e.value.status == 1
+    g.step_finish(w.dt)
+    mid = g.get_state()                                       # the un-forced W^{n+1}
+    assert np.isfinite(mid).all() and rel_linf(mid, Wref) > 1e-9
+    with pytest.raises(gks.GksError):
+        g.set_state(w.W0)
+    with pytest.raises(gks.GksError) as e:
+        g.step_force(0.5 * w.dt)
+    assert e.value.status == 1
+    g.step_force(w.dt)
+    assert rel_linf(g.get_state(), Wref) <= 1e-14             # IBM atomics: order only
+    g.set_state(w.W0)                                         # idle again: everything is allowed
+    g.debug_eval_flux(1)
+    g.close()
 
 
 def test_two_contexts_on_their_own_streams_do_not_interfere():

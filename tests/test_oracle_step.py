@@ -600,7 +600,7 @@ def test_P17_corrections():
         assert f[rad < 0.2].min() > 0.99 and f[-1] < 0.2
     assert np.abs(f_ax - f_tan).max() > 1e-3
     # worked value: N = 3, lambda = 7, r = 0.9 R, phi from a uniform wind: f = 2/pi acos(exp(-g1 N (R-r)/(2 r sin phi)))
-    # with the constants the paper prints (tests/golden/paper_constants.txt, PAPER.md:392), axial and tangential
+    # with the constants the paper prints (tests/golden/paper_constants.txt, PAPER.md:394), axial and tangential
     gold = {}
     with open(os.path.join(os.path.dirname(__file__), "golden", "paper_constants.txt")) as f:
         for line in f:
