@@ -167,10 +167,9 @@ __device__ __forceinline__ void weno5_edges_v(const double (&q)[5][N], double ep
     /* 1/prod = r0 (1 + e + e^2 + ...), e = 1 - prod r0 ~ 2^-23: the cubic truncation is below 2^-66 */
     const double e = fma(-prod[n], r0[n], 1.0);
     const double t = fma(e, e, e);
-    const double rw = r0[n] * w12;
-    const double yr = (numr[n] * denl[n]) * rw, yl = (numl[n] * denr[n]) * rw;
-    vr[n] = fma(yr, t, q[2][n] + yr);
-    vl[n] = fma(yl, t, q[2][n] + yl);
+    const double rw = fma(r0[n], t, r0[n]) * w12;
+    vr[n] = fma(numr[n] * denl[n], rw, q[2][n]);
+    vl[n] = fma(numl[n] * denr[n], rw, q[2][n]);
   }
 }
 
@@ -223,10 +222,9 @@ __device__ __forceinline__ void weno5_gauss_v(const double (&q)[5][N], double ep
     /* 1/prod = r0 (1 + e + e^2 + ...), e = 1 - prod r0 ~ 2^-23: the cubic truncation is below 2^-66 */
     const double e = fma(-prod[n], r0[n], 1.0);
     const double t = fma(e, e, e);
-    const double rh = r0[n] * h;
-    const double yp = (nump[n] * denm[n]) * rh, ym = (numm[n] * denp[n]) * rh;
-    vp[n] = fma(yp, t, q[2][n] + yp);
-    vm[n] = fma(-ym, t, q[2][n] - ym);
+    const double rh = fma(r0[n], t, r0[n]) * h;
+    vp[n] = fma(nump[n] * denm[n], rh, q[2][n]);
+    vm[n] = fma(-(numm[n] * denp[n]), rh, q[2][n]);
     sp[n] = fma(e4, D4[n], fma(e3, D3[n], fma(e2, D2[n], e1 * D1[n])));
     sm[n] = fma(e1, D4[n], fma(e2, D3[n], fma(e3, D2[n], e4 * D1[n])));
   }
