@@ -392,38 +392,43 @@ __device__ __forceinline__ void collision(const double Ql[4], const double Qr[4]
   Q0[1 + DIR] += Ql[0] * xl - Qr[0] * xr; /* rho_l (Ul el + xl) + rho_r (Ur er - xr) */
 }
 
-/* Gauss-point flux in closed form.  dQ[s][c] = d_s Q0_c, s = x,y,z.  F and dF/dt of direction DIR. */
+/* Gauss-point flux in closed form.  dQ[s][c] = d_s Q0_c, s = x,y,z.  F and dF/dt of direction DIR.
+ * Written with w_si = d_s m_i - U_i d_s rho (= rho d_s U_i), so that only the reciprocal of rho that the
+ * velocities need is taken:  Q_t = -div F_Euler,
+ *   rho_t = -sum_s d_s m_s,   m_i,t = -sum_s U_s d_s m_i - U_i sum_s w_ss - RT d_i rho,
+ *   dF/dt = (dF_Euler/dQ) Q_t:  dF_0 = m_n,t,  dF_i = U_n m_i,t + U_i (m_n,t - U_n rho_t) (+ RT rho_t for i = n),
+ *   F_0 = m_n,  F_i = m_i U_n - (mu / rho)(w_ni + w_in) (+ rho RT for i = n);   n = DIR. */
 template <int DIR, bool NEED_F>
 __device__ __forceinline__ void gauss_point_flux(const double Q0[4], const double dQ[3][4], double RT,
                                                  double mu, double F[4], double dF[4]) {
   const double rho = Q0[0];
-  const double ir = fast_rcp(rho);
+  const double ir = fast_rcp3(rho);
   const double u[3] = {Q0[1] * ir, Q0[2] * ir, Q0[3] * ir};
-  /* Q_t = -sum_s d_s F_Euler^s:  rho_t = -sum_s d_s m_s ;
-     m_i,t = -sum_s (U_s d_s m_i + m_i d_s U_s) - RT d_i rho,  d_s U_s = (d_s m_s - U_s d_s rho)/rho */
-  double du[3][3]; /* du[s][i] = d_s U_i */
+  const double ud = u[DIR];
+  double wd[3]; /* w_ss */
 #pragma unroll
-  for (int s = 0; s < 3; ++s)
-#pragma unroll
-    for (int i = 0; i < 3; ++i) du[s][i] = (dQ[s][1 + i] - u[i] * dQ[s][0]) * ir;
-  const double divm = dQ[0][1] + dQ[1][2] + dQ[2][3];
-  const double divu = du[0][0] + du[1][1] + du[2][2];
-  const double rho_t = -divm;
+  for (int i = 0; i < 3; ++i) wd[i] = fma(-u[i], dQ[i][0], dQ[i][1 + i]);
+  const double trw = (wd[0] + wd[1]) + wd[2];
+  const double divm = (dQ[0][1] + dQ[1][2]) + dQ[2][3]; /* -rho_t */
   double m_t[3];
 #pragma unroll
   for (int i = 0; i < 3; ++i)
-    m_t[i] = -(u[0] * dQ[0][1 + i] + u[1] * dQ[1][1 + i] + u[2] * dQ[2][1 + i]) - Q0[1 + i] * divu -
-             RT * dQ[i][0];
-  const double ud = u[DIR];
+    m_t[i] = fma(-u[0], dQ[0][1 + i], fma(-u[1], dQ[1][1 + i], fma(-u[2], dQ[2][1 + i], fma(-u[i], trw, -RT * dQ[i][0]))));
+  const double k = fma(ud, divm, m_t[DIR]); /* m_n,t - U_n rho_t */
   dF[0] = m_t[DIR];
 #pragma unroll
-  for (int i = 0; i < 3; ++i) dF[1 + i] = ud * m_t[i] + u[i] * m_t[DIR] - u[i] * ud * rho_t;
-  dF[1 + DIR] += RT * rho_t;
+  for (int i = 0; i < 3; ++i) dF[1 + i] = fma(u[i], k, ud * m_t[i]);
+  dF[1 + DIR] = fma(-RT, divm, dF[1 + DIR]);
   if (NEED_F) {
+    const double mir = mu * ir;
     F[0] = Q0[1 + DIR];
 #pragma unroll
-    for (int i = 0; i < 3; ++i) F[1 + i] = Q0[1 + i] * ud - mu * (du[DIR][i] + du[i][DIR]);
-    F[1 + DIR] += rho * RT;
+    for (int i = 0; i < 3; ++i) {
+      const double wsum = i == DIR ? wd[DIR] + wd[DIR]
+                                   : fma(-u[i], dQ[DIR][0], dQ[DIR][1 + i]) + fma(-ud, dQ[i][0], dQ[i][1 + DIR]);
+      F[1 + i] = fma(-mir, wsum, Q0[1 + i] * ud);
+    }
+    F[1 + DIR] = fma(rho, RT, F[1 + DIR]);
   }
 }
 
