@@ -102,7 +102,7 @@ Layout make_layout(const gks_config *c) {
   L.off_tmpN = take(8 * L.FS);
   L.off_tmpT = take(24 * L.FS);
 #endif
-  /* per axis: xf (n+7), xc, w, inv_w, inv_hn (n+6 each) */
+  /* per axis: xf (n+7), xc, w, inv_w, inv_12hn (n+6 each) */
   L.coords_doubles = 0;
   const int n[3] = {c->nx, c->ny, c->nz};
   for (int a = 0; a < 3; ++a) L.coords_doubles += 5 * (size_t)(n[a] + 8);
@@ -283,12 +283,12 @@ gks_status gks_create(const gks_config *cfg, void *workspace, size_t workspace_b
            *ihn = &tab[o + 4 * len];
     build_axis(n[a], faces[a], x0[a], dx[a], g.periodic[a], xf, xc, w);
     for (int i = 0; i < n[a] + 2 * GKS_NG; ++i) iw[i] = 1.0 / w[i];
-    for (int i = 1; i < n[a] + 2 * GKS_NG; ++i) ihn[i] = 1.0 / (xc[i] - xc[i - 1]);
+    for (int i = 1; i < n[a] + 2 * GKS_NG; ++i) ihn[i] = 1.0 / (12.0 * (xc[i] - xc[i - 1]));
     g.xf[a] = ctx->coords + o;
     g.xc[a] = ctx->coords + o + len;
     g.w[a] = ctx->coords + o + 2 * len;
     g.inv_w[a] = ctx->coords + o + 3 * len;
-    g.inv_hn[a] = ctx->coords + o + 4 * len;
+    g.inv_12hn[a] = ctx->coords + o + 4 * len;
     ctx->h_xf[a] = (double *)malloc(3 * len * sizeof(double));
     ctx->h_xc[a] = ctx->h_xf[a] + len;
     ctx->h_w[a] = ctx->h_xf[a] + 2 * len;
@@ -306,7 +306,7 @@ gks_status gks_create(const gks_config *cfg, void *workspace, size_t workspace_b
   ph.mu = cfg->rho_ref * cfg->nu;
   ph.theta = sqrt(ph.lambda);
   ph.cx = 0.5 / sqrt(3.14159265358979323846 * ph.lambda);
-  ph.weno_eps = cfg->weno_eps > 0 ? cfg->weno_eps : 1e-6;
+  ph.weno_eps4 = 4.0 * (cfg->weno_eps > 0 ? cfg->weno_eps : 1e-6);
   for (int i = 0; i < 4; ++i) ph.inflow[i] = cfg->inflow[i];
   for (int i = 0; i < 6; ++i) ph.bc[i] = cfg->bc[i];
 

@@ -31,7 +31,7 @@ struct GksGrid {
   const double *xc[3];     /* centres -3 .. n+2 */
   const double *w[3];      /* widths */
   const double *inv_w[3];  /* 1/width */
-  const double *inv_hn[3]; /* 1/(xc[f]-xc[f-1]) for face f = -2 .. n+2, stored at f+3 */
+  const double *inv_12hn[3]; /* 1/(12 (xc[f]-xc[f-1])) for face f = -2 .. n+2, stored at f+3 (normal slope S5) */
   int uniform[3];
   double x0[3], dx[3];
   int periodic[3];
@@ -43,7 +43,7 @@ struct GksGrid {
 };
 
 struct GksPhys {
-  double RT, lambda, mu, weno_eps; /* mu = rho_ref*nu */
+  double RT, lambda, mu, weno_eps4; /* mu = rho_ref*nu; 4 x the WENO epsilon (the smoothness indicators are carried x 4) */
   double theta, cx;                /* sqrt(lambda), 1/(2 sqrt(pi lambda)): collision constants */
   double inflow[4];
   int bc[6];

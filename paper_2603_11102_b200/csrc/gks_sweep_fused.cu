@@ -179,7 +179,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
 
   const int tid = threadIdx.x;
   const int n2 = g.n[T::AXM];
-  const double eps = ph.weno_eps;
+  const double eps = ph.weno_eps4;   /* 4 x the WENO epsilon (gks_math.cuh) */
   /* This CTA's plane list, addressed by a private index v in [0, L1):
    *   v <  nfull*n2 : whole columns blockIdx.x + gridDim.x*w, w = v / n2 - all CTAs march neighbouring
    *                   columns through the same planes at the same time (halo slabs are shared in L2);
@@ -321,7 +321,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
       if (cn < TN) { /* right edge = face cn: Ql, and the slope at that face */
         const int fh = T::NA ? ct * HA + cn : cn * HA + ct;
         SA[QLo + fh * 4 + cc] = vr;
-        SA[DNo + fh * 4 + cc] = dn * g.inv_hn[DIR][min(n0 + cn, g.n[DIR]) + GKS_NG];
+        SA[DNo + fh * 4 + cc] = dn * g.inv_12hn[DIR][min(n0 + cn, g.n[DIR]) + GKS_NG];
       }
     };
     auto edges_of_one = [&](int item) {
@@ -332,7 +332,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
 #pragma unroll
       for (int k = 0; k < 5; ++k) q[k][0] = w[(k - 2) * sn];
       gksd::weno5_edges_v<1>(q, eps, vl, vr);
-      store(cn, ct, cc, vl[0], vr[0], gksd::normal_slope(q[1][0], q[2][0], q[3][0], q[4][0]));
+      store(cn, ct, cc, vl[0], vr[0], gksd::normal_slope12(q[1][0], q[2][0], q[3][0], q[4][0]));
     };
     constexpr int NXA = NITEM - NT;
     static_assert(NXA >= 0 && NXA <= NT / 2, "stage A: at most two items per thread, extras on half the CTA");
@@ -346,7 +346,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
 #pragma unroll
       for (int k = 0; k < 5; ++k) q[k][0] = w[(k - 2) * sn];
       gksd::weno5_edges_v<1>(q, eps, a_vl, a_vr);
-      a_dn = gksd::normal_slope(q[1][0], q[2][0], q[3][0], q[4][0]);
+      a_dn = gksd::normal_slope12(q[1][0], q[2][0], q[3][0], q[4][0]);
     } else if (okA) {
       if (xa_id < NXA) {
         double q[5][2], vl[2], vr[2];
@@ -361,7 +361,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
         gksd::weno5_edges_v<2>(q, eps, vl, vr);
 #pragma unroll
         for (int u = 0; u < 2; ++u)
-          store(cnv[u], ctv[u], ccv[u], vl[u], vr[u], gksd::normal_slope(q[1][u], q[2][u], q[3][u], q[4][u]));
+          store(cnv[u], ctv[u], ccv[u], vl[u], vr[u], gksd::normal_slope12(q[1][u], q[2][u], q[3][u], q[4][u]));
       } else {
         edges_of_one(tid);
       }

@@ -39,16 +39,16 @@ __global__ void __launch_bounds__(256) k_normal(GksGrid g, GksPhys ph, Box3 box,
   if (!thread_cell(box, p)) return;
   const long long id = g.idx(p[0], p[1], p[2]);
   const long long sn = g.st[DIR];
-  const double ihn = g.inv_hn[DIR][p[DIR] + GKS_NG];
+  const double ihn = g.inv_12hn[DIR][p[DIR] + GKS_NG];
   double Ql[4], Qr[4], Dn[4], Q0[4];
 #pragma unroll
   for (int c = 0; c < 4; ++c) {
     const double *w = W + c * g.FS + id;
     const double q0 = w[-3 * sn], q1 = w[-2 * sn], q2 = w[-sn], q3 = w[0], q4 = w[sn], q5 = w[2 * sn];
     double dummy;
-    gksd::weno5_edges(q0, q1, q2, q3, q4, ph.weno_eps, dummy, Ql[c]); /* right edge of cell f-1 */
-    gksd::weno5_edges(q1, q2, q3, q4, q5, ph.weno_eps, Qr[c], dummy); /* left edge of cell f */
-    Dn[c] = gksd::normal_slope(q1, q2, q3, q4) * ihn;
+    gksd::weno5_edges(q0, q1, q2, q3, q4, ph.weno_eps4, dummy, Ql[c]); /* right edge of cell f-1 */
+    gksd::weno5_edges(q1, q2, q3, q4, q5, ph.weno_eps4, Qr[c], dummy); /* left edge of cell f */
+    Dn[c] = gksd::normal_slope12(q1, q2, q3, q4) * ihn;
   }
   gksd::collision<DIR>(Ql, Qr, ph.lambda, Q0);
 #pragma unroll
@@ -72,7 +72,7 @@ __global__ void __launch_bounds__(256) k_pass1(GksGrid g, GksPhys ph, Box3 box, 
     const double *q = N + f * g.FS + id;
     const double q0 = q[-2 * s1], q1 = q[-s1], q2 = q[0], q3 = q[s1], q4 = q[2 * s1];
     double vm, vp;
-    gksd::weno5_gauss(q0, q1, q2, q3, q4, ph.weno_eps, vm, vp, ph.tang_linear != 0);
+    gksd::weno5_gauss(q0, q1, q2, q3, q4, ph.weno_eps4, vm, vp, ph.tang_linear != 0);
     T[(0 * 12 + f) * g.FS + id] = vm;
     T[(1 * 12 + f) * g.FS + id] = vp;
     if (f < 4) {
@@ -101,7 +101,7 @@ __global__ void __launch_bounds__(256) k_pass2(GksGrid g, GksPhys ph, Box3 box, 
     for (int f = 0; f < 12; ++f) {
       const double *q = T + (g1 * 12 + f) * g.FS + id;
       const double q0 = q[-2 * s2], q1 = q[-s2], q2 = q[0], q3 = q[s2], q4 = q[2 * s2];
-      gksd::weno5_gauss(q0, q1, q2, q3, q4, ph.weno_eps, v[f][0], v[f][1], ph.tang_linear != 0);
+      gksd::weno5_gauss(q0, q1, q2, q3, q4, ph.weno_eps4, v[f][0], v[f][1], ph.tang_linear != 0);
       if (f < 4) {
         gksd::quartic_slope_gauss(q0, q1, q2, q3, q4, d2[f][0], d2[f][1]);
         d2[f][0] *= iw;
