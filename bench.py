@@ -166,8 +166,6 @@ def time_workload(gks, wl, name, device, steps, warmup=3, variant="weno"):
     for _ in range(warmup):
         one()
     g.synchronize()
-    g.profile_enable(True)
-    g.profile_read()
     l0 = g.launch_count
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(g.stream)
@@ -176,13 +174,92 @@ def time_workload(gks, wl, name, device, steps, warmup=3, variant="weno"):
     e1.record(g.stream)
     g.synchronize()
     ms = e0.elapsed_time(e1)
-    prof = g.profile_read()
     launches = g.launch_count - l0
+    g.profile_enable(True)          # the breakdown by kernel class: a second pass (see main)
+    g.profile_read()
+    for _ in range(steps):
+        one()
+    prof = g.profile_read()
     g.check_finite()
     g.close()
     return {"workload": "%s %s %dx%dx%d" % (name, w.name, *w.cfg.n), "value": w.cfg.cells * steps / (ms * 1e-3) / 1e6,
             "unit": UNIT, "steps": steps, "ms_per_step": ms / steps, "gpu_launches_per_step": launches / steps,
             "kernel_ms_per_step": {c: v[0] / steps for c, v in prof.items()}}
+
+
+def run_slab_proxy(args, w, gks, device):
+    """One interior sub-domain of `w` cut into N x-slabs, stepped on this GPU exactly as a rank of
+    the slab driver steps it - halo pack / unpack kernels of W^n and W* included, device buffers - with its own
+    opposite face as the neighbour on either side (= a periodic box of nx/N cells through the HALO path).  What it
+    shows: the cost of the sub-domain shape (n+1 x-faces on tiles, fewer columns per sweep, the extra kernels)
+    against 1/N of the single-domain step; the transfer itself (2 x 3 planes per stage over NVLink) is not in it."""
+    import torch
+    from paper_2603_11102_b200 import slab
+    N = args.slab_proxy
+    dec = slab.SlabDecomposition(w.cfg, N)
+    r = N // 2
+    cfg = dec.local_cfg(r)
+    assert cfg.bc[0] == slab.BC_HALO and cfg.bc[1] == slab.BC_HALO, "the proxy wants an interior slab (N >= 3, or periodic x)"
+    g = gks.Gks(cfg, device=device)
+    g.set_state(dec.scatter(w.W0, r))
+    with torch.cuda.stream(g.stream):
+        b = [torch.empty(g.halo_doubles(f), dtype=torch.float64, device=device) for f in (0, 1)]
+    g.synchronize()
+
+    def exchange(which):
+        g.halo_pack(which, 0, b[0])
+        g.halo_pack(which, 1, b[1])
+        g.halo_unpack(which, 0, b[1])
+        g.halo_unpack(which, 1, b[0])
+
+    def step():
+        exchange(0)
+        g.step_begin(w.dt)
+        exchange(1)
+        g.step_finish(w.dt)
+        g.step_force(w.dt)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    g.synchronize()
+    l0 = g.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(g.stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(g.stream)
+    g.synchronize()
+    ms = e0.elapsed_time(e1) / args.steps
+    launches = (g.launch_count - l0) / args.steps
+    g.profile_enable(True)
+    g.profile_read()
+    for _ in range(args.steps):
+        step()
+    prof = g.profile_read()
+    g.check_finite()
+    g.close()
+    # the single-domain step of the same workload, same run
+    g1 = setup_solver(w, gks, device)
+    g1.set_state(w.W0)
+    for _ in range(3):
+        g1.step(w.dt)
+    g1.synchronize()
+    e0.record(g1.stream)
+    for _ in range(args.steps):
+        g1.step(w.dt)
+    e1.record(g1.stream)
+    g1.synchronize()
+    ms1 = e0.elapsed_time(e1) / args.steps
+    g1.close()
+    print(json.dumps({
+        "metric": METRIC, "value": cfg.cells / (ms * 1e-3) / 1e6, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "%s x-slab %d of %d: %dx%dx%d cells, HALO faces on both sides" % (args.workload, r, N, *cfg.n),
+                   "note": "one sub-domain on one GPU, its own opposite face as the neighbours; no transfer"},
+        "gpu_launches_per_step": launches,
+        "single_domain_ms_per_step": ms1,
+        "strong_scaling_proxy": {"ideal_ms": ms1 / N, "slab_ms": ms, "efficiency": (ms1 / N) / ms},
+        "kernel_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()}}), flush=True)
 
 
 def main():
@@ -201,6 +278,10 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ref-box", type=int, default=256,
                     help="--impl reference: cells per axis of the Taylor-Green box the oracle is timed on (256 = M0)")
+    ap.add_argument("--slab-proxy", type=int, default=0,
+                    help="time ONE interior x-slab of the workload cut into N slabs on this GPU: HALO faces on both sides,\n"
+                         "halo pack / unpack inside the step, the slab's own opposite face standing in for the neighbours\n"
+                         "(a strong-scaling proxy that needs no second GPU; prints its own JSON line)")
     ap.add_argument("--no-configs", action="store_true", help="skip the C1..C5 throughput block of the JSON line")
     ap.add_argument("--ibm-passes", type=int, default=1, help="IBM multi-direct-forcing passes per step (workloads with IBM)")
     ap.add_argument("--e2e-steps", type=int, default=3)
@@ -234,6 +315,8 @@ def main():
     barrier()
 
     w = wl.by_name(args.workload)
+    if args.slab_proxy > 1:
+        return run_slab_proxy(args, w, gks, device)
     slab_mode = args.decomp == "slab" and world > 1
     stepper = None
     if slab_mode:
@@ -287,9 +370,9 @@ def main():
     # context figure only (the headline fraction is against the nominal unit count): DFMA throughput of this GPU
     fp64_peak = gks.fp64_peak(device) if rank == 0 else None
 
-    # ---- timed region: exactly K steps, device-resident state, CUDA events on the solver's stream
-    g.profile_enable(True)
-    g.profile_read()
+    # ---- timed region: exactly K steps, device-resident state, CUDA events on the solver's stream.  The per-class
+    # event recorder is OFF here (its event records between the kernels would keep a kernel's launch from overlapping
+    # the tail of its predecessor); the per-class breakdown comes from a second, untimed pass below.
     l0 = g.launch_count
     sampler = ClockSampler(local_rank)
     barrier()
@@ -304,9 +387,14 @@ def main():
     clocks = sampler.stop()
     ms = e0.elapsed_time(e1)
     launches = g.launch_count - l0
+    g.check_finite()
+    # ---- per-class kernel times (CUDA events around every class of kernels), same number of steps, not timed as a whole
+    g.profile_enable(True)
+    g.profile_read()
+    for _ in range(args.steps):
+        one_step()
     prof = g.profile_read()
     g.profile_enable(False)
-    g.check_finite()
 
     # ---- end to end through the C ABI with HOST buffers (pinned): H2D + step + D2H every step
     Hin = torch.from_numpy(w.W0.copy()).pin_memory()

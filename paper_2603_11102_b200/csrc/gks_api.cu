@@ -19,6 +19,9 @@ char g_create_error[512] = "";
 
 } /* namespace */
 
+thread_local cudaStream_t gks_pdl_prev = nullptr;
+thread_local bool gks_pdl_scope = false;
+
 gks_status gks_set_err(gks_ctx *ctx, gks_status st, const char *fmt, ...) {
   char *dst = ctx ? ctx->err : g_create_error;
   va_list ap;

@@ -134,6 +134,7 @@ gks_status gks_step_begin(gks_ctx *ctx, double dt) {
   if (ctx->mid_step) return gks_set_err(ctx, GKS_ERR_STATE, "gks_step_begin inside an unfinished step");
   if (gks_status st = gks_check_device(ctx)) return st;
   ctx->step_dt = dt;
+  GksPdlScope pdl(!ctx->prof_on);
   const GksGrid &g = ctx->g;
   const GksPhys &ph = ctx->ph;
   cudaStream_t s = ctx->stream;
@@ -156,6 +157,7 @@ gks_status gks_step_finish(gks_ctx *ctx, double dt) {
   if (!(dt > 0) || !std::isfinite(dt)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "dt must be > 0");
   if (dt != ctx->step_dt) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "gks_step_finish: dt = %.17g differs from the dt = %.17g of gks_step_begin", dt, ctx->step_dt);
   if (gks_status st = gks_check_device(ctx)) return st;
+  GksPdlScope pdl(!ctx->prof_on);
   const GksGrid &g = ctx->g;
   const GksPhys &ph = ctx->ph;
   cudaStream_t s = ctx->stream;
@@ -178,6 +180,7 @@ gks_status gks_step_force(gks_ctx *ctx, double dt) {
   if (!(dt > 0) || !std::isfinite(dt)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "dt must be > 0");
   if (dt != ctx->step_dt) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "gks_step_force: dt = %.17g differs from the dt = %.17g of gks_step_begin", dt, ctx->step_dt);
   if (gks_status st = gks_check_device(ctx)) return st;
+  GksPdlScope pdl(!ctx->prof_on);
   const GksGrid &g = ctx->g;
   const GksPhys &ph = ctx->ph;
   cudaStream_t s = ctx->stream;
@@ -210,8 +213,10 @@ gks_status gks_step_force(gks_ctx *ctx, double dt) {
     /* multi-direct-forcing passes (Eq. 11-12): pass k interpolates from the un-forced field plus the IBM
        increments of the passes before it, in place; nothing else has touched the momentum yet (S12) */
     unsigned long long *res = reinterpret_cast<unsigned long long *>(ctx->red + GKS_RED_IBM_RES);
-    if (ctx->ibm_maxit > 1)
+    if (ctx->ibm_maxit > 1) {
       CUDA_TRY(ctx, cudaMemsetAsync(res, 0, GKS_IBM_MAX_PASSES * sizeof(unsigned long long), s));
+      gks_pdl_break();                /* the next kernel must not overtake the memset */
+    }
     for (int pass = 0; pass < ctx->ibm_maxit; ++pass) {
       ctx->launches += gks_launch_ibm_interp(g, ctx->Wn, ctx->n_ibm, ctx->ibm_pos, ctx->ibm_vol, ctx->ibm_vel,
                                              ctx->ibm_coef, pass, ctx->ibm_tol, res, s);

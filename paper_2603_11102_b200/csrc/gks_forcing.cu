@@ -17,6 +17,7 @@ constexpr int RED_BLOCKS = GKS_RED_BULK_SUM;
 /* ---- bulk momentum: deterministic two-level sum of m_axis * |Omega| over the interior ---- */
 __global__ void __launch_bounds__(256) k_bulk_partial(GksGrid g, const double *__restrict__ W, int axis,
                                                       double *__restrict__ red) {
+  gks_pdl_enter();
   __shared__ double sh[256];
   const long long N = (long long)g.n[0] * g.n[1] * g.n[2];
   const long long per = (N + RED_BLOCKS - 1) / RED_BLOCKS;
@@ -39,6 +40,7 @@ __global__ void __launch_bounds__(256) k_bulk_partial(GksGrid g, const double *_
 }
 
 __global__ void __launch_bounds__(256) k_bulk_final(double *__restrict__ red) {
+  gks_pdl_enter();
   __shared__ double sh[256];
   double acc = 0.0;
   for (int t = threadIdx.x; t < RED_BLOCKS; t += 256) acc += red[t];
@@ -53,6 +55,7 @@ __global__ void __launch_bounds__(256) k_bulk_final(double *__restrict__ red) {
 
 /* ---- CFL time step: |U|_max over the interior, then dt = CFL dmin / (|U|_max + sqrt(RT)) ---- */
 __global__ void __launch_bounds__(256) k_umax(GksGrid g, const double *__restrict__ W, unsigned long long *__restrict__ out) {
+  gks_pdl_enter();
   __shared__ double sh[256];
   const long long N = (long long)g.n[0] * g.n[1] * g.n[2];
   double acc = 0.0;
@@ -76,6 +79,7 @@ __global__ void __launch_bounds__(256) k_umax(GksGrid g, const double *__restric
 
 __global__ void k_cfl_final(const unsigned long long *__restrict__ umax_bits, double cfl, double dmin, double cs,
                             double *__restrict__ dt) {
+  gks_pdl_enter();
   *dt = cfl * dmin / (__longlong_as_double((long long)*umax_bits) + cs);
 }
 
@@ -83,6 +87,7 @@ __global__ void k_cfl_final(const unsigned long long *__restrict__ umax_bits, do
 __global__ void __launch_bounds__(256) k_uniform_force(GksGrid g, double *__restrict__ W, double dt, double gx,
                                                        double gy, double gz, int bulk_axis, double target,
                                                        double total_volume, const double *__restrict__ red) {
+  gks_pdl_enter();
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
   const int k = blockIdx.z;
@@ -152,6 +157,7 @@ __global__ void __launch_bounds__(128) k_ibm_interp(GksGrid g, const double *__r
                                                     const double *__restrict__ pos, const double *__restrict__ vol,
                                                     const double *__restrict__ vel, double *__restrict__ coef,
                                                     int pass, double tol, unsigned long long *__restrict__ res) {
+  gks_pdl_enter();
   const int p = blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= n) return;
   if (pass >= 2 && ibm_below_tol(res, pass - 1, tol)) return;
@@ -184,6 +190,7 @@ __global__ void __launch_bounds__(128) k_ibm_interp(GksGrid g, const double *__r
 __global__ void __launch_bounds__(128) k_ibm_spread(GksGrid g, double *__restrict__ W, int n,
                                                     const double *__restrict__ pos, const double *__restrict__ coef,
                                                     int pass, double tol, const unsigned long long *__restrict__ res) {
+  gks_pdl_enter();
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const int p = (int)(t / 27);
   if (p >= n) return;
@@ -212,6 +219,7 @@ constexpr int ALM_CHUNK = 256;
 __global__ void __launch_bounds__(128) k_alm(GksGrid g, double *__restrict__ W, int n, const double *__restrict__ pos,
                                              const double *__restrict__ force, double eps, double dt, int lo0,
                                              int lo1, int lo2, int c0, int c1, int c2) {
+  gks_pdl_enter();
   __shared__ double sp[ALM_CHUNK * 3], sf[ALM_CHUNK * 3];
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const long long total = (long long)c0 * c1 * c2;
@@ -282,37 +290,37 @@ __global__ void __launch_bounds__(128) k_alm(GksGrid g, double *__restrict__ W, 
 } /* namespace */
 
 int gks_launch_bulk_reduce(const GksGrid &g, const double *W, int axis, double *red, cudaStream_t s) {
-  k_bulk_partial<<<RED_BLOCKS, 256, 0, s>>>(g, W, axis, red);
-  k_bulk_final<<<1, 256, 0, s>>>(red);
+  gks_launch(k_bulk_partial, RED_BLOCKS, dim3(256), 0, s, g, W, axis, red);
+  gks_launch(k_bulk_final, dim3(1), dim3(256), 0, s, red);
   return 2;
 }
 
 int gks_launch_cfl_dt(const GksGrid &g, const double *W, double cfl, double dmin, double cs, double *scratch,
                       cudaStream_t s) {
   /* scratch[0]: bit pattern of |U|_max (zeroed by the caller), scratch[1]: dt */
-  k_umax<<<RED_BLOCKS, 256, 0, s>>>(g, W, reinterpret_cast<unsigned long long *>(scratch));
-  k_cfl_final<<<1, 1, 0, s>>>(reinterpret_cast<const unsigned long long *>(scratch), cfl, dmin, cs, scratch + 1);
+  gks_launch(k_umax, RED_BLOCKS, dim3(256), 0, s, g, W, reinterpret_cast<unsigned long long *>(scratch));
+  gks_launch(k_cfl_final, dim3(1), dim3(1), 0, s, reinterpret_cast<const unsigned long long *>(scratch), cfl, dmin, cs, scratch + 1);
   return 2;
 }
 
 int gks_launch_uniform_force(const GksGrid &g, double *W, double dt, const double gacc[3], int bulk_axis,
                              double bulk_target, double total_volume, const double *red, cudaStream_t s) {
   dim3 blk(64, 4), grid((g.n[0] + 63) / 64, (g.n[1] + 3) / 4, g.n[2]);
-  k_uniform_force<<<grid, blk, 0, s>>>(g, W, dt, gacc[0], gacc[1], gacc[2], bulk_axis, bulk_target, total_volume, red);
+  gks_launch(k_uniform_force, grid, blk, 0, s, g, W, dt, gacc[0], gacc[1], gacc[2], bulk_axis, bulk_target, total_volume, red);
   return 1;
 }
 
 int gks_launch_ibm_interp(const GksGrid &g, const double *W, int n, const double *pos, const double *vol,
                           const double *vel, double *coef, int pass, double tol, unsigned long long *res,
                           cudaStream_t s) {
-  k_ibm_interp<<<(n + 127) / 128, 128, 0, s>>>(g, W, n, pos, vol, vel, coef, pass, tol, res);
+  gks_launch(k_ibm_interp, dim3((n + 127) / 128), dim3(128), 0, s, g, W, n, pos, vol, vel, coef, pass, tol, res);
   return 1;
 }
 
 int gks_launch_ibm_spread(const GksGrid &g, double *W, int n, const double *pos, const double *coef, int pass,
                           double tol, const unsigned long long *res, cudaStream_t s) {
   const long long t = (long long)n * 27;
-  k_ibm_spread<<<(unsigned)((t + 127) / 128), 128, 0, s>>>(g, W, n, pos, coef, pass, tol, res);
+  gks_launch(k_ibm_spread, dim3((unsigned)((t + 127) / 128)), dim3(128), 0, s, g, W, n, pos, coef, pass, tol, res);
   return 1;
 }
 
@@ -320,7 +328,7 @@ int gks_launch_alm(const GksGrid &g, double *W, int n, const double *pos, const 
                    double dt, const int lo[3], const int cnt[3], cudaStream_t s) {
   const long long t = (long long)cnt[0] * cnt[1] * cnt[2];
   if (t <= 0) return 0;
-  k_alm<<<(unsigned)((t + 127) / 128), 128, 0, s>>>(g, W, n, pos, force, eps, dt, lo[0], lo[1], lo[2], cnt[0], cnt[1],
+  gks_launch(k_alm, dim3((unsigned)((t + 127) / 128)), dim3(128), 0, s, g, W, n, pos, force, eps, dt, lo[0], lo[1], lo[2], cnt[0], cnt[1],
                                                     cnt[2]);
   return 1;
 }

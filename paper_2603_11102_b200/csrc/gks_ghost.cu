@@ -15,15 +15,19 @@ namespace {
 
 enum { BC_PERIODIC = 0, BC_NOSLIP = 1, BC_SLIP = 2, BC_INFLOW = 3, BC_OUTFLOW = 4, BC_EXTRAP = 5, BC_HALO = 6 };
 
-/* AX = axis being filled; (u,v) run over the two other axes: u the lower one */
+/* AX = axis being filled; (u,v) run over the two other axes: u the lower one.  One thread fills the 3 ghosts of
+ * ONE component of one line end: its (at most 3) source values are all loaded before the first store, so a thread
+ * pays one memory latency, and the pass has four times as many threads to hide it (the ghost passes are pure
+ * latency: a few MB per pass). */
 template <int AX>
 __global__ void __launch_bounds__(128) k_ghost(GksGrid g, GksPhys ph, double *W,
                                                const double *Wstate /* may alias W */, int ulo, int ucnt, int vlo,
                                                int vcnt) {
+  gks_pdl_enter();
   constexpr int UA = AX == 0 ? 1 : 0, VA = AX == 2 ? 1 : 2;
   const int iu = blockIdx.x * blockDim.x + threadIdx.x;
   const int iv = blockIdx.y;
-  const int side = blockIdx.z;
+  const int side = blockIdx.z & 1, c = blockIdx.z >> 1;
   if (iu >= ucnt || iv >= vcnt) return;
   int p[3];
   p[UA] = ulo + iu;
@@ -35,45 +39,41 @@ __global__ void __launch_bounds__(128) k_ghost(GksGrid g, GksPhys ph, double *W,
   const int kind = ph.bc[2 * AX + side];
   if (kind == BC_HALO) return;   /* ghosts of a cut face come from the neighbouring sub-domain */
   const int first = side == 0 ? 0 : n - 1;
-
-  double qin[4] = {0, 0, 0, 0};
+  double *w = W + c * g.FS + base;
+  double q[GKS_NG];
   if (kind == BC_INFLOW) {
     const double sign = side == 0 ? -1.0 : 1.0;
     const double rhoI = W[base + first * sa];
     const double UnI = sign * W[(1 + AX) * g.FS + base + first * sa] / rhoI;
     const double Unb = sign * ph.inflow[1 + AX];
     const double rhob = rhoI * exp((UnI - Unb) / sqrt(ph.RT));
-    qin[0] = rhob;
-    qin[1] = rhob * ph.inflow[1];
-    qin[2] = rhob * ph.inflow[2];
-    qin[3] = rhob * ph.inflow[3];
-  }
+    const double qin = c == 0 ? rhob : rhob * ph.inflow[c];
 #pragma unroll
-  for (int gi = 1; gi <= GKS_NG; ++gi) {
-    const int ghost = side == 0 ? -gi : n - 1 + gi;
-    const int mirror = side == 0 ? gi - 1 : n - gi;
-    const int image = side == 0 ? n - gi : gi - 1;
+    for (int gi = 1; gi <= GKS_NG; ++gi) q[gi - 1] = qin;
+  } else {
 #pragma unroll
-    for (int c = 0; c < 4; ++c) {
-      double *w = W + c * g.FS + base;
-      double q;
+    for (int gi = 1; gi <= GKS_NG; ++gi) {
+      const int ghost = side == 0 ? -gi : n - 1 + gi;
+      const int mirror = side == 0 ? gi - 1 : n - gi;
+      const int image = side == 0 ? n - gi : gi - 1;
       switch (kind) {
-        case BC_PERIODIC: q = w[image * sa]; break;
-        case BC_NOSLIP: q = c == 0 ? w[mirror * sa] : -w[mirror * sa]; break;
-        case BC_SLIP: q = c == 1 + AX ? -w[mirror * sa] : w[mirror * sa]; break;
-        case BC_INFLOW: q = qin[c]; break;
-        case BC_OUTFLOW: q = Wstate[c * g.FS + base + ghost * sa]; break;
-        default: q = w[first * sa]; break;
+        case BC_PERIODIC: q[gi - 1] = w[image * sa]; break;
+        case BC_NOSLIP: q[gi - 1] = c == 0 ? w[mirror * sa] : -w[mirror * sa]; break;
+        case BC_SLIP: q[gi - 1] = c == 1 + AX ? -w[mirror * sa] : w[mirror * sa]; break;
+        case BC_OUTFLOW: q[gi - 1] = Wstate[c * g.FS + base + ghost * sa]; break;
+        default: q[gi - 1] = w[first * sa]; break;
       }
-      w[ghost * sa] = q;
     }
   }
+#pragma unroll
+  for (int gi = 1; gi <= GKS_NG; ++gi) w[(side == 0 ? -gi : n - 1 + gi) * sa] = q[gi - 1];
 }
 
 /* S20: initialise (dt < 0) or advance (dt >= 0) the convective-outflow ghost state of axis AX */
 template <int AX>
 __global__ void __launch_bounds__(128) k_outflow(GksGrid g, GksPhys ph, double *__restrict__ W, double dt, int ulo,
                                                  int ucnt, int vlo, int vcnt) {
+  gks_pdl_enter();
   constexpr int UA = AX == 0 ? 1 : 0, VA = AX == 2 ? 1 : 2;
   const int iu = blockIdx.x * blockDim.x + threadIdx.x;
   const int iv = blockIdx.y;
@@ -111,6 +111,7 @@ __global__ void __launch_bounds__(128) k_outflow(GksGrid g, GksPhys ph, double *
 template <int AX>
 __global__ void __launch_bounds__(128) k_halo(GksGrid g, double *__restrict__ W, double *__restrict__ buf, int side,
                                               int unpack) {
+  gks_pdl_enter();
   constexpr int UA = AX == 0 ? 1 : 0, VA = AX == 2 ? 1 : 2;
   const int iu = blockIdx.x * blockDim.x + threadIdx.x;
   const int iv = blockIdx.y;
@@ -129,6 +130,7 @@ __global__ void __launch_bounds__(128) k_halo(GksGrid g, double *__restrict__ W,
 
 __global__ void __launch_bounds__(256) k_pack(GksGrid g, double *__restrict__ Wint, double *__restrict__ Wpad,
                                               int to_padded, int ex, int ey, int ez) {
+  gks_pdl_enter();
   /* interior box (n + e) per axis; e = 1 along the sweep direction for face arrays */
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
@@ -148,6 +150,7 @@ __global__ void __launch_bounds__(256) k_pack(GksGrid g, double *__restrict__ Wi
 }
 
 __global__ void __launch_bounds__(256) k_check_finite(GksGrid g, const double *__restrict__ W, int *flag) {
+  gks_pdl_enter();
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
   const int k = blockIdx.z;
@@ -172,8 +175,8 @@ struct PassLines {
 template <int AX>
 void launch_ghost_axis(const GksGrid &g, const GksPhys &ph, double *W, const double *Wstate, cudaStream_t s) {
   const PassLines<AX> L(g);
-  dim3 grid((L.ucnt + 127) / 128, L.vcnt, 2);
-  k_ghost<AX><<<grid, 128, 0, s>>>(g, ph, W, Wstate, L.ulo, L.ucnt, L.vlo, L.vcnt);
+  dim3 grid((L.ucnt + 127) / 128, L.vcnt, 8);       /* z: (side, component) */
+  gks_launch(k_ghost<AX>, grid, dim3(128), 0, s, g, ph, W, Wstate, L.ulo, L.ucnt, L.vlo, L.vcnt);
 }
 
 static bool outflow_on(const GksPhys &ph, int ax) {
@@ -185,7 +188,7 @@ int launch_outflow_axis(const GksGrid &g, const GksPhys &ph, double *W, double d
   if (!outflow_on(ph, AX)) return 0;
   const PassLines<AX> L(g);
   dim3 grid((L.ucnt + 127) / 128, L.vcnt, 8);
-  k_outflow<AX><<<grid, 128, 0, s>>>(g, ph, W, dt, L.ulo, L.ucnt, L.vlo, L.vcnt);
+  gks_launch(k_outflow<AX>, grid, dim3(128), 0, s, g, ph, W, dt, L.ulo, L.ucnt, L.vlo, L.vcnt);
   return 1;
 }
 
@@ -223,12 +226,12 @@ int gks_launch_outflow_advance(const GksGrid &g, const GksPhys &ph, double *W, d
 static dim3 grid2d(int nx, int ny, int nz) { return dim3((nx + 63) / 64, (ny + 3) / 4, nz); }
 
 int gks_launch_pack(const GksGrid &g, const double *Wint, double *Wpad, cudaStream_t s) {
-  k_pack<<<grid2d(g.n[0], g.n[1], g.n[2]), dim3(64, 4), 0, s>>>(g, const_cast<double *>(Wint), Wpad, 1, 0, 0, 0);
+  gks_launch(k_pack, dim3(grid2d(g.n[0], g.n[1], g.n[2])), dim3(64, 4), 0, s, g, const_cast<double *>(Wint), Wpad, 1, 0, 0, 0);
   return 1;
 }
 
 int gks_launch_unpack(const GksGrid &g, const double *Wpad, double *Wint, cudaStream_t s) {
-  k_pack<<<grid2d(g.n[0], g.n[1], g.n[2]), dim3(64, 4), 0, s>>>(g, Wint, const_cast<double *>(Wpad), 0, 0, 0, 0);
+  gks_launch(k_pack, dim3(grid2d(g.n[0], g.n[1], g.n[2])), dim3(64, 4), 0, s, g, Wint, const_cast<double *>(Wpad), 0, 0, 0, 0);
   return 1;
 }
 
@@ -236,20 +239,20 @@ int gks_launch_halo(const GksGrid &g, double *W, double *buf, int face, int unpa
   const int ax = face >> 1, side = face & 1;
   const int ua = ax == 0 ? 1 : 0, va = ax == 2 ? 1 : 2;
   dim3 grid((g.n[ua] + 127) / 128, g.n[va], 4 * GKS_NG);
-  if (ax == 0) k_halo<0><<<grid, 128, 0, s>>>(g, W, buf, side, unpack);
-  else if (ax == 1) k_halo<1><<<grid, 128, 0, s>>>(g, W, buf, side, unpack);
-  else k_halo<2><<<grid, 128, 0, s>>>(g, W, buf, side, unpack);
+  if (ax == 0) gks_launch(k_halo<0>, grid, dim3(128), 0, s, g, W, buf, side, unpack);
+  else if (ax == 1) gks_launch(k_halo<1>, grid, dim3(128), 0, s, g, W, buf, side, unpack);
+  else gks_launch(k_halo<2>, grid, dim3(128), 0, s, g, W, buf, side, unpack);
   return 1;
 }
 
 int gks_launch_unpack_faces(const GksGrid &g, int dir, const double *Fpad, double *Fout, cudaStream_t s) {
   const int ex = dir == 0, ey = dir == 1, ez = dir == 2;
-  k_pack<<<grid2d(g.n[0] + ex, g.n[1] + ey, g.n[2] + ez), dim3(64, 4), 0, s>>>(
+  gks_launch(k_pack, dim3(grid2d(g.n[0] + ex, g.n[1] + ey, g.n[2] + ez)), dim3(64, 4), 0, s, 
       g, Fout, const_cast<double *>(Fpad), 0, ex, ey, ez);
   return 1;
 }
 
 int gks_launch_check_finite(const GksGrid &g, const double *W, int *flag, cudaStream_t s) {
-  k_check_finite<<<grid2d(g.n[0], g.n[1], g.n[2]), dim3(64, 4), 0, s>>>(g, W, flag);
+  gks_launch(k_check_finite, dim3(grid2d(g.n[0], g.n[1], g.n[2])), dim3(64, 4), 0, s, g, W, flag);
   return 1;
 }

@@ -125,6 +125,66 @@ void gks_prof_begin(gks_ctx *ctx, int cat);
 void gks_prof_end(gks_ctx *ctx);
 void gks_prof_free(gks_ctx *ctx);
 
+/* ---- programmatic dependent launch (PDL) ----
+ * Every kernel of the library starts with gks_pdl_enter(): it lets the NEXT kernel on the stream be launched at once
+ * (griddepcontrol.launch_dependents) and then waits until the PREVIOUS one has completed and its memory is visible
+ * (griddepcontrol.wait) before it touches global memory - so the launch latency and the prologue of a kernel (barrier
+ * set-up, index arithmetic) hide behind the tail of its predecessor while the data dependences of the stream stay what
+ * they were.  gks_launch() launches with the attribute that allows this where it is safe (below); GKS_NO_PDL=1 in the
+ * environment turns the attribute off (the device side is then a no-op).  Matters on small grids: a step is 14-18
+ * short kernels.  The persistent sweep releases its successor only at its end (gks_sweep_fused.cu). */
+#ifdef __CUDACC__
+#include <cstdlib>
+#include <cstring>
+#include <utility>
+__device__ __forceinline__ void gks_pdl_enter() {
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+inline bool gks_pdl_allowed() {
+  static const bool on = [] {
+    const char *e = getenv("GKS_NO_PDL");
+    return !(e && e[0] == '1');
+  }();
+  return on;
+}
+/* The attribute replaces the stream dependency on the previous KERNEL by the programmatic one; it does not order the
+ * launch against a memset / memcpy / event record enqueued in between (found on B200: a reduction kernel launched this
+ * way overtook the memset of its accumulator).  So it is used only where the library itself has just launched the
+ * previous operation of the stream and that operation was a kernel: inside gks_step_begin / _finish / _force
+ * (GksPdlScope), from the second kernel of the call on, and not across a memset (gks_pdl_break). */
+extern thread_local cudaStream_t gks_pdl_prev;   /* stream whose latest operation is a kernel of the current scope */
+extern thread_local bool gks_pdl_scope;
+inline void gks_pdl_break() { gks_pdl_prev = nullptr; }
+struct GksPdlScope {
+  explicit GksPdlScope(bool on) {
+    gks_pdl_scope = on && gks_pdl_allowed();
+    gks_pdl_prev = nullptr;
+  }
+  ~GksPdlScope() {
+    gks_pdl_scope = false;
+    gks_pdl_prev = nullptr;
+  }
+};
+template <typename... KArgs, typename... Args>
+inline cudaError_t gks_launch(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, Args &&...args) {
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof(cfg));
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = (gks_pdl_scope && s != nullptr && gks_pdl_prev == s) ? 1 : 0;
+  const cudaError_t e = cudaLaunchKernelEx(&cfg, kern, std::forward<Args>(args)...);
+  gks_pdl_prev = gks_pdl_scope ? s : nullptr;
+  return e;
+}
+#endif
+
 /* ---- host helpers shared by the API translation units ---- */
 gks_status gks_set_err(gks_ctx *ctx, gks_status st, const char *fmt, ...);
 gks_status gks_check_device(gks_ctx *ctx);   /* GKS_ERR_STATE unless the context's device is the current one */

@@ -34,6 +34,7 @@ namespace {
 
 /* 8 independent DFMA chains per thread, all in registers */
 __global__ void __launch_bounds__(256) k_dfma(double *out, int iters, double a, double b) {
+  gks_pdl_enter();
   double x0 = threadIdx.x * 1e-9, x1 = x0 + 1e-3, x2 = x0 + 2e-3, x3 = x0 + 3e-3, x4 = x0 + 4e-3, x5 = x0 + 5e-3,
          x6 = x0 + 6e-3, x7 = x0 + 7e-3;
 #pragma unroll 4

@@ -97,6 +97,7 @@ __device__ double tip_factor(int N, double R, double r, double sinphi, double ts
 __global__ void __launch_bounds__(128) k_rotor_forces(GksGrid g, const double *__restrict__ W, GksRotor R, double time,
                                                       double eps, double *__restrict__ pos,
                                                       double *__restrict__ force) {
+  gks_pdl_enter();
   const int p = blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= R.nb * R.np) return;
   const int b = p / R.np, k = p - b * R.np;
@@ -143,19 +144,20 @@ __global__ void __launch_bounds__(128) k_rotor_forces(GksGrid g, const double *_
 namespace {
 /* x -> x + shift for n points (pos[3 p]): the image of a rotor beyond the seam of a periodic x axis */
 __global__ void k_shift_x(double *pos, int n, double shift) {
+  gks_pdl_enter();
   const int p = blockIdx.x * blockDim.x + threadIdx.x;
   if (p < n) pos[3 * p] += shift;
 }
 } /* namespace */
 
 int gks_launch_shift_x(double *pos, int n, double shift, cudaStream_t s) {
-  k_shift_x<<<(n + 127) / 128, 128, 0, s>>>(pos, n, shift);
+  gks_launch(k_shift_x, dim3((n + 127) / 128), dim3(128), 0, s, pos, n, shift);
   return 1;
 }
 
 int gks_launch_rotor_forces(const GksGrid &g, const double *W, const GksRotor &r, double time, double eps,
                             double *pos, double *force, cudaStream_t s) {
   const int n = r.nb * r.np;
-  k_rotor_forces<<<(n + 127) / 128, 128, 0, s>>>(g, W, r, time, eps, pos, force);
+  gks_launch(k_rotor_forces, dim3((n + 127) / 128), dim3(128), 0, s, g, W, r, time, eps, pos, force);
   return 1;
 }

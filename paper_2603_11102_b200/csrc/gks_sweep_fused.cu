@@ -38,6 +38,9 @@
 #include "gks_internal.h"
 #include "gks_math.cuh"
 
+#ifndef GKS_MIN_PPC
+#define GKS_MIN_PPC 2   /* remainder columns: fewest output planes per CTA (idle SMs are free; measured on C1-C3) */
+#endif
 #ifndef GKS_E_WIDTH
 #define GKS_E_WIDTH 3   /* pass-2 evaluations written side by side: 2, 3 or 6 (measured: 3 is best for all three tile shapes) */
 #endif
@@ -240,6 +243,10 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
     mbar_init(&bar[2], T::NW);
     fence_barrier_init();
   }
+  /* everything above ran in the shadow of the previous kernel's tail; global memory from here on.  The next kernel
+     is released when this CTA is done (end of the kernel): released at the start, its CTAs would queue for the whole
+     sweep (measured: slower) */
+  asm volatile("griddepcontrol.wait;" ::: "memory");
   __syncthreads();
 
   auto issue = [&](const Cur &c, int j) {       /* request staged plane j (described by cursor c) */
@@ -605,9 +612,9 @@ int launch_dir(gks_ctx *ctx, const CUtensorMap &map, double *flux) {
   int grid = ctx->num_sms, nfull = ncols / grid;
   long long rem = (long long)(ncols - nfull * grid) * n2;      /* planes of the columns that do not fill a wave */
   long long PPC = (rem + grid - 1) / grid;
-  if (PPC < 8) PPC = 8;                                        /* a range shorter than 8 planes is not worth its priming */
+  if (PPC < GKS_MIN_PPC) PPC = GKS_MIN_PPC;                    /* shortest range worth its 4 priming planes */
   if (nfull == 0) grid = (int)((rem + PPC - 1) / PPC);
-  kern<<<grid, T::NT, T::SMEM_BYTES, ctx->stream>>>(map, g, ctx->ph, flux, ga, nfull, rem, PPC);
+  gks_launch(kern, grid, dim3(T::NT), T::SMEM_BYTES, ctx->stream, map, g, ctx->ph, flux, ga, nfull, rem, PPC);
   return 1;
 }
 

@@ -35,6 +35,7 @@ __device__ __forceinline__ bool thread_cell(const Box3 &b, int p[3]) {
 template <int DIR>
 __global__ void __launch_bounds__(256) k_normal(GksGrid g, GksPhys ph, Box3 box, const double *__restrict__ W,
                                                 double *__restrict__ N) {
+  gks_pdl_enter();
   int p[3];
   if (!thread_cell(box, p)) return;
   const long long id = g.idx(p[0], p[1], p[2]);
@@ -61,6 +62,7 @@ __global__ void __launch_bounds__(256) k_normal(GksGrid g, GksPhys ph, Box3 box,
 template <int DIR>
 __global__ void __launch_bounds__(256) k_pass1(GksGrid g, GksPhys ph, Box3 box, const double *__restrict__ N,
                                                double *__restrict__ T) {
+  gks_pdl_enter();
   int p[3];
   if (!thread_cell(box, p)) return;
   constexpr int T1 = Axes<DIR>::T1;
@@ -87,6 +89,7 @@ __global__ void __launch_bounds__(256) k_pass1(GksGrid g, GksPhys ph, Box3 box, 
 template <int DIR, bool NEED_F>
 __global__ void __launch_bounds__(256) k_pass2(GksGrid g, GksPhys ph, Box3 box, const double *__restrict__ T,
                                                double *__restrict__ flux) {
+  gks_pdl_enter();
   int p[3];
   if (!thread_cell(box, p)) return;
   constexpr int A = Axes<DIR>::A, T1 = Axes<DIR>::T1, T2 = Axes<DIR>::T2;

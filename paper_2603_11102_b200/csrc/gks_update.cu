@@ -16,6 +16,7 @@ __global__ void __launch_bounds__(256) k_update(GksGrid g, const double *__restr
                                                 const double *__restrict__ fx, const double *__restrict__ fy,
                                                 const double *__restrict__ fz, double dt,
                                                 double *__restrict__ out1, double *__restrict__ out2) {
+  gks_pdl_enter();
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
   const int k = blockIdx.z;
@@ -47,13 +48,13 @@ __global__ void __launch_bounds__(256) k_update(GksGrid g, const double *__restr
 int gks_launch_stage1(const GksGrid &g, const double *Wn, double *const flux[3], double dt, double *Ws,
                       double *Pbuf, cudaStream_t s) {
   dim3 blk(64, 4), grid((g.n[0] + 63) / 64, (g.n[1] + 3) / 4, g.n[2]);
-  k_update<true><<<grid, blk, 0, s>>>(g, Wn, flux[0], flux[1], flux[2], dt, Ws, Pbuf);
+  gks_launch(k_update<true>, grid, blk, 0, s, g, Wn, flux[0], flux[1], flux[2], dt, Ws, Pbuf);
   return 1;
 }
 
 int gks_launch_stage2(const GksGrid &g, const double *Pbuf, double *const flux[3], double dt, double *Wn,
                       cudaStream_t s) {
   dim3 blk(64, 4), grid((g.n[0] + 63) / 64, (g.n[1] + 3) / 4, g.n[2]);
-  k_update<false><<<grid, blk, 0, s>>>(g, Pbuf, flux[0], flux[1], flux[2], dt, Wn, nullptr);
+  gks_launch(k_update<false>, grid, blk, 0, s, g, Pbuf, flux[0], flux[1], flux[2], dt, Wn, nullptr);
   return 1;
 }
