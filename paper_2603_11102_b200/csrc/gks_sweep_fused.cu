@@ -571,7 +571,7 @@ typedef CUresult (*encode_fn_t)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, 
 #define GKS_TILE_YZ_A 32
 #endif
 #ifndef GKS_TILE_X_A
-#define GKS_TILE_X_A 8
+#define GKS_TILE_X_A 4
 #endif
 template <int DIR> struct Shape {
   static constexpr int TA = DIR == 0 ? GKS_TILE_X_A : GKS_TILE_YZ_A, TB = 128 / TA;

@@ -43,18 +43,21 @@ __global__ void __launch_bounds__(256) k_update(GksGrid g, const double *__restr
   }
 }
 
+/* 256 threads; 64 along x unless the (sub-)domain is narrower (an x-slab of 32 cells would idle half of them) */
+dim3 update_block(const GksGrid &g) { return g.n[0] > 32 ? dim3(64, 4) : dim3(32, 8); }
+
 } /* namespace */
 
 int gks_launch_stage1(const GksGrid &g, const double *Wn, double *const flux[3], double dt, double *Ws,
                       double *Pbuf, cudaStream_t s) {
-  dim3 blk(64, 4), grid((g.n[0] + 63) / 64, (g.n[1] + 3) / 4, g.n[2]);
+  const dim3 blk = update_block(g), grid((g.n[0] + blk.x - 1) / blk.x, (g.n[1] + blk.y - 1) / blk.y, g.n[2]);
   gks_launch(k_update<true>, grid, blk, 0, s, g, Wn, flux[0], flux[1], flux[2], dt, Ws, Pbuf);
   return 1;
 }
 
 int gks_launch_stage2(const GksGrid &g, const double *Pbuf, double *const flux[3], double dt, double *Wn,
                       cudaStream_t s) {
-  dim3 blk(64, 4), grid((g.n[0] + 63) / 64, (g.n[1] + 3) / 4, g.n[2]);
+  const dim3 blk = update_block(g), grid((g.n[0] + blk.x - 1) / blk.x, (g.n[1] + blk.y - 1) / blk.y, g.n[2]);
   gks_launch(k_update<false>, grid, blk, 0, s, g, Pbuf, flux[0], flux[1], flux[2], dt, Wn, nullptr);
   return 1;
 }
