@@ -24,6 +24,20 @@ gks_status gks_debug_set_sweep(gks_ctx *ctx, int mode);
  * register-resident DFMA kernel on the context's stream (about 50 ms).  Synchronises. */
 gks_status gks_debug_fp64_peak(gks_ctx *ctx, double *tflops);
 
+/* Issue-rate probe (profiles/r2_microbench.md): clock cycles per round and warp of a loop that issues, per round and
+ * warp, KF DFMA on `chains` independent register chains and KI integer multiply-adds on 8 independent ones, with 512
+ * threads per CTA and one CTA per SM (4 warps per scheduler, as the fused sweep runs).  cycles[] receives
+ * GKS_DEBUG_PROBE_N numbers, for (KF, KI, chains) = (8,0,8) (8,4,8) (8,8,8) (8,12,8) (8,16,8) (4,8,8) (8,0,1) (8,0,2)
+ * (8,0,4).  Synchronises. */
+#define GKS_DEBUG_PROBE_N 9
+gks_status gks_debug_issue_probe(gks_ctx *ctx, double *cycles, int n);
+
+/* Phase timeline of the fused sweep: ticks[32][8] = for every warp of CTA 0 of the LAST sweep launch the clock64 ticks
+ * spent in the phases 0 loop bookkeeping, 1 hand-over wait, 2 TMA issue + cursor, 3 stage A, 4 stages BC + D + arrival,
+ * 5 pass 2 (E), 6 transposes + flux + store (F).  Only a library built with -DGKS_TRACE records them
+ * (`python -m paper_2603_11102_b200.trace`); any other returns GKS_ERR_STATE.  Synchronises. */
+gks_status gks_debug_trace(gks_ctx *ctx, unsigned long long *ticks);
+
 #ifdef __cplusplus
 }
 #endif

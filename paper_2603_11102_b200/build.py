@@ -19,7 +19,7 @@ NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
          "-Xcompiler", "-fPIC", "-ccbin", "/usr/bin/g++"]
 # translation units that do not look at GKS_DEBUG: one object serves both libraries
-SHARED_OBJECTS = ("gks_sweep_fused", "gks_update", "gks_ghost", "gks_forcing", "gks_rotor")
+SHARED_OBJECTS = ("gks_update", "gks_ghost", "gks_forcing", "gks_rotor")
 
 
 def _newer(target, deps):
@@ -72,6 +72,29 @@ def build(force=False, verbose=False, extra_flags=()):
             _run([NVCC, "-shared", "-o", lib] + lobjs + ["-gencode", "arch=compute_100a,code=sm_100a",
                                                          "-ccbin", "/usr/bin/g++", "-Xlinker", "--version-script=" + vs])
     return LIB
+
+
+def build_trace():
+    """libgks_b200_trace.so: the debug library with -DGKS_TRACE (phase timers in the fused sweep, include/gks_debug.h
+    gks_debug_trace).  Built on demand by paper_2603_11102_b200/trace.py; not a product artefact."""
+    lib = os.path.join(HERE, "libgks_b200_trace.so")
+    srcs = sorted(glob.glob(os.path.join(CSRC, "*.cu")))
+    hdrs = glob.glob(os.path.join(CSRC, "*.h")) + glob.glob(os.path.join(CSRC, "*.cuh")) + \
+        glob.glob(os.path.join(HERE, "..", "include", "*.h"))
+    objdir = os.path.join(HERE, "build", "trace")
+    os.makedirs(objdir, exist_ok=True)
+    jobs, objs = [], []
+    for s in srcs:
+        o = os.path.join(objdir, os.path.basename(s)[:-3] + ".o")
+        objs.append(o)
+        if _newer(o, [s] + hdrs):
+            jobs.append([NVCC] + FLAGS + ["-DGKS_DEBUG", "-DGKS_TRACE", "-c", s, "-o", o])
+    with ThreadPoolExecutor(max_workers=8) as ex:
+        list(ex.map(_run, jobs))
+    if jobs or _newer(lib, objs):
+        _run([NVCC, "-shared", "-o", lib] + objs + ["-gencode", "arch=compute_100a,code=sm_100a", "-ccbin", "/usr/bin/g++",
+                                                    "-Xlinker", "--version-script=" + os.path.join(CSRC, "gks_exports.map")])
+    return lib
 
 
 if __name__ == "__main__":

@@ -46,6 +46,50 @@ __global__ void __launch_bounds__(256) k_dfma(double *out, int iters, double a, 
   if (s == 12345.678) out[0] = s; /* never true: keeps the chains alive */
 }
 
+/* Issue-rate probe: per round KF DFMA on 8 independent register chains plus KI integer multiply-adds on 8 more, per
+ * warp; 512 threads per CTA, one CTA per SM (4 warps per scheduler, as the fused sweep runs).  Answers: does an
+ * instruction of another pipe cost the fp64 pipe an issue slot?  (DESIGN.md section 7.) */
+template <int KF, int KI, int CHAINS>
+__global__ void __launch_bounds__(512, 1) k_probe(double *out, int iters, double a, double b, int ia) {
+  double x[8];
+  int y[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    x[i] = threadIdx.x * 1e-9 + i;
+    y[i] = threadIdx.x + i;
+  }
+  const long long t0 = clock64();
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+#pragma unroll
+      for (int j = 0; j < KF; ++j) x[(r + j) % CHAINS] = fma(x[(r + j) % CHAINS], a, b);
+#pragma unroll
+      for (int j = 0; j < KI; ++j) y[(r + j) & 7] = y[(r + j) & 7] * ia + 7;
+    }
+  }
+  const long long t1 = clock64();
+  double s = 0;
+  int q = 0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    s += x[i];
+    q += y[i];
+  }
+  if (ia == 0x7fffffff) out[2 + threadIdx.x] = s + q; /* never true at run time: keeps the chains alive */
+  if (threadIdx.x == 0 && blockIdx.x == 0) out[1] = (double)(t1 - t0) / iters / 8;
+}
+
+template <int KF, int KI, int CHAINS>
+double run_probe(gks_ctx *ctx, int nsm) {
+  k_probe<KF, KI, CHAINS><<<nsm, 512, 0, ctx->stream>>>(ctx->red, 2000, 0.999999, 1e-7, 3);
+  double h[2] = {0, 0};
+  cudaMemcpyAsync(h, ctx->red, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream);
+  cudaStreamSynchronize(ctx->stream);
+  ctx->launches += 1;
+  return h[1];
+}
+
 } /* namespace */
 #endif
 
@@ -109,6 +153,27 @@ gks_status gks_debug_fp64_peak(gks_ctx *ctx, double *tflops) {
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return gks_set_err(ctx, GKS_ERR_CUDA, "fp64 peak: %s", cudaGetErrorString(e));
   *tflops = best;
+  return GKS_OK;
+}
+
+gks_status gks_debug_issue_probe(gks_ctx *ctx, double *cycles, int n) {
+  if (!ctx || !cycles || n < GKS_DEBUG_PROBE_N) return GKS_ERR_INVALID_ARG;
+  int dev = 0, nsm = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  int k = 0;
+  /* (KF, KI, chains): see include/gks_debug.h for the order */
+  cycles[k++] = run_probe<8, 0, 8>(ctx, nsm);
+  cycles[k++] = run_probe<8, 4, 8>(ctx, nsm);
+  cycles[k++] = run_probe<8, 8, 8>(ctx, nsm);
+  cycles[k++] = run_probe<8, 12, 8>(ctx, nsm);
+  cycles[k++] = run_probe<8, 16, 8>(ctx, nsm);
+  cycles[k++] = run_probe<4, 8, 8>(ctx, nsm);
+  cycles[k++] = run_probe<8, 0, 1>(ctx, nsm);
+  cycles[k++] = run_probe<8, 0, 2>(ctx, nsm);
+  cycles[k++] = run_probe<8, 0, 4>(ctx, nsm);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return gks_set_err(ctx, GKS_ERR_CUDA, "issue probe: %s", cudaGetErrorString(e));
   return GKS_OK;
 }
 #endif

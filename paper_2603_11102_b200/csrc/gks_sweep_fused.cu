@@ -45,6 +45,19 @@
 #define GKS_E_WIDTH 3   /* pass-2 evaluations written side by side: 2, 3 or 6 (measured: 3 is best for all three tile shapes) */
 #endif
 
+/* Phase timeline (build with -DGKS_TRACE, `python -m paper_2603_11102_b200.trace`): every warp of CTA 0 accumulates the
+ * clock64 ticks it spends in each phase of the plane loop; gks_debug_trace reads them back.  Off in the product. */
+#ifdef GKS_TRACE
+__device__ unsigned long long gks_trace_buf[32 * 8];   /* [warp][phase] */
+#define TR_DECL unsigned long long tr_[8] = {0, 0, 0, 0, 0, 0, 0, 0}; long long tr_t = clock64();
+#define TR(k) { const long long n_ = clock64(); tr_[k] += n_ - tr_t; tr_t = n_; }
+#define TR_DUMP if (blockIdx.x == 0 && (threadIdx.x & 31) == 0) { for (int q_ = 0; q_ < 8; ++q_) gks_trace_buf[(threadIdx.x >> 5) * 8 + q_] = tr_[q_]; }
+#else
+#define TR_DECL
+#define TR(k)
+#define TR_DUMP
+#endif
+
 namespace {
 
 #ifndef GKS_FUSE_BCD
@@ -286,17 +299,21 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
   gksd::series_coefficients((tid & 3) >> 1, bcf);
   constexpr int QLo = 0, QRo = FH * 4 + 2, DNo = 2 * FH * 4 + 4;   /* offsets inside a stage buffer */
 
+  TR_DECL
   for (int i = 0; i < J + 2; ++i) {
+    TR(0)   /* loop bookkeeping between two iterations */
     /* ONE hand-over per iteration: phase i-1 of the iteration barrier completes when every warp has finished
        A, BC, D of iteration i-1 AND the slab of plane i has landed - its TMA was issued at the top of iteration
        i-1, inside that phase, with its bytes expected on the same barrier (thread 0 arrives after it has issued,
        so the phase cannot complete before the expectation is registered).  Plane 0 has a barrier of its own. */
     if (i > 0) mbar_wait(&bar[2], (i - 1) & 1);
     else mbar_wait(&bar[0], 0);
+    TR(1)   /* hand-over wait */
     if (i + 1 < J) {
       if (tid == 0) issue(cT, i + 1);             /* slab (i+1)&1 was last read by stage A of iteration i-1 */
       cur_next(cT);
     }
+    TR(2)   /* TMA issue + cursor */
 
     /* ================= stage A: plane i =================
      * both WENO5 edge values of each cell, per component (one smoothness-indicator set serves the face on
@@ -375,6 +392,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
       cur_next(cA);
     }
 
+    TR(3)   /* stage A */
     /* ================= stages BC (plane i-1) and D (plane i-2) =================
      * BC, collision (S4): the 4 lanes of a halo face split the four half-Maxwellian factors (left / right side,
      * erf / exp series), exchange them by shuffle, and every lane forms its component of Q0 in place of QL.
@@ -467,6 +485,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
     /* this warp is done with the shared stage buffers of iteration i */
     __syncwarp();
     if ((tid & 31) == 0) mbar_arrive(&bar[2]);
+    TR(4)   /* stages BC + D, arrival */
     if (!have) continue;
 
     /* ================= stage EF: plane i-2 ================= */
@@ -514,6 +533,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
       }
     }
     __syncwarp();
+    TR(5)   /* pass 2 (E) */
     /* ---- F: flux at Gauss point gp = c of this face; sum over the 4 lanes; write ---- */
     {
       double Q0[4], dQ[3][4], F[4], dF[4];
@@ -554,7 +574,9 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
         flux[(4 + c) * g.FS + id] = 0.25 * dsel;
       }
     }
+    TR(6)   /* transposes, flux, face average, store (F) */
   }
+  TR_DUMP
 }
 
 } /* namespace */
@@ -619,6 +641,20 @@ int launch_dir(gks_ctx *ctx, const CUtensorMap &map, double *flux) {
 }
 
 } /* namespace */
+
+#ifdef GKS_DEBUG
+extern "C" gks_status gks_debug_trace(gks_ctx *ctx, unsigned long long *ticks) {
+  if (!ctx || !ticks) return GKS_ERR_INVALID_ARG;
+#ifdef GKS_TRACE
+  cudaError_t e = cudaStreamSynchronize(ctx->stream);
+  if (e == cudaSuccess) e = cudaMemcpyFromSymbol(ticks, gks_trace_buf, sizeof(gks_trace_buf));
+  if (e != cudaSuccess) return gks_set_err(ctx, GKS_ERR_CUDA, "trace read-back: %s", cudaGetErrorString(e));
+  return GKS_OK;
+#else
+  return gks_set_err(ctx, GKS_ERR_STATE, "this library was built without -DGKS_TRACE (python -m paper_2603_11102_b200.trace builds one)");
+#endif
+}
+#endif
 
 bool gks_fused_init(gks_ctx *ctx) {
   void *fn = nullptr;

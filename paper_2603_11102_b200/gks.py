@@ -23,7 +23,7 @@ EXPORTS = ["gks_workspace_bytes", "gks_create", "gks_destroy", "gks_set_state", 
            "gks_step_finish", "gks_step_force", "gks_bulk_partial", "gks_bulk_set_global", "gks_ibm_pass", "gks_ibm_residual",
            "gks_debug_eval_flux", "alm_rotor_supply",
            "gks_profile_enable", "gks_profile_read", "gks_check_finite", "gks_launch_count", "gks_last_error"]
-DEBUG_EXPORTS = ["gks_debug_set_sweep", "gks_debug_fp64_peak"]    # include/gks_debug.h: libgks_b200_debug.so only
+DEBUG_EXPORTS = ["gks_debug_set_sweep", "gks_debug_fp64_peak", "gks_debug_issue_probe", "gks_debug_trace"]    # include/gks_debug.h: libgks_b200_debug.so only
 
 
 class AlmRotor(C.Structure):
@@ -51,9 +51,13 @@ class GksError(RuntimeError):
 
 def lib(debug=False):
     """Load libgks_b200.so - or, debug=True, libgks_b200_debug.so, the same sources with the test hooks of
-    include/gks_debug.h - built in-tree by paper_2603_11102_b200/build.py.  Fails loudly if absent."""
+    include/gks_debug.h - built in-tree by paper_2603_11102_b200/build.py.  Fails loudly if absent.
+    debug="trace" loads libgks_b200_trace.so (the debug library with the phase timers of the fused sweep compiled in,
+    built on demand by paper_2603_11102_b200/trace.py)."""
     if debug not in _LIBS:
         path = _LIB_DEBUG_PATH if debug else _LIB_PATH
+        if debug == "trace":
+            path = os.path.join(_HERE, "libgks_b200_trace.so")
         if not os.path.exists(path):
             raise ImportError("%s is not built (run `python -m paper_2603_11102_b200.build`); "
                               "there is no CPU fallback" % os.path.basename(path))
@@ -96,6 +100,8 @@ def lib(debug=False):
         if debug:
             L.gks_debug_set_sweep.argtypes = [vp, C.c_int]
             L.gks_debug_fp64_peak.argtypes = [vp, _dp]
+            L.gks_debug_issue_probe.argtypes = [vp, _dp, C.c_int]
+            L.gks_debug_trace.argtypes = [vp, C.POINTER(C.c_ulonglong)]
         L.gks_launch_count.argtypes = [vp]
         L.gks_launch_count.restype = C.c_longlong
         L.gks_last_error.argtypes = [vp]
