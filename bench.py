@@ -213,10 +213,19 @@ def run_slab_proxy(args, w, gks, device):
         g.halo_unpack(which, 1, b[0])
 
     def step():
-        exchange(0)
-        g.step_begin(w.dt)
-        exchange(1)
-        g.step_finish(w.dt)
+        if args.overlap:      # the step in parts: pack, interior, unpack, rim (what a rank does while the halos travel)
+            for which, part in ((0, g.step_begin_part), (1, g.step_finish_part)):
+                g.halo_pack(which, 0, b[0])
+                g.halo_pack(which, 1, b[1])
+                part(w.dt, 0)
+                g.halo_unpack(which, 0, b[1])
+                g.halo_unpack(which, 1, b[0])
+                part(w.dt, 1)
+        else:
+            exchange(0)
+            g.step_begin(w.dt)
+            exchange(1)
+            g.step_finish(w.dt)
         g.step_force(w.dt)
 
     for _ in range(max(args.warmup, 3)):
@@ -255,6 +264,7 @@ def run_slab_proxy(args, w, gks, device):
         "metric": METRIC, "value": cfg.cells / (ms * 1e-3) / 1e6, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "dtype": "f64", "data": "synthetic",
         "config": {"workload": "%s x-slab %d of %d: %dx%dx%d cells, HALO faces on both sides" % (args.workload, r, N, *cfg.n),
+                   "step": "in parts (interior, then rim: gks_step_begin_part)" if args.overlap else "plain",
                    "note": "one sub-domain on one GPU, its own opposite face as the neighbours; no transfer"},
         "gpu_launches_per_step": launches,
         "single_domain_ms_per_step": ms1,
@@ -282,6 +292,7 @@ def main():
                     help="time ONE interior x-slab of the workload cut into N slabs on this GPU: HALO faces on both sides,\n"
                          "halo pack / unpack inside the step, the slab's own opposite face standing in for the neighbours\n"
                          "(a strong-scaling proxy that needs no second GPU; prints its own JSON line)")
+    ap.add_argument("--overlap", action="store_true", help="--slab-proxy: run the step in parts (interior, then rim)")
     ap.add_argument("--no-configs", action="store_true", help="skip the C1..C5 throughput block of the JSON line")
     ap.add_argument("--ibm-passes", type=int, default=1, help="IBM multi-direct-forcing passes per step (workloads with IBM)")
     ap.add_argument("--e2e-steps", type=int, default=3)

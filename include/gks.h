@@ -134,6 +134,20 @@ gks_status gks_step(gks_ctx *ctx, double dt);
  * gks_step = begin + finish + force.  The three parts of one step must be given the same dt.
  * Errors: GKS_ERR_INVALID_ARG (face without HALO, NULL, a dt that differs from gks_step_begin's), GKS_ERR_STATE
  * (order of the calls). */
+/* Overlapping the exchange with the sweeps.  Either half of the step can be given in two parts:
+ *   gks_step_begin_part(ctx, dt, 0)  ghosts of W^n (HALO ghosts may still be on their way), then the sweeps and the
+ *       stage update of the INTERIOR: the tiles and cells that read no HALO ghost (all cells further than 32 from a
+ *       HALO low face and further than 6 .. 37 from a HALO high face; none on a sub-domain narrower than about 70);
+ *   gks_step_begin_part(ctx, dt, 1)  HALO ghosts of W^n must be in place: the ghost passes over the ghost columns
+ *       beyond the HALO faces, then the sweeps and the stage update of the RIM.  Together = gks_step_begin, tile for
+ *       tile and cell for cell the same arithmetic.
+ *   gks_step_finish_part(ctx, dt, part) likewise for the second stage (HALO ghosts of W*).
+ * The driver posts the transfer of a stage's halos, runs part 0, completes the transfer (gks_halo_unpack is allowed
+ * between the parts), runs part 1 - and packs the next stage's halos right after it.  The kernels of the two parts
+ * are enqueued on the context's stream; a transfer overlaps them when the driver moves it on a stream of its own.
+ * Errors: GKS_ERR_STATE (order), GKS_ERR_INVALID_ARG (part, dt). */
+gks_status gks_step_begin_part(gks_ctx *ctx, double dt, int part /* 0 interior, 1 rim */);
+gks_status gks_step_finish_part(gks_ctx *ctx, double dt, int part);
 size_t gks_halo_doubles(const gks_ctx *ctx, int face);
 gks_status gks_halo_pack(gks_ctx *ctx, int which, int face, double *buf);
 gks_status gks_halo_unpack(gks_ctx *ctx, int which, int face, const double *buf);

@@ -322,6 +322,25 @@ gks_status gks_create(const gks_config *cfg, void *workspace, size_t workspace_b
     delete ctx;
     return GKS_ERR_CUDA;
   }
+  {
+    /* interior / rim split of a sub-domain (gks_step_begin_part): the interior is what reads no HALO ghost.  Tiles of
+       the y- and z-sweeps are 32 cells wide along x and stage cells a0-3 .. a0+33, tiles of the x-sweep hold 4 faces
+       and stage cells a0-3 .. a0+5: on a HALO low side the interior starts at cell 32, on a HALO high side it ends at
+       the largest multiple of 32 that leaves 6 cells to the face. */
+    int ta[3];
+    gks_fused_tiles_x(ta);
+    const int nx = g.n[0], big = ta[1];
+    int X0 = g.halo[0] ? big : 0;
+    int X1 = g.halo[1] ? ((nx - 6) / big) * big : nx;
+    if (X1 <= X0) X0 = X1 = 0;
+    ctx->part_x0 = X0;
+    ctx->part_x1 = X1;
+    for (int d = 0; d < 3; ++d) {
+      const int ext = nx + (d == 0 && !g.wrapf[0] ? 1 : 0), all = (ext + ta[d] - 1) / ta[d];
+      ctx->part_t0[d] = X0 / ta[d];
+      ctx->part_t1[d] = X1 <= X0 ? ctx->part_t0[d] : (g.halo[1] ? X1 / ta[d] + (d == 0 ? 1 : 0) : all);
+    }
+  }
   if (!gks_fused_init(ctx)) {
     set_err(nullptr, GKS_ERR_CUDA, "cuTensorMapEncodeTiled unavailable or failed (TMA descriptors of the fused sweep)");
     for (int a = 0; a < 3; ++a) free(ctx->h_xf[a]);

@@ -30,8 +30,8 @@ gks_status fetch_host(gks_ctx *ctx, const double *src, size_t count, std::vector
   return GKS_OK;
 }
 
-/* all sweeps of one stage into ctx->flux[] */
-void sweeps(gks_ctx *ctx, const double *W, bool need_F) {
+/* all sweeps of one stage into ctx->flux[]; part: 0 everything, 1 interior tiles, 2 rim tiles (gks_step_begin_part) */
+void sweeps(gks_ctx *ctx, const double *W, bool need_F, int part = 0) {
   for (int d = 0; d < 3; ++d) {
     gks_prof_begin(ctx, GKS_PROF_SWEEP_X + d);
 #ifdef GKS_DEBUG
@@ -40,7 +40,7 @@ void sweeps(gks_ctx *ctx, const double *W, bool need_F) {
                                                 ctx->stream);
     else
 #endif
-      ctx->launches += gks_launch_sweep_fused(ctx, d, W == ctx->Wn ? 0 : 1, ctx->flux[d], need_F);
+      ctx->launches += gks_launch_sweep_fused(ctx, d, W == ctx->Wn ? 0 : 1, ctx->flux[d], need_F, part);
     gks_prof_end(ctx);
   }
 }
@@ -242,6 +242,67 @@ gks_status gks_step(gks_ctx *ctx, double dt) {
   return gks_step_force(ctx, dt);
 }
 
+/* one stage in two parts (include/gks.h): part 0 = everything that reads no HALO ghost, part 1 = the rest */
+namespace {
+gks_status stage_part(gks_ctx *ctx, double dt, int stage, int part) {
+  const GksGrid &g = ctx->g;
+  const GksPhys &ph = ctx->ph;
+  cudaStream_t s = ctx->stream;
+  double *W = stage == 1 ? ctx->Wn : ctx->Ws;
+  GksPdlScope pdl(!ctx->prof_on);
+  gks_prof_begin(ctx, GKS_PROF_GHOST);
+  if (part == 0) ctx->launches += gks_launch_ghost_fill(g, ph, W, ctx->Wn, s);
+  else ctx->launches += gks_launch_ghost_fill_xcols(g, ph, W, ctx->Wn, s);
+  gks_prof_end(ctx);
+  const bool split = ctx->part_x1 > ctx->part_x0;      /* no interior: part 1 does everything */
+  if (part == 1 || split) {
+    sweeps(ctx, W, stage == 1, part == 0 ? 1 : 2);
+    gks_prof_begin(ctx, GKS_PROF_UPDATE);
+    const int nx = g.n[0], X0 = ctx->part_x0, X1 = ctx->part_x1;
+    const int lo[2] = {part == 0 ? X0 : 0, part == 0 ? 0 : X1}, hi[2] = {part == 0 ? X1 : X0, part == 0 ? 0 : nx};
+    for (int r = 0; r < 2; ++r) {
+      if (hi[r] <= lo[r]) continue;
+      if (stage == 1) ctx->launches += gks_launch_stage1(g, ctx->Wn, ctx->flux, dt, ctx->Ws, ctx->Pbuf, s, lo[r], hi[r]);
+      else ctx->launches += gks_launch_stage2(g, ctx->Pbuf, ctx->flux, dt, ctx->Wn, s, lo[r], hi[r]);
+    }
+    gks_prof_end(ctx);
+  }
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return gks_set_err(ctx, GKS_ERR_CUDA, "stage %d part %d: %s", stage, part, cudaGetErrorString(e));
+  return GKS_OK;
+}
+} /* namespace */
+
+gks_status gks_step_begin_part(gks_ctx *ctx, double dt, int part) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (part != 0 && part != 1) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "part must be 0 (interior) or 1 (rim)");
+  if (!ctx->have_state) return gks_set_err(ctx, GKS_ERR_STATE, "gks_step before gks_set_state");
+  if (!(dt > 0) || !std::isfinite(dt)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "dt must be > 0");
+  if (ctx->mid_step != (part == 0 ? 0 : 10))
+    return gks_set_err(ctx, GKS_ERR_STATE, "gks_step_begin_part(%d): wrong place in the step (state %d)", part, ctx->mid_step);
+  if (part == 1 && dt != ctx->step_dt) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "gks_step_begin_part: dt differs from part 0's");
+  if (ctx->sweep_mode != 0) return gks_set_err(ctx, GKS_ERR_STATE, "the split step runs the fused sweep only");
+  if (gks_status st = gks_check_device(ctx)) return st;
+  if (part == 0) ctx->step_dt = dt;
+  if (gks_status st = stage_part(ctx, dt, 1, part)) return st;
+  ctx->mid_step = part == 0 ? 10 : 1;
+  return GKS_OK;
+}
+
+gks_status gks_step_finish_part(gks_ctx *ctx, double dt, int part) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (part != 0 && part != 1) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "part must be 0 (interior) or 1 (rim)");
+  if (ctx->mid_step != (part == 0 ? 1 : 11))
+    return gks_set_err(ctx, GKS_ERR_STATE, "gks_step_finish_part(%d): wrong place in the step (state %d)", part, ctx->mid_step);
+  if (!(dt > 0) || !std::isfinite(dt) || dt != ctx->step_dt)
+    return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "gks_step_finish_part: dt must be the dt of gks_step_begin");
+  if (ctx->sweep_mode != 0) return gks_set_err(ctx, GKS_ERR_STATE, "the split step runs the fused sweep only");
+  if (gks_status st = gks_check_device(ctx)) return st;
+  if (gks_status st = stage_part(ctx, dt, 2, part)) return st;
+  ctx->mid_step = part == 0 ? 11 : 2;
+  return GKS_OK;
+}
+
 size_t gks_halo_doubles(const gks_ctx *ctx, int face) {
   if (!ctx || face < 0 || face > 5) return 0;
   const int ax = face >> 1, ua = ax == 0 ? 1 : 0, va = ax == 2 ? 1 : 2;
@@ -256,7 +317,10 @@ gks_status halo_move(gks_ctx *ctx, int which, int face, double *buf, int unpack)
     return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "face %d is not a GKS_BC_HALO face", face);
   if (which != 0 && which != 1) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "which must be 0 (W^n) or 1 (W*)");
   if (!ctx->have_state) return gks_set_err(ctx, GKS_ERR_STATE, "no state set");
-  if (which == 1 && ctx->mid_step != 1) return gks_set_err(ctx, GKS_ERR_STATE, "W* exists only between gks_step_begin and gks_step_finish");
+  if (which == 1 && ctx->mid_step != 1 && ctx->mid_step != 11)
+    return gks_set_err(ctx, GKS_ERR_STATE, "W* exists only between gks_step_begin and gks_step_finish");
+  if (which == 0 && ctx->mid_step == 11)
+    return gks_set_err(ctx, GKS_ERR_STATE, "between the two parts of gks_step_finish the buffer of W^n is half W^{n+1}");
   double *W = which == 0 ? ctx->Wn : ctx->Ws;
   const size_t bytes = gks_halo_doubles(ctx, face) * sizeof(double);
   if (gks_is_device_ptr(buf)) {

@@ -215,6 +215,20 @@ int gks_launch_ghost_fill(const GksGrid &g, const GksPhys &ph, double *W, const 
   return 3;
 }
 
+int gks_launch_ghost_fill_xcols(const GksGrid &g, const GksPhys &ph, double *W, const double *Wstate, cudaStream_t s) {
+  int n = 0;
+  for (int side = 0; side < 2; ++side) {
+    if (!g.halo[side]) continue;
+    const int ulo = side == 0 ? -GKS_NG : g.n[0];
+    const PassLines<1> Ly(g);
+    const PassLines<2> Lz(g);
+    gks_launch(k_ghost<1>, dim3(1, Ly.vcnt, 8), dim3(128), 0, s, g, ph, W, Wstate, ulo, GKS_NG, Ly.vlo, Ly.vcnt);
+    gks_launch(k_ghost<2>, dim3(1, Lz.vcnt, 8), dim3(128), 0, s, g, ph, W, Wstate, ulo, GKS_NG, Lz.vlo, Lz.vcnt);
+    n += 2;
+  }
+  return n;
+}
+
 int gks_launch_outflow_init(const GksGrid &g, const GksPhys &ph, double *W, cudaStream_t s) {
   return outflow_state(g, ph, W, -1.0, s);
 }

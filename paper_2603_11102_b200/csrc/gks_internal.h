@@ -110,6 +110,9 @@ struct gks_ctx {
   /* TMA tensor maps of the two state buffers (Wn, Ws) for the three sweep directions (opaque CUtensorMap) */
   alignas(64) unsigned char tmaps[2][3][128];
   int num_sms;                 /* SMs of the device: the fused sweep launches persistent CTAs */
+  /* interior / rim split of a sub-domain (gks_step_begin_part): tiles [part_t0, part_t1) along x of every sweep
+     direction and cells [part_x0, part_x1) read no HALO ghost; empty interior: part_x1 <= part_x0 */
+  int part_t0[3], part_t1[3], part_x0, part_x1;
 
   /* per-class event timing (gks_profile.cu) */
   int prof_on, prof_n;
@@ -208,12 +211,16 @@ int gks_launch_sweep_unfused(const GksGrid &g, const GksPhys &ph, int dir, const
 
 /* fused sweep (gks_sweep_fused.cu); which = 0 reads Wn, 1 reads Ws */
 bool gks_fused_init(gks_ctx *ctx);
-int gks_launch_sweep_fused(gks_ctx *ctx, int dir, int which, double *flux, bool need_F);
+int gks_launch_sweep_fused(gks_ctx *ctx, int dir, int which, double *flux, bool need_F, int part = 0);
+void gks_fused_tiles_x(int ta[3]);
 
+/* stage updates of the cells with x index in [x0, x1) (x1 < 0: the whole grid) */
 int gks_launch_stage1(const GksGrid &g, const double *Wn, double *const flux[3], double dt, double *Ws,
-                      double *Pbuf, cudaStream_t s);
+                      double *Pbuf, cudaStream_t s, int x0 = 0, int x1 = -1);
 int gks_launch_stage2(const GksGrid &g, const double *Pbuf, double *const flux[3], double dt, double *Wn,
-                      cudaStream_t s);
+                      cudaStream_t s, int x0 = 0, int x1 = -1);
+/* y and z ghost passes over the x-ghost columns beyond the HALO faces only (after a halo unpack) */
+int gks_launch_ghost_fill_xcols(const GksGrid &g, const GksPhys &ph, double *W, const double *Wstate, cudaStream_t s);
 
 int gks_launch_bulk_reduce(const GksGrid &g, const double *W, int axis, double *red, cudaStream_t s);
 int gks_launch_uniform_force(const GksGrid &g, double *W, double dt, const double gacc[3], int bulk_axis,

@@ -180,7 +180,7 @@ struct Seg {
 template <int DIR, bool NEED_F, bool LIN, int TA, int TB>
 __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
     k_sweep_fused(const __grid_constant__ CUtensorMap tmap, GksGrid g, GksPhys ph, double *__restrict__ flux,
-                  int ncol_a, int nfull, long long rem, long long PPC) {
+                  int ncol_a, int nfull, long long rem, long long PPC, int ta0, int tlen0, int ta1) {
   using T = Tile<DIR, TA, TB>;
   constexpr int TN = T::TN, NF = T::NF, NT = T::NT, EA = T::EA, EB = T::EB, HA = T::HA, FH = T::FH;
   constexpr bool FUSE_BCD = GKS_FUSE_BCD == 1 || GKS_FUSE_BCD == 3 || (GKS_FUSE_BCD == 2 && DIR != 0);
@@ -221,7 +221,10 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
       len = (int)(left < (long long)(n2 - mb) ? left : (long long)(n2 - mb));
     }
     Seg s;
-    s.a0 = (col % ncol_a) * TA;
+    /* the launch covers the tiles [ta0, ta0 + tlen0) and [ta1, ta1 + ncol_a - tlen0) along a (all of them, or the
+       interior, or the two rims next to cut faces: gks_step_begin_part) */
+    const int ia = col % ncol_a;
+    s.a0 = (ia < tlen0 ? ta0 + ia : ta1 + ia - tlen0) * TA;
     s.b0 = (col / ncol_a) * TB;
     s.p0 = mb - 2;
     s.np = len + 4;
@@ -612,8 +615,17 @@ bool encode_dir(encode_fn_t enc, const GksGrid &g, double *base, CUtensorMap *ou
              CU_TENSOR_MAP_FLOAT_OOB_FILL_NAN_REQUEST_ZERO_FMA) == CUDA_SUCCESS;
 }
 
+/* tiles along a of direction DIR: all of them */
+template <int DIR>
+int tiles_a(const GksGrid &g) {
+  constexpr int TA = Shape<DIR>::TA;
+  const int ext_a = g.n[0] + (DIR == 0 && !g.wrapf[0] ? 1 : 0);
+  return (ext_a + TA - 1) / TA;
+}
+
+/* launch over the a-tiles [ta0, ta0 + len0) and [ta1, ta1 + len1) (len1 may be 0); returns the launches made */
 template <int DIR, bool NEED_F, bool LIN>
-int launch_dir(gks_ctx *ctx, const CUtensorMap &map, double *flux) {
+int launch_dir(gks_ctx *ctx, const CUtensorMap &map, double *flux, int ta0, int len0, int ta1, int len1) {
   constexpr int TA = Shape<DIR>::TA, TB = Shape<DIR>::TB;
   using T = Tile<DIR, TA, TB>;
   const GksGrid &g = ctx->g;
@@ -627,7 +639,9 @@ int launch_dir(gks_ctx *ctx, const CUtensorMap &map, double *flux) {
   }
   const int ext_a = g.n[0] + (T::NA && !g.wrapf[0] ? 1 : 0), ext_b = g.n[T::AXB] + (!T::NA && !g.wrapf[T::AXB] ? 1 : 0);
   const int n2 = g.n[T::AXM];
-  const int ga = (ext_a + TA - 1) / TA, gb = (ext_b + TB - 1) / TB;
+  const int ga = len0 + len1, gb = (ext_b + TB - 1) / TB;
+  (void)ext_a;
+  if (ga <= 0) return 0;
   /* persistent CTAs: the (column, plane) list is cut into equal contiguous ranges, one per resident CTA;
      a range shorter than 8 planes is not worth its 4 priming planes */
   const int ncols = ga * gb;
@@ -636,7 +650,7 @@ int launch_dir(gks_ctx *ctx, const CUtensorMap &map, double *flux) {
   long long PPC = (rem + grid - 1) / grid;
   if (PPC < GKS_MIN_PPC) PPC = GKS_MIN_PPC;                    /* shortest range worth its 4 priming planes */
   if (nfull == 0) grid = (int)((rem + PPC - 1) / PPC);
-  gks_launch(kern, grid, dim3(T::NT), T::SMEM_BYTES, ctx->stream, map, g, ctx->ph, flux, ga, nfull, rem, PPC);
+  gks_launch(kern, grid, dim3(T::NT), T::SMEM_BYTES, ctx->stream, map, g, ctx->ph, flux, ga, nfull, rem, PPC, ta0, len0, ta1);
   return 1;
 }
 
@@ -681,16 +695,38 @@ bool gks_fused_init(gks_ctx *ctx) {
   return true;
 }
 
-int gks_launch_sweep_fused(gks_ctx *ctx, int dir, int which, double *flux, bool need_F) {
+/* part: 0 = the whole direction, 1 = interior tiles only, 2 = rim tiles only (ctx->part_*: gks_step_begin_part) */
+int gks_launch_sweep_fused(gks_ctx *ctx, int dir, int which, double *flux, bool need_F, int part) {
   const CUtensorMap &m = *reinterpret_cast<const CUtensorMap *>(ctx->tmaps[which][dir]);
   const bool lin = ctx->ph.tang_linear != 0;
-#define GKS_DISPATCH(D)                                                                                   \
-  (need_F ? (lin ? launch_dir<D, true, true>(ctx, m, flux) : launch_dir<D, true, false>(ctx, m, flux))  \
-          : (lin ? launch_dir<D, false, true>(ctx, m, flux) : launch_dir<D, false, false>(ctx, m, flux)))
+  const int all = dir == 0 ? tiles_a<0>(ctx->g) : tiles_a<1>(ctx->g);
+  int ta0 = 0, len0 = all, ta1 = 0, len1 = 0;
+  if (part != 0) {
+    const int t0 = ctx->part_t0[dir], t1 = ctx->part_t1[dir];   /* interior tiles [t0, t1) */
+    if (part == 1) {
+      ta0 = t0;
+      len0 = t1 - t0;
+    } else {
+      ta0 = 0;
+      len0 = t0;
+      ta1 = t1;
+      len1 = all - t1;
+    }
+  }
+#define GKS_DISPATCH(D)                                                                                                       \
+  (need_F ? (lin ? launch_dir<D, true, true>(ctx, m, flux, ta0, len0, ta1, len1) : launch_dir<D, true, false>(ctx, m, flux, ta0, len0, ta1, len1))  \
+          : (lin ? launch_dir<D, false, true>(ctx, m, flux, ta0, len0, ta1, len1) : launch_dir<D, false, false>(ctx, m, flux, ta0, len0, ta1, len1)))
   switch (dir) {
     case 0: return GKS_DISPATCH(0);
     case 1: return GKS_DISPATCH(1);
     default: return GKS_DISPATCH(2);
   }
 #undef GKS_DISPATCH
+}
+
+/* tile sizes along x of the three sweep directions (for the interior / rim split of a sub-domain) */
+void gks_fused_tiles_x(int ta[3]) {
+  ta[0] = Shape<0>::TA;
+  ta[1] = Shape<1>::TA;
+  ta[2] = Shape<2>::TA;
 }

@@ -15,12 +15,12 @@ template <bool STAGE1>
 __global__ void __launch_bounds__(256) k_update(GksGrid g, const double *__restrict__ Win,
                                                 const double *__restrict__ fx, const double *__restrict__ fy,
                                                 const double *__restrict__ fz, double dt,
-                                                double *__restrict__ out1, double *__restrict__ out2) {
+                                                double *__restrict__ out1, double *__restrict__ out2, int x0, int x1) {
   gks_pdl_enter();
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int i = x0 + blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
   const int k = blockIdx.z;
-  if (i >= g.n[0] || j >= g.n[1]) return;
+  if (i >= x1 || j >= g.n[1]) return;
   const long long id = g.idx(i, j, k);
   const double iwx = g.inv_w[0][i + GKS_NG], iwy = g.inv_w[1][j + GKS_NG], iwz = g.inv_w[2][k + GKS_NG];
   /* upper face of the cell along each axis; where face n of an axis is face 0 (g.wrapf: periodic axis) the sweep
@@ -44,20 +44,24 @@ __global__ void __launch_bounds__(256) k_update(GksGrid g, const double *__restr
 }
 
 /* 256 threads; 64 along x unless the (sub-)domain is narrower (an x-slab of 32 cells would idle half of them) */
-dim3 update_block(const GksGrid &g) { return g.n[0] > 32 ? dim3(64, 4) : dim3(32, 8); }
+dim3 update_block(int nx) { return nx > 32 ? dim3(64, 4) : dim3(32, 8); }
 
 } /* namespace */
 
 int gks_launch_stage1(const GksGrid &g, const double *Wn, double *const flux[3], double dt, double *Ws,
-                      double *Pbuf, cudaStream_t s) {
-  const dim3 blk = update_block(g), grid((g.n[0] + blk.x - 1) / blk.x, (g.n[1] + blk.y - 1) / blk.y, g.n[2]);
-  gks_launch(k_update<true>, grid, blk, 0, s, g, Wn, flux[0], flux[1], flux[2], dt, Ws, Pbuf);
+                      double *Pbuf, cudaStream_t s, int x0, int x1) {
+  if (x1 < 0) x1 = g.n[0];
+  if (x1 <= x0) return 0;
+  const dim3 blk = update_block(x1 - x0), grid((x1 - x0 + blk.x - 1) / blk.x, (g.n[1] + blk.y - 1) / blk.y, g.n[2]);
+  gks_launch(k_update<true>, grid, blk, 0, s, g, Wn, flux[0], flux[1], flux[2], dt, Ws, Pbuf, x0, x1);
   return 1;
 }
 
 int gks_launch_stage2(const GksGrid &g, const double *Pbuf, double *const flux[3], double dt, double *Wn,
-                      cudaStream_t s) {
-  const dim3 blk = update_block(g), grid((g.n[0] + blk.x - 1) / blk.x, (g.n[1] + blk.y - 1) / blk.y, g.n[2]);
-  gks_launch(k_update<false>, grid, blk, 0, s, g, Pbuf, flux[0], flux[1], flux[2], dt, Wn, nullptr);
+                      cudaStream_t s, int x0, int x1) {
+  if (x1 < 0) x1 = g.n[0];
+  if (x1 <= x0) return 0;
+  const dim3 blk = update_block(x1 - x0), grid((x1 - x0 + blk.x - 1) / blk.x, (g.n[1] + blk.y - 1) / blk.y, g.n[2]);
+  gks_launch(k_update<false>, grid, blk, 0, s, g, Pbuf, flux[0], flux[1], flux[2], dt, Wn, (double *)nullptr, x0, x1);
   return 1;
 }

@@ -21,7 +21,7 @@ STATUS = {0: "GKS_OK", 1: "GKS_ERR_INVALID_ARG", 2: "GKS_ERR_WORKSPACE", 3: "GKS
 EXPORTS = ["gks_workspace_bytes", "gks_create", "gks_destroy", "gks_set_state", "gks_get_state", "gks_step",
            "gks_set_body_force", "gks_set_bulk_flux", "alm_set_points", "ibm_set_points", "ibm_set_velocities", "ibm_set_iterations", "gks_cfl_dt", "alm_set_rotor", "alm_rotor_eval", "alm_rotor_points", "gks_set_reconstruction", "gks_halo_doubles", "gks_halo_pack", "gks_halo_unpack", "gks_step_begin",
            "gks_step_finish", "gks_step_force", "gks_bulk_partial", "gks_bulk_set_global", "gks_ibm_pass", "gks_ibm_residual",
-           "gks_debug_eval_flux", "alm_rotor_supply",
+           "gks_debug_eval_flux", "alm_rotor_supply", "gks_step_begin_part", "gks_step_finish_part",
            "gks_profile_enable", "gks_profile_read", "gks_check_finite", "gks_launch_count", "gks_last_error"]
 DEBUG_EXPORTS = ["gks_debug_set_sweep", "gks_debug_fp64_peak", "gks_debug_issue_probe", "gks_debug_trace"]    # include/gks_debug.h: libgks_b200_debug.so only
 
@@ -88,6 +88,8 @@ def lib(debug=False):
         L.gks_step_begin.argtypes = [vp, C.c_double]
         L.gks_step_finish.argtypes = [vp, C.c_double]
         L.gks_step_force.argtypes = [vp, C.c_double]
+        L.gks_step_begin_part.argtypes = [vp, C.c_double, C.c_int]
+        L.gks_step_finish_part.argtypes = [vp, C.c_double, C.c_int]
         L.gks_bulk_partial.argtypes = [vp, vp, C.POINTER(C.c_double)]
         L.gks_bulk_set_global.argtypes = [vp, vp, C.c_double]
         L.gks_ibm_pass.argtypes = [vp, C.c_int, C.c_int]
@@ -323,6 +325,13 @@ class Gks:
 
     def step_force(self, dt):
         self._c("gks_step_force", float(dt))
+
+    def step_begin_part(self, dt, part):
+        """part 0: interior (reads no HALO ghost), part 1: rim (HALO ghosts of W^n in place)"""
+        self._c("gks_step_begin_part", float(dt), int(part))
+
+    def step_finish_part(self, dt, part):
+        self._c("gks_step_finish_part", float(dt), int(part))
 
     def ibm_pass(self, k, phase):
         self._c("gks_ibm_pass", int(k), int(phase))

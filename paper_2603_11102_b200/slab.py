@@ -173,6 +173,26 @@ class LocalTransport:
             solvers[dst].halo_unpack(which, dst_face, buf)
 
 
+    # the same exchange in two halves, for the overlapped step (nothing overlaps inside one process: the hand-over
+    # is a pointer; the split is what is exercised)
+    def exchange_begin(self, solvers, which, new_buffer):
+        for s in solvers:
+            s.synchronize()
+        self._packed = {}
+        for r, s in enumerate(solvers):
+            for face, dst, dst_face in self.d.schedule(r):
+                buf = new_buffer(s, face, "send")
+                s.halo_pack(which, face, buf)
+                self._packed[(dst, dst_face)] = buf
+
+    def exchange_end(self, solvers, which, new_buffer):
+        for s in solvers:
+            s.synchronize()
+        for (dst, dst_face), buf in self._packed.items():
+            solvers[dst].halo_unpack(which, dst_face, buf)
+        self._packed = {}
+
+
 class DistTransport:
     """One process per sub-domain; point-to-point messages through torch.distributed (nccl or gloo)."""
 
@@ -208,6 +228,50 @@ class DistTransport:
                     req.wait()
         for face, rbuf in recvs:
             solver.halo_unpack(which, face, rbuf)
+
+    def exchange_begin(self, solver, which, new_buffer):
+        """pack the halos of state `which` and post the messages; returns at once.  Device buffers (NCCL): the
+        messages travel on a communication stream of their own, ordered behind the packs by an event, so the kernels
+        the solver enqueues next (part 0 of a stage: everything that reads no HALO ghost) run beside the transfer."""
+        import torch
+        dist = self.dist
+        sched = self.d.schedule(self.rank)
+        ops, self._recvs, cuda = [], [], False
+        for face, dst, dst_face in sched:
+            sbuf = new_buffer(solver, face, "send")
+            cuda = cuda or sbuf.is_cuda
+            solver.halo_pack(which, face, sbuf)
+            ops.append(dist.P2POp(dist.isend, sbuf, dst, group=self.group, tag=face))
+        for face, dst, dst_face in sorted(sched, key=lambda e: e[2]):      # receives in the SENDER's order (see exchange)
+            rbuf = new_buffer(solver, face, "recv")
+            self._recvs.append((face, rbuf))
+            ops.append(dist.P2POp(dist.irecv, rbuf, dst, group=self.group, tag=dst_face))
+        self._reqs, self._comm = [], None
+        if ops:
+            if cuda:
+                if getattr(self, "_comm_stream", None) is None:
+                    self._comm_stream = torch.cuda.Stream(device=solver.device)
+                self._comm = self._comm_stream
+                self._comm.wait_stream(solver.stream)                        # behind the packs
+                with torch.cuda.stream(self._comm):
+                    self._reqs = dist.batch_isend_irecv(ops)
+            else:
+                self._reqs = dist.batch_isend_irecv(ops)                     # gloo: the packs have synchronised
+
+    def exchange_end(self, solver, which, new_buffer):
+        """complete the messages posted by exchange_begin and unpack them into the HALO ghosts"""
+        import torch
+        if self._comm is not None:
+            with torch.cuda.stream(self._comm):
+                for req in self._reqs:
+                    req.wait()
+            solver.stream.wait_stream(self._comm)                            # the unpacks behind the transfer
+        else:
+            for req in self._reqs:
+                req.wait()
+        for face, rbuf in self._recvs:
+            solver.halo_unpack(which, face, rbuf)
+        self._reqs, self._recvs = [], []
 
     def all_reduce_sum(self, solver, scalar, volume):
         """(sum over ranks of a 1-element tensor, sum of the host number `volume`)"""
@@ -375,18 +439,30 @@ class SlabStepper:
             for s in sols:
                 s.ibm_pass(k, 1)
 
-    def step(self, dt, before_forcing=None, ibm=False, rotor=None, bulk=False, ibm_passes=1):
+    def step(self, dt, before_forcing=None, ibm=False, rotor=None, bulk=False, ibm_passes=1, overlap=False):
         """before_forcing(solver): e.g. alm_set_points for this step (replicated point list);
         ibm: Lagrangian points are set (on any rank): the un-forced W^{n+1} is exchanged before the forcing;
         rotor: a RotorDriver (on-line actuator lines), evaluated on the un-forced W^{n+1} as well;
         bulk: the bulk-flux forcing is set: its global sum is assembled before the forcing;
-        ibm_passes: the max_iter given to ibm_set_iterations on every sub-domain, when > 1"""
+        ibm_passes: the max_iter given to ibm_set_iterations on every sub-domain, when > 1;
+        overlap: the halos of either stage travel while the stage's interior is swept (PAPER.md:193-197 exchanges per
+        flux evaluation; include/gks.h gks_step_begin_part): post, part 0, complete, part 1"""
         if before_forcing is not None:
             self._each(before_forcing)
-        self.t.exchange(self.solvers, 0, self.new_buffer)      # ghosts of W^n
-        self._each(lambda s: s.step_begin(dt))
-        self.t.exchange(self.solvers, 1, self.new_buffer)      # ghosts of W*
-        self._each(lambda s: s.step_finish(dt))
+        if overlap:
+            self.t.exchange_begin(self.solvers, 0, self.new_buffer)     # ghosts of W^n on their way
+            self._each(lambda s: s.step_begin_part(dt, 0))              # interior of stage 1
+            self.t.exchange_end(self.solvers, 0, self.new_buffer)
+            self._each(lambda s: s.step_begin_part(dt, 1))              # rim of stage 1: W* complete
+            self.t.exchange_begin(self.solvers, 1, self.new_buffer)     # ghosts of W* on their way
+            self._each(lambda s: s.step_finish_part(dt, 0))
+            self.t.exchange_end(self.solvers, 1, self.new_buffer)
+            self._each(lambda s: s.step_finish_part(dt, 1))
+        else:
+            self.t.exchange(self.solvers, 0, self.new_buffer)      # ghosts of W^n
+            self._each(lambda s: s.step_begin(dt))
+            self.t.exchange(self.solvers, 1, self.new_buffer)      # ghosts of W*
+            self._each(lambda s: s.step_finish(dt))
         if ibm or rotor is not None:
             self.t.exchange(self.solvers, 0, self.new_buffer)  # ghosts of the un-forced W^{n+1}
         if rotor is not None:

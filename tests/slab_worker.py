@@ -3,7 +3,7 @@ torch.distributed.run): its own `Gks` context on cuda:0, `slab.DistTransport` ov
 buffers, the scalar all-reduces (bulk flux, IBM stop rule) and the rotor broadcast.  Every rank shares the one GPU of
 the box; the ranks synchronise on the host between kernels (gloo), no kernel waits on another process.
 
-    python -m torch.distributed.run --nproc-per-node W tests/slab_worker.py CASE STEPS OUTDIR
+    python -m torch.distributed.run --nproc-per-node W tests/slab_worker.py CASE STEPS OUTDIR [overlap]
 """
 import os
 import sys
@@ -19,6 +19,8 @@ def case_setup(name):
     from paper_2603_11102_b200 import workloads as wl
     if name == "taylor_green":
         return wl.by_name("C1"), 1, None
+    if name == "cylinder_full":                 # 256 x 128 x 64: slabs wide enough to have an interior (overlapped step)
+        return wl.by_name("C3"), 1, None
     if name == "channel":                       # bulk-flux forcing: one scalar all-reduce per step
         return wl.by_name("C2", small=True), 1, None
     if name == "cylinder":                      # IBM body cut through by a slab boundary
@@ -42,6 +44,7 @@ def main():
     import torch.distributed as dist
     from paper_2603_11102_b200 import gks, slab
     case, steps, outdir = sys.argv[1], int(sys.argv[2]), sys.argv[3]
+    overlap = len(sys.argv) > 4 and sys.argv[4] == "overlap"
     os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
     dist.init_process_group("gloo")
     rank, world = dist.get_rank(), dist.get_world_size()
@@ -63,7 +66,7 @@ def main():
             pts = d.alm_points(rank, *w.alm(k))
             hook = lambda s, pts=pts: s.alm_set_points(*pts)
         stepper.step(w.dt, before_forcing=hook, ibm=w.ibm is not None, rotor=rot, bulk=w.bulk_flux is not None,
-                     ibm_passes=passes)
+                     ibm_passes=passes, overlap=overlap)
     np.save(os.path.join(outdir, "part%d.npy" % rank), g.get_state())
     launches = g.launch_count
     g.close()

@@ -11,7 +11,7 @@ from paper_2603_11102_b200 import slab, workloads as wl
 pytestmark = pytest.mark.gpu
 
 
-def run_slabs(w, world, steps, linear=False):
+def run_slabs(w, world, steps, linear=False, overlap=False):
     from paper_2603_11102_b200 import gks
     d = slab.SlabDecomposition(w.cfg, world)
     solvers = [gks.Gks(d.local_cfg(r)) for r in range(world)]
@@ -28,7 +28,7 @@ def run_slabs(w, world, steps, linear=False):
     for k in range(steps):
         pts = w.alm(k) if w.alm is not None else None
         stepper.step(w.dt, before_forcing=(lambda s: s.alm_set_points(*pts)) if pts is not None else None,
-                     ibm=w.ibm is not None, bulk=w.bulk_flux is not None)
+                     ibm=w.ibm is not None, bulk=w.bulk_flux is not None, overlap=overlap)
     W = d.gather([s.get_state() for s in solvers])
     for s in solvers:
         s.close()
@@ -330,3 +330,32 @@ def test_rotor_and_points_at_the_seam_of_a_periodic_x_axis():
             free.step(dt)
         assert np.abs(W1 - free.get_state())[..., -3:].max() > 1e-6
         free.close()
+
+
+@pytest.mark.parametrize("name,world,small", [("C1", 2, True), ("TG160", 2, False), ("C3", 2, False), ("C4", 3, True), ("C2", 2, False)])
+def test_overlapped_step_equals_the_plain_step(name, world, small):
+    """gks_step_begin_part / gks_step_finish_part (interior while the halos travel, then the rim): the same tiles and
+    cells in another order - bit for bit the plain decomposed step on a periodic box (no interior at 16 cells per
+    slab: the rim is everything; cells 32 .. 64 of 80 on the 160^3 box), to the order of the fp64 atomics with IBM; and the call order is enforced.
+    C3 at its full 256 x 128 x 64 (slabs of 128 cells: interior 32 .. 96) has inflow / outflow along x and the body
+    in the rim-interior seam of slab 0; C2 at 128 x 96 x 64 adds the bulk-flux all-reduce"""
+    from paper_2603_11102_b200 import gks
+    w = wl.taylor_green(160) if name == "TG160" else wl.by_name(name, small=small)   # 160: slabs of 80, interior 32 .. 64
+    steps = 2
+    Wp, Wo = run_slabs(w, world, steps), run_slabs(w, world, steps, overlap=True)
+    if w.ibm is None:
+        assert np.array_equal(Wo, Wp)
+    else:
+        assert rel_linf(Wo, Wp) <= 1e-14
+    assert rel_linf(Wo, run_single(w, steps)) <= 1e-13
+    d = slab.SlabDecomposition(w.cfg, world)
+    g = gks.Gks(d.local_cfg(0))
+    g.set_state(d.scatter(w.W0, 0))
+    with pytest.raises(gks.GksError):
+        g.step_begin_part(w.dt, 1)                           # the rim before the interior
+    g.step_begin_part(w.dt, 0)
+    with pytest.raises(gks.GksError):
+        g.step_begin_part(w.dt, 0)
+    with pytest.raises(gks.GksError):
+        g.step_finish(w.dt)
+    g.close()

@@ -41,13 +41,17 @@ def single_domain(case):
     return W
 
 
-@pytest.mark.parametrize("case,world", [("taylor_green", 2), ("taylor_green", 3), ("cylinder", 2), ("cylinder_passes", 3),
-                                        ("channel", 2), ("turbine", 3), ("rotor_online", 4)])
-def test_ranks_with_the_real_library_reproduce_the_single_domain(case, world, tmp_path):
-    port = 29650 + (hash((case, world)) % 200)
+@pytest.mark.parametrize("case,world,mode", [("taylor_green", 2, "plain"), ("taylor_green", 3, "plain"),
+                                             ("cylinder", 2, "plain"), ("cylinder_passes", 3, "plain"),
+                                             ("channel", 2, "plain"), ("turbine", 3, "plain"), ("rotor_online", 4, "plain"),
+                                             ("cylinder_full", 2, "overlap"), ("taylor_green", 2, "overlap")])
+def test_ranks_with_the_real_library_reproduce_the_single_domain(case, world, mode, tmp_path):
+    """mode "overlap": the step in parts (slab.SlabStepper.step(overlap=True)): messages are posted before the interior
+    is swept and completed before the rim"""
+    port = 29650 + (hash((case, world, mode)) % 200)
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(world),
            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.join(ROOT, "tests", "slab_worker.py"),
-           case, str(STEPS), str(tmp_path)]
+           case, str(STEPS), str(tmp_path), mode]
     r = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT)
     assert r.returncode == 0, (r.stdout[-1500:], r.stderr[-3000:])
     Ws = np.concatenate([np.load(os.path.join(tmp_path, "part%d.npy" % k)) for k in range(world)], axis=-1)
