@@ -328,7 +328,7 @@ gks_status gks_create(const gks_config *cfg, void *workspace, size_t workspace_b
        and stage cells a0-3 .. a0+5: on a HALO low side the interior starts at cell 32, on a HALO high side it ends at
        the largest multiple of 32 that leaves 6 cells to the face. */
     int ta[3];
-    gks_fused_tiles_x(ta);
+    gks_fused_tiles_x(g, ta);
     const int nx = g.n[0], big = ta[1];
     int X0 = g.halo[0] ? big : 0;
     int X1 = g.halo[1] ? ((nx - 6) / big) * big : nx;

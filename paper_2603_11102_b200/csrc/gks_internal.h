@@ -212,7 +212,7 @@ int gks_launch_sweep_unfused(const GksGrid &g, const GksPhys &ph, int dir, const
 /* fused sweep (gks_sweep_fused.cu); which = 0 reads Wn, 1 reads Ws */
 bool gks_fused_init(gks_ctx *ctx);
 int gks_launch_sweep_fused(gks_ctx *ctx, int dir, int which, double *flux, bool need_F, int part = 0);
-void gks_fused_tiles_x(int ta[3]);
+void gks_fused_tiles_x(const GksGrid &g, int ta[3]);
 
 /* stage updates of the cells with x index in [x0, x1) (x1 < 0: the whole grid) */
 int gks_launch_stage1(const GksGrid &g, const double *Wn, double *const flux[3], double dt, double *Ws,

@@ -224,7 +224,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
     /* the launch covers the tiles [ta0, ta0 + tlen0) and [ta1, ta1 + ncol_a - tlen0) along a (all of them, or the
        interior, or the two rims next to cut faces: gks_step_begin_part) */
     const int ia = col % ncol_a;
-    s.a0 = (ia < tlen0 ? ta0 + ia : ta1 + ia - tlen0) * TA;
+    s.a0 = (ia + (ia < tlen0 ? ta0 : ta1)) * TA;      /* ta1: already less tlen0 */
     s.b0 = (col / ncol_a) * TB;
     s.p0 = mb - 2;
     s.np = len + 4;
@@ -591,20 +591,22 @@ typedef CUresult (*encode_fn_t)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, 
                                 const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
                                 CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-/* tile shapes: 128 faces per CTA; x-faces 8 (normal, along a) x 16 (t1), y/z-faces 32 (t1, along a) x 4 (normal): measured */
+/* tile shapes: 128 faces per CTA.  y- and z-faces: 32 (t1, along a) x 4 (normal).  x-faces: 8 (normal, along a) x 16 (t1)
+   on a periodic x axis, 4 x 32 where face n+1 exists (walls, inflow / outflow, cut faces of a sub-domain): the two are
+   equally fast per tile, the narrow one wastes less of the tile that hangs over the last face (257 faces: 1.2 % instead
+   of 2.7 %; 33 faces of a 32-cell slab: 9 % instead of 21 %) but stages 9 cells for 4 faces along x and re-reads more of
+   the slab halo from DRAM (measured 1.39 GB instead of 0.91 GB read per launch at 256^3): chosen per context */
 #ifndef GKS_TILE_YZ_A
 #define GKS_TILE_YZ_A 32
 #endif
-#ifndef GKS_TILE_X_A
-#define GKS_TILE_X_A 4
-#endif
-template <int DIR> struct Shape {
-  static constexpr int TA = DIR == 0 ? GKS_TILE_X_A : GKS_TILE_YZ_A, TB = 128 / TA;
+template <int DIR, int XA> struct Shape {
+  static constexpr int TA = DIR == 0 ? XA : GKS_TILE_YZ_A, TB = 128 / TA;
 };
+inline int x_tile_a(const GksGrid &g) { return g.wrapf[0] ? 8 : 4; }
 
-template <int DIR>
+template <int DIR, int XA>
 bool encode_dir(encode_fn_t enc, const GksGrid &g, double *base, CUtensorMap *out) {
-  using T = Tile<DIR, Shape<DIR>::TA, Shape<DIR>::TB>;
+  using T = Tile<DIR, Shape<DIR, XA>::TA, Shape<DIR, XA>::TB>;
   const cuuint64_t dims[4] = {(cuuint64_t)g.P[0], (cuuint64_t)g.P[1], (cuuint64_t)g.P[2], 4};
   const cuuint64_t strides[3] = {(cuuint64_t)g.P[0] * 8, (cuuint64_t)g.P[0] * g.P[1] * 8, (cuuint64_t)g.FS * 8};
   cuuint32_t box[4] = {(cuuint32_t)T::EA, 1, 1, 4};
@@ -615,18 +617,17 @@ bool encode_dir(encode_fn_t enc, const GksGrid &g, double *base, CUtensorMap *ou
              CU_TENSOR_MAP_FLOAT_OOB_FILL_NAN_REQUEST_ZERO_FMA) == CUDA_SUCCESS;
 }
 
-/* tiles along a of direction DIR: all of them */
-template <int DIR>
-int tiles_a(const GksGrid &g) {
-  constexpr int TA = Shape<DIR>::TA;
-  const int ext_a = g.n[0] + (DIR == 0 && !g.wrapf[0] ? 1 : 0);
+/* tiles along a of direction dir: all of them */
+int tiles_a(const GksGrid &g, int dir) {
+  const int TA = dir == 0 ? x_tile_a(g) : GKS_TILE_YZ_A;
+  const int ext_a = g.n[0] + (dir == 0 && !g.wrapf[0] ? 1 : 0);
   return (ext_a + TA - 1) / TA;
 }
 
 /* launch over the a-tiles [ta0, ta0 + len0) and [ta1, ta1 + len1) (len1 may be 0); returns the launches made */
-template <int DIR, bool NEED_F, bool LIN>
+template <int DIR, bool NEED_F, bool LIN, int XA>
 int launch_dir(gks_ctx *ctx, const CUtensorMap &map, double *flux, int ta0, int len0, int ta1, int len1) {
-  constexpr int TA = Shape<DIR>::TA, TB = Shape<DIR>::TB;
+  constexpr int TA = Shape<DIR, XA>::TA, TB = Shape<DIR, XA>::TB;
   using T = Tile<DIR, TA, TB>;
   const GksGrid &g = ctx->g;
   auto kern = k_sweep_fused<DIR, NEED_F, LIN, TA, TB>;
@@ -650,7 +651,7 @@ int launch_dir(gks_ctx *ctx, const CUtensorMap &map, double *flux, int ta0, int 
   long long PPC = (rem + grid - 1) / grid;
   if (PPC < GKS_MIN_PPC) PPC = GKS_MIN_PPC;                    /* shortest range worth its 4 priming planes */
   if (nfull == 0) grid = (int)((rem + PPC - 1) / PPC);
-  gks_launch(kern, grid, dim3(T::NT), T::SMEM_BYTES, ctx->stream, map, g, ctx->ph, flux, ga, nfull, rem, PPC, ta0, len0, ta1);
+  gks_launch(kern, grid, dim3(T::NT), T::SMEM_BYTES, ctx->stream, map, g, ctx->ph, flux, ga, nfull, rem, PPC, ta0, len0, ta1 - len0);
   return 1;
 }
 
@@ -688,9 +689,9 @@ bool gks_fused_init(gks_ctx *ctx) {
   double *bases[2] = {ctx->Wn, ctx->Ws};
   for (int b = 0; b < 2; ++b) {
     CUtensorMap *m = reinterpret_cast<CUtensorMap *>(ctx->tmaps[b][0]);
-    if (!encode_dir<0>(enc, ctx->g, bases[b], m)) return false;
-    if (!encode_dir<1>(enc, ctx->g, bases[b], reinterpret_cast<CUtensorMap *>(ctx->tmaps[b][1]))) return false;
-    if (!encode_dir<2>(enc, ctx->g, bases[b], reinterpret_cast<CUtensorMap *>(ctx->tmaps[b][2]))) return false;
+    if (!(x_tile_a(ctx->g) == 8 ? encode_dir<0, 8>(enc, ctx->g, bases[b], m) : encode_dir<0, 4>(enc, ctx->g, bases[b], m))) return false;
+    if (!encode_dir<1, 8>(enc, ctx->g, bases[b], reinterpret_cast<CUtensorMap *>(ctx->tmaps[b][1]))) return false;
+    if (!encode_dir<2, 8>(enc, ctx->g, bases[b], reinterpret_cast<CUtensorMap *>(ctx->tmaps[b][2]))) return false;
   }
   return true;
 }
@@ -699,7 +700,7 @@ bool gks_fused_init(gks_ctx *ctx) {
 int gks_launch_sweep_fused(gks_ctx *ctx, int dir, int which, double *flux, bool need_F, int part) {
   const CUtensorMap &m = *reinterpret_cast<const CUtensorMap *>(ctx->tmaps[which][dir]);
   const bool lin = ctx->ph.tang_linear != 0;
-  const int all = dir == 0 ? tiles_a<0>(ctx->g) : tiles_a<1>(ctx->g);
+  const int all = tiles_a(ctx->g, dir);
   int ta0 = 0, len0 = all, ta1 = 0, len1 = 0;
   if (part != 0) {
     const int t0 = ctx->part_t0[dir], t1 = ctx->part_t1[dir];   /* interior tiles [t0, t1) */
@@ -713,20 +714,20 @@ int gks_launch_sweep_fused(gks_ctx *ctx, int dir, int which, double *flux, bool 
       len1 = all - t1;
     }
   }
-#define GKS_DISPATCH(D)                                                                                                       \
-  (need_F ? (lin ? launch_dir<D, true, true>(ctx, m, flux, ta0, len0, ta1, len1) : launch_dir<D, true, false>(ctx, m, flux, ta0, len0, ta1, len1))  \
-          : (lin ? launch_dir<D, false, true>(ctx, m, flux, ta0, len0, ta1, len1) : launch_dir<D, false, false>(ctx, m, flux, ta0, len0, ta1, len1)))
+#define GKS_DISPATCH(D, XA)                                                                                                   \
+  (need_F ? (lin ? launch_dir<D, true, true, XA>(ctx, m, flux, ta0, len0, ta1, len1) : launch_dir<D, true, false, XA>(ctx, m, flux, ta0, len0, ta1, len1))  \
+          : (lin ? launch_dir<D, false, true, XA>(ctx, m, flux, ta0, len0, ta1, len1) : launch_dir<D, false, false, XA>(ctx, m, flux, ta0, len0, ta1, len1)))
   switch (dir) {
-    case 0: return GKS_DISPATCH(0);
-    case 1: return GKS_DISPATCH(1);
-    default: return GKS_DISPATCH(2);
+    case 0: return x_tile_a(ctx->g) == 8 ? GKS_DISPATCH(0, 8) : GKS_DISPATCH(0, 4);
+    case 1: return GKS_DISPATCH(1, 8);
+    default: return GKS_DISPATCH(2, 8);
   }
 #undef GKS_DISPATCH
 }
 
 /* tile sizes along x of the three sweep directions (for the interior / rim split of a sub-domain) */
-void gks_fused_tiles_x(int ta[3]) {
-  ta[0] = Shape<0>::TA;
-  ta[1] = Shape<1>::TA;
-  ta[2] = Shape<2>::TA;
+void gks_fused_tiles_x(const GksGrid &g, int ta[3]) {
+  ta[0] = x_tile_a(g);
+  ta[1] = GKS_TILE_YZ_A;
+  ta[2] = GKS_TILE_YZ_A;
 }
