@@ -292,7 +292,12 @@ def main():
                     help="time ONE interior x-slab of the workload cut into N slabs on this GPU: HALO faces on both sides,\n"
                          "halo pack / unpack inside the step, the slab's own opposite face standing in for the neighbours\n"
                          "(a strong-scaling proxy that needs no second GPU; prints its own JSON line)")
-    ap.add_argument("--overlap", action="store_true", help="--slab-proxy: run the step in parts (interior, then rim)")
+    ap.add_argument("--overlap", action="store_true",
+                    help="--slab-proxy / --decomp slab: the step in parts (interior while the halos travel, then the rim)")
+    ap.add_argument("--online-rotor", action="store_true",
+                    help="workloads with an ALM rotor (C4, C5): the on-line blade-element rotor (alm_set_rotor: sampling,\n"
+                         "Eq. 9, tip and free-stream corrections on the device, synthetic blade data) instead of prescribed\n"
+                         "point forces re-set from the host every step")
     ap.add_argument("--no-configs", action="store_true", help="skip the C1..C5 throughput block of the JSON line")
     ap.add_argument("--ibm-passes", type=int, default=1, help="IBM multi-direct-forcing passes per step (workloads with IBM)")
     ap.add_argument("--e2e-steps", type=int, default=3)
@@ -359,12 +364,27 @@ def main():
     g.stream.synchronize()
     g.set_state(Wd)
     step_no = [0]
+    rotor_drv = None
+    if args.online_rotor:
+        if w.alm is None:
+            raise SystemExit("--online-rotor needs a workload with an ALM rotor (C4, C5)")
+        w_ref = w_global if slab_mode else w
+        pos0, _, eps = w_ref.alm(0)
+        hub = pos0.reshape(3, -1, 3).mean(axis=(0, 1))          # the prescribed blades are 120 degrees apart
+        rot = wl.synthetic_rotor(hub=hub, R=float(np.linalg.norm(pos0 - hub, axis=1).max() * 64.5 / 64.0), eps=eps,
+                                 freestream_correction=True, tip_correction=True)
+        if slab_mode:
+            rotor_drv = slab.RotorDriver(dec, rot, device)
+        else:
+            g.alm_set_rotor(rot)
+        from dataclasses import replace as _rep
+        w = _rep(w, alm=None)                                   # no prescribed points any more
 
     def slab_step(k):
         # actuator points reach a slab through dec.alm_points (supports across cuts, images beyond a periodic seam)
         hook = (lambda s: s.alm_set_points(*dec.alm_points(rank, *w.alm(k)))) if w.alm is not None else None
         stepper.step(w.dt, before_forcing=hook, ibm=w_global.ibm is not None, bulk=w.bulk_flux is not None,
-                     ibm_passes=args.ibm_passes)
+                     ibm_passes=args.ibm_passes, rotor=rotor_drv, overlap=args.overlap)
 
     def one_step():
         if stepper is not None:
@@ -461,6 +481,8 @@ def main():
             "scaling": "strong" if slab_mode else "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": "%s %s %dx%dx%d" % (args.workload, w.name, *(w_global if slab_mode else w).cfg.n),
                        "sweep": "fused" if args.sweep == 0 else "unfused", "variant": args.variant,
+                       "alm": ("on-line rotor (alm_set_rotor, synthetic blade data)" if args.online_rotor else
+                               ("prescribed point forces" if (w_global if slab_mode else w).alm is not None else None)),
                        "multi_gpu": ("x-slabs with halo exchange" if slab_mode else "replicas only") if world > 1 else "single GPU",
                        "l2": "inputs larger than L2 (state %.0f MB per field set)" % (cells * 32 / 1e6)},
             "clocks": clocks,
