@@ -27,7 +27,8 @@ class GksoRotor(C.Structure):
                 ("R", C.c_double), ("r_hub", C.c_double), ("omega", C.c_double), ("theta0", C.c_double),
                 ("u_ref", C.c_double), ("eps", C.c_double), ("chord", _dp), ("twist", _dp),
                 ("npolar", C.c_int), ("alpha", _dp), ("cl", _dp), ("cd", _dp),
-                ("freestream_correction", C.c_int), ("tip_correction", C.c_int)]
+                ("freestream_correction", C.c_int), ("tip_correction", C.c_int),
+                ("radius", _dp), ("width", _dp), ("nsections", C.c_int), ("section_r", _dp)]
 
 
 def build(force=False):
@@ -227,7 +228,9 @@ class Oracle:
             self._rotor_n = 0
             return
         keep = [_arr(x) for x in (r.chord, r.twist, r.alpha, r.cl, r.cd)]
-        assert len(keep[0]) == r.npts and len(keep[1]) == r.npts and len(keep[3]) == len(keep[2]) == len(keep[4])
+        sec_r = getattr(r, "section_r", None)
+        ns = 1 if sec_r is None else len(sec_r)
+        assert len(keep[0]) == r.npts and len(keep[1]) == r.npts and keep[3].size == ns * len(keep[2]) == keep[4].size
         c = GksoRotor()
         c.nblades, c.npts = r.nblades, r.npts
         c.hub = (C.c_double * 3)(*r.hub)
@@ -235,6 +238,13 @@ class Oracle:
         c.chord, c.twist, c.alpha, c.cl, c.cd = [_p(x) for x in keep]
         c.npolar = len(keep[2])
         c.freestream_correction, c.tip_correction = int(r.freestream_correction), int(r.tip_correction)
+        if getattr(r, "radius", None) is not None:       # S28: explicit stations, section-blended polars
+            keep += [_arr(r.radius), _arr(r.width)]
+            assert len(keep[-1]) == r.npts == len(keep[-2])
+            c.radius, c.width = _p(keep[-2]), _p(keep[-1])
+        if sec_r is not None:
+            keep.append(_arr(sec_r))
+            c.nsections, c.section_r = ns, _p(keep[-1])
         _check(lib().gkso_alm_set_rotor(self._h, C.byref(c)))
         self._rotor_n = r.nblades * r.npts
 

@@ -375,6 +375,8 @@ struct gkso_ctx {
     int nb = 0, np = 0, fs_corr = 0, tip_corr = 0;
     double hub[3] = {0, 0, 0}, R = 0, rhub = 0, omega = 0, theta0 = 0, uref = 0, time = 0;
     std::vector<double> chord, twist, pa, pcl, pcd;
+    std::vector<double> radius, width;   /* per station (S28); even spacing when the caller gave none */
+    std::vector<double> sec_r;           /* radii of the airfoil sections; pcl, pcd: [section][alpha] */
   } rotor;
   bool tangential_linear = false; /* scheme variant: linear weights in the two tangential passes (f4) */
   int ibm_maxit = 1;       /* multi-direct-forcing passes per step; 1 = single pass (S15) */
@@ -709,16 +711,33 @@ void sample_trilinear(const gkso_ctx &s, const std::vector<double> &Wp, const do
       }
 }
 
-/* tabulated 2-D airfoil data, linear in alpha, end values beyond the table */
-void polar_lookup(const gkso_ctx::Rotor &r, double alpha, double &cl, double &cd) {
+/* tabulated 2-D airfoil data of one section (table `sec`), linear in alpha, end values beyond the table */
+void polar_lookup_section(const gkso_ctx::Rotor &r, int sec, double alpha, double &cl, double &cd) {
   const int n = (int)r.pa.size();
-  if (alpha <= r.pa[0]) { cl = r.pcl[0]; cd = r.pcd[0]; return; }
-  if (alpha >= r.pa[n - 1]) { cl = r.pcl[n - 1]; cd = r.pcd[n - 1]; return; }
+  const double *pcl = r.pcl.data() + (size_t)sec * n, *pcd = r.pcd.data() + (size_t)sec * n;
+  if (alpha <= r.pa[0]) { cl = pcl[0]; cd = pcd[0]; return; }
+  if (alpha >= r.pa[n - 1]) { cl = pcl[n - 1]; cd = pcd[n - 1]; return; }
   int m = 0;
   while (r.pa[m + 1] < alpha) ++m;
   const double t = (alpha - r.pa[m]) / (r.pa[m + 1] - r.pa[m]);
-  cl = r.pcl[m] + t * (r.pcl[m + 1] - r.pcl[m]);
-  cd = r.pcd[m] + t * (r.pcd[m + 1] - r.pcd[m]);
+  cl = pcl[m] + t * (pcl[m + 1] - pcl[m]);
+  cd = pcd[m] + t * (pcd[m + 1] - pcd[m]);
+}
+
+/* C_L, C_D of the station at radius rad: linear in the radius between the two nearby airfoil sections
+ * (reading S28), the first / last section's inside / outside of them */
+void polar_lookup(const gkso_ctx::Rotor &r, double rad, double alpha, double &cl, double &cd) {
+  const int ns = (int)r.sec_r.size();
+  if (ns <= 1 || rad <= r.sec_r[0]) { polar_lookup_section(r, 0, alpha, cl, cd); return; }
+  if (rad >= r.sec_r[ns - 1]) { polar_lookup_section(r, ns - 1, alpha, cl, cd); return; }
+  int m = 0;
+  while (r.sec_r[m + 1] < rad) ++m;
+  const double t = (rad - r.sec_r[m]) / (r.sec_r[m + 1] - r.sec_r[m]);
+  double cl0, cd0, cl1, cd1;
+  polar_lookup_section(r, m, alpha, cl0, cd0);
+  polar_lookup_section(r, m + 1, alpha, cl1, cd1);
+  cl = cl0 + t * (cl1 - cl0);
+  cd = cd0 + t * (cd1 - cd0);
 }
 
 /* Eq. 14: f_tip = 2/pi acos(exp(-g1 N (R - r)/(2 r sin phi))), g1 = exp(-c1 (N lambda - c2)) + 0.1 */
@@ -730,32 +749,32 @@ double tip_factor(int N, double R, double r, double sinphi, double tsr, double c
 
 /* positions of the actuator points at the rotor's clock and the point forces ON THE FLUID.
  * Rotor axis +x; blade b at azimuth psi = theta0 + omega t + 2 pi b/N; radial unit (0, cos psi, sin psi),
- * rotational unit e_theta = (0, -sin psi, cos psi); station k at r = r_hub + (k + 1/2) w, w = (R - r_hub)/npts. */
+ * rotational unit e_theta = (0, -sin psi, cos psi); station k at r = r_hub + (k + 1/2) w, w = (R - r_hub)/npts, unless
+ * the caller gave radii and widths (S28). */
 void rotor_forces(const gkso_ctx &s, const std::vector<double> &Wp, std::vector<double> &pos,
                   std::vector<double> &force) {
   const gkso_ctx::Rotor &R = s.rotor;
   pos.assign(3 * (size_t)R.nb * R.np, 0.0);
   force.assign(3 * (size_t)R.nb * R.np, 0.0);
-  const double w = (R.R - R.rhub) / R.np;
   for (int b = 0; b < R.nb; ++b) {
     const double psi = R.theta0 + R.omega * R.time + 2.0 * PI * b / R.nb;
     const double er[3] = {0.0, std::cos(psi), std::sin(psi)}, et[3] = {0.0, -std::sin(psi), std::cos(psi)};
     for (int k = 0; k < R.np; ++k) {
       const size_t p = (size_t)b * R.np + k;
-      const double r = R.rhub + (k + 0.5) * w, c = R.chord[k];
+      const double r = R.radius[k], w = R.width[k], c = R.chord[k];   /* station radius, element width (S28) */
       double X[3], q[4];
       for (int a = 0; a < 3; ++a) X[a] = R.hub[a] + r * er[a];
       sample_trilinear(s, Wp, X, q);                         /* flow sampling */
       double Ux = q[1], Ut = q[2] * et[1] + q[3] * et[2];   /* U^2D = (U_x, U_theta) */
       double phi = std::atan2(Ux, R.omega * r - Ut);         /* flow angle between U_rel and the rotor plane */
       double cl, cd;
-      polar_lookup(R, phi - R.twist[k], cl, cd);             /* alpha = phi - gamma */
+      polar_lookup(R, r, phi - R.twist[k], cl, cd);          /* alpha = phi - gamma */
       if (R.fs_corr) { /* U_inf^2D = U^2D / (1 - C_D c /(4 sqrt(pi) eps)), then U_rel again */
         const double f = 1.0 / (1.0 - cd * c / (4.0 * std::sqrt(PI) * s.alm_eps));
         Ux *= f;
         Ut *= f;
         phi = std::atan2(Ux, R.omega * r - Ut);
-        polar_lookup(R, phi - R.twist[k], cl, cd);
+        polar_lookup(R, r, phi - R.twist[k], cl, cd);
       }
       const double urel2 = Ux * Ux + (Ut - R.omega * r) * (Ut - R.omega * r);
       const double L = 0.5 * q[0] * c * w * cl * urel2, D = 0.5 * q[0] * c * w * cd * urel2; /* Eq. 9 */
@@ -1159,6 +1178,15 @@ int gkso_alm_set_rotor(gkso_ctx *s, const gkso_rotor *r) {
   if (r->tip_correction && !(r->u_ref > 0)) return fail("rotor: the tip correction needs u_ref > 0 (tip speed ratio)");
   for (int m = 1; m < r->npolar; ++m)
     if (!(r->alpha[m] > r->alpha[m - 1])) return fail("rotor: polar angles must increase");
+  if ((r->radius == nullptr) != (r->width == nullptr)) return fail("rotor: radius and width come together");
+  if (r->radius)
+    for (int k = 0; k < r->npts; ++k)
+      if (!(r->radius[k] > 0) || !(r->radius[k] <= r->R) || !(r->width[k] > 0)) return fail("rotor: need 0 < radius <= R and width > 0");
+  if (r->nsections > 1) {
+    if (!r->section_r) return fail("rotor: section radii missing");
+    for (int m = 1; m < r->nsections; ++m)
+      if (!(r->section_r[m] > r->section_r[m - 1])) return fail("rotor: section radii must increase");
+  }
   for (int a = 0; a < 3; ++a) {
     const Axis &A = s->ax[a];
     if (A.periodic && 2.0 * s->alm_cut * r->eps > A.len()) return fail("alm: support wider than a periodic axis");
@@ -1171,9 +1199,19 @@ int gkso_alm_set_rotor(gkso_ctx *s, const gkso_rotor *r) {
   R.fs_corr = r->freestream_correction; R.tip_corr = r->tip_correction;
   R.chord.assign(r->chord, r->chord + r->npts);
   R.twist.assign(r->twist, r->twist + r->npts);
+  const int ns = r->nsections > 1 ? r->nsections : 1;
   R.pa.assign(r->alpha, r->alpha + r->npolar);
-  R.pcl.assign(r->cl, r->cl + r->npolar);
-  R.pcd.assign(r->cd, r->cd + r->npolar);
+  R.pcl.assign(r->cl, r->cl + (size_t)ns * r->npolar);
+  R.pcd.assign(r->cd, r->cd + (size_t)ns * r->npolar);
+  R.sec_r.clear();
+  if (ns > 1) R.sec_r.assign(r->section_r, r->section_r + ns);
+  R.radius.resize(r->npts);
+  R.width.resize(r->npts);
+  for (int k = 0; k < r->npts; ++k) {
+    const double w = (r->R - r->r_hub) / r->npts;
+    R.radius[k] = r->radius ? r->radius[k] : r->r_hub + (k + 0.5) * w;
+    R.width[k] = r->width ? r->width[k] : w;
+  }
   s->alm_eps = r->eps;
   s->n_alm = 0;
   return 0;

@@ -73,6 +73,16 @@ typedef struct {
   const double *alpha, *cl, *cd;       /* tabulated 2-D airfoil data, alpha [rad] increasing */
   int freestream_correction;           /* U_inf^2D = U^2D / (1 - C_D c/(4 sqrt(pi) eps)) */
   int tip_correction;                  /* Eq. 14, (c1, c2) = (0.1219, 21.52) axial, (0.0984, 13.026) tangential */
+  /* optional refinements, reading S28 (NULL / 0: the even stations and the single polar above):
+     radius, width: npts each - station radii r_k and element widths w_k of Eq. 9, for actuator points "locally refined
+       at the tip and root of the blade";
+     nsections > 1: cl and cd hold nsections tables of npolar values each, [section][alpha], of airfoil sections at the
+       radii section_r[] (increasing); C_L, C_D at a station are linear in r between the two nearby sections ("the
+       interpolation of the lift and drag tables between nearby airfoil sections"), the first / last
+       section's inside / outside of them */
+  const double *radius, *width;
+  int nsections;
+  const double *section_r;
 } gkso_rotor;
 int gkso_alm_set_rotor(gkso_ctx *ctx, const gkso_rotor *rotor);
 int gkso_alm_rotor_eval(gkso_ctx *ctx, double *pos, double *force); /* test hook: nblades*npts*3 each */

@@ -86,21 +86,43 @@ class Rotor:
     cd: np.ndarray
     freestream_correction: bool = False
     tip_correction: bool = False
+    # optional (reading S28): explicit stations - radii and element widths, (npts,) each - and airfoil sections:
+    # section_r (nsec,) increasing, then cl and cd are (nsec, npolar) and are blended linearly in r
+    radius: Optional[np.ndarray] = None
+    width: Optional[np.ndarray] = None
+    section_r: Optional[np.ndarray] = None
 
 
-def synthetic_rotor(hub, R, eps, u_ref=U_INF, tsr=7.0, nblades=3, npts=64, seed=20260314, **switches):
+def synthetic_rotor(hub, R, eps, u_ref=U_INF, tsr=7.0, nblades=3, npts=64, seed=20260314, refine=False, nsections=1,
+                    **switches):
     """A seeded stand-in for the paper's blade data (NREL 5 MW / NTNU tables are not available): tapered
-    chord, twist falling from root to tip, and a smooth polar with a linear range, stall and a drag bucket."""
+    chord, twist falling from root to tip, and a smooth polar with a linear range, stall and a drag bucket.
+    refine: stations clustered at the root and the tip instead of evenly spaced; nsections > 1:
+    that many airfoil sections between root and tip, thicker (less lift slope, more drag) towards the root."""
     rng = np.random.default_rng(seed)
-    s = (np.arange(npts) + 0.5) / npts
+    r_hub = 0.05 * R
+    if refine:
+        edges = r_hub + (R - r_hub) * 0.5 * (1.0 - np.cos(np.pi * np.arange(npts + 1) / npts))
+        radius, width = 0.5 * (edges[:-1] + edges[1:]), np.diff(edges)
+        s = (radius - r_hub) / (R - r_hub)
+    else:
+        radius = width = None
+        s = (np.arange(npts) + 0.5) / npts
     chord = R * (0.09 - 0.055 * s) * (1.0 + 0.03 * rng.standard_normal(npts))
     twist = np.deg2rad(14.0 * (1.0 - s) ** 1.5 - 1.0 + 0.2 * rng.standard_normal(npts))
     alpha = np.deg2rad(np.linspace(-30.0, 40.0, 71))
     a_st = np.deg2rad(13.0)
     cl = 2 * np.pi * 0.9 * a_st * np.tanh(alpha / a_st) * (1.0 - 0.25 * np.clip((np.abs(alpha) - a_st) / a_st, 0, 1))
     cd = 0.008 + 0.9 * np.sin(alpha) ** 2
-    return Rotor(nblades=nblades, npts=npts, hub=tuple(hub), R=R, r_hub=0.05 * R, omega=tsr * u_ref / R, theta0=0.1,
-                 u_ref=u_ref, eps=eps, chord=chord, twist=twist, alpha=alpha, cl=cl, cd=cd, **switches)
+    section_r = None
+    if nsections > 1:
+        section_r = r_hub + (R - r_hub) * (np.arange(nsections) + 0.5) / nsections
+        thick = np.linspace(1.0, 0.0, nsections)[:, None]           # 1 at the root section, 0 at the tip section
+        cl = cl[None, :] * (1.0 - 0.35 * thick)
+        cd = cd[None, :] * (1.0 + 1.5 * thick) + 0.004 * thick
+    return Rotor(nblades=nblades, npts=npts, hub=tuple(hub), R=R, r_hub=r_hub, omega=tsr * u_ref / R, theta0=0.1,
+                 u_ref=u_ref, eps=eps, chord=chord, twist=twist, alpha=alpha, cl=cl, cd=cd, radius=radius, width=width,
+                 section_r=section_r, **switches)
 
 
 # ----------------------------------------------------------------------------------------------

@@ -945,3 +945,69 @@ def test_P23_the_mirrored_problem_gives_the_mirrored_result(bc, with_ibm):
         Wb = flip(solve((yf[-1] - yf)[::-1] if a == 1 else yf, bcm, inflm, flip(W0), mirror(alm_pos),
                         alm_force * sign[1:], mirror(ibm_pos)))
         assert np.abs(Wa - Wb).max() < TOL_SYMMETRY, a
+
+
+# ---------------------------------------------------------------- P24 stations and airfoil sections (reading S28)
+def test_P24_explicit_stations_and_section_blended_polars():
+    """PAPER.md:376 (actuator points refined at tip and root) and :127 (lift and drag tables interpolated between nearby
+    airfoil sections).  Pinned on special cases that reduce to the single-table, evenly spaced rotor of P17 and on the
+    linearity of Eq. 9 in the element width and in the tabulated coefficients."""
+    from dataclasses import replace
+    cfg, r = rotor_case()
+    rng = np.random.default_rng(5)
+    W = const_state(cfg.n, (1.05, 0.1, 0.01, -0.02))
+    W += 1e-3 * rng.standard_normal(W.shape) * np.array([1.0, 0.1, 0.1, 0.1])[:, None, None, None]
+
+    def forces(rot):
+        o = ob.Oracle(cfg)
+        o.set_state(W)
+        o.alm_set_rotor(rot)
+        out = o.alm_rotor_eval()
+        o.close()
+        return out
+
+    p0, f0 = forces(r)
+    w = (r.R - r.r_hub) / r.npts
+    even_r, even_w = r.r_hub + (np.arange(r.npts) + 0.5) * w, np.full(r.npts, w)
+    # (i) the default stations given explicitly: the same bits
+    p1, f1 = forces(replace(r, radius=even_r, width=even_w))
+    assert np.array_equal(p1, p0) and np.array_equal(f1, f0)
+    # (ii) Eq. 9 is linear in the element width w: doubling the width of station 5 doubles its force and no other
+    w2 = even_w.copy()
+    w2[5] *= 2.0
+    _, f2 = forces(replace(r, radius=even_r, width=w2))
+    f0b, f2b = f0.reshape(r.nblades, r.npts, 3), f2.reshape(r.nblades, r.npts, 3)
+    assert np.array_equal(f2b[:, 5], 2.0 * f0b[:, 5]) and np.array_equal(np.delete(f2b, 5, 1), np.delete(f0b, 5, 1))
+    # (iii) the points sit at the given radii on the blade's azimuth (refined stations of the synthetic recipe)
+    rr = wl.synthetic_rotor(hub=r.hub, R=r.R, eps=r.eps, npts=r.npts, refine=True)
+    assert rr.width.sum() == pytest.approx(r.R - r.r_hub, rel=1e-14) and rr.width[0] < 0.3 * rr.width[r.npts // 2]
+    p3, _ = forces(rr)
+    d = p3 - np.asarray(r.hub)
+    assert np.allclose(np.hypot(d[:, 1], d[:, 2]).reshape(r.nblades, r.npts), rr.radius[None, :], rtol=1e-14)
+    assert np.allclose(np.arctan2(d[:, 2], d[:, 1]).reshape(r.nblades, r.npts)[0], r.theta0)
+    # (iv) airfoil sections.  Two identical sections are the single table ...
+    two = replace(r, cl=np.stack([r.cl, r.cl]), cd=np.stack([r.cd, r.cd]), section_r=np.array([0.3, 0.8]))
+    assert np.array_equal(forces(two)[1], f0)
+    # ... inside the first / outside the last section their own tables act, and between them C_L and C_D are linear in
+    # r, i.e. (both look-ups being linear in the table values) the force of a station is the one a single table
+    # blended with the same weight gives
+    clb, cdb = 0.6 * r.cl + 0.1, 1.7 * r.cd + 0.01
+    sec = np.array([even_r[4], even_r[10]])                                  # sections AT stations 4 and 10
+    mixed = replace(r, cl=np.stack([r.cl, clb]), cd=np.stack([r.cd, cdb]), section_r=sec)
+    fm = forces(mixed)[1].reshape(r.nblades, r.npts, 3)
+    fa = f0b
+    fb = forces(replace(r, cl=clb, cd=cdb))[1].reshape(r.nblades, r.npts, 3)
+    assert np.array_equal(fm[:, :5], fa[:, :5]) and np.array_equal(fm[:, 10:], fb[:, 10:])
+    for k in range(5, 10):
+        t = (even_r[k] - sec[0]) / (sec[1] - sec[0])
+        fk = forces(replace(r, cl=(1 - t) * r.cl + t * clb, cd=(1 - t) * r.cd + t * cdb))[1].reshape(r.nblades, r.npts, 3)
+        assert np.abs(fm[:, k] - fk[:, k]).max() <= 1e-14 * np.abs(fk[:, k]).max(), k
+    assert np.abs(fm[:, 7] - fa[:, 7]).max() > 1e-3 * np.abs(fa[:, 7]).max()     # the blend does change the force
+    # refusals: radius without width, decreasing section radii, a station beyond the tip
+    o = ob.Oracle(cfg)
+    o.set_state(W)
+    for bad in (replace(r, radius=even_r), replace(mixed, section_r=sec[::-1].copy()),
+                replace(r, radius=even_r * 2.0, width=even_w)):
+        with pytest.raises(Exception):
+            o.alm_set_rotor(bad)
+    o.close()
