@@ -175,7 +175,7 @@ gks_status alm_set_points(gks_ctx *ctx, int n, const double *pos, const double *
 
 /* On-line actuator-line rotor (Eq. 9, Eq. 14; S26-S27): instead of prescribed point
  * forces, every gks_step (i) places nblades*npts actuator points - rotor axis +x, blade b at azimuth
- * theta0 + omega t + 2 pi b/nblades, station k at r_hub + (k+1/2)(R - r_hub)/npts, t = the rotor clock, 0 at this
+ * theta0 + omega t + 2 pi b/nblades, station k at r_hub + (k+1/2)(R - r_hub)/npts (or at radius[k]), t = the rotor clock, 0 at this
  * call and advanced by dt per step -, (ii) samples (rho, U) of the un-forced W^{n+1} at the points by trilinear
  * interpolation, (iii) evaluates lift and drag (Eq. 9) from the tabulated polar at alpha = phi - twist,
  * phi = atan2(U_x, omega r - U_theta), optionally with the free-stream correction of PAPER.md:107 and the tip
@@ -191,6 +191,16 @@ typedef struct {
   int npolar;
   const double *alpha, *cl, *cd;
   int freestream_correction, tip_correction;
+  /* optional refinements, S28 (NULL / 0: the even stations and the single polar above).
+     radius, width: npts each - station radii r_k (0 < r_k <= R) and element widths w_k of Eq. 9, for actuator points
+       "locally refined at the tip and root of the blade"; they come together.
+     nsections > 1 (<= 16, nsections * npolar <= 4096): cl and cd hold nsections tables of npolar values each,
+       [section][alpha], of airfoil sections at the radii section_r[] (increasing); C_L, C_D at a station are linear in r
+       between the two nearby sections ("the interpolation of the lift and drag tables between nearby airfoil sections",
+       PAPER.md:127), the first / last section's inside / outside of them. */
+  const double *radius, *width;
+  int nsections;
+  const double *section_r;
 } alm_rotor;
 gks_status alm_set_rotor(gks_ctx *ctx, const alm_rotor *rotor);
 /* Test hook: positions and forces ON THE FLUID (nblades*npts*3 doubles each, host or device) of the actuator

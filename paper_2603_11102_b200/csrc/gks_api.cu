@@ -113,7 +113,7 @@ Layout make_layout(const gks_config *c) {
   L.off_red = take(2048);
   L.off_alm_pos = take(3 * (size_t)GKS_MAX_ALM_POINTS);
   L.off_alm_force = take(3 * (size_t)GKS_MAX_ALM_POINTS);
-  L.off_rotor = take(2 * (size_t)GKS_MAX_ROTOR_STATIONS + 3 * (size_t)GKS_MAX_POLAR);
+  L.off_rotor = take((size_t)GKS_ROTOR_TAB_DOUBLES);
   L.off_rotor_out = take(6 * (size_t)GKS_MAX_ALM_POINTS);
   /* IBM capacity: one point per 8 cells, at least 65536, at most GKS_MAX_IBM_POINTS */
   size_t cap = (size_t)c->nx * c->ny * c->nz / 8;

@@ -464,8 +464,10 @@ gks_status alm_set_points(gks_ctx *ctx, int n, const double *pos, const double *
 namespace {
 /* validate a rotor description, copy its tables to the device and fill the kernel's view of it */
 gks_status upload_rotor(gks_ctx *ctx, const alm_rotor *r, GksRotor &R) {
+  const int ns = r->nsections > 1 ? r->nsections : 1;
   if (r->nblades < 1 || r->npts < 1 || r->npts > GKS_MAX_ROTOR_STATIONS || r->npolar < 2 || r->npolar > GKS_MAX_POLAR ||
-      (long long)r->nblades * r->npts > GKS_MAX_ALM_POINTS)
+      (long long)r->nblades * r->npts > GKS_MAX_ALM_POINTS || ns > GKS_MAX_SECTIONS ||
+      (long long)ns * r->npolar > 4 * GKS_MAX_POLAR)
     return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "rotor: sizes out of range");
   if (!r->chord || !r->twist || !r->alpha || !r->cl || !r->cd) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "rotor: NULL table");
   if (!(r->R > r->r_hub) || !(r->r_hub >= 0) || !(r->eps > 0) || !std::isfinite(r->R) || !std::isfinite(r->eps) ||
@@ -473,25 +475,46 @@ gks_status upload_rotor(gks_ctx *ctx, const alm_rotor *r, GksRotor &R) {
     return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "rotor: need R > r_hub >= 0, eps > 0 and finite parameters");
   if (r->tip_correction && !(r->u_ref > 0))
     return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "rotor: the tip correction needs u_ref > 0 (tip speed ratio)");
-  std::vector<double> t[5];
-  const double *src[5] = {r->chord, r->twist, r->alpha, r->cl, r->cd};
-  const size_t cnt5[5] = {(size_t)r->npts, (size_t)r->npts, (size_t)r->npolar, (size_t)r->npolar, (size_t)r->npolar};
-  for (int q = 0; q < 5; ++q)
-    if (gks_status st = fetch_host(ctx, src[q], cnt5[q], t[q])) return st;
+  if ((r->radius == nullptr) != (r->width == nullptr))
+    return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "rotor: radius and width come together");
+  if (ns > 1 && !r->section_r) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "rotor: section radii missing");
+  /* tables on the host: chord, twist, radius, width, alpha, cl, cd, section radii */
+  enum { CHORD, TWIST, RADIUS, WIDTH, ALPHA, CL, CD, SECR, NT };
+  std::vector<double> t[NT];
+  const double *src[NT] = {r->chord, r->twist, r->radius, r->width, r->alpha, r->cl, r->cd, ns > 1 ? r->section_r : nullptr};
+  const size_t cnt[NT] = {(size_t)r->npts, (size_t)r->npts, (size_t)r->npts, (size_t)r->npts, (size_t)r->npolar,
+                          (size_t)ns * r->npolar, (size_t)ns * r->npolar, ns > 1 ? (size_t)ns : 0};
+  for (int q = 0; q < NT; ++q)
+    if (src[q])
+      if (gks_status st = fetch_host(ctx, src[q], cnt[q], t[q])) return st;
+  if (!r->radius) { /* the default stations: r_hub + (k + 1/2) w, w = (R - r_hub) / npts */
+    const double w = (r->R - r->r_hub) / r->npts;
+    t[RADIUS].resize(r->npts);
+    t[WIDTH].assign(r->npts, w);
+    for (int k = 0; k < r->npts; ++k) t[RADIUS][k] = r->r_hub + (k + 0.5) * w;
+  }
+  for (int k = 0; k < r->npts; ++k)
+    if (!(t[RADIUS][k] > 0) || !(t[RADIUS][k] <= r->R) || !(t[WIDTH][k] > 0))
+      return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "rotor: need 0 < radius <= R and width > 0 at every station");
   for (int m = 1; m < r->npolar; ++m)
-    if (!(t[2][m] > t[2][m - 1])) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "rotor: polar angles must increase");
-  const size_t off[5] = {0, GKS_MAX_ROTOR_STATIONS, 2 * GKS_MAX_ROTOR_STATIONS, 2 * GKS_MAX_ROTOR_STATIONS + GKS_MAX_POLAR,
-                         2 * GKS_MAX_ROTOR_STATIONS + 2 * GKS_MAX_POLAR};
-  for (int q = 0; q < 5; ++q)
-    CUDA_TRY(ctx, cudaMemcpyAsync(ctx->rotor_tab + off[q], t[q].data(), cnt5[q] * sizeof(double), cudaMemcpyHostToDevice,
-                                  ctx->stream));
+    if (!(t[ALPHA][m] > t[ALPHA][m - 1])) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "rotor: polar angles must increase");
+  for (int m = 1; m < ns; ++m)
+    if (!(t[SECR][m] > t[SECR][m - 1])) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "rotor: section radii must increase");
+  const size_t S = GKS_MAX_ROTOR_STATIONS, P = GKS_MAX_POLAR;
+  const size_t off[NT] = {0, S, 2 * S, 3 * S, 4 * S, 4 * S + P, 4 * S + 5 * P, 4 * S + 9 * P};
+  for (int q = 0; q < NT; ++q)
+    if (!t[q].empty())
+      CUDA_TRY(ctx, cudaMemcpyAsync(ctx->rotor_tab + off[q], t[q].data(), t[q].size() * sizeof(double),
+                                    cudaMemcpyHostToDevice, ctx->stream));
   CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));   /* the staging vectors go out of scope */
-  R.nb = r->nblades; R.np = r->npts; R.npolar = r->npolar;
+  R.nb = r->nblades; R.np = r->npts; R.npolar = r->npolar; R.nsec = ns;
   R.fs_corr = r->freestream_correction != 0; R.tip_corr = r->tip_correction != 0;
   for (int a = 0; a < 3; ++a) R.hub[a] = r->hub[a];
   R.R = r->R; R.rhub = r->r_hub; R.omega = r->omega; R.theta0 = r->theta0; R.uref = r->u_ref;
-  R.chord = ctx->rotor_tab + off[0]; R.twist = ctx->rotor_tab + off[1]; R.alpha = ctx->rotor_tab + off[2];
-  R.cl = ctx->rotor_tab + off[3]; R.cd = ctx->rotor_tab + off[4];
+  R.chord = ctx->rotor_tab + off[CHORD]; R.twist = ctx->rotor_tab + off[TWIST];
+  R.radius = ctx->rotor_tab + off[RADIUS]; R.width = ctx->rotor_tab + off[WIDTH];
+  R.alpha = ctx->rotor_tab + off[ALPHA]; R.cl = ctx->rotor_tab + off[CL]; R.cd = ctx->rotor_tab + off[CD];
+  R.sec_r = ctx->rotor_tab + off[SECR];
   return GKS_OK;
 }
 } /* namespace */

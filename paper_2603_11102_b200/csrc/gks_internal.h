@@ -52,12 +52,15 @@ struct GksPhys {
 
 /* on-line actuator-line rotor handed to the kernel by value; table pointers are device memory */
 struct GksRotor {
-  int nb, np, npolar, fs_corr, tip_corr;
+  int nb, np, npolar, fs_corr, tip_corr, nsec;
   double hub[3], R, rhub, omega, theta0, uref;
-  const double *chord, *twist, *alpha, *cl, *cd;
+  const double *chord, *twist, *radius, *width;   /* np each; radius / width always filled (even spacing by default) */
+  const double *alpha, *cl, *cd, *sec_r;          /* alpha npolar; cl, cd [nsec][npolar]; sec_r nsec */
 };
 #define GKS_MAX_ROTOR_STATIONS 4096
 #define GKS_MAX_POLAR 1024
+#define GKS_MAX_SECTIONS 16                        /* nsections * npolar <= GKS_MAX_SECTIONS * GKS_MAX_POLAR / 4 */
+#define GKS_ROTOR_TAB_DOUBLES (4 * GKS_MAX_ROTOR_STATIONS + GKS_MAX_POLAR + 2 * 4 * GKS_MAX_POLAR + GKS_MAX_SECTIONS)
 
 struct gks_ctx {
   gks_config cfg;
@@ -102,7 +105,8 @@ struct gks_ctx {
   int rotor_external;          /* sub-domain: this step's actuator points were supplied with alm_rotor_supply */
   double rotor_time;           /* rotor clock: 0 at alm_set_rotor, + dt per step */
   double *rotor_out;           /* device scratch of alm_rotor_points: pos, force (GKS_MAX_ALM_POINTS*3 each) */
-  double *rotor_tab;           /* device: chord, twist (GKS_MAX_ROTOR_STATIONS each), alpha, cl, cd (GKS_MAX_POLAR each) */
+  double *rotor_tab;           /* device: chord, twist, radius, width (GKS_MAX_ROTOR_STATIONS each), alpha (GKS_MAX_POLAR),
+                                  cl, cd (4 GKS_MAX_POLAR each: all sections), section radii: GKS_ROTOR_TAB_DOUBLES */
   int n_ibm;
   int ibm_maxit;               /* multi-direct-forcing passes per step (1 = single pass) */
   double ibm_tol;              /* stop once max_p |v_p - U_p| < tol, from the second pass on */

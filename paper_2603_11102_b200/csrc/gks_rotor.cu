@@ -72,19 +72,39 @@ __device__ void sample_trilinear(const GksGrid &g, const double *__restrict__ W,
       }
 }
 
-/* tabulated 2-D airfoil data: linear in alpha, end values beyond the table (binary search) */
-__device__ void polar_lookup(const GksRotor &r, double alpha, double &cl, double &cd) {
+/* tabulated 2-D airfoil data of one airfoil section: linear in alpha, end values beyond the table (binary search) */
+__device__ void polar_lookup_section(const GksRotor &r, int sec, double alpha, double &cl, double &cd) {
   const int n = r.npolar;
-  if (alpha <= r.alpha[0]) { cl = r.cl[0]; cd = r.cd[0]; return; }
-  if (alpha >= r.alpha[n - 1]) { cl = r.cl[n - 1]; cd = r.cd[n - 1]; return; }
+  const double *tcl = r.cl + (size_t)sec * n, *tcd = r.cd + (size_t)sec * n;
+  if (alpha <= r.alpha[0]) { cl = tcl[0]; cd = tcd[0]; return; }
+  if (alpha >= r.alpha[n - 1]) { cl = tcl[n - 1]; cd = tcd[n - 1]; return; }
   int lo = 0, hi = n - 1;                 /* alpha[lo] < alpha <= alpha[hi] */
   while (hi - lo > 1) {
     const int mid = (lo + hi) >> 1;
     if (r.alpha[mid] < alpha) lo = mid; else hi = mid;
   }
   const double t = (alpha - r.alpha[lo]) / (r.alpha[lo + 1] - r.alpha[lo]);
-  cl = r.cl[lo] + t * (r.cl[lo + 1] - r.cl[lo]);
-  cd = r.cd[lo] + t * (r.cd[lo + 1] - r.cd[lo]);
+  cl = tcl[lo] + t * (tcl[lo + 1] - tcl[lo]);
+  cd = tcd[lo] + t * (tcd[lo + 1] - tcd[lo]);
+}
+
+/* C_L, C_D of the station at radius rad (S28): linear in r between the two nearby airfoil
+ * sections, the first / last section's inside / outside of them; one section: its table */
+__device__ void polar_lookup(const GksRotor &r, double rad, double alpha, double &cl, double &cd) {
+  const int ns = r.nsec;
+  if (ns <= 1 || rad <= r.sec_r[0]) { polar_lookup_section(r, 0, alpha, cl, cd); return; }
+  if (rad >= r.sec_r[ns - 1]) { polar_lookup_section(r, ns - 1, alpha, cl, cd); return; }
+  int lo = 0, hi = ns - 1;                /* sec_r[lo] < rad <= sec_r[hi] */
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if (r.sec_r[mid] < rad) lo = mid; else hi = mid;
+  }
+  const double t = (rad - r.sec_r[lo]) / (r.sec_r[lo + 1] - r.sec_r[lo]);
+  double cl0, cd0, cl1, cd1;
+  polar_lookup_section(r, lo, alpha, cl0, cd0);
+  polar_lookup_section(r, lo + 1, alpha, cl1, cd1);
+  cl = cl0 + t * (cl1 - cl0);
+  cd = cd0 + t * (cd1 - cd0);
 }
 
 /* Eq. 14 */
@@ -101,8 +121,7 @@ __global__ void __launch_bounds__(128) k_rotor_forces(GksGrid g, const double *_
   const int p = blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= R.nb * R.np) return;
   const int b = p / R.np, k = p - b * R.np;
-  const double w = (R.R - R.rhub) / R.np;
-  const double r = R.rhub + (k + 0.5) * w, c = R.chord[k];
+  const double r = R.radius[k], w = R.width[k], c = R.chord[k];   /* station radius and element width (S28) */
   const double psi = R.theta0 + R.omega * time + 2.0 * PI_D * b / R.nb;
   double sp, cp;
   sincos(psi, &sp, &cp);
@@ -114,13 +133,13 @@ __global__ void __launch_bounds__(128) k_rotor_forces(GksGrid g, const double *_
   double Ux = q[1], Ut = q[2] * et[1] + q[3] * et[2];
   double phi = atan2(Ux, R.omega * r - Ut);
   double cl, cd;
-  polar_lookup(R, phi - R.twist[k], cl, cd);
+  polar_lookup(R, r, phi - R.twist[k], cl, cd);
   if (R.fs_corr) {
     const double f = 1.0 / (1.0 - cd * c / (4.0 * sqrt(PI_D) * eps));
     Ux *= f;
     Ut *= f;
     phi = atan2(Ux, R.omega * r - Ut);
-    polar_lookup(R, phi - R.twist[k], cl, cd);
+    polar_lookup(R, r, phi - R.twist[k], cl, cd);
   }
   const double urel2 = Ux * Ux + (Ut - R.omega * r) * (Ut - R.omega * r);
   const double L = 0.5 * q[0] * c * w * cl * urel2, D = 0.5 * q[0] * c * w * cd * urel2;

@@ -31,7 +31,8 @@ class AlmRotor(C.Structure):
                 ("R", C.c_double), ("r_hub", C.c_double), ("omega", C.c_double), ("theta0", C.c_double),
                 ("u_ref", C.c_double), ("eps", C.c_double), ("chord", _dp), ("twist", _dp),
                 ("npolar", C.c_int), ("alpha", _dp), ("cl", _dp), ("cd", _dp),
-                ("freestream_correction", C.c_int), ("tip_correction", C.c_int)]
+                ("freestream_correction", C.c_int), ("tip_correction", C.c_int),
+                ("radius", _dp), ("width", _dp), ("nsections", C.c_int), ("section_r", _dp)]
 
 
 class GksConfig(C.Structure):
@@ -275,6 +276,15 @@ class Gks:
         c.chord, c.twist, c.alpha, c.cl, c.cd = [x.ctypes.data_as(_dp) for x in keep]
         c.npolar = len(keep[2])
         c.freestream_correction, c.tip_correction = int(r.freestream_correction), int(r.tip_correction)
+        if getattr(r, "radius", None) is not None or getattr(r, "width", None) is not None:
+            for name in ("radius", "width"):             # the library refuses one without the other
+                v = getattr(r, name, None)
+                if v is not None:
+                    keep.append(np.ascontiguousarray(np.asarray(v, dtype=np.float64)))
+                    setattr(c, name, keep[-1].ctypes.data_as(_dp))
+        if getattr(r, "section_r", None) is not None:
+            keep.append(np.ascontiguousarray(np.asarray(r.section_r, dtype=np.float64)))
+            c.nsections, c.section_r = len(keep[-1]), keep[-1].ctypes.data_as(_dp)
         return c, keep
 
     def alm_set_rotor(self, r):

@@ -262,10 +262,12 @@ def test_cfl_dt_matches_the_oracle():
         o.close()
 
 
-@pytest.mark.parametrize("switches", [{}, {"freestream_correction": True, "tip_correction": True}])
+@pytest.mark.parametrize("switches", [{}, {"freestream_correction": True, "tip_correction": True},
+                                      {"refine": True, "nsections": 3, "freestream_correction": True, "tip_correction": True}])
 def test_online_rotor_matches_the_oracle(switches):
-    """actuator-line front half on the device (S26-S27): point positions and forces of the test hook, then 1 and
-    10 steps of the small rotor (C4) and turbine (C5: rotor + IBM nacelle and tower) boxes with the rotor on line"""
+    """actuator-line front half on the device (S26-S28): point positions and forces of the test hook, then 1 and
+    10 steps of the small rotor (C4) and turbine (C5: rotor + IBM nacelle and tower) boxes with the rotor on line;
+    third variant: stations refined at root and tip with their own widths, three airfoil sections blended in r"""
     from oracle import binding as ob
     from paper_2603_11102_b200 import gks
     for name in ("C4", "C5"):
@@ -301,6 +303,14 @@ def test_online_rotor_matches_the_oracle(switches):
     g = gks.Gks(wl.by_name("C4", small=True).cfg)
     bad = wl.synthetic_rotor(hub=(1, 1, 1), R=0.5, eps=0.1)
     bad.alpha = bad.alpha[::-1].copy()
+    with pytest.raises(gks.GksError):
+        g.alm_set_rotor(bad)
+    bad = wl.synthetic_rotor(hub=(1, 1, 1), R=0.5, eps=0.1, refine=True, nsections=3)
+    bad.width = None                                             # radius without width
+    with pytest.raises(gks.GksError):
+        g.alm_set_rotor(bad)
+    bad = wl.synthetic_rotor(hub=(1, 1, 1), R=0.5, eps=0.1, nsections=3)
+    bad.section_r = bad.section_r[::-1].copy()
     with pytest.raises(gks.GksError):
         g.alm_set_rotor(bad)
     g.alm_set_rotor(None)
