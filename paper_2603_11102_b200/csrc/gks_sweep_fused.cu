@@ -41,6 +41,9 @@
 #ifndef GKS_MIN_PPC
 #define GKS_MIN_PPC 2   /* remainder columns: fewest output planes per CTA (idle SMs are free; measured on C1-C3) */
 #endif
+#ifndef GKS_XHALF
+#define GKS_XHALF 1   /* 1: the 4x4 transposes go through the warp-private buffer two fields at a time (32 doubles per face) */
+#endif
 #ifndef GKS_E_WIDTH
 #define GKS_E_WIDTH 3   /* pass-2 evaluations written side by side: 2, 3 or 6 (measured: 3 is best for all three tile shapes) */
 #endif
@@ -145,7 +148,8 @@ struct Tile {
                                                               between the QL and QR rows of a face (stage BC) */
   static constexpr int OFF_S = OFF_W + 2 * WSLAB_PAD;      /* 3 stage buffers (plane j lives in buffer j % 3) */
   static constexpr int OFF_XB = OFF_S + 3 * SBUF;          /* transpose buffer, 64 doubles per face, XOR-swizzled */
-  static constexpr int OFF_RING = OFF_XB + NF * 64;        /* 4-plane ring of pass-1 results [4][6][NF][4] */
+  static constexpr int XF = GKS_XHALF ? 32 : 64;           /* doubles of the transpose buffer per face */
+  static constexpr int OFF_RING = OFF_XB + NF * XF;        /* 4-plane ring of pass-1 results [4][6][NF][4] */
   static constexpr int RING = 4 * 6 * NF * 4;
   static constexpr int OFF_BAR = OFF_RING + RING;          /* mbarriers: [0] first slab, [2] iteration barrier */
   static constexpr size_t SMEM_BYTES = (size_t)(OFF_BAR + 4) * 8;
@@ -292,8 +296,8 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
   /* transpose buffer: element (field, component cc, Gauss point gq) of face fid lives at
    * fid*64 + field*16 + 4*(cc ^ (fid&3)) + (gq ^ cc): conflict-free for the component-major writes
    * and for the Gauss-point-major reads of a half warp */
-  double *const xw = XBuf + fid * 64 + 4 * (c ^ (fid & 3));                /* writes: + field*16 + (gq ^ c) */
-  const double *const xr = XBuf + fid * 64;                                 /* reads:  + field*16 + ro[cc] */
+  double *const xw = XBuf + fid * T::XF + 4 * (c ^ (fid & 3));             /* writes: + field*16 + (gq ^ c) */
+  const double *const xr = XBuf + fid * T::XF;                              /* reads:  + field*16 + ro[cc] */
   int ro[4];
 #pragma unroll
   for (int cc = 0; cc < 4; ++cc) ro[cc] = 4 * (cc ^ (fid & 3)) + (c ^ cc);
@@ -512,6 +516,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
     /* the six evaluations (field Q0, Dn, Dt1) x (g1 = -, +) run EW at a time, statement-interleaved */
     constexpr int EW = GKS_E_WIDTH;
     static_assert(6 % EW == 0, "E width");
+    double late[8];                               /* GKS_XHALF: Dn and Dt1 at the 4 Gauss points */
 #pragma unroll
     for (int e0 = 0; e0 < 6; e0 += EW) {
       double qq[5][EW], vm[EW], vp[EW], sm_[EW], sp_[EW];
@@ -527,11 +532,16 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
 #pragma unroll
       for (int u = 0; u < EW; ++u) {              /* evaluation e = 2*fld + g1; Gauss point gq = 2*g1 + g2 */
         const int fld = (e0 + u) >> 1, g1 = (e0 + u) & 1;
-        xw[fld * 16 + ((2 * g1) ^ c)] = vm[u];
-        xw[fld * 16 + ((2 * g1 + 1) ^ c)] = vp[u];
+        if (GKS_XHALF && fld != 0) {              /* Dn and Dt1 wait in registers for the second round */
+          late[(fld - 1) * 4 + 2 * g1] = vm[u];
+          late[(fld - 1) * 4 + 2 * g1 + 1] = vp[u];
+        } else {
+          xw[fld * 16 + ((2 * g1) ^ c)] = vm[u];
+          xw[fld * 16 + ((2 * g1 + 1) ^ c)] = vp[u];
+        }
         if (fld == 0) {
-          xw[3 * 16 + ((2 * g1) ^ c)] = sm_[u] * iw2;
-          xw[3 * 16 + ((2 * g1 + 1) ^ c)] = sp_[u] * iw2;
+          xw[(GKS_XHALF ? 1 : 3) * 16 + ((2 * g1) ^ c)] = sm_[u] * iw2;
+          xw[(GKS_XHALF ? 1 : 3) * 16 + ((2 * g1 + 1) ^ c)] = sp_[u] * iw2;
         }
       }
     }
@@ -540,19 +550,41 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
     /* ---- F: flux at Gauss point gp = c of this face; sum over the 4 lanes; write ---- */
     {
       double Q0[4], dQ[3][4], F[4], dF[4];
+      if (GKS_XHALF) {
+        /* two rounds through 32 doubles per face: Q0 and Dt2 (complete after the first three evaluations), then Dn
+           and Dt1 */
 #pragma unroll
-      for (int cc = 0; cc < 4; ++cc) {
-        Q0[cc] = xr[0 * 16 + ro[cc]];
-        dQ[DIR][cc] = xr[1 * 16 + ro[cc]];
-        dQ[T::AXT1][cc] = xr[2 * 16 + ro[cc]];
-        dQ[T::AXM][cc] = xr[3 * 16 + ro[cc]];
+        for (int cc = 0; cc < 4; ++cc) {
+          Q0[cc] = xr[0 * 16 + ro[cc]];
+          dQ[T::AXM][cc] = xr[1 * 16 + ro[cc]];
+        }
+        __syncwarp();
+#pragma unroll
+        for (int gq = 0; gq < 4; ++gq) {
+          xw[0 * 16 + (gq ^ c)] = late[gq];
+          xw[1 * 16 + (gq ^ c)] = late[4 + gq];
+        }
+        __syncwarp();
+#pragma unroll
+        for (int cc = 0; cc < 4; ++cc) {
+          dQ[DIR][cc] = xr[0 * 16 + ro[cc]];
+          dQ[T::AXT1][cc] = xr[1 * 16 + ro[cc]];
+        }
+      } else {
+#pragma unroll
+        for (int cc = 0; cc < 4; ++cc) {
+          Q0[cc] = xr[0 * 16 + ro[cc]];
+          dQ[DIR][cc] = xr[1 * 16 + ro[cc]];
+          dQ[T::AXT1][cc] = xr[2 * 16 + ro[cc]];
+          dQ[T::AXM][cc] = xr[3 * 16 + ro[cc]];
+        }
       }
       gksd::gauss_point_flux<DIR, NEED_F>(Q0, dQ, ph.RT, ph.mu, F, dF);
       __syncwarp();                               /* every lane has consumed its reads: the buffer is reusable */
       /* face average: the 4 lanes of a face (one Gauss point each) leave their F, dF in the warp-private
          buffer, lane c sums component c in the order (g0+g1)+(g2+g3).  Row v of face fid sits at
          ((v ^ (fid&3)) * 4 + gp): conflict-free 64-bit stores and loads */
-      double *const xs = XBuf + fid * 64;
+      double *const xs = XBuf + fid * T::XF;
       const int f3 = fid & 3;
 #pragma unroll
       for (int v = 0; v < 4; ++v) {
