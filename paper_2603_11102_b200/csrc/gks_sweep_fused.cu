@@ -41,6 +41,10 @@
 #ifndef GKS_MIN_PPC
 #define GKS_MIN_PPC 2   /* remainder columns: fewest output planes per CTA (idle SMs are free; measured on C1-C3) */
 #endif
+#ifndef GKS_NF
+#define GKS_NF 128      /* faces per CTA tile: 128 = one CTA of 512 threads per SM; 64 = two CTAs of 256 threads per SM */
+#endif
+#define GKS_CTAS_PER_SM (128 / GKS_NF)
 #ifndef GKS_XHALF
 #define GKS_XHALF 1   /* 1: the 4x4 transposes go through the warp-private buffer two fields at a time (32 doubles per face) */
 #endif
@@ -153,7 +157,7 @@ struct Tile {
   static constexpr int RING = 4 * 6 * NF * 4;
   static constexpr int OFF_BAR = OFF_RING + RING;          /* mbarriers: [0] first slab, [2] iteration barrier */
   static constexpr size_t SMEM_BYTES = (size_t)(OFF_BAR + 4) * 8;
-  static_assert(SMEM_BYTES + 1024 <= 233472, "the CTA must fit in shared memory");
+  static_assert((SMEM_BYTES + 1024) * GKS_CTAS_PER_SM <= 233472, "the CTA(s) must fit in shared memory");
   static_assert(NT <= 1024 && NT % 32 == 0 && (NT & (NT - 1)) == 0, "whole warps, power of two");
 };
 
@@ -182,7 +186,7 @@ struct Seg {
  * straight-line block (GKS_FUSE_BCD): BC's serial chain issues in the shadow of D's arithmetic.
  */
 template <int DIR, bool NEED_F, bool LIN, int TA, int TB>
-__global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
+__global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
     k_sweep_fused(const __grid_constant__ CUtensorMap tmap, GksGrid g, GksPhys ph, double *__restrict__ flux,
                   int ncol_a, int nfull, long long rem, long long PPC, int ta0, int tlen0, int ta1) {
   using T = Tile<DIR, TA, TB>;
@@ -366,7 +370,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
       store(cn, ct, cc, vl[0], vr[0], gksd::normal_slope12(q[1][0], q[2][0], q[3][0], q[4][0]));
     };
     constexpr int NXA = NITEM - NT;
-    static_assert(NXA >= 0 && NXA <= NT / 2, "stage A: at most two items per thread, extras on half the CTA");
+    static_assert(NXA >= 0 && NXA <= NT, "stage A: at most two items per thread");
     const int xa_id = (tid - 32 * ((i * 5) % T::NW)) & (NT - 1);
     double a_vl[1], a_vr[1], a_dn = 0.0;
     int a_cn = 0, a_ct = 0, a_cc = 0;
@@ -418,7 +422,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, 1)
       static_assert((FH * 4) % 32 == 0, "whole warps in the collision stage");
       const int gl = (tid & 31) & ~3;               /* first lane of this face group */
       constexpr int NXB = FH * 4 - NT;              /* extra items: a rotating window of whole warps, disjoint from A's */
-      static_assert(NXB >= 0 && NXB <= NT / 4 && NXB % 32 == 0, "stage BC: extras on whole warps");
+      static_assert(NXB >= 0 && NXB <= NT / 2 && NXB % 32 == 0, "stage BC: extras on whole warps");
       const int xb_id = (tid - 32 * ((i * 5 + T::NW / 2) % T::NW)) & (NT - 1);
       auto collide = [&](int item) {
         const int cc = item & 3, fh = item >> 2, side = cc & 1, func = cc >> 1;
@@ -632,7 +636,7 @@ typedef CUresult (*encode_fn_t)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, 
 #define GKS_TILE_YZ_A 32
 #endif
 template <int DIR, int XA> struct Shape {
-  static constexpr int TA = DIR == 0 ? XA : GKS_TILE_YZ_A, TB = 128 / TA;
+  static constexpr int TA = DIR == 0 ? XA : GKS_TILE_YZ_A, TB = GKS_NF / TA;
 };
 inline int x_tile_a(const GksGrid &g) { return g.wrapf[0] ? 8 : 4; }
 
@@ -678,7 +682,7 @@ int launch_dir(gks_ctx *ctx, const CUtensorMap &map, double *flux, int ta0, int 
   /* persistent CTAs: the (column, plane) list is cut into equal contiguous ranges, one per resident CTA;
      a range shorter than 8 planes is not worth its 4 priming planes */
   const int ncols = ga * gb;
-  int grid = ctx->num_sms, nfull = ncols / grid;
+  int grid = ctx->num_sms * GKS_CTAS_PER_SM, nfull = ncols / grid;
   long long rem = (long long)(ncols - nfull * grid) * n2;      /* planes of the columns that do not fill a wave */
   long long PPC = (rem + grid - 1) / grid;
   if (PPC < GKS_MIN_PPC) PPC = GKS_MIN_PPC;                    /* shortest range worth its 4 priming planes */
