@@ -151,6 +151,22 @@ gks_status gks_step_finish_part(gks_ctx *ctx, double dt, int part);
 size_t gks_halo_doubles(const gks_ctx *ctx, int face);
 gks_status gks_halo_pack(gks_ctx *ctx, int which, int face, double *buf);
 gks_status gks_halo_unpack(gks_ctx *ctx, int which, int face, const double *buf);
+/* The exchange without buffers (one node: NVLink 5 / NVSwitch peer memory, or sub-domains that share a GPU).
+ * gks_halo_window_get(ctx, which, &w) describes where a neighbour may write this context's padded state `which`
+ * directly: device base pointer, extents and pitches.  gks_halo_push(ctx, which, face, &w_neighbour) writes the 3
+ * interior planes next to x face `face` of THIS context straight into the ghost planes beyond the OPPOSITE x face of
+ * the neighbour - pack, transfer and unpack in one kernel on this context's stream; with the neighbour on another GPU
+ * the stores travel peer to peer (the driver enables peer access or maps the window through CUDA IPC, and orders the
+ * neighbour's stream behind the push, e.g. with an event).  The window stays valid for the life of the neighbour's
+ * context.  Errors: GKS_ERR_INVALID_ARG (not a HALO x face, NULL, y / z extents differ), GKS_ERR_STATE (as gks_halo_pack). */
+typedef struct {
+  double *W;                       /* device: padded state [c][k][j][i], 3 ghost layers on every side */
+  int nx, ny, nz;                  /* interior cells of the neighbour */
+  int pitch_x, pitch_y;            /* padded row length (>= nx + 6) and rows per plane (ny + 6), in doubles / rows */
+  long long field_stride;          /* doubles between two components */
+} gks_halo_window;
+gks_status gks_halo_window_get(gks_ctx *ctx, int which, gks_halo_window *out);
+gks_status gks_halo_push(gks_ctx *ctx, int which, int face, const gks_halo_window *to);
 gks_status gks_step_begin(gks_ctx *ctx, double dt);
 gks_status gks_step_finish(gks_ctx *ctx, double dt);
 gks_status gks_step_force(gks_ctx *ctx, double dt);

@@ -342,6 +342,40 @@ gks_status gks_halo_unpack(gks_ctx *ctx, int which, int face, const double *buf)
   return halo_move(ctx, which, face, const_cast<double *>(buf), 1);
 }
 
+gks_status gks_halo_window_get(gks_ctx *ctx, int which, gks_halo_window *out) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (!out || (which != 0 && which != 1)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "out is NULL or which is not 0 / 1");
+  out->W = which == 0 ? ctx->Wn : ctx->Ws;
+  out->nx = ctx->g.n[0];
+  out->ny = ctx->g.n[1];
+  out->nz = ctx->g.n[2];
+  out->pitch_x = ctx->g.P[0];
+  out->pitch_y = ctx->g.P[1];
+  out->field_stride = ctx->g.FS;
+  return GKS_OK;
+}
+
+gks_status gks_halo_push(gks_ctx *ctx, int which, int face, const gks_halo_window *to) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  if (!to || !to->W) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "the neighbour's window is NULL");
+  if ((face != 0 && face != 1) || ctx->ph.bc[face] != GKS_BC_HALO)
+    return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "face %d is not a GKS_BC_HALO x face", face);
+  if (which != 0 && which != 1) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "which must be 0 (W^n) or 1 (W*)");
+  if (!ctx->have_state) return gks_set_err(ctx, GKS_ERR_STATE, "no state set");
+  if (which == 1 && ctx->mid_step != 1 && ctx->mid_step != 11)
+    return gks_set_err(ctx, GKS_ERR_STATE, "W* exists only between gks_step_begin and gks_step_finish");
+  if (which == 0 && ctx->mid_step == 11)
+    return gks_set_err(ctx, GKS_ERR_STATE, "between the two parts of gks_step_finish the buffer of W^n is half W^{n+1}");
+  if (to->ny != ctx->g.n[1] || to->nz != ctx->g.n[2] || to->nx < 6 || to->pitch_x < to->nx + 2 * GKS_NG ||
+      to->pitch_y != to->ny + 2 * GKS_NG)
+    return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "the neighbour's window does not match this sub-domain's y, z extents");
+  if (gks_status st = gks_check_device(ctx)) return st;
+  ctx->launches += gks_launch_halo_push(ctx->g, which == 0 ? ctx->Wn : ctx->Ws, face, to->W, to->nx, to->pitch_x,
+                                        to->pitch_y, to->field_stride, ctx->stream);
+  CUDA_TRY(ctx, cudaGetLastError());
+  return GKS_OK;
+}
+
 gks_status gks_set_body_force(gks_ctx *ctx, double gx, double gy, double gz) {
   if (!ctx) return GKS_ERR_INVALID_ARG;
   if (!std::isfinite(gx) || !std::isfinite(gy) || !std::isfinite(gz))

@@ -128,6 +128,22 @@ __global__ void __launch_bounds__(128) k_halo(GksGrid g, double *__restrict__ W,
   else buf[b] = W[id];
 }
 
+/* the 3 interior planes next to an x face of THIS context straight into the ghost planes beyond the opposite x face of
+ * a NEIGHBOUR's padded state (its window: base pointer, pitches, nx): pack, transfer and unpack in one kernel - the
+ * stores travel peer-to-peer when the window lives on another GPU of the NVSwitch domain */
+__global__ void __launch_bounds__(128) k_halo_push(GksGrid g, const double *__restrict__ W, int side, double *__restrict__ dstW,
+                                                   int dnx, int dPX, int dPY, long long dFS) {
+  gks_pdl_enter();
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  const int k = blockIdx.y;
+  const int layer = blockIdx.z % GKS_NG, c = blockIdx.z / GKS_NG;
+  if (j >= g.n[1] || k >= g.n[2]) return;
+  const int isrc = side == 0 ? layer : g.n[0] - GKS_NG + layer;
+  const int idst = side == 0 ? dnx + layer : -GKS_NG + layer;      /* my low face feeds the neighbour's HIGH ghosts */
+  const long long d = c * dFS + ((long long)(k + GKS_NG) * dPY + (j + GKS_NG)) * dPX + (idst + GKS_NG);
+  dstW[d] = W[c * g.FS + g.idx(isrc, j, k)];
+}
+
 __global__ void __launch_bounds__(256) k_pack(GksGrid g, double *__restrict__ Wint, double *__restrict__ Wpad,
                                               int to_padded, int ex, int ey, int ez) {
   gks_pdl_enter();
@@ -256,6 +272,13 @@ int gks_launch_halo(const GksGrid &g, double *W, double *buf, int face, int unpa
   if (ax == 0) gks_launch(k_halo<0>, grid, dim3(128), 0, s, g, W, buf, side, unpack);
   else if (ax == 1) gks_launch(k_halo<1>, grid, dim3(128), 0, s, g, W, buf, side, unpack);
   else gks_launch(k_halo<2>, grid, dim3(128), 0, s, g, W, buf, side, unpack);
+  return 1;
+}
+
+int gks_launch_halo_push(const GksGrid &g, const double *W, int side, double *dstW, int dnx, int dPX, int dPY,
+                         long long dFS, cudaStream_t s) {
+  dim3 grid((g.n[1] + 127) / 128, g.n[2], 4 * GKS_NG);
+  gks_launch(k_halo_push, grid, dim3(128), 0, s, g, W, side, dstW, dnx, dPX, dPY, dFS);
   return 1;
 }
 

@@ -205,6 +205,8 @@ int gks_launch_outflow_advance(const GksGrid &g, const GksPhys &ph, double *W, d
 int gks_launch_pack(const GksGrid &g, const double *Wint, double *Wpad, cudaStream_t s);
 int gks_launch_unpack(const GksGrid &g, const double *Wpad, double *Wint, cudaStream_t s);
 int gks_launch_halo(const GksGrid &g, double *W, double *buf, int face, int unpack, cudaStream_t s);
+int gks_launch_halo_push(const GksGrid &g, const double *W, int side, double *dstW, int dnx, int dPX, int dPY,
+                         long long dFS, cudaStream_t s);
 int gks_launch_unpack_faces(const GksGrid &g, int dir, const double *Fpad, double *Fout, cudaStream_t s);
 
 #ifdef GKS_DEBUG

@@ -21,7 +21,7 @@ STATUS = {0: "GKS_OK", 1: "GKS_ERR_INVALID_ARG", 2: "GKS_ERR_WORKSPACE", 3: "GKS
 EXPORTS = ["gks_workspace_bytes", "gks_create", "gks_destroy", "gks_set_state", "gks_get_state", "gks_step",
            "gks_set_body_force", "gks_set_bulk_flux", "alm_set_points", "ibm_set_points", "ibm_set_velocities", "ibm_set_iterations", "gks_cfl_dt", "alm_set_rotor", "alm_rotor_eval", "alm_rotor_points", "gks_set_reconstruction", "gks_halo_doubles", "gks_halo_pack", "gks_halo_unpack", "gks_step_begin",
            "gks_step_finish", "gks_step_force", "gks_bulk_partial", "gks_bulk_set_global", "gks_ibm_pass", "gks_ibm_residual",
-           "gks_debug_eval_flux", "alm_rotor_supply", "gks_step_begin_part", "gks_step_finish_part",
+           "gks_debug_eval_flux", "alm_rotor_supply", "gks_step_begin_part", "gks_step_finish_part", "gks_halo_window_get", "gks_halo_push",
            "gks_profile_enable", "gks_profile_read", "gks_check_finite", "gks_launch_count", "gks_last_error"]
 DEBUG_EXPORTS = ["gks_debug_set_sweep", "gks_debug_fp64_peak", "gks_debug_issue_probe", "gks_debug_trace"]    # include/gks_debug.h: libgks_b200_debug.so only
 
@@ -33,6 +33,11 @@ class AlmRotor(C.Structure):
                 ("npolar", C.c_int), ("alpha", _dp), ("cl", _dp), ("cd", _dp),
                 ("freestream_correction", C.c_int), ("tip_correction", C.c_int),
                 ("radius", _dp), ("width", _dp), ("nsections", C.c_int), ("section_r", _dp)]
+
+
+class HaloWindow(C.Structure):
+    _fields_ = [("W", C.c_void_p), ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("pitch_x", C.c_int),
+                ("pitch_y", C.c_int), ("field_stride", C.c_longlong)]
 
 
 class GksConfig(C.Structure):
@@ -86,6 +91,8 @@ def lib(debug=False):
         L.gks_halo_doubles.restype = C.c_size_t
         L.gks_halo_pack.argtypes = [vp, C.c_int, C.c_int, vp]
         L.gks_halo_unpack.argtypes = [vp, C.c_int, C.c_int, vp]
+        L.gks_halo_window_get.argtypes = [vp, C.c_int, C.POINTER(HaloWindow)]
+        L.gks_halo_push.argtypes = [vp, C.c_int, C.c_int, C.POINTER(HaloWindow)]
         L.gks_step_begin.argtypes = [vp, C.c_double]
         L.gks_step_finish.argtypes = [vp, C.c_double]
         L.gks_step_force.argtypes = [vp, C.c_double]
@@ -371,6 +378,16 @@ class Gks:
     def halo_unpack(self, which, face, buf):
         assert buf.is_contiguous() and buf.numel() == self.halo_doubles(face)
         self._c("gks_halo_unpack", int(which), int(face), buf.data_ptr())
+
+    def halo_window(self, which):
+        """where a neighbour may write this context's padded state `which` directly (gks_halo_push)"""
+        w = HaloWindow()
+        self._c("gks_halo_window_get", int(which), C.byref(w))
+        return w
+
+    def halo_push(self, which, face, window):
+        """my 3 interior planes next to `face` straight into the neighbour's ghost planes (its `halo_window`)"""
+        self._c("gks_halo_push", int(which), int(face), C.byref(window))
 
     def set_reconstruction(self, tangential_linear):
         self._c("gks_set_reconstruction", int(tangential_linear))

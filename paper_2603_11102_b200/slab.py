@@ -173,6 +173,19 @@ class LocalTransport:
             solvers[dst].halo_unpack(which, dst_face, buf)
 
 
+    def exchange_push(self, solvers, which):
+        """the exchange without buffers: every sub-domain writes its boundary planes straight into its neighbours'
+        ghost layers (gks_halo_push: pack, transfer and unpack in one kernel; peer-to-peer stores when the
+        neighbour's window lives on another GPU).  Streams are ordered on the host here; a multi-GPU driver would
+        record an event behind the push and let the neighbour's stream wait for it."""
+        for s in solvers:                         # the neighbours have finished reading the ghosts we overwrite
+            s.synchronize()
+        for r, s in enumerate(solvers):
+            for face, dst, dst_face in self.d.schedule(r):
+                s.halo_push(which, face, solvers[dst].halo_window(which))
+        for s in solvers:
+            s.synchronize()
+
     # the same exchange in two halves, for the overlapped step (nothing overlaps inside one process: the hand-over
     # is a pointer; the split is what is exercised)
     def exchange_begin(self, solvers, which, new_buffer):
@@ -439,14 +452,16 @@ class SlabStepper:
             for s in sols:
                 s.ibm_pass(k, 1)
 
-    def step(self, dt, before_forcing=None, ibm=False, rotor=None, bulk=False, ibm_passes=1, overlap=False):
+    def step(self, dt, before_forcing=None, ibm=False, rotor=None, bulk=False, ibm_passes=1, overlap=False, push=False):
         """before_forcing(solver): e.g. alm_set_points for this step (replicated point list);
         ibm: Lagrangian points are set (on any rank): the un-forced W^{n+1} is exchanged before the forcing;
         rotor: a RotorDriver (on-line actuator lines), evaluated on the un-forced W^{n+1} as well;
         bulk: the bulk-flux forcing is set: its global sum is assembled before the forcing;
         ibm_passes: the max_iter given to ibm_set_iterations on every sub-domain, when > 1;
         overlap: the halos of either stage travel while the stage's interior is swept (PAPER.md:193-197 exchanges per
-        flux evaluation; include/gks.h gks_step_begin_part): post, part 0, complete, part 1"""
+        flux evaluation; include/gks.h gks_step_begin_part): post, part 0, complete, part 1;
+        push: (sub-domains that can address one another's memory: LocalTransport) the two stage exchanges without
+        buffers, every sub-domain writing into its neighbours' ghost layers (gks_halo_push)"""
         if before_forcing is not None:
             self._each(before_forcing)
         if overlap:
@@ -458,6 +473,11 @@ class SlabStepper:
             self._each(lambda s: s.step_finish_part(dt, 0))
             self.t.exchange_end(self.solvers, 1, self.new_buffer)
             self._each(lambda s: s.step_finish_part(dt, 1))
+        elif push:
+            self.t.exchange_push(self.solvers, 0)                  # ghosts of W^n, written by the neighbours
+            self._each(lambda s: s.step_begin(dt))
+            self.t.exchange_push(self.solvers, 1)                  # ghosts of W*
+            self._each(lambda s: s.step_finish(dt))
         else:
             self.t.exchange(self.solvers, 0, self.new_buffer)      # ghosts of W^n
             self._each(lambda s: s.step_begin(dt))

@@ -11,7 +11,7 @@ from paper_2603_11102_b200 import slab, workloads as wl
 pytestmark = pytest.mark.gpu
 
 
-def run_slabs(w, world, steps, linear=False, overlap=False):
+def run_slabs(w, world, steps, linear=False, overlap=False, push=False):
     from paper_2603_11102_b200 import gks
     d = slab.SlabDecomposition(w.cfg, world)
     solvers = [gks.Gks(d.local_cfg(r)) for r in range(world)]
@@ -28,7 +28,7 @@ def run_slabs(w, world, steps, linear=False, overlap=False):
     for k in range(steps):
         pts = w.alm(k) if w.alm is not None else None
         stepper.step(w.dt, before_forcing=(lambda s: s.alm_set_points(*pts)) if pts is not None else None,
-                     ibm=w.ibm is not None, bulk=w.bulk_flux is not None, overlap=overlap)
+                     ibm=w.ibm is not None, bulk=w.bulk_flux is not None, overlap=overlap, push=push)
     W = d.gather([s.get_state() for s in solvers])
     for s in solvers:
         s.close()
@@ -359,3 +359,33 @@ def test_overlapped_step_equals_the_plain_step(name, world, small):
     with pytest.raises(gks.GksError):
         g.step_finish(w.dt)
     g.close()
+
+
+@pytest.mark.parametrize("name,world", [("C1", 3), ("C3", 4), ("C5", 3), ("C2", 2)])
+def test_exchange_by_direct_push_equals_the_buffered_exchange(name, world):
+    """gks_halo_push: every sub-domain writes its boundary planes straight into its neighbours' ghost layers (pack,
+    transfer and unpack in one kernel; slabs of unequal width have different pitches and field strides) - the same
+    bits as the exchange through buffers; refusals"""
+    from paper_2603_11102_b200 import gks
+    w = wl.by_name(name, small=name != "C1")
+    Wb, Wp = run_slabs(w, world, 2), run_slabs(w, world, 2, push=True)
+    if w.ibm is None:
+        assert np.array_equal(Wp, Wb)
+    else:
+        assert rel_linf(Wp, Wb) <= 1e-14
+    d = slab.SlabDecomposition(w.cfg, world)
+    g0, g1 = gks.Gks(d.local_cfg(0)), gks.Gks(d.local_cfg(1))
+    g0.set_state(d.scatter(w.W0, 0))
+    g1.set_state(d.scatter(w.W0, 1))
+    win = g1.halo_window(0)
+    assert win.nx == d.local_cfg(1).n[0] and win.pitch_x >= win.nx + 6 and win.W
+    g0.halo_push(0, 1, win)
+    with pytest.raises(gks.GksError):
+        g0.halo_push(0, 2, win)                              # not an x face
+    with pytest.raises(gks.GksError):
+        g0.halo_push(1, 1, win)                              # W* only exists inside a step
+    win.ny += 1
+    with pytest.raises(gks.GksError):
+        g0.halo_push(0, 1, win)                              # extents differ
+    g0.close()
+    g1.close()
