@@ -217,3 +217,38 @@ def test_C5_turbine_ten_steps_sampled():
         p = w.alm(s)[0] / w.cfg.spacing[0]
         assert all((p[:, a] > lo[a] + 8).all() and (p[:, a] < lo[a] + size[a] - 8).all() for a in range(3))
     check_samples(w, Wg, [lo], size=size, need=[("alm", "ibm")], steps=10, tol=1e-9, margin=64)
+
+
+def test_maximum_size_box_beyond_32_bit_indices():
+    """768 x 640 x 576 = 283 M cells (84 GB of workspace of the 180 GB): the padded field has 2.9e8 doubles, so the
+    flux arrays (8 fields) and the state are indexed beyond 2^31 - every index must be 64-bit.  One step on a
+    periodic box: conservation to round-off (P7 holds at any size), finiteness, and parity with the oracle on
+    sub-boxes at the origin, in the middle and at the far corner (the largest indices), where a wrapped index would
+    read or write the wrong cell"""
+    from paper_2603_11102_b200 import gks
+    n = (768, 640, 576)
+    L = 2.0 * np.pi
+    cfg = GridConfig(n=n, spacing=tuple(L / m for m in n), nu=1e-4, bc=(wl.BC_PERIODIC,) * 6)
+    x, y, z = [cfg.centres(a) for a in range(3)]
+    sx, cx, sy, cy, sz, cz = np.sin(x), np.cos(x), np.sin(y), np.cos(y), np.sin(z), np.cos(z)
+    W0 = np.empty((4, n[2], n[1], n[0]))
+    W0[0] = 1.0 + 0.01 * (np.cos(2 * z)[:, None, None] * cy[None, :, None] * sx[None, None, :])
+    W0[1] = 0.1 * (cz[:, None, None] * cy[None, :, None] * sx[None, None, :])
+    W0[2] = -0.1 * (cz[:, None, None] * sy[None, :, None] * cx[None, None, :])
+    W0[3] = 0.02 * (sz[:, None, None] * np.sin(2 * y)[None, :, None] * np.cos(3 * x)[None, None, :])
+    W0[1:] *= W0[0]
+    w = wl.Workload("max_size", cfg, W0, 0.4 * min(cfg.spacing) / 1.15, 1)
+    g = gks.Gks(cfg)
+    assert g.workspace_bytes > 8 * 2 ** 31                     # 8 flux fields alone pass 2^31 doubles
+    g.set_state(W0)
+    g.step(w.dt)
+    Wg = g.get_state()
+    g.close()
+    assert np.isfinite(Wg).all()
+    mscale = float(np.abs(W0[1:]).sum(dtype=np.longdouble))
+    for c in range(4):
+        s0, s1 = W0[c].sum(dtype=np.longdouble), Wg[c].sum(dtype=np.longdouble)
+        ref = abs(float(s0)) if c == 0 else 1e-3 * mscale
+        assert abs(float(s1 - s0)) <= 1e-12 * ref, (c, float(s1 - s0), ref)
+    boxes = [(-14, -14, -14), (370, 300, 280), (n[0] - 20, n[1] - 20, n[2] - 20), (n[0] - 30, 5, n[2] - 40)]
+    check_samples(w, Wg, boxes)
