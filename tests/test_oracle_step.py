@@ -1011,3 +1011,38 @@ def test_P24_explicit_stations_and_section_blended_polars():
         with pytest.raises(Exception):
             o.alm_set_rotor(bad)
     o.close()
+
+
+# ---------------------------------------------------------------- P25 ghost cells by their definitions (S17, S18, S21)
+def test_P25_ghost_cells_by_definition():
+    """the ghost fill read back (`get_padded`) against the definitions of DESIGN.md, written out with numpy on the input
+    array: extrapolation = the nearest interior cell in all three layers (S21: zero gradient, NOT a linear
+    extrapolation - the data below have a gradient, so any other constant or linear rule fails), no-slip wall = mirror
+    image with all momenta odd (S17), slip wall = mirror image with the normal momentum odd (S18), periodic = image;
+    pass order x, y, z: an edge ghost is the y-rule applied to the x-ghost"""
+    rng = np.random.default_rng(31)
+    n = (7, 8, 9)
+    W = np.empty((4, n[2], n[1], n[0]))
+    x, y, z = np.meshgrid(np.arange(n[2]), np.arange(n[1]), np.arange(n[0]), indexing="ij")
+    W[0] = 1.0 + 0.01 * z + 0.02 * y + 0.015 * x + 1e-3 * rng.standard_normal(W[0].shape)
+    W[1:] = 0.1 + 0.01 * rng.standard_normal(W[1:].shape) + 0.005 * (x + 2 * y - z)
+    cfg = GridConfig(n=n, spacing=(0.1, 0.1, 0.1), bc=(EX, EX, NS, SL, P, P))
+    o = ob.Oracle(cfg)
+    o.set_state(W)
+    G = o.get_padded()                                          # (4, nz+6, ny+6, nx+6)
+    o.close()
+    I = G[:, 3:-3, 3:-3, 3:-3]
+    assert np.array_equal(I, W)
+    # x faces: extrapolation, both sides, all three layers = the first / last interior cell
+    for g in range(1, 4):
+        assert np.array_equal(G[:, 3:-3, 3:-3, 3 - g], W[..., 0]) and np.array_equal(G[:, 3:-3, 3:-3, 2 + n[0] + g], W[..., -1])
+    # y low: no-slip wall (rho even, momenta odd); y high: slip wall (rho, tangential momenta even, normal momentum odd)
+    for g in range(1, 4):
+        lo, hi = G[:, 3:-3, 3 - g, 3:-3], G[:, 3:-3, 2 + n[1] + g, 3:-3]
+        assert np.array_equal(lo[0], W[0, :, g - 1, :]) and np.array_equal(lo[1:], -W[1:, :, g - 1, :])
+        assert np.array_equal(hi[[0, 1, 3]], W[[0, 1, 3]][:, :, n[1] - g, :]) and np.array_equal(hi[2], -W[2, :, n[1] - g, :])
+    # z: periodic image
+    for g in range(1, 4):
+        assert np.array_equal(G[:, 3 - g, 3:-3, 3:-3], W[:, n[2] - g]) and np.array_equal(G[:, 2 + n[2] + g, 3:-3, 3:-3], W[:, g - 1])
+    # an x-y edge: the y-rule (no-slip mirror) applied to the x-ghost column (pass order x, then y)
+    assert np.array_equal(G[0, 3:-3, 2, 1], W[0, :, 0, 0]) and np.array_equal(G[2, 3:-3, 1, 3 + n[0]], -W[2, :, 1, -1])
