@@ -71,6 +71,14 @@ def random_case(seed, wide=False, anywhere=False):
             extras["rotor"] = synthetic_rotor(hub, R, eps, u_ref=0.1, tsr=5.0, nblades=int(rng.integers(2, 4)), npts=8,
                                               seed=seed, freestream_correction=bool(rng.integers(2)),
                                               tip_correction=bool(rng.integers(2)))
+    # (drawn last, so that the cases above stay what they were) moving Lagrangian points; a rotor with stations refined at
+    # root and tip and three airfoil sections (reading S28)
+    extras["ibm_vel"] = 0.05 * rng.standard_normal((len(ibm[0]), 3)) if ibm and rng.random() < 0.5 else None
+    if extras["rotor"] is not None and rng.random() < 0.5:
+        r0 = extras["rotor"]
+        extras["rotor"] = synthetic_rotor(r0.hub, r0.R, r0.eps, u_ref=0.1, tsr=5.0, nblades=r0.nblades, npts=8, seed=seed,
+                                          refine=True, nsections=3, freestream_correction=r0.freestream_correction,
+                                          tip_correction=r0.tip_correction)
     return cfg, W0, alm, ibm, body, bulk, dt, extras
 
 
@@ -87,6 +95,8 @@ def two_steps(solver, cfg, W0, alm, ibm, body, bulk, dt, extras):
             s.ibm_set_points(*ibm)
             if extras["passes"]:
                 s.ibm_set_iterations(extras["passes"], 0.0)
+            if extras["ibm_vel"] is not None:
+                s.ibm_set_velocities(extras["ibm_vel"])
         if body:
             s.set_body_force(*body)
         if bulk:
@@ -133,7 +143,8 @@ def slab_case(seed):
     raise AssertionError("no cuttable case")
 
 
-def slab_two_steps(case, world):
+def slab_two_steps(case, world, mode="plain"):
+    """mode: plain (exchange through buffers), overlap (the step in parts), push (neighbours write the ghosts directly)"""
     from paper_2603_11102_b200 import gks, slab
     cfg, W0, alm, ibm, body, bulk, dt, extras = case
     d = slab.SlabDecomposition(cfg, world)
@@ -146,6 +157,8 @@ def slab_two_steps(case, world):
                 s.ibm_set_points(*d.ibm_points(r, *ibm))
                 if extras["passes"]:
                     s.ibm_set_iterations(extras["passes"], 0.0)
+                if extras["ibm_vel"] is not None:
+                    s.ibm_set_velocities(d.ibm_velocities(r, ibm[0], extras["ibm_vel"]))
             if body:
                 s.set_body_force(*body)
             if bulk:
@@ -156,7 +169,8 @@ def slab_two_steps(case, world):
         for _ in range(2):
             stepper.step(dt, before_forcing=(lambda s: s.alm_set_points(*d.alm_points(solvers.index(s), *alm))) if alm else None,
                          ibm=bool(ibm),
-                         bulk=bool(bulk), rotor=rot, ibm_passes=max(extras["passes"], 1))
+                         bulk=bool(bulk), rotor=rot, ibm_passes=max(extras["passes"], 1), overlap=mode == "overlap",
+                         push=mode == "push")
         return d.gather([s.get_state() for s in solvers])
     finally:
         for s in solvers:
@@ -172,7 +186,7 @@ def test_fifteen_random_configurations_cut_into_x_slabs(first):
     from paper_2603_11102_b200 import gks
     for seed in range(first, first + 15):
         case, world = slab_case(seed)
-        Ws = slab_two_steps(case, world)
+        Ws = slab_two_steps(case, world, ("plain", "overlap", "push")[seed % 3])
         W1 = two_steps(gks.Gks, *case)[0]
         assert rel_linf(Ws, W1) <= 1e-13, (seed, world, case[0].n, case[0].bc)
         assert rel_linf(Ws, two_steps(ob.Oracle, *case)[0]) <= 1e-11, (seed, world)
