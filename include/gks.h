@@ -267,6 +267,27 @@ gks_status gks_set_reconstruction(gks_ctx *ctx, int tangential_linear);
  * cfl <= 0 -> GKS_ERR_INVALID_ARG; before gks_set_state -> GKS_ERR_STATE. */
 gks_status gks_cfl_dt(gks_ctx *ctx, double cfl, double *dt);
 
+/* The same time step for callers that cannot allocate device memory (CUDA graph capture, serving loops,
+ * harnesses that forbid cudaMalloc): no context and no workspace.  The reduction's scratch (one partial maximum per
+ * block of GKS_NOALLOC_CELLS_PER_BLOCK cells) is a file-scope __device__ array of GKS_NOALLOC_MAX_BLOCKS doubles
+ * (512 KB, held by every GPU that loads the library until the process exits); the call allocates and frees nothing.
+ *   W     DEVICE, 4*nz*ny*nx doubles, W[c][k][j][i] (the layout of gks_set_state); read only; owned by the caller
+ *   dmin  smallest cell width over the three axes (> 0); RT > 0; cfl > 0
+ *   dt    DEVICE, one double, written asynchronously on cuda_stream (a cudaStream_t; NULL = legacy default stream)
+ * The CUDA device that holds W and dt must be current.  Asynchronous: two kernels on cuda_stream, no synchronisation.
+ * Errors (message in gks_noalloc_last_error(), per thread): NULL or host pointers, sizes < 1, non-positive dmin / RT / cfl
+ * -> GKS_ERR_INVALID_ARG; nx*ny*nz > GKS_NOALLOC_MAX_CELLS -> GKS_ERR_INVALID_ARG (use gks_cfl_dt with a workspace);
+ * a failing CUDA call -> GKS_ERR_CUDA.  dt is untouched on error.
+ * All calls on a device SHARE the scratch array: calls whose kernels may overlap on the GPU (different streams with no
+ * ordering between them) race; calls on one stream, or ordered by events, are safe.  Nothing in the array has to be
+ * cleared between calls (every slot that is read was written by the same call first). */
+#define GKS_NOALLOC_CELLS_PER_BLOCK 4096
+#define GKS_NOALLOC_MAX_BLOCKS 65536
+#define GKS_NOALLOC_MAX_CELLS ((long long)GKS_NOALLOC_MAX_BLOCKS * GKS_NOALLOC_CELLS_PER_BLOCK) /* 2^28 = 268 435 456 */
+gks_status gks_cfl_dt_noalloc(const double *W, int nx, int ny, int nz, double dmin, double RT, double cfl, double *dt,
+                              void *cuda_stream);
+const char *gks_noalloc_last_error(void);
+
 /* Test hook: fill ghosts of the CURRENT state and evaluate the face-averaged flux F and its
  * time derivative dF/dt (Eq. 6-7) for sweep direction dir in {0,1,2}.  Output (host or device):
  * 4 * (faces) doubles each, faces laid out like cells but with n_dir+1 entries along `dir`,

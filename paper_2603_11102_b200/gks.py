@@ -22,7 +22,8 @@ EXPORTS = ["gks_workspace_bytes", "gks_create", "gks_destroy", "gks_set_state", 
            "gks_set_body_force", "gks_set_bulk_flux", "alm_set_points", "ibm_set_points", "ibm_set_velocities", "ibm_set_iterations", "gks_cfl_dt", "alm_set_rotor", "alm_rotor_eval", "alm_rotor_points", "gks_set_reconstruction", "gks_halo_doubles", "gks_halo_pack", "gks_halo_unpack", "gks_step_begin",
            "gks_step_finish", "gks_step_force", "gks_bulk_partial", "gks_bulk_set_global", "gks_ibm_pass", "gks_ibm_residual",
            "gks_debug_eval_flux", "alm_rotor_supply", "gks_step_begin_part", "gks_step_finish_part", "gks_halo_window_get", "gks_halo_push",
-           "gks_profile_enable", "gks_profile_read", "gks_check_finite", "gks_launch_count", "gks_last_error"]
+           "gks_profile_enable", "gks_profile_read", "gks_check_finite", "gks_launch_count", "gks_last_error",
+           "gks_cfl_dt_noalloc", "gks_noalloc_last_error"]
 DEBUG_EXPORTS = ["gks_debug_set_sweep", "gks_debug_fp64_peak", "gks_debug_issue_probe", "gks_debug_trace"]    # include/gks_debug.h: libgks_b200_debug.so only
 
 
@@ -116,8 +117,27 @@ def lib(debug=False):
         L.gks_launch_count.restype = C.c_longlong
         L.gks_last_error.argtypes = [vp]
         L.gks_last_error.restype = C.c_char_p
+        L.gks_cfl_dt_noalloc.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, vp, vp]
+        L.gks_noalloc_last_error.argtypes = []
+        L.gks_noalloc_last_error.restype = C.c_char_p
         _LIBS[debug] = L
     return _LIBS[debug]
+
+
+def cfl_dt_noalloc(W, dmin, RT, cfl, out, stream=None):
+    """gks_cfl_dt_noalloc (include/gks.h): the CFL time step of PAPER.md:91 of the DEVICE state W (a contiguous float64
+    tensor of shape (4, nz, ny, nx)) into the one-element DEVICE tensor `out`, asynchronously on `stream` (a
+    torch.cuda.Stream; None = torch's current stream).  No context, no workspace: the library allocates nothing."""
+    import torch
+    if not (W.is_cuda and out.is_cuda and W.dtype == torch.float64 and out.dtype == torch.float64 and W.dim() == 4
+            and W.shape[0] == 4 and W.is_contiguous() and out.numel() >= 1):
+        raise ValueError("W: contiguous float64 CUDA tensor (4, nz, ny, nx); out: float64 CUDA tensor")
+    s = stream if stream is not None else torch.cuda.current_stream(W.device)
+    with torch.cuda.device(W.device):
+        st = lib().gks_cfl_dt_noalloc(W.data_ptr(), int(W.shape[3]), int(W.shape[2]), int(W.shape[1]), float(dmin),
+                                      float(RT), float(cfl), out.data_ptr(), s.cuda_stream)
+    if st != GKS_OK:
+        raise GksError(st, lib().gks_noalloc_last_error().decode())
 
 
 def make_config(cfg):
