@@ -301,6 +301,7 @@ def main():
     ap.add_argument("--no-configs", action="store_true", help="skip the C1..C5 throughput block of the JSON line")
     ap.add_argument("--ibm-passes", type=int, default=1, help="IBM multi-direct-forcing passes per step (workloads with IBM)")
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--e2e-depth", type=int, default=2, help="contexts in rotation in the pipelined end-to-end leg")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -450,16 +451,63 @@ def main():
     barrier()
     e2e_s = time.perf_counter() - t0
 
-    t = torch.tensor([ms, e2e_s * 1e3], dtype=torch.float64, device=device)
+    # ---- the same with INDEPENDENT batches through two contexts in rotation (gks.HostPipeline): every batch is still
+    # copied in from pinned host memory, stepped and copied back inside the timed region, but the copies of one batch
+    # run on the copy engines while the other context computes.  Timed from the first submit to the last batch back in
+    # host memory (pipeline fill and drain included).
+    pipe_s, pipe_batches = 0.0, 0
+    if stepper is None and args.sweep == 0 and not args.online_rotor:
+        def setup(gp):
+            if w.bulk_flux is not None:
+                gp.set_bulk_flux(*w.bulk_flux)
+            if w.ibm is not None:
+                gp.ibm_set_points(*w.ibm)
+                if args.ibm_passes > 1:
+                    gp.ibm_set_iterations(args.ibm_passes, 0.0)
+            if args.variant == "linear":
+                gp.set_reconstruction(1)
+        pipe = gks.HostPipeline(w.cfg, depth=args.e2e_depth, device=device, setup=setup)
+        nd = args.e2e_depth
+        Hi = [torch.from_numpy(w.W0.copy()).pin_memory() for _ in range(nd)]
+        Ho = [torch.empty_like(Hi[0]).pin_memory() for _ in range(nd)]
+        hook = (lambda gp, s_: gp.alm_set_points(*w.alm(0))) if w.alm is not None else None
+        for b in range(nd):                                  # untimed: every context once
+            pipe.submit(Hi[b], Ho[b], w.dt, before_step=hook)
+        pipe.drain()
+        pipe_batches = 3 * args.e2e_steps + 3
+        barrier()
+        t0 = time.perf_counter()
+        for b in range(pipe_batches):
+            pipe.submit(Hi[b % nd], Ho[b % nd], w.dt, before_step=hook)
+        pipe.drain()
+        barrier()
+        pipe_s = time.perf_counter() - t0
+        pipe.close()
+        del pipe, Hi, Ho
+
+    t = torch.tensor([ms, e2e_s * 1e3, pipe_s * 1e3], dtype=torch.float64, device=device)
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms, e2e_ms = t.tolist()
+    ms, e2e_ms, pipe_ms = t.tolist()
     if rank == 0:
         peaks, peak_src = read_peaks()
         # replicas: every rank steps its own copy of the workload; slab: the ranks share ONE workload
         total_cells = w_global.cfg.cells if slab_mode else cells * world
         value = total_cells * args.steps / (ms * 1e-3) / 1e6
         e2e_value = total_cells * args.e2e_steps / (e2e_ms * 1e-3) / 1e6
+        serial = {"value": e2e_value, "steps": args.e2e_steps,
+                  "mode": "one context; copy in, step, copy out in sequence (each step's input is the previous output)"}
+        if pipe_batches:
+            e2e = {"value": total_cells * pipe_batches / (pipe_ms * 1e-3) / 1e6, "unit": UNIT,
+                   "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes, "steps": pipe_batches,
+                   "depth": args.e2e_depth,
+                   "mode": "independent batches through %d contexts in rotation (gks.HostPipeline): every batch is copied "
+                           "in from pinned host memory, stepped and copied back; the copies overlap the other context's "
+                           "step; timed from the first submit to the last batch in host memory" % args.e2e_depth,
+                   "serial": serial}
+        else:
+            e2e = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
+                   "steps": args.e2e_steps, "mode": serial["mode"]}
         sweep_ms = sum(prof[k][0] for k in ("sweep_x", "sweep_y", "sweep_z"))
         sweep_n = sum(prof[k][1] for k in ("sweep_x", "sweep_y", "sweep_z"))
         faces = cells  # one face per cell and direction (+ one boundary plane, < 0.5 %)
@@ -486,8 +534,7 @@ def main():
                        "multi_gpu": ("x-slabs with halo exchange" if slab_mode else "replicas only") if world > 1 else "single GPU",
                        "l2": "inputs larger than L2 (state %.0f MB per field set)" % (cells * 32 / 1e6)},
             "clocks": clocks,
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
-                    "steps": args.e2e_steps},
+            "e2e": e2e,
             "gpu_launches": int(launches),
             # headline fraction: against the NOMINAL fp64 rate (unit count x clock; neither MEASURED_PEAKS.json nor the
             # profiling guide carries an fp64 figure).  frac_pipe: ncu "fp64 pipe active" of the same kernels from the

@@ -498,3 +498,74 @@ def run_workload(w, steps=None, sweep=None):
     W = g.get_state()
     g.close()
     return W
+
+
+class HostPipeline:
+    """Independent batches with HOST buffers through `depth` solver contexts in rotation (host logic only; every step
+    runs in the library's kernels).  A batch is one state in host memory that is copied to the device, advanced `steps`
+    steps and copied back; the batches do not depend on one another.  Each context has its own stream, so while one
+    computes, the host->device copy of the next batch and the device->host copy of the previous one run on the copy
+    engines: in steady state a batch costs max(compute, copy in, copy out) instead of their sum (depth 2), and with
+    depth 3 the two copies of different batches also overlap each other.
+
+        pipe = HostPipeline(cfg, depth=2, setup=lambda g: g.ibm_set_points(pos, vol))
+        for W_in, W_out in batches:                 # pinned host arrays (torch.Tensor.pin_memory) keep the copies asynchronous
+            done = pipe.submit(W_in, W_out, dt)     # returns the W_out of an EARLIER batch that is now complete, or None
+        pipe.drain()                                # completes the rest, in order
+
+    W_in must stay untouched until the batch is complete; W_out is valid once submit / drain has returned it."""
+
+    def __init__(self, cfg, depth=2, device="cuda:0", setup=None):
+        if depth < 1:
+            raise ValueError("depth must be >= 1")
+        self.ctx = [Gks(cfg, device=device) for _ in range(depth)]
+        for g in self.ctx:
+            if setup is not None:
+                setup(g)
+        self._pending = []      # (context index, W_out) in submission order
+        self._step_done = None  # event behind the last step enqueued
+        self._next = 0
+
+    def _complete_oldest(self):
+        k, out = self._pending.pop(0)
+        self.ctx[k].get_state(out)          # unpack + device->host copy on that context's stream, then synchronises it
+        return out
+
+    def submit(self, W_in, W_out, dt, steps=1, before_step=None):
+        """enqueue set_state(W_in), `steps` x step(dt) on the next context (asynchronous), then complete the oldest
+        batch if every context is busy.  before_step(g, s): optional hook called before step s (e.g. alm_set_points)."""
+        k = self._next
+        assert all(p[0] != k for p in self._pending)
+        g = self.ctx[k]
+        g.set_state(W_in)
+        # the steps of successive batches run one after the other, in submission order: without this the kernels of two
+        # contexts interleave on the SMs, both batches finish late and neither copy has a step left to hide behind
+        # (measured on B200, 256^3: 26 ms per batch instead of 20)
+        if self._step_done is not None:
+            g.stream.wait_event(self._step_done)
+        for s in range(steps):
+            if before_step is not None:
+                before_step(g, s)
+            g.step(dt)
+        self._step_done = g._torch.cuda.Event()
+        self._step_done.record(g.stream)
+        self._pending.append((k, W_out))
+        self._next = (k + 1) % len(self.ctx)
+        if len(self._pending) == len(self.ctx):
+            return self._complete_oldest()
+        return None
+
+    def drain(self):
+        done = []
+        while self._pending:
+            done.append(self._complete_oldest())
+        return done
+
+    @property
+    def launch_count(self):
+        return sum(g.launch_count for g in self.ctx)
+
+    def close(self):
+        for g in self.ctx:
+            g.close()
+        self.ctx = []
