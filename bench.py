@@ -474,7 +474,7 @@ def main():
         for b in range(nd):                                  # untimed: every context once
             pipe.submit(Hi[b], Ho[b], w.dt, before_step=hook)
         pipe.drain()
-        pipe_batches = 3 * args.e2e_steps + 3
+        pipe_batches = 8 * args.e2e_steps
         barrier()
         t0 = time.perf_counter()
         for b in range(pipe_batches):

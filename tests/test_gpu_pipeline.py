@@ -59,3 +59,34 @@ def test_pipelined_batches_equal_the_serial_path(name, depth, steps):
         else:                                   # the IBM spreading adds with fp64 atomics: order varies run to run
             assert rel_linf(outs[b].numpy(), ref[b]) <= 1e-13, b
         assert not np.array_equal(ref[b], ref[(b + 1) % nb])        # the batches differ
+
+
+@pytest.mark.parametrize("name", ["C1", "C2", "C3"])
+def test_a_step_can_be_captured_in_a_cuda_graph(name):
+    """gks_step allocates nothing, never synchronises and reads no host memory, so a caller may capture it (stream
+    capture on the context's stream, programmatic dependent launches included) and replay it: same bits as the plain
+    calls where the step is deterministic, 1e-13 with the fp64 atomics of the IBM spreading"""
+    import torch
+    from paper_2603_11102_b200 import gks
+    w = wl.by_name(name, small=(name != "C1"))
+    g = gks.Gks(w.cfg)
+    _setup_for(w)(g)
+    g.set_state(w.W0)
+    for _ in range(4):
+        g.step(w.dt)
+    ref = g.get_state()
+    g.set_state(w.W0)
+    g.step(w.dt)                      # every kernel has run once before the capture
+    g.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=g.stream):
+        g.step(w.dt)                  # captured, not executed
+    with torch.cuda.stream(g.stream):
+        for _ in range(3):
+            graph.replay()
+    out = g.get_state()
+    g.close()
+    if w.ibm is None:
+        assert np.array_equal(out, ref)
+    else:
+        assert rel_linf(out, ref) <= 1e-13
