@@ -300,6 +300,9 @@ def main():
                          "point forces re-set from the host every step")
     ap.add_argument("--no-configs", action="store_true", help="skip the C1..C5 throughput block of the JSON line")
     ap.add_argument("--ibm-passes", type=int, default=1, help="IBM multi-direct-forcing passes per step (workloads with IBM)")
+    ap.add_argument("--halo", choices=["messages", "push"], default="messages",
+                    help="--decomp slab: halos as NCCL messages between pack / unpack kernels, or written straight into the\n"
+                         "neighbour process's ghost layers through CUDA IPC mappings (slab.IpcPushTransport)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--e2e-depth", type=int, default=2, help="contexts in rotation in the pipelined end-to-end leg")
     args = ap.parse_args()
@@ -356,7 +359,8 @@ def main():
     if args.ibm_passes > 1 and w.ibm is not None:
         g.ibm_set_iterations(args.ibm_passes, 0.0)
     if slab_mode:
-        stepper = slab.SlabStepper(slab.DistTransport(dec, rank), g, slab.BufferPool(device))
+        transport = slab.IpcPushTransport(dec, rank, g) if args.halo == "push" else slab.DistTransport(dec, rank)
+        stepper = slab.SlabStepper(transport, g, slab.BufferPool(device))
     if args.variant == "linear":
         g.set_reconstruction(1)
     cells = w.cfg.cells
@@ -385,7 +389,7 @@ def main():
         # actuator points reach a slab through dec.alm_points (supports across cuts, images beyond a periodic seam)
         hook = (lambda s: s.alm_set_points(*dec.alm_points(rank, *w.alm(k)))) if w.alm is not None else None
         stepper.step(w.dt, before_forcing=hook, ibm=w_global.ibm is not None, bulk=w.bulk_flux is not None,
-                     ibm_passes=args.ibm_passes, rotor=rotor_drv, overlap=args.overlap)
+                     ibm_passes=args.ibm_passes, rotor=rotor_drv, overlap=args.overlap, push=args.halo == "push")
 
     def one_step():
         if stepper is not None:
@@ -531,7 +535,7 @@ def main():
                        "sweep": "fused" if args.sweep == 0 else "unfused", "variant": args.variant,
                        "alm": ("on-line rotor (alm_set_rotor, synthetic blade data)" if args.online_rotor else
                                ("prescribed point forces" if (w_global if slab_mode else w).alm is not None else None)),
-                       "multi_gpu": ("x-slabs with halo exchange" if slab_mode else "replicas only") if world > 1 else "single GPU",
+                       "multi_gpu": (("x-slabs, halos pushed into the neighbour's ghosts (CUDA IPC)" if args.halo == "push" else "x-slabs with halo exchange") if slab_mode else "replicas only") if world > 1 else "single GPU",
                        "l2": "inputs larger than L2 (state %.0f MB per field set)" % (cells * 32 / 1e6)},
             "clocks": clocks,
             "e2e": e2e,
@@ -558,6 +562,8 @@ def main():
         }
         if slab_mode:
             line["config"]["note"] = "x-slab numbers over NCCL are UNVERIFIED: validated on one GPU and over gloo only"
+    if slab_mode and args.halo == "push":
+        transport.close()              # unmap the neighbours' workspaces before anyone frees
     g.close()
     if rank == 0:
         if not args.no_configs and world == 1 and args.workload == "M0" and args.sweep == 0:

@@ -167,6 +167,26 @@ typedef struct {
 } gks_halo_window;
 gks_status gks_halo_window_get(gks_ctx *ctx, int which, gks_halo_window *out);
 gks_status gks_halo_push(gks_ctx *ctx, int which, int face, const gks_halo_window *to);
+/* The windows of a sub-domain owned by ANOTHER PROCESS (one process per GPU), mapped with CUDA IPC:
+ *   gks_halo_export_get(ctx, &e)        (owner) describes the device allocation that holds the workspace and where the
+ *       padded states W^n and W* lie in it; `e` is plain bytes and may be sent to the neighbour's process.  The workspace
+ *       must lie inside ONE cudaMalloc allocation (GKS_ERR_WORKSPACE / GKS_ERR_CUDA otherwise).
+ *   gks_halo_export_open(&e, win, &map) (neighbour, with the device it pushes from current) maps that allocation -
+ *       peer to peer over NVLink when it lives on another GPU - and fills win[0] (W^n) and win[1] (W*) for gks_halo_push.
+ *       An allocation opens once per process: open once per neighbour rank.  GKS_ERR_CUDA if it cannot be mapped (also in
+ *       the process that owns it); message in gks_last_error(NULL).
+ *   gks_halo_export_close(map)          unmaps; the windows are dead afterwards.  Close before the owner frees.
+ * The ORDER between the processes is the driver's (paper_2603_11102_b200/slab.py IpcPushTransport: interprocess events -
+ * the owner's stream waits for "landed", the pusher's stream for "ghosts free"). */
+typedef struct {
+  unsigned char mem[64];           /* cudaIpcMemHandle_t of the allocation that holds the workspace */
+  unsigned long long offset[2];    /* bytes from the allocation's base to the padded state W^n ([0]) and W* ([1]) */
+  int nx, ny, nz, pitch_x, pitch_y;
+  long long field_stride;
+} gks_halo_export;
+gks_status gks_halo_export_get(gks_ctx *ctx, gks_halo_export *out);
+gks_status gks_halo_export_open(const gks_halo_export *in, gks_halo_window win[2], void **mapping);
+gks_status gks_halo_export_close(void *mapping);
 gks_status gks_step_begin(gks_ctx *ctx, double dt);
 gks_status gks_step_finish(gks_ctx *ctx, double dt);
 gks_status gks_step_force(gks_ctx *ctx, double dt);

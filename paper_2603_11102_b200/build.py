@@ -19,7 +19,7 @@ NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
          "-Xcompiler", "-fPIC", "-ccbin", "/usr/bin/g++"]
 # translation units that do not look at GKS_DEBUG: one object serves both libraries
-SHARED_OBJECTS = ("gks_update", "gks_ghost", "gks_forcing", "gks_rotor", "gks_noalloc")
+SHARED_OBJECTS = ("gks_update", "gks_ghost", "gks_forcing", "gks_rotor", "gks_noalloc", "gks_ipc")
 
 
 def _newer(target, deps):

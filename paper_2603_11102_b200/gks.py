@@ -23,7 +23,7 @@ EXPORTS = ["gks_workspace_bytes", "gks_create", "gks_destroy", "gks_set_state", 
            "gks_step_finish", "gks_step_force", "gks_bulk_partial", "gks_bulk_set_global", "gks_ibm_pass", "gks_ibm_residual",
            "gks_debug_eval_flux", "alm_rotor_supply", "gks_step_begin_part", "gks_step_finish_part", "gks_halo_window_get", "gks_halo_push",
            "gks_profile_enable", "gks_profile_read", "gks_check_finite", "gks_launch_count", "gks_last_error",
-           "gks_cfl_dt_noalloc", "gks_noalloc_last_error"]
+           "gks_cfl_dt_noalloc", "gks_noalloc_last_error", "gks_halo_export_get", "gks_halo_export_open", "gks_halo_export_close"]
 DEBUG_EXPORTS = ["gks_debug_set_sweep", "gks_debug_fp64_peak", "gks_debug_issue_probe", "gks_debug_trace"]    # include/gks_debug.h: libgks_b200_debug.so only
 
 
@@ -39,6 +39,12 @@ class AlmRotor(C.Structure):
 class HaloWindow(C.Structure):
     _fields_ = [("W", C.c_void_p), ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("pitch_x", C.c_int),
                 ("pitch_y", C.c_int), ("field_stride", C.c_longlong)]
+
+
+class HaloExport(C.Structure):
+    """gks_halo_export: a sub-domain's windows as plain bytes for another process (bytes(e) / HaloExport.from_buffer_copy)"""
+    _fields_ = [("mem", C.c_ubyte * 64), ("offset", C.c_ulonglong * 2), ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
+                ("pitch_x", C.c_int), ("pitch_y", C.c_int), ("field_stride", C.c_longlong)]
 
 
 class GksConfig(C.Structure):
@@ -118,6 +124,9 @@ def lib(debug=False):
         L.gks_last_error.argtypes = [vp]
         L.gks_last_error.restype = C.c_char_p
         L.gks_cfl_dt_noalloc.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, vp, vp]
+        L.gks_halo_export_get.argtypes = [vp, C.POINTER(HaloExport)]
+        L.gks_halo_export_open.argtypes = [C.POINTER(HaloExport), C.POINTER(HaloWindow), C.POINTER(vp)]
+        L.gks_halo_export_close.argtypes = [vp]
         L.gks_noalloc_last_error.argtypes = []
         L.gks_noalloc_last_error.restype = C.c_char_p
         _LIBS[debug] = L
@@ -138,6 +147,26 @@ def cfl_dt_noalloc(W, dmin, RT, cfl, out, stream=None):
                                       float(RT), float(cfl), out.data_ptr(), s.cuda_stream)
     if st != GKS_OK:
         raise GksError(st, lib().gks_noalloc_last_error().decode())
+
+
+def halo_export_open(blob, device="cuda:0"):
+    """map the workspace of a sub-domain owned by another process (blob = its Gks.halo_export()) with `device` current;
+    returns ([window of W^n, window of W*], mapping) - give the mapping to halo_export_close when done"""
+    import torch
+    e = HaloExport.from_buffer_copy(blob)
+    win = (HaloWindow * 2)()
+    m = C.c_void_p()
+    with torch.cuda.device(device):
+        st = lib().gks_halo_export_open(C.byref(e), win, C.byref(m))
+    if st != GKS_OK:
+        raise GksError(st, lib().gks_last_error(None).decode())
+    return [win[0], win[1]], m
+
+
+def halo_export_close(mapping):
+    st = lib().gks_halo_export_close(mapping)
+    if st != GKS_OK:
+        raise GksError(st, lib().gks_last_error(None).decode())
 
 
 def make_config(cfg):
@@ -404,6 +433,12 @@ class Gks:
         w = HaloWindow()
         self._c("gks_halo_window_get", int(which), C.byref(w))
         return w
+
+    def halo_export(self):
+        """this sub-domain's windows for ANOTHER process: bytes to send; the receiver calls halo_export_open"""
+        e = HaloExport()
+        self._c("gks_halo_export_get", C.byref(e))
+        return bytes(e)
 
     def halo_push(self, which, face, window):
         """my 3 interior planes next to `face` straight into the neighbour's ghost planes (its `halo_window`)"""

@@ -315,6 +315,79 @@ class DistTransport:
                 self.dist.broadcast(t, src=src, group=self.group)
 
 
+
+class IpcPushTransport(DistTransport):
+    """One process per sub-domain, halos WITHOUT buffers and without messages: every rank maps the workspaces of its
+    neighbours (CUDA IPC: gks_halo_export_get / _open - peer-to-peer over NVLink when the neighbour sits on another GPU)
+    and writes its boundary planes straight into their ghost layers (gks_halo_push: pack, transfer and unpack in one
+    kernel).  Nothing but the order travels between the processes:
+
+        ghosts_free[r]  interprocess event, recorded on r's stream when r calls the exchange: everything r enqueued before
+                        (the sweeps that read its ghosts) precedes it; a neighbour's stream waits for it before it pushes
+        landed[r]       recorded on r's stream behind its pushes; a neighbour's stream waits for it before it goes on
+
+    A stream that waits for an interprocess event waits for the LAST record the host has issued, so the waiting host must
+    know that the record has been issued: one host barrier of the control group (gloo: no device work, no stream is
+    synchronised) between a record and the waits for it.  Per exchange: record, barrier, waits + pushes + record,
+    barrier, waits - the GPUs never idle for the host as long as the hosts run ahead of them.
+
+    Every exchange of the step goes this way (both stages, the un-forced W^{n+1} for IBM / rotor, between IBM passes);
+    the scalar reductions and the rotor broadcast stay DistTransport's."""
+
+    def __init__(self, decomposition, rank, solver, group=None, control_group=None):
+        import torch
+        from . import gks
+        super().__init__(decomposition, rank, group)
+        dist = self.dist
+        if decomposition.world < 2:
+            raise ValueError("IpcPushTransport needs at least two sub-domains")
+        # control plane: host-only barriers and the one-off exchange of handles
+        self.control = control_group if control_group is not None else (
+            group if dist.get_backend(group) == "gloo" else dist.new_group(backend="gloo"))
+        self.solver = solver
+        self.ev_free = torch.cuda.Event(interprocess=True)
+        self.ev_landed = torch.cuda.Event(interprocess=True)
+        with torch.cuda.device(solver.device):
+            self.ev_free.record(solver.stream)          # an event has an IPC handle once it exists on the device
+            self.ev_landed.record(solver.stream)
+            mine = (solver.halo_export(), self.ev_free.ipc_handle(), self.ev_landed.ipc_handle())
+        everyone = [None] * decomposition.world
+        dist.all_gather_object(everyone, mine, group=self.control)
+        self.win, self.peer_free, self.peer_landed, self._maps = {}, {}, {}, []
+        for n in sorted({dst for _, dst, _ in decomposition.schedule(rank)}):
+            blob, h_free, h_landed = everyone[n]
+            wins, m = gks.halo_export_open(blob, solver.device)        # once per neighbour RANK
+            self.win[n] = wins
+            self._maps.append(m)
+            self.peer_free[n] = torch.cuda.Event.from_ipc_handle(solver.device, h_free)
+            self.peer_landed[n] = torch.cuda.Event.from_ipc_handle(solver.device, h_landed)
+
+    def exchange_push(self, solver, which):
+        st = solver.stream
+        self.ev_free.record(st)                          # my ghosts may be overwritten once this has passed
+        self.dist.barrier(group=self.control)            # every neighbour's record has been issued
+        for ev in self.peer_free.values():
+            st.wait_event(ev)
+        for face, dst, dst_face in self.d.schedule(self.rank):
+            solver.halo_push(which, face, self.win[dst][which])
+        self.ev_landed.record(st)
+        self.dist.barrier(group=self.control)
+        for ev in self.peer_landed.values():             # the neighbours' planes are in my ghosts
+            st.wait_event(ev)
+
+    def exchange(self, solver, which, new_buffer=None):
+        self.exchange_push(solver, which)
+
+    def close(self):
+        """unmap the neighbours' workspaces (before they are freed): every stream idle, then a barrier"""
+        from . import gks
+        self.solver.synchronize()
+        self.dist.barrier(group=self.control)
+        for m in self._maps:
+            gks.halo_export_close(m)
+        self._maps = []
+        self.dist.barrier(group=self.control)
+
 class RotorDriver:
     """The on-line actuator-line rotor on sub-domains: every sub-domain is given the rotor with `alm_set_rotor` and
     keeps its clock in the library (advanced by dt in every `gks_step_force`); the disc x = hub_x lies in ONE slab

@@ -3,7 +3,10 @@ torch.distributed.run): its own `Gks` context on cuda:0, `slab.DistTransport` ov
 buffers, the scalar all-reduces (bulk flux, IBM stop rule) and the rotor broadcast.  Every rank shares the one GPU of
 the box; the ranks synchronise on the host between kernels (gloo), no kernel waits on another process.
 
-    python -m torch.distributed.run --nproc-per-node W tests/slab_worker.py CASE STEPS OUTDIR [overlap]
+    python -m torch.distributed.run --nproc-per-node W tests/slab_worker.py CASE STEPS OUTDIR [overlap | push]
+
+"push": no halo buffers and no messages - `slab.IpcPushTransport` maps the neighbours' workspaces with CUDA IPC and every
+rank writes its boundary planes into its neighbours' ghost layers, ordered by interprocess events.
 """
 import os
 import sys
@@ -45,6 +48,9 @@ def main():
     from paper_2603_11102_b200 import gks, slab
     case, steps, outdir = sys.argv[1], int(sys.argv[2]), sys.argv[3]
     overlap = len(sys.argv) > 4 and sys.argv[4] == "overlap"
+    push = len(sys.argv) > 4 and sys.argv[4].startswith("push")   # halos written straight into the neighbour PROCESS's ghosts
+    delay = len(sys.argv) > 4 and sys.argv[4] == "push-delay"     # one rank's GPU work runs late: only the interprocess
+                                                                  # events keep its neighbours from reading stale ghosts
     os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
     dist.init_process_group("gloo")
     rank, world = dist.get_rank(), dist.get_world_size()
@@ -58,15 +64,21 @@ def main():
     if w.bulk_flux is not None:
         g.set_bulk_flux(*w.bulk_flux)
     g.set_state(d.scatter(w.W0, rank))
-    stepper = slab.SlabStepper(slab.DistTransport(d, rank), g, slab.BufferPool("cpu"))
+    transport = slab.IpcPushTransport(d, rank, g) if push else slab.DistTransport(d, rank)
+    stepper = slab.SlabStepper(transport, g, slab.BufferPool("cpu"))
     rot = slab.RotorDriver(d, rotor, "cpu") if rotor is not None else None
     for k in range(steps):
+        if delay and rank == k % world:
+            with torch.cuda.stream(g.stream):
+                torch.cuda._sleep(60_000_000)       # about 30 ms of GPU time ahead of this rank's pushes and sweeps
         hook = None
         if w.alm is not None and rotor is None:
             pts = d.alm_points(rank, *w.alm(k))
             hook = lambda s, pts=pts: s.alm_set_points(*pts)
         stepper.step(w.dt, before_forcing=hook, ibm=w.ibm is not None, rotor=rot, bulk=w.bulk_flux is not None,
-                     ibm_passes=passes, overlap=overlap)
+                     ibm_passes=passes, overlap=overlap, push=push)
+    if push:
+        transport.close()
     np.save(os.path.join(outdir, "part%d.npy" % rank), g.get_state())
     launches = g.launch_count
     g.close()
