@@ -329,7 +329,8 @@ class IpcPushTransport(DistTransport):
     A stream that waits for an interprocess event waits for the LAST record the host has issued, so the waiting host must
     know that the record has been issued: one host barrier of the control group (gloo: no device work, no stream is
     synchronised) between a record and the waits for it.  Per exchange: record, barrier, waits + pushes + record,
-    barrier, waits - the GPUs never idle for the host as long as the hosts run ahead of them.
+    barrier, waits - the GPUs never idle for the host as long as the hosts run ahead of them.  No KERNEL waits for
+    another rank (the waits are the stream's, cudaStreamWaitEvent), so the ranks may also share one GPU.
 
     Every exchange of the step goes this way (both stages, the un-forced W^{n+1} for IBM / rotor, between IBM passes);
     the scalar reductions and the rotor broadcast stay DistTransport's."""
@@ -377,6 +378,24 @@ class IpcPushTransport(DistTransport):
 
     def exchange(self, solver, which, new_buffer=None):
         self.exchange_push(solver, which)
+
+    # the same in two halves for the step in parts (SlabStepper.step(overlap=True)): the pushes are enqueued ahead of
+    # the interior sweeps, which read no HALO ghost; the rim waits for the neighbours' `landed` - recorded at the START
+    # of their stage, so it has long passed when the interior is done
+    def exchange_begin(self, solver, which, new_buffer=None):
+        st = solver.stream
+        self.ev_free.record(st)
+        self.dist.barrier(group=self.control)
+        for ev in self.peer_free.values():
+            st.wait_event(ev)
+        for face, dst, dst_face in self.d.schedule(self.rank):
+            solver.halo_push(which, face, self.win[dst][which])
+        self.ev_landed.record(st)
+
+    def exchange_end(self, solver, which, new_buffer=None):
+        self.dist.barrier(group=self.control)
+        for ev in self.peer_landed.values():
+            solver.stream.wait_event(ev)
 
     def close(self):
         """unmap the neighbours' workspaces (before they are freed): every stream idle, then a barrier"""

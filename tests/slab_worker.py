@@ -47,7 +47,7 @@ def main():
     import torch.distributed as dist
     from paper_2603_11102_b200 import gks, slab
     case, steps, outdir = sys.argv[1], int(sys.argv[2]), sys.argv[3]
-    overlap = len(sys.argv) > 4 and sys.argv[4] == "overlap"
+    overlap = len(sys.argv) > 4 and sys.argv[4] in ("overlap", "push-overlap")
     push = len(sys.argv) > 4 and sys.argv[4].startswith("push")   # halos written straight into the neighbour PROCESS's ghosts
     delay = len(sys.argv) > 4 and sys.argv[4] == "push-delay"     # one rank's GPU work runs late: only the interprocess
                                                                   # events keep its neighbours from reading stale ghosts

@@ -48,14 +48,16 @@ def single_domain(case):
                                              ("taylor_green", 2, "push"), ("taylor_green", 3, "push"),
                                              ("cylinder_passes", 3, "push"), ("channel", 2, "push"),
                                              ("rotor_online", 4, "push"), ("turbine", 3, "push"),
-                                             ("taylor_green", 3, "push-delay"), ("cylinder_passes", 2, "push-delay")])
+                                             ("taylor_green", 3, "push-delay"), ("cylinder_passes", 2, "push-delay"),
+                                             ("cylinder_full", 2, "push-overlap"), ("taylor_green", 2, "push-overlap")])
 def test_ranks_with_the_real_library_reproduce_the_single_domain(case, world, mode, tmp_path):
     """mode "overlap": the step in parts (slab.SlabStepper.step(overlap=True)): messages are posted before the interior
     is swept and completed before the rim; mode "push": no buffers, no messages - every rank writes its boundary planes
     into the ghost layers of its neighbour PROCESSES through CUDA IPC mappings, ordered by interprocess events
     (slab.IpcPushTransport), in every exchange of the step; "push-delay": the same with one rank's stream held back by
     30 ms in every step (another rank each step), so that its pushes land late and its ghosts stay in use late: the
-    hosts run ahead, only the events order the GPUs"""
+    hosts run ahead, only the events order the GPUs; "push-overlap": the step in parts with the pushes enqueued ahead of
+    the interior sweeps"""
     port = 29650 + (hash((case, world, mode)) % 200)
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(world),
            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.join(ROOT, "tests", "slab_worker.py"),
