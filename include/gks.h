@@ -188,6 +188,14 @@ gks_status gks_halo_export_get(gks_ctx *ctx, gks_halo_export *out);
 gks_status gks_halo_export_open(const gks_halo_export *in, gks_halo_window win[2], void **mapping);
 gks_status gks_halo_export_close(void *mapping);
 gks_status gks_step_begin(gks_ctx *ctx, double dt);
+/* gks_step_begin whose stage update ALSO writes the 3 planes of W* next to the low / high x face into the ghost planes of
+ * the neighbour given for that face (to_lo: the sub-domain beyond my low face, to_hi: beyond my high face; its window of
+ * state 1 from gks_halo_window_get or gks_halo_export_open; NULL: nobody) - update, pack, transfer and unpack in one
+ * kernel, peer-to-peer stores while the rest of the update runs.  Equal to gks_step_begin followed by
+ * gks_halo_push(ctx, 1, face, to) for those faces.  The neighbour's W* ghosts must be free (its previous step's second
+ * stage has run) and the neighbour must wait for this call's kernels before its gks_step_finish (the driver's order, as
+ * for gks_halo_push).  Errors as gks_step_begin and gks_halo_push. */
+gks_status gks_step_begin_push(gks_ctx *ctx, double dt, const gks_halo_window *to_lo, const gks_halo_window *to_hi);
 gks_status gks_step_finish(gks_ctx *ctx, double dt);
 gks_status gks_step_force(gks_ctx *ctx, double dt);
 gks_status gks_ibm_pass(gks_ctx *ctx, int pass, int phase /* 0 interpolate, 1 spread */);

@@ -127,7 +127,35 @@ gks_status gks_get_state(gks_ctx *ctx, double *W) {
   return GKS_OK;
 }
 
-gks_status gks_step_begin(gks_ctx *ctx, double dt) {
+namespace {
+gks_status step_begin_impl(gks_ctx *ctx, double dt, const GksPush *push);
+}
+
+gks_status gks_step_begin(gks_ctx *ctx, double dt) { return step_begin_impl(ctx, dt, nullptr); }
+
+gks_status gks_step_begin_push(gks_ctx *ctx, double dt, const gks_halo_window *to_lo, const gks_halo_window *to_hi) {
+  if (!ctx) return GKS_ERR_INVALID_ARG;
+  GksPush push;
+  memset(&push, 0, sizeof(push));
+  const gks_halo_window *to[2] = {to_lo, to_hi};
+  for (int f = 0; f < 2; ++f) {
+    if (!to[f]) continue;
+    if (!to[f]->W) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "the neighbour's window is NULL");
+    if (ctx->ph.bc[f] != GKS_BC_HALO) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "face %d is not a GKS_BC_HALO x face", f);
+    if (to[f]->ny != ctx->g.n[1] || to[f]->nz != ctx->g.n[2] || to[f]->nx < 6 || to[f]->pitch_x < to[f]->nx + 2 * GKS_NG ||
+        to[f]->pitch_y != to[f]->ny + 2 * GKS_NG)
+      return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "the neighbour's window does not match this sub-domain's y, z extents");
+    push.W[f] = to[f]->W;
+    push.nx[f] = to[f]->nx;
+    push.PX[f] = to[f]->pitch_x;
+    push.PY[f] = to[f]->pitch_y;
+    push.FS[f] = to[f]->field_stride;
+  }
+  return step_begin_impl(ctx, dt, &push);
+}
+
+namespace {
+gks_status step_begin_impl(gks_ctx *ctx, double dt, const GksPush *push) {
   if (!ctx) return GKS_ERR_INVALID_ARG;
   if (!ctx->have_state) return gks_set_err(ctx, GKS_ERR_STATE, "gks_step before gks_set_state");
   if (!(dt > 0) || !std::isfinite(dt)) return gks_set_err(ctx, GKS_ERR_INVALID_ARG, "dt must be > 0");
@@ -144,12 +172,13 @@ gks_status gks_step_begin(gks_ctx *ctx, double dt) {
   gks_prof_end(ctx);
   sweeps(ctx, ctx->Wn, true);
   gks_prof_begin(ctx, GKS_PROF_UPDATE);
-  ctx->launches += gks_launch_stage1(g, ctx->Wn, ctx->flux, dt, ctx->Ws, ctx->Pbuf, s);
+  ctx->launches += gks_launch_stage1(g, ctx->Wn, ctx->flux, dt, ctx->Ws, ctx->Pbuf, s, 0, -1, push);
   gks_prof_end(ctx);
   CUDA_TRY(ctx, cudaGetLastError());
   ctx->mid_step = 1;
   return GKS_OK;
 }
+} /* namespace */
 
 gks_status gks_step_finish(gks_ctx *ctx, double dt) {
   if (!ctx) return GKS_ERR_INVALID_ARG;

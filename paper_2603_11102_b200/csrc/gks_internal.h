@@ -220,9 +220,16 @@ bool gks_fused_init(gks_ctx *ctx);
 int gks_launch_sweep_fused(gks_ctx *ctx, int dir, int which, double *flux, bool need_F, int part = 0);
 void gks_fused_tiles_x(const GksGrid &g, int ta[3]);
 
+/* where the stage-1 update also stores the 3 planes of W* next to a cut x face: the padded state of the sub-domain
+   beyond my low face ([0]: its HIGH ghosts) and beyond my high face ([1]: its low ghosts); W = NULL: nobody */
+struct GksPush {
+  double *W[2];
+  int nx[2], PX[2], PY[2];
+  long long FS[2];
+};
 /* stage updates of the cells with x index in [x0, x1) (x1 < 0: the whole grid) */
 int gks_launch_stage1(const GksGrid &g, const double *Wn, double *const flux[3], double dt, double *Ws,
-                      double *Pbuf, cudaStream_t s, int x0 = 0, int x1 = -1);
+                      double *Pbuf, cudaStream_t s, int x0 = 0, int x1 = -1, const GksPush *push = nullptr);
 int gks_launch_stage2(const GksGrid &g, const double *Pbuf, double *const flux[3], double dt, double *Wn,
                       cudaStream_t s, int x0 = 0, int x1 = -1);
 /* y and z ghost passes over the x-ghost columns beyond the HALO faces only (after a halo unpack) */

@@ -23,7 +23,7 @@ EXPORTS = ["gks_workspace_bytes", "gks_create", "gks_destroy", "gks_set_state", 
            "gks_step_finish", "gks_step_force", "gks_bulk_partial", "gks_bulk_set_global", "gks_ibm_pass", "gks_ibm_residual",
            "gks_debug_eval_flux", "alm_rotor_supply", "gks_step_begin_part", "gks_step_finish_part", "gks_halo_window_get", "gks_halo_push",
            "gks_profile_enable", "gks_profile_read", "gks_check_finite", "gks_launch_count", "gks_last_error",
-           "gks_cfl_dt_noalloc", "gks_noalloc_last_error", "gks_halo_export_get", "gks_halo_export_open", "gks_halo_export_close"]
+           "gks_cfl_dt_noalloc", "gks_noalloc_last_error", "gks_halo_export_get", "gks_halo_export_open", "gks_halo_export_close", "gks_step_begin_push"]
 DEBUG_EXPORTS = ["gks_debug_set_sweep", "gks_debug_fp64_peak", "gks_debug_issue_probe", "gks_debug_trace"]    # include/gks_debug.h: libgks_b200_debug.so only
 
 
@@ -101,6 +101,7 @@ def lib(debug=False):
         L.gks_halo_window_get.argtypes = [vp, C.c_int, C.POINTER(HaloWindow)]
         L.gks_halo_push.argtypes = [vp, C.c_int, C.c_int, C.POINTER(HaloWindow)]
         L.gks_step_begin.argtypes = [vp, C.c_double]
+        L.gks_step_begin_push.argtypes = [vp, C.c_double, C.POINTER(HaloWindow), C.POINTER(HaloWindow)]
         L.gks_step_finish.argtypes = [vp, C.c_double]
         L.gks_step_force.argtypes = [vp, C.c_double]
         L.gks_step_begin_part.argtypes = [vp, C.c_double, C.c_int]
@@ -385,6 +386,12 @@ class Gks:
 
     def step_begin(self, dt):
         self._c("gks_step_begin", float(dt))
+
+    def step_begin_push(self, dt, to_lo=None, to_hi=None):
+        """step_begin whose stage update also writes W*'s boundary planes into the neighbours' ghost layers
+        (to_lo / to_hi: the HaloWindow of state 1 of the sub-domain beyond my low / high x face, or None)"""
+        self._c("gks_step_begin_push", float(dt), None if to_lo is None else C.byref(to_lo),
+                None if to_hi is None else C.byref(to_hi))
 
     def step_finish(self, dt):
         self._c("gks_step_finish", float(dt))

@@ -186,6 +186,19 @@ class LocalTransport:
         for s in solvers:
             s.synchronize()
 
+    def step_begin_push(self, solvers, dt):
+        """stage 1 with the exchange of W* fused into its update kernel (gks_step_begin_push): every sub-domain's
+        update also writes its boundary planes of W* into its neighbours' ghost layers"""
+        for s in solvers:                         # the neighbours' W* ghosts are free (their previous stage 2 has run)
+            s.synchronize()
+        for r, s in enumerate(solvers):
+            to = {face: solvers[dst].halo_window(1) for face, dst, dst_face in self.d.schedule(r)}
+            s.step_begin_push(dt, to.get(XLO), to.get(XHI))
+
+    def exchange_landed(self, solvers):
+        for s in solvers:                         # every update (and with it every push) has run
+            s.synchronize()
+
     # the same exchange in two halves, for the overlapped step (nothing overlaps inside one process: the hand-over
     # is a pointer; the split is what is exercised)
     def exchange_begin(self, solvers, which, new_buffer):
@@ -379,6 +392,20 @@ class IpcPushTransport(DistTransport):
     def exchange(self, solver, which, new_buffer=None):
         self.exchange_push(solver, which)
 
+    def step_begin_push(self, solver, dt):
+        """stage 1 with the exchange of W* fused into its update kernel.  The neighbours' W* ghosts are free: they
+        were last read by the neighbours' second stage of the step before, which precedes their `landed` of this
+        step's first exchange - and this stream has waited for that."""
+        to = {face: self.win[dst][1] for face, dst, dst_face in self.d.schedule(self.rank)}
+        solver.step_begin_push(dt, to.get(XLO), to.get(XHI))
+
+    def exchange_landed(self, solver):
+        """what is left of the second exchange: the order"""
+        self.ev_landed.record(solver.stream)
+        self.dist.barrier(group=self.control)
+        for ev in self.peer_landed.values():
+            solver.stream.wait_event(ev)
+
     # the same in two halves for the step in parts (SlabStepper.step(overlap=True)): the pushes are enqueued ahead of
     # the interior sweeps, which read no HALO ghost; the rim waits for the neighbours' `landed` - recorded at the START
     # of their stage, so it has long passed when the interior is done
@@ -552,8 +579,9 @@ class SlabStepper:
         ibm_passes: the max_iter given to ibm_set_iterations on every sub-domain, when > 1;
         overlap: the halos of either stage travel while the stage's interior is swept (PAPER.md:193-197 exchanges per
         flux evaluation; include/gks.h gks_step_begin_part): post, part 0, complete, part 1;
-        push: (sub-domains that can address one another's memory: LocalTransport) the two stage exchanges without
-        buffers, every sub-domain writing into its neighbours' ghost layers (gks_halo_push)"""
+        push: (sub-domains that can address one another's memory: LocalTransport, IpcPushTransport) the two stage
+        exchanges without buffers, every sub-domain writing into its neighbours' ghost layers (gks_halo_push);
+        push="fused": the exchange of W* is part of the stage-1 update kernel itself (gks_step_begin_push)"""
         if before_forcing is not None:
             self._each(before_forcing)
         if overlap:
@@ -565,6 +593,11 @@ class SlabStepper:
             self._each(lambda s: s.step_finish_part(dt, 0))
             self.t.exchange_end(self.solvers, 1, self.new_buffer)
             self._each(lambda s: s.step_finish_part(dt, 1))
+        elif push == "fused":
+            self.t.exchange_push(self.solvers, 0)                  # ghosts of W^n, written by the neighbours
+            self.t.step_begin_push(self.solvers, dt)               # the stage update writes the ghosts of W* as well
+            self.t.exchange_landed(self.solvers)
+            self._each(lambda s: s.step_finish(dt))
         elif push:
             self.t.exchange_push(self.solvers, 0)                  # ghosts of W^n, written by the neighbours
             self._each(lambda s: s.step_begin(dt))

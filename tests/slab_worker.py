@@ -49,7 +49,8 @@ def main():
     case, steps, outdir = sys.argv[1], int(sys.argv[2]), sys.argv[3]
     overlap = len(sys.argv) > 4 and sys.argv[4] in ("overlap", "push-overlap")
     push = len(sys.argv) > 4 and sys.argv[4].startswith("push")   # halos written straight into the neighbour PROCESS's ghosts
-    delay = len(sys.argv) > 4 and sys.argv[4] == "push-delay"     # one rank's GPU work runs late: only the interprocess
+    fused = len(sys.argv) > 4 and sys.argv[4].startswith("push-fused")   # W* travels inside the stage-1 update kernel
+    delay = len(sys.argv) > 4 and sys.argv[4] in ("push-delay", "push-fused-delay")     # one rank's GPU work runs late: only the interprocess
                                                                   # events keep its neighbours from reading stale ghosts
     os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
     dist.init_process_group("gloo")
@@ -76,7 +77,7 @@ def main():
             pts = d.alm_points(rank, *w.alm(k))
             hook = lambda s, pts=pts: s.alm_set_points(*pts)
         stepper.step(w.dt, before_forcing=hook, ibm=w.ibm is not None, rotor=rot, bulk=w.bulk_flux is not None,
-                     ibm_passes=passes, overlap=overlap, push=push)
+                     ibm_passes=passes, overlap=overlap, push=("fused" if fused else push))
     if push:
         transport.close()
     np.save(os.path.join(outdir, "part%d.npy" % rank), g.get_state())

@@ -389,3 +389,36 @@ def test_exchange_by_direct_push_equals_the_buffered_exchange(name, world):
         g0.halo_push(0, 1, win)                              # extents differ
     g0.close()
     g1.close()
+
+
+@pytest.mark.parametrize("name,world", [("C1", 2), ("C1", 3), ("C3", 4), ("C5", 3), ("C2", 2)])
+def test_stage_update_that_writes_the_neighbours_ghosts_equals_the_buffered_exchange(name, world):
+    """gks_step_begin_push: the stage-1 update kernel also stores the boundary planes of W* into the ghost layers of the
+    sub-domains beyond its cut faces (update, pack, transfer and unpack in one kernel): the same bits as the exchange
+    through buffers (two slabs on a periodic axis: the same neighbour on both sides); refusals"""
+    from paper_2603_11102_b200 import gks
+    w = wl.by_name(name, small=name != "C1")
+    Wb, Wf = run_slabs(w, world, 3), run_slabs(w, world, 3, push="fused")
+    if w.ibm is None:
+        assert np.array_equal(Wf, Wb)
+    else:
+        assert rel_linf(Wf, Wb) <= 1e-14
+    d = slab.SlabDecomposition(w.cfg, world)
+    g0, g1 = gks.Gks(d.local_cfg(0)), gks.Gks(d.local_cfg(1))
+    g0.set_state(d.scatter(w.W0, 0))
+    g1.set_state(d.scatter(w.W0, 1))
+    win = g1.halo_window(1)
+    if d.local_cfg(0).bc[0] != slab.BC_HALO:
+        with pytest.raises(gks.GksError):
+            g0.step_begin_push(w.dt, win, None)              # my low face is not a cut
+    win.nz += 1
+    with pytest.raises(gks.GksError):
+        g0.step_begin_push(w.dt, None, win)                  # extents differ
+    win.nz -= 1
+    with pytest.raises(gks.GksError):
+        g0.step_begin_push(-1.0, None, win)
+    g0.step_begin_push(w.dt, None, win)                      # accepted; the step is open now
+    with pytest.raises(gks.GksError):
+        g0.step_begin_push(w.dt, None, win)
+    g0.close()
+    g1.close()

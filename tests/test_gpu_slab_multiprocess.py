@@ -49,7 +49,9 @@ def single_domain(case):
                                              ("cylinder_passes", 3, "push"), ("channel", 2, "push"),
                                              ("rotor_online", 4, "push"), ("turbine", 3, "push"),
                                              ("taylor_green", 3, "push-delay"), ("cylinder_passes", 2, "push-delay"),
-                                             ("cylinder_full", 2, "push-overlap"), ("taylor_green", 2, "push-overlap")])
+                                             ("cylinder_full", 2, "push-overlap"), ("taylor_green", 2, "push-overlap"),
+                                             ("taylor_green", 2, "push-fused"), ("turbine", 3, "push-fused"),
+                                             ("cylinder_passes", 3, "push-fused-delay"), ("rotor_online", 4, "push-fused")])
 def test_ranks_with_the_real_library_reproduce_the_single_domain(case, world, mode, tmp_path):
     """mode "overlap": the step in parts (slab.SlabStepper.step(overlap=True)): messages are posted before the interior
     is swept and completed before the rim; mode "push": no buffers, no messages - every rank writes its boundary planes
@@ -57,7 +59,8 @@ def test_ranks_with_the_real_library_reproduce_the_single_domain(case, world, mo
     (slab.IpcPushTransport), in every exchange of the step; "push-delay": the same with one rank's stream held back by
     30 ms in every step (another rank each step), so that its pushes land late and its ghosts stay in use late: the
     hosts run ahead, only the events order the GPUs; "push-overlap": the step in parts with the pushes enqueued ahead of
-    the interior sweeps"""
+    the interior sweeps; "push-fused": the exchange of W* is part of the stage-1 update kernel (gks_step_begin_push writes
+    into the neighbour process's ghost layers as it computes), only the order is exchanged"""
     port = 29650 + (hash((case, world, mode)) % 200)
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(world),
            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.join(ROOT, "tests", "slab_worker.py"),
