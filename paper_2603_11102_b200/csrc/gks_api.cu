@@ -263,6 +263,8 @@ gks_status gks_create(const gks_config *cfg, void *workspace, size_t workspace_b
     g.uniform[a] = faces[a] == nullptr;
     g.x0[a] = x0[a];
     g.dx[a] = dx[a];
+    g.inv_w_u[a] = 1.0 / dx[a];
+    g.inv_12hn_u[a] = 1.0 / (12.0 * dx[a]);
     g.periodic[a] = cfg->bc[2 * a] == GKS_BC_PERIODIC;
     g.halo[2 * a] = cfg->bc[2 * a] == GKS_BC_HALO;
     g.halo[2 * a + 1] = cfg->bc[2 * a + 1] == GKS_BC_HALO;

@@ -34,6 +34,7 @@ struct GksGrid {
   const double *inv_12hn[3]; /* 1/(12 (xc[f]-xc[f-1])) for face f = -2 .. n+2, stored at f+3 (normal slope S5) */
   int uniform[3];
   double x0[3], dx[3];
+  double inv_w_u[3], inv_12hn_u[3];   /* uniform axis: the one value of inv_w / inv_12hn (kernel-parameter operands) */
   int periodic[3];
   int halo[6];       /* face carries GKS_BC_HALO: its ghost layers hold the neighbouring sub-domain's cells */
   int wrapf[3];      /* face n of this axis is not stored: it is face 0 (periodic axis, see gks_create) */

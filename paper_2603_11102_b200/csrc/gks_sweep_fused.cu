@@ -356,7 +356,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
       if (cn < TN) { /* right edge = face cn: Ql, and the slope at that face */
         const int fh = T::NA ? ct * HA + cn : cn * HA + ct;
         SA[QLo + fh * 4 + cc] = vr;
-        SA[DNo + fh * 4 + cc] = dn * g.inv_12hn[DIR][min(n0 + cn, g.n[DIR]) + GKS_NG];
+        SA[DNo + fh * 4 + cc] = dn * (g.uniform[DIR] ? g.inv_12hn_u[DIR] : g.inv_12hn[DIR][min(n0 + cn, g.n[DIR]) + GKS_NG]);
       }
     };
     auto edges_of_one = [&](int item) {
@@ -442,7 +442,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
         ga = cD.s.a0 + fa;
         gb = cD.s.b0 + fb;
         const int t1_glob = T::NA ? gb : ga;
-        const double iw1 = g.inv_w[T::AXT1][min(t1_glob, g.n[T::AXT1] - 1) + GKS_NG];
+        const double iw1 = g.uniform[T::AXT1] ? g.inv_w_u[T::AXT1] : g.inv_w[T::AXT1][min(t1_glob, g.n[T::AXT1] - 1) + GKS_NG];
         const double *q = Sb + ((i + 1) % 3) * T::SBUF + QLo + fh0 * 4 + c; /* Q0 of plane i-2 */
         const double *d = q + DNo;                                          /* Dn */
         double qq[5][2], vm[2], vp[2], sm_[2], sp_[2];
@@ -513,7 +513,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
     }
     /* ---- E: tangential pass 2 (along t2, the marched axis) for plane m = it-2; the ring holds planes
      *         it-4 .. it-1 (plane it-4+k in slot (it+k)&3), plane it comes straight from d6 ---- */
-    const double iw2 = g.inv_w[T::AXM][m + GKS_NG];
+    const double iw2 = g.uniform[T::AXM] ? g.inv_w_u[T::AXM] : g.inv_w[T::AXM][m + GKS_NG];
     const double *rs[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) rs[k] = rg + ((it + k) & 3) * RS;
