@@ -608,6 +608,8 @@ class HostPipeline:
         return sum(g.launch_count for g in self.ctx)
 
     def close(self):
+        """batches still in flight are abandoned: their streams are drained before the workspaces go"""
         for g in self.ctx:
+            g.synchronize()
             g.close()
-        self.ctx = []
+        self.ctx, self._pending = [], []
