@@ -9,6 +9,8 @@
  * the ghosts of the lower axes): initialised and advanced per axis, with the passes of the lower axes run in
  * between, so that a periodic / mirrored tangential ghost line carries the image of the ghost state.
  */
+#include <cstdlib>
+
 #include "gks_internal.h"
 
 namespace {
@@ -67,6 +69,68 @@ __global__ void __launch_bounds__(128) k_ghost(GksGrid g, GksPhys ph, double *W,
   }
 #pragma unroll
   for (int gi = 1; gi <= GKS_NG; ++gi) w[(side == 0 ? -gi : n - 1 + gi) * sa] = q[gi - 1];
+}
+
+/* The passes of several axes in ONE kernel, for the boundary kinds whose ghost is a signed copy of one cell (periodic
+ * image, wall mirrors, zero-gradient extrapolation): a ghost cell of the pass order x, y, z is then the signed copy of
+ * the interior cell that the per-axis index maps lead to, the sign being the product of the mirrors' - the value the
+ * three passes produce, bit for bit, without their launch-to-launch dependencies (a step of a small grid is a chain of
+ * short kernels).  WITH_X: x, y and z (x faces of those kinds or GKS_BC_HALO, whose ghosts are left alone and serve as
+ * sources of the y and z maps); otherwise y and z only, behind an x pass of the general kernel (inflow / outflow on x).
+ * Regions (blockIdx.y): 0 = the k-ghost planes, 1 = j-ghost rows of interior planes, 2 = i-ghost cells of interior rows. */
+__device__ __forceinline__ int ghost_map(int idx, int n, int kind_lo, int kind_hi, int axis, int c, double &sign) {
+  if (idx >= 0 && idx < n) return idx;
+  const int kind = idx < 0 ? kind_lo : kind_hi;
+  switch (kind) {
+    case BC_PERIODIC: return idx < 0 ? idx + n : idx - n;
+    case BC_NOSLIP:
+      if (c != 0) sign = -sign;
+      return idx < 0 ? -1 - idx : 2 * n - 1 - idx;
+    case BC_SLIP:
+      if (c == 1 + axis) sign = -sign;
+      return idx < 0 ? -1 - idx : 2 * n - 1 - idx;
+    case BC_EXTRAP: return idx < 0 ? 0 : n - 1;
+    default: return idx;   /* HALO (x only): the ghost holds the neighbouring sub-domain's cell */
+  }
+}
+
+template <bool WITH_X>
+__global__ void __launch_bounds__(256) k_ghost_fused(GksGrid g, GksPhys ph, double *W) {
+  gks_pdl_enter();
+  const int region = blockIdx.y, c = blockIdx.z;
+  const int n0 = g.n[0], n1 = g.n[1], n2 = g.n[2];
+  const int PXn = n0 + 2 * GKS_NG, PYn = n1 + 2 * GKS_NG;
+  const long long t = (long long)blockIdx.x * 256 + threadIdx.x;
+  int i, j, k;
+  if (region == 0) {
+    const long long per = (long long)PXn * PYn;
+    if (t >= 2 * GKS_NG * per) return;
+    const int l = (int)(t / per), r = (int)(t - l * per);
+    k = l < GKS_NG ? l - GKS_NG : n2 + l - GKS_NG;
+    j = r / PXn - GKS_NG;
+    i = r % PXn - GKS_NG;
+  } else if (region == 1) {
+    const long long per = (long long)PXn * 2 * GKS_NG;
+    if (t >= per * n2) return;
+    k = (int)(t / per);
+    const int r = (int)(t - k * per), l = r / PXn;
+    j = l < GKS_NG ? l - GKS_NG : n1 + l - GKS_NG;
+    i = r % PXn - GKS_NG;
+  } else {
+    const long long per = (long long)2 * GKS_NG * n1;
+    if (!WITH_X || t >= per * n2) return;
+    k = (int)(t / per);
+    const int r = (int)(t - k * per), l = r % (2 * GKS_NG);
+    j = r / (2 * GKS_NG);
+    i = l < GKS_NG ? l - GKS_NG : n0 + l - GKS_NG;
+    if (ph.bc[i < 0 ? 0 : 1] == BC_HALO) return;
+  }
+  double sign = 1.0;
+  const int is = WITH_X ? ghost_map(i, n0, ph.bc[0], ph.bc[1], 0, c, sign) : i;
+  const int js = ghost_map(j, n1, ph.bc[2], ph.bc[3], 1, c, sign);
+  const int ks = ghost_map(k, n2, ph.bc[4], ph.bc[5], 2, c, sign);
+  double *w = W + c * g.FS;
+  w[g.idx(i, j, k)] = sign * w[g.idx(is, js, ks)];
 }
 
 /* S20: initialise (dt < 0) or advance (dt >= 0) the convective-outflow ghost state of axis AX */
@@ -224,7 +288,29 @@ int outflow_state(const GksGrid &g, const GksPhys &ph, double *W, double dt, cud
 
 } /* namespace */
 
+static bool copy_kind(int kind) { return kind == BC_PERIODIC || kind == BC_NOSLIP || kind == BC_SLIP || kind == BC_EXTRAP; }
+
 int gks_launch_ghost_fill(const GksGrid &g, const GksPhys &ph, double *W, const double *Wstate, cudaStream_t s) {
+  static const bool fused_on = [] {
+    const char *e = getenv("GKS_GHOST_FUSED");        /* GKS_GHOST_FUSED=0: always the three passes */
+    return !(e && e[0] == '0');
+  }();
+  const bool yz = copy_kind(ph.bc[2]) && copy_kind(ph.bc[3]) && copy_kind(ph.bc[4]) && copy_kind(ph.bc[5]);
+  const bool x = (copy_kind(ph.bc[0]) || ph.bc[0] == BC_HALO) && (copy_kind(ph.bc[1]) || ph.bc[1] == BC_HALO);
+  if (fused_on && yz) {
+    const long long PXn = g.n[0] + 2 * GKS_NG, PYn = g.n[1] + 2 * GKS_NG;
+    long long most = 2 * GKS_NG * PXn * PYn;                                        /* region 0 */
+    if (2 * GKS_NG * PXn * g.n[2] > most) most = 2 * GKS_NG * PXn * g.n[2];         /* region 1 */
+    if (x && (long long)2 * GKS_NG * g.n[1] * g.n[2] > most) most = (long long)2 * GKS_NG * g.n[1] * g.n[2];
+    const dim3 grid((unsigned)((most + 255) / 256), x ? 3 : 2, 4);
+    if (x) {
+      gks_launch(k_ghost_fused<true>, grid, dim3(256), 0, s, g, ph, W);
+      return 1;
+    }
+    launch_ghost_axis<0>(g, ph, W, Wstate, s);
+    gks_launch(k_ghost_fused<false>, grid, dim3(256), 0, s, g, ph, W);
+    return 2;
+  }
   launch_ghost_axis<0>(g, ph, W, Wstate, s);
   launch_ghost_axis<1>(g, ph, W, Wstate, s);
   launch_ghost_axis<2>(g, ph, W, Wstate, s);
