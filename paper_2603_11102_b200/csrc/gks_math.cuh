@@ -354,7 +354,7 @@ __device__ __forceinline__ void series_coefficients(int func, double (&cf)[8]) {
 #pragma unroll
   for (int n = 0; n < 8; ++n) cf[n] = func ? GK_EXP[n] : GK_ERF[n];
 }
-__device__ __forceinline__ double erf_or_expm2_warp(double z, int func, const double (&cf)[8]) {
+__device__ __forceinline__ double erf_or_expm2_warp(double z, int func, const double *cf /* 8 coefficients of this lane's function */) {
   const double w = z * z;
   const bool small = !(w > 1.0 / 64.0);
   if (__all_sync(0xffffffffu, small)) {
