@@ -312,12 +312,13 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
   constexpr int RS = 6 * NF * 4, RF = NF * 4;   /* ring strides: plane slot, field */
   /* transpose buffer: element (field, component cc, Gauss point gq) of face fid lives at
    * fid*64 + field*16 + 4*(cc ^ (fid&3)) + (gq ^ cc): conflict-free for the component-major writes
-   * and for the Gauss-point-major reads of a half warp */
-  double *const xw = XBuf + fid * T::XF + 4 * (c ^ (fid & 3));             /* writes: + field*16 + (gq ^ c) */
-  const double *const xr = XBuf + fid * T::XF;                              /* reads:  + field*16 + ro[cc] */
-  int ro[4];
-#pragma unroll
-  for (int cc = 0; cc < 4; ++cc) ro[cc] = 4 * (cc ^ (fid & 3)) + (c ^ cc);
+   * and for the Gauss-point-major reads of a half warp.
+   * Both offsets are ONE xor of a per-thread constant with a compile-time one: a write of Gauss point gq goes to
+   * Kw ^ gq, Kw = 4 (c ^ (fid&3)) + c; a read of component cc comes from Kr ^ 5 cc, Kr = 4 (fid&3) + c. */
+  double *const xb = XBuf + fid * T::XF;
+  const int Kw = ((c ^ (fid & 3)) << 2) | c, Kr = ((fid & 3) << 2) | c;
+#define XW(field, gq) xb[(field) * 16 + (Kw ^ (gq))]
+#define XR(field, cc) xb[(field) * 16 + (Kr ^ (5 * (cc)))]
   constexpr int sn = T::NA ? 1 : EA;            /* slab stride along the normal */
   double bcf[8];                                /* the same coefficients per thread, for the out-of-line collision items
                                                    (extra halo faces, the long series): measured, handing those the
@@ -555,12 +556,12 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
           late[(fld - 1) * 4 + 2 * g1] = vm[u];
           late[(fld - 1) * 4 + 2 * g1 + 1] = vp[u];
         } else {
-          xw[fld * 16 + ((2 * g1) ^ c)] = vm[u];
-          xw[fld * 16 + ((2 * g1 + 1) ^ c)] = vp[u];
+          XW(fld, 2 * g1) = vm[u];
+          XW(fld, 2 * g1 + 1) = vp[u];
         }
         if (fld == 0) {
-          xw[(GKS_XHALF ? 1 : 3) * 16 + ((2 * g1) ^ c)] = sm_[u] * iw2;
-          xw[(GKS_XHALF ? 1 : 3) * 16 + ((2 * g1 + 1) ^ c)] = sp_[u] * iw2;
+          XW(GKS_XHALF ? 1 : 3, 2 * g1) = sm_[u] * iw2;
+          XW(GKS_XHALF ? 1 : 3, 2 * g1 + 1) = sp_[u] * iw2;
         }
       }
     }
@@ -574,28 +575,28 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
            and Dt1 */
 #pragma unroll
         for (int cc = 0; cc < 4; ++cc) {
-          Q0[cc] = xr[0 * 16 + ro[cc]];
-          dQ[T::AXM][cc] = xr[1 * 16 + ro[cc]];
+          Q0[cc] = XR(0, cc);
+          dQ[T::AXM][cc] = XR(1, cc);
         }
         __syncwarp();
 #pragma unroll
         for (int gq = 0; gq < 4; ++gq) {
-          xw[0 * 16 + (gq ^ c)] = late[gq];
-          xw[1 * 16 + (gq ^ c)] = late[4 + gq];
+          XW(0, gq) = late[gq];
+          XW(1, gq) = late[4 + gq];
         }
         __syncwarp();
 #pragma unroll
         for (int cc = 0; cc < 4; ++cc) {
-          dQ[DIR][cc] = xr[0 * 16 + ro[cc]];
-          dQ[T::AXT1][cc] = xr[1 * 16 + ro[cc]];
+          dQ[DIR][cc] = XR(0, cc);
+          dQ[T::AXT1][cc] = XR(1, cc);
         }
       } else {
 #pragma unroll
         for (int cc = 0; cc < 4; ++cc) {
-          Q0[cc] = xr[0 * 16 + ro[cc]];
-          dQ[DIR][cc] = xr[1 * 16 + ro[cc]];
-          dQ[T::AXT1][cc] = xr[2 * 16 + ro[cc]];
-          dQ[T::AXM][cc] = xr[3 * 16 + ro[cc]];
+          Q0[cc] = XR(0, cc);
+          dQ[DIR][cc] = XR(1, cc);
+          dQ[T::AXT1][cc] = XR(2, cc);
+          dQ[T::AXM][cc] = XR(3, cc);
         }
       }
       gksd::gauss_point_flux<DIR, NEED_F>(Q0, dQ, ph.RT, ph.mu, F, dF);
