@@ -189,7 +189,7 @@ struct Seg {
 template <int DIR, bool NEED_F, bool LIN, int TA, int TB>
 __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
     k_sweep_fused(const __grid_constant__ CUtensorMap tmap, GksGrid g, GksPhys ph, double *__restrict__ flux,
-                  int ncol_a, int nfull, long long rem, long long PPC, int ta0, int tlen0, int ta1) {
+                  int ncol_a, int nfull, long long rem, long long PPC, int ta0, int tlen0, int ta1, int n_a, int n_b) {
   using T = Tile<DIR, TA, TB>;
   constexpr int TN = T::TN, NF = T::NF, NT = T::NT, EA = T::EA, EB = T::EB, HA = T::HA, FH = T::FH;
   constexpr bool FUSE_BCD = GKS_FUSE_BCD == 1 || GKS_FUSE_BCD == 3 || (GKS_FUSE_BCD == 2 && DIR != 0);
@@ -304,7 +304,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
   const int c = tid & 3, fid = tid >> 2;
   const int fa = fid % TA, fb = fid / TA;       /* a fastest: coalesced output */
   /* faces to store: n+1 along the normal, n on a periodic axis (face n is face 0) */
-  const int n_a = g.n[0] + (T::NA && !g.wrapf[0] ? 1 : 0), n_b = g.n[T::AXB] + (!T::NA && !g.wrapf[T::AXB] ? 1 : 0);
+  /* n_a, n_b (kernel parameters): n + 1 along the normal unless that axis wraps */
   const int t1_local = T::NA ? fb : fa;
   constexpr int s1 = T::NA ? HA : 1;            /* halo-face stride along t1 */
   const int fh0 = T::NA ? (t1_local + 2) * HA + fa : fb * HA + (t1_local + 2);
@@ -326,8 +326,15 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
   gksd::series_coefficients((tid & 3) >> 1, bcf);
   constexpr int QLo = 0, QRo = FH * 4 + 2, DNo = 2 * FH * 4 + 4;   /* offsets inside a stage buffer */
 
+  /* offsets of the three stage buffers in turn, rotated once per iteration: plane i lives in buffer i % 3, so stage A
+     works at (i % 3) SBUF, BC at ((i + 2) % 3) SBUF, D at ((i + 1) % 3) SBUF (three moves instead of three mod-3) */
+  int sA = 0, sB = 2 * T::SBUF, sD = T::SBUF;
   TR_DECL
   for (int i = 0; i < J + 2; ++i) {
+    const int oA = sA, oB = sB, oD = sD;
+    sA = oD;
+    sB = oA;
+    sD = oB;
     TR(0)   /* loop bookkeeping between two iterations */
     /* ONE hand-over per iteration: phase i-1 of the iteration barrier completes when every warp has finished
        A, BC, D of iteration i-1 AND the slab of plane i has landed - its TMA was issued at the top of iteration
@@ -352,7 +359,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
      * stores and the extra item follow that block. */
     const bool okA = i < J;
     const double *const W = Wp + (i & 1) * T::WSLAB_PAD;
-    double *const SA = Sb + (i % 3) * T::SBUF;
+    double *const SA = Sb + oA;
     constexpr int NITEM = T::NCA * T::NCB * 4;
     const int n0 = T::NA ? cA.s.a0 : cA.s.b0;     /* global index of normal face 0 of the tile */
     auto locate = [&](int item, const double *&w, int &cn, int &ct, int &cc) {
@@ -434,7 +441,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
     double d6[6];
     int ga = 0, gb = 0;
     {
-      double *const S = Sb + ((i + 2) % 3) * T::SBUF;               /* plane i-1 */
+      double *const S = Sb + oB;                                    /* plane i-1 */
       static_assert((FH * 4) % 32 == 0, "whole warps in the collision stage");
       const int gl = (tid & 31) & ~3;               /* first lane of this face group */
       constexpr int NXB = FH * 4 - NT;              /* extra items: a rotating window of whole warps, disjoint from A's */
@@ -459,7 +466,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
         gb = cD.s.b0 + fb;
         const int t1_glob = T::NA ? gb : ga;
         const double iw1 = g.uniform[T::AXT1] ? g.inv_w_u[T::AXT1] : g.inv_w[T::AXT1][min(t1_glob, g.n[T::AXT1] - 1) + GKS_NG];
-        const double *q = Sb + ((i + 1) % 3) * T::SBUF + QLo + fh0 * 4 + c; /* Q0 of plane i-2 */
+        const double *q = Sb + oD + QLo + fh0 * 4 + c;                      /* Q0 of plane i-2 */
         const double *d = q + DNo;                                          /* Dn */
         double qq[5][2], vm[2], vp[2], sm_[2], sp_[2];
 #pragma unroll
@@ -693,7 +700,6 @@ int launch_dir(gks_ctx *ctx, const CUtensorMap &map, double *flux, int ta0, int 
   const int ext_a = g.n[0] + (T::NA && !g.wrapf[0] ? 1 : 0), ext_b = g.n[T::AXB] + (!T::NA && !g.wrapf[T::AXB] ? 1 : 0);
   const int n2 = g.n[T::AXM];
   const int ga = len0 + len1, gb = (ext_b + TB - 1) / TB;
-  (void)ext_a;
   if (ga <= 0) return 0;
   /* persistent CTAs: the (column, plane) list is cut into equal contiguous ranges, one per resident CTA;
      a range shorter than 8 planes is not worth its 4 priming planes */
@@ -703,7 +709,7 @@ int launch_dir(gks_ctx *ctx, const CUtensorMap &map, double *flux, int ta0, int 
   long long PPC = (rem + grid - 1) / grid;
   if (PPC < GKS_MIN_PPC) PPC = GKS_MIN_PPC;                    /* shortest range worth its 4 priming planes */
   if (nfull == 0) grid = (int)((rem + PPC - 1) / PPC);
-  gks_launch(kern, grid, dim3(T::NT), T::SMEM_BYTES, ctx->stream, map, g, ctx->ph, flux, ga, nfull, rem, PPC, ta0, len0, ta1 - len0);
+  gks_launch(kern, grid, dim3(T::NT), T::SMEM_BYTES, ctx->stream, map, g, ctx->ph, flux, ga, nfull, rem, PPC, ta0, len0, ta1 - len0, ext_a, ext_b);
   return 1;
 }
 
