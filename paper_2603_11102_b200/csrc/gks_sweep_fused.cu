@@ -258,10 +258,10 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
       if (c.l < L1) c.s = seg_at(c.l);
     }
   };
-  Cur cT, cA, cD;
+  Cur cT, cD;
   cT.l = L0; cT.s = seg_at(L0); cT.it = 0;
-  cA = cT;
   cD = cT;
+  int n0_next = T::NA ? cT.s.a0 : cT.s.b0;     /* stage A: normal face 0 of the tile of the plane it works on next */
 
   /* stage BC: the 8 Maclaurin coefficients of erf (lanes with func = 0) and of exp(-z^2) (func = 1) sit in shared memory;
      a lane reads its own set every plane (two addresses per warp: one wavefront) - cheaper than what the compiler makes
@@ -329,12 +329,23 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
   /* offsets of the three stage buffers in turn, rotated once per iteration: plane i lives in buffer i % 3, so stage A
      works at (i % 3) SBUF, BC at ((i + 2) % 3) SBUF, D at ((i + 1) % 3) SBUF (three moves instead of three mod-3) */
   int sA = 0, sB = 2 * T::SBUF, sD = T::SBUF;
+  int rq0 = 2 * (6 * NF * 4), rq1 = 3 * (6 * NF * 4), rq2 = 0, rq3 = 6 * NF * 4;   /* slots of planes i-6 .. i-3 at i = 0 */
   TR_DECL
   for (int i = 0; i < J + 2; ++i) {
     const int oA = sA, oB = sB, oD = sD;
     sA = oD;
     sB = oA;
     sD = oB;
+    /* ring slots likewise: the plane that stage D produces in iteration i sits in slot (i - 2) & 3 (slots follow the
+       iteration count, not the position in the column segment: a new segment primes 4 planes before pass 2 reads any) */
+    const int q0 = rq0, q1 = rq1, q2 = rq2, q3 = rq3;
+    rq0 = q1;
+    rq1 = q2;
+    rq2 = q3;
+    rq3 = q0;
+    /* cT describes plane i + 1 here: what stage A needs of it in the NEXT iteration */
+    const int n0_A = n0_next;
+    n0_next = T::NA ? cT.s.a0 : cT.s.b0;
     TR(0)   /* loop bookkeeping between two iterations */
     /* ONE hand-over per iteration: phase i-1 of the iteration barrier completes when every warp has finished
        A, BC, D of iteration i-1 AND the slab of plane i has landed - its TMA was issued at the top of iteration
@@ -361,7 +372,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
     const double *const W = Wp + (i & 1) * T::WSLAB_PAD;
     double *const SA = Sb + oA;
     constexpr int NITEM = T::NCA * T::NCB * 4;
-    const int n0 = T::NA ? cA.s.a0 : cA.s.b0;     /* global index of normal face 0 of the tile */
+    const int n0 = n0_A;                          /* global index of normal face 0 of the tile */
     auto locate = [&](int item, const double *&w, int &cn, int &ct, int &cc) {
       cc = item & 3;
       const int cell = item >> 2;
@@ -423,7 +434,6 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
       } else {
         edges_of_one(tid);
       }
-      cur_next(cA);
     }
 
     TR(3)   /* stage A */
@@ -514,7 +524,6 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
     if (FUSE_A && okA) {
       store(a_cn, a_ct, a_cc, a_vl[0], a_vr[0], a_dn);
       if (xa_id < NXA) edges_of_one(NT + xa_id);
-      cur_next(cA);
     }
     /* this warp is done with the shared stage buffers of iteration i */
     __syncwarp();
@@ -528,7 +537,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
     const bool face_ok = ga < n_a && gb < n_b;
     cur_next(cD);
 
-    double *const rnew = rg + (it & 3) * RS;     /* slot of plane it-4, dead once pass 2 below has read it */
+    double *const rnew = rg + q0;                /* slot of the plane four back, dead once pass 2 below has read it */
     if (it < 4) {
 #pragma unroll
       for (int v = 0; v < 6; ++v) rnew[v * RF] = d6[v];
@@ -537,9 +546,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
     /* ---- E: tangential pass 2 (along t2, the marched axis) for plane m = it-2; the ring holds planes
      *         it-4 .. it-1 (plane it-4+k in slot (it+k)&3), plane it comes straight from d6 ---- */
     const double iw2 = g.uniform[T::AXM] ? g.inv_w_u[T::AXM] : g.inv_w[T::AXM][m + GKS_NG];
-    const double *rs[4];
-#pragma unroll
-    for (int k = 0; k < 4; ++k) rs[k] = rg + ((it + k) & 3) * RS;
+    const double *const rs[4] = {rg + q0, rg + q1, rg + q2, rg + q3};
     /* the six evaluations (field Q0, Dn, Dt1) x (g1 = -, +) run EW at a time, statement-interleaved */
     constexpr int EW = GKS_E_WIDTH;
     static_assert(6 % EW == 0, "E width");
