@@ -45,6 +45,9 @@ size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 const char *validate(const gks_config *c) {
   if (!c) return "config is NULL";
   if (c->nx < 6 || c->ny < 6 || c->nz < 6) return "nx, ny, nz must each be >= 6";
+  /* kernels index a padded field with 32 bits (a field of 2^31 doubles is 17 GB; 36 of them exceed any one GPU) */
+  if (((long long)c->nx + 9) * ((long long)c->ny + 6) * ((long long)c->nz + 6) >= 2147483647LL)
+    return "too many cells: a padded field must hold fewer than 2^31 doubles";
   if (!(c->RT > 0)) return "RT must be > 0";
   if (!(c->nu >= 0)) return "nu must be >= 0";
   if (!(c->rho_ref > 0)) return "rho_ref must be > 0";

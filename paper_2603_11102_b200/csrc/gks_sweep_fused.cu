@@ -316,7 +316,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
    * Both offsets are ONE xor of a per-thread constant with a compile-time one: a write of Gauss point gq goes to
    * Kw ^ gq, Kw = 4 (c ^ (fid&3)) + c; a read of component cc comes from Kr ^ 5 cc, Kr = 4 (fid&3) + c. */
   double *const xb = XBuf + fid * T::XF;
-  const int Kw = ((c ^ (fid & 3)) << 2) | c, Kr = ((fid & 3) << 2) | c;
+  const int Kr = tid & 15, Kw = Kr ^ ((tid & 3) << 2);   /* fid = tid >> 2, c = tid & 3 */
 #define XW(field, gq) xb[(field) * 16 + (Kw ^ (gq))]
 #define XR(field, cc) xb[(field) * 16 + (Kr ^ (5 * (cc)))]
   constexpr int sn = T::NA ? 1 : EA;            /* slab stride along the normal */
@@ -390,7 +390,9 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
       if (cn < TN) { /* right edge = face cn: Ql, and the slope at that face */
         const int fh = T::NA ? ct * HA + cn : cn * HA + ct;
         SA[QLo + fh * 4 + cc] = vr;
-        SA[DNo + fh * 4 + cc] = dn * (g.uniform[DIR] ? g.inv_12hn_u[DIR] : g.inv_12hn[DIR][min(n0 + cn, g.n[DIR]) + GKS_NG]);
+        double mf = g.inv_12hn_u[DIR];
+        if (!g.uniform[DIR]) mf = g.inv_12hn[DIR][min(n0 + cn, g.n[DIR]) + GKS_NG];
+        SA[DNo + fh * 4 + cc] = dn * mf;
       }
     };
     auto edges_of_one = [&](int item) {
@@ -475,7 +477,8 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
         ga = cD.s.a0 + fa;
         gb = cD.s.b0 + fb;
         const int t1_glob = T::NA ? gb : ga;
-        const double iw1 = g.uniform[T::AXT1] ? g.inv_w_u[T::AXT1] : g.inv_w[T::AXT1][min(t1_glob, g.n[T::AXT1] - 1) + GKS_NG];
+        double iw1 = g.inv_w_u[T::AXT1];
+        if (!g.uniform[T::AXT1]) iw1 = g.inv_w[T::AXT1][min(t1_glob, g.n[T::AXT1] - 1) + GKS_NG];
         const double *q = Sb + oD + QLo + fh0 * 4 + c;                      /* Q0 of plane i-2 */
         const double *d = q + DNo;                                          /* Dn */
         double qq[5][2], vm[2], vp[2], sm_[2], sp_[2];
@@ -545,7 +548,8 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
     }
     /* ---- E: tangential pass 2 (along t2, the marched axis) for plane m = it-2; the ring holds planes
      *         it-4 .. it-1 (plane it-4+k in slot (it+k)&3), plane it comes straight from d6 ---- */
-    const double iw2 = g.uniform[T::AXM] ? g.inv_w_u[T::AXM] : g.inv_w[T::AXM][m + GKS_NG];
+    double iw2 = g.inv_w_u[T::AXM];
+    if (!g.uniform[T::AXM]) iw2 = g.inv_w[T::AXM][m + GKS_NG];
     const double *const rs[4] = {rg + q0, rg + q1, rg + q2, rg + q3};
     /* the six evaluations (field Q0, Dn, Dt1) x (g1 = -, +) run EW at a time, statement-interleaved */
     constexpr int EW = GKS_E_WIDTH;
@@ -618,17 +622,15 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
       /* face average: the 4 lanes of a face (one Gauss point each) leave their F, dF in the warp-private
          buffer, lane c sums component c in the order (g0+g1)+(g2+g3).  Row v of face fid sits at
          ((v ^ (fid&3)) * 4 + gp): conflict-free 64-bit stores and loads */
-      double *const xs = XBuf + fid * T::XF;
-      const int f3 = fid & 3;
 #pragma unroll
-      for (int v = 0; v < 4; ++v) {
-        if (NEED_F) xs[(v ^ f3) * 4 + c] = F[v];
-        xs[16 + (v ^ f3) * 4 + c] = dF[v];
+      for (int v = 0; v < 4; ++v) {               /* (v ^ (fid&3)) * 4 + c = Kr ^ 4 v */
+        if (NEED_F) xb[Kr ^ (4 * v)] = F[v];
+        xb[16 + (Kr ^ (4 * v))] = dF[v];
       }
       __syncwarp();
       double fsel = 0.0, dsel;
       {
-        const double *r = xs + (c ^ f3) * 4;
+        const double *r = xb + (Kw & 12);         /* (c ^ (fid&3)) * 4 */
         if (NEED_F) fsel = (r[0] + r[1]) + (r[2] + r[3]);
         dsel = (r[16] + r[17]) + (r[18] + r[19]);
       }
@@ -638,9 +640,11 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
         pidx[0] = ga;
         pidx[T::AXB] = gb;
         pidx[T::AXM] = m;
-        const long long id = g.idx(pidx[0], pidx[1], pidx[2]);
-        if (NEED_F) flux[c * g.FS + id] = 0.25 * fsel;
-        flux[(4 + c) * g.FS + id] = 0.25 * dsel;
+        /* a padded field holds fewer than 2^31 doubles (gks_create): the cell index is a 32-bit number */
+        const int id = ((pidx[2] + GKS_NG) * g.P[1] + (pidx[1] + GKS_NG)) * g.P[0] + (pidx[0] + GKS_NG);
+        double *const fc = flux + c * g.FS;
+        if (NEED_F) fc[id] = 0.25 * fsel;
+        fc[4 * g.FS + id] = 0.25 * dsel;
       }
     }
     TR(6)   /* transposes, flux, face average, store (F) */
