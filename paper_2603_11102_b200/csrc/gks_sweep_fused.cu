@@ -329,7 +329,9 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
   /* offsets of the three stage buffers in turn, rotated once per iteration: plane i lives in buffer i % 3, so stage A
      works at (i % 3) SBUF, BC at ((i + 2) % 3) SBUF, D at ((i + 1) % 3) SBUF (three moves instead of three mod-3) */
   int sA = 0, sB = 2 * T::SBUF, sD = T::SBUF;
-  int rq0 = 2 * (6 * NF * 4), rq1 = 3 * (6 * NF * 4), rq2 = 0, rq3 = 6 * NF * 4;   /* slots of planes i-6 .. i-3 at i = 0 */
+  const double *wA = Wp, *wB = Wp + T::WSLAB_PAD;
+  /* slots of planes i-6 .. i-3 at i = 0, as pointers to this thread's column */
+  double *rq0 = rg + 2 * (6 * NF * 4), *rq1 = rg + 3 * (6 * NF * 4), *rq2 = rg, *rq3 = rg + 6 * NF * 4;
   TR_DECL
   for (int i = 0; i < J + 2; ++i) {
     const int oA = sA, oB = sB, oD = sD;
@@ -338,11 +340,14 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
     sD = oB;
     /* ring slots likewise: the plane that stage D produces in iteration i sits in slot (i - 2) & 3 (slots follow the
        iteration count, not the position in the column segment: a new segment primes 4 planes before pass 2 reads any) */
-    const int q0 = rq0, q1 = rq1, q2 = rq2, q3 = rq3;
+    double *const q0 = rq0, *const q1 = rq1, *const q2 = rq2, *const q3 = rq3;
     rq0 = q1;
     rq1 = q2;
     rq2 = q3;
     rq3 = q0;
+    const double *const wcur = wA;                /* slab of plane i; the other one receives plane i + 1 */
+    wA = wB;
+    wB = wcur;
     /* cT describes plane i + 1 here: what stage A needs of it in the NEXT iteration */
     const int n0_A = n0_next;
     n0_next = T::NA ? cT.s.a0 : cT.s.b0;
@@ -369,7 +374,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
      * result dropped) as the head of the straight-line block that continues through BC and D below, and the
      * stores and the extra item follow that block. */
     const bool okA = i < J;
-    const double *const W = Wp + (i & 1) * T::WSLAB_PAD;
+    const double *const W = wcur;
     double *const SA = Sb + oA;
     constexpr int NITEM = T::NCA * T::NCB * 4;
     const int n0 = n0_A;                          /* global index of normal face 0 of the tile */
@@ -540,7 +545,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
     const bool face_ok = ga < n_a && gb < n_b;
     cur_next(cD);
 
-    double *const rnew = rg + q0;                /* slot of the plane four back, dead once pass 2 below has read it */
+    double *const rnew = q0;                     /* slot of the plane four back, dead once pass 2 below has read it */
     if (it < 4) {
 #pragma unroll
       for (int v = 0; v < 6; ++v) rnew[v * RF] = d6[v];
@@ -550,7 +555,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
      *         it-4 .. it-1 (plane it-4+k in slot (it+k)&3), plane it comes straight from d6 ---- */
     double iw2 = g.inv_w_u[T::AXM];
     if (!g.uniform[T::AXM]) iw2 = g.inv_w[T::AXM][m + GKS_NG];
-    const double *const rs[4] = {rg + q0, rg + q1, rg + q2, rg + q3};
+    const double *const rs[4] = {q0, q1, q2, q3};
     /* the six evaluations (field Q0, Dn, Dt1) x (g1 = -, +) run EW at a time, statement-interleaved */
     constexpr int EW = GKS_E_WIDTH;
     static_assert(6 % EW == 0, "E width");
