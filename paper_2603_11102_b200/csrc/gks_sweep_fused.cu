@@ -412,7 +412,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
     };
     constexpr int NXA = NITEM - NT;
     static_assert(NXA >= 0 && NXA <= NT, "stage A: at most two items per thread");
-    const int xa_id = (tid - 32 * ((i * 5) % T::NW)) & (NT - 1);
+    const int xa_id = (tid - 160 * i) & (NT - 1);   /* = (tid - 32 ((5 i) mod NW)) mod NT: the window moves 5 warps per iteration */
     double a_vl[1], a_vr[1], a_dn = 0.0;
     int a_cn = 0, a_ct = 0, a_cc = 0;
     if (FUSE_A) {
@@ -463,7 +463,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
       const int gl = (tid & 31) & ~3;               /* first lane of this face group */
       constexpr int NXB = FH * 4 - NT;              /* extra items: a rotating window of whole warps, disjoint from A's */
       static_assert(NXB >= 0 && NXB <= NT / 2 && NXB % 32 == 0, "stage BC: extras on whole warps");
-      const int xb_id = (tid - 32 * ((i * 5 + T::NW / 2) % T::NW)) & (NT - 1);
+      const int xb_id = xa_id ^ (NT / 2);           /* the same window half the warps further on */
       auto collide = [&](int item) {
         const int cc = item & 3, fh = item >> 2, side = cc & 1, func = cc >> 1;
         const double *qs = S + (side ? QRo : QLo) + fh * 4;
