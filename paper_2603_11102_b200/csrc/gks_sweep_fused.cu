@@ -186,7 +186,7 @@ struct Seg {
  * an iteration without anyone waiting.  A thread's own BC item and its D item are written as one
  * straight-line block (GKS_FUSE_BCD): BC's serial chain issues in the shadow of D's arithmetic.
  */
-template <int DIR, bool NEED_F, bool LIN, int TA, int TB>
+template <int DIR, bool NEED_F, bool LIN, int TA, int TB, bool UNIF>
 __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
     k_sweep_fused(const __grid_constant__ CUtensorMap tmap, GksGrid g, GksPhys ph, double *__restrict__ flux,
                   int ncol_a, int nfull, long long rem, long long PPC, int ta0, int tlen0, int ta1, int n_a, int n_b) {
@@ -396,7 +396,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
         const int fh = T::NA ? ct * HA + cn : cn * HA + ct;
         SA[QLo + fh * 4 + cc] = vr;
         double mf = g.inv_12hn_u[DIR];
-        if (!g.uniform[DIR]) mf = g.inv_12hn[DIR][min(n0 + cn, g.n[DIR]) + GKS_NG];
+        if (!UNIF && !g.uniform[DIR]) mf = g.inv_12hn[DIR][min(n0 + cn, g.n[DIR]) + GKS_NG];
         SA[DNo + fh * 4 + cc] = dn * mf;
       }
     };
@@ -483,7 +483,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
         gb = cD.s.b0 + fb;
         const int t1_glob = T::NA ? gb : ga;
         double iw1 = g.inv_w_u[T::AXT1];
-        if (!g.uniform[T::AXT1]) iw1 = g.inv_w[T::AXT1][min(t1_glob, g.n[T::AXT1] - 1) + GKS_NG];
+        if (!UNIF && !g.uniform[T::AXT1]) iw1 = g.inv_w[T::AXT1][min(t1_glob, g.n[T::AXT1] - 1) + GKS_NG];
         const double *q = Sb + oD + QLo + fh0 * 4 + c;                      /* Q0 of plane i-2 */
         const double *d = q + DNo;                                          /* Dn */
         double qq[5][2], vm[2], vp[2], sm_[2], sp_[2];
@@ -554,7 +554,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
     /* ---- E: tangential pass 2 (along t2, the marched axis) for plane m = it-2; the ring holds planes
      *         it-4 .. it-1 (plane it-4+k in slot (it+k)&3), plane it comes straight from d6 ---- */
     double iw2 = g.inv_w_u[T::AXM];
-    if (!g.uniform[T::AXM]) iw2 = g.inv_w[T::AXM][m + GKS_NG];
+    if (!UNIF && !g.uniform[T::AXM]) iw2 = g.inv_w[T::AXM][m + GKS_NG];
     const double *const rs[4] = {q0, q1, q2, q3};
     /* the six evaluations (field Q0, Dn, Dt1) x (g1 = -, +) run EW at a time, statement-interleaved */
     constexpr int EW = GKS_E_WIDTH;
@@ -700,12 +700,12 @@ int tiles_a(const GksGrid &g, int dir) {
 }
 
 /* launch over the a-tiles [ta0, ta0 + len0) and [ta1, ta1 + len1) (len1 may be 0); returns the launches made */
-template <int DIR, bool NEED_F, bool LIN, int XA>
+template <int DIR, bool NEED_F, bool LIN, int XA, bool UNIF>
 int launch_dir(gks_ctx *ctx, const CUtensorMap &map, double *flux, int ta0, int len0, int ta1, int len1) {
   constexpr int TA = Shape<DIR, XA>::TA, TB = Shape<DIR, XA>::TB;
   using T = Tile<DIR, TA, TB>;
   const GksGrid &g = ctx->g;
-  auto kern = k_sweep_fused<DIR, NEED_F, LIN, TA, TB>;
+  auto kern = k_sweep_fused<DIR, NEED_F, LIN, TA, TB, UNIF>;   /* UNIF: all three axes uniform - no metric tables */
   static bool attr_done[64] = {};                /* the attribute is per device: one process may hold contexts on several */
   int dev = 0;
   cudaGetDevice(&dev);
@@ -788,14 +788,19 @@ int gks_launch_sweep_fused(gks_ctx *ctx, int dir, int which, double *flux, bool 
       len1 = all - t1;
     }
   }
-#define GKS_DISPATCH(D, XA)                                                                                                   \
-  (need_F ? (lin ? launch_dir<D, true, true, XA>(ctx, m, flux, ta0, len0, ta1, len1) : launch_dir<D, true, false, XA>(ctx, m, flux, ta0, len0, ta1, len1))  \
-          : (lin ? launch_dir<D, false, true, XA>(ctx, m, flux, ta0, len0, ta1, len1) : launch_dir<D, false, false, XA>(ctx, m, flux, ta0, len0, ta1, len1)))
+  const bool unif = ctx->g.uniform[0] && ctx->g.uniform[1] && ctx->g.uniform[2];
+#define GKS_DISPATCH3(D, XA, NF_, LIN_)                                                                      \
+  (unif ? launch_dir<D, NF_, LIN_, XA, true>(ctx, m, flux, ta0, len0, ta1, len1)                             \
+        : launch_dir<D, NF_, LIN_, XA, false>(ctx, m, flux, ta0, len0, ta1, len1))
+#define GKS_DISPATCH(D, XA)                                                                                  \
+  (need_F ? (lin ? GKS_DISPATCH3(D, XA, true, true) : GKS_DISPATCH3(D, XA, true, false))                     \
+          : (lin ? GKS_DISPATCH3(D, XA, false, true) : GKS_DISPATCH3(D, XA, false, false)))
   switch (dir) {
     case 0: return x_tile_a(ctx->g) == 8 ? GKS_DISPATCH(0, 8) : GKS_DISPATCH(0, 4);
     case 1: return GKS_DISPATCH(1, 8);
     default: return GKS_DISPATCH(2, 8);
   }
+#undef GKS_DISPATCH3
 #undef GKS_DISPATCH
 }
 
