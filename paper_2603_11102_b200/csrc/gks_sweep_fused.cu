@@ -110,6 +110,17 @@ __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, u
       : "memory");
 }
 
+/* one arrival per warp, by lane 0, predicated inside the instruction (no divergent branch around it) */
+__device__ __forceinline__ void mbar_arrive_lane0(uint64_t *bar, int lane) {
+  asm volatile(
+      "{\n"
+      ".reg .pred P2;\n"
+      "setp.eq.s32 P2, %1, 0;\n"
+      "@P2 mbarrier.arrive.shared::cta.b64 _, [%0];\n"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(lane)
+      : "memory");
+}
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
@@ -316,6 +327,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
    * Both offsets are ONE xor of a per-thread constant with a compile-time one: a write of Gauss point gq goes to
    * Kw ^ gq, Kw = 4 (c ^ (fid&3)) + c; a read of component cc comes from Kr ^ 5 cc, Kr = 4 (fid&3) + c. */
   double *const xb = XBuf + fid * T::XF;
+  double *const flux_d = flux + (4 + c) * g.FS;   /* this thread's output field: dF/dt of component c */
   const int Kr = tid & 15, Kw = Kr ^ ((tid & 3) << 2);   /* fid = tid >> 2, c = tid & 3 */
 #define XW(field, gq) xb[(field) * 16 + (Kw ^ (gq))]
 #define XR(field, cc) xb[(field) * 16 + (Kr ^ (5 * (cc)))]
@@ -535,7 +547,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
     }
     /* this warp is done with the shared stage buffers of iteration i */
     __syncwarp();
-    if ((tid & 31) == 0) mbar_arrive(&bar[2]);
+    mbar_arrive_lane0(&bar[2], tid & 31);
     TR(4)   /* stages BC + D, arrival */
     if (!have) continue;
 
@@ -647,9 +659,9 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
         pidx[T::AXM] = m;
         /* a padded field holds fewer than 2^31 doubles (gks_create): the cell index is a 32-bit number */
         const int id = ((pidx[2] + GKS_NG) * g.P[1] + (pidx[1] + GKS_NG)) * g.P[0] + (pidx[0] + GKS_NG);
-        double *const fc = flux + c * g.FS;
-        if (NEED_F) fc[id] = 0.25 * fsel;
-        fc[4 * g.FS + id] = 0.25 * dsel;
+        double *const fd = flux_d + id;           /* dF/dt of component c; F sits 4 fields below */
+        if (NEED_F) fd[-4 * g.FS] = 0.25 * fsel;
+        fd[0] = 0.25 * dsel;
       }
     }
     TR(6)   /* transposes, flux, face average, store (F) */
