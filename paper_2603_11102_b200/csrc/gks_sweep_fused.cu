@@ -328,7 +328,8 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
    * Kw ^ gq, Kw = 4 (c ^ (fid&3)) + c; a read of component cc comes from Kr ^ 5 cc, Kr = 4 (fid&3) + c. */
   double *const xb = XBuf + fid * T::XF;
   double *const flux_d = flux + (4 + c) * g.FS;   /* this thread's output field: dF/dt of component c */
-  const int Kr = tid & 15, Kw = Kr ^ ((tid & 3) << 2);   /* fid = tid >> 2, c = tid & 3 */
+  int Kr = tid & 15, Kw = Kr ^ ((tid & 3) << 2);   /* fid = tid >> 2, c = tid & 3 */
+  asm volatile("" : "+r"(Kr), "+r"(Kw));           /* kept in registers: otherwise re-derived from tid every plane */
 #define XW(field, gq) xb[(field) * 16 + (Kw ^ (gq))]
 #define XR(field, cc) xb[(field) * 16 + (Kr ^ (5 * (cc)))]
   constexpr int sn = T::NA ? 1 : EA;            /* slab stride along the normal */
