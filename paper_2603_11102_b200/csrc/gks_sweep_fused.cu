@@ -342,6 +342,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
   /* offsets of the three stage buffers in turn, rotated once per iteration: plane i lives in buffer i % 3, so stage A
      works at (i % 3) SBUF, BC at ((i + 2) % 3) SBUF, D at ((i + 1) % 3) SBUF (three moves instead of three mod-3) */
   int sA = 0, sB = 2 * T::SBUF, sD = T::SBUF;
+  int idseg = -1;                              /* stage F: cell index of this thread's face in marched plane 0 of the segment */
   const double *wA = Wp, *wB = Wp + T::WSLAB_PAD;
   /* slots of planes i-6 .. i-3 at i = 0, as pointers to this thread's column */
   double *rq0 = rg + 2 * (6 * NF * 4), *rq1 = rg + 3 * (6 * NF * 4), *rq2 = rg, *rq3 = rg + 6 * NF * 4;
@@ -555,13 +556,21 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
     /* ================= stage EF: plane i-2 ================= */
     const int it = cD.it;
     const int m = cD.s.p0 + it - 2;
-    const bool face_ok = ga < n_a && gb < n_b;
     cur_next(cD);
 
     double *const rnew = q0;                     /* slot of the plane four back, dead once pass 2 below has read it */
     if (it < 4) {
 #pragma unroll
       for (int v = 0; v < 6; ++v) rnew[v * RF] = d6[v];
+      /* what the stores of this column segment need, once per segment (here, in the priming planes, it costs the plane loop
+         nothing): the cell index of marched plane 0, or -1 for a face beyond the last one (overhanging tile) */
+      int pidx[3];
+      pidx[0] = ga;
+      pidx[T::AXB] = gb;
+      pidx[T::AXM] = 0;
+      idseg = (ga < n_a && gb < n_b)
+                  ? ((pidx[2] + GKS_NG) * g.P[1] + (pidx[1] + GKS_NG)) * g.P[0] + (pidx[0] + GKS_NG)
+                  : -1;
       continue;
     }
     /* ---- E: tangential pass 2 (along t2, the marched axis) for plane m = it-2; the ring holds planes
@@ -653,13 +662,9 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
         dsel = (r[16] + r[17]) + (r[18] + r[19]);
       }
       __syncwarp();                               /* pass 2 of the next plane writes the buffer again */
-      if (face_ok) {
-        int pidx[3];
-        pidx[0] = ga;
-        pidx[T::AXB] = gb;
-        pidx[T::AXM] = m;
+      if (idseg >= 0) {
         /* a padded field holds fewer than 2^31 doubles (gks_create): the cell index is a 32-bit number */
-        const int id = ((pidx[2] + GKS_NG) * g.P[1] + (pidx[1] + GKS_NG)) * g.P[0] + (pidx[0] + GKS_NG);
+        const int id = idseg + m * (T::AXM == 2 ? g.P[0] * g.P[1] : g.P[0]);
         double *const fd = flux_d + id;           /* dF/dt of component c; F sits 4 fields below */
         if (NEED_F) fd[-4 * g.FS] = 0.25 * fsel;
         fd[0] = 0.25 * dsel;
