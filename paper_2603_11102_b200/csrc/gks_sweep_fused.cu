@@ -364,7 +364,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
     wB = wcur;
     /* cT describes plane i + 1 here: what stage A needs of it in the NEXT iteration */
     const int n0_A = n0_next;
-    n0_next = T::NA ? cT.s.a0 : cT.s.b0;
+    if (!UNIF) n0_next = T::NA ? cT.s.a0 : cT.s.b0;
     TR(0)   /* loop bookkeeping between two iterations */
     /* ONE hand-over per iteration: phase i-1 of the iteration barrier completes when every warp has finished
        A, BC, D of iteration i-1 AND the slab of plane i has landed - its TMA was issued at the top of iteration
@@ -374,8 +374,11 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
     else mbar_wait(&bar[0], 0);
     TR(1)   /* hand-over wait */
     if (i + 1 < J) {
-      if (tid == 0) issue(cT, i + 1);             /* slab (i+1)&1 was last read by stage A of iteration i-1 */
-      cur_next(cT);
+      /* on a uniform grid only the issuing thread needs the TMA cursor: the other warps do not walk it */
+      if (!UNIF || tid < 32) {
+        if (tid == 0) issue(cT, i + 1);           /* slab (i+1)&1 was last read by stage A of iteration i-1 */
+        cur_next(cT);
+      }
     }
     TR(2)   /* TMA issue + cursor */
 
