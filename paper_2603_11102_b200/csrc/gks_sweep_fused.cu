@@ -197,11 +197,14 @@ struct Seg {
  * an iteration without anyone waiting.  A thread's own BC item and its D item are written as one
  * straight-line block (GKS_FUSE_BCD): BC's serial chain issues in the shadow of D's arithmetic.
  */
-template <int DIR, bool NEED_F, bool LIN, int TA, int TB, bool UNIF>
+template <int DIR, bool NEED_F, bool LIN, int TA, int TB, int UMASK>
 __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
     k_sweep_fused(const __grid_constant__ CUtensorMap tmap, GksGrid g, GksPhys ph, double *__restrict__ flux,
                   int ncol_a, int nfull, long long rem, long long PPC, int ta0, int tlen0, int ta1, int n_a, int n_b) {
   using T = Tile<DIR, TA, TB>;
+  /* UMASK: bit a set = axis a is KNOWN to be uniform (its metric factors are kernel parameters, no table code); the
+     instantiations are 7 (all three), 5 (x and z: the channel, stretched between its walls) and 0 (nothing known) */
+  constexpr bool UN_N = (UMASK >> DIR) & 1, UN_T1 = (UMASK >> T::AXT1) & 1, UN_M = (UMASK >> T::AXM) & 1;
   constexpr int TN = T::TN, NF = T::NF, NT = T::NT, EA = T::EA, EB = T::EB, HA = T::HA, FH = T::FH;
   constexpr bool FUSE_BCD = GKS_FUSE_BCD == 1 || GKS_FUSE_BCD == 3 || (GKS_FUSE_BCD == 2 && DIR != 0);
   constexpr bool FUSE_A = GKS_FUSE_BCD == 3;
@@ -364,7 +367,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
     wB = wcur;
     /* cT describes plane i + 1 here: what stage A needs of it in the NEXT iteration */
     const int n0_A = n0_next;
-    if (!UNIF) n0_next = T::NA ? cT.s.a0 : cT.s.b0;
+    if (!UN_N) n0_next = T::NA ? cT.s.a0 : cT.s.b0;
     TR(0)   /* loop bookkeeping between two iterations */
     /* ONE hand-over per iteration: phase i-1 of the iteration barrier completes when every warp has finished
        A, BC, D of iteration i-1 AND the slab of plane i has landed - its TMA was issued at the top of iteration
@@ -375,7 +378,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
     TR(1)   /* hand-over wait */
     if (i + 1 < J) {
       /* on a uniform grid only the issuing thread needs the TMA cursor: the other warps do not walk it */
-      if (!UNIF || tid < 32) {
+      if (!UN_N || tid < 32) {
         if (tid == 0) issue(cT, i + 1);           /* slab (i+1)&1 was last read by stage A of iteration i-1 */
         cur_next(cT);
       }
@@ -413,7 +416,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
         const int fh = T::NA ? ct * HA + cn : cn * HA + ct;
         SA[QLo + fh * 4 + cc] = vr;
         double mf = g.inv_12hn_u[DIR];
-        if (!UNIF && !g.uniform[DIR]) mf = g.inv_12hn[DIR][min(n0 + cn, g.n[DIR]) + GKS_NG];
+        if (!UN_N && !g.uniform[DIR]) mf = g.inv_12hn[DIR][min(n0 + cn, g.n[DIR]) + GKS_NG];
         SA[DNo + fh * 4 + cc] = dn * mf;
       }
     };
@@ -500,7 +503,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
         gb = cD.s.b0 + fb;
         const int t1_glob = T::NA ? gb : ga;
         double iw1 = g.inv_w_u[T::AXT1];
-        if (!UNIF && !g.uniform[T::AXT1]) iw1 = g.inv_w[T::AXT1][min(t1_glob, g.n[T::AXT1] - 1) + GKS_NG];
+        if (!UN_T1 && !g.uniform[T::AXT1]) iw1 = g.inv_w[T::AXT1][min(t1_glob, g.n[T::AXT1] - 1) + GKS_NG];
         const double *q = Sb + oD + QLo + fh0 * 4 + c;                      /* Q0 of plane i-2 */
         const double *d = q + DNo;                                          /* Dn */
         double qq[5][2], vm[2], vp[2], sm_[2], sp_[2];
@@ -579,7 +582,7 @@ __global__ void __launch_bounds__(Tile<DIR, TA, TB>::NT, GKS_CTAS_PER_SM)
     /* ---- E: tangential pass 2 (along t2, the marched axis) for plane m = it-2; the ring holds planes
      *         it-4 .. it-1 (plane it-4+k in slot (it+k)&3), plane it comes straight from d6 ---- */
     double iw2 = g.inv_w_u[T::AXM];
-    if (!UNIF && !g.uniform[T::AXM]) iw2 = g.inv_w[T::AXM][m + GKS_NG];
+    if (!UN_M && !g.uniform[T::AXM]) iw2 = g.inv_w[T::AXM][m + GKS_NG];
     const double *const rs[4] = {q0, q1, q2, q3};
     /* the six evaluations (field Q0, Dn, Dt1) x (g1 = -, +) run EW at a time, statement-interleaved */
     constexpr int EW = GKS_E_WIDTH;
@@ -721,12 +724,12 @@ int tiles_a(const GksGrid &g, int dir) {
 }
 
 /* launch over the a-tiles [ta0, ta0 + len0) and [ta1, ta1 + len1) (len1 may be 0); returns the launches made */
-template <int DIR, bool NEED_F, bool LIN, int XA, bool UNIF>
+template <int DIR, bool NEED_F, bool LIN, int XA, int UMASK>
 int launch_dir(gks_ctx *ctx, const CUtensorMap &map, double *flux, int ta0, int len0, int ta1, int len1) {
   constexpr int TA = Shape<DIR, XA>::TA, TB = Shape<DIR, XA>::TB;
   using T = Tile<DIR, TA, TB>;
   const GksGrid &g = ctx->g;
-  auto kern = k_sweep_fused<DIR, NEED_F, LIN, TA, TB, UNIF>;   /* UNIF: all three axes uniform - no metric tables */
+  auto kern = k_sweep_fused<DIR, NEED_F, LIN, TA, TB, UMASK>;
   static bool attr_done[64] = {};                /* the attribute is per device: one process may hold contexts on several */
   int dev = 0;
   cudaGetDevice(&dev);
@@ -809,10 +812,12 @@ int gks_launch_sweep_fused(gks_ctx *ctx, int dir, int which, double *flux, bool 
       len1 = all - t1;
     }
   }
-  const bool unif = ctx->g.uniform[0] && ctx->g.uniform[1] && ctx->g.uniform[2];
+  const int ubits = (ctx->g.uniform[0] ? 1 : 0) | (ctx->g.uniform[1] ? 2 : 0) | (ctx->g.uniform[2] ? 4 : 0);
+  const int umask = ubits == 7 ? 7 : ((ubits & 5) == 5 ? 5 : 0);
 #define GKS_DISPATCH3(D, XA, NF_, LIN_)                                                                      \
-  (unif ? launch_dir<D, NF_, LIN_, XA, true>(ctx, m, flux, ta0, len0, ta1, len1)                             \
-        : launch_dir<D, NF_, LIN_, XA, false>(ctx, m, flux, ta0, len0, ta1, len1))
+  (umask == 7 ? launch_dir<D, NF_, LIN_, XA, 7>(ctx, m, flux, ta0, len0, ta1, len1)                          \
+   : umask == 5 ? launch_dir<D, NF_, LIN_, XA, 5>(ctx, m, flux, ta0, len0, ta1, len1)                        \
+                : launch_dir<D, NF_, LIN_, XA, 0>(ctx, m, flux, ta0, len0, ta1, len1))
 #define GKS_DISPATCH(D, XA)                                                                                  \
   (need_F ? (lin ? GKS_DISPATCH3(D, XA, true, true) : GKS_DISPATCH3(D, XA, true, false))                     \
           : (lin ? GKS_DISPATCH3(D, XA, false, true) : GKS_DISPATCH3(D, XA, false, false)))
